@@ -1,0 +1,150 @@
+/* symdel.h — C ABI of libsymdel: symmetric-deletion (SymDel) Levenshtein neighbour search on one
+ * NVIDIA B200 (sm_100a).  arxiv/paper_2403_09010, "Lightning-fast adaptive immune receptor
+ * similarity search by symmetric deletion lookup".
+ *
+ * The operation (App. F.1 steps 0-5; App. F.3): "Given an array
+ * {s_i} of AIR sequences and a distance threshold ... return {(i, i', d(s_i, s_i'))}", computed by
+ * (1) generating every deletion variant with up to d deletions of every sequence, (2) a sort-merge
+ * join of the variants (§I.B), (3) candidate-pair emission and deduplication,
+ * (4) exact edit-distance verification on the full sequences.  The two-set form
+ * ("for both the query and reference sets"; Fig. 1) is symdel_cross.
+ *
+ * Result contract
+ *   symdel_self : every pair 0 <= i < j < n with lev(s_i, s_j) <= d exactly once, dist = the exact
+ *                 unit-cost Levenshtein distance (0..d), sorted ascending by (i, j).
+ *   symdel_cross: every (q, r) with lev(query_q, ref_r) <= d exactly once, sorted ascending by (q, r).
+ *   Indices are positions in the caller's arrays.  Exact duplicates are legal and reported at
+ *   dist 0 (the paper only recommends collapsing them).  Empty sequences are legal.
+ *
+ * Sequences are CSR: `seqs` int8 residue codes 1..31 (0 is reserved), `offsets` int64[n+1] with
+ * offsets[0] == 0, non-decreasing; sequence i is seqs[offsets[i] .. offsets[i+1]).
+ *
+ * Pointers are DEVICE pointers unless the parameter name ends in `_host`.  The library never
+ * allocates or frees caller memory; device entry points never call cudaMalloc (the caller passes a
+ * workspace); the *_host entry points stage through a device arena owned by the context.
+ * Every function returns SYMDEL_OK (0) or a negative SYMDEL_E_* code; nothing throws or aborts
+ * across the ABI.  On error the outputs are unspecified unless stated.  All calls are synchronous
+ * with respect to the result: when they return, outputs and *n_pairs_host are final.
+ * There is no CPU fallback: without a CUDA device every compute entry point fails with SYMDEL_E_CUDA.
+ */
+#ifndef SYMDEL_H
+#define SYMDEL_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define SYMDEL_API __attribute__((visibility("default")))
+#else
+#define SYMDEL_API
+#endif
+
+#define SYMDEL_D_MAX 4   /* largest distance threshold accepted (the paper benchmarks d <= 5; configs need <= 3) */
+#define SYMDEL_L_MAX 64  /* longest sequence accepted = one 64-bit word of the bit-parallel verifier (configs need <= 30) */
+
+enum {
+    SYMDEL_OK = 0,
+    SYMDEL_E_ARG = -1,       /* null pointer, n < 0, d < 0 or d > SYMDEL_D_MAX, bad option */
+    SYMDEL_E_OFFSETS = -2,   /* offsets[0] != 0 or offsets decreasing */
+    SYMDEL_E_TOO_LONG = -3,  /* some sequence longer than SYMDEL_L_MAX */
+    SYMDEL_E_RESIDUE = -4,   /* residue code outside 1..31 */
+    SYMDEL_E_TOO_MANY = -5,  /* n_a + n_b >= 2^30 */
+    SYMDEL_E_WORKSPACE = -6, /* workspace too small even at maximum chunking */
+    SYMDEL_E_CAPACITY = -7,  /* more result pairs than `capacity`: *n_pairs_host = required count, the first `capacity` pairs are valid */
+    SYMDEL_E_CUDA = -8,      /* CUDA error (sticky); code via symdel_last_cuda_error */
+    SYMDEL_E_INTERNAL = -9   /* internal consistency check failed (never expected) */
+};
+
+typedef struct symdel_ctx symdel_ctx; /* opaque; owns small pinned scratch, stats and (host entry points only) a device arena */
+
+/* Stage counters and timings of the LAST call (Table S1's columns).
+ * n_candidates / n_unique depend on the key hash and are not comparable with the paper's. */
+typedef struct {
+    int64_t n_records;     /* (variant key, id) records generated = distinct (variant, id) tuples */
+    int64_t n_candidates;  /* candidate pairs emitted by the join (distinct ids, before dedup) */
+    int64_t n_unique;      /* candidates after dedup */
+    int64_t n_outputs;     /* verified pairs */
+    int64_t n_chunks;      /* key-range chunks used (S5) */
+    int64_t n_flushes;     /* candidate-buffer flushes (dedup+verify rounds) */
+    int64_t n_launches;    /* kernels launched */
+    int32_t hash_bits;     /* key bits sorted per record */
+    int32_t id_bits;       /* id bits per record */
+    float ms_prepare, ms_generate, ms_sort, ms_emit, ms_dedup, ms_verify, ms_total; /* CUDA-event times; 0 unless SYMDEL_OPT_TIMING is set */
+    float ms_sort_pass_avg; /* average duration of one onesweep pass over the variant records */
+    int64_t sort_pass_records; /* records moved by one such pass */
+} symdel_stats;
+
+/* Options (symdel_set_option); defaults in brackets. */
+enum {
+    SYMDEL_OPT_TIMING = 1,        /* [0] 1: bracket each stage with CUDA events (adds stream syncs at the end only) */
+    SYMDEL_OPT_FORCE_CHUNKS = 2,  /* [0] >0: use exactly this many key-range chunks (test hook for S5) */
+    SYMDEL_OPT_CAND_CAPACITY = 3, /* [0] >0: cap the candidate buffer at this many pairs (test hook for multi-flush) */
+    SYMDEL_OPT_HASH_BITS = 4,     /* [0] 0 = automatic; else 8..56 (multiple of 8): key bits sorted per record */
+    SYMDEL_OPT_NO_THINNING = 5    /* [0] 1: emit one record per deletion SET instead of per distinct variant (test hook) */
+};
+
+/* ---- context ------------------------------------------------------------------------------- */
+SYMDEL_API int symdel_create(symdel_ctx** ctx, int device);  /* selects `device`; SYMDEL_E_CUDA if none */
+SYMDEL_API void symdel_destroy(symdel_ctx* ctx);
+SYMDEL_API int symdel_set_option(symdel_ctx* ctx, int option, int64_t value);
+SYMDEL_API int symdel_get_stats(const symdel_ctx* ctx, symdel_stats* stats_host);
+SYMDEL_API int symdel_last_cuda_error(const symdel_ctx* ctx); /* cudaError_t of the last SYMDEL_E_CUDA, else 0 */
+SYMDEL_API const char* symdel_strerror(int code);             /* static string */
+
+/* Recommended workspace size for an un-chunked run.  n_b = 0 and residues_b = 0 for self-search.
+ * max_len = longest sequence (<= SYMDEL_L_MAX).  Any workspace >= the minimum the library needs
+ * works: a smaller one makes symdel_* split the key space into chunks (S5).  Pure host arithmetic. */
+SYMDEL_API int symdel_workspace_bytes(int64_t n_a, int64_t residues_a, int64_t n_b, int64_t residues_b, int max_len, int d,
+                           int64_t* bytes_host);
+
+/* ---- the hot path, device-resident inputs and outputs ---------------------------------------
+ * out_i/out_j/out_dist: caller-owned device arrays of `capacity` int32 each.
+ * workspace: caller-owned device memory, 256-byte aligned, contents destroyed.
+ * cuda_stream: a cudaStream_t (may be NULL = default stream); all work is issued on it. */
+SYMDEL_API int symdel_self(symdel_ctx* ctx, const int8_t* seqs, const int64_t* offsets, int64_t n, int d, void* workspace,
+                int64_t workspace_bytes, int32_t* out_i, int32_t* out_j, int32_t* out_dist, int64_t capacity,
+                int64_t* n_pairs_host, void* cuda_stream);
+
+SYMDEL_API int symdel_cross(symdel_ctx* ctx, const int8_t* q_seqs, const int64_t* q_offsets, int64_t n_q, const int8_t* r_seqs,
+                 const int64_t* r_offsets, int64_t n_r, int d, void* workspace, int64_t workspace_bytes,
+                 int32_t* out_i, int32_t* out_j, int32_t* out_dist, int64_t capacity, int64_t* n_pairs_host,
+                 void* cuda_stream);
+
+/* ---- the same calls with HOST buffers (inputs copied host->device and results device->host
+ * inside the call; pinned host memory makes the copies asynchronous) ---------------------------- */
+SYMDEL_API int symdel_self_host(symdel_ctx* ctx, const int8_t* seqs_host, const int64_t* offsets_host, int64_t n, int d,
+                     int32_t* out_i_host, int32_t* out_j_host, int32_t* out_dist_host, int64_t capacity,
+                     int64_t* n_pairs_host);
+
+SYMDEL_API int symdel_cross_host(symdel_ctx* ctx, const int8_t* q_seqs_host, const int64_t* q_offsets_host, int64_t n_q,
+                      const int8_t* r_seqs_host, const int64_t* r_offsets_host, int64_t n_r, int d,
+                      int32_t* out_i_host, int32_t* out_j_host, int32_t* out_dist_host, int64_t capacity,
+                      int64_t* n_pairs_host);
+
+/* ---- stage-level entry points (kernel parity tests and micro-benchmarks) ---------------------
+ * S2/K2: stable LSD radix sort of n 64-bit keys on bits [begin_bit, end_bit) (end - begin a
+ *   multiple of 8).  keys and tmp: device arrays of n; the sorted result is left in `keys`.
+ *   workspace: device scratch of at least symdel_stage_sort_workspace_bytes(n) bytes. */
+SYMDEL_API int64_t symdel_stage_sort_workspace_bytes(int64_t n);
+SYMDEL_API int symdel_stage_sort_u64(symdel_ctx* ctx, uint64_t* keys, uint64_t* tmp, int64_t n, int begin_bit, int end_bit,
+                          void* workspace, int64_t workspace_bytes, void* cuda_stream);
+
+/* S1/K1: (key, id) records of one sequence set, unsorted, in id order: records[t] =
+ *   (hash >> (64 - hash_bits)) << id_bits | id.  Returns the count through *n_records_host.
+ *   thinning = 1: one record per distinct variant (leftmost embedding); 0: one per deletion set. */
+SYMDEL_API int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const int64_t* offsets, int64_t n, int d, int hash_bits,
+                          int id_bits, int thinning, uint64_t* records, int64_t records_capacity,
+                          int64_t* n_records_host, void* workspace, int64_t workspace_bytes, void* cuda_stream);
+
+/* S4/K6: dist[t] = lev(a_{ia[t]}, b_{ib[t]}) by the bit-parallel verifier, for n_pairs index pairs. */
+SYMDEL_API int symdel_stage_lev(symdel_ctx* ctx, const int8_t* a_seqs, const int64_t* a_offsets, int64_t n_a,
+                     const int8_t* b_seqs, const int64_t* b_offsets, int64_t n_b, const int32_t* ia,
+                     const int32_t* ib, int64_t n_pairs, int32_t* dist, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SYMDEL_H */

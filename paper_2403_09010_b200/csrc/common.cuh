@@ -1,0 +1,134 @@
+// common.cuh — device helpers shared by the libsymdel kernels (sm_100a).
+// Nothing here is shared with oracle/ (the CPU oracle has its own, different, arithmetic).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+typedef uint64_t u64;
+typedef uint32_t u32;
+typedef int64_t i64;
+typedef int32_t i32;
+
+#define SD_FULL 0xffffffffu
+
+// ---- device status block (one per call, in the workspace; copied to pinned host memory) --------
+struct DevInfo {
+    u64 nmax;        // sum over sequences of V(L, d) (deletion sets)
+    u64 n_records;   // records written by the last generate
+    u64 n_cand;      // candidate pairs counted by the last emit
+    u64 n_surv;      // survivors appended so far
+    u64 n_out;       // final output pairs
+    u64 n_unique;    // unique candidates seen by verify (statistics)
+    u32 maxlen;      // longest sequence
+    u32 err;         // bit flags, see below
+    u32 ticket[8];   // dynamic tile tickets (one per kernel family)
+    u32 pad[6];
+};
+enum { SD_ERR_OFFSETS = 1, SD_ERR_TOO_LONG = 2, SD_ERR_RESIDUE = 4, SD_ERR_INTERNAL = 8, SD_ERR_OVERFLOW = 16 };
+enum { SD_TK_SORT = 0, SD_TK_EMIT = 1, SD_TK_VERIFY = 2, SD_TK_FINAL = 3, SD_TK_SCAN = 4 };
+
+// ---- decoupled look-back, one 64-bit value per tile ---------------------------------------------
+// status word: bits 63:62 = flag (0 invalid, 1 aggregate, 2 inclusive prefix), bits 61:0 = value.
+// A tile publishes its aggregate, then walks its predecessors summing aggregates until it meets an
+// inclusive prefix, then publishes its own inclusive prefix.  Tiles get their index from an atomic
+// ticket, so every predecessor has started and the spin always terminates.  Flag and value share
+// one word, so a single relaxed 64-bit store/load is enough (no fence between flag and payload).
+#define SD_LB_AGG (1ull << 62)
+#define SD_LB_PRE (2ull << 62)
+#define SD_LB_MASK ((1ull << 62) - 1)
+
+__device__ __forceinline__ u64 sd_ld_relaxed(const u64* p) {
+    u64 v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sd_st_relaxed(u64* p, u64 v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ u32 sd_ld_relaxed32(const u32* p) {
+    u32 v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sd_st_relaxed32(u32* p, u32 v) {
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Called by ONE thread of the tile.  Returns the exclusive prefix of `aggregate` over tiles < tile.
+__device__ __forceinline__ u64 sd_lookback(u64* status, u32 tile, u64 aggregate) {
+    if (tile == 0) {
+        sd_st_relaxed(status, SD_LB_PRE | aggregate);
+        return 0;
+    }
+    sd_st_relaxed(status + tile, SD_LB_AGG | aggregate);
+    u64 excl = 0;
+    i64 p = (i64)tile - 1;
+    while (true) {
+        u64 s;
+        do { s = sd_ld_relaxed(status + p); } while ((s >> 62) == 0);
+        excl += s & SD_LB_MASK;
+        if ((s >> 62) == 2) break;
+        --p;
+    }
+    sd_st_relaxed(status + tile, SD_LB_PRE | (excl + aggregate));
+    return excl;
+}
+
+// ---- block-wide exclusive scans (THREADS a multiple of 32, <= 1024) ------------------------------
+template <int THREADS>
+__device__ __forceinline__ u32 sd_block_excl_sum(u32 v, u32* total, u32* s_warp /* [THREADS/32 + 1] */) {
+    const u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    u32 inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        u32 t = __shfl_up_sync(SD_FULL, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        u32 w = lane < THREADS / 32 ? s_warp[lane] : 0;
+        u32 winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            u32 t = __shfl_up_sync(SD_FULL, winc, o);
+            if (lane >= o) winc += t;
+        }
+        if (lane < THREADS / 32) s_warp[lane] = winc - w;
+        if (lane == 31) s_warp[THREADS / 32] = winc;
+    }
+    __syncthreads();
+    u32 r = s_warp[warp] + inc - v;
+    *total = s_warp[THREADS / 32];
+    __syncthreads();  // s_warp may be reused by the caller
+    return r;
+}
+
+// exclusive max-scan of signed positions (identity = -1)
+template <int THREADS>
+__device__ __forceinline__ i32 sd_block_excl_max(i32 v, i32* s_warp /* [THREADS/32] */) {
+    const u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    i32 inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        i32 t = __shfl_up_sync(SD_FULL, inc, o);
+        if (lane >= o) inc = max(inc, t);
+    }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    i32 carry = -1;
+    for (u32 w = 0; w < warp; ++w) carry = max(carry, s_warp[w]);
+    i32 prev = __shfl_up_sync(SD_FULL, inc, 1);
+    if (lane == 0) prev = -1;
+    __syncthreads();
+    return max(carry, prev);
+}
+
+__device__ __forceinline__ u64 sd_mix64(u64 x) {  // bijective finaliser
+    x ^= x >> 32;
+    x *= 0xd6e8feb86659fd93ull;
+    x ^= x >> 32;
+    x *= 0xd6e8feb86659fd93ull;
+    x ^= x >> 32;
+    return x;
+}

@@ -1,0 +1,464 @@
+// generate.cu — S0 (input validation, record counting, offsets) and S1/K1 (variant generation).
+//
+// "First, generate an array containing all tuples of deletion variants and original strings for
+// both the query and reference sets." (§I.B step 1; App. F.1 step 1, PAPER.md:327;
+// App. F.3 step 1).  A sequence of length L has sum_{k<=d} C(L, k) deletion sets
+// (reading A-1: the 0-deletion original is included).  As in SymScan, the tuple holds
+// a hash of the variant and the index of the sequence, (h_ij, i) (footnote 1):
+//     record = (top hash_bits of H(variant)) << id_bits | id
+// H is a polynomial hash over 5-bit residue codes, H(v) = mix64(sum_k R[v_k] * B^k + len * K) mod
+// 2^64 (B odd).  With the prefix sums A[j] = sum_{t<j} R[s_t] * B^t of the SOURCE sequence, the hash of
+// the variant that deletes positions p_1 < ... < p_k is
+//     sum_{m=0..k} B^{-m} * (A[p_{m+1}] - A[p_m + 1]),   p_0 = -1, p_{k+1} = L,
+// so a variant costs k+1 multiply-adds instead of a pass over its residues.
+//
+// Thinning (reading A-2; SymScan "sort ... and deduplicate"): a deletion set is kept
+// only if it is the LEFTMOST embedding of its variant, i.e. no deleted position p has
+// s[p] == s[q] with q the next kept position after p.  Exactly one set per distinct (variant, id)
+// survives, so repeated residues produce no duplicate records.
+//
+// Order: records are written in ascending id, at rec_off[id] + rank, where rec_off is the exclusive
+// scan of the per-sequence counts produced by the count pass — no atomics, deterministic layout,
+// and (with the stable sort) ids ascend inside every run of equal keys.
+#include "kernels.h"
+
+namespace {
+
+__constant__ u64 c_R[32];
+__constant__ u64 c_Bpow[SD_L_MAX + 1];
+__constant__ u64 c_Binv[SD_D_MAX + 1];
+__constant__ u32 c_binom[(SD_L_MAX + 1) * (SD_D_MAX + 1)];  // C(n, k)
+__constant__ u32 c_vcum[(SD_L_MAX + 1) * (SD_D_MAX + 2)];   // sum_{j<k} C(n, j)
+
+constexpr u64 K_LEN = 0x9fb21c651e98df25ull;
+
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, DevInfo* info) {
+    u64 nmax = 0;
+    u32 maxlen = 0, err = 0;
+    const i64 stride = (i64)gridDim.x * blockDim.x;
+    const i64 t0 = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    for (i64 i = t0; i < s.n; i += stride) {
+        i64 a = s.off[i], b = s.off[i + 1];
+        if (i == 0 && a != 0) err |= SD_ERR_OFFSETS;
+        i64 L = b - a;
+        if (L < 0 || a < 0) err |= SD_ERR_OFFSETS;
+        else if (L > SD_L_MAX) err |= SD_ERR_TOO_LONG;
+        else {
+            nmax += c_vcum[L * (SD_D_MAX + 2) + d + 1];
+            maxlen = max(maxlen, (u32)L);
+        }
+    }
+    const i64 total = s.n > 0 ? s.off[s.n] : 0;
+    for (i64 t = t0; t < total; t += stride) {
+        int c = s.seqs[t];
+        if (c < 1 || c > 31) err |= SD_ERR_RESIDUE;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        nmax += __shfl_xor_sync(SD_FULL, nmax, o);
+        maxlen = max(maxlen, __shfl_xor_sync(SD_FULL, maxlen, o));
+        err |= __shfl_xor_sync(SD_FULL, err, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (nmax) atomicAdd((unsigned long long*)&info->nmax, (unsigned long long)nmax);
+        if (maxlen) atomicMax(&info->maxlen, maxlen);
+        if (err) atomicOr(&info->err, err);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// exclusive scan of u32 counts into u64 offsets, single pass, decoupled look-back
+constexpr int SC_THREADS = 256, SC_IPT = 8, SC_TILE = SC_THREADS * SC_IPT;
+
+__global__ void __launch_bounds__(SC_THREADS) k_scan_counts(const u32* __restrict__ cnt, i64 n, u64* __restrict__ rec_off,
+                                                           u64* lb_status, DevInfo* info) {
+    __shared__ u32 s_warp[SC_THREADS / 32 + 1];
+    __shared__ u32 s_tile;
+    __shared__ u64 s_excl;
+    const u32 tid = threadIdx.x;
+    if (tid == 0) {
+        s_tile = atomicAdd(&info->ticket[SD_TK_SCAN], 1u);
+        if (s_tile == gridDim.x - 1) info->ticket[SD_TK_SCAN] = 0;  // every ticket has been taken
+    }
+    __syncthreads();
+    const u32 tile = s_tile;
+    const i64 base = (i64)tile * SC_TILE + (i64)tid * SC_IPT;
+    u32 v[SC_IPT], sum = 0;
+#pragma unroll
+    for (int k = 0; k < SC_IPT; ++k) {
+        v[k] = (base + k) < n ? cnt[base + k] : 0;
+        sum += v[k];
+    }
+    u32 total;
+    u32 excl = sd_block_excl_sum<SC_THREADS>(sum, &total, s_warp);
+    if (tid == 0) s_excl = sd_lookback(lb_status, tile, total);
+    __syncthreads();
+    u64 run = s_excl + excl;
+#pragma unroll
+    for (int k = 0; k < SC_IPT; ++k) {
+        if ((base + k) < n) rec_off[base + k] = run;
+        run += v[k];
+    }
+    if (tile == gridDim.x - 1 && tid == SC_THREADS - 1) {
+        rec_off[n] = s_excl + total;
+        info->n_records = s_excl + total;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+constexpr int GEN_THREADS = 256, GEN_G = 32, GEN_R = 4, GEN_NW = GEN_THREADS / 32;
+constexpr int SEQ_STRIDE = SD_L_MAX + 4;
+
+struct GenParams {
+    SeqSetDev a, b;
+    i64 groups_a, groups_total;
+    i64 n_a;
+    int d, width, thinning, hash_bits, id_bits, npass;
+    u32 n_chunks, chunk;
+    const u64* rec_off;
+    u64* records;
+    u32* cnt;
+    u32* ghist;
+    DevInfo* info;
+};
+
+struct GenShared {
+    u64 A[GEN_G][SD_L_MAX + 1];
+    u64 R[32];
+    u64 Bpow[SD_L_MAX + 1];
+    i64 off[GEN_G];
+    u32 binom[(SD_L_MAX + 1) * (SD_D_MAX + 1)];
+    u32 vcum[(SD_L_MAX + 1) * (SD_D_MAX + 2)];
+    u32 vbase[GEN_G + 1];
+    u32 len[GEN_G];
+    u32 cnt[GEN_G];
+    u32 wtot[GEN_NW];
+    u32 running;
+    unsigned char seq[GEN_G][SEQ_STRIDE];
+};
+
+// Decodes deletion set number `idx` among the C(L, K) sets of size K (colexicographic order),
+// applies the leftmost-embedding rule and hashes the variant.  Returns false if thinned out.
+template <int K>
+__device__ __forceinline__ bool gen_set(const GenShared& sh, u32 g, u32 L, u32 idx, bool thinning, u64* hash_out) {
+    int p[K > 0 ? K : 1];
+    if (K > 0) {
+        int c = (int)L - 1;
+#pragma unroll
+        for (int j = K; j >= 1; --j) {
+            if (j == 1) {
+                c = (int)idx;
+            } else if (j == 2) {
+                // largest c with c(c-1)/2 <= idx
+                int e = (int)((1.0f + sqrtf(1.0f + 8.0f * (float)idx)) * 0.5f);
+                e = min(e, c);
+                while ((u32)(e * (e - 1) / 2) > idx) --e;
+                while (e < c && (u32)((e + 1) * e / 2) <= idx) ++e;
+                c = e;
+            } else {
+                while (sh.binom[c * (SD_D_MAX + 1) + j] > idx) --c;
+            }
+            p[j - 1] = c;
+            idx -= sh.binom[c * (SD_D_MAX + 1) + j];
+            c = c - 1;
+        }
+    }
+    const unsigned char* s = sh.seq[g];
+    if (thinning && K > 0) {
+        bool canon = true;
+#pragma unroll
+        for (int m = 0; m < K; ++m) {
+            int q = p[m] + 1;
+#pragma unroll
+            for (int m2 = m + 1; m2 < K; ++m2)
+                if (p[m2] == q) ++q;
+            canon = canon && (q >= (int)L || s[p[m]] != s[q]);
+        }
+        if (!canon) return false;
+    }
+    const u64* A = sh.A[g];
+    u64 h = 0;
+    int prev = 0;
+#pragma unroll
+    for (int m = 0; m <= K; ++m) {
+        int end = (m < K) ? p[m < K ? m : 0] : (int)L;
+        u64 term = A[end] - A[prev];
+        h += (m == 0) ? term : c_Binv[m] * term;
+        if (m < K) prev = p[m] + 1;
+    }
+    h += (u64)(L - K + 1) * K_LEN;
+    *hash_out = sd_mix64(h);
+    return true;
+}
+
+template <bool COUNT_ONLY>
+__global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
+    extern __shared__ __align__(16) unsigned char gen_smem[];
+    GenShared& sh = *reinterpret_cast<GenShared*>(gen_smem);
+    u32* s_hist = reinterpret_cast<u32*>(gen_smem + sizeof(GenShared));  // [npass][256], generation only
+
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 lane_lt = (1u << lane) - 1u;
+    for (int i = tid; i < (SD_L_MAX + 1) * (SD_D_MAX + 1); i += GEN_THREADS) sh.binom[i] = c_binom[i];
+    for (int i = tid; i < (SD_L_MAX + 1) * (SD_D_MAX + 2); i += GEN_THREADS) sh.vcum[i] = c_vcum[i];
+    if (tid < 32) sh.R[tid] = c_R[tid];
+    if (tid <= SD_L_MAX) sh.Bpow[tid] = c_Bpow[tid];
+    if (!COUNT_ONLY)
+        for (int i = tid; i < P.npass * 256; i += GEN_THREADS) s_hist[i] = 0;
+    const int d = P.d;
+    const bool thinning = P.thinning != 0;
+
+    for (i64 gi = blockIdx.x; gi < P.groups_total; gi += gridDim.x) {
+        const bool in_b = gi >= P.groups_a;
+        const SeqSetDev& S = in_b ? P.b : P.a;
+        const i64 first = (in_b ? gi - P.groups_a : gi) * GEN_G;
+        const u32 ng = (u32)min((i64)GEN_G, S.n - first);
+        const u64 gid0 = (u64)first + (in_b ? (u64)P.n_a : 0ull);
+        __syncthreads();  // previous group fully consumed (also orders the table fill above)
+        if (tid < GEN_G) {
+            u32 L = 0;
+            if (tid < ng) {
+                i64 a = S.off[first + tid];
+                L = (u32)(S.off[first + tid + 1] - a);
+                sh.off[tid] = a;
+            }
+            sh.len[tid] = L;
+            sh.cnt[tid] = 0;
+            // inclusive scan of V(L, d) over the group (warp 0)
+            u32 v = tid < ng ? sh.vcum[L * (SD_D_MAX + 2) + d + 1] : 0, inc = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                u32 t = __shfl_up_sync(SD_FULL, inc, o);
+                if (lane >= (u32)o) inc += t;
+            }
+            sh.vbase[tid + 1] = inc;
+            if (tid == 0) {
+                sh.vbase[0] = 0;
+                sh.running = 0;
+            }
+        }
+        __syncthreads();
+        for (u32 idx = tid; idx < ng * (u32)P.width; idx += GEN_THREADS) {
+            u32 g = idx / (u32)P.width, p = idx - g * (u32)P.width;
+            sh.seq[g][p] = p < sh.len[g] ? (unsigned char)S.seqs[sh.off[g] + p] : (unsigned char)0;
+        }
+        __syncthreads();
+        if (tid < ng) {
+            u64 acc = 0;
+            const u32 L = sh.len[tid];
+            sh.A[tid][0] = 0;
+            for (u32 p = 0; p < L; ++p) {
+                acc += sh.R[sh.seq[tid][p] & 31] * sh.Bpow[p];
+                sh.A[tid][p + 1] = acc;
+            }
+        }
+        __syncthreads();
+
+        const u32 T = sh.vbase[ng];
+        const u64 base_out = COUNT_ONLY ? 0ull : P.rec_off[gid0];
+        for (u32 rb = 0; rb < T; rb += GEN_THREADS * GEN_R) {
+            u64 rec[GEN_R];
+            u32 ball[GEN_R];
+            u32 wt = 0;
+#pragma unroll
+            for (int r = 0; r < GEN_R; ++r) {
+                const u32 f = rb + warp * (32 * GEN_R) + r * 32 + lane;
+                bool valid = false;
+                u32 g = 0;
+                rec[r] = 0;
+                if (f < T) {
+                    u32 lo = 0, hi = ng;
+                    while (hi - lo > 1) {
+                        u32 mid = (lo + hi) >> 1;
+                        if (sh.vbase[mid] <= f) lo = mid; else hi = mid;
+                    }
+                    g = lo;
+                    const u32 rr = f - sh.vbase[g], L = sh.len[g];
+                    const u32* vc = sh.vcum + L * (SD_D_MAX + 2);
+                    int k = 0;
+                    while (k < d && rr >= vc[k + 1]) ++k;
+                    const u32 idx = rr - vc[k];
+                    u64 h = 0;
+                    switch (k) {
+                        case 0: valid = gen_set<0>(sh, g, L, idx, thinning, &h); break;
+                        case 1: valid = gen_set<1>(sh, g, L, idx, thinning, &h); break;
+                        case 2: valid = gen_set<2>(sh, g, L, idx, thinning, &h); break;
+                        case 3: valid = gen_set<3>(sh, g, L, idx, thinning, &h); break;
+                        default: valid = gen_set<4>(sh, g, L, idx, thinning, &h); break;
+                    }
+                    if (valid && P.n_chunks > 1) valid = __umulhi((u32)h, P.n_chunks) == P.chunk;
+                    rec[r] = ((h >> (64 - P.hash_bits)) << P.id_bits) | (gid0 + g);
+                }
+                ball[r] = __ballot_sync(SD_FULL, valid);
+                wt += __popc(ball[r]);
+                if (COUNT_ONLY) {
+                    // lanes of one sequence are contiguous: one shared-memory add per (warp, sequence) segment
+                    const u32 gprev = __shfl_up_sync(SD_FULL, g, 1);
+                    const bool head = (lane == 0) || (gprev != g);
+                    const u32 heads = __ballot_sync(SD_FULL, head);
+                    if (head) {
+                        const u32 higher = (lane == 31) ? 0u : (heads & (~0u << (lane + 1)));
+                        const u32 end = higher ? (u32)(__ffs(higher) - 1) : 32u;
+                        const u32 seg = (~0u << lane) & (end == 32 ? ~0u : ((1u << end) - 1u));
+                        const u32 c = __popc(ball[r] & seg);
+                        if (c) atomicAdd(&sh.cnt[g], c);
+                    }
+                }
+            }
+            if (!COUNT_ONLY) {
+                if (lane == 0) sh.wtot[warp] = wt;
+                __syncthreads();
+                u32 woff = sh.running, all = 0;
+#pragma unroll
+                for (int w = 0; w < GEN_NW; ++w) {
+                    u32 c = sh.wtot[w];
+                    if ((u32)w < warp) woff += c;
+                    all += c;
+                }
+                __syncthreads();
+                if (tid == 0) sh.running += all;
+                u32 pre = 0;
+#pragma unroll
+                for (int r = 0; r < GEN_R; ++r) {
+                    if (ball[r] & (1u << lane)) {
+                        const u32 pos = woff + pre + __popc(ball[r] & lane_lt);
+                        P.records[base_out + pos] = rec[r];
+                        const u64 key = rec[r] >> P.id_bits;
+                        for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
+                    }
+                    pre += __popc(ball[r]);
+                }
+            }
+        }
+        __syncthreads();
+        if (COUNT_ONLY) {
+            if (tid < ng) P.cnt[gid0 + tid] = sh.cnt[tid];
+        } else if (tid == 0) {
+            if ((u64)sh.running != P.rec_off[gid0 + ng] - base_out) atomicOr(&P.info->err, (u32)SD_ERR_INTERNAL);
+        }
+    }
+    if (!COUNT_ONLY) {
+        __syncthreads();
+        for (int i = tid; i < P.npass * 256; i += GEN_THREADS)
+            if (s_hist[i]) atomicAdd(&P.ghist[i], s_hist[i]);
+    }
+}
+
+u64 splitmix64(u64& x) {
+    u64 z = (x += 0x9e3779b97f4a7c15ull);
+    z = (z ^ (z >> 30)) * 0xbf58476d1ce4e5b9ull;
+    z = (z ^ (z >> 27)) * 0x94d049bb133111ebull;
+    return z ^ (z >> 31);
+}
+
+GenParams make_params(SeqSetDev a, SeqSetDev b, const Layout& lay, int width) {
+    GenParams P{};
+    P.a = a;
+    P.b = b;
+    P.n_a = a.n;
+    P.groups_a = (a.n + GEN_G - 1) / GEN_G;
+    P.groups_total = P.groups_a + (b.n + GEN_G - 1) / GEN_G;
+    P.d = lay.d;
+    P.width = width;
+    P.thinning = lay.thinning;
+    P.hash_bits = lay.hash_bits;
+    P.id_bits = lay.id_bits;
+    P.n_chunks = lay.n_chunks;
+    P.chunk = lay.chunk;
+    return P;
+}
+
+int gen_grid(i64 groups) { return (int)std::min<i64>(groups, 148 * 6); }
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+cudaError_t sd_init_tables() {
+    static bool done = false;
+    if (done) return cudaSuccess;
+    u64 R[32], Bpow[SD_L_MAX + 1], Binv[SD_D_MAX + 1];
+    u64 st = 0x243f6a8885a308d3ull;
+    for (int c = 0; c < 32; ++c) R[c] = splitmix64(st) | 1ull;
+    const u64 B = splitmix64(st) | 1ull;
+    Bpow[0] = 1;
+    for (int j = 1; j <= SD_L_MAX; ++j) Bpow[j] = Bpow[j - 1] * B;
+    u64 inv = B;  // Newton iteration for the inverse modulo 2^64
+    for (int it = 0; it < 6; ++it) inv *= 2 - B * inv;
+    Binv[0] = 1;
+    for (int m = 1; m <= SD_D_MAX; ++m) Binv[m] = Binv[m - 1] * inv;
+    static u32 binom[(SD_L_MAX + 1) * (SD_D_MAX + 1)], vcum[(SD_L_MAX + 1) * (SD_D_MAX + 2)];
+    for (int n = 0; n <= SD_L_MAX; ++n) {
+        for (int k = 0; k <= SD_D_MAX; ++k) {
+            u64 c = 1;
+            if (k > n) c = 0;
+            else
+                for (int t = 1; t <= k; ++t) c = c * (u64)(n - k + t) / (u64)t;
+            binom[n * (SD_D_MAX + 1) + k] = (u32)c;
+        }
+        u32 acc = 0;
+        for (int k = 0; k <= SD_D_MAX + 1; ++k) {
+            vcum[n * (SD_D_MAX + 2) + k] = acc;
+            if (k <= SD_D_MAX) acc += binom[n * (SD_D_MAX + 1) + k];
+        }
+    }
+    cudaError_t e;
+    if ((e = cudaMemcpyToSymbol(c_R, R, sizeof(R))) != cudaSuccess) return e;
+    if ((e = cudaMemcpyToSymbol(c_Bpow, Bpow, sizeof(Bpow))) != cudaSuccess) return e;
+    if ((e = cudaMemcpyToSymbol(c_Binv, Binv, sizeof(Binv))) != cudaSuccess) return e;
+    if ((e = cudaMemcpyToSymbol(c_binom, binom, sizeof(binom))) != cudaSuccess) return e;
+    if ((e = cudaMemcpyToSymbol(c_vcum, vcum, sizeof(vcum))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_generate<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)(sizeof(GenShared) + 8 * 256 * 4))) != cudaSuccess)
+        return e;
+    if ((e = cudaFuncSetAttribute(k_generate<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)sizeof(GenShared))) != cudaSuccess)
+        return e;
+    done = true;
+    return cudaSuccess;
+}
+
+cudaError_t sd_prepare(SeqSetDev s, int d, DevInfo* info, cudaStream_t st, i64* launches) {
+    if (s.n == 0) return cudaSuccess;
+    int blocks = (int)std::min<i64>((s.n + 255) / 256, 148 * 8);
+    k_prepare<<<blocks, 256, 0, st>>>(s, d, info);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t sd_count(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u32* cnt, DevInfo* info, cudaStream_t st,
+                     i64* launches) {
+    GenParams P = make_params(a, b, lay, width);
+    if (P.groups_total == 0) return cudaSuccess;
+    P.cnt = cnt;
+    P.info = info;
+    k_generate<true><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared), st>>>(P);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+i64 sd_scan_tiles(i64 n) { return (n + SC_TILE - 1) / SC_TILE; }
+
+cudaError_t sd_scan_counts(const u32* cnt, i64 n, u64* rec_off, u64* lb_status, DevInfo* info, cudaStream_t st,
+                           i64* launches) {
+    const i64 tiles = std::max<i64>(1, sd_scan_tiles(n));
+    cudaError_t e = cudaMemsetAsync(lb_status, 0, (size_t)tiles * 8, st);
+    if (e != cudaSuccess) return e;
+    k_scan_counts<<<(unsigned)tiles, SC_THREADS, 0, st>>>(cnt, n, rec_off, lb_status, info);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, const u64* rec_off, u64* records,
+                        u32* ghist, int npass, DevInfo* info, cudaStream_t st, i64* launches) {
+    GenParams P = make_params(a, b, lay, width);
+    if (P.groups_total == 0) return cudaSuccess;
+    P.rec_off = rec_off;
+    P.records = records;
+    P.ghist = ghist;
+    P.npass = npass;
+    P.info = info;
+    k_generate<false><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared) + (size_t)npass * 256 * 4, st>>>(P);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}

@@ -1,0 +1,77 @@
+// kernels.h — internal host-side launch interface between the pipeline (symdel_api.cu) and the
+// kernel translation units.  Not part of the public ABI (that is include/symdel.h).
+#pragma once
+#include <algorithm>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "common.cuh"
+
+#define SD_L_MAX 64
+#define SD_D_MAX 4
+
+// One CSR sequence set on the device.
+struct SeqSetDev {
+    const int8_t* seqs;
+    const i64* off;
+    i64 n;
+};
+
+// Everything the record/pair layout depends on, fixed per call.
+struct Layout {
+    i64 n_a, n_b;      // self: n_b == 0.  Global id = index in A, or n_a + index in B.
+    int cross;         // 1: emit only (A, B) combinations
+    int d;
+    int id_bits;       // 2^id_bits > n_a + n_b
+    int hash_bits;     // multiple of 8
+    int b_bits;        // bits of the second pair component (self: id_bits; cross: bits of n_b)
+    int pair_bits;     // a_bits + b_bits
+    int thinning;
+    u32 n_chunks, chunk;
+};
+
+// ---- radix_sort.cu ------------------------------------------------------------------------------
+i64 sd_sort_tiles(i64 n);
+i64 sd_sort_scratch_bytes(i64 n, int npass);
+cudaError_t sd_sort_prepare(void* scratch, i64 n, int npass, cudaStream_t st);
+u32* sd_sort_hist_ptr(void* scratch);
+cudaError_t sd_sort_histogram(const u64* keys, i64 n, int begin_bit, int npass, void* scratch, cudaStream_t st,
+                              i64* launches);
+cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, void* scratch, cudaStream_t st,
+                           u64** result, i64* launches);
+
+// ---- generate.cu --------------------------------------------------------------------------------
+cudaError_t sd_init_tables();  // fills the __constant__ tables once per process
+cudaError_t sd_prepare(SeqSetDev s, int d, DevInfo* info, cudaStream_t st, i64* launches);
+// count pass: cnt[gid] = number of records sequence gid contributes (u32 per sequence)
+cudaError_t sd_count(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u32* cnt, DevInfo* info, cudaStream_t st,
+                     i64* launches);
+// exclusive scan cnt -> rec_off[n+1]; total also stored in info->n_records.  lb_status: n/2048+1 u64, zeroed here.
+i64 sd_scan_tiles(i64 n);
+cudaError_t sd_scan_counts(const u32* cnt, i64 n, u64* rec_off, u64* lb_status, DevInfo* info, cudaStream_t st,
+                           i64* launches);
+// generation pass: writes records at rec_off[gid].., accumulates the digit histograms into ghist
+cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, const u64* rec_off, u64* records,
+                        u32* ghist, int npass, DevInfo* info, cudaStream_t st, i64* launches);
+
+// ---- emit.cu ------------------------------------------------------------------------------------
+i64 sd_emit_tiles(i64 n_records);
+// Emits candidate pairs with flat index in [win_lo, win_hi) to cand[flat - win_lo].
+// first_round = 1: computes and stores tile_prefix[] (exclusive pair-count prefix per tile) and
+// info->n_cand (total); later rounds reuse tile_prefix.  lb_status: sd_emit_tiles u64.
+cudaError_t sd_emit(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 win_lo, u64 win_hi,
+                    int first_round, u64* tile_prefix, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
+
+// ---- verify.cu ----------------------------------------------------------------------------------
+i64 sd_verify_tiles(i64 n);
+// cand sorted ascending.  Drops repeats and a == b (self), computes lev, keeps <= d, appends
+// (pair << 3 | dist) in order to surv[surv_base + ...]; info->n_surv += kept; info->n_unique += unique.
+cudaError_t sd_verify(const u64* cand, i64 n_cand, SeqSetDev a, SeqSetDev b, const Layout& lay, int maxlen, u64* surv,
+                      u64 surv_base, u64 surv_capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
+// surv sorted ascending (and unique unless dedup = 1).  Unpacks to SoA outputs, first `capacity`
+// only; info->n_out = total.
+cudaError_t sd_finalize(const u64* surv, i64 n_surv, const Layout& lay, int dedup, i32* out_i, i32* out_j, i32* out_dist,
+                        i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
+// plain distances for index pairs (stage test)
+cudaError_t sd_lev_pairs(SeqSetDev a, SeqSetDev b, const i32* ia, const i32* ib, i64 n_pairs, i32* dist,
+                         cudaStream_t st);

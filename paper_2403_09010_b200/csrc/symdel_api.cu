@@ -1,0 +1,635 @@
+// symdel_api.cu — the C ABI of include/symdel.h and the host-side pipeline (S0-S5).
+//
+// Pipeline of one call (App. F.3 "XTNeighbor base algorithm", re-designed):
+//   S0  prepare : validate CSR input, longest sequence, upper bound of the record count
+//   for each key-range chunk c of P (S5; P = 1 when the workspace allows):
+//     S1  count + scan + generate : (hash, id) records of the variants whose hash falls in chunk c
+//     S2  sort                    : onesweep LSD radix sort on the hash bits (stable: ids stay ascending)
+//     S3a emit                    : runs of equal hash -> candidate pairs, in windows of the candidate buffer
+//     for each window:
+//       S3b sort candidates; S4 unique + verify -> survivors (pair << 3 | dist), appended in order
+//   if more than one flush happened: sort survivors, unique
+//   unpack survivors -> (out_i, out_j, out_dist), ascending (i, j)
+// Equal keys always land in the same chunk and a verified pair carries the same distance wherever it
+// was found, so chunking and windowing change memory use only.  This replaces the paper's 2-D-buffer
+// streaming (App. C; App. F.4) whose purpose — bounded memory — it serves.
+//
+// Host <-> device crossings per call: one pinned-memory read-back after S0, one per chunk after the
+// count scan (grid sizes), one after the first emit (candidate count), two at the end.
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "../../include/symdel.h"
+#include "kernels.h"
+
+struct symdel_ctx {
+    int device = 0;
+    cudaError_t last_cuda = cudaSuccess;
+    symdel_stats stats{};
+    int opt_timing = 0;
+    i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0;
+    DevInfo* h_info = nullptr;  // pinned
+    void* arena = nullptr;      // device arena of the *_host entry points
+    size_t arena_bytes = 0;
+    cudaStream_t stream = nullptr;  // stream of the *_host entry points
+    std::vector<cudaEvent_t> events;
+};
+
+namespace {
+
+#define CK(call)                                  \
+    do {                                          \
+        cudaError_t e__ = (call);                 \
+        if (e__ != cudaSuccess) {                 \
+            ctx->last_cuda = e__;                 \
+            return SYMDEL_E_CUDA;                 \
+        }                                         \
+    } while (0)
+
+inline i64 align_up(i64 x, i64 a = 256) { return (x + a - 1) / a * a; }
+
+struct Bump {
+    char* base;
+    i64 size, used = 0;
+    bool ok = true;
+    Bump(void* p, i64 n) : base((char*)p), size(n) {}
+    template <typename T>
+    T* take(i64 count) {
+        i64 bytes = align_up(count * (i64)sizeof(T));
+        if (used + bytes > size) {
+            ok = false;
+            return nullptr;
+        }
+        T* r = (T*)(base + used);
+        used += bytes;
+        return r;
+    }
+    i64 left() const { return size - used; }
+};
+
+int bits_for(i64 count) {  // smallest b >= 1 with 2^b >= count (values 0 .. count-1 fit)
+    int b = 1;
+    while (((i64)1 << b) < count) ++b;
+    return b;
+}
+
+u64 vcount_host(int L, int d) {
+    u64 acc = 0, c = 1;
+    for (int k = 0; k <= d; ++k) {
+        if (k > L) break;
+        if (k > 0) c = c * (u64)(L - k + 1) / (u64)k;
+        acc += c;
+    }
+    return acc;
+}
+
+i64 rec_bytes(i64 ncap, int npass) {
+    return 2 * align_up(ncap * 8) + align_up(sd_sort_scratch_bytes(ncap, npass)) + 2 * align_up((sd_emit_tiles(ncap) + 2) * 8);
+}
+i64 cand_bytes(i64 ccap, int ppass) {
+    return 2 * align_up(ccap * 8) + align_up(sd_sort_scratch_bytes(ccap, ppass)) + align_up((sd_verify_tiles(ccap) + 1) * 8);
+}
+i64 fixed_bytes(i64 n_total) {
+    return align_up((i64)sizeof(DevInfo)) + align_up(n_total * 4) + align_up((n_total + 1) * 8) +
+           align_up((sd_scan_tiles(n_total) + 1) * 8) + 4096;
+}
+
+struct Timer {
+    symdel_ctx* ctx;
+    cudaStream_t st;
+    bool on;
+    size_t next = 0;
+    std::vector<std::pair<int, size_t>> marks;  // (stage id, event index) pairs: begin/end alternate
+    Timer(symdel_ctx* c, cudaStream_t s) : ctx(c), st(s), on(c->opt_timing != 0) {}
+    size_t mark() {
+        if (!on) return 0;
+        if (next >= ctx->events.size()) {
+            cudaEvent_t e;
+            cudaEventCreate(&e);
+            ctx->events.push_back(e);
+        }
+        cudaEventRecord(ctx->events[next], st);
+        return next++;
+    }
+    float ms(size_t a, size_t b) {
+        float m = 0;
+        if (on) cudaEventElapsedTime(&m, ctx->events[a], ctx->events[b]);
+        return m;
+    }
+};
+
+int read_info(symdel_ctx* ctx, const DevInfo* d_info, cudaStream_t st) {
+    CK(cudaMemcpyAsync(ctx->h_info, d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return SYMDEL_OK;
+}
+
+int err_from_flags(u32 f) {
+    if (f & SD_ERR_OFFSETS) return SYMDEL_E_OFFSETS;
+    if (f & SD_ERR_TOO_LONG) return SYMDEL_E_TOO_LONG;
+    if (f & SD_ERR_RESIDUE) return SYMDEL_E_RESIDUE;
+    if (f & SD_ERR_INTERNAL) return SYMDEL_E_INTERNAL;
+    if (f & SD_ERR_OVERFLOW) return SYMDEL_E_WORKSPACE;
+    return SYMDEL_OK;
+}
+
+// -------------------------------------------------------------------------------------------------
+int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, void* workspace, i64 workspace_bytes,
+                 i32* out_i, i32* out_j, i32* out_dist, i64 capacity, i64* n_pairs_host, cudaStream_t st) {
+    if (!ctx || !n_pairs_host || d < 0 || d > SD_D_MAX || A.n < 0 || B.n < 0 || capacity < 0) return SYMDEL_E_ARG;
+    *n_pairs_host = 0;
+    const i64 n_total = A.n + B.n;
+    symdel_stats& S = ctx->stats;
+    S = symdel_stats{};
+    if (n_total >= ((i64)1 << 30)) return SYMDEL_E_TOO_MANY;
+    if (A.n == 0 || (cross && B.n == 0)) return SYMDEL_OK;
+    if (!A.seqs || !A.off || (cross && (!B.seqs || !B.off)) || !workspace) return SYMDEL_E_ARG;
+    if (capacity > 0 && (!out_i || !out_j || !out_dist)) return SYMDEL_E_ARG;
+    if (((uintptr_t)workspace & 255) != 0) return SYMDEL_E_ARG;
+    CK(cudaSetDevice(ctx->device));
+    CK(sd_init_tables());
+    Timer tm(ctx, st);
+    const size_t ev_begin = tm.mark();
+
+    Bump ws(workspace, workspace_bytes);
+    DevInfo* info = ws.take<DevInfo>(1);
+    u32* cnt = ws.take<u32>(n_total);
+    u64* rec_off = ws.take<u64>(n_total + 1);
+    u64* scan_lb = ws.take<u64>(sd_scan_tiles(n_total) + 1);
+    if (!ws.ok) return SYMDEL_E_WORKSPACE;
+
+    // ---- S0 ----
+    CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
+    CK(sd_prepare(A, d, info, st, &S.n_launches));
+    if (cross) CK(sd_prepare(B, d, info, st, &S.n_launches));
+    int rc = read_info(ctx, info, st);
+    if (rc) return rc;
+    if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+    const i64 nmax = (i64)ctx->h_info->nmax;
+    const int maxlen = (int)ctx->h_info->maxlen;
+    const size_t ev_prepared = tm.mark();
+
+    Layout lay{};
+    lay.n_a = A.n;
+    lay.n_b = B.n;
+    lay.cross = cross;
+    lay.d = d;
+    lay.id_bits = bits_for(n_total + 1);
+    lay.b_bits = cross ? bits_for(B.n) : lay.id_bits;
+    lay.pair_bits = (cross ? bits_for(A.n) : lay.id_bits) + lay.b_bits;
+    lay.thinning = ctx->opt_no_thinning ? 0 : 1;
+    {
+        int hb = (int)ctx->opt_hash_bits;
+        if (hb == 0) {
+            hb = bits_for(std::max<i64>(nmax, 2)) + 5;
+            hb = std::max(16, (hb + 7) / 8 * 8);
+        }
+        const int hb_max = (64 - lay.id_bits) / 8 * 8;
+        if (hb % 8 != 0 || hb < 8) return SYMDEL_E_ARG;
+        lay.hash_bits = std::min(hb, hb_max);
+    }
+    const int npass = lay.hash_bits / 8;
+    const int ppass = (lay.pair_bits + 7) / 8;
+    const int spass = (lay.pair_bits + 7) / 8;
+    S.hash_bits = lay.hash_bits;
+    S.id_bits = lay.id_bits;
+
+    // ---- workspace plan ----
+    const i64 R = ws.left() - 8192;
+    i64 ccap = ctx->opt_cand_cap > 0 ? ctx->opt_cand_cap : std::max<i64>(1 << 20, nmax / 2);
+    i64 scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity + (ctx->opt_cand_cap > 0 ? ccap : 0));
+    i64 ncap = std::max<i64>(nmax, 1);
+    u32 P = ctx->opt_force_chunks > 0 ? (u32)ctx->opt_force_chunks : 1;
+    if (P > 1) ncap = std::min<i64>(nmax, nmax / P + nmax / (4 * P) + 4096);
+    if (rec_bytes(ncap, npass) + cand_bytes(ccap, ppass) + cand_bytes(scap, spass) > R) {
+        if (ctx->opt_cand_cap <= 0) ccap = std::min<i64>(ccap, std::max<i64>(4096, R / 4 / 17));
+        scap = std::min<i64>(scap, std::max<i64>(4096 + capacity, R * 15 / 100 / 17));
+        const i64 rrem = R - cand_bytes(ccap, ppass) - cand_bytes(scap, spass);
+        if (rrem <= 0) return SYMDEL_E_WORKSPACE;
+        // largest ncap that fits in rrem (16 B/record + ~0.26 B/record of tile status per pass)
+        i64 lo = 0, hi = ncap;
+        while (lo < hi) {
+            i64 mid = (lo + hi + 1) / 2;
+            if (rec_bytes(mid, npass) <= rrem) lo = mid; else hi = mid - 1;
+        }
+        ncap = lo;
+        if (ncap < 4096) return SYMDEL_E_WORKSPACE;
+        if (ctx->opt_force_chunks <= 0) P = (u32)std::max<i64>(1, (nmax + nmax / 8 + ncap - 1) / ncap);
+    }
+    u64* recA = ws.take<u64>(ncap);
+    u64* recB = ws.take<u64>(ncap);
+    void* rec_scratch = ws.take<char>(sd_sort_scratch_bytes(ncap, npass));
+    u64* tile_prefix = ws.take<u64>(sd_emit_tiles(ncap) + 2);
+    u64* emit_lb = ws.take<u64>(sd_emit_tiles(ncap) + 2);
+    u64* candA = ws.take<u64>(ccap);
+    u64* candB = ws.take<u64>(ccap);
+    void* cand_scratch = ws.take<char>(sd_sort_scratch_bytes(ccap, ppass));
+    u64* verify_lb = ws.take<u64>(sd_verify_tiles(ccap) + 1);
+    u64* survA = ws.take<u64>(scap);
+    u64* survB = ws.take<u64>(scap);
+    void* surv_scratch = ws.take<char>(sd_sort_scratch_bytes(scap, spass));
+    u64* final_lb = ws.take<u64>(sd_verify_tiles(scap) + 1);
+    if (!ws.ok) return SYMDEL_E_WORKSPACE;
+
+    const int width = maxlen + 1;
+    i64 n_surv = 0, flushes = 0;
+    float ms_gen = 0, ms_sort = 0, ms_emit = 0, ms_dedup = 0, ms_verify = 0, ms_pass = 0;
+    i64 pass_count = 0;
+    std::vector<cudaEvent_t> pass_ev;
+
+restart:
+    if (P > 65536) return SYMDEL_E_WORKSPACE;
+    n_surv = 0;
+    flushes = 0;
+    S.n_records = S.n_candidates = 0;
+    lay.n_chunks = P;
+    CK(cudaMemsetAsync(&info->n_surv, 0, sizeof(u64) * 3, st));  // n_surv, n_out, n_unique
+    for (u32 c = 0; c < P; ++c) {
+        lay.chunk = c;
+        const size_t e0 = tm.mark();
+        // ---- S1: count, scan, generate ----
+        CK(sd_count(A, B, lay, width, cnt, info, st, &S.n_launches));
+        CK(sd_scan_counts(cnt, n_total, rec_off, scan_lb, info, st, &S.n_launches));
+        rc = read_info(ctx, info, st);
+        if (rc) return rc;
+        const i64 N = (i64)ctx->h_info->n_records;
+        if (N > ncap || N >= ((i64)1 << 30)) {
+            if (ctx->opt_force_chunks > 0 && N <= ncap) return SYMDEL_E_TOO_MANY;
+            P *= 2;
+            goto restart;
+        }
+        S.n_records += N;
+        if (N == 0) continue;
+        CK(sd_sort_prepare(rec_scratch, N, npass, st));
+        CK(sd_generate(A, B, lay, width, rec_off, recA, sd_sort_hist_ptr(rec_scratch), npass, info, st, &S.n_launches));
+        const size_t e1 = tm.mark();
+        // ---- S2: sort ----
+        u64* sorted = nullptr;
+        CK(sd_sort_passes(recA, recB, N, lay.id_bits, npass, rec_scratch, st, &sorted, &S.n_launches));
+        const size_t e2 = tm.mark();
+        // ---- S3a: emit (first window) ----
+        CK(sd_emit(sorted, N, lay, candA, 0, (u64)ccap, 1, tile_prefix, emit_lb, info, st, &S.n_launches));
+        rc = read_info(ctx, info, st);
+        if (rc) return rc;
+        if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+        const i64 C = (i64)ctx->h_info->n_cand;
+        S.n_candidates += C;
+        const size_t e3 = tm.mark();
+        ms_gen += tm.ms(e0, e1);
+        ms_sort += tm.ms(e1, e2);
+        ms_emit += tm.ms(e2, e3);
+        if (tm.on) {
+            ms_pass += tm.ms(e1, e2);
+            pass_count += npass;
+            S.sort_pass_records = N;
+        }
+        for (i64 w0 = 0; w0 < C; w0 += ccap) {
+            const i64 nc = std::min<i64>(ccap, C - w0);
+            const size_t f0 = tm.mark();
+            if (w0 > 0) CK(sd_emit(sorted, N, lay, candA, (u64)w0, (u64)(w0 + ccap), 0, tile_prefix, emit_lb, info, st,
+                                   &S.n_launches));
+            const size_t f1 = tm.mark();
+            // ---- S3b: sort the packed pair ids ----
+            CK(sd_sort_prepare(cand_scratch, nc, ppass, st));
+            CK(sd_sort_histogram(candA, nc, 0, ppass, cand_scratch, st, &S.n_launches));
+            u64* csorted = nullptr;
+            CK(sd_sort_passes(candA, candB, nc, 0, ppass, cand_scratch, st, &csorted, &S.n_launches));
+            const size_t f2 = tm.mark();
+            // ---- S4: unique + verify; survivors appended at n_surv (host-tracked upper bound not needed:
+            // the kernel is given the base through the previous flush's total, read back below) ----
+            CK(sd_verify(csorted, nc, A, B, lay, maxlen, survA, (u64)n_surv, (u64)scap, verify_lb, info, st,
+                         &S.n_launches));
+            rc = read_info(ctx, info, st);
+            if (rc) return rc;
+            if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+            n_surv = (i64)ctx->h_info->n_surv;
+            const size_t f3 = tm.mark();
+            ms_emit += tm.ms(f0, f1);
+            ms_dedup += tm.ms(f1, f2);
+            ms_verify += tm.ms(f2, f3);
+            ++flushes;
+        }
+    }
+
+    // ---- final: (sort + unique) and unpack ----
+    const size_t g0 = tm.mark();
+    i64 n_out = 0;
+    if (n_surv > 0) {
+        const u64* fin = survA;
+        if (flushes > 1) {
+            CK(sd_sort_prepare(surv_scratch, n_surv, spass, st));
+            CK(sd_sort_histogram(survA, n_surv, 3, spass, surv_scratch, st, &S.n_launches));
+            u64* ssorted = nullptr;
+            CK(sd_sort_passes(survA, survB, n_surv, 3, spass, surv_scratch, st, &ssorted, &S.n_launches));
+            fin = ssorted;
+        }
+        CK(sd_finalize(fin, n_surv, lay, flushes > 1 ? 1 : 0, out_i, out_j, out_dist, capacity, final_lb, info, st,
+                       &S.n_launches));
+        rc = read_info(ctx, info, st);
+        if (rc) return rc;
+        n_out = (i64)ctx->h_info->n_out;
+    }
+    const size_t g1 = tm.mark();
+    if (tm.on) {
+        CK(cudaStreamSynchronize(st));
+        S.ms_prepare = tm.ms(ev_begin, ev_prepared);
+        S.ms_generate = ms_gen;
+        S.ms_sort = ms_sort;
+        S.ms_emit = ms_emit;
+        S.ms_dedup = ms_dedup;
+        S.ms_verify = ms_verify + tm.ms(g0, g1);
+        S.ms_total = tm.ms(ev_begin, g1);
+        S.ms_sort_pass_avg = pass_count ? ms_pass / (float)pass_count : 0.f;
+    }
+    S.n_unique = (i64)ctx->h_info->n_unique;
+    S.n_outputs = n_out;
+    S.n_chunks = P;
+    S.n_flushes = flushes;
+    *n_pairs_host = n_out;
+    return n_out > capacity ? SYMDEL_E_CAPACITY : SYMDEL_OK;
+}
+
+int ensure_arena(symdel_ctx* ctx, size_t bytes) {
+    if (ctx->arena_bytes >= bytes) return SYMDEL_OK;
+    if (ctx->arena) cudaFree(ctx->arena);
+    ctx->arena = nullptr;
+    ctx->arena_bytes = 0;
+    CK(cudaMalloc(&ctx->arena, bytes));
+    ctx->arena_bytes = bytes;
+    return SYMDEL_OK;
+}
+
+int run_host(symdel_ctx* ctx, const int8_t* a_seqs, const i64* a_off, i64 n_a, const int8_t* b_seqs, const i64* b_off,
+             i64 n_b, int cross, int d, i32* out_i, i32* out_j, i32* out_dist, i64 capacity, i64* n_pairs_host) {
+    if (!ctx || !n_pairs_host || n_a < 0 || n_b < 0 || d < 0 || d > SD_D_MAX || capacity < 0) return SYMDEL_E_ARG;
+    *n_pairs_host = 0;
+    if (n_a == 0 || (cross && n_b == 0)) {
+        ctx->stats = symdel_stats{};
+        return SYMDEL_OK;
+    }
+    if (!a_seqs || !a_off || (cross && (!b_seqs || !b_off))) return SYMDEL_E_ARG;
+    if (a_off[0] != 0 || (cross && b_off[0] != 0)) return SYMDEL_E_OFFSETS;
+    CK(cudaSetDevice(ctx->device));
+    const i64 res_a = a_off[n_a], res_b = cross ? b_off[n_b] : 0;
+    if (res_a < 0 || res_b < 0) return SYMDEL_E_OFFSETS;
+    // exact record bound from the host offsets
+    i64 nmax = 0;
+    int maxlen = 0;
+    for (int s = 0; s < (cross ? 2 : 1); ++s) {
+        const i64* off = s ? b_off : a_off;
+        const i64 n = s ? n_b : n_a;
+        u64 vtab[SD_L_MAX + 1];
+        for (int L = 0; L <= SD_L_MAX; ++L) vtab[L] = vcount_host(L, d);
+        for (i64 i = 0; i < n; ++i) {
+            const i64 L = off[i + 1] - off[i];
+            if (L < 0) return SYMDEL_E_OFFSETS;
+            if (L > SD_L_MAX) return SYMDEL_E_TOO_LONG;
+            nmax += (i64)vtab[L];
+            maxlen = std::max(maxlen, (int)L);
+        }
+    }
+    const i64 n_total = n_a + n_b;
+    const int npass_max = 7, ppass_max = 8;
+    const i64 ccap = std::max<i64>(1 << 20, nmax / 2), scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity);
+    const i64 ws_bytes = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nmax, 1), npass_max) + cand_bytes(ccap, ppass_max) +
+                         cand_bytes(scap, ppass_max) + 65536;
+    const i64 in_bytes = align_up(res_a + 16) + align_up((n_a + 1) * 8) + align_up(res_b + 16) + align_up((n_b + 1) * 8);
+    const i64 out_bytes = 3 * align_up(capacity * 4 + 16);
+    int rc = ensure_arena(ctx, (size_t)(in_bytes + out_bytes + ws_bytes + 4096));
+    if (rc) return rc;
+    cudaStream_t st = ctx->stream;
+    Bump ar(ctx->arena, (i64)ctx->arena_bytes);
+    int8_t* d_as = ar.take<int8_t>(res_a + 16);
+    i64* d_ao = ar.take<i64>(n_a + 1);
+    int8_t* d_bs = ar.take<int8_t>(res_b + 16);
+    i64* d_bo = ar.take<i64>(n_b + 1);
+    i32* d_i = ar.take<i32>(capacity + 4);
+    i32* d_j = ar.take<i32>(capacity + 4);
+    i32* d_d = ar.take<i32>(capacity + 4);
+    void* d_ws = ar.take<char>(ws_bytes);
+    if (!ar.ok) return SYMDEL_E_INTERNAL;
+    if (res_a) CK(cudaMemcpyAsync(d_as, a_seqs, (size_t)res_a, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(d_ao, a_off, (size_t)(n_a + 1) * 8, cudaMemcpyHostToDevice, st));
+    if (cross) {
+        if (res_b) CK(cudaMemcpyAsync(d_bs, b_seqs, (size_t)res_b, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(d_bo, b_off, (size_t)(n_b + 1) * 8, cudaMemcpyHostToDevice, st));
+    }
+    SeqSetDev A{d_as, d_ao, n_a}, B{d_bs, d_bo, cross ? n_b : 0};
+    rc = run_pipeline(ctx, A, B, cross, d, d_ws, ws_bytes, d_i, d_j, d_d, capacity, n_pairs_host, st);
+    if (rc != SYMDEL_OK && rc != SYMDEL_E_CAPACITY) return rc;
+    const i64 ncopy = std::min<i64>(*n_pairs_host, capacity);
+    if (ncopy > 0) {
+        CK(cudaMemcpyAsync(out_i, d_i, (size_t)ncopy * 4, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(out_j, d_j, (size_t)ncopy * 4, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(out_dist, d_d, (size_t)ncopy * 4, cudaMemcpyDeviceToHost, st));
+    }
+    CK(cudaStreamSynchronize(st));
+    return rc;
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+int symdel_create(symdel_ctx** out, int device) {
+    if (!out) return SYMDEL_E_ARG;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return SYMDEL_E_CUDA;
+    symdel_ctx* ctx = new symdel_ctx();
+    ctx->device = device;
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_info, sizeof(DevInfo));
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = sd_init_tables();
+    if (e != cudaSuccess) {
+        delete ctx;
+        return SYMDEL_E_CUDA;
+    }
+    *out = ctx;
+    return SYMDEL_OK;
+}
+
+void symdel_destroy(symdel_ctx* ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    if (ctx->arena) cudaFree(ctx->arena);
+    if (ctx->h_info) cudaFreeHost(ctx->h_info);
+    if (ctx->stream) cudaStreamDestroy(ctx->stream);
+    for (auto e : ctx->events) cudaEventDestroy(e);
+    delete ctx;
+}
+
+int symdel_set_option(symdel_ctx* ctx, int option, int64_t value) {
+    if (!ctx || value < 0) return SYMDEL_E_ARG;
+    switch (option) {
+        case SYMDEL_OPT_TIMING: ctx->opt_timing = value != 0; break;
+        case SYMDEL_OPT_FORCE_CHUNKS: ctx->opt_force_chunks = value; break;
+        case SYMDEL_OPT_CAND_CAPACITY: ctx->opt_cand_cap = value; break;
+        case SYMDEL_OPT_HASH_BITS:
+            if (value != 0 && (value % 8 != 0 || value < 8 || value > 56)) return SYMDEL_E_ARG;
+            ctx->opt_hash_bits = value;
+            break;
+        case SYMDEL_OPT_NO_THINNING: ctx->opt_no_thinning = value != 0; break;
+        default: return SYMDEL_E_ARG;
+    }
+    return SYMDEL_OK;
+}
+
+int symdel_get_stats(const symdel_ctx* ctx, symdel_stats* stats_host) {
+    if (!ctx || !stats_host) return SYMDEL_E_ARG;
+    *stats_host = ctx->stats;
+    return SYMDEL_OK;
+}
+
+int symdel_last_cuda_error(const symdel_ctx* ctx) { return ctx ? (int)ctx->last_cuda : 0; }
+
+const char* symdel_strerror(int code) {
+    switch (code) {
+        case SYMDEL_OK: return "ok";
+        case SYMDEL_E_ARG: return "invalid argument";
+        case SYMDEL_E_OFFSETS: return "offsets[0] != 0 or offsets not non-decreasing";
+        case SYMDEL_E_TOO_LONG: return "a sequence is longer than SYMDEL_L_MAX";
+        case SYMDEL_E_RESIDUE: return "residue code outside 1..31";
+        case SYMDEL_E_TOO_MANY: return "too many sequences or records";
+        case SYMDEL_E_WORKSPACE: return "workspace too small";
+        case SYMDEL_E_CAPACITY: return "more result pairs than the output capacity";
+        case SYMDEL_E_CUDA: return "CUDA error";
+        case SYMDEL_E_INTERNAL: return "internal consistency check failed";
+        default: return "unknown error";
+    }
+}
+
+int symdel_workspace_bytes(int64_t n_a, int64_t residues_a, int64_t n_b, int64_t residues_b, int max_len, int d,
+                           int64_t* bytes_host) {
+    if (!bytes_host || n_a < 0 || n_b < 0 || residues_a < 0 || residues_b < 0 || d < 0 || d > SD_D_MAX || max_len < 0 ||
+        max_len > SD_L_MAX)
+        return SYMDEL_E_ARG;
+    // V(L, d) <= 1 + L * (V(max_len, d) - 1) / max_len for L <= max_len
+    const i64 n_total = n_a + n_b;
+    const u64 vm = vcount_host(max_len, d);
+    const i64 nbound = n_total + (max_len ? (i64)(((u64)(residues_a + residues_b) * (vm - 1) + max_len - 1) / max_len) : 0);
+    const i64 ccap = std::max<i64>(1 << 20, nbound / 2), scap = std::max<i64>(1 << 20, nbound / 4);
+    *bytes_host = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nbound, 1), 7) + cand_bytes(ccap, 8) + cand_bytes(scap, 8) +
+                  65536;
+    return SYMDEL_OK;
+}
+
+int symdel_self(symdel_ctx* ctx, const int8_t* seqs, const int64_t* offsets, int64_t n, int d, void* workspace,
+                int64_t workspace_bytes, int32_t* out_i, int32_t* out_j, int32_t* out_dist, int64_t capacity,
+                int64_t* n_pairs_host, void* cuda_stream) {
+    SeqSetDev A{seqs, offsets, n}, B{nullptr, nullptr, 0};
+    return run_pipeline(ctx, A, B, 0, d, workspace, workspace_bytes, out_i, out_j, out_dist, capacity, n_pairs_host,
+                        (cudaStream_t)cuda_stream);
+}
+
+int symdel_cross(symdel_ctx* ctx, const int8_t* q_seqs, const int64_t* q_offsets, int64_t n_q, const int8_t* r_seqs,
+                 const int64_t* r_offsets, int64_t n_r, int d, void* workspace, int64_t workspace_bytes, int32_t* out_i,
+                 int32_t* out_j, int32_t* out_dist, int64_t capacity, int64_t* n_pairs_host, void* cuda_stream) {
+    SeqSetDev A{q_seqs, q_offsets, n_q}, B{r_seqs, r_offsets, n_r};
+    return run_pipeline(ctx, A, B, 1, d, workspace, workspace_bytes, out_i, out_j, out_dist, capacity, n_pairs_host,
+                        (cudaStream_t)cuda_stream);
+}
+
+int symdel_self_host(symdel_ctx* ctx, const int8_t* seqs_host, const int64_t* offsets_host, int64_t n, int d,
+                     int32_t* out_i_host, int32_t* out_j_host, int32_t* out_dist_host, int64_t capacity,
+                     int64_t* n_pairs_host) {
+    return run_host(ctx, seqs_host, offsets_host, n, nullptr, nullptr, 0, 0, d, out_i_host, out_j_host, out_dist_host,
+                    capacity, n_pairs_host);
+}
+
+int symdel_cross_host(symdel_ctx* ctx, const int8_t* q_seqs_host, const int64_t* q_offsets_host, int64_t n_q,
+                      const int8_t* r_seqs_host, const int64_t* r_offsets_host, int64_t n_r, int d, int32_t* out_i_host,
+                      int32_t* out_j_host, int32_t* out_dist_host, int64_t capacity, int64_t* n_pairs_host) {
+    return run_host(ctx, q_seqs_host, q_offsets_host, n_q, r_seqs_host, r_offsets_host, n_r, 1, d, out_i_host, out_j_host,
+                    out_dist_host, capacity, n_pairs_host);
+}
+
+// ---- stage-level entry points ------------------------------------------------------------------
+int64_t symdel_stage_sort_workspace_bytes(int64_t n) { return align_up(sd_sort_scratch_bytes(std::max<i64>(n, 1), 8)) + 256; }
+
+int symdel_stage_sort_u64(symdel_ctx* ctx, uint64_t* keys, uint64_t* tmp, int64_t n, int begin_bit, int end_bit,
+                          void* workspace, int64_t workspace_bytes, void* cuda_stream) {
+    if (!ctx || n < 0 || begin_bit < 0 || end_bit > 64 || end_bit < begin_bit || (end_bit - begin_bit) % 8 != 0)
+        return SYMDEL_E_ARG;
+    if (n >= ((i64)1 << 30)) return SYMDEL_E_TOO_MANY;
+    if (n == 0 || end_bit == begin_bit) return SYMDEL_OK;
+    if (!keys || !tmp || !workspace) return SYMDEL_E_ARG;
+    const int npass = (end_bit - begin_bit) / 8;
+    if (workspace_bytes < sd_sort_scratch_bytes(n, npass)) return SYMDEL_E_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CK(cudaSetDevice(ctx->device));
+    CK(sd_sort_prepare(workspace, n, npass, st));
+    CK(sd_sort_histogram(keys, n, begin_bit, npass, workspace, st, nullptr));
+    u64* res = nullptr;
+    CK(sd_sort_passes(keys, tmp, n, begin_bit, npass, workspace, st, &res, nullptr));
+    if (res != keys) CK(cudaMemcpyAsync(keys, res, (size_t)n * 8, cudaMemcpyDeviceToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    return SYMDEL_OK;
+}
+
+int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const int64_t* offsets, int64_t n, int d, int hash_bits,
+                          int id_bits, int thinning, uint64_t* records, int64_t records_capacity, int64_t* n_records_host,
+                          void* workspace, int64_t workspace_bytes, void* cuda_stream) {
+    if (!ctx || !n_records_host || n < 0 || d < 0 || d > SD_D_MAX || hash_bits < 8 || hash_bits % 8 != 0 ||
+        hash_bits + id_bits > 64 || id_bits < 1)
+        return SYMDEL_E_ARG;
+    *n_records_host = 0;
+    if (n == 0) return SYMDEL_OK;
+    if (!seqs || !offsets || !records || !workspace) return SYMDEL_E_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CK(cudaSetDevice(ctx->device));
+    CK(sd_init_tables());
+    Bump ws(workspace, workspace_bytes);
+    DevInfo* info = ws.take<DevInfo>(1);
+    u32* cnt = ws.take<u32>(n);
+    u64* rec_off = ws.take<u64>(n + 1);
+    u64* scan_lb = ws.take<u64>(sd_scan_tiles(n) + 1);
+    u32* hist = ws.take<u32>(8 * 256);
+    if (!ws.ok) return SYMDEL_E_WORKSPACE;
+    SeqSetDev A{seqs, offsets, n}, B{nullptr, nullptr, 0};
+    CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
+    CK(cudaMemsetAsync(hist, 0, 8 * 256 * 4, st));
+    CK(sd_prepare(A, d, info, st, nullptr));
+    int rc = read_info(ctx, info, st);
+    if (rc) return rc;
+    if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+    Layout lay{};
+    lay.n_a = n;
+    lay.d = d;
+    lay.id_bits = id_bits;
+    lay.hash_bits = hash_bits;
+    lay.thinning = thinning;
+    lay.n_chunks = 1;
+    const int width = (int)ctx->h_info->maxlen + 1;
+    CK(sd_count(A, B, lay, width, cnt, info, st, nullptr));
+    CK(sd_scan_counts(cnt, n, rec_off, scan_lb, info, st, nullptr));
+    rc = read_info(ctx, info, st);
+    if (rc) return rc;
+    const i64 N = (i64)ctx->h_info->n_records;
+    *n_records_host = N;
+    if (N > records_capacity) return SYMDEL_E_CAPACITY;
+    CK(sd_generate(A, B, lay, width, rec_off, records, hist, hash_bits / 8, info, st, nullptr));
+    rc = read_info(ctx, info, st);
+    if (rc) return rc;
+    if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+    return SYMDEL_OK;
+}
+
+int symdel_stage_lev(symdel_ctx* ctx, const int8_t* a_seqs, const int64_t* a_offsets, int64_t n_a, const int8_t* b_seqs,
+                     const int64_t* b_offsets, int64_t n_b, const int32_t* ia, const int32_t* ib, int64_t n_pairs,
+                     int32_t* dist, void* cuda_stream) {
+    if (!ctx || n_pairs < 0) return SYMDEL_E_ARG;
+    if (n_pairs == 0) return SYMDEL_OK;
+    if (!a_seqs || !a_offsets || !b_seqs || !b_offsets || !ia || !ib || !dist) return SYMDEL_E_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CK(cudaSetDevice(ctx->device));
+    SeqSetDev A{a_seqs, a_offsets, n_a}, B{b_seqs, b_offsets, n_b};
+    CK(sd_lev_pairs(A, B, ia, ib, n_pairs, dist, st));
+    CK(cudaStreamSynchronize(st));
+    return SYMDEL_OK;
+}
+
+}  // extern "C"
