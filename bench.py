@@ -1,0 +1,286 @@
+#!/usr/bin/env python
+"""bench.py — BASELINE.json metric on its workload: 1M-CDR3 d=2 self-search (config 3).
+
+    python bench.py --gpus N --steps K --warmup W            # the CUDA path (libsymdel)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle as it stands (slow)
+
+A step = one pass of the whole hot path (prepare, generate, sort, emit, dedup, verify) over the
+synthetic repertoire.  `value` = verified pairs/s with inputs resident in HBM; `e2e` = the same
+through symdel_self_host with pinned HOST buffers (H2D of the sequences and D2H of the result inside
+the timed region).  Timing: CUDA events on the launching stream, per step, with an L2 flush
+(512 MiB memset, untimed) between steps; max over ranks.  N > 1 runs N independent replicas (the
+path does not shard: DESIGN.md §Multi-GPU), one process per GPU, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+METRIC = "1M-CDR3 d=2 self-search wall time (s), verified pairs/sec, HBM GB/s vs peak"
+UNIT = "verified pairs/s"
+WORKLOAD = "config 3: self-search d=2, 1,000,000 synthetic TCRb CDR3 (seed 2), 995,218 after dedup"
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def load_peak():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return float(json.loads(p.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def load_traffic():
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture."""
+    p = ROOT / "profiles" / "traffic.json"
+    if p.exists():
+        try:
+            return json.loads(p.read_text()).get("k_onesweep_records_dram_bytes_per_launch")
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        rows = [r for ts, r in self.rows if t0 <= ts <= t1 + 0.1] or [r for _, r in self.rows]
+        sm, mx, reasons = [], None, set()
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def cpu_baseline_run(n_sample: int, d: int, s):
+    """The oracle as it stands on a bounded sample: the workload's generator and seed at n_sample
+    sequences (a prefix of the 1M set would hold seeds only, i.e. no neighbours)."""
+    from oracle import oracle
+    from paper_2403_09010_b200 import synth
+
+    sub = synth.tcr_set(n_sample, synth.CONFIGS[3]["seed"])
+    t0 = time.time()
+    i, j, dist = oracle.symdel_self(sub.seqs, sub.offsets, d)
+    dt = time.time() - t0
+    return len(i), dt
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle (oracle_symdel_self, App. F.1 hash map, 1 thread)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2403_09010_b200 import synth
+
+    kind, d, (s,) = synth.config(3)
+    n_sample = min(s.n, args.ref_sample)
+    times, pairs = [], 0
+    for it in range(args.warmup + args.steps):
+        pairs, dt = cpu_baseline_run(n_sample, d, s)
+        if it >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    value = pairs / (ms / 1e3)
+    sample = f"same generator and seed at n={n_sample}, d={d}: {pairs} pairs per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int64", "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="symdel", choices=["symdel", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); the metric is quoted on 3")
+    ap.add_argument("--ref-sample", type=int, default=80000, help="sequences in the oracle's bounded sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+
+    from paper_2403_09010_b200 import symdel, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    kind, d, sets = synth.config(args.config)
+    assert kind == "self"
+    s = sets[0]
+    ctx = symdel.Context(local)
+    ctx.symdel_set_option(symdel.OPT_TIMING, 1)
+    dev = torch.device("cuda", local)
+    seqs_d = torch.from_numpy(s.seqs).to(dev)
+    offs_d = torch.from_numpy(s.offsets).to(dev)
+    ws_bytes = symdel.symdel_workspace_bytes(s.n, s.seqs.size, 0, 0, int(s.lengths.max()), d)
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+    cap = 4 << 20
+    out = tuple(torch.empty(cap, dtype=torch.int32, device=dev) for _ in range(3))
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    # host buffers of the end-to-end arm (pinned)
+    seqs_h = torch.from_numpy(s.seqs).pin_memory()
+    offs_h = torch.from_numpy(s.offsets).pin_memory()
+    out_h = tuple(torch.empty(cap, dtype=torch.int32).pin_memory() for _ in range(3))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    stream = torch.cuda.current_stream()
+    n_out = 0
+    stats_acc = []
+
+    def step_device(timed):
+        nonlocal n_out
+        flush.zero_()  # L2 flush, outside the timed events
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        i, j, dd = ctx.symdel_self(seqs_d, offs_d, d, workspace=ws, out=out)
+        e1.record(stream)
+        e1.synchronize()
+        n_out = int(i.numel())
+        if timed:
+            stats_acc.append(ctx.symdel_get_stats())
+        return e0.elapsed_time(e1)
+
+    def step_host():
+        flush.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        k = ctx.symdel_self_host(seqs_h, offs_h, d, out_h)
+        return 1e3 * (time.perf_counter() - t0), k
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    for _ in range(args.warmup):
+        step_device(False)
+    barrier()
+    t_begin = time.time()
+    ms_steps = [step_device(True) for _ in range(args.steps)]
+    barrier()
+    t_end = time.time()
+    clocks = sampler.stop(t_begin, t_end) if sampler else None
+
+    for _ in range(max(1, args.warmup)):
+        step_host()
+    barrier()
+    e2e = [step_host() for _ in range(args.steps)]
+    barrier()
+    e2e_ms = float(np.mean([x[0] for x in e2e]))
+    assert e2e[0][1] == n_out
+
+    ms = float(np.mean(ms_steps))
+    if dist is not None:
+        t = torch.tensor([ms, e2e_ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_ms = float(t[0]), float(t[1])
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    st = stats_acc[-1]
+    n_rec = st["sort_pass_records"]
+    pass_ms = float(np.mean([x["ms_sort_pass_avg"] for x in stats_acc]))
+    peak, peak_src = load_peak()
+    achieved = 16.0 * n_rec / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
+    stage = {k: float(np.mean([x[k] for x in stats_acc])) for k in
+             ("ms_prepare", "ms_generate", "ms_sort", "ms_emit", "ms_dedup", "ms_verify", "ms_total")}
+    # algorithmic bytes of the whole step: 8 (gen write) + 16/pass + 8 (emit read) per record,
+    # 8 + 8 + 16/pass + 8 per candidate, 12 per output, + inputs
+    npass = st["hash_bits"] // 8
+    ppass = (2 * st["id_bits"] + 7) // 8
+    step_bytes = n_rec * (8 + 16 * npass + 8) + st["n_candidates"] * (8 + 8 + 16 * ppass + 8) + n_out * 12 + s.seqs.size + 8 * (s.n + 1)
+    line = {
+        "metric": METRIC, "value": world * n_out / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u64", "data": "synthetic",
+        "config": {"workload": WORKLOAD if args.config == 3 else f"config {args.config}", "n": s.n, "d": d,
+                   "pairs_per_step": n_out, "records": n_rec, "candidates": st["n_candidates"],
+                   "unique_candidates": st["n_unique"], "hash_bits": st["hash_bits"], "id_bits": st["id_bits"],
+                   "chunks": st["n_chunks"], "l2": "flushed between steps (512 MiB memset, untimed)",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "wall_time_s": ms * 1e-3, "records_per_s": world * n_rec / (ms * 1e-3),
+        "step_hbm_gbs": step_bytes / (ms * 1e-3) / 1e9, "step_hbm_frac": step_bytes / (ms * 1e-3) / 1e9 / peak,
+        "stage_ms": stage,
+        "e2e": {"value": world * n_out / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": int(s.seqs.nbytes + s.offsets.nbytes), "d2h_bytes_per_step": int(12 * n_out),
+                "api": "symdel_self_host (pinned host buffers)"},
+        "gpu_launches": int(sum(x["n_launches"] for x in stats_acc)),
+        "roofline": {"bound": "hbm", "kernel": "k_onesweep (one 8-bit LSD pass over the variant records)",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": load_traffic(), "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": 16 * n_rec, "launch_ms": pass_ms,
+                     "frac_of_nominal_8000": achieved / 8000.0},
+        "clocks": clocks,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        n_sample = min(s.n, args.ref_sample)
+        pairs, dt = cpu_baseline_run(n_sample, d, s)
+        line["cpu_baseline"] = {"value": pairs / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"same generator and seed at n={n_sample}, d={d}: {pairs} pairs in {dt:.1f} s "
+                                          "(oracle_symdel_self, App. F.1 hash map)"}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

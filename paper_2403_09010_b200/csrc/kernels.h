@@ -32,11 +32,13 @@ struct Layout {
 
 // ---- radix_sort.cu ------------------------------------------------------------------------------
 i64 sd_sort_tiles(i64 n);
+int sd_sort_set_variant(int v);  // tuning hook: tile shape of k_onesweep
 i64 sd_sort_scratch_bytes(i64 n, int npass);
 cudaError_t sd_sort_prepare(void* scratch, i64 n, int npass, cudaStream_t st);
 u32* sd_sort_hist_ptr(void* scratch);
 cudaError_t sd_sort_histogram(const u64* keys, i64 n, int begin_bit, int npass, void* scratch, cudaStream_t st,
                               i64* launches);
+cudaError_t sd_sort_hist_scan(void* scratch, int npass, cudaStream_t st, i64* launches);
 cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, void* scratch, cudaStream_t st,
                            u64** result, i64* launches);
 

@@ -47,77 +47,82 @@ __global__ void __launch_bounds__(256) k_hist_scan(u32* __restrict__ ghist) {
 #define OS_FLAG_PRE (2u << 30)
 #define OS_MASK ((1u << 30) - 1)
 
-template <int THREADS, int IPT>
-__global__ void __launch_bounds__(THREADS) k_onesweep(const u64* __restrict__ in, u64* __restrict__ out, u32 n, int shift,
-                                                     const u32* __restrict__ gbase, u32* __restrict__ status,
-                                                     u32* __restrict__ ticket) {
-    constexpr int TILE = THREADS * IPT, NW = THREADS / 32;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    u64* skeys = reinterpret_cast<u64*>(smem_raw);   // TILE keys, digit order
-    u32* whist = reinterpret_cast<u32*>(skeys + TILE);  // NW x 256 per-warp digit counters
-    u32* s_tstart = whist + NW * 256;                 // 256: start of each digit inside the tile
-    u32* s_gofs = s_tstart + 256;                     // 256: global offset of digit d minus s_tstart[d]
-    __shared__ u32 s_tile;
-    __shared__ u32 s_warp[NW + 1];
+// Peer mask of the lanes holding the same 8-bit digit, built from 8 ballots (the MATCH.ANY
+// instruction measured ~170 cycles per warp on sm_100a; 8 x (VOTE + LOP3) is ~10x cheaper).
+__device__ __forceinline__ u32 os_match8(u32 dg, u32 init) {
+    u32 peers = init;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+        const bool bit = (dg >> b) & 1u;
+        const u32 v = __ballot_sync(SD_FULL, bit);
+        peers &= bit ? v : ~v;
+    }
+    return peers;
+}
 
+template <int THREADS, int IPT, bool FULLT>
+__device__ __forceinline__ void os_tile(const u64* __restrict__ in, u64* __restrict__ out, const u32 base, const u32 tile_n,
+                                        const u32 tile, const int shift, const u32* __restrict__ gbase,
+                                        u32* __restrict__ status, u64* skeys, u32* whist, u32* s_gofs, u32* s_warp) {
+    constexpr int NW = THREADS / 32;
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
-    for (int i = tid; i < NW * 256; i += THREADS) whist[i] = 0;
-    __syncthreads();
-    const u32 tile = s_tile;
-    const u32 base = tile * TILE;
-    const u32 tile_n = min((u32)TILE, n - base);
     const u32 wbase = warp * (32 * IPT);
+    const u32 lane_lt = (1u << lane) - 1u;
 
     // ---- load, warp-striped: item k of lane l is tile position wbase + 32k + l (coalesced) ----
     u64 key[IPT];
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
-        u32 pos = wbase + 32 * k + lane;
-        key[k] = pos < tile_n ? in[base + pos] : ~0ull;
+        const u32 pos = wbase + 32 * k + lane;
+        key[k] = (FULLT || pos < tile_n) ? in[base + pos] : ~0ull;
     }
 
-    // ---- rank inside the warp's chunk (stable: position order = (k, lane)) ----
+    // ---- early counts: per-warp digit histograms by shared-memory atomics ----
     u32* myhist = whist + warp * 256;
-    const u32 lane_lt = (1u << lane) - 1u;
-    unsigned short rank[IPT];
 #pragma unroll
-    for (int k = 0; k < IPT; ++k) {
-        const bool valid = (wbase + 32 * k + lane) < tile_n;
-        const u32 dg = valid ? ((u32)(key[k] >> shift) & 255u) : 256u;
-        const u32 peers = __match_any_sync(SD_FULL, dg);
-        const u32 below = __popc(peers & lane_lt);
-        u32 pre = 0;
-        if (below == 0 && valid) {
-            pre = myhist[dg];
-            myhist[dg] = pre + __popc(peers);
-        }
-        pre = __shfl_sync(SD_FULL, pre, __ffs(peers) - 1);
-        rank[k] = (unsigned short)(pre + below);
-        __syncwarp();
-    }
+    for (int k = 0; k < IPT; ++k)
+        if (FULLT || (wbase + 32 * k + lane) < tile_n) atomicAdd(&myhist[(u32)(key[k] >> shift) & 255u], 1u);
     __syncthreads();
 
-    // ---- per-digit: exclusive offsets across warps, tile total, look-back ----
+    // ---- per digit: exclusive offsets across warps, tile total; publish the aggregate EARLY so that
+    //      successors never wait on this tile's ranking ----
     u32 total = 0;
+    u32* st = status + (u64)tile * 256 + tid;
     if (tid < 256) {
 #pragma unroll
         for (int w = 0; w < NW; ++w) {
-            u32 c = whist[w * 256 + tid];
+            const u32 c = whist[w * 256 + tid];
             whist[w * 256 + tid] = total;
             total += c;
         }
+        sd_st_relaxed32(st, (tile == 0 ? OS_FLAG_PRE : OS_FLAG_AGG) | total);
     }
     u32 tile_sum;
-    u32 tstart = sd_block_excl_sum<THREADS>(total, &tile_sum, s_warp);
+    const u32 tstart = sd_block_excl_sum<THREADS>(total, &tile_sum, s_warp);
     if (tid < 256) {
-        s_tstart[tid] = tstart;
+#pragma unroll
+        for (int w = 0; w < NW; ++w) whist[w * 256 + tid] += tstart;  // now: next free slot of (warp, digit)
+    }
+    __syncthreads();
+
+    // ---- rank inside the warp's chunk (stable: position order = (k, lane)) and stage in digit order ----
+#pragma unroll
+    for (int k = 0; k < IPT; ++k) {
+        const bool valid = FULLT || (wbase + 32 * k + lane) < tile_n;
+        const u32 dg = (u32)(key[k] >> shift) & 255u;
+        const u32 peers = os_match8(dg, FULLT ? SD_FULL : __ballot_sync(SD_FULL, valid));
+        const u32 pre = myhist[dg];
+        __syncwarp();
+        const u32 below = __popc(peers & lane_lt);
+        if (valid && below == 0) myhist[dg] = pre + __popc(peers);
+        __syncwarp();
+        if (valid) skeys[pre + below] = key[k];
+    }
+
+    // ---- decoupled look-back per digit (predecessors published their aggregates before ranking) ----
+    if (tid < 256) {
         u32 excl = 0;
-        u32* st = status + (u64)tile * 256 + tid;
-        if (tile == 0) {
-            sd_st_relaxed32(st, OS_FLAG_PRE | total);
-        } else {
-            sd_st_relaxed32(st, OS_FLAG_AGG | total);
+        if (tile != 0) {
             const u32* p = st - 256;
             while (true) {
                 u32 s;
@@ -132,37 +137,67 @@ __global__ void __launch_bounds__(THREADS) k_onesweep(const u64* __restrict__ in
     }
     __syncthreads();
 
-    // ---- scatter into shared memory in digit order ----
-#pragma unroll
-    for (int k = 0; k < IPT; ++k) {
-        if ((wbase + 32 * k + lane) < tile_n) {
-            const u32 dg = (u32)(key[k] >> shift) & 255u;
-            skeys[s_tstart[dg] + myhist[dg] + rank[k]] = key[k];
-        }
-    }
-    __syncthreads();
-
     // ---- write out: consecutive threads -> consecutive slots of one digit's global segment ----
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
-        u32 pos = tid + k * THREADS;
-        if (pos < tile_n) {
-            u64 kk = skeys[pos];
-            u32 dg = (u32)(kk >> shift) & 255u;
-            out[s_gofs[dg] + pos] = kk;
+        const u32 pos = tid + k * THREADS;
+        if (FULLT || pos < tile_n) {
+            const u64 kk = skeys[pos];
+            out[s_gofs[(u32)(kk >> shift) & 255u] + pos] = kk;
         }
     }
 }
 
-constexpr int OS_THREADS = 256;
-constexpr int OS_IPT = 16;
-constexpr int OS_TILE = OS_THREADS * OS_IPT;
-constexpr size_t OS_SMEM = (size_t)OS_TILE * 8 + (OS_THREADS / 32) * 256 * 4 + 2 * 256 * 4;
+template <int THREADS, int IPT, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB) k_onesweep(const u64* __restrict__ in, u64* __restrict__ out, u32 n, int shift,
+                                                           const u32* __restrict__ gbase, u32* __restrict__ status,
+                                                           u32* __restrict__ ticket) {
+    constexpr int TILE = THREADS * IPT, NW = THREADS / 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    u64* skeys = reinterpret_cast<u64*>(smem_raw);      // TILE keys, digit order
+    u32* whist = reinterpret_cast<u32*>(skeys + TILE);  // NW x 256 per-warp digit counters / slot pointers
+    u32* s_gofs = whist + NW * 256;                     // 256: global offset of digit d minus its tile start
+    __shared__ u32 s_tile;
+    __shared__ u32 s_warp[NW + 1];
+
+    const u32 tid = threadIdx.x;
+    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+    for (int i = tid; i < NW * 256; i += THREADS) whist[i] = 0;
+    __syncthreads();
+    const u32 tile = s_tile;
+    const u32 base = tile * TILE;
+    const u32 tile_n = min((u32)TILE, n - base);
+    if (tile_n == (u32)TILE)
+        os_tile<THREADS, IPT, true>(in, out, base, tile_n, tile, shift, gbase, status, skeys, whist, s_gofs, s_warp);
+    else
+        os_tile<THREADS, IPT, false>(in, out, base, tile_n, tile, shift, gbase, status, skeys, whist, s_gofs, s_warp);
+}
+
+struct OsVariant {
+    int threads, ipt;
+    size_t smem;
+    void (*kernel)(const u64*, u64*, u32, int, const u32*, u32*, u32*);
+};
+template <int THREADS, int IPT, int MINB>
+constexpr OsVariant os_variant() {
+    return {THREADS, IPT, (size_t)THREADS * IPT * 8 + (THREADS / 32) * 256 * 4 + 256 * 4, k_onesweep<THREADS, IPT, MINB>};
+}
+const OsVariant OS_VARIANTS[] = {os_variant<256, 16, 4>(), os_variant<512, 16, 2>(), os_variant<384, 18, 2>(),
+                                 os_variant<256, 20, 3>(), os_variant<512, 12, 2>(), os_variant<256, 12, 4>()};
+constexpr int OS_NVARIANTS = sizeof(OS_VARIANTS) / sizeof(OS_VARIANTS[0]);
+constexpr int OS_MIN_TILE = 256 * 12;  // scratch is sized for the smallest tile of any variant
+int g_os_variant = 0;
 
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------
-i64 sd_sort_tiles(i64 n) { return (n + OS_TILE - 1) / OS_TILE; }
+i64 sd_sort_tiles(i64 n) { return (n + OS_MIN_TILE - 1) / OS_MIN_TILE; }
+
+int sd_sort_set_variant(int v) {
+    if (v < 0 || v >= OS_NVARIANTS) return -1;
+    g_os_variant = v;
+    return 0;
+}
 
 // scratch layout: [npass][256] u32 histograms | [npass] tickets (padded to 256 B) | [npass][tiles][256] u32 status
 i64 sd_sort_scratch_bytes(i64 n, int npass) {
@@ -185,29 +220,40 @@ cudaError_t sd_sort_histogram(const u64* keys, i64 n, int begin_bit, int npass, 
     return cudaGetLastError();
 }
 
-// Runs the passes.  The histograms in `scratch` must be complete (raw counts).  Returns in *result
-// the buffer (keys or tmp) that holds the sorted records.
+// Turns the raw per-digit counts into exclusive bin bases (one tiny launch).
+cudaError_t sd_sort_hist_scan(void* scratch, int npass, cudaStream_t st, i64* launches) {
+    if (npass == 0) return cudaSuccess;
+    k_hist_scan<<<npass, 256, 0, st>>>(sd_sort_hist_ptr(scratch));
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+// Runs the passes.  The histograms in `scratch` must hold exclusive bin bases (sd_sort_hist_scan).
+// Returns in *result the buffer (keys or tmp) that holds the sorted records.
 cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, void* scratch, cudaStream_t st,
                            u64** result, i64* launches) {
     *result = keys;
     if (n == 0 || npass == 0) return cudaSuccess;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(k_onesweep<OS_THREADS, OS_IPT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)OS_SMEM);
-        if (e != cudaSuccess) return e;
+        for (int v = 0; v < OS_NVARIANTS; ++v) {
+            cudaError_t e = cudaFuncSetAttribute(OS_VARIANTS[v].kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                 (int)OS_VARIANTS[v].smem);
+            if (e != cudaSuccess) return e;
+        }
         attr_set = true;
     }
+    const OsVariant& V = OS_VARIANTS[g_os_variant];
     u32* hist = sd_sort_hist_ptr(scratch);
     u32* tickets = hist + npass * 256;
     u32* status = tickets + 64;
-    const i64 tiles = sd_sort_tiles(n);
-    k_hist_scan<<<npass, 256, 0, st>>>(hist);
-    if (launches) ++*launches;
+    const i64 tile = (i64)V.threads * V.ipt;
+    const i64 tiles = (n + tile - 1) / tile;
+    const i64 status_stride = sd_sort_tiles(n) * 256;
     u64 *src = keys, *dst = tmp;
     for (int p = 0; p < npass; ++p) {
-        k_onesweep<OS_THREADS, OS_IPT><<<(unsigned)tiles, OS_THREADS, OS_SMEM, st>>>(
-            src, dst, (u32)n, begin_bit + 8 * p, hist + p * 256, status + (size_t)p * tiles * 256, tickets + p);
+        V.kernel<<<(unsigned)tiles, V.threads, V.smem, st>>>(src, dst, (u32)n, begin_bit + 8 * p, hist + p * 256,
+                                                             status + (size_t)p * status_stride, tickets + p);
         if (launches) ++*launches;
         std::swap(src, dst);
     }

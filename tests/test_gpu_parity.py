@@ -1,0 +1,400 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle.  All tests need a B200.
+
+Bar: bit-exact — identical pair sets, identical distances, identical order (integer work).
+Element-by-element at sizes the oracle finishes in seconds (several tiles + ragged tails); at the
+BASELINE.json full sizes by the stored oracle digests (tests/golden/config_*.json, written by
+tests/golden/make_golden.py from the oracle alone) plus sampled rows recomputed by brute force.
+"""
+import hashlib
+import json
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+from paper_2403_09010_b200 import synth
+
+pytestmark = pytest.mark.gpu
+GOLD = Path(__file__).parent / "golden"
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+
+    assert t.cuda.is_available(), "gpu tests need a CUDA device"
+    return t
+
+
+@pytest.fixture(scope="module")
+def sd(torch):
+    from paper_2403_09010_b200 import symdel
+
+    symdel.lib()  # must load: there is no fallback
+    return symdel
+
+
+@pytest.fixture()
+def ctx(sd):
+    c = sd.Context(0)
+    yield c
+    c.close()
+
+
+def run_self(sd, ctx, s, d, **kw):
+    ds, do = sd.to_device(s)
+    return [t.cpu().numpy() for t in ctx.symdel_self(ds, do, d, **kw)]
+
+
+def run_cross(sd, ctx, q, r, d, **kw):
+    qs, qo = sd.to_device(q)
+    rs, ro = sd.to_device(r)
+    return [t.cpu().numpy() for t in ctx.symdel_cross(qs, qo, rs, ro, d, **kw)]
+
+
+def assert_same(got, exp):
+    assert len(got[0]) == len(exp[0]), (len(got[0]), len(exp[0]))
+    for a, b in zip(got, exp[:3]):
+        assert a.dtype == np.int32 and np.array_equal(a, b)
+
+
+def digest(i, j, d):
+    h = hashlib.sha256()
+    for a in (i, j, d):
+        h.update(np.ascontiguousarray(a, dtype=np.int32).tobytes())
+    return h.hexdigest()
+
+
+# ---- S2/K2: radix sort -----------------------------------------------------------------------------
+def _keys(kind, n, seed):
+    rng = np.random.default_rng(seed)
+    if kind == "rand":
+        return rng.integers(0, 2**64, n, dtype=np.uint64)
+    if kind == "equal":
+        return np.full(n, 0xDEADBEEF12345678, dtype=np.uint64)
+    if kind == "few":
+        return rng.integers(0, 3, n, dtype=np.uint64) << np.uint64(20)
+    if kind == "sorted":
+        return np.sort(rng.integers(0, 2**64, n, dtype=np.uint64))
+    if kind == "reverse":
+        return np.sort(rng.integers(0, 2**64, n, dtype=np.uint64))[::-1].copy()
+    if kind == "onebin":  # every key in one bin except a sprinkle: match-any ranking degenerates
+        k = np.zeros(n, dtype=np.uint64)
+        k[rng.integers(0, max(n, 1), max(n // 100, 1))] = np.uint64(255)
+        return k | (rng.integers(0, 2**32, n, dtype=np.uint64) << np.uint64(32))
+    raise ValueError(kind)
+
+
+@pytest.mark.parametrize("n", [0, 1, 31, 4095, 4096, 4097, 12289, 1_000_003])
+def test_sort_sizes(torch, sd, ctx, n):
+    k = _keys("rand", n, n)
+    t = torch.from_numpy(k.view(np.int64).copy()).cuda()
+    ctx.symdel_stage_sort_u64(t, 0, 64)
+    assert np.array_equal(t.cpu().numpy().view(np.uint64), np.sort(k, kind="stable"))
+
+
+@pytest.mark.parametrize("kind", ["equal", "few", "sorted", "reverse", "onebin"])
+@pytest.mark.parametrize("bits", [(0, 8), (0, 32), (20, 52), (24, 64)])
+def test_sort_stability_and_bit_ranges(torch, sd, ctx, kind, bits):
+    b, e = bits
+    k = _keys(kind, 70_001, 5)
+    t = torch.from_numpy(k.view(np.int64).copy()).cuda()
+    ctx.symdel_stage_sort_u64(t, b, e)
+    field = (k >> np.uint64(b)) & np.uint64((1 << (e - b)) - 1)
+    exp = k[np.argsort(field, kind="stable")]  # stable: ties keep input order
+    assert np.array_equal(t.cpu().numpy().view(np.uint64), exp)
+
+
+def test_sort_many_tiny_tiles_stress(torch, sd, ctx):
+    """Look-back stress: many tiles, repeated (the ticket/status protocol must never deadlock or mis-sum)."""
+    for rep in range(5):
+        k = _keys("rand", 3_000_000 + rep, rep) & np.uint64(0xFFFF)
+        t = torch.from_numpy(k.view(np.int64).copy()).cuda()
+        ctx.symdel_stage_sort_u64(t, 0, 16)
+        assert np.array_equal(t.cpu().numpy().view(np.uint64), np.sort(k, kind="stable"))
+
+
+# ---- S4/K6: bit-parallel distance --------------------------------------------------------------------
+def test_lev_exhaustive_small(torch, sd, ctx, oracle):
+    import itertools
+
+    strs = [()]
+    for L in range(1, 6):
+        strs += list(itertools.product((1, 2, 3), repeat=L))
+    rows = np.zeros((len(strs), 5), np.int8)
+    lens = np.array([len(s) for s in strs])
+    for i, s in enumerate(strs):
+        rows[i, :len(s)] = s
+    ss = synth.from_padded(rows, lens)
+    ia, ib = np.meshgrid(np.arange(ss.n, dtype=np.int32), np.arange(ss.n, dtype=np.int32))
+    ia, ib = ia.ravel(), ib.ravel()
+    ds, do = sd.to_device(ss)
+    got = ctx.symdel_stage_lev(ds, do, ds, do, torch.from_numpy(ia).cuda(), torch.from_numpy(ib).cuda()).cpu().numpy()
+    # oracle distances through its brute-force routine with an unreachable threshold
+    _, j, dist = oracle.bruteforce_cross(ss.seqs, ss.offsets, ss.seqs, ss.offsets, 99)
+    exp = dist.reshape(ss.n, ss.n)  # row q, column r
+    assert np.array_equal(got.reshape(ss.n, ss.n).T, exp)
+    assert len(ia) == 364 * 364
+
+
+def test_lev_random_up_to_L_MAX(torch, sd, ctx, oracle):
+    rng = np.random.default_rng(1)
+    n = 3000
+    lens = rng.integers(0, 65, n)
+    lens[:4] = (0, 64, 32, 33)
+    rows = rng.integers(1, 5, (n, 64)).astype(np.int8)
+    rows[n // 2:] = rows[: n - n // 2]  # near-duplicates: small distances as well as large
+    flip = rng.random((n, 64)) < 0.05
+    rows[flip] = rng.integers(1, 32, flip.sum())
+    rows[np.arange(64)[None, :] >= lens[:, None]] = 0
+    ss = synth.from_padded(rows, lens)
+    ia = rng.integers(0, n, 30000).astype(np.int32)
+    ib = np.where(rng.random(30000) < 0.5, (ia + n // 2) % n, rng.integers(0, n, 30000)).astype(np.int32)
+    ds, do = sd.to_device(ss)
+    got = ctx.symdel_stage_lev(ds, do, ds, do, torch.from_numpy(ia).cuda(), torch.from_numpy(ib).cuda()).cpu().numpy()
+    exp = np.array([oracle.lev(ss.seq(a), ss.seq(b)) for a, b in zip(ia, ib)])
+    assert np.array_equal(got, exp)
+
+
+# ---- S1/K1: variant generation -----------------------------------------------------------------------
+@pytest.mark.parametrize("d", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("thinning", [True, False])
+def test_generate_groups_match_oracle_variants(torch, sd, ctx, oracle, d, thinning):
+    """The multiset of id-groups sharing a key equals the oracle's groups sharing a variant string
+    (hash consistent and collision-free at 48 bits on this input); record count = number of distinct
+    (variant, id) with thinning (P-11), = sum C(L, k) without."""
+    s = synth.repeat_heavy_set(70, 3, alphabet=3, lo=0, hi=9 if d < 4 else 8)
+    ds, do = sd.to_device(s)
+    id_bits, hash_bits = 8, 48
+    rec = ctx.symdel_stage_generate(ds, do, d, hash_bits, id_bits, thinning, 1 << 20).cpu().numpy().view(np.uint64)
+    ids = (rec & np.uint64(255)).astype(np.int64)
+    keys = rec >> np.uint64(id_bits)
+    assert (np.diff(ids) >= 0).all()  # written in id order
+    var = [oracle.deletion_variants(s.seq(i), d) for i in range(s.n)]
+    if thinning:
+        exp_cnt = np.array([len(set(v)) for v in var])
+    else:
+        exp_cnt = np.array([len(v) for v in var])
+    assert np.array_equal(np.bincount(ids, minlength=s.n), exp_cnt)
+    got_groups = {}
+    for k, i in zip(keys.tolist(), ids.tolist()):
+        got_groups.setdefault(k, []).append(i)
+    exp_groups = {}
+    for i, v in enumerate(var):
+        for x in (set(v) if thinning else v):
+            exp_groups.setdefault(x, []).append(i)
+    assert sorted(map(tuple, got_groups.values())) == sorted(map(tuple, (sorted(g) for g in exp_groups.values())))
+
+
+# ---- full path: small / structured inputs -------------------------------------------------------------
+def test_hand_worked_cases(sd, ctx, oracle):
+    s = synth.from_strings(["ACDEF", "ACDF", "ACGEF", "AB", "BA", "", "A", "ACCD", "ACD", "AAAA", "AAA", "CDEFA", "B"])
+    for d in range(0, 5):
+        assert_same(run_self(sd, ctx, s, d), oracle.bruteforce_self(s.seqs, s.offsets, d))
+
+
+def test_degenerate_inputs(torch, sd, ctx, oracle):
+    one = synth.from_strings(["ACD"])
+    assert len(run_self(sd, ctx, one, 2)[0]) == 0
+    empties = synth.from_strings(["", "", ""])
+    assert_same(run_self(sd, ctx, empties, 1), oracle.bruteforce_self(empties.seqs, empties.offsets, 1))
+    same = synth.from_strings(["ACDEFGH"] * 40)  # one long run: 780 pairs at distance 0
+    got = run_self(sd, ctx, same, 2)
+    assert_same(got, oracle.bruteforce_self(same.seqs, same.offsets, 2))
+    assert len(got[0]) == 780 and (got[2] == 0).all()
+    # n = 0 through the raw ABI
+    z8 = torch.zeros(1, dtype=torch.int8, device="cuda")
+    z64 = torch.zeros(1, dtype=torch.int64, device="cuda")
+    assert len(ctx.symdel_self(z8, z64, 2)[0]) == 0
+    # maximum length 64 and d = 4
+    rng = np.random.default_rng(3)
+    rows = np.tile(rng.integers(1, 21, (1, 64)), (12, 1)).astype(np.int8)
+    for t in range(1, 12):
+        rows[t, rng.integers(0, 64, t % 5)] = 20 + t
+    lens = np.full(12, 64)
+    lens[5:] = 63
+    big = synth.from_padded(rows, lens)
+    assert_same(run_self(sd, ctx, big, 4), oracle.bruteforce_self(big.seqs, big.offsets, 4))
+
+
+def test_error_codes(torch, sd, ctx):
+    s = synth.tcr_set(200, 1)
+    ds, do = sd.to_device(s)
+    bad = ds.clone()
+    bad[5] = 0
+    with pytest.raises(sd.SymdelError) as e:
+        ctx.symdel_self(bad, do, 1)
+    assert e.value.code == sd.E_RESIDUE
+    bad_off = do.clone()
+    bad_off[3] = bad_off[4] + 1
+    with pytest.raises(sd.SymdelError) as e:
+        ctx.symdel_self(ds, bad_off, 1)
+    assert e.value.code == sd.E_OFFSETS
+    long = synth.from_padded(np.ones((2, 70), np.int8), np.array([70, 70]))
+    ls, lo = sd.to_device(long)
+    with pytest.raises(sd.SymdelError) as e:
+        ctx.symdel_self(ls, lo, 1)
+    assert e.value.code == sd.E_TOO_LONG
+    with pytest.raises(sd.SymdelError) as e:
+        ctx.symdel_self(ds, do, 5)
+    assert e.value.code == sd.E_ARG
+    with pytest.raises(sd.SymdelError) as e:
+        ctx.symdel_self(ds, do, 2, capacity=3)
+    assert e.value.code == sd.E_CAPACITY and ctx.last_required > 3
+    with pytest.raises(sd.SymdelError) as e:
+        ctx.symdel_self(ds, do, 2, workspace=torch.empty(4096, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == sd.E_WORKSPACE
+
+
+@pytest.mark.parametrize("d", [0, 1, 2, 3, 4])
+def test_repeat_heavy(sd, ctx, oracle, d):
+    s = synth.repeat_heavy_set(400, 5, alphabet=2, lo=0, hi=9)
+    assert_same(run_self(sd, ctx, s, d), oracle.bruteforce_self(s.seqs, s.offsets, d))
+
+
+@pytest.mark.parametrize("family", ["tcr", "bcr"])
+@pytest.mark.parametrize("d", [1, 2, 3])
+def test_validation_protocol_5000(sd, ctx, oracle, family, d):
+    """5,000 sequences at d = 1, 2, 3 against the brute-force double loop."""
+    s = synth.tcr_set(5000, 100) if family == "tcr" else synth.bcr_set(5000, 101, n_lineages=500)
+    assert_same(run_self(sd, ctx, s, d), oracle.bruteforce_self(s.seqs, s.offsets, d))
+
+
+@pytest.mark.parametrize("opts", [
+    {"FORCE_CHUNKS": 4}, {"FORCE_CHUNKS": 16}, {"CAND_CAPACITY": 4999}, {"HASH_BITS": 8}, {"HASH_BITS": 48},
+    {"NO_THINNING": 1}, {"FORCE_CHUNKS": 3, "CAND_CAPACITY": 777, "HASH_BITS": 16},
+])
+def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
+    """P-11: chunk count, candidate-buffer windows, key width and thinning change memory use and
+    candidate counts only, never the result."""
+    s = synth.tcr_set(6000, 21)
+    exp = oracle.symdel_self(s.seqs, s.offsets, 2)
+    c = sd.Context(0)
+    for k, v in opts.items():
+        c.symdel_set_option(getattr(sd, "OPT_" + k), v)
+    assert_same(run_self(sd, c, s, 2), exp)
+    st = c.symdel_get_stats()
+    if "FORCE_CHUNKS" in opts:
+        assert st["n_chunks"] == opts["FORCE_CHUNKS"]
+    if "CAND_CAPACITY" in opts:
+        assert st["n_flushes"] > 1
+
+
+def test_small_workspace_forces_chunking(torch, sd, ctx, oracle):
+    s = synth.tcr_set(20000, 22)
+    exp = oracle.symdel_self(s.seqs, s.offsets, 2)
+    ds, do = sd.to_device(s)
+    ws = torch.empty(24 << 20, dtype=torch.uint8, device="cuda")  # ~1/3 of the un-chunked need
+    got = [t.cpu().numpy() for t in ctx.symdel_self(ds, do, 2, workspace=ws)]
+    assert_same(got, exp)
+    assert ctx.symdel_get_stats()["n_chunks"] > 1
+
+
+def test_shuffle_invariance(sd, ctx):
+    """results invariant under random shuffling of the input."""
+    s = synth.tcr_set(8000, 23)
+    i, j, d = run_self(sd, ctx, s, 2)
+    perm = np.random.default_rng(1).permutation(s.n)
+    i2, j2, d2 = run_self(sd, ctx, s.take(perm), 2)
+    a = {(int(x), int(y), int(z)) for x, y, z in zip(i, j, d)}
+    b = {(int(min(perm[x], perm[y])), int(max(perm[x], perm[y])), int(z)) for x, y, z in zip(i2, j2, d2)}
+    assert a == b
+
+
+@pytest.mark.parametrize("d", [1, 2])
+def test_cross_small(sd, ctx, oracle, d):
+    q, r = synth.cross_sets(600, 8000, 103)
+    assert_same(run_cross(sd, ctx, q, r, d), oracle.bruteforce_cross(q.seqs, q.offsets, r.seqs, r.offsets, d))
+
+
+def test_cross_symmetry_and_self_relation(sd, ctx):
+    a, b = synth.tcr_set(3000, 12), synth.tcr_set(4000, 11)
+    ab = run_cross(sd, ctx, a, b, 2)
+    ba = run_cross(sd, ctx, b, a, 2)
+    assert {(x, y, z) for x, y, z in zip(*map(np.ndarray.tolist, ab))} == {(y, x, z) for x, y, z in zip(*map(np.ndarray.tolist, ba))}
+    ss = run_cross(sd, ctx, a, a, 2)
+    self_ = run_self(sd, ctx, a, 2)
+    tri = {(x, y, z) for x, y, z in zip(*map(np.ndarray.tolist, ss)) if x < y}
+    assert tri == {(x, y, z) for x, y, z in zip(*map(np.ndarray.tolist, self_))}
+    assert sum(1 for x, y, z in zip(*map(np.ndarray.tolist, ss)) if x == y and z == 0) == a.n
+
+
+def test_cross_chunked_windowed(sd, oracle):
+    q, r = synth.cross_sets(600, 8000, 103)
+    c = sd.Context(0)
+    c.symdel_set_option(sd.OPT_FORCE_CHUNKS, 3)
+    c.symdel_set_option(sd.OPT_CAND_CAPACITY, 300)
+    assert_same(run_cross(sd, c, q, r, 2), oracle.symdel_cross(q.seqs, q.offsets, r.seqs, r.offsets, 2))
+
+
+def test_host_entry_points(torch, sd, ctx, oracle):
+    s = synth.tcr_set(4000, 31)
+    out = tuple(torch.empty(100000, dtype=torch.int32).pin_memory() for _ in range(3))
+    hs = torch.from_numpy(s.seqs).pin_memory()
+    ho = torch.from_numpy(s.offsets).pin_memory()
+    k = ctx.symdel_self_host(hs, ho, 2, out)
+    assert_same([o[:k].numpy() for o in out], oracle.symdel_self(s.seqs, s.offsets, 2))
+    q, r = synth.cross_sets(300, 5000, 9)
+    out2 = tuple(np.empty(100000, np.int32) for _ in range(3))
+    k = ctx.symdel_cross_host(q.seqs, q.offsets, r.seqs, r.offsets, 2, out2)
+    assert_same([o[:k] for o in out2], oracle.symdel_cross(q.seqs, q.offsets, r.seqs, r.offsets, 2))
+
+
+# ---- BASELINE.json configs at full size ---------------------------------------------------------------
+def _golden(name):
+    p = GOLD / name
+    if not p.exists():
+        pytest.skip(f"{name} not generated")
+    return json.loads(p.read_text())
+
+
+def _check_sampled_rows(oracle, s, d, i, j, dist, n_rows, seed):
+    """Completeness on sampled rows: all neighbours of sequence t by brute force over the whole set."""
+    rng = np.random.default_rng(seed)
+    hit = np.unique(np.concatenate([i[:: max(1, len(i) // (n_rows // 2))][: n_rows // 2], rng.integers(0, s.n, n_rows // 2)]))
+    for t in hit:
+        r, dd = oracle.bruteforce_row(s.seq(int(t)), s.seqs, s.offsets, d)
+        keep = r != t
+        exp = {(int(min(t, x)), int(max(t, x)), int(y)) for x, y in zip(r[keep], dd[keep])}
+        m = (i == t) | (j == t)
+        got = {(int(a), int(b), int(c)) for a, b, c in zip(i[m], j[m], dist[m])}
+        assert got == exp, int(t)
+
+
+@pytest.mark.parametrize("num", [1, 2, 3, 5])
+def test_config_full_size(sd, ctx, oracle, num):
+    g = _golden(f"config_{num}.json")
+    kind, d, (s,) = synth.config(num)
+    assert s.sha256() == g["input_sha256"] and s.n == g["n"]
+    i, j, dist = run_self(sd, ctx, s, d)
+    assert len(i) == g["n_out"]
+    assert np.bincount(dist, minlength=d + 1).tolist() == g["dist_hist"]
+    assert digest(i, j, dist) == g["out_sha256"]  # identical pairs, distances and order as the oracle
+    assert (i < j).all() and (np.diff(i.astype(np.int64) * (1 << 31) + j) > 0).all()
+    _check_sampled_rows(oracle, s, d, i, j, dist, 24 if num >= 3 else 60, num)
+    # every reported distance re-derived by the oracle's full-table recurrence (sample at full size)
+    step = max(1, len(i) // 20000)
+    for a, b, c in zip(i[::step], j[::step], dist[::step]):
+        assert oracle.lev(s.seq(int(a)), s.seq(int(b))) == c
+
+
+def test_config4_scaled(sd, ctx, oracle):
+    g = _golden("config_4_scale0.1.json")
+    kind, d, (q, r) = synth.config(4, 0.1)
+    assert q.sha256() + r.sha256() == g["input_sha256"]
+    i, j, dist = run_cross(sd, ctx, q, r, d)
+    assert len(i) == g["n_out"] and digest(i, j, dist) == g["out_sha256"]
+
+
+def test_config4_full_size(sd, ctx, oracle):
+    g = _golden("config_4.json")
+    kind, d, (q, r) = synth.config(4)
+    assert q.sha256() + r.sha256() == g["input_sha256"]
+    i, j, dist = run_cross(sd, ctx, q, r, d)
+    assert len(i) == g["n_out"] and np.bincount(dist, minlength=d + 1).tolist() == g["dist_hist"]
+    assert digest(i, j, dist) == g["out_sha256"]
+    rng = np.random.default_rng(4)
+    for t in np.unique(np.concatenate([i[:: max(1, len(i) // 10)][:10], rng.integers(0, q.n, 6)])):
+        rr, dd = oracle.bruteforce_row(q.seq(int(t)), r.seqs, r.offsets, d)
+        m = i == t
+        assert np.array_equal(j[m], rr) and np.array_equal(dist[m], dd)
