@@ -84,6 +84,7 @@ enum {
     SYMDEL_OPT_CAND_CAPACITY = 3, /* [0] >0: cap the candidate buffer at this many pairs (test hook for multi-flush) */
     SYMDEL_OPT_HASH_BITS = 4,     /* [0] 0 = automatic; else 8..56 (multiple of 8): key bits sorted per record */
     SYMDEL_OPT_NO_THINNING = 5,   /* [0] 1: emit one record per deletion SET instead of per distinct variant (test hook) */
+    SYMDEL_OPT_GENERAL_GENERATE = 7, /* [0] 1: use the general (any d, any length) generation kernel even where the d <= 2 fast path applies (test hook) */
     SYMDEL_OPT_SORT_VARIANT = 6   /* [0] tile shape of the onesweep kernel (process-wide tuning hook; results are identical) */
 };
 

@@ -74,6 +74,37 @@ __device__ __forceinline__ u64 sd_lookback(u64* status, u32 tile, u64 aggregate)
     return excl;
 }
 
+// Warp-parallel variant: called by all 32 lanes of ONE converged warp; inspects 32 predecessors per
+// round trip (lane 0 = nearest), so the walk back to the closest inclusive prefix costs
+// ceil(depth / 32) L2 latencies instead of depth.  Returns the exclusive prefix to every lane.
+__device__ __forceinline__ u64 sd_lookback_warp(u64* status, u32 tile, u64 aggregate) {
+    const u32 lane = threadIdx.x & 31;
+    if (tile == 0) {
+        if (lane == 0) sd_st_relaxed(status, SD_LB_PRE | aggregate);
+        return 0;
+    }
+    if (lane == 0) sd_st_relaxed(status + tile, SD_LB_AGG | aggregate);
+    u64 excl = 0;
+    i64 hi = (i64)tile;
+    while (true) {
+        const i64 idx = hi - 1 - (i64)lane;
+        u64 s = SD_LB_PRE;  // virtual tile before tile 0: inclusive prefix 0
+        if (idx >= 0) {
+            do { s = sd_ld_relaxed(status + idx); } while ((s >> 62) == 0);
+        }
+        const u32 pre = __ballot_sync(SD_FULL, (s >> 62) == 2);
+        u64 v = s & SD_LB_MASK;
+        if (pre && lane > (u32)(__ffs(pre) - 1)) v = 0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(SD_FULL, v, o);
+        excl += v;
+        if (pre) break;
+        hi -= 32;
+    }
+    if (lane == 0) sd_st_relaxed(status + tile, SD_LB_PRE | (excl + aggregate));
+    return excl;
+}
+
 // ---- block-wide exclusive scans (THREADS a multiple of 32, <= 1024) ------------------------------
 template <int THREADS>
 __device__ __forceinline__ u32 sd_block_excl_sum(u32 v, u32* total, u32* s_warp /* [THREADS/32 + 1] */) {

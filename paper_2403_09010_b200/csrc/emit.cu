@@ -12,8 +12,8 @@
 //   cross: records are sorted by (hash, id) and query ids are below reference ids, so a run is
 //          [q .. q r .. r]; a reference record pairs with [run_start, first reference of the run),
 //          a query record with nothing.
-// The per-record counts are scanned inside the tile, the tile totals across tiles by decoupled
-// look-back; pairs are then written by FLAT pair index (binary search into the scanned counts), so a
+// The per-record counts are scanned inside the tile; a tile claims its output range with one atomic
+// add (candidate order is irrelevant: they are sorted next); pairs are then written by FLAT pair index (binary search into the scanned counts), so a
 // long run is spread over the whole block instead of serialising one thread.  Only pairs whose flat
 // index lies in [win_lo, win_hi) are written: when the candidate buffer is smaller than the total,
 // the host replays the kernel once per window (later rounds reuse the saved tile prefixes).
@@ -53,24 +53,15 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(const u64* __restrict__ rec
     __shared__ i64 s_a[EM_TILE];         // partner range start (global position)
     __shared__ u64 s_warp64[EM_THREADS / 32 + 1];
     __shared__ i32 s_warp32[EM_THREADS / 32];
-    __shared__ u32 s_tile;
     __shared__ i64 s_tile_rs;
     __shared__ u64 s_excl;
 
     const u32 tid = threadIdx.x;
-    const u32 ntiles = gridDim.x;
-    if (first_round) {
-        if (tid == 0) {
-            s_tile = atomicAdd(&info->ticket[SD_TK_EMIT], 1u);
-            if (s_tile == ntiles - 1) info->ticket[SD_TK_EMIT] = 0;
-        }
-        __syncthreads();
-    }
-    const u32 tile = first_round ? s_tile : blockIdx.x;
+    const u32 tile = blockIdx.x;
     if (!first_round) {
         // skip tiles whose pairs lie entirely outside the window
-        const u64 lo = tile_prefix[tile], hi = tile_prefix[tile + 1];
-        if (hi <= win_lo || lo >= win_hi || hi == lo) return;
+        const u64 lo = tile_prefix[2 * tile], cnt = tile_prefix[2 * tile + 1];
+        if (cnt == 0 || lo + cnt <= win_lo || lo >= win_hi) return;
     }
     const u64 base = (u64)tile * EM_TILE;
     const u32 tile_n = (u32)min((u64)EM_TILE, n - base);
@@ -152,16 +143,16 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(const u64* __restrict__ rec
     }
     if (tid == 0) {
         s_scan[tile_n] = T;
+        // Output slots: the ORDER of candidates is irrelevant (they are sorted next), so a tile claims
+        // its range with one atomic add instead of an ordered scan across tiles; the claimed base is
+        // saved so that later windows of the same call see the same numbering.
         u64 excl;
         if (first_round) {
-            excl = sd_lookback(lb_status, tile, T);
-            tile_prefix[tile] = excl;
-            if (tile == ntiles - 1) {
-                tile_prefix[ntiles] = excl + T;
-                info->n_cand = excl + T;
-            }
+            excl = T ? (u64)atomicAdd((unsigned long long*)&info->n_cand, (unsigned long long)T) : 0ull;
+            tile_prefix[2 * tile] = excl;
+            tile_prefix[2 * tile + 1] = T;
         } else {
-            excl = tile_prefix[tile];
+            excl = tile_prefix[2 * tile];
         }
         s_excl = excl;
     }
@@ -196,7 +187,7 @@ cudaError_t sd_emit(const u64* records, i64 n_records, const Layout& lay, u64* c
     const i64 tiles = sd_emit_tiles(n_records);
     if (tiles == 0) return cudaSuccess;
     if (first_round) {
-        cudaError_t e = cudaMemsetAsync(lb_status, 0, (size_t)tiles * 8, st);
+        cudaError_t e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st);
         if (e != cudaSuccess) return e;
     }
     k_emit<<<(unsigned)tiles, EM_THREADS, 0, st>>>(records, (u64)n_records, lay, cand, win_lo, win_hi, first_round,

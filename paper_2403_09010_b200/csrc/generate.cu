@@ -32,6 +32,10 @@ __constant__ u32 c_vcum[(SD_L_MAX + 1) * (SD_D_MAX + 2)];   // sum_{j<k} C(n, j)
 
 constexpr u64 K_LEN = 0x9fb21c651e98df25ull;
 
+// Key-range chunk of a variant hash (S5): a function of the LOW word only, so the sorted key (the top
+// hash_bits) stays uniformly distributed inside every chunk.
+__device__ __forceinline__ u32 gen_chunk_of(u64 h, u32 n_chunks) { return __umulhi((u32)h * 0x9e3779b1u, n_chunks); }
+
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, DevInfo* info) {
     u64 nmax = 0;
@@ -92,7 +96,10 @@ __global__ void __launch_bounds__(SC_THREADS) k_scan_counts(const u32* __restric
     }
     u32 total;
     u32 excl = sd_block_excl_sum<SC_THREADS>(sum, &total, s_warp);
-    if (tid == 0) s_excl = sd_lookback(lb_status, tile, total);
+    if (tid < 32) {
+        const u64 e = sd_lookback_warp(lb_status, tile, total);
+        if (tid == 0) s_excl = e;
+    }
     __syncthreads();
     u64 run = s_excl + excl;
 #pragma unroll
@@ -188,7 +195,7 @@ __device__ __forceinline__ bool gen_set(const GenShared& sh, u32 g, u32 L, u32 i
         if (m < K) prev = p[m] + 1;
     }
     h += (u64)(L - K + 1) * K_LEN;
-    *hash_out = sd_mix64(h);
+    *hash_out = h;
     return true;
 }
 
@@ -287,7 +294,7 @@ __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
                         case 3: valid = gen_set<3>(sh, g, L, idx, thinning, &h); break;
                         default: valid = gen_set<4>(sh, g, L, idx, thinning, &h); break;
                     }
-                    if (valid && P.n_chunks > 1) valid = __umulhi((u32)h, P.n_chunks) == P.chunk;
+                    if (valid && P.n_chunks > 1) valid = gen_chunk_of(h, P.n_chunks) == P.chunk;
                     rec[r] = ((h >> (64 - P.hash_bits)) << P.id_bits) | (gid0 + g);
                 }
                 ball[r] = __ballot_sync(SD_FULL, valid);
@@ -345,6 +352,189 @@ __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Fast path (d <= 2, longest sequence <= 32): one warp per batch of consecutive sequences packed into
+// its 32 lanes, lane = residue position.  The pairs {p1 < p2} of a length-L sequence are enumerated as
+// {a, (a + delta) mod L} for delta = 1 .. (L-1)/2 (plus half a round at delta = L/2 when L is even):
+// every lane of a sequence does the same number of rounds, no unranking, no search.  Per sequence the
+// warp keeps U[p] = A[p] - Binv*A[p+1] and V[p] = Binv*U[p] in shared memory, so that
+//     H({})      = A[L]                              + (L+1)*K
+//     H({p})     = U[p]         + Binv*A[L]          + L*K
+//     H({p1,p2}) = U[p1] + V[p2] + Binv^2*A[L]       + (L-1)*K
+// (the same function as the general path) costs two shared loads and two adds per variant.
+// The leftmost-embedding rule needs two ballots per batch: canon1 (s[p] != s[p+1] or p last) and
+// adjok (the adjacent pair {p, p+1} is canonical); a non-adjacent pair is canonical iff both ends are.
+// Without chunking the record count has the closed form
+//     1 + B + B(B-1)/2 - #{p: canon1[p] & canon1[p+1]} + #adjok,   B = popcount(canon1)
+// so the count pass never enters the delta loop.
+constexpr int G2_THREADS = 256, G2_NW = G2_THREADS / 32;
+
+struct Gen2Shared {
+    u64 U[G2_NW][32];
+    u64 V[G2_NW][32];
+    u64 R[32];
+    u64 Bpow[33];
+    unsigned char map[G2_NW][32];
+};
+
+template <bool COUNT_ONLY>
+__global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
+    extern __shared__ __align__(16) unsigned char gen_smem[];
+    Gen2Shared& sh = *reinterpret_cast<Gen2Shared*>(gen_smem);
+    u32* s_hist = reinterpret_cast<u32*>(gen_smem + sizeof(Gen2Shared));
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 lane_lt = (1u << lane) - 1u;
+    if (tid < 32) sh.R[tid] = c_R[tid];
+    if (tid < 33) sh.Bpow[tid] = c_Bpow[tid];
+    if (!COUNT_ONLY)
+        for (int i = tid; i < P.npass * 256; i += G2_THREADS) s_hist[i] = 0;
+    __syncthreads();
+    const int d = P.d;
+    const bool thinning = P.thinning != 0;
+    const bool chunked = P.n_chunks > 1;
+    const u64 binv1 = c_Binv[1], binv2 = c_Binv[2];
+    const int kshift = 64 - P.hash_bits;
+
+    // warp task = 32 consecutive sequences of one set; groups_* count warp tasks here
+    for (i64 wt = (i64)blockIdx.x * G2_NW + warp; wt < P.groups_total; wt += (i64)gridDim.x * G2_NW) {
+        const bool in_b = wt >= P.groups_a;
+        const SeqSetDev& S = in_b ? P.b : P.a;
+        const i64 first = (in_b ? wt - P.groups_a : wt) * 32;
+        const u32 ns = (u32)min((i64)32, S.n - first);
+        const u64 gid0 = (u64)first + (in_b ? (u64)P.n_a : 0ull);
+        i64 o0 = 0;
+        u32 Li = 0;
+        if (lane < ns) {
+            o0 = S.off[first + lane];
+            Li = (u32)(S.off[first + lane + 1] - o0);
+        }
+        u32 cum_incl = Li;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const u32 t = __shfl_up_sync(SD_FULL, cum_incl, o);
+            if (lane >= (u32)o) cum_incl += t;
+        }
+        const u32 cum_excl = cum_incl - Li;
+        const i64 obase = __shfl_sync(SD_FULL, o0, 0);
+        u64 rec_base_i = 0;
+        if (!COUNT_ONLY && lane < ns) rec_base_i = P.rec_off[gid0 + lane];
+
+        u32 s = 0;
+        while (s < ns) {
+            const u32 base = __shfl_sync(SD_FULL, cum_excl, s);
+            const u32 fit = __ballot_sync(SD_FULL, lane >= s && lane < ns && (cum_incl - base) <= 32u);
+            const u32 e = s + __popc(fit);
+            const u32 total = __shfl_sync(SD_FULL, cum_incl, e - 1) - base;
+            const bool mine = lane >= s && lane < e;  // lane as SEQUENCE index of this batch
+            // ---- empty sequences: one record (the empty variant) each ----
+            if (mine && Li == 0) {
+                const u64 h = K_LEN;  // A[L] = 0, (L + 1) * K
+                const bool ok = !chunked || gen_chunk_of(h, P.n_chunks) == P.chunk;
+                if (COUNT_ONLY) {
+                    P.cnt[gid0 + lane] = ok ? 1u : 0u;
+                } else if (ok) {
+                    const u64 key = h >> kshift;
+                    P.records[rec_base_i] = (key << P.id_bits) | (gid0 + lane);
+                    for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
+                }
+            }
+            if (total > 0) {
+                // ---- lane as POSITION: which sequence, which offset inside it ----
+                const u32 hbit = (mine && Li > 0) ? (1u << (cum_excl - base)) : 0u;
+                const u32 heads = __reduce_or_sync(SD_FULL, hbit);
+                if (mine && Li > 0) sh.map[warp][cum_excl - base] = (unsigned char)lane;
+                __syncwarp();
+                const bool active = lane < total;
+                const u32 seg_start = active ? (31u - __clz(heads & (0xffffffffu >> (31u - lane)))) : 0u;
+                const u32 si = active ? sh.map[warp][seg_start] : 0u;  // sequence index within the task
+                const u32 L = __shfl_sync(SD_FULL, Li, si);
+                const u64 rec_base = __shfl_sync(SD_FULL, rec_base_i, si);
+                const u32 a = lane - seg_start;
+                const u64 gid = gid0 + si;
+                const u32 segmask = active ? (((L == 32u) ? 0xffffffffu : ((1u << L) - 1u)) << seg_start) : 0u;
+                const u32 c = active ? ((u32)(unsigned char)S.seqs[obase + base + lane] & 31u) : 0u;
+                const u32 cn = __shfl_down_sync(SD_FULL, c, 1), cnn = __shfl_down_sync(SD_FULL, c, 2);
+                const bool has1 = a + 1 < L, has2 = a + 2 < L;
+                const bool canon1 = active && (!thinning || !has1 || c != cn);
+                const bool adjok = active && has1 && (!thinning || !has2 || (c != cnn && cn != cnn));
+                const u32 m1 = __ballot_sync(SD_FULL, canon1), madj = __ballot_sync(SD_FULL, adjok);
+
+                u32 run = 0;  // records of this lane's sequence so far (uniform inside a segment)
+                if (COUNT_ONLY && !chunked) {
+                    const u32 B = __popc(m1 & segmask);
+                    run = 1;
+                    if (d >= 1) run += B;
+                    if (d >= 2) {
+                        const u32 inner = segmask & (segmask >> 1);  // positions p with p + 1 inside the segment
+                        run += B * (B - 1) / 2 - __popc(m1 & (m1 >> 1) & inner) + __popc(madj & segmask);
+                    }
+                } else {
+                    // ---- prefix hashes of the source sequences (segmented scan over lanes) ----
+                    const u64 term = active ? sh.R[c] * sh.Bpow[a] : 0ull;
+                    u64 aincl = term;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const u64 t = __shfl_up_sync(SD_FULL, aincl, o);
+                        if (a >= (u32)o) aincl += t;
+                    }
+                    const u64 aexcl = aincl - term;
+                    const u64 AL = __shfl_sync(SD_FULL, aincl, active ? seg_start + L - 1 : 0);
+                    const u64 Uv = aexcl - binv1 * aincl;
+                    sh.U[warp][lane] = Uv;
+                    sh.V[warp][lane] = binv1 * Uv;
+                    __syncwarp();
+                    const u64 C0 = AL + (u64)(L + 1) * K_LEN;
+                    const u64 C1 = binv1 * AL + (u64)L * K_LEN;
+                    const u64 C2 = binv2 * AL + (u64)(L - 1) * K_LEN;
+
+                    auto emit = [&](bool valid, u64 h) {
+                        if (chunked) valid = valid && gen_chunk_of(h, P.n_chunks) == P.chunk;
+                        const u32 bal = __ballot_sync(SD_FULL, valid) & segmask;
+                        if (!COUNT_ONLY && valid) {
+                            const u64 key = h >> kshift;
+                            P.records[rec_base + run + __popc(bal & lane_lt)] = (key << P.id_bits) | gid;
+                            for (int ps = 0; ps < P.npass; ++ps)
+                                atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
+                        }
+                        run += __popc(bal);
+                    };
+                    emit(active && a == 0, C0);
+                    if (d >= 1) emit(canon1, Uv + C1);
+                    if (d >= 2) {
+                        const u32 half = __reduce_max_sync(SD_FULL, active ? (L >> 1) : 0u);
+                        for (u32 dl = 1; dl <= half; ++dl) {
+                            const bool on = active && (2 * dl < L || (2 * dl == L && a < dl));
+                            u32 b = a + dl;
+                            if (b >= L) b -= L;
+                            bool canon = false;
+                            u64 h = 0;
+                            if (on) {
+                                const u32 p1 = min(a, b), p2 = max(a, b);
+                                const u32 l1 = seg_start + p1, l2 = seg_start + p2;
+                                canon = (p2 - p1 == 1u) ? ((madj >> l1) & 1u) : (((m1 >> l1) & (m1 >> l2)) & 1u);
+                                h = sh.U[warp][l1] + sh.V[warp][l2] + C2;
+                            }
+                            emit(canon, h);
+                        }
+                    }
+                    __syncwarp();  // U/V/map are reused by the next batch
+                }
+                if (active && a == 0) {
+                    if (COUNT_ONLY) P.cnt[gid] = run;
+                    else if ((u64)run != P.rec_off[gid + 1] - rec_base) atomicOr(&P.info->err, (u32)SD_ERR_INTERNAL);
+                }
+            }
+            s = e;
+        }
+    }
+    if (!COUNT_ONLY) {
+        __syncthreads();
+        for (int i = tid; i < P.npass * 256; i += G2_THREADS)
+            if (s_hist[i]) atomicAdd(&P.ghist[i], s_hist[i]);
+    }
+}
+
 u64 splitmix64(u64& x) {
     u64 z = (x += 0x9e3779b97f4a7c15ull);
     z = (z ^ (z >> 30)) * 0xbf58476d1ce4e5b9ull;
@@ -370,6 +560,16 @@ GenParams make_params(SeqSetDev a, SeqSetDev b, const Layout& lay, int width) {
 }
 
 int gen_grid(i64 groups) { return (int)std::min<i64>(groups, 148 * 6); }
+
+bool use_fast(const Layout& lay, int width) { return lay.d <= 2 && width - 1 <= 32 && !lay.force_general; }
+
+GenParams make_params2(SeqSetDev a, SeqSetDev b, const Layout& lay, int width) {
+    GenParams P = make_params(a, b, lay, width);
+    P.groups_a = (a.n + 31) / 32;  // warp tasks of 32 sequences
+    P.groups_total = P.groups_a + (b.n + 31) / 32;
+    return P;
+}
+int gen2_grid(i64 wtasks) { return (int)std::min<i64>((wtasks + G2_NW - 1) / G2_NW, 148 * 8); }
 
 }  // namespace
 
@@ -414,6 +614,9 @@ cudaError_t sd_init_tables() {
     if ((e = cudaFuncSetAttribute(k_generate<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)sizeof(GenShared))) != cudaSuccess)
         return e;
+    if ((e = cudaFuncSetAttribute(k_gen2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)(sizeof(Gen2Shared) + 8 * 256 * 4))) != cudaSuccess)
+        return e;
     done = true;
     return cudaSuccess;
 }
@@ -428,11 +631,13 @@ cudaError_t sd_prepare(SeqSetDev s, int d, DevInfo* info, cudaStream_t st, i64* 
 
 cudaError_t sd_count(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u32* cnt, DevInfo* info, cudaStream_t st,
                      i64* launches) {
-    GenParams P = make_params(a, b, lay, width);
+    const bool fast = use_fast(lay, width);
+    GenParams P = fast ? make_params2(a, b, lay, width) : make_params(a, b, lay, width);
     if (P.groups_total == 0) return cudaSuccess;
     P.cnt = cnt;
     P.info = info;
-    k_generate<true><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared), st>>>(P);
+    if (fast) k_gen2<true><<<gen2_grid(P.groups_total), G2_THREADS, sizeof(Gen2Shared), st>>>(P);
+    else k_generate<true><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared), st>>>(P);
     if (launches) ++*launches;
     return cudaGetLastError();
 }
@@ -451,14 +656,18 @@ cudaError_t sd_scan_counts(const u32* cnt, i64 n, u64* rec_off, u64* lb_status, 
 
 cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, const u64* rec_off, u64* records,
                         u32* ghist, int npass, DevInfo* info, cudaStream_t st, i64* launches) {
-    GenParams P = make_params(a, b, lay, width);
+    const bool fast = use_fast(lay, width);
+    GenParams P = fast ? make_params2(a, b, lay, width) : make_params(a, b, lay, width);
     if (P.groups_total == 0) return cudaSuccess;
     P.rec_off = rec_off;
     P.records = records;
     P.ghist = ghist;
     P.npass = npass;
     P.info = info;
-    k_generate<false><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared) + (size_t)npass * 256 * 4, st>>>(P);
+    if (fast)
+        k_gen2<false><<<gen2_grid(P.groups_total), G2_THREADS, sizeof(Gen2Shared) + (size_t)npass * 256 * 4, st>>>(P);
+    else
+        k_generate<false><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared) + (size_t)npass * 256 * 4, st>>>(P);
     if (launches) ++*launches;
     return cudaGetLastError();
 }

@@ -27,6 +27,7 @@ struct Layout {
     int b_bits;        // bits of the second pair component (self: id_bits; cross: bits of n_b)
     int pair_bits;     // a_bits + b_bits
     int thinning;
+    int force_general;  // test hook: never take the d <= 2 fast generation path
     u32 n_chunks, chunk;
 };
 

@@ -28,7 +28,7 @@ struct symdel_ctx {
     cudaError_t last_cuda = cudaSuccess;
     symdel_stats stats{};
     int opt_timing = 0;
-    i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0;
+    i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0, opt_general_gen = 0;
     DevInfo* h_info = nullptr;  // pinned
     void* arena = nullptr;      // device arena of the *_host entry points
     size_t arena_bytes = 0;
@@ -85,7 +85,7 @@ u64 vcount_host(int L, int d) {
 }
 
 i64 rec_bytes(i64 ncap, int npass) {
-    return 2 * align_up(ncap * 8) + align_up(sd_sort_scratch_bytes(ncap, npass)) + 2 * align_up((sd_emit_tiles(ncap) + 2) * 8);
+    return 2 * align_up(ncap * 8) + align_up(sd_sort_scratch_bytes(ncap, npass)) + align_up((2 * sd_emit_tiles(ncap) + 2) * 8);
 }
 i64 cand_bytes(i64 ccap, int ppass) {
     return 2 * align_up(ccap * 8) + align_up(sd_sort_scratch_bytes(ccap, ppass)) + align_up((sd_verify_tiles(ccap) + 1) * 8);
@@ -179,6 +179,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     lay.b_bits = cross ? bits_for(B.n) : lay.id_bits;
     lay.pair_bits = (cross ? bits_for(A.n) : lay.id_bits) + lay.b_bits;
     lay.thinning = ctx->opt_no_thinning ? 0 : 1;
+    lay.force_general = ctx->opt_general_gen ? 1 : 0;
     {
         int hb = (int)ctx->opt_hash_bits;
         if (hb == 0) {
@@ -220,8 +221,8 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     u64* recA = ws.take<u64>(ncap);
     u64* recB = ws.take<u64>(ncap);
     void* rec_scratch = ws.take<char>(sd_sort_scratch_bytes(ncap, npass));
-    u64* tile_prefix = ws.take<u64>(sd_emit_tiles(ncap) + 2);
-    u64* emit_lb = ws.take<u64>(sd_emit_tiles(ncap) + 2);
+    u64* tile_prefix = ws.take<u64>(2 * sd_emit_tiles(ncap) + 2);
+    u64* emit_lb = nullptr;
     u64* candA = ws.take<u64>(ccap);
     u64* candB = ws.take<u64>(ccap);
     void* cand_scratch = ws.take<char>(sd_sort_scratch_bytes(ccap, ppass));
@@ -476,6 +477,7 @@ int symdel_set_option(symdel_ctx* ctx, int option, int64_t value) {
             ctx->opt_hash_bits = value;
             break;
         case SYMDEL_OPT_NO_THINNING: ctx->opt_no_thinning = value != 0; break;
+        case SYMDEL_OPT_GENERAL_GENERATE: ctx->opt_general_gen = value != 0; break;
         case SYMDEL_OPT_SORT_VARIANT:
             if (sd_sort_set_variant((int)value)) return SYMDEL_E_ARG;
             break;
@@ -609,6 +611,7 @@ int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const int64_t* of
     lay.id_bits = id_bits;
     lay.hash_bits = hash_bits;
     lay.thinning = thinning;
+    lay.force_general = ctx->opt_general_gen ? 1 : 0;
     lay.n_chunks = 1;
     const int width = (int)ctx->h_info->maxlen + 1;
     CK(sd_count(A, B, lay, width, cnt, info, st, nullptr));

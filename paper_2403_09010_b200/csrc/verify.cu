@@ -103,11 +103,13 @@ __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ c
     u32 total;
     const u32 rank = sd_block_excl_sum<VF_THREADS>(keep ? 1u : 0u, &total, s_warp);
     const u32 nuniq = __syncthreads_count(uniq);
-    if (tid == 0) {
-        const u64 excl = sd_lookback(lb_status, tile, total);
-        s_excl = excl;
-        if (nuniq) atomicAdd((unsigned long long*)&info->n_unique, (unsigned long long)nuniq);
-        if (tile == gridDim.x - 1) info->n_surv = surv_base + excl + total;
+    if (tid < 32) {
+        const u64 excl = sd_lookback_warp(lb_status, tile, total);
+        if (tid == 0) {
+            s_excl = excl;
+            if (nuniq) atomicAdd((unsigned long long*)&info->n_unique, (unsigned long long)nuniq);
+            if (tile == gridDim.x - 1) info->n_surv = surv_base + excl + total;
+        }
     }
     __syncthreads();
     if (keep) {
@@ -142,10 +144,12 @@ __global__ void __launch_bounds__(FN_THREADS) k_finalize(const u64* __restrict__
     }
     u32 total;
     const u32 rank = sd_block_excl_sum<FN_THREADS>(keep ? 1u : 0u, &total, s_warp);
-    if (tid == 0) {
-        const u64 excl = sd_lookback(lb_status, tile, total);
-        s_excl = excl;
-        if (tile == gridDim.x - 1) info->n_out = excl + total;
+    if (tid < 32) {
+        const u64 excl = sd_lookback_warp(lb_status, tile, total);
+        if (tid == 0) {
+            s_excl = excl;
+            if (tile == gridDim.x - 1) info->n_out = excl + total;
+        }
     }
     __syncthreads();
     if (keep) {

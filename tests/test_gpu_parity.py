@@ -157,6 +157,26 @@ def test_lev_random_up_to_L_MAX(torch, sd, ctx, oracle):
 
 
 # ---- S1/K1: variant generation -----------------------------------------------------------------------
+def test_generate_fast_and_general_paths_agree(torch, sd, oracle):
+    """The d <= 2 warp-per-batch kernel and the general kernel compute the same hash function and the
+    same thinning: identical record multisets per sequence (their enumeration orders differ)."""
+    s = synth.SeqSet(*[np.concatenate(x) for x in zip(
+        (synth.tcr_set(3000, 5).seqs, synth.tcr_set(3000, 5).offsets[:-1]),
+        (synth.repeat_heavy_set(500, 6, alphabet=2, lo=0, hi=32).seqs,
+         synth.repeat_heavy_set(500, 6, alphabet=2, lo=0, hi=32).offsets + synth.tcr_set(3000, 5).offsets[-1]))])
+    ds, do = sd.to_device(s)
+    for d in (0, 1, 2):
+        for thinning in (True, False):
+            recs = []
+            for general in (0, 1):
+                c = sd.Context(0)
+                c.symdel_set_option(sd.OPT_GENERAL_GENERATE, general)
+                r = c.symdel_stage_generate(ds, do, d, 40, 13, thinning, 4_000_000).cpu().numpy().view(np.uint64)
+                assert (np.diff((r & np.uint64(8191)).astype(np.int64)) >= 0).all()
+                recs.append(np.sort(r))
+            assert np.array_equal(recs[0], recs[1]), (d, thinning)
+
+
 @pytest.mark.parametrize("d", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("thinning", [True, False])
 def test_generate_groups_match_oracle_variants(torch, sd, ctx, oracle, d, thinning):
@@ -262,7 +282,8 @@ def test_validation_protocol_5000(sd, ctx, oracle, family, d):
 
 @pytest.mark.parametrize("opts", [
     {"FORCE_CHUNKS": 4}, {"FORCE_CHUNKS": 16}, {"CAND_CAPACITY": 4999}, {"HASH_BITS": 8}, {"HASH_BITS": 48},
-    {"NO_THINNING": 1}, {"FORCE_CHUNKS": 3, "CAND_CAPACITY": 777, "HASH_BITS": 16},
+    {"NO_THINNING": 1}, {"FORCE_CHUNKS": 3, "CAND_CAPACITY": 777, "HASH_BITS": 16}, {"GENERAL_GENERATE": 1},
+    {"GENERAL_GENERATE": 1, "FORCE_CHUNKS": 5}, {"SORT_VARIANT": 1}, {"SORT_VARIANT": 3},
 ])
 def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
     """P-11: chunk count, candidate-buffer windows, key width and thinning change memory use and
@@ -272,7 +293,10 @@ def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
     c = sd.Context(0)
     for k, v in opts.items():
         c.symdel_set_option(getattr(sd, "OPT_" + k), v)
-    assert_same(run_self(sd, c, s, 2), exp)
+    try:
+        assert_same(run_self(sd, c, s, 2), exp)
+    finally:
+        c.symdel_set_option(sd.OPT_SORT_VARIANT, 0)  # process-wide hook: restore
     st = c.symdel_get_stats()
     if "FORCE_CHUNKS" in opts:
         assert st["n_chunks"] == opts["FORCE_CHUNKS"]
