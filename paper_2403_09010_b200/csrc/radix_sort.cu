@@ -51,12 +51,27 @@ __global__ void __launch_bounds__(256) k_hist_scan(u32* __restrict__ ghist) {
 // instruction measured ~170 cycles per warp on sm_100a; 8 x (VOTE + LOP3) is ~10x cheaper).
 __device__ __forceinline__ u32 os_match8(u32 dg, u32 init) {
     u32 peers = init;
-#pragma unroll
-    for (int b = 0; b < 8; ++b) {
-        const bool bit = (dg >> b) & 1u;
-        const u32 v = __ballot_sync(SD_FULL, bit);
-        peers &= bit ? v : ~v;
-    }
+    // per bit: LOP3 (test -> predicate), VOTE, one of two predicated LOP3s (peers &= v / peers &= ~v)
+#define OS_MATCH_BIT(B)                                                                          \
+    asm volatile(                                                                                \
+        "{\n\t.reg .pred p;\n\t.reg .b32 t, v;\n\t"                                              \
+        "and.b32 t, %1, " #B ";\n\t"                                                             \
+        "setp.ne.u32 p, t, 0;\n\t"                                                               \
+        "vote.sync.ballot.b32 v, p, 0xffffffff;\n\t"                                             \
+        "@p and.b32 %0, %0, v;\n\t"                                                              \
+        "@!p lop3.b32 %0, %0, v, 0, 0x30;\n\t"                                                   \
+        "}"                                                                                      \
+        : "+r"(peers)                                                                            \
+        : "r"(dg))
+    OS_MATCH_BIT(1);
+    OS_MATCH_BIT(2);
+    OS_MATCH_BIT(4);
+    OS_MATCH_BIT(8);
+    OS_MATCH_BIT(16);
+    OS_MATCH_BIT(32);
+    OS_MATCH_BIT(64);
+    OS_MATCH_BIT(128);
+#undef OS_MATCH_BIT
     return peers;
 }
 
@@ -123,13 +138,29 @@ __device__ __forceinline__ void os_tile(const u64* __restrict__ in, u64* __restr
     if (tid < 256) {
         u32 excl = 0;
         if (tile != 0) {
-            const u32* p = st - 256;
-            while (true) {
-                u32 s;
-                do { s = sd_ld_relaxed32(p); } while ((s >> 30) == 0);
-                excl += s & OS_MASK;
-                if ((s >> 30) == 2) break;
-                p -= 256;
+            // four predecessors per round trip: the walk back to the nearest inclusive prefix is a chain
+            // of L2 latencies, so loads are issued in batches and consumed in order
+            const u32* p = st;
+            u32 rem = tile;
+            bool done = false;
+            while (!done) {
+                u32 sv[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) sv[j] = ((u32)j < rem) ? sd_ld_relaxed32(p - 256 * (j + 1)) : OS_FLAG_PRE;
+                int used = 0;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    if (!done && used == j) {
+                        const u32 f = sv[j] >> 30;
+                        if (f != 0) {
+                            excl += sv[j] & OS_MASK;
+                            used = j + 1;
+                            done = (f == 2);
+                        }
+                    }
+                }
+                p -= 256 * used;
+                rem -= (u32)used;
             }
             sd_st_relaxed32(st, OS_FLAG_PRE | (excl + total));
         }

@@ -100,8 +100,15 @@ struct Timer {
     cudaStream_t st;
     bool on;
     size_t next = 0;
-    std::vector<std::pair<int, size_t>> marks;  // (stage id, event index) pairs: begin/end alternate
+    struct Span { int stage; size_t a, b; };
+    std::vector<Span> spans;  // evaluated after the final synchronize (events must have completed)
     Timer(symdel_ctx* c, cudaStream_t s) : ctx(c), st(s), on(c->opt_timing != 0) {}
+    void span(int stage, size_t a, size_t b) { if (on) spans.push_back({stage, a, b}); }
+    float total(int stage) {
+        float t = 0;
+        for (auto& sp : spans) if (sp.stage == stage) t += ms(sp.a, sp.b);
+        return t;
+    }
     size_t mark() {
         if (!on) return 0;
         if (next >= ctx->events.size()) {
@@ -235,12 +242,13 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
 
     const int width = maxlen + 1;
     i64 n_surv = 0, flushes = 0;
-    float ms_gen = 0, ms_sort = 0, ms_emit = 0, ms_dedup = 0, ms_verify = 0, ms_pass = 0;
+    enum { ST_GEN, ST_SORT, ST_EMIT, ST_DEDUP, ST_VERIFY };
     i64 pass_count = 0;
-    std::vector<cudaEvent_t> pass_ev;
 
 restart:
     if (P > 65536) return SYMDEL_E_WORKSPACE;
+    tm.spans.clear();
+    pass_count = 0;
     n_surv = 0;
     flushes = 0;
     S.n_records = S.n_candidates = 0;
@@ -278,14 +286,11 @@ restart:
         const i64 C = (i64)ctx->h_info->n_cand;
         S.n_candidates += C;
         const size_t e3 = tm.mark();
-        ms_gen += tm.ms(e0, e1);
-        ms_sort += tm.ms(e1, e2);
-        ms_emit += tm.ms(e2, e3);
-        if (tm.on) {
-            ms_pass += tm.ms(e1, e2);
-            pass_count += npass;
-            S.sort_pass_records = N;
-        }
+        tm.span(ST_GEN, e0, e1);
+        tm.span(ST_SORT, e1, e2);
+        tm.span(ST_EMIT, e2, e3);
+        pass_count += npass;
+        S.sort_pass_records = N;
         for (i64 w0 = 0; w0 < C; w0 += ccap) {
             const i64 nc = std::min<i64>(ccap, C - w0);
             const size_t f0 = tm.mark();
@@ -308,9 +313,9 @@ restart:
             if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
             n_surv = (i64)ctx->h_info->n_surv;
             const size_t f3 = tm.mark();
-            ms_emit += tm.ms(f0, f1);
-            ms_dedup += tm.ms(f1, f2);
-            ms_verify += tm.ms(f2, f3);
+            tm.span(ST_EMIT, f0, f1);
+            tm.span(ST_DEDUP, f1, f2);
+            tm.span(ST_VERIFY, f2, f3);
             ++flushes;
         }
     }
@@ -338,13 +343,13 @@ restart:
     if (tm.on) {
         CK(cudaStreamSynchronize(st));
         S.ms_prepare = tm.ms(ev_begin, ev_prepared);
-        S.ms_generate = ms_gen;
-        S.ms_sort = ms_sort;
-        S.ms_emit = ms_emit;
-        S.ms_dedup = ms_dedup;
-        S.ms_verify = ms_verify + tm.ms(g0, g1);
+        S.ms_generate = tm.total(ST_GEN);
+        S.ms_sort = tm.total(ST_SORT);
+        S.ms_emit = tm.total(ST_EMIT);
+        S.ms_dedup = tm.total(ST_DEDUP);
+        S.ms_verify = tm.total(ST_VERIFY) + tm.ms(g0, g1);
         S.ms_total = tm.ms(ev_begin, g1);
-        S.ms_sort_pass_avg = pass_count ? ms_pass / (float)pass_count : 0.f;
+        S.ms_sort_pass_avg = pass_count ? S.ms_sort / (float)pass_count : 0.f;
     }
     S.n_unique = (i64)ctx->h_info->n_unique;
     S.n_outputs = n_out;
