@@ -141,10 +141,12 @@ SYMDEL_API int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const 
                           int id_bits, int thinning, uint64_t* records, int64_t records_capacity,
                           int64_t* n_records_host, void* workspace, int64_t workspace_bytes, void* cuda_stream);
 
-/* S4/K6: dist[t] = lev(a_{ia[t]}, b_{ib[t]}) by the bit-parallel verifier, for n_pairs index pairs. */
+/* S4/K6: dist[t] = lev(a_{ia[t]}, b_{ib[t]}) by the bit-parallel verifier, for n_pairs index pairs.
+ *   workspace: device scratch of at least 512 + 48 * (n_a + n_b) bytes (the packed bit-plane table). */
 SYMDEL_API int symdel_stage_lev(symdel_ctx* ctx, const int8_t* a_seqs, const int64_t* a_offsets, int64_t n_a,
                      const int8_t* b_seqs, const int64_t* b_offsets, int64_t n_b, const int32_t* ia,
-                     const int32_t* ib, int64_t n_pairs, int32_t* dist, void* cuda_stream);
+                     const int32_t* ib, int64_t n_pairs, int32_t* dist, void* workspace, int64_t workspace_bytes,
+                     void* cuda_stream);
 
 #ifdef __cplusplus
 }

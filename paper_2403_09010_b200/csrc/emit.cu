@@ -12,140 +12,86 @@
 //   cross: records are sorted by (hash, id) and query ids are below reference ids, so a run is
 //          [q .. q r .. r]; a reference record pairs with [run_start, first reference of the run),
 //          a query record with nothing.
-// The per-record counts are scanned inside the tile; a tile claims its output range with one atomic
-// add (candidate order is irrelevant: they are sorted next); pairs are then written by FLAT pair index (binary search into the scanned counts), so a
-// long run is spread over the whole block instead of serialising one thread.  Only pairs whose flat
-// index lies in [win_lo, win_hi) are written: when the candidate buffer is smaller than the total,
-// the host replays the kernel once per window (later rounds reuse the saved tile prefixes).
+// Runs are short on this workload (a run of m records holds m distinct sequences sharing one variant),
+// so each record finds its partners by walking BACKWARDS from its own position while the hash matches
+// (shared memory inside the tile, global memory beyond its start); the walk costs what the pairs it
+// emits cost.  Counts are scanned inside the block, the tile claims its output range with ONE atomic
+// add (candidate order is irrelevant: they are sorted next) and every record then writes its own
+// pairs.  Only pairs whose flat index lies in [win_lo, win_hi) are written: when the candidate buffer
+// is smaller than the total, the host replays the kernel once per window (later rounds reuse the
+// saved per-tile base and count, so the numbering is the same in every round of one call).
 #include "kernels.h"
 
 namespace {
 
-constexpr int EM_THREADS = 256, EM_IPT = 4, EM_TILE = EM_THREADS * EM_IPT;
-
-__device__ __forceinline__ u64 block_excl_sum64(u64 v, u64* total, u64* s_warp /* [EM_THREADS/32 + 1] */) {
-    const u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    u64 inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        u64 t = __shfl_up_sync(SD_FULL, inc, o);
-        if (lane >= (u32)o) inc += t;
-    }
-    if (lane == 31) s_warp[warp] = inc;
-    __syncthreads();
-    u64 carry = 0, all = 0;
-#pragma unroll
-    for (int w = 0; w < EM_THREADS / 32; ++w) {
-        u64 c = s_warp[w];
-        if ((u32)w < warp) carry += c;
-        all += c;
-    }
-    *total = all;
-    __syncthreads();
-    return carry + inc - v;
-}
+constexpr int EM_THREADS = 256, EM_IPT = 16, EM_TILE = EM_THREADS * EM_IPT;
 
 __global__ void __launch_bounds__(EM_THREADS) k_emit(const u64* __restrict__ rec, u64 n, Layout lay, u64* __restrict__ cand,
                                                     u64 win_lo, u64 win_hi, int first_round, u64* tile_prefix,
-                                                    u64* lb_status, DevInfo* info) {
-    __shared__ u64 s_rec[EM_TILE + 1];   // s_rec[0] = record before the tile
-    __shared__ u64 s_scan[EM_TILE + 1];  // exclusive pair offsets inside the tile
-    __shared__ i64 s_a[EM_TILE];         // partner range start (global position)
-    __shared__ u64 s_warp64[EM_THREADS / 32 + 1];
-    __shared__ i32 s_warp32[EM_THREADS / 32];
-    __shared__ i64 s_tile_rs;
+                                                    DevInfo* info) {
+    __shared__ u64 s_rec[EM_TILE + 1];  // s_rec[0] = record before the tile
+    __shared__ u64 s_wsum[EM_THREADS / 32];
     __shared__ u64 s_excl;
 
-    const u32 tid = threadIdx.x;
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const u32 tile = blockIdx.x;
     if (!first_round) {
-        // skip tiles whose pairs lie entirely outside the window
         const u64 lo = tile_prefix[2 * tile], cnt = tile_prefix[2 * tile + 1];
-        if (cnt == 0 || lo + cnt <= win_lo || lo >= win_hi) return;
+        if (cnt == 0 || lo + cnt <= win_lo || lo >= win_hi) return;  // nothing of this tile in the window
     }
-    const u64 base = (u64)tile * EM_TILE;
-    const u32 tile_n = (u32)min((u64)EM_TILE, n - base);
+    const i64 base = (i64)tile * EM_TILE;
+    const u32 tile_n = (u32)min((u64)EM_TILE, n - (u64)base);
     const int idb = lay.id_bits;
     const u64 idmask = (1ull << idb) - 1ull;
+    const u64 n_a = (u64)lay.n_a;
+    const bool cross = lay.cross != 0;
 
     for (u32 i = tid; i < tile_n; i += EM_THREADS) s_rec[i + 1] = rec[base + i];
     if (tid == 0) s_rec[0] = base > 0 ? rec[base - 1] : 0ull;
     __syncthreads();
 
-    if (tid == 0) {
-        // run start of the tile's first record when that run began in an earlier tile
-        i64 rs = (i64)base;
-        if (base > 0 && (s_rec[0] >> idb) == (s_rec[1] >> idb)) {
-            const u64 target = (s_rec[1] >> idb) << idb;  // smallest record with this hash
-            u64 lo = 0, hi = base - 1;                     // rec[hi] has the hash; find first pos with rec >= target
-            while (lo < hi) {
-                u64 mid = (lo + hi) >> 1;
-                if (rec[mid] >= target) hi = mid; else lo = mid + 1;
-            }
-            rs = (i64)lo;
-        }
-        s_tile_rs = rs;
-    }
+    auto at = [&](i64 gp) -> u64 { return gp >= base - 1 ? s_rec[gp - base + 1] : rec[gp]; };
 
-    // ---- run starts: max-scan of head positions ----
-    i32 rs_local[EM_IPT];
-    i32 last = -1;
+    // ---- phase 1: partners per record ----
+    u32 cnt[EM_IPT];
+    u64 tsum = 0;
 #pragma unroll
     for (int k = 0; k < EM_IPT; ++k) {
-        const u32 pos = tid * EM_IPT + k;
+        const u32 pos = k * EM_THREADS + tid;
+        u32 c = 0;
         if (pos < tile_n) {
-            const bool head = (base + pos == 0) || ((s_rec[pos] >> idb) != (s_rec[pos + 1] >> idb));
-            if (head) last = (i32)pos;
-        }
-        rs_local[k] = last;
-    }
-    const i32 carry = sd_block_excl_max<EM_THREADS>(last, s_warp32);  // contains __syncthreads: s_tile_rs visible
-    const i64 tile_rs = s_tile_rs;
-
-    // ---- partner ranges and pair counts ----
-    u64 pc[EM_IPT], tsum = 0;
-#pragma unroll
-    for (int k = 0; k < EM_IPT; ++k) {
-        const u32 pos = tid * EM_IPT + k;
-        pc[k] = 0;
-        if (pos < tile_n) {
-            const i32 r = rs_local[k] >= 0 ? rs_local[k] : carry;
-            const i64 rs = r >= 0 ? (i64)base + r : tile_rs;
-            const i64 gpos = (i64)base + pos;
-            i64 b = gpos;
-            if (lay.cross) {
-                const u64 me = s_rec[pos + 1];
-                if ((me & idmask) < (u64)lay.n_a) {
-                    b = rs;  // query record: pairs with nothing
-                } else {
-                    // first position in [rs, gpos] whose id is a reference id
-                    i64 lo = rs, hi = gpos;
-                    while (lo < hi) {
-                        i64 mid = (lo + hi) >> 1;
-                        const u64 x = mid >= (i64)base - 1 ? s_rec[mid - (i64)base + 1] : rec[mid];
-                        if ((x & idmask) >= (u64)lay.n_a) hi = mid; else lo = mid + 1;
-                    }
-                    b = lo;
+            const u64 me = s_rec[pos + 1];
+            const u64 h = me >> idb;
+            if (!cross || (me & idmask) >= n_a) {  // cross: only reference records collect partners
+                i64 gp = base + pos - 1;
+                while (gp >= 0) {
+                    const u64 x = at(gp);
+                    if ((x >> idb) != h) break;
+                    c += (!cross || (x & idmask) < n_a) ? 1u : 0u;  // cross: partners are the run's queries
+                    --gp;
                 }
             }
-            s_a[pos] = rs;
-            pc[k] = (u64)(b - rs);
-            tsum += pc[k];
         }
+        cnt[k] = c;
+        tsum += c;
     }
-    u64 T;
-    u64 run = block_excl_sum64(tsum, &T, s_warp64);
+    // ---- block exclusive scan of the per-thread totals ----
+    u64 inc = tsum;
 #pragma unroll
-    for (int k = 0; k < EM_IPT; ++k) {
-        const u32 pos = tid * EM_IPT + k;
-        if (pos < tile_n) s_scan[pos] = run;
-        run += pc[k];
+    for (int o = 1; o < 32; o <<= 1) {
+        const u64 t = __shfl_up_sync(SD_FULL, inc, o);
+        if (lane >= (u32)o) inc += t;
+    }
+    if (lane == 31) s_wsum[warp] = inc;
+    __syncthreads();
+    u64 carry = 0, T = 0;
+#pragma unroll
+    for (int w = 0; w < EM_THREADS / 32; ++w) {
+        const u64 c = s_wsum[w];
+        if ((u32)w < warp) carry += c;
+        T += c;
     }
     if (tid == 0) {
-        s_scan[tile_n] = T;
-        // Output slots: the ORDER of candidates is irrelevant (they are sorted next), so a tile claims
-        // its range with one atomic add instead of an ordered scan across tiles; the claimed base is
-        // saved so that later windows of the same call see the same numbering.
         u64 excl;
         if (first_round) {
             excl = T ? (u64)atomicAdd((unsigned long long*)&info->n_cand, (unsigned long long)T) : 0ull;
@@ -157,24 +103,29 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(const u64* __restrict__ rec
         s_excl = excl;
     }
     __syncthreads();
-    const u64 excl = s_excl;
-    if (T == 0 || excl + T <= win_lo || excl >= win_hi) return;
+    if (T == 0) return;
+    u64 flat = s_excl + carry + inc - tsum;  // flat index of this thread's first pair
+    if (flat + tsum <= win_lo || flat >= win_hi) return;
 
-    // ---- write pairs by flat index ----
-    const u64 p_lo = win_lo > excl ? win_lo - excl : 0ull;
-    const u64 p_hi = min(T, win_hi - excl);
-    for (u64 p = p_lo + tid; p < p_hi; p += EM_THREADS) {
-        u32 lo = 0, hi = tile_n;  // largest idx with s_scan[idx] <= p
-        while (hi - lo > 1) {
-            u32 mid = (lo + hi) >> 1;
-            if (s_scan[mid] <= p) lo = mid; else hi = mid;
+    // ---- phase 2: every record writes its own pairs ----
+#pragma unroll
+    for (int k = 0; k < EM_IPT; ++k) {
+        if (cnt[k] == 0) continue;
+        const u32 pos = k * EM_THREADS + tid;
+        const u64 me = s_rec[pos + 1];
+        const u64 h = me >> idb;
+        const u64 b_id = cross ? (me & idmask) - n_a : (me & idmask);
+        i64 gp = base + pos - 1;
+        u32 left = cnt[k];
+        while (left) {
+            const u64 x = at(gp);
+            --gp;
+            if (cross && (x & idmask) >= n_a) continue;  // a reference record of the same run
+            if (flat >= win_lo && flat < win_hi) cand[flat - win_lo] = ((x & idmask) << lay.b_bits) | b_id;
+            ++flat;
+            --left;
         }
-        const i64 ppos = s_a[lo] + (i64)(p - s_scan[lo]);
-        const u64 partner = ppos >= (i64)base - 1 ? s_rec[ppos - (i64)base + 1] : rec[ppos];
-        const u64 a_id = partner & idmask;
-        u64 b_id = s_rec[lo + 1] & idmask;
-        if (lay.cross) b_id -= (u64)lay.n_a;
-        cand[excl + p - win_lo] = (a_id << lay.b_bits) | b_id;
+        (void)h;
     }
 }
 
@@ -190,8 +141,9 @@ cudaError_t sd_emit(const u64* records, i64 n_records, const Layout& lay, u64* c
         cudaError_t e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st);
         if (e != cudaSuccess) return e;
     }
+    (void)lb_status;
     k_emit<<<(unsigned)tiles, EM_THREADS, 0, st>>>(records, (u64)n_records, lay, cand, win_lo, win_hi, first_round,
-                                                    tile_prefix, lb_status, info);
+                                                    tile_prefix, info);
     if (launches) ++*launches;
     return cudaGetLastError();
 }

@@ -67,14 +67,17 @@ cudaError_t sd_emit(const u64* records, i64 n_records, const Layout& lay, u64* c
 
 // ---- verify.cu ----------------------------------------------------------------------------------
 i64 sd_verify_tiles(i64 n);
+// packed bit-plane table of all sequences (A then B): 32 B (maxlen <= 32) or 48 B per sequence
+i64 sd_pack_bytes(i64 n_total, int maxlen);
+cudaError_t sd_pack(SeqSetDev a, SeqSetDev b, int maxlen, void* slots, cudaStream_t st, i64* launches);
 // cand sorted ascending.  Drops repeats and a == b (self), computes lev, keeps <= d, appends
-// (pair << 3 | dist) in order to surv[surv_base + ...]; info->n_surv += kept; info->n_unique += unique.
-cudaError_t sd_verify(const u64* cand, i64 n_cand, SeqSetDev a, SeqSetDev b, const Layout& lay, int maxlen, u64* surv,
+// (pair << 3 | dist) in order to surv[surv_base + ...]; info->n_surv = total; info->n_unique += unique.
+cudaError_t sd_verify(const u64* cand, i64 n_cand, const void* slots, const Layout& lay, int maxlen, u64* surv,
                       u64 surv_base, u64 surv_capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
 // surv sorted ascending (and unique unless dedup = 1).  Unpacks to SoA outputs, first `capacity`
 // only; info->n_out = total.
 cudaError_t sd_finalize(const u64* surv, i64 n_surv, const Layout& lay, int dedup, i32* out_i, i32* out_j, i32* out_dist,
                         i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
-// plain distances for index pairs (stage test)
-cudaError_t sd_lev_pairs(SeqSetDev a, SeqSetDev b, const i32* ia, const i32* ib, i64 n_pairs, i32* dist,
+// plain distances for index pairs (stage test); slots = sd_pack of (A, B)
+cudaError_t sd_lev_pairs(const void* slots, i64 n_a, int maxlen, const i32* ia, const i32* ib, i64 n_pairs, i32* dist,
                          cudaStream_t st);

@@ -92,7 +92,7 @@ i64 cand_bytes(i64 ccap, int ppass) {
 }
 i64 fixed_bytes(i64 n_total) {
     return align_up((i64)sizeof(DevInfo)) + align_up(n_total * 4) + align_up((n_total + 1) * 8) +
-           align_up((sd_scan_tiles(n_total) + 1) * 8) + 4096;
+           align_up((sd_scan_tiles(n_total) + 1) * 8) + align_up(n_total * 48) + 4096;
 }
 
 struct Timer {
@@ -203,6 +203,11 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     S.hash_bits = lay.hash_bits;
     S.id_bits = lay.id_bits;
 
+    // ---- packed bit-plane table for the verifier ----
+    void* slots = ws.take<char>(sd_pack_bytes(n_total, maxlen));
+    if (!ws.ok) return SYMDEL_E_WORKSPACE;
+    CK(sd_pack(A, B, maxlen, slots, st, &S.n_launches));
+
     // ---- workspace plan ----
     const i64 R = ws.left() - 8192;
     i64 ccap = ctx->opt_cand_cap > 0 ? ctx->opt_cand_cap : std::max<i64>(1 << 20, nmax / 2);
@@ -306,7 +311,7 @@ restart:
             const size_t f2 = tm.mark();
             // ---- S4: unique + verify; survivors appended at n_surv (host-tracked upper bound not needed:
             // the kernel is given the base through the previous flush's total, read back below) ----
-            CK(sd_verify(csorted, nc, A, B, lay, maxlen, survA, (u64)n_surv, (u64)scap, verify_lb, info, st,
+            CK(sd_verify(csorted, nc, slots, lay, maxlen, survA, (u64)n_surv, (u64)scap, verify_lb, info, st,
                          &S.n_launches));
             rc = read_info(ctx, info, st);
             if (rc) return rc;
@@ -635,14 +640,26 @@ int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const int64_t* of
 
 int symdel_stage_lev(symdel_ctx* ctx, const int8_t* a_seqs, const int64_t* a_offsets, int64_t n_a, const int8_t* b_seqs,
                      const int64_t* b_offsets, int64_t n_b, const int32_t* ia, const int32_t* ib, int64_t n_pairs,
-                     int32_t* dist, void* cuda_stream) {
-    if (!ctx || n_pairs < 0) return SYMDEL_E_ARG;
+                     int32_t* dist, void* workspace, int64_t workspace_bytes, void* cuda_stream) {
+    if (!ctx || n_pairs < 0 || n_a < 0 || n_b < 0) return SYMDEL_E_ARG;
     if (n_pairs == 0) return SYMDEL_OK;
-    if (!a_seqs || !a_offsets || !b_seqs || !b_offsets || !ia || !ib || !dist) return SYMDEL_E_ARG;
+    if (!a_seqs || !a_offsets || !b_seqs || !b_offsets || !ia || !ib || !dist || !workspace) return SYMDEL_E_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CK(cudaSetDevice(ctx->device));
     SeqSetDev A{a_seqs, a_offsets, n_a}, B{b_seqs, b_offsets, n_b};
-    CK(sd_lev_pairs(A, B, ia, ib, n_pairs, dist, st));
+    Bump ws(workspace, workspace_bytes);
+    DevInfo* info = ws.take<DevInfo>(1);
+    void* slots = ws.take<char>(sd_pack_bytes(n_a + n_b, SD_L_MAX));
+    if (!ws.ok) return SYMDEL_E_WORKSPACE;
+    CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
+    CK(sd_prepare(A, 0, info, st, nullptr));
+    CK(sd_prepare(B, 0, info, st, nullptr));
+    int rc = read_info(ctx, info, st);
+    if (rc) return rc;
+    if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+    const int maxlen = (int)ctx->h_info->maxlen;
+    CK(sd_pack(A, B, maxlen, slots, st, nullptr));
+    CK(sd_lev_pairs(slots, n_a, maxlen, ia, ib, n_pairs, dist, st));
     CK(cudaStreamSynchronize(st));
     return SYMDEL_OK;
 }

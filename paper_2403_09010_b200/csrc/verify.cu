@@ -10,39 +10,90 @@
 // the left neighbour, fused into the verifier.  The distance is the bit-parallel global edit
 // distance of Myers (1999) in Hyyro's (2003) formulation: one machine word holds a column of
 // vertical deltas of the Wagner-Fischer table (pattern length <= 64, or <= 32 on the 32-bit path);
-// per text character it costs ~15 bit operations instead of a column of min/add.  The match mask
-// Eq[c] is rebuilt from five bit-planes of the pattern's 5-bit residue codes (3 logic ops per plane
-// pair) rather than looked up in a 32-entry table, which keeps the whole state in registers.
+// per text character it costs ~15 bit operations instead of a column of min/add.  Sequences are
+// pre-packed (k_pack) into five bit-planes of their 5-bit residue codes; the match mask Eq[c] is
+// rebuilt from the pattern's and the text's planes rather than looked up in a 32-entry table, which
+// keeps the whole state in registers and makes each sequence one aligned 32/48-byte gather.
 // Survivors are compacted in order (block scan + decoupled look-back), so the output stays sorted.
 #include "kernels.h"
 
 namespace {
 
+// ---- packed sequences: five bit-planes of the 5-bit residue codes + the length ---------------------
+// plane k, bit j = bit k of residue j.  NARROW (longest sequence <= 32): 8 x u32 = 32 B per sequence
+// {b0, b1, b2, b3, b4, len, 0, 0}; WIDE: 6 x u64 = 48 B {b0 .. b4, len}.  One aligned 32/48-byte gather
+// per sequence replaces two offset loads and ~15 unaligned byte loads in the verifier.
 template <typename W>
-__device__ __forceinline__ int myers_lev(const int8_t* __restrict__ p, int m, const int8_t* __restrict__ t, int n) {
+struct Planes {
+    W b[5];
+    int len;
+};
+
+template <typename W>
+__device__ __forceinline__ Planes<W> load_planes(const void* slots, u64 id);
+template <>
+__device__ __forceinline__ Planes<u32> load_planes<u32>(const void* slots, u64 id) {
+    const uint4* p = reinterpret_cast<const uint4*>(slots) + 2 * id;
+    const uint4 lo = __ldg(p), hi = __ldg(p + 1);
+    Planes<u32> r;
+    r.b[0] = lo.x, r.b[1] = lo.y, r.b[2] = lo.z, r.b[3] = lo.w, r.b[4] = hi.x;
+    r.len = (int)hi.y;
+    return r;
+}
+template <>
+__device__ __forceinline__ Planes<u64> load_planes<u64>(const void* slots, u64 id) {
+    const ulonglong2* p = reinterpret_cast<const ulonglong2*>(slots) + 3 * id;
+    const ulonglong2 x = __ldg(p), y = __ldg(p + 1), z = __ldg(p + 2);
+    Planes<u64> r;
+    r.b[0] = x.x, r.b[1] = x.y, r.b[2] = y.x, r.b[3] = y.y, r.b[4] = z.x;
+    r.len = (int)z.y;
+    return r;
+}
+
+template <typename W>
+__global__ void __launch_bounds__(256) k_pack(SeqSetDev A, SeqSetDev B, void* slots) {
+    const i64 g = (i64)blockIdx.x * 256 + threadIdx.x;
+    if (g >= A.n + B.n) return;
+    const SeqSetDev& S = g < A.n ? A : B;
+    const i64 i = g < A.n ? g : g - A.n;
+    const i64 o = S.off[i];
+    const int L = (int)(S.off[i + 1] - o);
+    W b[5] = {0, 0, 0, 0, 0};
+    for (int j = 0; j < L; ++j) {
+        const W c = (W)(unsigned char)S.seqs[o + j];
+#pragma unroll
+        for (int k = 0; k < 5; ++k) b[k] |= ((c >> k) & 1) << j;
+    }
+    if (sizeof(W) == 4) {
+        uint4* p = reinterpret_cast<uint4*>(slots) + 2 * g;
+        p[0] = make_uint4((u32)b[0], (u32)b[1], (u32)b[2], (u32)b[3]);
+        p[1] = make_uint4((u32)b[4], (u32)L, 0u, 0u);
+    } else {
+        ulonglong2* p = reinterpret_cast<ulonglong2*>(slots) + 3 * g;
+        p[0] = make_ulonglong2(b[0], b[1]);
+        p[1] = make_ulonglong2(b[2], b[3]);
+        p[2] = make_ulonglong2(b[4], (u64)L);
+    }
+}
+
+// Bit-parallel global edit distance (Myers 1999 / Hyyro 2003).  Pattern and text both arrive as
+// bit-planes; the match mask of text character i is Eq = AND_k ~(P_k xor -(T_k >> i & 1)).
+template <typename W>
+__device__ __forceinline__ int myers_lev(const Planes<W>& P, const Planes<W>& T) {
+    const int m = P.len, n = T.len;
     if (m == 0) return n;
     if (n == 0) return m;
-    W b0 = 0, b1 = 0, b2 = 0, b3 = 0, b4 = 0;
-    for (int j = 0; j < m; ++j) {
-        const W c = (W)(unsigned char)p[j];
-        b0 |= (c & 1) << j;
-        b1 |= ((c >> 1) & 1) << j;
-        b2 |= ((c >> 2) & 1) << j;
-        b3 |= ((c >> 3) & 1) << j;
-        b4 |= ((c >> 4) & 1) << j;
-    }
     const W mask = (m == (int)(8 * sizeof(W))) ? ~(W)0 : (((W)1 << m) - 1);
     const W top = (W)1 << (m - 1);
     W Pv = mask, Mv = 0;
     int score = m;
     for (int i = 0; i < n; ++i) {
-        const unsigned c = (unsigned char)t[i];
         W Eq = mask;
-        Eq &= (c & 1) ? b0 : ~b0;
-        Eq &= (c & 2) ? b1 : ~b1;
-        Eq &= (c & 4) ? b2 : ~b2;
-        Eq &= (c & 8) ? b3 : ~b3;
-        Eq &= (c & 16) ? b4 : ~b4;
+#pragma unroll
+        for (int k = 0; k < 5; ++k) {
+            const W mk = (W)0 - ((T.b[k] >> i) & 1);
+            Eq &= ~(P.b[k] ^ mk);
+        }
         const W Xv = Eq | Mv;
         const W Xh = (((Eq & Pv) + Pv) ^ Pv) | Eq;
         W Ph = Mv | ~(Xh | Pv);
@@ -57,19 +108,11 @@ __device__ __forceinline__ int myers_lev(const int8_t* __restrict__ p, int m, co
     return score;
 }
 
-__device__ __forceinline__ int lev_dispatch(const int8_t* p, int m, const int8_t* t, int n, bool narrow) {
-    // the shorter string is the pattern (fewer word bits; the distance is symmetric)
-    if (m > n) {
-        const int8_t* x = p; p = t; t = x;
-        int y = m; m = n; n = y;
-    }
-    return narrow ? myers_lev<u32>(p, m, t, n) : myers_lev<u64>(p, m, t, n);
-}
-
 constexpr int VF_THREADS = 256;
 
-__global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ cand, u64 n, SeqSetDev A, SeqSetDev B,
-                                                      Layout lay, int narrow, u64* __restrict__ surv, u64 surv_base,
+template <typename W>
+__global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ cand, u64 n, const void* __restrict__ slots,
+                                                      Layout lay, u64* __restrict__ surv, u64 surv_base,
                                                       u64 surv_capacity, u64* lb_status, DevInfo* info) {
     __shared__ u32 s_warp[VF_THREADS / 32 + 1];
     __shared__ u32 s_tile;
@@ -91,11 +134,11 @@ __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ c
         const u64 a = c >> lay.b_bits, b = c & ((1ull << lay.b_bits) - 1ull);
         if (!lay.cross && a == b) uniq = false;  // same sequence twice in one run (hash collision / no thinning)
         if (uniq) {
-            const i64 pa = A.off[a], pb = B.off[b];
-            const int la = (int)(A.off[a + 1] - pa), lb = (int)(B.off[b + 1] - pb);
-            const int dl = la > lb ? la - lb : lb - la;
+            const Planes<W> pa = load_planes<W>(slots, a);
+            const Planes<W> pb = load_planes<W>(slots, lay.cross ? (u64)lay.n_a + b : b);
+            const int dl = pa.len > pb.len ? pa.len - pb.len : pb.len - pa.len;
             if (dl <= lay.d) {
-                dist = lev_dispatch(A.seqs + pa, la, B.seqs + pb, lb, narrow != 0);
+                dist = myers_lev<W>(pa, pb);
                 keep = dist <= lay.d;
             }
         }
@@ -163,29 +206,42 @@ __global__ void __launch_bounds__(FN_THREADS) k_finalize(const u64* __restrict__
     }
 }
 
-__global__ void __launch_bounds__(256) k_lev_pairs(SeqSetDev A, SeqSetDev B, const i32* __restrict__ ia,
+template <typename W>
+__global__ void __launch_bounds__(256) k_lev_pairs(const void* __restrict__ slots, i64 n_a, const i32* __restrict__ ia,
                                                    const i32* __restrict__ ib, i64 n, i32* __restrict__ dist) {
     const i64 t = (i64)blockIdx.x * 256 + threadIdx.x;
     if (t >= n) return;
-    const i64 a = ia[t], b = ib[t];
-    const i64 pa = A.off[a], pb = B.off[b];
-    const int la = (int)(A.off[a + 1] - pa), lb = (int)(B.off[b + 1] - pb);
-    const bool narrow = (t & 1) && la <= 32 && lb <= 32;  // exercise both word widths
-    dist[t] = lev_dispatch(A.seqs + pa, la, B.seqs + pb, lb, narrow);
+    dist[t] = myers_lev<W>(load_planes<W>(slots, (u64)ia[t]), load_planes<W>(slots, (u64)(n_a + ib[t])));
 }
 
 }  // namespace
 
 i64 sd_verify_tiles(i64 n) { return (n + VF_THREADS - 1) / VF_THREADS; }
 
-cudaError_t sd_verify(const u64* cand, i64 n_cand, SeqSetDev a, SeqSetDev b, const Layout& lay, int maxlen, u64* surv,
+i64 sd_pack_bytes(i64 n_total, int maxlen) { return n_total * (maxlen <= 32 ? 32 : 48); }
+
+cudaError_t sd_pack(SeqSetDev a, SeqSetDev b, int maxlen, void* slots, cudaStream_t st, i64* launches) {
+    const i64 n = a.n + b.n;
+    if (n == 0) return cudaSuccess;
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    if (maxlen <= 32) k_pack<u32><<<blocks, 256, 0, st>>>(a, b, slots);
+    else k_pack<u64><<<blocks, 256, 0, st>>>(a, b, slots);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t sd_verify(const u64* cand, i64 n_cand, const void* slots, const Layout& lay, int maxlen, u64* surv,
                       u64 surv_base, u64 surv_capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches) {
     const i64 tiles = sd_verify_tiles(n_cand);
     if (tiles == 0) return cudaSuccess;
     cudaError_t e = cudaMemsetAsync(lb_status, 0, (size_t)tiles * 8, st);
     if (e != cudaSuccess) return e;
-    k_verify<<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, a, lay.cross ? b : a, lay, maxlen <= 32 ? 1 : 0, surv,
-                                                     surv_base, surv_capacity, lb_status, info);
+    if (maxlen <= 32)
+        k_verify<u32><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, surv, surv_base, surv_capacity,
+                                                              lb_status, info);
+    else
+        k_verify<u64><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, surv, surv_base, surv_capacity,
+                                                              lb_status, info);
     if (launches) ++*launches;
     return cudaGetLastError();
 }
@@ -202,9 +258,12 @@ cudaError_t sd_finalize(const u64* surv, i64 n_surv, const Layout& lay, int dedu
     return cudaGetLastError();
 }
 
-cudaError_t sd_lev_pairs(SeqSetDev a, SeqSetDev b, const i32* ia, const i32* ib, i64 n_pairs, i32* dist,
+// distances for index pairs (stage test): slots hold set A followed by set B
+cudaError_t sd_lev_pairs(const void* slots, i64 n_a, int maxlen, const i32* ia, const i32* ib, i64 n_pairs, i32* dist,
                          cudaStream_t st) {
     if (n_pairs == 0) return cudaSuccess;
-    k_lev_pairs<<<(unsigned)((n_pairs + 255) / 256), 256, 0, st>>>(a, b, ia, ib, n_pairs, dist);
+    const unsigned blocks = (unsigned)((n_pairs + 255) / 256);
+    if (maxlen <= 32) k_lev_pairs<u32><<<blocks, 256, 0, st>>>(slots, n_a, ia, ib, n_pairs, dist);
+    else k_lev_pairs<u64><<<blocks, 256, 0, st>>>(slots, n_a, ia, ib, n_pairs, dist);
     return cudaGetLastError();
 }

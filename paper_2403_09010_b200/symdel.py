@@ -75,7 +75,7 @@ def lib():
         L.symdel_stage_sort_workspace_bytes.restype = i64
         L.symdel_stage_sort_u64.argtypes = [vp, vp, vp, i64, i32, i32, vp, i64, vp]
         L.symdel_stage_generate.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, i64, C.POINTER(i64), vp, i64, vp]
-        L.symdel_stage_lev.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp]
+        L.symdel_stage_lev.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp]
         _lib = L
     return _lib
 
@@ -227,8 +227,11 @@ class Context:
         torch = _torch()
         dist = torch.empty(ia.numel(), dtype=torch.int32, device=ia.device)
         q = lambda t: C.c_void_p(t.data_ptr())
+        wsb = 1024 + 48 * (a_offsets.numel() + b_offsets.numel())
+        ws = torch.empty(wsb, dtype=torch.uint8, device=ia.device)
         rc = lib().symdel_stage_lev(self._h, q(a_seqs), q(a_offsets), a_offsets.numel() - 1, q(b_seqs), q(b_offsets),
-                                    b_offsets.numel() - 1, q(ia), q(ib), ia.numel(), q(dist), _stream_ptr(torch))
+                                    b_offsets.numel() - 1, q(ia), q(ib), ia.numel(), q(dist), q(ws), wsb,
+                                    _stream_ptr(torch))
         if rc:
             self._raise(rc, "symdel_stage_lev")
         return dist

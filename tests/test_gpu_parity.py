@@ -309,7 +309,7 @@ def test_small_workspace_forces_chunking(torch, sd, ctx, oracle):
     exp = oracle.symdel_self(s.seqs, s.offsets, 2)
     ds, do = sd.to_device(s)
     ws = torch.empty(24 << 20, dtype=torch.uint8, device="cuda")  # ~1/3 of the un-chunked need
-    got = [t.cpu().numpy() for t in ctx.symdel_self(ds, do, 2, workspace=ws)]
+    got = [t.cpu().numpy() for t in ctx.symdel_self(ds, do, 2, workspace=ws, capacity=200_000)]
     assert_same(got, exp)
     assert ctx.symdel_get_stats()["n_chunks"] > 1
 
