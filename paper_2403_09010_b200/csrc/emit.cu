@@ -14,8 +14,9 @@
 //          a query record with nothing.
 // Runs are short on this workload (a run of m records holds m distinct sequences sharing one variant),
 // so each record finds its partners by walking BACKWARDS from its own position while the hash matches
-// (shared memory inside the tile, global memory beyond its start); the walk costs what the pairs it
-// emits cost.  Counts are scanned inside the block, the tile claims its output range with ONE atomic
+// (plain global loads: they hit L1/L2, the tile was just streamed in); the walk costs what the pairs it
+// emits cost.  The kernel keeps no tile in shared memory: one coalesced 8-byte load per record, the
+// left neighbour by warp shuffle.  Counts are scanned inside the block, the tile claims its output range with ONE atomic
 // add (candidate order is irrelevant: they are sorted next) and every record then writes its own
 // pairs.  Only pairs whose flat index lies in [win_lo, win_hi) are written: when the candidate buffer
 // is smaller than the total, the host replays the kernel once per window (later rounds reuse the
@@ -29,7 +30,6 @@ constexpr int EM_THREADS = 256, EM_IPT = 16, EM_TILE = EM_THREADS * EM_IPT;
 __global__ void __launch_bounds__(EM_THREADS) k_emit(const u64* __restrict__ rec, u64 n, Layout lay, u64* __restrict__ cand,
                                                     u64 win_lo, u64 win_hi, int first_round, u64* tile_prefix,
                                                     DevInfo* info) {
-    __shared__ u64 s_rec[EM_TILE + 1];  // s_rec[0] = record before the tile
     __shared__ u64 s_wsum[EM_THREADS / 32];
     __shared__ u64 s_excl;
 
@@ -46,29 +46,33 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(const u64* __restrict__ rec
     const u64 n_a = (u64)lay.n_a;
     const bool cross = lay.cross != 0;
 
-    for (u32 i = tid; i < tile_n; i += EM_THREADS) s_rec[i + 1] = rec[base + i];
-    if (tid == 0) s_rec[0] = base > 0 ? rec[base - 1] : 0ull;
-    __syncthreads();
-
-    auto at = [&](i64 gp) -> u64 { return gp >= base - 1 ? s_rec[gp - base + 1] : rec[gp]; };
-
-    // ---- phase 1: partners per record ----
+    // ---- phase 1: every record and its left neighbour straight from global memory (coalesced; the
+    //      neighbour comes from the lane below).  Only the few records that continue a run walk back. ----
+    u64 me[EM_IPT];
     u32 cnt[EM_IPT];
+#pragma unroll
+    for (int k = 0; k < EM_IPT; ++k) {
+        const u32 pos = k * EM_THREADS + tid;
+        me[k] = pos < tile_n ? rec[base + pos] : 0ull;
+    }
     u64 tsum = 0;
 #pragma unroll
     for (int k = 0; k < EM_IPT; ++k) {
         const u32 pos = k * EM_THREADS + tid;
+        const i64 g = base + pos;
+        u64 prev = __shfl_up_sync(SD_FULL, me[k], 1);
+        if (lane == 0) prev = (pos < tile_n && g > 0) ? rec[g - 1] : 0ull;
         u32 c = 0;
-        if (pos < tile_n) {
-            const u64 me = s_rec[pos + 1];
-            const u64 h = me >> idb;
-            if (!cross || (me & idmask) >= n_a) {  // cross: only reference records collect partners
-                i64 gp = base + pos - 1;
-                while (gp >= 0) {
-                    const u64 x = at(gp);
-                    if ((x >> idb) != h) break;
+        if (pos < tile_n && g > 0) {
+            const u64 h = me[k] >> idb;
+            if ((prev >> idb) == h && (!cross || (me[k] & idmask) >= n_a)) {  // cross: only references collect partners
+                i64 gp = g - 1;
+                u64 x = prev;
+                while (true) {
                     c += (!cross || (x & idmask) < n_a) ? 1u : 0u;  // cross: partners are the run's queries
-                    --gp;
+                    if (--gp < 0) break;
+                    x = rec[gp];
+                    if ((x >> idb) != h) break;
                 }
             }
         }
@@ -91,10 +95,14 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(const u64* __restrict__ rec
         if ((u32)w < warp) carry += c;
         T += c;
     }
+    if (T == 0) {
+        if (first_round && tid == 0) tile_prefix[2 * tile] = 0, tile_prefix[2 * tile + 1] = 0;
+        return;
+    }
     if (tid == 0) {
         u64 excl;
         if (first_round) {
-            excl = T ? (u64)atomicAdd((unsigned long long*)&info->n_cand, (unsigned long long)T) : 0ull;
+            excl = (u64)atomicAdd((unsigned long long*)&info->n_cand, (unsigned long long)T);
             tile_prefix[2 * tile] = excl;
             tile_prefix[2 * tile + 1] = T;
         } else {
@@ -103,29 +111,24 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(const u64* __restrict__ rec
         s_excl = excl;
     }
     __syncthreads();
-    if (T == 0) return;
     u64 flat = s_excl + carry + inc - tsum;  // flat index of this thread's first pair
-    if (flat + tsum <= win_lo || flat >= win_hi) return;
+    if (tsum == 0 || flat + tsum <= win_lo || flat >= win_hi) return;
 
     // ---- phase 2: every record writes its own pairs ----
 #pragma unroll
     for (int k = 0; k < EM_IPT; ++k) {
-        if (cnt[k] == 0) continue;
-        const u32 pos = k * EM_THREADS + tid;
-        const u64 me = s_rec[pos + 1];
-        const u64 h = me >> idb;
-        const u64 b_id = cross ? (me & idmask) - n_a : (me & idmask);
-        i64 gp = base + pos - 1;
         u32 left = cnt[k];
+        if (left == 0) continue;
+        const u64 b_id = cross ? (me[k] & idmask) - n_a : (me[k] & idmask);
+        i64 gp = base + (i64)(k * EM_THREADS + tid) - 1;
         while (left) {
-            const u64 x = at(gp);
+            const u64 x = rec[gp];
             --gp;
             if (cross && (x & idmask) >= n_a) continue;  // a reference record of the same run
             if (flat >= win_lo && flat < win_hi) cand[flat - win_lo] = ((x & idmask) << lay.b_bits) | b_id;
             ++flat;
             --left;
         }
-        (void)h;
     }
 }
 

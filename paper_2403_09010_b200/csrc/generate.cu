@@ -378,7 +378,30 @@ struct Gen2Shared {
     unsigned char map[G2_NW][32];
 };
 
-template <bool COUNT_ONLY>
+// One emission round of the fast path: lanes with `valid` append (hash, id) to their sequence's
+// record range (rank by ballot inside the sequence's lane segment) and count the key's digits.
+template <bool COUNT_ONLY, bool CHUNKED, int NPASS>
+__device__ __forceinline__ void g2_emit(bool valid, u64 h, const GenParams& P, u32 segmask, u32 lane_lt, u64 gid,
+                                        int kshift, u64*& out, u32& run, u32* s_hist) {
+    if (CHUNKED) valid = valid && gen_chunk_of(h, P.n_chunks) == P.chunk;
+    const u32 bal = __ballot_sync(SD_FULL, valid) & segmask;
+    if (!COUNT_ONLY) {
+        if (valid) {
+            const u64 key = h >> kshift;
+            out[__popc(bal & lane_lt)] = (key << P.id_bits) | gid;
+            if (NPASS > 0) {
+#pragma unroll
+                for (int ps = 0; ps < NPASS; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
+            } else {
+                for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
+            }
+        }
+        out += __popc(bal);
+    }
+    run += __popc(bal);
+}
+
+template <bool COUNT_ONLY, bool CHUNKED, int NPASS>
 __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
     extern __shared__ __align__(16) unsigned char gen_smem[];
     Gen2Shared& sh = *reinterpret_cast<Gen2Shared*>(gen_smem);
@@ -392,9 +415,10 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
     __syncthreads();
     const int d = P.d;
     const bool thinning = P.thinning != 0;
-    const bool chunked = P.n_chunks > 1;
     const u64 binv1 = c_Binv[1], binv2 = c_Binv[2];
     const int kshift = 64 - P.hash_bits;
+    u64* const Uw = sh.U[warp];
+    u64* const Vw = sh.V[warp];
 
     // warp task = 32 consecutive sequences of one set; groups_* count warp tasks here
     for (i64 wt = (i64)blockIdx.x * G2_NW + warp; wt < P.groups_total; wt += (i64)gridDim.x * G2_NW) {
@@ -430,7 +454,7 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
             // ---- empty sequences: one record (the empty variant) each ----
             if (mine && Li == 0) {
                 const u64 h = K_LEN;  // A[L] = 0, (L + 1) * K
-                const bool ok = !chunked || gen_chunk_of(h, P.n_chunks) == P.chunk;
+                const bool ok = !CHUNKED || gen_chunk_of(h, P.n_chunks) == P.chunk;
                 if (COUNT_ONLY) {
                     P.cnt[gid0 + lane] = ok ? 1u : 0u;
                 } else if (ok) {
@@ -448,7 +472,8 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
                 const bool active = lane < total;
                 const u32 seg_start = active ? (31u - __clz(heads & (0xffffffffu >> (31u - lane)))) : 0u;
                 const u32 si = active ? sh.map[warp][seg_start] : 0u;  // sequence index within the task
-                const u32 L = __shfl_sync(SD_FULL, Li, si);
+                const u32 Lsrc = __shfl_sync(SD_FULL, Li, si);
+                const u32 L = active ? Lsrc : 0u;  // idle lanes: L = 0 switches every later predicate off
                 const u64 rec_base = __shfl_sync(SD_FULL, rec_base_i, si);
                 const u32 a = lane - seg_start;
                 const u64 gid = gid0 + si;
@@ -461,7 +486,7 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
                 const u32 m1 = __ballot_sync(SD_FULL, canon1), madj = __ballot_sync(SD_FULL, adjok);
 
                 u32 run = 0;  // records of this lane's sequence so far (uniform inside a segment)
-                if (COUNT_ONLY && !chunked) {
+                if (COUNT_ONLY && !CHUNKED) {
                     const u32 B = __popc(m1 & segmask);
                     run = 1;
                     if (d >= 1) run += B;
@@ -481,41 +506,32 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
                     const u64 aexcl = aincl - term;
                     const u64 AL = __shfl_sync(SD_FULL, aincl, active ? seg_start + L - 1 : 0);
                     const u64 Uv = aexcl - binv1 * aincl;
-                    sh.U[warp][lane] = Uv;
-                    sh.V[warp][lane] = binv1 * Uv;
+                    Uw[lane] = Uv;
+                    Vw[lane] = binv1 * Uv;
                     __syncwarp();
                     const u64 C0 = AL + (u64)(L + 1) * K_LEN;
                     const u64 C1 = binv1 * AL + (u64)L * K_LEN;
                     const u64 C2 = binv2 * AL + (u64)(L - 1) * K_LEN;
+                    u64* out = P.records + rec_base;
 
-                    auto emit = [&](bool valid, u64 h) {
-                        if (chunked) valid = valid && gen_chunk_of(h, P.n_chunks) == P.chunk;
-                        const u32 bal = __ballot_sync(SD_FULL, valid) & segmask;
-                        if (!COUNT_ONLY && valid) {
-                            const u64 key = h >> kshift;
-                            P.records[rec_base + run + __popc(bal & lane_lt)] = (key << P.id_bits) | gid;
-                            for (int ps = 0; ps < P.npass; ++ps)
-                                atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
-                        }
-                        run += __popc(bal);
-                    };
-                    emit(active && a == 0, C0);
-                    if (d >= 1) emit(canon1, Uv + C1);
+                    g2_emit<COUNT_ONLY, CHUNKED, NPASS>(active && a == 0, C0, P, segmask, lane_lt, gid, kshift, out, run, s_hist);
+                    if (d >= 1)
+                        g2_emit<COUNT_ONLY, CHUNKED, NPASS>(canon1, Uv + C1, P, segmask, lane_lt, gid, kshift, out, run, s_hist);
                     if (d >= 2) {
-                        const u32 half = __reduce_max_sync(SD_FULL, active ? (L >> 1) : 0u);
+                        const u32 half = __reduce_max_sync(SD_FULL, L >> 1);
+                        const u32 m1s = m1 >> seg_start, madjs = madj >> seg_start;  // segment-relative masks
+                        const u64* const Us = Uw + seg_start;
+                        const u64* const Vs = Vw + seg_start;
                         for (u32 dl = 1; dl <= half; ++dl) {
-                            const bool on = active && (2 * dl < L || (2 * dl == L && a < dl));
                             u32 b = a + dl;
-                            if (b >= L) b -= L;
-                            bool canon = false;
-                            u64 h = 0;
-                            if (on) {
-                                const u32 p1 = min(a, b), p2 = max(a, b);
-                                const u32 l1 = seg_start + p1, l2 = seg_start + p2;
-                                canon = (p2 - p1 == 1u) ? ((madj >> l1) & 1u) : (((m1 >> l1) & (m1 >> l2)) & 1u);
-                                h = sh.U[warp][l1] + sh.V[warp][l2] + C2;
-                            }
-                            emit(canon, h);
+                            b = (b >= L) ? b - L : b;
+                            const u32 p1 = min(a, b) & 31u, p2 = max(a, b) & 31u;
+                            const bool on = (2 * dl < L) || (2 * dl == L && a < dl);  // false on idle lanes (L = 0)
+                            const u32 both = (m1s >> p1) & (m1s >> p2);
+                            const u32 t = (p2 - p1 == 1u) ? (madjs >> p1) : both;
+                            const u64 h = Us[p1] + Vs[p2] + C2;
+                            g2_emit<COUNT_ONLY, CHUNKED, NPASS>(on && (t & 1u), h, P, segmask, lane_lt, gid, kshift, out, run,
+                                                                s_hist);
                         }
                     }
                     __syncwarp();  // U/V/map are reused by the next batch
@@ -532,6 +548,19 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
         __syncthreads();
         for (int i = tid; i < P.npass * 256; i += G2_THREADS)
             if (s_hist[i]) atomicAdd(&P.ghist[i], s_hist[i]);
+    }
+}
+
+typedef void (*Gen2Kernel)(GenParams);
+template <bool COUNT_ONLY>
+Gen2Kernel gen2_pick(bool chunked, int npass) {
+    if (chunked) return k_gen2<COUNT_ONLY, true, 0>;
+    if (COUNT_ONLY) return k_gen2<COUNT_ONLY, false, 0>;
+    switch (npass) {
+        case 3: return k_gen2<COUNT_ONLY, false, 3>;
+        case 4: return k_gen2<COUNT_ONLY, false, 4>;
+        case 5: return k_gen2<COUNT_ONLY, false, 5>;
+        default: return k_gen2<COUNT_ONLY, false, 0>;
     }
 }
 
@@ -614,9 +643,7 @@ cudaError_t sd_init_tables() {
     if ((e = cudaFuncSetAttribute(k_generate<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)sizeof(GenShared))) != cudaSuccess)
         return e;
-    if ((e = cudaFuncSetAttribute(k_gen2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)(sizeof(Gen2Shared) + 8 * 256 * 4))) != cudaSuccess)
-        return e;
+
     done = true;
     return cudaSuccess;
 }
@@ -636,7 +663,7 @@ cudaError_t sd_count(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u32
     if (P.groups_total == 0) return cudaSuccess;
     P.cnt = cnt;
     P.info = info;
-    if (fast) k_gen2<true><<<gen2_grid(P.groups_total), G2_THREADS, sizeof(Gen2Shared), st>>>(P);
+    if (fast) gen2_pick<true>(lay.n_chunks > 1, 0)<<<gen2_grid(P.groups_total), G2_THREADS, sizeof(Gen2Shared), st>>>(P);
     else k_generate<true><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared), st>>>(P);
     if (launches) ++*launches;
     return cudaGetLastError();
@@ -665,7 +692,8 @@ cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     P.npass = npass;
     P.info = info;
     if (fast)
-        k_gen2<false><<<gen2_grid(P.groups_total), G2_THREADS, sizeof(Gen2Shared) + (size_t)npass * 256 * 4, st>>>(P);
+        gen2_pick<false>(lay.n_chunks > 1, npass)<<<gen2_grid(P.groups_total), G2_THREADS,
+                                                      sizeof(Gen2Shared) + (size_t)npass * 256 * 4, st>>>(P);
     else
         k_generate<false><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared) + (size_t)npass * 256 * 4, st>>>(P);
     if (launches) ++*launches;
