@@ -47,37 +47,30 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(const u64* __restrict__ rec
     const bool cross = lay.cross != 0;
 
     // ---- phase 1: every record and its left neighbour straight from global memory (coalesced; the
-    //      neighbour comes from the lane below).  Only the few records that continue a run walk back. ----
-    u64 me[EM_IPT];
-    u32 cnt[EM_IPT];
+    //      neighbour comes from the lane below).  `cont` marks the few records that continue a run;
+    //      only those walk back, in a compact loop (keeps the unrolled part tiny). ----
+    const u64 hlim = 1ull << idb;  // same hash <=> (x ^ y) < 2^id_bits
+    u32 cont = 0;
 #pragma unroll
     for (int k = 0; k < EM_IPT; ++k) {
         const u32 pos = k * EM_THREADS + tid;
-        me[k] = pos < tile_n ? rec[base + pos] : 0ull;
+        const u64 me = pos < tile_n ? rec[base + pos] : ~0ull;
+        u64 prev = __shfl_up_sync(SD_FULL, me, 1);
+        if (lane == 0) prev = (pos < tile_n && base + pos > 0) ? rec[base + pos - 1] : ~me;
+        const bool same = pos < tile_n && ((me ^ prev) < hlim) && (!cross || (me & idmask) >= n_a);
+        cont |= (same ? 1u : 0u) << k;
     }
     u64 tsum = 0;
-#pragma unroll
-    for (int k = 0; k < EM_IPT; ++k) {
-        const u32 pos = k * EM_THREADS + tid;
-        const i64 g = base + pos;
-        u64 prev = __shfl_up_sync(SD_FULL, me[k], 1);
-        if (lane == 0) prev = (pos < tile_n && g > 0) ? rec[g - 1] : 0ull;
-        u32 c = 0;
-        if (pos < tile_n && g > 0) {
-            const u64 h = me[k] >> idb;
-            if ((prev >> idb) == h && (!cross || (me[k] & idmask) >= n_a)) {  // cross: only references collect partners
-                i64 gp = g - 1;
-                u64 x = prev;
-                while (true) {
-                    c += (!cross || (x & idmask) < n_a) ? 1u : 0u;  // cross: partners are the run's queries
-                    if (--gp < 0) break;
-                    x = rec[gp];
-                    if ((x >> idb) != h) break;
-                }
-            }
+    for (u32 m = cont; m; m &= m - 1) {
+        const i64 g = base + (i64)((__ffs(m) - 1) * EM_THREADS + tid);
+        const u64 me = rec[g];
+        i64 gp = g - 1;
+        while (gp >= 0) {
+            const u64 x = rec[gp];
+            if ((x ^ me) >= hlim) break;
+            tsum += (!cross || (x & idmask) < n_a) ? 1u : 0u;  // cross: partners are the run's queries
+            --gp;
         }
-        cnt[k] = c;
-        tsum += c;
     }
     // ---- block exclusive scan of the per-thread totals ----
     u64 inc = tsum;
@@ -114,20 +107,19 @@ __global__ void __launch_bounds__(EM_THREADS) k_emit(const u64* __restrict__ rec
     u64 flat = s_excl + carry + inc - tsum;  // flat index of this thread's first pair
     if (tsum == 0 || flat + tsum <= win_lo || flat >= win_hi) return;
 
-    // ---- phase 2: every record writes its own pairs ----
-#pragma unroll
-    for (int k = 0; k < EM_IPT; ++k) {
-        u32 left = cnt[k];
-        if (left == 0) continue;
-        const u64 b_id = cross ? (me[k] & idmask) - n_a : (me[k] & idmask);
-        i64 gp = base + (i64)(k * EM_THREADS + tid) - 1;
-        while (left) {
+    // ---- phase 2: every run-continuing record writes its own pairs (same walk) ----
+    for (u32 m = cont; m; m &= m - 1) {
+        const i64 g = base + (i64)((__ffs(m) - 1) * EM_THREADS + tid);
+        const u64 me = rec[g];
+        const u64 b_id = cross ? (me & idmask) - n_a : (me & idmask);
+        i64 gp = g - 1;
+        while (gp >= 0) {
             const u64 x = rec[gp];
+            if ((x ^ me) >= hlim) break;
             --gp;
             if (cross && (x & idmask) >= n_a) continue;  // a reference record of the same run
             if (flat >= win_lo && flat < win_hi) cand[flat - win_lo] = ((x & idmask) << lay.b_bits) | b_id;
             ++flat;
-            --left;
         }
     }
 }

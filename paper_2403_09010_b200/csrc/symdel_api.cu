@@ -88,7 +88,7 @@ i64 rec_bytes(i64 ncap, int npass) {
     return 2 * align_up(ncap * 8) + align_up(sd_sort_scratch_bytes(ncap, npass)) + align_up((2 * sd_emit_tiles(ncap) + 2) * 8);
 }
 i64 cand_bytes(i64 ccap, int ppass) {
-    return 2 * align_up(ccap * 8) + align_up(sd_sort_scratch_bytes(ccap, ppass)) + align_up((sd_verify_tiles(ccap) + 1) * 8);
+    return 2 * align_up(ccap * 8) + align_up(sd_sort_scratch_bytes(ccap, ppass)) + align_up((ccap / 256 + 2) * 8);
 }
 i64 fixed_bytes(i64 n_total) {
     return align_up((i64)sizeof(DevInfo)) + align_up(n_total * 4) + align_up((n_total + 1) * 8) +
@@ -238,11 +238,11 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     u64* candA = ws.take<u64>(ccap);
     u64* candB = ws.take<u64>(ccap);
     void* cand_scratch = ws.take<char>(sd_sort_scratch_bytes(ccap, ppass));
-    u64* verify_lb = ws.take<u64>(sd_verify_tiles(ccap) + 1);
+    u64* verify_lb = ws.take<u64>(ccap / 256 + 2);
     u64* survA = ws.take<u64>(scap);
     u64* survB = ws.take<u64>(scap);
     void* surv_scratch = ws.take<char>(sd_sort_scratch_bytes(scap, spass));
-    u64* final_lb = ws.take<u64>(sd_verify_tiles(scap) + 1);
+    u64* final_lb = ws.take<u64>(scap / 256 + 2);
     if (!ws.ok) return SYMDEL_E_WORKSPACE;
 
     const int width = maxlen + 1;

@@ -108,44 +108,76 @@ __device__ __forceinline__ int myers_lev(const Planes<W>& P, const Planes<W>& T)
     return score;
 }
 
-constexpr int VF_THREADS = 256;
+constexpr int VF_THREADS = 256, VF_IPT = 4, VF_TILE = VF_THREADS * VF_IPT;
 
+// Tile of 1024 sorted candidates: (1) flag the unique ones and compact their positions into shared
+// memory, (2) spread the COMPACTED list over the threads for the distance computation (after dedup
+// only a fraction of the candidates is left: this keeps every lane busy), (3) ordered compaction of
+// the survivors (block scan + 32-wide decoupled look-back) so the output stays sorted.
 template <typename W>
 __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ cand, u64 n, const void* __restrict__ slots,
                                                       Layout lay, u64* __restrict__ surv, u64 surv_base,
                                                       u64 surv_capacity, u64* lb_status, DevInfo* info) {
+    __shared__ unsigned short s_list[VF_TILE];
+    __shared__ unsigned char s_res[VF_TILE];
     __shared__ u32 s_warp[VF_THREADS / 32 + 1];
-    __shared__ u32 s_tile;
+    __shared__ u32 s_tile, s_nuniq;
     __shared__ u64 s_excl;
-    const u32 tid = threadIdx.x;
+    const u32 tid = threadIdx.x, lane = tid & 31;
     if (tid == 0) {
         s_tile = atomicAdd(&info->ticket[SD_TK_VERIFY], 1u);
         if (s_tile == gridDim.x - 1) info->ticket[SD_TK_VERIFY] = 0;
+        s_nuniq = 0;
     }
     __syncthreads();
     const u32 tile = s_tile;
-    const u64 t = (u64)tile * VF_THREADS + tid;
-    bool uniq = false, keep = false;
-    u64 c = 0;
-    int dist = 0;
-    if (t < n) {
-        c = cand[t];
-        uniq = (t == 0) || (cand[t - 1] != c);
-        const u64 a = c >> lay.b_bits, b = c & ((1ull << lay.b_bits) - 1ull);
-        if (!lay.cross && a == b) uniq = false;  // same sequence twice in one run (hash collision / no thinning)
-        if (uniq) {
-            const Planes<W> pa = load_planes<W>(slots, a);
-            const Planes<W> pb = load_planes<W>(slots, lay.cross ? (u64)lay.n_a + b : b);
-            const int dl = pa.len > pb.len ? pa.len - pb.len : pb.len - pa.len;
-            if (dl <= lay.d) {
-                dist = myers_lev<W>(pa, pb);
-                keep = dist <= lay.d;
-            }
+    const u64 base = (u64)tile * VF_TILE;
+    const u32 tile_n = (u32)min((u64)VF_TILE, n - base);
+    const u64 bmask = (1ull << lay.b_bits) - 1ull;
+
+    // ---- (1) unique flags, compacted positions ----
+#pragma unroll
+    for (int k = 0; k < VF_IPT; ++k) {
+        const u32 pos = k * VF_THREADS + tid;
+        const u64 c = pos < tile_n ? cand[base + pos] : 0ull;
+        u64 prev = __shfl_up_sync(SD_FULL, c, 1);
+        if (lane == 0) prev = (pos < tile_n && base + pos > 0) ? cand[base + pos - 1] : ~c;
+        bool uniq = pos < tile_n && c != prev;
+        if (!lay.cross && (c >> lay.b_bits) == (c & bmask)) uniq = false;  // same sequence twice in one run
+        const u32 bal = __ballot_sync(SD_FULL, uniq);
+        u32 wbase = 0;
+        if (lane == 0 && bal) wbase = atomicAdd(&s_nuniq, (u32)__popc(bal));
+        wbase = __shfl_sync(SD_FULL, wbase, 0);
+        if (uniq) s_list[wbase + __popc(bal & ((1u << lane) - 1u))] = (unsigned short)pos;
+        if (pos < VF_TILE) s_res[pos] = 0xff;
+    }
+    __syncthreads();
+    const u32 nuniq = s_nuniq;
+
+    // ---- (2) distances over the compacted list ----
+    for (u32 e = tid; e < nuniq; e += VF_THREADS) {
+        const u32 pos = s_list[e];
+        const u64 c = cand[base + pos];
+        const u64 a = c >> lay.b_bits, b = c & bmask;
+        const Planes<W> pa = load_planes<W>(slots, a);
+        const Planes<W> pb = load_planes<W>(slots, lay.cross ? (u64)lay.n_a + b : b);
+        const int dl = pa.len > pb.len ? pa.len - pb.len : pb.len - pa.len;
+        if (dl <= lay.d) {
+            const int dist = myers_lev<W>(pa, pb);
+            if (dist <= lay.d) s_res[pos] = (unsigned char)dist;
         }
     }
+    __syncthreads();
+
+    // ---- (3) ordered compaction (thread owns VF_IPT consecutive positions) ----
+    u32 keepmask = 0, cntk = 0;
+#pragma unroll
+    for (int k = 0; k < VF_IPT; ++k) {
+        const u32 pos = tid * VF_IPT + k;
+        if (s_res[pos] != 0xff) keepmask |= 1u << k, ++cntk;
+    }
     u32 total;
-    const u32 rank = sd_block_excl_sum<VF_THREADS>(keep ? 1u : 0u, &total, s_warp);
-    const u32 nuniq = __syncthreads_count(uniq);
+    const u32 rank = sd_block_excl_sum<VF_THREADS>(cntk, &total, s_warp);
     if (tid < 32) {
         const u64 excl = sd_lookback_warp(lb_status, tile, total);
         if (tid == 0) {
@@ -155,10 +187,15 @@ __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ c
         }
     }
     __syncthreads();
-    if (keep) {
-        const u64 pos = surv_base + s_excl + rank;
-        if (pos < surv_capacity) surv[pos] = (c << 3) | (u64)dist;
-        else atomicOr(&info->err, (u32)SD_ERR_OVERFLOW);
+    u64 out = surv_base + s_excl + rank;
+#pragma unroll
+    for (int k = 0; k < VF_IPT; ++k) {
+        if (keepmask & (1u << k)) {
+            const u32 pos = tid * VF_IPT + k;
+            if (out < surv_capacity) surv[out] = (cand[base + pos] << 3) | (u64)s_res[pos];
+            else atomicOr(&info->err, (u32)SD_ERR_OVERFLOW);
+            ++out;
+        }
     }
 }
 
@@ -216,7 +253,7 @@ __global__ void __launch_bounds__(256) k_lev_pairs(const void* __restrict__ slot
 
 }  // namespace
 
-i64 sd_verify_tiles(i64 n) { return (n + VF_THREADS - 1) / VF_THREADS; }
+i64 sd_verify_tiles(i64 n) { return (n + VF_TILE - 1) / VF_TILE; }
 
 i64 sd_pack_bytes(i64 n_total, int maxlen) { return n_total * (maxlen <= 32 ? 32 : 48); }
 
