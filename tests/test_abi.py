@@ -93,13 +93,12 @@ def test_no_gpu_fails_loudly(lib):
 
 
 def test_product_never_touches_the_oracle():
+    """Neither side imports, includes or loads the other (shared: only the input generator)."""
+    bad = ("import", "#include", "CDLL", "dlopen", "LoadLibrary")
     for p in list((ROOT / "paper_2403_09010_b200").rglob("*.py")) + list((ROOT / "paper_2403_09010_b200" / "csrc").glob("*")):
-        txt = p.read_text(errors="ignore")
-        assert "oracle" not in txt.replace("no CPU oracle", "").replace("oracle/", "ORACLE_DIR_MENTION") or all(
-            "import" not in ln and "#include" not in ln and "dlopen" not in ln and "CDLL" not in ln
-            for ln in txt.splitlines() if "oracle" in ln), p
+        for ln in p.read_text(errors="ignore").splitlines():
+            assert not ("oracle" in ln and any(b in ln for b in bad)), (p, ln)
     for p in (ROOT / "oracle").glob("*"):
         if p.suffix in (".py", ".cpp"):
-            txt = p.read_text()
-            assert "symdel.h" not in txt and "libsymdel" not in txt and "csrc" not in txt.replace("csrc/", "CSRC_MENTION") or True
-            assert "import paper_2403_09010_b200" not in txt and "from paper_2403_09010_b200" not in txt
+            for ln in p.read_text().splitlines():
+                assert not (("symdel" in ln or "paper_2403_09010_b200" in ln or "csrc" in ln) and any(b in ln for b in bad)), (p, ln)
