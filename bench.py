@@ -185,9 +185,9 @@ def main():
     dev = torch.device("cuda", local)
     seqs_d = torch.from_numpy(s.seqs).to(dev)
     offs_d = torch.from_numpy(s.offsets).to(dev)
-    ws_bytes = symdel.symdel_workspace_bytes(s.n, s.seqs.size, 0, 0, int(s.lengths.max()), d)
-    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
     cap = 4 << 20
+    ws_bytes = symdel.symdel_workspace_bytes(s.n, s.seqs.size, 0, 0, int(s.lengths.max()), d, cap)
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
     out = tuple(torch.empty(cap, dtype=torch.int32, device=dev) for _ in range(3))
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
     # host buffers of the end-to-end arm (pinned)

@@ -97,10 +97,11 @@ SYMDEL_API int symdel_last_cuda_error(const symdel_ctx* ctx); /* cudaError_t of 
 SYMDEL_API const char* symdel_strerror(int code);             /* static string */
 
 /* Recommended workspace size for an un-chunked run.  n_b = 0 and residues_b = 0 for self-search.
- * max_len = longest sequence (<= SYMDEL_L_MAX).  Any workspace >= the minimum the library needs
- * works: a smaller one makes symdel_* split the key space into chunks (S5).  Pure host arithmetic. */
+ * max_len = longest sequence (<= SYMDEL_L_MAX); capacity = the output capacity that will be passed.
+ * Any workspace >= the minimum the library needs works: a smaller one makes symdel_* split the key
+ * space into chunks (S5).  Pure host arithmetic. */
 SYMDEL_API int symdel_workspace_bytes(int64_t n_a, int64_t residues_a, int64_t n_b, int64_t residues_b, int max_len, int d,
-                           int64_t* bytes_host);
+                           int64_t capacity, int64_t* bytes_host);
 
 /* ---- the hot path, device-resident inputs and outputs ---------------------------------------
  * out_i/out_j/out_dist: caller-owned device arrays of `capacity` int32 each.

@@ -37,7 +37,7 @@ constexpr u64 K_LEN = 0x9fb21c651e98df25ull;
 __device__ __forceinline__ u32 gen_chunk_of(u64 h, u32 n_chunks) { return __umulhi((u32)h * 0x9e3779b1u, n_chunks); }
 
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, DevInfo* info) {
+__global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, DevInfo* info) {
     u64 nmax = 0;
     u32 maxlen = 0, err = 0;
     const i64 stride = (i64)gridDim.x * blockDim.x;
@@ -66,6 +66,7 @@ __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, DevInfo* in
     }
     if ((threadIdx.x & 31) == 0) {
         if (nmax) atomicAdd((unsigned long long*)&info->nmax, (unsigned long long)nmax);
+        if (nmax && is_b) atomicAdd((unsigned long long*)&info->nmax_b, (unsigned long long)nmax);
         if (maxlen) atomicMax(&info->maxlen, maxlen);
         if (err) atomicOr(&info->err, err);
     }
@@ -648,10 +649,10 @@ cudaError_t sd_init_tables() {
     return cudaSuccess;
 }
 
-cudaError_t sd_prepare(SeqSetDev s, int d, DevInfo* info, cudaStream_t st, i64* launches) {
+cudaError_t sd_prepare(SeqSetDev s, int d, int is_b, DevInfo* info, cudaStream_t st, i64* launches) {
     if (s.n == 0) return cudaSuccess;
     int blocks = (int)std::min<i64>((s.n + 255) / 256, 148 * 8);
-    k_prepare<<<blocks, 256, 0, st>>>(s, d, info);
+    k_prepare<<<blocks, 256, 0, st>>>(s, d, is_b, info);
     if (launches) ++*launches;
     return cudaGetLastError();
 }

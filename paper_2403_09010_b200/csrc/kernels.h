@@ -45,7 +45,7 @@ cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass,
 
 // ---- generate.cu --------------------------------------------------------------------------------
 cudaError_t sd_init_tables();  // fills the __constant__ tables once per process
-cudaError_t sd_prepare(SeqSetDev s, int d, DevInfo* info, cudaStream_t st, i64* launches);
+cudaError_t sd_prepare(SeqSetDev s, int d, int is_b, DevInfo* info, cudaStream_t st, i64* launches);
 // count pass: cnt[gid] = number of records sequence gid contributes (u32 per sequence)
 cudaError_t sd_count(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u32* cnt, DevInfo* info, cudaStream_t st,
                      i64* launches);

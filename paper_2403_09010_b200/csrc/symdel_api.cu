@@ -16,6 +16,7 @@
 //
 // Host <-> device crossings per call: one pinned-memory read-back after S0, one per chunk after the
 // count scan (grid sizes), one after the first emit (candidate count), two at the end.
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <vector>
@@ -168,8 +169,8 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
 
     // ---- S0 ----
     CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
-    CK(sd_prepare(A, d, info, st, &S.n_launches));
-    if (cross) CK(sd_prepare(B, d, info, st, &S.n_launches));
+    CK(sd_prepare(A, d, 0, info, st, &S.n_launches));
+    if (cross) CK(sd_prepare(B, d, 1, info, st, &S.n_launches));
     int rc = read_info(ctx, info, st);
     if (rc) return rc;
     if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
@@ -190,8 +191,16 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     {
         int hb = (int)ctx->opt_hash_bits;
         if (hb == 0) {
-            hb = bits_for(std::max<i64>(nmax, 2)) + 5;
-            hb = std::max(16, (hb + 7) / 8 * 8);
+            // Key width: every 8 bits cost one more pass over all records (16 B/record); too few bits
+            // cost spurious candidates (~n_x * n_y / 2^bits colliding pairs, ~150 B of traffic each
+            // through emit, pair sort and verify).  Pick the cheapest width.
+            const double nb = (double)ctx->h_info->nmax_b, na = (double)nmax - nb;
+            double best = 0;
+            for (int h = 16; h <= 56; h += 8) {
+                const double pairs = (cross ? na * nb : 0.5 * na * na) / std::pow(2.0, h);
+                const double cost = (double)nmax * 16.0 * (h / 8) + pairs * 150.0;
+                if (hb == 0 || cost < best) best = cost, hb = h;
+            }
         }
         const int hb_max = (64 - lay.id_bits) / 8 * 8;
         if (hb % 8 != 0 || hb < 8) return SYMDEL_E_ARG;
@@ -217,7 +226,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     if (P > 1) ncap = std::min<i64>(nmax, nmax / P + nmax / (4 * P) + 4096);
     if (rec_bytes(ncap, npass) + cand_bytes(ccap, ppass) + cand_bytes(scap, spass) > R) {
         if (ctx->opt_cand_cap <= 0) ccap = std::min<i64>(ccap, std::max<i64>(4096, R / 4 / 17));
-        scap = std::min<i64>(scap, std::max<i64>(4096 + capacity, R * 15 / 100 / 17));
+        scap = std::min<i64>(scap, std::max<i64>(4096, R * 15 / 100 / 17));
         const i64 rrem = R - cand_bytes(ccap, ppass) - cand_bytes(scap, spass);
         if (rrem <= 0) return SYMDEL_E_WORKSPACE;
         // largest ncap that fits in rrem (16 B/record + ~0.26 B/record of tile status per pass)
@@ -521,15 +530,15 @@ const char* symdel_strerror(int code) {
 }
 
 int symdel_workspace_bytes(int64_t n_a, int64_t residues_a, int64_t n_b, int64_t residues_b, int max_len, int d,
-                           int64_t* bytes_host) {
+                           int64_t capacity, int64_t* bytes_host) {
     if (!bytes_host || n_a < 0 || n_b < 0 || residues_a < 0 || residues_b < 0 || d < 0 || d > SD_D_MAX || max_len < 0 ||
-        max_len > SD_L_MAX)
+        max_len > SD_L_MAX || capacity < 0)
         return SYMDEL_E_ARG;
     // V(L, d) <= 1 + L * (V(max_len, d) - 1) / max_len for L <= max_len
     const i64 n_total = n_a + n_b;
     const u64 vm = vcount_host(max_len, d);
     const i64 nbound = n_total + (max_len ? (i64)(((u64)(residues_a + residues_b) * (vm - 1) + max_len - 1) / max_len) : 0);
-    const i64 ccap = std::max<i64>(1 << 20, nbound / 2), scap = std::max<i64>(1 << 20, nbound / 4);
+    const i64 ccap = std::max<i64>(1 << 20, nbound / 2), scap = std::max<i64>(std::max<i64>(1 << 20, nbound / 4), capacity);
     *bytes_host = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nbound, 1), 7) + cand_bytes(ccap, 8) + cand_bytes(scap, 8) +
                   65536;
     return SYMDEL_OK;
@@ -611,7 +620,7 @@ int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const int64_t* of
     SeqSetDev A{seqs, offsets, n}, B{nullptr, nullptr, 0};
     CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
     CK(cudaMemsetAsync(hist, 0, 8 * 256 * 4, st));
-    CK(sd_prepare(A, d, info, st, nullptr));
+    CK(sd_prepare(A, d, 0, info, st, nullptr));
     int rc = read_info(ctx, info, st);
     if (rc) return rc;
     if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
@@ -652,8 +661,8 @@ int symdel_stage_lev(symdel_ctx* ctx, const int8_t* a_seqs, const int64_t* a_off
     void* slots = ws.take<char>(sd_pack_bytes(n_a + n_b, SD_L_MAX));
     if (!ws.ok) return SYMDEL_E_WORKSPACE;
     CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
-    CK(sd_prepare(A, 0, info, st, nullptr));
-    CK(sd_prepare(B, 0, info, st, nullptr));
+    CK(sd_prepare(A, 0, 0, info, st, nullptr));
+    CK(sd_prepare(B, 0, 1, info, st, nullptr));
     int rc = read_info(ctx, info, st);
     if (rc) return rc;
     if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);

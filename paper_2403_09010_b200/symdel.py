@@ -66,7 +66,7 @@ def lib():
         L.symdel_last_cuda_error.argtypes = [vp]
         L.symdel_strerror.argtypes = [i32]
         L.symdel_strerror.restype = C.c_char_p
-        L.symdel_workspace_bytes.argtypes = [i64, i64, i64, i64, i32, i32, C.POINTER(i64)]
+        L.symdel_workspace_bytes.argtypes = [i64, i64, i64, i64, i32, i32, i64, C.POINTER(i64)]
         L.symdel_self.argtypes = [vp, vp, vp, i64, i32, vp, i64, vp, vp, vp, i64, C.POINTER(i64), vp]
         L.symdel_cross.argtypes = [vp, vp, vp, i64, vp, vp, i64, i32, vp, i64, vp, vp, vp, i64, C.POINTER(i64), vp]
         L.symdel_self_host.argtypes = [vp, vp, vp, i64, i32, vp, vp, vp, i64, C.POINTER(i64)]
@@ -80,9 +80,9 @@ def lib():
     return _lib
 
 
-def symdel_workspace_bytes(n_a, residues_a, n_b=0, residues_b=0, max_len=L_MAX, d=2) -> int:
+def symdel_workspace_bytes(n_a, residues_a, n_b=0, residues_b=0, max_len=L_MAX, d=2, capacity=0) -> int:
     out = C.c_int64(0)
-    rc = lib().symdel_workspace_bytes(n_a, residues_a, n_b, residues_b, max_len, d, C.byref(out))
+    rc = lib().symdel_workspace_bytes(n_a, residues_a, n_b, residues_b, max_len, d, capacity, C.byref(out))
     if rc:
         raise SymdelError(rc, "symdel_workspace_bytes")
     return int(out.value)
@@ -151,13 +151,13 @@ class Context:
         cross = b_off is not None
         n_a = a_off.numel() - 1
         n_b = b_off.numel() - 1 if cross else 0
-        if workspace is None:
-            nbytes = symdel_workspace_bytes(n_a, a_seqs.numel(), n_b, b_seqs.numel() if cross else 0, L_MAX, d)
-            workspace = torch.empty(nbytes, dtype=torch.uint8, device=a_off.device)
         if out is None:
             cap = capacity if capacity is not None else max(1 << 20, 4 * (n_a + n_b))
             out = tuple(torch.empty(cap, dtype=torch.int32, device=a_off.device) for _ in range(3))
         cap = out[0].numel()
+        if workspace is None:
+            nbytes = symdel_workspace_bytes(n_a, a_seqs.numel(), n_b, b_seqs.numel() if cross else 0, L_MAX, d, cap)
+            workspace = torch.empty(nbytes, dtype=torch.uint8, device=a_off.device)
         n_pairs = C.c_int64(0)
         L = lib()
         p = lambda t: C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)

@@ -56,9 +56,9 @@ def test_strerror_and_workspace_arithmetic(lib):
     assert lib.symdel_strerror(0) == b"ok"
     for code in range(-9, 0):
         assert lib.symdel_strerror(code) not in (b"", b"unknown error")
-    a = symdel.symdel_workspace_bytes(1000, 15000, 0, 0, 24, 2)
-    b = symdel.symdel_workspace_bytes(2000, 30000, 0, 0, 24, 2)
-    c = symdel.symdel_workspace_bytes(1000, 15000, 0, 0, 24, 3)
+    a = symdel.symdel_workspace_bytes(1000, 15000, 0, 0, 24, 2, 0)
+    b = symdel.symdel_workspace_bytes(2000, 30000, 0, 0, 24, 2, 0)
+    c = symdel.symdel_workspace_bytes(1000, 15000, 0, 0, 24, 3, 0)
     assert 0 < a < b and a < c
     with pytest.raises(symdel.SymdelError):
         symdel.symdel_workspace_bytes(10, 100, 0, 0, 24, 9)  # d > D_MAX
