@@ -115,7 +115,24 @@ __global__ void __launch_bounds__(SC_THREADS) k_scan_counts(const u32* __restric
 }
 
 // ---------------------------------------------------------------------------------------------
-constexpr int GEN_THREADS = 256, GEN_G = 32, GEN_R = 4, GEN_NW = GEN_THREADS / 32;
+// General path (any d <= 4, any length <= 64).
+//
+// Count pass without chunking: k_count_dp, one thread per sequence, the classic distinct-subsequence
+// recurrence restricted to the band of <= d deletions (h[i][j] = number of distinct strings obtained
+// from the prefix of length i by deleting exactly j residues):
+//     h[i][j] = h[i-1][j] + h[i-1][j-1] - h[l-1][j-(i-l)],   l = nearest earlier position of s_i
+// (the subtracted term only exists when i - l <= j).  The sum over j <= d equals the number of
+// leftmost-embedding deletion sets, i.e. the records k_generate writes (checked at run time).
+//
+// Generation: a block takes 32 sequences; the deletion sets of the group are numbered consecutively
+// (sequence, then size k, then colexicographic rank) and every thread walks GEN_R CONSECUTIVE numbers:
+// one unranking per thread and round, then the colex successor.  Per set: the leftmost-embedding rule
+// from the per-sequence masks NE_j (bit t: s[t] != s[t+j] or t+j beyond the end), and the hash
+//     H = C_k + U[p_1] + Binv*U[p_2] + Binv^2*U[p_3] + Binv^3*U[p_4]
+// from the per-sequence table U[p] = A[p] - Binv*A[p+1] (same function as the fast path).  A round is
+// two sweeps over the same sets: count the survivors (no hash unless chunked), block scan, then hash
+// and write at the scanned offsets — no register arrays, no unrolled decode.
+constexpr int GEN_THREADS = 256, GEN_G = 32, GEN_R = 8, GEN_NW = GEN_THREADS / 32;
 constexpr int SEQ_STRIDE = SD_L_MAX + 4;
 
 struct GenParams {
@@ -131,8 +148,50 @@ struct GenParams {
     DevInfo* info;
 };
 
+__global__ void __launch_bounds__(128) k_count_dp(SeqSetDev A, SeqSetDev B, int d, int thinning, u32* __restrict__ cnt) {
+    const i64 g = (i64)blockIdx.x * 128 + threadIdx.x;
+    if (g >= A.n + B.n) return;
+    const SeqSetDev& S = g < A.n ? A : B;
+    const i64 i0 = g < A.n ? g : g - A.n;
+    const i64 o = S.off[i0];
+    const int L = (int)(S.off[i0 + 1] - o);
+    if (!thinning) {
+        cnt[g] = c_vcum[L * (SD_D_MAX + 2) + d + 1];
+        return;
+    }
+    // ring of the last d + 2 rows of h (row i lives in slot i % RING)
+    constexpr int RING = SD_D_MAX + 2, W = SD_D_MAX + 1;
+    u32 h[RING][W];
+#pragma unroll
+    for (int r = 0; r < RING; ++r)
+#pragma unroll
+        for (int j = 0; j < W; ++j) h[r][j] = 0;
+    h[0][0] = 1;
+    for (int i = 1; i <= L; ++i) {
+        const int c = S.seqs[o + i - 1];
+        int back = 0;  // i - l for the nearest earlier equal residue within d positions, 0 = none
+        for (int t = 1; t <= d && t < i; ++t)
+            if (S.seqs[o + i - 1 - t] == c) {
+                back = t;
+                break;
+            }
+        const int cur = i % RING, prv = (i - 1) % RING;
+        const int dup = back ? (i - back - 1) % RING : 0;  // row l - 1 = i - back - 1
+        for (int j = 0; j <= d; ++j) {
+            u32 v = h[prv][j] + (j > 0 ? h[prv][j - 1] : 0u);
+            if (back && j >= back) v -= h[dup][j - back];
+            h[cur][j] = j <= i ? v : 0u;
+        }
+    }
+    u32 total = 0;
+    for (int j = 0; j <= d; ++j) total += h[L % RING][j];
+    cnt[g] = total;
+}
+
 struct GenShared {
-    u64 A[GEN_G][SD_L_MAX + 1];
+    u64 U[GEN_G][SD_L_MAX];          // U[p] = A[p] - Binv * A[p + 1]
+    u64 C[GEN_G][SD_D_MAX + 1];      // C[k] = Binv^k * A[L] + (L - k + 1) * K_LEN
+    u64 NE[GEN_G][SD_D_MAX];         // NE[j-1] bit t: t + j >= L or s[t] != s[t + j]
     u64 R[32];
     u64 Bpow[SD_L_MAX + 1];
     i64 off[GEN_G];
@@ -146,68 +205,94 @@ struct GenShared {
     unsigned char seq[GEN_G][SEQ_STRIDE];
 };
 
-// Decodes deletion set number `idx` among the C(L, K) sets of size K (colexicographic order),
-// applies the leftmost-embedding rule and hashes the variant.  Returns false if thinned out.
-template <int K>
-__device__ __forceinline__ bool gen_set(const GenShared& sh, u32 g, u32 L, u32 idx, bool thinning, u64* hash_out) {
-    int p[K > 0 ? K : 1];
-    if (K > 0) {
-        int c = (int)L - 1;
-#pragma unroll
-        for (int j = K; j >= 1; --j) {
-            if (j == 1) {
-                c = (int)idx;
-            } else if (j == 2) {
-                // largest c with c(c-1)/2 <= idx
-                int e = (int)((1.0f + sqrtf(1.0f + 8.0f * (float)idx)) * 0.5f);
-                e = min(e, c);
-                while ((u32)(e * (e - 1) / 2) > idx) --e;
-                while (e < c && (u32)((e + 1) * e / 2) <= idx) ++e;
-                c = e;
-            } else {
-                while (sh.binom[c * (SD_D_MAX + 1) + j] > idx) --c;
+// Walks the deletion sets numbered [f, fend) of the group and calls fn(g, L, k, p) for each.
+template <typename Fn>
+__device__ __forceinline__ void gen_walk(const GenShared& sh, u32 f, u32 fend, u32 ng, int d, Fn&& fn) {
+    int p[4] = {0, 0, 0, 0};
+    u32 g = 0, L = 0, left = 0;  // left = sets remaining in the current (sequence, k) class
+    int k = 0;
+    while (f < fend) {
+        if (left == 0) {
+            u32 lo = 0, hi = ng;  // largest g with vbase[g] <= f
+            while (hi - lo > 1) {
+                const u32 mid = (lo + hi) >> 1;
+                if (sh.vbase[mid] <= f) lo = mid; else hi = mid;
             }
-            p[j - 1] = c;
-            idx -= sh.binom[c * (SD_D_MAX + 1) + j];
-            c = c - 1;
+            g = lo;
+            L = sh.len[g];
+            const u32 rr = f - sh.vbase[g];
+            const u32* vc = sh.vcum + L * (SD_D_MAX + 2);
+            k = 0;
+            while (k < d && rr >= vc[k + 1]) ++k;
+            u32 idx = rr - vc[k];
+            left = sh.binom[L * (SD_D_MAX + 1) + k] - idx;
+            int c = (int)L - 1;  // colexicographic unranking
+#pragma unroll
+            for (int j = 4; j >= 1; --j) {
+                if (j <= k) {
+                    if (j == 1) c = (int)idx;
+                    else
+                        while (sh.binom[c * (SD_D_MAX + 1) + j] > idx) --c;
+                    p[j - 1] = c;
+                    idx -= sh.binom[c * (SD_D_MAX + 1) + j];
+                    c -= 1;
+                }
+            }
         }
-    }
-    const unsigned char* s = sh.seq[g];
-    if (thinning && K > 0) {
-        bool canon = true;
+        fn(g, L, k, p);
+        // colex successor: bump the first element that can move, reset the ones below it
+        bool done = false;
 #pragma unroll
-        for (int m = 0; m < K; ++m) {
-            int q = p[m] + 1;
-#pragma unroll
-            for (int m2 = m + 1; m2 < K; ++m2)
-                if (p[m2] == q) ++q;
-            canon = canon && (q >= (int)L || s[p[m]] != s[q]);
+        for (int i = 0; i < 4; ++i) {
+            if (!done && i < k) {
+                if (i == k - 1 || p[i] + 1 < p[i + 1 < 4 ? i + 1 : 3]) {
+                    ++p[i];
+                    done = true;
+                } else {
+                    p[i] = i;
+                }
+            }
         }
-        if (!canon) return false;
+        ++f;
+        --left;
     }
-    const u64* A = sh.A[g];
-    u64 h = 0;
-    int prev = 0;
-#pragma unroll
-    for (int m = 0; m <= K; ++m) {
-        int end = (m < K) ? p[m < K ? m : 0] : (int)L;
-        u64 term = A[end] - A[prev];
-        h += (m == 0) ? term : c_Binv[m] * term;
-        if (m < K) prev = p[m] + 1;
-    }
-    h += (u64)(L - K + 1) * K_LEN;
-    *hash_out = h;
-    return true;
 }
 
-template <bool COUNT_ONLY>
+__device__ __forceinline__ bool gen_canonical(const GenShared& sh, u32 g, int k, const int* p) {
+    bool ok = true;
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        if (m < k) {
+            int j = 1;  // distance to the next KEPT position after p[m]
+            if (m + 1 < k && p[(m + 1) & 3] == p[m] + 1) {
+                j = 2;
+                if (m + 2 < k && p[(m + 2) & 3] == p[m] + 2) {
+                    j = 3;
+                    if (m + 3 < k && p[(m + 3) & 3] == p[m] + 3) j = 4;
+                }
+            }
+            ok = ok && ((sh.NE[g][j - 1] >> p[m]) & 1ull);
+        }
+    }
+    return ok;
+}
+
+__device__ __forceinline__ u64 gen_hash(const GenShared& sh, u32 g, int k, const int* p) {
+    u64 h = sh.C[g][k];
+    if (k > 0) h += sh.U[g][p[0]];
+    if (k > 1) h += c_Binv[1] * sh.U[g][p[1]];
+    if (k > 2) h += c_Binv[2] * sh.U[g][p[2]];
+    if (k > 3) h += c_Binv[3] * sh.U[g][p[3]];
+    return h;
+}
+
+template <bool COUNT_ONLY, bool CHUNKED>
 __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
     extern __shared__ __align__(16) unsigned char gen_smem[];
     GenShared& sh = *reinterpret_cast<GenShared*>(gen_smem);
     u32* s_hist = reinterpret_cast<u32*>(gen_smem + sizeof(GenShared));  // [npass][256], generation only
 
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const u32 lane_lt = (1u << lane) - 1u;
     for (int i = tid; i < (SD_L_MAX + 1) * (SD_D_MAX + 1); i += GEN_THREADS) sh.binom[i] = c_binom[i];
     for (int i = tid; i < (SD_L_MAX + 1) * (SD_D_MAX + 2); i += GEN_THREADS) sh.vcum[i] = c_vcum[i];
     if (tid < 32) sh.R[tid] = c_R[tid];
@@ -216,6 +301,7 @@ __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
         for (int i = tid; i < P.npass * 256; i += GEN_THREADS) s_hist[i] = 0;
     const int d = P.d;
     const bool thinning = P.thinning != 0;
+    const int kshift = 64 - P.hash_bits;
 
     for (i64 gi = blockIdx.x; gi < P.groups_total; gi += gridDim.x) {
         const bool in_b = gi >= P.groups_a;
@@ -227,17 +313,16 @@ __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
         if (tid < GEN_G) {
             u32 L = 0;
             if (tid < ng) {
-                i64 a = S.off[first + tid];
+                const i64 a = S.off[first + tid];
                 L = (u32)(S.off[first + tid + 1] - a);
                 sh.off[tid] = a;
             }
             sh.len[tid] = L;
             sh.cnt[tid] = 0;
-            // inclusive scan of V(L, d) over the group (warp 0)
-            u32 v = tid < ng ? sh.vcum[L * (SD_D_MAX + 2) + d + 1] : 0, inc = v;
+            u32 v = tid < ng ? sh.vcum[L * (SD_D_MAX + 2) + d + 1] : 0, inc = v;  // V(L, d), scanned over the group
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
-                u32 t = __shfl_up_sync(SD_FULL, inc, o);
+                const u32 t = __shfl_up_sync(SD_FULL, inc, o);
                 if (lane >= (u32)o) inc += t;
             }
             sh.vbase[tid + 1] = inc;
@@ -248,17 +333,25 @@ __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
         }
         __syncthreads();
         for (u32 idx = tid; idx < ng * (u32)P.width; idx += GEN_THREADS) {
-            u32 g = idx / (u32)P.width, p = idx - g * (u32)P.width;
-            sh.seq[g][p] = p < sh.len[g] ? (unsigned char)S.seqs[sh.off[g] + p] : (unsigned char)0;
+            const u32 g = idx / (u32)P.width, q = idx - g * (u32)P.width;
+            sh.seq[g][q] = q < sh.len[g] ? (unsigned char)S.seqs[sh.off[g] + q] : (unsigned char)0;
         }
         __syncthreads();
-        if (tid < ng) {
-            u64 acc = 0;
+        if (tid < ng) {  // per-sequence tables
             const u32 L = sh.len[tid];
-            sh.A[tid][0] = 0;
-            for (u32 p = 0; p < L; ++p) {
-                acc += sh.R[sh.seq[tid][p] & 31] * sh.Bpow[p];
-                sh.A[tid][p + 1] = acc;
+            const unsigned char* sq = sh.seq[tid];
+            u64 acc = 0;
+            for (u32 q = 0; q < L; ++q) {
+                const u64 nxt = acc + sh.R[sq[q] & 31] * sh.Bpow[q];
+                sh.U[tid][q] = acc - c_Binv[1] * nxt;
+                acc = nxt;
+            }
+            for (int k = 0; k <= SD_D_MAX; ++k) sh.C[tid][k] = c_Binv[k] * acc + (u64)(L - k + 1) * K_LEN;
+            for (int j = 1; j <= SD_D_MAX; ++j) {
+                u64 m = 0;
+                for (u32 q = 0; q < L; ++q)
+                    if (!thinning || q + j >= L || sq[q] != sq[q + j]) m |= 1ull << q;
+                sh.NE[tid][j - 1] = m;
             }
         }
         __syncthreads();
@@ -266,78 +359,53 @@ __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
         const u32 T = sh.vbase[ng];
         const u64 base_out = COUNT_ONLY ? 0ull : P.rec_off[gid0];
         for (u32 rb = 0; rb < T; rb += GEN_THREADS * GEN_R) {
-            u64 rec[GEN_R];
-            u32 ball[GEN_R];
-            u32 wt = 0;
-#pragma unroll
-            for (int r = 0; r < GEN_R; ++r) {
-                const u32 f = rb + warp * (32 * GEN_R) + r * 32 + lane;
-                bool valid = false;
-                u32 g = 0;
-                rec[r] = 0;
-                if (f < T) {
-                    u32 lo = 0, hi = ng;
-                    while (hi - lo > 1) {
-                        u32 mid = (lo + hi) >> 1;
-                        if (sh.vbase[mid] <= f) lo = mid; else hi = mid;
-                    }
-                    g = lo;
-                    const u32 rr = f - sh.vbase[g], L = sh.len[g];
-                    const u32* vc = sh.vcum + L * (SD_D_MAX + 2);
-                    int k = 0;
-                    while (k < d && rr >= vc[k + 1]) ++k;
-                    const u32 idx = rr - vc[k];
-                    u64 h = 0;
-                    switch (k) {
-                        case 0: valid = gen_set<0>(sh, g, L, idx, thinning, &h); break;
-                        case 1: valid = gen_set<1>(sh, g, L, idx, thinning, &h); break;
-                        case 2: valid = gen_set<2>(sh, g, L, idx, thinning, &h); break;
-                        case 3: valid = gen_set<3>(sh, g, L, idx, thinning, &h); break;
-                        default: valid = gen_set<4>(sh, g, L, idx, thinning, &h); break;
-                    }
-                    if (valid && P.n_chunks > 1) valid = gen_chunk_of(h, P.n_chunks) == P.chunk;
-                    rec[r] = ((h >> (64 - P.hash_bits)) << P.id_bits) | (gid0 + g);
-                }
-                ball[r] = __ballot_sync(SD_FULL, valid);
-                wt += __popc(ball[r]);
+            const u32 f0 = min(T, rb + tid * GEN_R), f1 = min(T, f0 + GEN_R);
+            // ---- sweep 1: survivors of this thread's range ----
+            u32 mine = 0, gcur = 0xffffffffu, gacc = 0;
+            gen_walk(sh, f0, f1, ng, d, [&](u32 g, u32, int k, const int* p) {
+                bool ok = gen_canonical(sh, g, k, p);
+                if (CHUNKED && ok) ok = gen_chunk_of(gen_hash(sh, g, k, p), P.n_chunks) == P.chunk;
                 if (COUNT_ONLY) {
-                    // lanes of one sequence are contiguous: one shared-memory add per (warp, sequence) segment
-                    const u32 gprev = __shfl_up_sync(SD_FULL, g, 1);
-                    const bool head = (lane == 0) || (gprev != g);
-                    const u32 heads = __ballot_sync(SD_FULL, head);
-                    if (head) {
-                        const u32 higher = (lane == 31) ? 0u : (heads & (~0u << (lane + 1)));
-                        const u32 end = higher ? (u32)(__ffs(higher) - 1) : 32u;
-                        const u32 seg = (~0u << lane) & (end == 32 ? ~0u : ((1u << end) - 1u));
-                        const u32 c = __popc(ball[r] & seg);
-                        if (c) atomicAdd(&sh.cnt[g], c);
+                    if (g != gcur) {
+                        if (gacc) atomicAdd(&sh.cnt[gcur], gacc);
+                        gcur = g, gacc = 0;
                     }
+                    gacc += ok ? 1u : 0u;
                 }
+                mine += ok ? 1u : 0u;
+            });
+            if (COUNT_ONLY) {
+                if (gacc) atomicAdd(&sh.cnt[gcur], gacc);
+                continue;
             }
-            if (!COUNT_ONLY) {
-                if (lane == 0) sh.wtot[warp] = wt;
-                __syncthreads();
-                u32 woff = sh.running, all = 0;
+            // ---- block exclusive scan of the survivor counts ----
+            u32 inc = mine;
 #pragma unroll
-                for (int w = 0; w < GEN_NW; ++w) {
-                    u32 c = sh.wtot[w];
-                    if ((u32)w < warp) woff += c;
-                    all += c;
-                }
-                __syncthreads();
-                if (tid == 0) sh.running += all;
-                u32 pre = 0;
-#pragma unroll
-                for (int r = 0; r < GEN_R; ++r) {
-                    if (ball[r] & (1u << lane)) {
-                        const u32 pos = woff + pre + __popc(ball[r] & lane_lt);
-                        P.records[base_out + pos] = rec[r];
-                        const u64 key = rec[r] >> P.id_bits;
-                        for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
-                    }
-                    pre += __popc(ball[r]);
-                }
+            for (int o = 1; o < 32; o <<= 1) {
+                const u32 t = __shfl_up_sync(SD_FULL, inc, o);
+                if (lane >= (u32)o) inc += t;
             }
+            if (lane == 31) sh.wtot[warp] = inc;
+            __syncthreads();
+            u32 woff = sh.running, all = 0;
+#pragma unroll
+            for (int w = 0; w < GEN_NW; ++w) {
+                const u32 c = sh.wtot[w];
+                if ((u32)w < warp) woff += c;
+                all += c;
+            }
+            __syncthreads();
+            if (tid == 0) sh.running += all;
+            // ---- sweep 2: hash and write ----
+            u64* out = P.records + base_out + woff + inc - mine;
+            gen_walk(sh, f0, f1, ng, d, [&](u32 g, u32, int k, const int* p) {
+                if (!gen_canonical(sh, g, k, p)) return;
+                const u64 h = gen_hash(sh, g, k, p);
+                if (CHUNKED && gen_chunk_of(h, P.n_chunks) != P.chunk) return;
+                const u64 key = h >> kshift;
+                *out++ = (key << P.id_bits) | (gid0 + g);
+                for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
+            });
         }
         __syncthreads();
         if (COUNT_ONLY) {
@@ -352,7 +420,6 @@ __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
             if (s_hist[i]) atomicAdd(&P.ghist[i], s_hist[i]);
     }
 }
-
 
 // ---------------------------------------------------------------------------------------------
 // Fast path (d <= 2, longest sequence <= 32): one warp per batch of consecutive sequences packed into
@@ -638,12 +705,10 @@ cudaError_t sd_init_tables() {
     if ((e = cudaMemcpyToSymbol(c_Binv, Binv, sizeof(Binv))) != cudaSuccess) return e;
     if ((e = cudaMemcpyToSymbol(c_binom, binom, sizeof(binom))) != cudaSuccess) return e;
     if ((e = cudaMemcpyToSymbol(c_vcum, vcum, sizeof(vcum))) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_generate<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)(sizeof(GenShared) + 8 * 256 * 4))) != cudaSuccess)
-        return e;
-    if ((e = cudaFuncSetAttribute(k_generate<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)sizeof(GenShared))) != cudaSuccess)
-        return e;
+    const int gsm = (int)(sizeof(GenShared) + 8 * 256 * 4);
+    if ((e = cudaFuncSetAttribute(k_generate<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, gsm)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_generate<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, gsm)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_generate<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, gsm)) != cudaSuccess) return e;
 
     done = true;
     return cudaSuccess;
@@ -665,7 +730,8 @@ cudaError_t sd_count(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u32
     P.cnt = cnt;
     P.info = info;
     if (fast) gen2_pick<true>(lay.n_chunks > 1, 0)<<<gen2_grid(P.groups_total), G2_THREADS, sizeof(Gen2Shared), st>>>(P);
-    else k_generate<true><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared), st>>>(P);
+    else if (lay.n_chunks > 1) k_generate<true, true><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared), st>>>(P);
+    else k_count_dp<<<(unsigned)((a.n + b.n + 127) / 128), 128, 0, st>>>(a, b, lay.d, lay.thinning, cnt);
     if (launches) ++*launches;
     return cudaGetLastError();
 }
@@ -695,8 +761,10 @@ cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     if (fast)
         gen2_pick<false>(lay.n_chunks > 1, npass)<<<gen2_grid(P.groups_total), G2_THREADS,
                                                       sizeof(Gen2Shared) + (size_t)npass * 256 * 4, st>>>(P);
+    else if (lay.n_chunks > 1)
+        k_generate<false, true><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared) + (size_t)npass * 256 * 4, st>>>(P);
     else
-        k_generate<false><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared) + (size_t)npass * 256 * 4, st>>>(P);
+        k_generate<false, false><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared) + (size_t)npass * 256 * 4, st>>>(P);
     if (launches) ++*launches;
     return cudaGetLastError();
 }

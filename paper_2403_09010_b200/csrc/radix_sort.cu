@@ -46,6 +46,9 @@ __global__ void __launch_bounds__(256) k_hist_scan(u32* __restrict__ ghist) {
 #define OS_FLAG_AGG (1u << 30)
 #define OS_FLAG_PRE (2u << 30)
 #define OS_MASK ((1u << 30) - 1)
+#ifndef OS_LB
+#define OS_LB 4
+#endif
 
 // Peer mask of the lanes holding the same 8-bit digit, built from 8 ballots (the MATCH.ANY
 // instruction measured ~170 cycles per warp on sm_100a; 8 x (VOTE + LOP3) is ~10x cheaper).
@@ -138,18 +141,18 @@ __device__ __forceinline__ void os_tile(const u64* __restrict__ in, u64* __restr
     if (tid < 256) {
         u32 excl = 0;
         if (tile != 0) {
-            // four predecessors per round trip: the walk back to the nearest inclusive prefix is a chain
+            // OS_LB predecessors per round trip: the walk back to the nearest inclusive prefix is a chain
             // of L2 latencies, so loads are issued in batches and consumed in order
             const u32* p = st;
             u32 rem = tile;
             bool done = false;
             while (!done) {
-                u32 sv[4];
+                u32 sv[OS_LB];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) sv[j] = ((u32)j < rem) ? sd_ld_relaxed32(p - 256 * (j + 1)) : OS_FLAG_PRE;
+                for (int j = 0; j < OS_LB; ++j) sv[j] = ((u32)j < rem) ? sd_ld_relaxed32(p - 256 * (j + 1)) : OS_FLAG_PRE;
                 int used = 0;
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
+                for (int j = 0; j < OS_LB; ++j) {
                     if (!done && used == j) {
                         const u32 f = sv[j] >> 30;
                         if (f != 0) {
