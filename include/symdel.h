@@ -70,8 +70,10 @@ typedef struct {
     int64_t n_chunks;      /* key-range chunks used (S5) */
     int64_t n_flushes;     /* candidate-buffer flushes (dedup+verify rounds) */
     int64_t n_launches;    /* kernels launched */
-    int32_t hash_bits;     /* key bits sorted per record */
+    int32_t hash_bits;     /* hash bits carried per record (64 - id_bits unless narrowed) */
     int32_t id_bits;       /* id bits per record */
+    int32_t sort_bits;     /* top hash bits radix-partitioned by S2 (8 per onesweep pass); the join compares the rest */
+    int32_t pad_;
     float ms_prepare, ms_generate, ms_sort, ms_emit, ms_dedup, ms_verify, ms_total; /* CUDA-event times; 0 unless SYMDEL_OPT_TIMING is set */
     float ms_sort_pass_avg; /* average duration of one onesweep pass over the variant records */
     int64_t sort_pass_records; /* records moved by one such pass */
@@ -82,10 +84,13 @@ enum {
     SYMDEL_OPT_TIMING = 1,        /* [0] 1: bracket each stage with CUDA events (adds stream syncs at the end only) */
     SYMDEL_OPT_FORCE_CHUNKS = 2,  /* [0] >0: use exactly this many key-range chunks (test hook for S5) */
     SYMDEL_OPT_CAND_CAPACITY = 3, /* [0] >0: cap the candidate buffer at this many pairs (test hook for multi-flush) */
-    SYMDEL_OPT_HASH_BITS = 4,     /* [0] 0 = automatic; else 8..56 (multiple of 8): key bits sorted per record */
+    SYMDEL_OPT_HASH_BITS = 4,     /* [0] 0 = every bit the id leaves free; else 1..63: hash bits kept per record (test hook: a narrow hash makes colliding variants, the result is unchanged) */
     SYMDEL_OPT_NO_THINNING = 5,   /* [0] 1: emit one record per deletion SET instead of per distinct variant (test hook) */
     SYMDEL_OPT_GENERAL_GENERATE = 7, /* [0] 1: use the general (any d, any length) generation kernel even where the d <= 2 fast path applies (test hook) */
-    SYMDEL_OPT_SORT_VARIANT = 6   /* [0] tile shape of the onesweep kernel (process-wide tuning hook; results are identical) */
+    SYMDEL_OPT_SORT_VARIANT = 6,  /* [0] tile shape of the onesweep kernel (process-wide tuning hook; results are identical) */
+    SYMDEL_OPT_SORT_BITS = 8,     /* [0] 0 = automatic; 8..56 (multiple of 8): top hash bits that S2 radix-partitions; 255 = none (one bucket: the join chunks it) */
+    SYMDEL_OPT_SORT_STABLE = 9,   /* [0] 1: every S2 pass takes the stable (ties keep input order) tile path (test hook; results are identical) */
+    SYMDEL_OPT_SORT_GROUPING = 10 /* [0] 1: symdel_stage_sort_u64 sorts keys only: ties land in arbitrary order (the mode the pipeline uses) */
 };
 
 /* ---- context ------------------------------------------------------------------------------- */

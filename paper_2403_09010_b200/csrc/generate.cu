@@ -139,7 +139,7 @@ struct GenParams {
     SeqSetDev a, b;
     i64 groups_a, groups_total;
     i64 n_a;
-    int d, width, thinning, hash_bits, id_bits, npass;
+    int d, width, thinning, hash_bits, id_bits, npass, hshift;  // hshift: bit of the KEY where the first counted digit starts
     u32 n_chunks, chunk;
     const u64* rec_off;
     u64* records;
@@ -404,7 +404,7 @@ __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
                 if (CHUNKED && gen_chunk_of(h, P.n_chunks) != P.chunk) return;
                 const u64 key = h >> kshift;
                 *out++ = (key << P.id_bits) | (gid0 + g);
-                for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
+                for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (P.hshift + 8 * ps)) & 255u)], 1u);
             });
         }
         __syncthreads();
@@ -459,9 +459,9 @@ __device__ __forceinline__ void g2_emit(bool valid, u64 h, const GenParams& P, u
             out[__popc(bal & lane_lt)] = (key << P.id_bits) | gid;
             if (NPASS > 0) {
 #pragma unroll
-                for (int ps = 0; ps < NPASS; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
+                for (int ps = 0; ps < NPASS; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (P.hshift + 8 * ps)) & 255u)], 1u);
             } else {
-                for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
+                for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (P.hshift + 8 * ps)) & 255u)], 1u);
             }
         }
         out += __popc(bal);
@@ -528,7 +528,7 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
                 } else if (ok) {
                     const u64 key = h >> kshift;
                     P.records[rec_base_i] = (key << P.id_bits) | (gid0 + lane);
-                    for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (8 * ps)) & 255u)], 1u);
+                    for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (P.hshift + 8 * ps)) & 255u)], 1u);
                 }
             }
             if (total > 0) {
@@ -625,9 +625,9 @@ Gen2Kernel gen2_pick(bool chunked, int npass) {
     if (chunked) return k_gen2<COUNT_ONLY, true, 0>;
     if (COUNT_ONLY) return k_gen2<COUNT_ONLY, false, 0>;
     switch (npass) {
+        case 1: return k_gen2<COUNT_ONLY, false, 1>;
+        case 2: return k_gen2<COUNT_ONLY, false, 2>;
         case 3: return k_gen2<COUNT_ONLY, false, 3>;
-        case 4: return k_gen2<COUNT_ONLY, false, 4>;
-        case 5: return k_gen2<COUNT_ONLY, false, 5>;
         default: return k_gen2<COUNT_ONLY, false, 0>;
     }
 }
@@ -749,7 +749,7 @@ cudaError_t sd_scan_counts(const u32* cnt, i64 n, u64* rec_off, u64* lb_status, 
 }
 
 cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, const u64* rec_off, u64* records,
-                        u32* ghist, int npass, DevInfo* info, cudaStream_t st, i64* launches) {
+                        u32* ghist, int hist_bit, int npass, DevInfo* info, cudaStream_t st, i64* launches) {
     const bool fast = use_fast(lay, width);
     GenParams P = fast ? make_params2(a, b, lay, width) : make_params(a, b, lay, width);
     if (P.groups_total == 0) return cudaSuccess;
@@ -757,6 +757,7 @@ cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     P.records = records;
     P.ghist = ghist;
     P.npass = npass;
+    P.hshift = hist_bit - lay.id_bits;
     P.info = info;
     if (fast)
         gen2_pick<false>(lay.n_chunks > 1, npass)<<<gen2_grid(P.groups_total), G2_THREADS,

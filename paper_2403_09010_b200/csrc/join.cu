@@ -1,0 +1,301 @@
+// join.cu — S3a/K3: run boundaries and candidate-pair emission, as a shared-memory hash join over
+// the buckets left by the radix partition.
+//
+// "Use the sorted array to identify groups of input strings that generate identical deletion
+// variants, and transform this to an array of neighbor candidates" (App. F.2 step 3);
+// "For each group v_g, generate all possible matching sequence pairs {(i', i'')} within the group"
+// (App. F.3 step 3); a variant shared by m sequences yields m(m-1)/2 pairs
+// (PAPER.md:96).  Output slots are allocated by prefix sums before anything is written ("avoid race
+// condition by preallocating the outputs", Fig. S8).
+//
+// The records arrive partitioned on their top `sort_bits` hash bits only (S2 stops there): a BUCKET is
+// a maximal range of records agreeing on those bits, a few thousand records by construction.  Equal
+// variants always share a bucket, so the join is local to it: a block loads whole buckets into shared
+// memory, chains the records by the next hash bits (one atomic exchange each) and every record walks
+// its chain for EARLIER records with the same full hash — the remaining sort passes over all records
+// and the read of the sorted array are replaced by one read.  Neither the order of the records inside
+// a bucket nor the order of the buckets matters.
+//
+// Work split: tile t owns the buckets that START in [t*T, (t+1)*T).  It loads T + slack records, finds
+// the first bucket boundary at or after each end of its range and joins what lies between.  A region
+// that does not fit (a huge bucket: one variant shared by many thousands of sequences) is processed in
+// chunks: build the table on a chunk, join it with itself, then stream the rest of its last bucket
+// through the table.
+//
+// Numbering: a record's pairs get consecutive flat indices (thread-local order is fixed by the record
+// positions, so it is the same in every round); a round writes the records whose FIRST index lies in
+// [win_lo, win_hi), whole, at cand[index - win_lo] — the buffer keeps n_total + 64 slots of slack for
+// the overhang — and reports the end of what it wrote in info->win_end, where the next round starts.
+#include "kernels.h"
+
+namespace {
+
+constexpr int JN_THREADS = 512, JN_T = 4096, JN_CAP = 6144, JN_SLOT_BITS = 13, JN_SLOTS = 1 << JN_SLOT_BITS;
+constexpr u32 JN_NIL = 0xffffu, JN_NONE = 0xffffffffu;
+static_assert(JN_CAP < 0xffff && JN_CAP % JN_THREADS == 0 && JN_CAP / JN_THREADS <= 32, "node index / nzmask width");
+
+struct JoinParams {
+    const u64* rec;
+    u64 n;
+    u64 topmask;  // the radix-partitioned bits: a bucket = maximal range agreeing on them (0: one bucket)
+    u64 hlim;     // 1 << id_bits: same hash <=> (x ^ y) < hlim
+    u64 idmask, n_a;
+    int slot_shift, tag_shift, b_bits, cross;
+    u64* cand;
+    u64 cand_cap;  // physical slots of cand
+    u64 win_lo, win_hi;
+    int first_round;
+    u64* tile_prefix;
+    DevInfo* info;
+};
+
+__device__ __forceinline__ bool jn_pair(u64 x, u64 y, const JoinParams& P, u64& packed) {
+    const u64 a = x & P.idmask, b = y & P.idmask;
+    if (P.cross) {
+        const bool ax = a < P.n_a, bx = b < P.n_a;
+        if (ax == bx) return false;
+        packed = ((ax ? a : b) << P.b_bits) | ((ax ? b : a) - P.n_a);
+    } else {
+        if (a == b) return false;  // one sequence twice under one key (thinning off, or a hash collision)
+        packed = (min(a, b) << P.b_bits) | max(a, b);
+    }
+    return true;
+}
+
+__global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
+    extern __shared__ __align__(16) unsigned char jn_smem[];
+    u64* s_rec = reinterpret_cast<u64*>(jn_smem);  // [0] = record before the window, [1 + r] = record sb + r
+    u32* s_head = reinterpret_cast<u32*>(s_rec + JN_CAP + 2);
+    u32* s_node = s_head + JN_SLOTS;  // per record: tag << 16 | next
+    __shared__ u32 s_lo, s_hi;
+    __shared__ u64 s_wsum[JN_THREADS / 32];
+    __shared__ u64 s_excl;
+
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 tile = blockIdx.x;
+    if (!P.first_round) {
+        const u64 lo = P.tile_prefix[2 * tile], cnt = P.tile_prefix[2 * tile + 1];
+        if (cnt == 0 || lo + cnt <= P.win_lo || lo >= P.win_hi) return;  // nothing of this tile starts in the window
+    }
+    const u64 N = P.n;
+    const u64 g0 = (u64)tile * JN_T;
+    const u64 E = min(g0 + (u64)JN_T, N);  // the region ends at the first boundary >= E
+
+    // loads records [sb - 1, sb + CAP] (one before, one lookahead) and returns the usable count W
+    auto load = [&](u64 sb) -> u32 {
+        const u32 cnt = (u32)min((u64)(JN_CAP + 1), N - sb);
+        for (u32 r = tid; r < cnt; r += JN_THREADS) s_rec[1 + r] = P.rec[sb + r];
+        if (tid == 0) s_rec[0] = sb > 0 ? P.rec[sb - 1] : 0ull;
+        return min(cnt, (u32)JN_CAP);
+    };
+    // position sb + r starts a bucket (r in [0, W]; position N counts as a boundary)
+    auto isb = [&](u64 sb, u32 r) -> bool {
+        const u64 g = sb + r;
+        return g == 0 || g == N || ((s_rec[r] ^ s_rec[1 + r]) & P.topmask) != 0;
+    };
+    auto build = [&](u32 r0, u32 r1) {
+        for (u32 i = tid; i < JN_SLOTS / 4; i += JN_THREADS)
+            reinterpret_cast<uint4*>(s_head)[i] = make_uint4(JN_NIL, JN_NIL, JN_NIL, JN_NIL);
+        __syncthreads();
+        for (u32 r = r0 + tid; r < r1; r += JN_THREADS) {
+            const u64 x = s_rec[1 + r];
+            const u32 prev = atomicExch(&s_head[(u32)(x >> P.slot_shift) & (JN_SLOTS - 1)], r);
+            s_node[r] = (((u32)(x >> P.tag_shift) & 0xffffu) << 16) | prev;
+        }
+        __syncthreads();
+    };
+    u64 wend = 0;
+    // pairs of record x with the table records at chunk positions < lim; returns their number and, when
+    // `store`, writes them from cand[at]
+    auto walk = [&](u64 x, u32 lim, bool store, u64 at) -> u32 {
+        const u32 tag = (u32)(x >> P.tag_shift) & 0xffffu;
+        u32 c = 0;
+        for (u32 j = s_head[(u32)(x >> P.slot_shift) & (JN_SLOTS - 1)]; j != JN_NIL;) {
+            const u32 w = s_node[j];
+            if (j < lim && (w >> 16) == tag) {
+                const u64 y = s_rec[1 + j];
+                u64 packed;
+                if ((x ^ y) < P.hlim && jn_pair(x, y, P, packed)) {
+                    if (store) {
+                        if (at + c < P.cand_cap) P.cand[at + c] = packed;
+                        else atomicOr(&P.info->err, (u32)SD_ERR_OVERFLOW);
+                    }
+                    ++c;
+                }
+            }
+            j = w & 0xffffu;
+        }
+        return c;
+    };
+    auto visit = [&](u64 x, u32 lim, bool write, u64& flat) -> u32 {
+        const bool inwin = write && flat >= P.win_lo && flat < P.win_hi;
+        const u32 c = walk(x, lim, inwin, flat - P.win_lo);
+        flat += c;
+        if (inwin && c) wend = max(wend, flat);
+        return c;
+    };
+
+    // ---- first chunk: the window of this tile; which buckets start in it? ----
+    if (tid == 0) s_lo = JN_NONE, s_hi = JN_NONE;
+    u32 W = load(g0);
+    __syncthreads();
+    {
+        u32 mlo = JN_NONE, mhi = JN_NONE;  // r ascends: keep the first of each kind
+        for (u32 r = tid; r <= W; r += JN_THREADS)
+            if (isb(g0, r)) {
+                if (g0 + r < E) mlo = min(mlo, r);
+                else mhi = min(mhi, r);
+            }
+        mlo = __reduce_min_sync(SD_FULL, mlo);
+        mhi = __reduce_min_sync(SD_FULL, mhi);
+        if (lane == 0 && mlo != JN_NONE) atomicMin(&s_lo, mlo);
+        if (lane == 0 && mhi != JN_NONE) atomicMin(&s_hi, mhi);
+    }
+    __syncthreads();
+    const u32 lo = s_lo, hi0 = s_hi;
+    if (lo == JN_NONE) {  // no bucket starts here
+        if (P.first_round && tid == 0) P.tile_prefix[2 * tile] = 0, P.tile_prefix[2 * tile + 1] = 0;
+        return;
+    }
+    const bool single = hi0 != JN_NONE;  // the whole region sits in shared memory
+    u32 nzmask = 0;                      // single: which of this thread's records have pairs
+
+    u64 flat = 0;
+    for (int phase = 0; phase < 2; ++phase) {
+        const bool write = phase == 1;
+        u64 sb = g0;
+        u32 r0 = lo, r1 = single ? hi0 : (u32)JN_CAP;
+        bool last = single;
+        for (bool first = true;; first = false) {
+            if (!first || (write && !single)) {  // an oversized region: (re)load the chunk that starts at sb
+                __syncthreads();
+                if (tid == 0) s_hi = JN_NONE;
+                W = load(sb);
+                __syncthreads();
+                if (!first) {
+                    u32 mhi = JN_NONE;
+                    for (u32 r = 1 + tid; r <= W; r += JN_THREADS)
+                        if (isb(sb, r)) mhi = min(mhi, r);
+                    mhi = __reduce_min_sync(SD_FULL, mhi);
+                    if (lane == 0 && mhi != JN_NONE) atomicMin(&s_hi, mhi);
+                    __syncthreads();
+                    last = s_hi != JN_NONE;
+                    r0 = 0;
+                    r1 = last ? s_hi : (u32)JN_CAP;
+                }
+            }
+            if (!(single && write)) build(r0, r1);
+            // ---- the chunk with itself ----
+            if (single && write) {
+                for (u32 m = nzmask, k = 0; m; m >>= 1, ++k) {
+                    const u32 r = r0 + tid + k * JN_THREADS;
+                    if (m & 1u) visit(s_rec[1 + r], r, true, flat);
+                }
+            } else {
+                u32 k = 0;
+                for (u32 r = r0 + tid; r < r1; r += JN_THREADS, ++k)
+                    if (visit(s_rec[1 + r], r, write, flat) && single) nzmask |= 1u << k;
+            }
+            if (last) break;
+            // ---- the rest of the chunk's last bucket against the chunk ----
+            if (!isb(sb, JN_CAP)) {
+                const u64 lastx = s_rec[JN_CAP];
+                for (u64 q0 = sb + JN_CAP;; q0 += JN_THREADS) {
+                    const u64 q = q0 + tid;
+                    u64 x = 0;
+                    bool inb = q < N;
+                    if (inb) {
+                        x = P.rec[q];
+                        inb = ((x ^ lastx) & P.topmask) == 0;
+                    }
+                    if (inb) visit(x, JN_CAP, write, flat);
+                    if (!__syncthreads_and(inb)) break;
+                }
+            }
+            sb += JN_CAP;
+        }
+        if (write) break;
+
+        // ---- block exclusive scan of the per-thread totals; the tile claims its index range ----
+        const u64 tsum = flat;
+        u64 inc = tsum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const u64 t = __shfl_up_sync(SD_FULL, inc, o);
+            if (lane >= (u32)o) inc += t;
+        }
+        if (lane == 31) s_wsum[warp] = inc;
+        __syncthreads();
+        u64 carry = 0, T = 0;
+#pragma unroll
+        for (int w = 0; w < JN_THREADS / 32; ++w) {
+            const u64 c = s_wsum[w];
+            if ((u32)w < warp) carry += c;
+            T += c;
+        }
+        if (T == 0) {
+            if (P.first_round && tid == 0) P.tile_prefix[2 * tile] = 0, P.tile_prefix[2 * tile + 1] = 0;
+            return;
+        }
+        if (tid == 0) {
+            u64 excl;
+            if (P.first_round) {
+                excl = (u64)atomicAdd((unsigned long long*)&P.info->n_cand, (unsigned long long)T);
+                P.tile_prefix[2 * tile] = excl;
+                P.tile_prefix[2 * tile + 1] = T;
+            } else {
+                excl = P.tile_prefix[2 * tile];
+            }
+            s_excl = excl;
+        }
+        __syncthreads();
+        flat = s_excl + carry + inc - tsum;  // flat index of this thread's first pair
+        if (single && (tsum == 0 || flat + tsum <= P.win_lo || flat >= P.win_hi)) break;  // nothing of mine in the window
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) wend = max(wend, __shfl_xor_sync(SD_FULL, wend, o));
+    if (lane == 0 && wend) atomicMax((unsigned long long*)&P.info->win_end, (unsigned long long)wend);
+}
+
+}  // namespace
+
+i64 sd_join_tiles(i64 n_records) { return (n_records + JN_T - 1) / JN_T; }
+
+cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 cand_cap, u64 win_lo, u64 win_hi,
+                    int first_round, u64* tile_prefix, DevInfo* info, cudaStream_t st, i64* launches) {
+    const i64 tiles = sd_join_tiles(n_records);
+    if (tiles == 0) return cudaSuccess;
+    constexpr size_t smem = (size_t)(JN_CAP + 2) * 8 + (size_t)JN_SLOTS * 4 + (size_t)JN_CAP * 4;
+    static bool attr_set = false;
+    cudaError_t e;
+    if (!attr_set) {
+        if ((e = cudaFuncSetAttribute(k_join, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        attr_set = true;
+    }
+    if (first_round && (e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(&info->win_end, 0, sizeof(u64), st)) != cudaSuccess) return e;
+    JoinParams P{};
+    P.rec = records;
+    P.n = (u64)n_records;
+    const int top = lay.id_bits + lay.hash_bits, sort_bits = lay.sort_bits;  // the hash field is bits [id_bits, top)
+    P.topmask = sort_bits > 0 ? (~0ull >> (64 - sort_bits)) << (top - sort_bits) : 0ull;
+    P.hlim = 1ull << lay.id_bits;
+    P.idmask = P.hlim - 1ull;
+    P.n_a = (u64)lay.n_a;
+    // chain slot = the hash bits right below the partitioned ones, tag = the 16 bits below those (both
+    // clamped to the hash field: with few hash bits they overlap the bucket bits, which is harmless)
+    P.slot_shift = std::max(lay.id_bits, top - sort_bits - JN_SLOT_BITS);
+    P.tag_shift = std::max(lay.id_bits, P.slot_shift - 16);
+    P.b_bits = lay.b_bits;
+    P.cross = lay.cross;
+    P.cand = cand;
+    P.cand_cap = cand_cap;
+    P.win_lo = win_lo;
+    P.win_hi = win_hi;
+    P.first_round = first_round;
+    P.tile_prefix = tile_prefix;
+    P.info = info;
+    k_join<<<(unsigned)tiles, JN_THREADS, smem, st>>>(P);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}

@@ -23,7 +23,8 @@ struct Layout {
     int cross;         // 1: emit only (A, B) combinations
     int d;
     int id_bits;       // 2^id_bits > n_a + n_b
-    int hash_bits;     // multiple of 8
+    int hash_bits;     // hash bits kept per record: the record is (hash >> (64 - hash_bits)) << id_bits | id
+    int sort_bits;     // multiple of 8, <= hash_bits: the top bits of the hash field that S2 radix-partitions
     int b_bits;        // bits of the second pair component (self: id_bits; cross: bits of n_b)
     int pair_bits;     // a_bits + b_bits
     int thinning;
@@ -40,7 +41,7 @@ u32* sd_sort_hist_ptr(void* scratch);
 cudaError_t sd_sort_histogram(const u64* keys, i64 n, int begin_bit, int npass, void* scratch, cudaStream_t st,
                               i64* launches);
 cudaError_t sd_sort_hist_scan(void* scratch, int npass, cudaStream_t st, i64* launches);
-cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, void* scratch, cudaStream_t st,
+cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, int stable, void* scratch, cudaStream_t st,
                            u64** result, i64* launches);
 
 // ---- generate.cu --------------------------------------------------------------------------------
@@ -53,17 +54,20 @@ cudaError_t sd_count(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u32
 i64 sd_scan_tiles(i64 n);
 cudaError_t sd_scan_counts(const u32* cnt, i64 n, u64* rec_off, u64* lb_status, DevInfo* info, cudaStream_t st,
                            i64* launches);
-// generation pass: writes records at rec_off[gid].., accumulates the digit histograms into ghist
+// generation pass: writes records at rec_off[gid].., accumulates the histograms of the npass 8-bit
+// digits starting at bit hist_bit of the record into ghist
 cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, const u64* rec_off, u64* records,
-                        u32* ghist, int npass, DevInfo* info, cudaStream_t st, i64* launches);
+                        u32* ghist, int hist_bit, int npass, DevInfo* info, cudaStream_t st, i64* launches);
 
-// ---- emit.cu ------------------------------------------------------------------------------------
-i64 sd_emit_tiles(i64 n_records);
-// Emits candidate pairs with flat index in [win_lo, win_hi) to cand[flat - win_lo].
-// first_round = 1: computes and stores tile_prefix[] (exclusive pair-count prefix per tile) and
-// info->n_cand (total); later rounds reuse tile_prefix.  lb_status: sd_emit_tiles u64.
-cudaError_t sd_emit(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 win_lo, u64 win_hi,
-                    int first_round, u64* tile_prefix, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
+// ---- join.cu ------------------------------------------------------------------------------------
+i64 sd_join_tiles(i64 n_records);
+// records: partitioned on the top lay.sort_bits bits of the hash field.  Emits the candidate pairs of
+// the records whose first flat pair index lies in [win_lo, win_hi) to cand[index - win_lo] (cand_cap
+// physical slots: the window plus slack for the last record's overhang); info->win_end = end of what
+// was written.  first_round = 1: numbers the pairs (tile_prefix[2 * tiles], info->n_cand = total);
+// later rounds reuse the numbering.
+cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 cand_cap, u64 win_lo, u64 win_hi,
+                    int first_round, u64* tile_prefix, DevInfo* info, cudaStream_t st, i64* launches);
 
 // ---- verify.cu ----------------------------------------------------------------------------------
 i64 sd_verify_tiles(i64 n);

@@ -18,6 +18,7 @@
 // count scan (grid sizes), one after the first emit (candidate count), two at the end.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -30,6 +31,7 @@ struct symdel_ctx {
     symdel_stats stats{};
     int opt_timing = 0;
     i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0, opt_general_gen = 0;
+    i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0;
     DevInfo* h_info = nullptr;  // pinned
     void* arena = nullptr;      // device arena of the *_host entry points
     size_t arena_bytes = 0;
@@ -86,7 +88,7 @@ u64 vcount_host(int L, int d) {
 }
 
 i64 rec_bytes(i64 ncap, int npass) {
-    return 2 * align_up(ncap * 8) + align_up(sd_sort_scratch_bytes(ncap, npass)) + align_up((2 * sd_emit_tiles(ncap) + 2) * 8);
+    return 2 * align_up(ncap * 8) + align_up(sd_sort_scratch_bytes(ncap, npass)) + align_up((2 * sd_join_tiles(ncap) + 2) * 8);
 }
 i64 cand_bytes(i64 ccap, int ppass) {
     return 2 * align_up(ccap * 8) + align_up(sd_sort_scratch_bytes(ccap, ppass)) + align_up((ccap / 256 + 2) * 8);
@@ -189,24 +191,21 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     lay.thinning = ctx->opt_no_thinning ? 0 : 1;
     lay.force_general = ctx->opt_general_gen ? 1 : 0;
     {
-        int hb = (int)ctx->opt_hash_bits;
-        if (hb == 0) {
-            // Key width: every 8 bits cost one more pass over all records (16 B/record); too few bits
-            // cost spurious candidates (~n_x * n_y / 2^bits colliding pairs, ~150 B of traffic each
-            // through emit, pair sort and verify).  Pick the cheapest width.
-            const double nb = (double)ctx->h_info->nmax_b, na = (double)nmax - nb;
-            double best = 0;
-            for (int h = 16; h <= 56; h += 8) {
-                const double pairs = (cross ? na * nb : 0.5 * na * na) / std::pow(2.0, h);
-                const double cost = (double)nmax * 16.0 * (h / 8) + pairs * 150.0;
-                if (hb == 0 || cost < best) best = cost, hb = h;
-            }
-        }
-        const int hb_max = (64 - lay.id_bits) / 8 * 8;
-        if (hb % 8 != 0 || hb < 8) return SYMDEL_E_ARG;
-        lay.hash_bits = std::min(hb, hb_max);
+        // Hash field: every bit the id leaves free (SYMDEL_OPT_HASH_BITS narrows it: more colliding
+        // variants, same result).  S2 radix-partitions only its top sort_bits: enough 8-bit digits for the
+        // average bucket to fit the join kernel's shared-memory window; the join compares the rest.
+        const int hb_max = 64 - lay.id_bits;
+        lay.hash_bits = ctx->opt_hash_bits > 0 ? (int)std::min<i64>(ctx->opt_hash_bits, hb_max) : hb_max;
     }
-    const int npass = lay.hash_bits / 8;
+    // sort_bits is fixed per chunk from its actual record count; the workspace is planned for the bound
+    auto pick_sort_bits = [&](i64 nrec) {
+        int sb = 0;
+        if (ctx->opt_sort_bits >= 0) sb = (int)ctx->opt_sort_bits;
+        else
+            while (sb < 56 && (double)nrec / std::pow(2.0, sb) > 1850.0) sb += 8;
+        return std::min(sb, lay.hash_bits / 8 * 8);
+    };
+    const int npass_max = pick_sort_bits(nmax) / 8;
     const int ppass = (lay.pair_bits + 7) / 8;
     const int spass = (lay.pair_bits + 7) / 8;
     S.hash_bits = lay.hash_bits;
@@ -219,21 +218,23 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
 
     // ---- workspace plan ----
     const i64 R = ws.left() - 8192;
+    // a window of the candidate buffer ends with a whole record's pairs: at most one per other sequence
+    const i64 cslack = n_total + 64;
     i64 ccap = ctx->opt_cand_cap > 0 ? ctx->opt_cand_cap : std::max<i64>(1 << 20, nmax / 2);
     i64 scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity + (ctx->opt_cand_cap > 0 ? ccap : 0));
     i64 ncap = std::max<i64>(nmax, 1);
     u32 P = ctx->opt_force_chunks > 0 ? (u32)ctx->opt_force_chunks : 1;
     if (P > 1) ncap = std::min<i64>(nmax, nmax / P + nmax / (4 * P) + 4096);
-    if (rec_bytes(ncap, npass) + cand_bytes(ccap, ppass) + cand_bytes(scap, spass) > R) {
-        if (ctx->opt_cand_cap <= 0) ccap = std::min<i64>(ccap, std::max<i64>(4096, R / 4 / 17));
+    if (rec_bytes(ncap, npass_max) + cand_bytes(ccap + cslack, ppass) + cand_bytes(scap, spass) > R) {
+        if (ctx->opt_cand_cap <= 0) ccap = std::min<i64>(ccap, std::max<i64>(4096, R / 4 / 17 - cslack));
         scap = std::min<i64>(scap, std::max<i64>(4096, R * 15 / 100 / 17));
-        const i64 rrem = R - cand_bytes(ccap, ppass) - cand_bytes(scap, spass);
+        const i64 rrem = R - cand_bytes(ccap + cslack, ppass) - cand_bytes(scap, spass);
         if (rrem <= 0) return SYMDEL_E_WORKSPACE;
         // largest ncap that fits in rrem (16 B/record + ~0.26 B/record of tile status per pass)
         i64 lo = 0, hi = ncap;
         while (lo < hi) {
             i64 mid = (lo + hi + 1) / 2;
-            if (rec_bytes(mid, npass) <= rrem) lo = mid; else hi = mid - 1;
+            if (rec_bytes(mid, npass_max) <= rrem) lo = mid; else hi = mid - 1;
         }
         ncap = lo;
         if (ncap < 4096) return SYMDEL_E_WORKSPACE;
@@ -241,13 +242,13 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     }
     u64* recA = ws.take<u64>(ncap);
     u64* recB = ws.take<u64>(ncap);
-    void* rec_scratch = ws.take<char>(sd_sort_scratch_bytes(ncap, npass));
-    u64* tile_prefix = ws.take<u64>(2 * sd_emit_tiles(ncap) + 2);
-    u64* emit_lb = nullptr;
-    u64* candA = ws.take<u64>(ccap);
-    u64* candB = ws.take<u64>(ccap);
-    void* cand_scratch = ws.take<char>(sd_sort_scratch_bytes(ccap, ppass));
-    u64* verify_lb = ws.take<u64>(ccap / 256 + 2);
+    void* rec_scratch = ws.take<char>(sd_sort_scratch_bytes(ncap, npass_max));
+    u64* tile_prefix = ws.take<u64>(2 * sd_join_tiles(ncap) + 2);
+    const i64 cphys = ccap + cslack;
+    u64* candA = ws.take<u64>(cphys);
+    u64* candB = ws.take<u64>(cphys);
+    void* cand_scratch = ws.take<char>(sd_sort_scratch_bytes(cphys, ppass));
+    u64* verify_lb = ws.take<u64>(cphys / 256 + 2);
     u64* survA = ws.take<u64>(scap);
     u64* survB = ws.take<u64>(scap);
     void* surv_scratch = ws.take<char>(sd_sort_scratch_bytes(scap, spass));
@@ -284,20 +285,27 @@ restart:
         }
         S.n_records += N;
         if (N == 0) continue;
+        lay.sort_bits = pick_sort_bits(N);
+        S.sort_bits = lay.sort_bits;
+        const int npass = lay.sort_bits / 8;
+        const int sort_begin = lay.id_bits + lay.hash_bits - lay.sort_bits;  // first radix-partitioned bit of a record
         CK(sd_sort_prepare(rec_scratch, N, npass, st));
-        CK(sd_generate(A, B, lay, width, rec_off, recA, sd_sort_hist_ptr(rec_scratch), npass, info, st, &S.n_launches));
+        CK(sd_generate(A, B, lay, width, rec_off, recA, sd_sort_hist_ptr(rec_scratch), sort_begin, npass, info, st,
+                       &S.n_launches));
         CK(sd_sort_hist_scan(rec_scratch, npass, st, &S.n_launches));
         const size_t e1 = tm.mark();
-        // ---- S2: sort (exactly npass onesweep launches between e1 and e2) ----
+        // ---- S2: radix partition on the top sort_bits (exactly npass onesweep launches between e1 and e2) ----
         u64* sorted = nullptr;
-        CK(sd_sort_passes(recA, recB, N, lay.id_bits, npass, rec_scratch, st, &sorted, &S.n_launches));
+        CK(sd_sort_passes(recA, recB, N, sort_begin, npass, ctx->opt_sort_stable ? 1 : 0, rec_scratch, st, &sorted,
+                          &S.n_launches));
         const size_t e2 = tm.mark();
-        // ---- S3a: emit (first window) ----
-        CK(sd_emit(sorted, N, lay, candA, 0, (u64)ccap, 1, tile_prefix, emit_lb, info, st, &S.n_launches));
+        // ---- S3a: join (first window) ----
+        CK(sd_join(sorted, N, lay, candA, (u64)cphys, 0, (u64)ccap, 1, tile_prefix, info, st, &S.n_launches));
         rc = read_info(ctx, info, st);
         if (rc) return rc;
         if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
         const i64 C = (i64)ctx->h_info->n_cand;
+        i64 wend = (i64)ctx->h_info->win_end;
         S.n_candidates += C;
         const size_t e3 = tm.mark();
         tm.span(ST_GEN, e0, e1);
@@ -305,21 +313,27 @@ restart:
         tm.span(ST_EMIT, e2, e3);
         pass_count += npass;
         S.sort_pass_records = N;
-        for (i64 w0 = 0; w0 < C; w0 += ccap) {
-            const i64 nc = std::min<i64>(ccap, C - w0);
+        for (i64 w0 = 0; w0 < C;) {
             const size_t f0 = tm.mark();
-            if (w0 > 0) CK(sd_emit(sorted, N, lay, candA, (u64)w0, (u64)(w0 + ccap), 0, tile_prefix, emit_lb, info, st,
-                                   &S.n_launches));
+            if (w0 > 0) {
+                CK(sd_join(sorted, N, lay, candA, (u64)cphys, (u64)w0, (u64)(w0 + ccap), 0, tile_prefix, info, st,
+                           &S.n_launches));
+                rc = read_info(ctx, info, st);
+                if (rc) return rc;
+                if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+                wend = (i64)ctx->h_info->win_end;
+            }
+            const i64 nc = wend - w0;  // the records that start in [w0, w0 + ccap), whole
+            if (nc <= 0 || nc > cphys) return SYMDEL_E_INTERNAL;
             const size_t f1 = tm.mark();
             // ---- S3b: sort the packed pair ids ----
             CK(sd_sort_prepare(cand_scratch, nc, ppass, st));
             CK(sd_sort_histogram(candA, nc, 0, ppass, cand_scratch, st, &S.n_launches));
             CK(sd_sort_hist_scan(cand_scratch, ppass, st, &S.n_launches));
             u64* csorted = nullptr;
-            CK(sd_sort_passes(candA, candB, nc, 0, ppass, cand_scratch, st, &csorted, &S.n_launches));
+            CK(sd_sort_passes(candA, candB, nc, 0, ppass, 0, cand_scratch, st, &csorted, &S.n_launches));
             const size_t f2 = tm.mark();
-            // ---- S4: unique + verify; survivors appended at n_surv (host-tracked upper bound not needed:
-            // the kernel is given the base through the previous flush's total, read back below) ----
+            // ---- S4: unique + verify; survivors appended at n_surv ----
             CK(sd_verify(csorted, nc, slots, lay, maxlen, survA, (u64)n_surv, (u64)scap, verify_lb, info, st,
                          &S.n_launches));
             rc = read_info(ctx, info, st);
@@ -331,6 +345,7 @@ restart:
             tm.span(ST_DEDUP, f1, f2);
             tm.span(ST_VERIFY, f2, f3);
             ++flushes;
+            w0 = wend;
         }
     }
 
@@ -344,7 +359,7 @@ restart:
             CK(sd_sort_histogram(survA, n_surv, 3, spass, surv_scratch, st, &S.n_launches));
             CK(sd_sort_hist_scan(surv_scratch, spass, st, &S.n_launches));
             u64* ssorted = nullptr;
-            CK(sd_sort_passes(survA, survB, n_surv, 3, spass, surv_scratch, st, &ssorted, &S.n_launches));
+            CK(sd_sort_passes(survA, survB, n_surv, 3, spass, 0, surv_scratch, st, &ssorted, &S.n_launches));
             fin = ssorted;
         }
         CK(sd_finalize(fin, n_surv, lay, flushes > 1 ? 1 : 0, out_i, out_j, out_dist, capacity, final_lb, info, st,
@@ -415,7 +430,7 @@ int run_host(symdel_ctx* ctx, const int8_t* a_seqs, const i64* a_off, i64 n_a, c
     const i64 n_total = n_a + n_b;
     const int npass_max = 7, ppass_max = 8;
     const i64 ccap = std::max<i64>(1 << 20, nmax / 2), scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity);
-    const i64 ws_bytes = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nmax, 1), npass_max) + cand_bytes(ccap, ppass_max) +
+    const i64 ws_bytes = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nmax, 1), npass_max) + cand_bytes(ccap + n_total + 64, ppass_max) +
                          cand_bytes(scap, ppass_max) + 65536;
     const i64 in_bytes = align_up(res_a + 16) + align_up((n_a + 1) * 8) + align_up(res_b + 16) + align_up((n_b + 1) * 8);
     const i64 out_bytes = 3 * align_up(capacity * 4 + 16);
@@ -492,9 +507,15 @@ int symdel_set_option(symdel_ctx* ctx, int option, int64_t value) {
         case SYMDEL_OPT_FORCE_CHUNKS: ctx->opt_force_chunks = value; break;
         case SYMDEL_OPT_CAND_CAPACITY: ctx->opt_cand_cap = value; break;
         case SYMDEL_OPT_HASH_BITS:
-            if (value != 0 && (value % 8 != 0 || value < 8 || value > 56)) return SYMDEL_E_ARG;
+            if (value > 63) return SYMDEL_E_ARG;
             ctx->opt_hash_bits = value;
             break;
+        case SYMDEL_OPT_SORT_BITS:
+            if (value != 255 && (value % 8 != 0 || value > 56)) return SYMDEL_E_ARG;
+            ctx->opt_sort_bits = value == 0 ? -1 : value == 255 ? 0 : value;
+            break;
+        case SYMDEL_OPT_SORT_STABLE: ctx->opt_sort_stable = value != 0; break;
+        case SYMDEL_OPT_SORT_GROUPING: ctx->opt_sort_grouping = value != 0; break;
         case SYMDEL_OPT_NO_THINNING: ctx->opt_no_thinning = value != 0; break;
         case SYMDEL_OPT_GENERAL_GENERATE: ctx->opt_general_gen = value != 0; break;
         case SYMDEL_OPT_SORT_VARIANT:
@@ -539,7 +560,7 @@ int symdel_workspace_bytes(int64_t n_a, int64_t residues_a, int64_t n_b, int64_t
     const u64 vm = vcount_host(max_len, d);
     const i64 nbound = n_total + (max_len ? (i64)(((u64)(residues_a + residues_b) * (vm - 1) + max_len - 1) / max_len) : 0);
     const i64 ccap = std::max<i64>(1 << 20, nbound / 2), scap = std::max<i64>(std::max<i64>(1 << 20, nbound / 4), capacity);
-    *bytes_host = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nbound, 1), 7) + cand_bytes(ccap, 8) + cand_bytes(scap, 8) +
+    *bytes_host = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nbound, 1), 7) + cand_bytes(ccap + n_total + 64, 8) + cand_bytes(scap, 8) +
                   65536;
     return SYMDEL_OK;
 }
@@ -592,7 +613,7 @@ int symdel_stage_sort_u64(symdel_ctx* ctx, uint64_t* keys, uint64_t* tmp, int64_
     CK(sd_sort_histogram(keys, n, begin_bit, npass, workspace, st, nullptr));
     CK(sd_sort_hist_scan(workspace, npass, st, nullptr));
     u64* res = nullptr;
-    CK(sd_sort_passes(keys, tmp, n, begin_bit, npass, workspace, st, &res, nullptr));
+    CK(sd_sort_passes(keys, tmp, n, begin_bit, npass, ctx->opt_sort_grouping ? 0 : 1, workspace, st, &res, nullptr));
     if (res != keys) CK(cudaMemcpyAsync(keys, res, (size_t)n * 8, cudaMemcpyDeviceToDevice, st));
     CK(cudaStreamSynchronize(st));
     return SYMDEL_OK;
@@ -601,8 +622,7 @@ int symdel_stage_sort_u64(symdel_ctx* ctx, uint64_t* keys, uint64_t* tmp, int64_
 int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const int64_t* offsets, int64_t n, int d, int hash_bits,
                           int id_bits, int thinning, uint64_t* records, int64_t records_capacity, int64_t* n_records_host,
                           void* workspace, int64_t workspace_bytes, void* cuda_stream) {
-    if (!ctx || !n_records_host || n < 0 || d < 0 || d > SD_D_MAX || hash_bits < 8 || hash_bits % 8 != 0 ||
-        hash_bits + id_bits > 64 || id_bits < 1)
+    if (!ctx || !n_records_host || n < 0 || d < 0 || d > SD_D_MAX || hash_bits < 1 || hash_bits + id_bits > 64 || id_bits < 1)
         return SYMDEL_E_ARG;
     *n_records_host = 0;
     if (n == 0) return SYMDEL_OK;
@@ -640,7 +660,7 @@ int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const int64_t* of
     const i64 N = (i64)ctx->h_info->n_records;
     *n_records_host = N;
     if (N > records_capacity) return SYMDEL_E_CAPACITY;
-    CK(sd_generate(A, B, lay, width, rec_off, records, hist, hash_bits / 8, info, st, nullptr));
+    CK(sd_generate(A, B, lay, width, rec_off, records, hist, id_bits, 0, info, st, nullptr));
     rc = read_info(ctx, info, st);
     if (rc) return rc;
     if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);

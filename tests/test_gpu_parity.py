@@ -284,6 +284,9 @@ def test_validation_protocol_5000(sd, ctx, oracle, family, d):
     {"FORCE_CHUNKS": 4}, {"FORCE_CHUNKS": 16}, {"CAND_CAPACITY": 4999}, {"HASH_BITS": 8}, {"HASH_BITS": 48},
     {"NO_THINNING": 1}, {"FORCE_CHUNKS": 3, "CAND_CAPACITY": 777, "HASH_BITS": 16}, {"GENERAL_GENERATE": 1},
     {"GENERAL_GENERATE": 1, "FORCE_CHUNKS": 5}, {"SORT_VARIANT": 1}, {"SORT_VARIANT": 3},
+    {"SORT_BITS": 255}, {"SORT_BITS": 8}, {"SORT_BITS": 24}, {"SORT_BITS": 40}, {"SORT_STABLE": 1},
+    {"SORT_BITS": 255, "CAND_CAPACITY": 1500}, {"HASH_BITS": 13, "SORT_BITS": 8},
+    {"SORT_BITS": 8, "HASH_BITS": 12, "CAND_CAPACITY": 100000, "FORCE_CHUNKS": 2},
 ])
 def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
     """P-11: chunk count, candidate-buffer windows, key width and thinning change memory use and
