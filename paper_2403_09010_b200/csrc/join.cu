@@ -11,10 +11,15 @@
 // The records arrive partitioned on their top `sort_bits` hash bits only (S2 stops there): a BUCKET is
 // a maximal range of records agreeing on those bits, a few thousand records by construction.  Equal
 // variants always share a bucket, so the join is local to it: a block loads whole buckets into shared
-// memory, chains the records by the next hash bits (one atomic exchange each) and every record walks
-// its chain for EARLIER records with the same full hash — the remaining sort passes over all records
-// and the read of the sorted array are replaced by one read.  Neither the order of the records inside
-// a bucket nor the order of the buckets matters.
+// memory and
+//   1. filters: every record sets one bit of a "seen" bitmap addressed by the next 16 hash bits and,
+//      if it was already set, the same bit of a "seen twice" bitmap; only records whose "seen twice"
+//      bit is set can have a partner (a few per cent on sparse data) — one atomic per record;
+//   2. compacts those records, in position order, into a list;
+//   3. chains the listed records by further hash bits (one atomic exchange each) and lets each walk its
+//      chain for EARLIER records with the same full hash.
+// The remaining sort passes over all records and the read of the sorted array are replaced by one read.
+// Neither the order of the records inside a bucket nor the order of the buckets matters.
 //
 // Work split: tile t owns the buckets that START in [t*T, (t+1)*T).  It loads T + slack records, finds
 // the first bucket boundary at or after each end of its range and joins what lies between.  A region
@@ -28,11 +33,15 @@
 // the overhang — and reports the end of what it wrote in info->win_end, where the next round starts.
 #include "kernels.h"
 
+
 namespace {
 
-constexpr int JN_THREADS = 512, JN_T = 4096, JN_CAP = 6144, JN_SLOT_BITS = 13, JN_SLOTS = 1 << JN_SLOT_BITS;
+constexpr int JN_THREADS = 512, JN_NW = JN_THREADS / 32, JN_T = 4096, JN_CAP = 6144;
+constexpr int JN_IT = JN_CAP / JN_THREADS;                     // strided iterations that cover a full window
+constexpr int JN_SLOT_BITS = 12, JN_SLOTS = 1 << JN_SLOT_BITS;  // chain heads
+constexpr int JN_BM_BITS = 16, JN_BM_WORDS = (1 << JN_BM_BITS) / 32;
 constexpr u32 JN_NIL = 0xffffu, JN_NONE = 0xffffffffu;
-static_assert(JN_CAP < 0xffff && JN_CAP % JN_THREADS == 0 && JN_CAP / JN_THREADS <= 32, "node index / nzmask width");
+static_assert(JN_CAP < 0xffff && JN_CAP % JN_THREADS == 0 && JN_IT <= 32, "node index / nzmask width");
 
 struct JoinParams {
     const u64* rec;
@@ -40,7 +49,7 @@ struct JoinParams {
     u64 topmask;  // the radix-partitioned bits: a bucket = maximal range agreeing on them (0: one bucket)
     u64 hlim;     // 1 << id_bits: same hash <=> (x ^ y) < hlim
     u64 idmask, n_a;
-    int slot_shift, tag_shift, b_bits, cross;
+    int bm_shift, slot_shift, b_bits, cross;
     u64* cand;
     u64 cand_cap;  // physical slots of cand
     u64 win_lo, win_hi;
@@ -62,16 +71,25 @@ __device__ __forceinline__ bool jn_pair(u64 x, u64 y, const JoinParams& P, u64& 
     return true;
 }
 
+struct JoinSmem {
+    u64 rec[JN_CAP + 2];     // [0] = record before the window, [1 + r] = record sb + r
+    u32 bit_a[JN_BM_WORDS];  // seen
+    u32 bit_b[JN_BM_WORDS];  // seen twice
+    u32 head[JN_SLOTS];      // chain heads (window position of the last listed record of the slot)
+    unsigned short next[JN_CAP];
+    unsigned short list[JN_CAP];  // window positions of the records that may have a partner, ascending
+    u64 wsum[JN_NW];
+    u64 excl;
+    u32 wcnt[JN_NW];
+    u32 lo, hi;
+};
+
 __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
     extern __shared__ __align__(16) unsigned char jn_smem[];
-    u64* s_rec = reinterpret_cast<u64*>(jn_smem);  // [0] = record before the window, [1 + r] = record sb + r
-    u32* s_head = reinterpret_cast<u32*>(s_rec + JN_CAP + 2);
-    u32* s_node = s_head + JN_SLOTS;  // per record: tag << 16 | next
-    __shared__ u32 s_lo, s_hi;
-    __shared__ u64 s_wsum[JN_THREADS / 32];
-    __shared__ u64 s_excl;
+    JoinSmem& S = *reinterpret_cast<JoinSmem*>(jn_smem);
 
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 lane_lt = (1u << lane) - 1u;
     const u32 tile = blockIdx.x;
     if (!P.first_round) {
         const u64 lo = P.tile_prefix[2 * tile], cnt = P.tile_prefix[2 * tile + 1];
@@ -84,36 +102,90 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
     // loads records [sb - 1, sb + CAP] (one before, one lookahead) and returns the usable count W
     auto load = [&](u64 sb) -> u32 {
         const u32 cnt = (u32)min((u64)(JN_CAP + 1), N - sb);
-        for (u32 r = tid; r < cnt; r += JN_THREADS) s_rec[1 + r] = P.rec[sb + r];
-        if (tid == 0) s_rec[0] = sb > 0 ? P.rec[sb - 1] : 0ull;
+        for (u32 r = tid; r < cnt; r += JN_THREADS) S.rec[1 + r] = P.rec[sb + r];
+        if (tid == 0) S.rec[0] = sb > 0 ? P.rec[sb - 1] : 0ull;
         return min(cnt, (u32)JN_CAP);
     };
     // position sb + r starts a bucket (r in [0, W]; position N counts as a boundary)
     auto isb = [&](u64 sb, u32 r) -> bool {
         const u64 g = sb + r;
-        return g == 0 || g == N || ((s_rec[r] ^ s_rec[1 + r]) & P.topmask) != 0;
+        return g == 0 || g == N || ((S.rec[r] ^ S.rec[1 + r]) & P.topmask) != 0;
     };
-    auto build = [&](u32 r0, u32 r1) {
+    auto slot_of = [&](u64 x) -> u32 { return (u32)(x >> P.slot_shift) & (JN_SLOTS - 1); };
+
+    // Lists the window positions in [r0, r1) that may have a partner (filter: only those whose "seen
+    // twice" bit is set; else all), ascending, and chains the listed records.  Every warp owns a
+    // contiguous span, so the list order is the position order whatever the timing.
+    auto prepare = [&](u32 r0, u32 r1, bool filter) -> u32 {
         for (u32 i = tid; i < JN_SLOTS / 4; i += JN_THREADS)
-            reinterpret_cast<uint4*>(s_head)[i] = make_uint4(JN_NIL, JN_NIL, JN_NIL, JN_NIL);
+            reinterpret_cast<uint4*>(S.head)[i] = make_uint4(JN_NIL, JN_NIL, JN_NIL, JN_NIL);
+        if (filter)
+            for (u32 i = tid; i < 2 * JN_BM_WORDS / 4; i += JN_THREADS)
+                reinterpret_cast<uint4*>(S.bit_a)[i] = make_uint4(0u, 0u, 0u, 0u);  // bit_a and bit_b are adjacent
         __syncthreads();
-        for (u32 r = r0 + tid; r < r1; r += JN_THREADS) {
-            const u64 x = s_rec[1 + r];
-            const u32 prev = atomicExch(&s_head[(u32)(x >> P.slot_shift) & (JN_SLOTS - 1)], r);
-            s_node[r] = (((u32)(x >> P.tag_shift) & 0xffffu) << 16) | prev;
+        const u32 span = (r1 - r0 + JN_THREADS - 1) / JN_THREADS * 32;  // per warp, a multiple of 32, <= 32 * JN_IT
+        const u32 wbeg = r0 + warp * span;
+        u32 bal[JN_IT];
+        u32 cnt = 0;
+        if (filter) {
+            u32 bm[JN_IT];
+#pragma unroll
+            for (int it = 0; it < JN_IT; ++it) {
+                const u32 r = wbeg + it * 32 + lane;
+                bm[it] = JN_NONE;
+                if ((u32)(it * 32) < span && r < r1) {
+                    const u32 b = (u32)(S.rec[1 + r] >> P.bm_shift) & ((1u << JN_BM_BITS) - 1u);
+                    bm[it] = b;
+                    const u32 bit = 1u << (b & 31u);
+                    if (atomicOr(&S.bit_a[b >> 5], bit) & bit) atomicOr(&S.bit_b[b >> 5], bit);
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int it = 0; it < JN_IT; ++it) {
+                const bool c = bm[it] != JN_NONE && ((S.bit_b[bm[it] >> 5] >> (bm[it] & 31u)) & 1u);
+                bal[it] = __ballot_sync(SD_FULL, c);
+                cnt += __popc(bal[it]);
+            }
+        } else {
+#pragma unroll
+            for (int it = 0; it < JN_IT; ++it) {
+                const bool c = (u32)(it * 32) < span && wbeg + it * 32 + lane < r1;
+                bal[it] = __ballot_sync(SD_FULL, c);
+                cnt += __popc(bal[it]);
+            }
+        }
+        if (lane == 0) S.wcnt[warp] = cnt;
+        __syncthreads();
+        u32 base = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < JN_NW; ++w) {
+            const u32 c = S.wcnt[w];
+            if ((u32)w < warp) base += c;
+            total += c;
+        }
+#pragma unroll
+        for (int it = 0; it < JN_IT; ++it) {
+            if ((bal[it] >> lane) & 1u) S.list[base + __popc(bal[it] & lane_lt)] = (unsigned short)(wbeg + it * 32 + lane);
+            base += __popc(bal[it]);
         }
         __syncthreads();
+        for (u32 i = tid; i < total; i += JN_THREADS) {
+            const u32 r = S.list[i];
+            S.next[r] = (unsigned short)atomicExch(&S.head[slot_of(S.rec[1 + r])], r);
+        }
+        __syncthreads();
+        return total;
     };
+
     u64 wend = 0;
-    // pairs of record x with the table records at chunk positions < lim; returns their number and, when
-    // `store`, writes them from cand[at]
+    // pairs of record x with the chained records at window positions < lim; returns their number and,
+    // when `store`, writes them from cand[at]
     auto walk = [&](u64 x, u32 lim, bool store, u64 at) -> u32 {
-        const u32 tag = (u32)(x >> P.tag_shift) & 0xffffu;
         u32 c = 0;
-        for (u32 j = s_head[(u32)(x >> P.slot_shift) & (JN_SLOTS - 1)]; j != JN_NIL;) {
-            const u32 w = s_node[j];
-            if (j < lim && (w >> 16) == tag) {
-                const u64 y = s_rec[1 + j];
+        for (u32 j = S.head[slot_of(x)]; j != JN_NIL; j = S.next[j]) {
+            if (j < lim) {
+                const u64 y = S.rec[1 + j];
                 u64 packed;
                 if ((x ^ y) < P.hlim && jn_pair(x, y, P, packed)) {
                     if (store) {
@@ -123,7 +195,6 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
                     ++c;
                 }
             }
-            j = w & 0xffffu;
         }
         return c;
     };
@@ -136,7 +207,7 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
     };
 
     // ---- first chunk: the window of this tile; which buckets start in it? ----
-    if (tid == 0) s_lo = JN_NONE, s_hi = JN_NONE;
+    if (tid == 0) S.lo = JN_NONE, S.hi = JN_NONE;
     u32 W = load(g0);
     __syncthreads();
     {
@@ -148,17 +219,17 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
             }
         mlo = __reduce_min_sync(SD_FULL, mlo);
         mhi = __reduce_min_sync(SD_FULL, mhi);
-        if (lane == 0 && mlo != JN_NONE) atomicMin(&s_lo, mlo);
-        if (lane == 0 && mhi != JN_NONE) atomicMin(&s_hi, mhi);
+        if (lane == 0 && mlo != JN_NONE) atomicMin(&S.lo, mlo);
+        if (lane == 0 && mhi != JN_NONE) atomicMin(&S.hi, mhi);
     }
     __syncthreads();
-    const u32 lo = s_lo, hi0 = s_hi;
+    const u32 lo = S.lo, hi0 = S.hi;
     if (lo == JN_NONE) {  // no bucket starts here
         if (P.first_round && tid == 0) P.tile_prefix[2 * tile] = 0, P.tile_prefix[2 * tile + 1] = 0;
         return;
     }
     const bool single = hi0 != JN_NONE;  // the whole region sits in shared memory
-    u32 nzmask = 0;                      // single: which of this thread's records have pairs
+    u32 nzmask = 0;                      // single: which of this thread's listed records have pairs
 
     u64 flat = 0;
     for (int phase = 0; phase < 2; ++phase) {
@@ -169,7 +240,7 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
         for (bool first = true;; first = false) {
             if (!first || (write && !single)) {  // an oversized region: (re)load the chunk that starts at sb
                 __syncthreads();
-                if (tid == 0) s_hi = JN_NONE;
+                if (tid == 0) S.hi = JN_NONE;
                 W = load(sb);
                 __syncthreads();
                 if (!first) {
@@ -177,29 +248,33 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
                     for (u32 r = 1 + tid; r <= W; r += JN_THREADS)
                         if (isb(sb, r)) mhi = min(mhi, r);
                     mhi = __reduce_min_sync(SD_FULL, mhi);
-                    if (lane == 0 && mhi != JN_NONE) atomicMin(&s_hi, mhi);
+                    if (lane == 0 && mhi != JN_NONE) atomicMin(&S.hi, mhi);
                     __syncthreads();
-                    last = s_hi != JN_NONE;
+                    last = S.hi != JN_NONE;
                     r0 = 0;
-                    r1 = last ? s_hi : (u32)JN_CAP;
+                    r1 = last ? S.hi : (u32)JN_CAP;
                 }
             }
-            if (!(single && write)) build(r0, r1);
             // ---- the chunk with itself ----
             if (single && write) {
-                for (u32 m = nzmask, k = 0; m; m >>= 1, ++k) {
-                    const u32 r = r0 + tid + k * JN_THREADS;
-                    if (m & 1u) visit(s_rec[1 + r], r, true, flat);
-                }
+                for (u32 m = nzmask, k = 0; m; m >>= 1, ++k)
+                    if (m & 1u) {
+                        const u32 r = S.list[tid + k * JN_THREADS];
+                        visit(S.rec[1 + r], r, true, flat);
+                    }
             } else {
+                // the filter needs whole buckets in the table: not when later records are streamed through it
+                const u32 nl = prepare(r0, r1, single);
                 u32 k = 0;
-                for (u32 r = r0 + tid; r < r1; r += JN_THREADS, ++k)
-                    if (visit(s_rec[1 + r], r, write, flat) && single) nzmask |= 1u << k;
+                for (u32 i = tid; i < nl; i += JN_THREADS, ++k) {
+                    const u32 r = S.list[i];
+                    if (visit(S.rec[1 + r], r, write, flat) && single) nzmask |= 1u << k;
+                }
             }
             if (last) break;
             // ---- the rest of the chunk's last bucket against the chunk ----
             if (!isb(sb, JN_CAP)) {
-                const u64 lastx = s_rec[JN_CAP];
+                const u64 lastx = S.rec[JN_CAP];
                 for (u64 q0 = sb + JN_CAP;; q0 += JN_THREADS) {
                     const u64 q = q0 + tid;
                     u64 x = 0;
@@ -224,12 +299,12 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
             const u64 t = __shfl_up_sync(SD_FULL, inc, o);
             if (lane >= (u32)o) inc += t;
         }
-        if (lane == 31) s_wsum[warp] = inc;
+        if (lane == 31) S.wsum[warp] = inc;
         __syncthreads();
         u64 carry = 0, T = 0;
 #pragma unroll
-        for (int w = 0; w < JN_THREADS / 32; ++w) {
-            const u64 c = s_wsum[w];
+        for (int w = 0; w < JN_NW; ++w) {
+            const u64 c = S.wsum[w];
             if ((u32)w < warp) carry += c;
             T += c;
         }
@@ -246,10 +321,10 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
             } else {
                 excl = P.tile_prefix[2 * tile];
             }
-            s_excl = excl;
+            S.excl = excl;
         }
         __syncthreads();
-        flat = s_excl + carry + inc - tsum;  // flat index of this thread's first pair
+        flat = S.excl + carry + inc - tsum;  // flat index of this thread's first pair
         if (single && (tsum == 0 || flat + tsum <= P.win_lo || flat >= P.win_hi)) break;  // nothing of mine in the window
     }
 #pragma unroll
@@ -265,7 +340,7 @@ cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* c
                     int first_round, u64* tile_prefix, DevInfo* info, cudaStream_t st, i64* launches) {
     const i64 tiles = sd_join_tiles(n_records);
     if (tiles == 0) return cudaSuccess;
-    constexpr size_t smem = (size_t)(JN_CAP + 2) * 8 + (size_t)JN_SLOTS * 4 + (size_t)JN_CAP * 4;
+    constexpr size_t smem = sizeof(JoinSmem);
     static bool attr_set = false;
     cudaError_t e;
     if (!attr_set) {
@@ -282,10 +357,10 @@ cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* c
     P.hlim = 1ull << lay.id_bits;
     P.idmask = P.hlim - 1ull;
     P.n_a = (u64)lay.n_a;
-    // chain slot = the hash bits right below the partitioned ones, tag = the 16 bits below those (both
-    // clamped to the hash field: with few hash bits they overlap the bucket bits, which is harmless)
-    P.slot_shift = std::max(lay.id_bits, top - sort_bits - JN_SLOT_BITS);
-    P.tag_shift = std::max(lay.id_bits, P.slot_shift - 16);
+    // bitmap position = the hash bits right below the partitioned ones, chain slot = the bits below those
+    // (both clamped to the hash field: with few hash bits they overlap, which only lengthens chains)
+    P.bm_shift = std::max(lay.id_bits, top - sort_bits - JN_BM_BITS);
+    P.slot_shift = std::max(lay.id_bits, P.bm_shift - JN_SLOT_BITS);
     P.b_bits = lay.b_bits;
     P.cross = lay.cross;
     P.cand = cand;
