@@ -73,7 +73,7 @@ typedef struct {
     int32_t hash_bits;     /* hash bits carried per record (64 - id_bits unless narrowed) */
     int32_t id_bits;       /* id bits per record */
     int32_t sort_bits;     /* top hash bits radix-partitioned by S2 (8 per onesweep pass); the join compares the rest */
-    int32_t pad_;
+    int32_t join_general;  /* chunks whose join ran the general (windowed) kernel instead of the fast one */
     float ms_prepare, ms_generate, ms_sort, ms_emit, ms_dedup, ms_verify, ms_total; /* CUDA-event times; 0 unless SYMDEL_OPT_TIMING is set */
     float ms_sort_pass_avg; /* average duration of one onesweep pass over the variant records */
     int64_t sort_pass_records; /* records moved by one such pass */
@@ -90,6 +90,7 @@ enum {
     SYMDEL_OPT_SORT_VARIANT = 6,  /* [0] tile shape of the onesweep kernel (process-wide tuning hook; results are identical) */
     SYMDEL_OPT_SORT_BITS = 8,     /* [0] 0 = automatic; 8..56 (multiple of 8): top hash bits that S2 radix-partitions; 255 = none (one bucket: the join chunks it) */
     SYMDEL_OPT_SORT_STABLE = 9,   /* [0] 1: every S2 pass takes the stable (ties keep input order) tile path (test hook; results are identical) */
+    SYMDEL_OPT_JOIN_GENERAL = 11, /* [0] 1: always run the general join kernel (windowed output, chunked buckets) instead of trying the fast one first (test hook; results are identical) */
     SYMDEL_OPT_SORT_GROUPING = 10 /* [0] 1: symdel_stage_sort_u64 sorts keys only: ties land in arbitrary order (the mode the pipeline uses) */
 };
 

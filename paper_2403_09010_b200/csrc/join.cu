@@ -332,23 +332,197 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
     if (lane == 0 && wend) atomicMax((unsigned long long*)&P.info->win_end, (unsigned long long)wend);
 }
 
+
+// =================================================================================================
+// Fast path: k_join_fast.  Same join, for the common case — every pair of the call fits the candidate
+// buffer (one window) and no tile lists more than JF_LMAX records.  It keeps NO copy of the tile in
+// shared memory: a tile streams its records twice through registers (the second time from L1/L2),
+//   1. "seen" / "seen twice" bitmaps as above (one shared-memory atomic per record),
+//   2. the records whose "seen twice" bit is set (a few per cent on sparse data) are appended to a
+//      shared-memory list,
+//   3. the listed records are chained by further hash bits; each walks the part of its chain that was
+//      inserted BEFORE it (an exchange-built chain is in reverse insertion order), so every unordered
+//      pair is met exactly once,
+//   4. count, block scan, ONE global atomic per tile claims the output range, second walk writes.
+// No bucket boundary is searched: tile t owns the buckets that start in [t*T, (t+1)*T), i.e. the
+// records of its range whose partitioned bits differ from those of record t*T - 1, plus the records
+// after the range that continue its last bucket (streamed until the partitioned bits change).
+// The order of the candidates is arbitrary (they are sorted next).  If the claim runs past the
+// buffer or a list overflows, the tile raises info->join_fallback and the host reruns the general
+// kernel above, which windows the output and chunks oversized buckets.
+constexpr int JF_THREADS = 512, JF_NW = JF_THREADS / 32, JF_IT = 8, JF_T = JF_THREADS * JF_IT;
+constexpr int JF_LMAX = 6144, JF_LIT = JF_LMAX / JF_THREADS;
+constexpr int JF_SLOT_BITS = 12, JF_SLOTS = 1 << JF_SLOT_BITS;
+constexpr int JF_BM_BITS = 16, JF_BM_WORDS = (1 << JF_BM_BITS) / 32;
+static_assert(JF_T == JN_T, "both kernels share sd_join_tiles");
+static_assert(JF_LMAX < 0xffff && JF_LIT <= 16, "node index width / nzmask width");
+
+struct JoinFastSmem {
+    u64 list[JF_LMAX];
+    u32 bit_a[JF_BM_WORDS];
+    u32 bit_b[JF_BM_WORDS];
+    u32 head[JF_SLOTS];
+    unsigned short next[JF_LMAX];
+    u32 wsum[JF_NW];
+    u32 nlist;
+    u64 base;
+};
+
+__global__ void __launch_bounds__(JF_THREADS, 2) k_join_fast(const JoinParams P) {
+    extern __shared__ __align__(16) unsigned char jn_smem[];
+    JoinFastSmem& S = *reinterpret_cast<JoinFastSmem*>(jn_smem);
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 lane_lt = (1u << lane) - 1u;
+    const u64 N = P.n;
+    const u64 g0 = (u64)blockIdx.x * JF_T;
+    const u64 E = min(g0 + (u64)JF_T, N);
+    const u64 v0 = g0 > 0 ? (P.rec[g0 - 1] & P.topmask) : 0ull;  // bucket of the record before the range
+    const u64 v1 = P.rec[E - 1] & P.topmask;                     // bucket that may continue after the range
+    if (g0 > 0 && v1 == v0) return;                              // no bucket starts here
+
+    for (u32 i = tid; i < 2 * JF_BM_WORDS / 4; i += JF_THREADS)
+        reinterpret_cast<uint4*>(S.bit_a)[i] = make_uint4(0u, 0u, 0u, 0u);  // bit_a and bit_b are adjacent
+    for (u32 i = tid; i < JF_SLOTS / 4; i += JF_THREADS)
+        reinterpret_cast<uint4*>(S.head)[i] = make_uint4(JN_NIL, JN_NIL, JN_NIL, JN_NIL);
+    if (tid == 0) S.nlist = 0;
+
+    // ---- the range, two records per 16-byte load: thread holds records 2*(tid + k*THREADS) + {0, 1} ----
+    u64 x[JF_IT];
+    u32 mine = 0;
+    const bool full = E - g0 == (u64)JF_T;
+#pragma unroll
+    for (int k = 0; k < JF_IT / 2; ++k) {
+        const u32 r = 2 * (tid + k * JF_THREADS);
+        if (full || g0 + r + 1 < E) {
+            const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(P.rec + g0 + r);
+            x[2 * k] = t.x, x[2 * k + 1] = t.y;
+            mine |= 3u << (2 * k);
+        } else if (g0 + r < E) {
+            x[2 * k] = P.rec[g0 + r], x[2 * k + 1] = 0;
+            mine |= 1u << (2 * k);
+        } else {
+            x[2 * k] = x[2 * k + 1] = 0;
+        }
+    }
+    if (g0 > 0) {
+#pragma unroll
+        for (int k = 0; k < JF_IT; ++k)
+            if ((x[k] & P.topmask) == v0) mine &= ~(1u << k);
+    }
+    __syncthreads();
+    auto bm_of = [&](u64 y) -> u32 { return (u32)(y >> P.bm_shift) & ((1u << JF_BM_BITS) - 1u); };
+    auto mark = [&](u64 y) {
+        const u32 b = bm_of(y), bit = 1u << (b & 31u);
+        if (atomicOr(&S.bit_a[b >> 5], bit) & bit) atomicOr(&S.bit_b[b >> 5], bit);
+    };
+    // ---- 1. bitmaps ----
+#pragma unroll
+    for (int k = 0; k < JF_IT; ++k)
+        if ((mine >> k) & 1u) mark(x[k]);
+    // the records after the range that continue its last bucket; every thread sees the same stride ends
+    for (u64 q0 = E; q0 < N; q0 += JF_THREADS) {
+        const u64 q = q0 + tid;
+        if (q < N) {
+            const u64 y = P.rec[q];
+            if ((y & P.topmask) == v1) mark(y);
+        }
+        if ((P.rec[min(q0 + JF_THREADS, N) - 1] & P.topmask) != v1) break;
+    }
+    __syncthreads();
+    // ---- 2. list the records whose "seen twice" bit is set ----
+    auto listed = [&](u64 y) -> bool {
+        const u32 b = bm_of(y);
+        return (S.bit_b[b >> 5] >> (b & 31u)) & 1u;
+    };
+    auto append = [&](bool c, u64 y) {
+        const u32 bal = __ballot_sync(SD_FULL, c);
+        if (bal == 0) return;
+        u32 at = 0;
+        if (lane == 0) at = atomicAdd(&S.nlist, (u32)__popc(bal));
+        at = __shfl_sync(SD_FULL, at, 0) + __popc(bal & lane_lt);
+        if (c && at < (u32)JF_LMAX) S.list[at] = y;
+    };
+#pragma unroll
+    for (int k = 0; k < JF_IT; ++k) append(((mine >> k) & 1u) && listed(x[k]), x[k]);
+    for (u64 q0 = E; q0 < N; q0 += JF_THREADS) {
+        const u64 q = q0 + tid;
+        u64 y = 0;
+        bool c = false;
+        if (q < N) {
+            y = P.rec[q];
+            c = (y & P.topmask) == v1 && listed(y);
+        }
+        append(c, y);
+        if ((P.rec[min(q0 + JF_THREADS, N) - 1] & P.topmask) != v1) break;
+    }
+    __syncthreads();
+    const u32 nl = S.nlist;
+    if (nl == 0) return;
+    if (nl > (u32)JF_LMAX) {
+        if (tid == 0) atomicOr(&P.info->join_fallback, 1u);
+        return;
+    }
+    // ---- 3. chains ----
+    auto slot_of = [&](u64 y) -> u32 { return (u32)(y >> P.slot_shift) & (JF_SLOTS - 1); };
+    for (u32 i = tid; i < nl; i += JF_THREADS) S.next[i] = (unsigned short)atomicExch(&S.head[slot_of(S.list[i])], i);
+    __syncthreads();
+    // ---- 4. count, claim, write ----
+    u32 cnt = 0, nzmask = 0;
+    {
+        u32 k = 0;
+        for (u32 i = tid; i < nl; i += JF_THREADS, ++k) {
+            const u64 y = S.list[i];
+            u32 c = 0;
+            for (u32 j = S.next[i]; j != JN_NIL; j = S.next[j]) {
+                const u64 z = S.list[j];
+                u64 packed;
+                if ((y ^ z) < P.hlim && jn_pair(y, z, P, packed)) ++c;
+            }
+            if (c) nzmask |= 1u << k;
+            cnt += c;
+        }
+    }
+    u32 inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const u32 t = __shfl_up_sync(SD_FULL, inc, o);
+        if (lane >= (u32)o) inc += t;
+    }
+    if (lane == 31) S.wsum[warp] = inc;
+    __syncthreads();
+    u32 carry = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < JF_NW; ++w) {
+        const u32 c = S.wsum[w];
+        if ((u32)w < warp) carry += c;
+        total += c;
+    }
+    if (total == 0) return;
+    if (tid == 0) {
+        const u64 base = (u64)atomicAdd((unsigned long long*)&P.info->n_cand, (unsigned long long)total);
+        if (base + total > P.win_hi) atomicOr(&P.info->join_fallback, 2u);  // does not fit the window: nothing is written
+        S.base = base;
+    }
+    __syncthreads();
+    u64 at = S.base + carry + inc - cnt;
+    if (S.base + total > P.win_hi) return;
+    for (u32 m = nzmask, k = 0; m; m >>= 1, ++k)
+        if (m & 1u) {
+            const u32 i = tid + k * JF_THREADS;
+            const u64 y = S.list[i];
+            for (u32 j = S.next[i]; j != JN_NIL; j = S.next[j]) {
+                const u64 z = S.list[j];
+                u64 packed;
+                if ((y ^ z) < P.hlim && jn_pair(y, z, P, packed)) P.cand[at++] = packed;
+            }
+        }
+}
+
 }  // namespace
 
 i64 sd_join_tiles(i64 n_records) { return (n_records + JN_T - 1) / JN_T; }
 
-cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 cand_cap, u64 win_lo, u64 win_hi,
-                    int first_round, u64* tile_prefix, DevInfo* info, cudaStream_t st, i64* launches) {
-    const i64 tiles = sd_join_tiles(n_records);
-    if (tiles == 0) return cudaSuccess;
-    constexpr size_t smem = sizeof(JoinSmem);
-    static bool attr_set = false;
-    cudaError_t e;
-    if (!attr_set) {
-        if ((e = cudaFuncSetAttribute(k_join, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        attr_set = true;
-    }
-    if (first_round && (e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
-    if ((e = cudaMemsetAsync(&info->win_end, 0, sizeof(u64), st)) != cudaSuccess) return e;
+static JoinParams jn_params(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 cand_cap, DevInfo* info) {
     JoinParams P{};
     P.rec = records;
     P.n = (u64)n_records;
@@ -365,11 +539,51 @@ cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* c
     P.cross = lay.cross;
     P.cand = cand;
     P.cand_cap = cand_cap;
+    P.info = info;
+    return P;
+}
+
+// Fast path: all pairs in one window of `window` slots, arbitrary order; info->n_cand = total,
+// info->join_fallback != 0 if the general kernel has to redo the join (nothing usable was written).
+cudaError_t sd_join_fast(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, DevInfo* info,
+                         cudaStream_t st, i64* launches) {
+    const i64 tiles = sd_join_tiles(n_records);
+    if (tiles == 0) return cudaSuccess;
+    constexpr size_t smem = sizeof(JoinFastSmem);
+    static bool attr_set = false;
+    cudaError_t e;
+    if (!attr_set) {
+        if ((e = cudaFuncSetAttribute(k_join_fast, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        attr_set = true;
+    }
+    if ((e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(&info->join_fallback, 0, sizeof(u32), st)) != cudaSuccess) return e;
+    JoinParams P = jn_params(records, n_records, lay, cand, window, info);
+    P.win_lo = 0;
+    P.win_hi = window;
+    k_join_fast<<<(unsigned)tiles, JF_THREADS, smem, st>>>(P);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 cand_cap, u64 win_lo, u64 win_hi,
+                    int first_round, u64* tile_prefix, DevInfo* info, cudaStream_t st, i64* launches) {
+    const i64 tiles = sd_join_tiles(n_records);
+    if (tiles == 0) return cudaSuccess;
+    constexpr size_t smem = sizeof(JoinSmem);
+    static bool attr_set = false;
+    cudaError_t e;
+    if (!attr_set) {
+        if ((e = cudaFuncSetAttribute(k_join, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        attr_set = true;
+    }
+    if (first_round && (e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(&info->win_end, 0, sizeof(u64), st)) != cudaSuccess) return e;
+    JoinParams P = jn_params(records, n_records, lay, cand, cand_cap, info);
     P.win_lo = win_lo;
     P.win_hi = win_hi;
     P.first_round = first_round;
     P.tile_prefix = tile_prefix;
-    P.info = info;
     k_join<<<(unsigned)tiles, JN_THREADS, smem, st>>>(P);
     if (launches) ++*launches;
     return cudaGetLastError();

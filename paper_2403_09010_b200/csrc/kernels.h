@@ -69,6 +69,11 @@ i64 sd_join_tiles(i64 n_records);
 cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 cand_cap, u64 win_lo, u64 win_hi,
                     int first_round, u64* tile_prefix, DevInfo* info, cudaStream_t st, i64* launches);
 
+// Fast path of the join (one window, arbitrary candidate order).  info->n_cand = number of pairs;
+// info->join_fallback != 0: redo with sd_join (the pairs exceed `window` or a tile overflowed its list).
+cudaError_t sd_join_fast(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, DevInfo* info,
+                         cudaStream_t st, i64* launches);
+
 // ---- verify.cu ----------------------------------------------------------------------------------
 i64 sd_verify_tiles(i64 n);
 // packed bit-plane table of all sequences (A then B): 32 B (maxlen <= 32) or 48 B per sequence

@@ -31,7 +31,7 @@ struct symdel_ctx {
     symdel_stats stats{};
     int opt_timing = 0;
     i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0, opt_general_gen = 0;
-    i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0;
+    i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0, opt_join_general = 0;
     DevInfo* h_info = nullptr;  // pinned
     void* arena = nullptr;      // device arena of the *_host entry points
     size_t arena_bytes = 0;
@@ -299,11 +299,23 @@ restart:
         CK(sd_sort_passes(recA, recB, N, sort_begin, npass, ctx->opt_sort_stable ? 1 : 0, rec_scratch, st, &sorted,
                           &S.n_launches));
         const size_t e2 = tm.mark();
-        // ---- S3a: join (first window) ----
-        CK(sd_join(sorted, N, lay, candA, (u64)cphys, 0, (u64)ccap, 1, tile_prefix, info, st, &S.n_launches));
-        rc = read_info(ctx, info, st);
-        if (rc) return rc;
-        if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+        // ---- S3a: join (first window): the fast kernel when everything fits one window, else the general one ----
+        bool general = ctx->opt_join_general != 0;
+        if (!general) {
+            CK(sd_join_fast(sorted, N, lay, candA, (u64)ccap, info, st, &S.n_launches));
+            rc = read_info(ctx, info, st);
+            if (rc) return rc;
+            if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+            general = ctx->h_info->join_fallback != 0;
+            ctx->h_info->win_end = ctx->h_info->n_cand;
+        }
+        if (general) {
+            ++S.join_general;
+            CK(sd_join(sorted, N, lay, candA, (u64)cphys, 0, (u64)ccap, 1, tile_prefix, info, st, &S.n_launches));
+            rc = read_info(ctx, info, st);
+            if (rc) return rc;
+            if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+        }
         const i64 C = (i64)ctx->h_info->n_cand;
         i64 wend = (i64)ctx->h_info->win_end;
         S.n_candidates += C;
@@ -516,6 +528,7 @@ int symdel_set_option(symdel_ctx* ctx, int option, int64_t value) {
             break;
         case SYMDEL_OPT_SORT_STABLE: ctx->opt_sort_stable = value != 0; break;
         case SYMDEL_OPT_SORT_GROUPING: ctx->opt_sort_grouping = value != 0; break;
+        case SYMDEL_OPT_JOIN_GENERAL: ctx->opt_join_general = value != 0; break;
         case SYMDEL_OPT_NO_THINNING: ctx->opt_no_thinning = value != 0; break;
         case SYMDEL_OPT_GENERAL_GENERATE: ctx->opt_general_gen = value != 0; break;
         case SYMDEL_OPT_SORT_VARIANT:

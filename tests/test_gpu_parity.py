@@ -281,12 +281,13 @@ def test_validation_protocol_5000(sd, ctx, oracle, family, d):
 
 
 @pytest.mark.parametrize("opts", [
-    {"FORCE_CHUNKS": 4}, {"FORCE_CHUNKS": 16}, {"CAND_CAPACITY": 4999}, {"HASH_BITS": 8}, {"HASH_BITS": 48},
+    {}, {"FORCE_CHUNKS": 4}, {"FORCE_CHUNKS": 16}, {"CAND_CAPACITY": 4999}, {"HASH_BITS": 8}, {"HASH_BITS": 48},
     {"NO_THINNING": 1}, {"FORCE_CHUNKS": 3, "CAND_CAPACITY": 777, "HASH_BITS": 16}, {"GENERAL_GENERATE": 1},
     {"GENERAL_GENERATE": 1, "FORCE_CHUNKS": 5}, {"SORT_VARIANT": 1}, {"SORT_VARIANT": 3},
     {"SORT_BITS": 255}, {"SORT_BITS": 8}, {"SORT_BITS": 24}, {"SORT_BITS": 40}, {"SORT_STABLE": 1},
     {"SORT_BITS": 255, "CAND_CAPACITY": 1500}, {"HASH_BITS": 13, "SORT_BITS": 8},
     {"SORT_BITS": 8, "HASH_BITS": 12, "CAND_CAPACITY": 100000, "FORCE_CHUNKS": 2},
+    {"JOIN_GENERAL": 1}, {"JOIN_GENERAL": 1, "FORCE_CHUNKS": 3}, {"JOIN_GENERAL": 1, "SORT_BITS": 255},
 ])
 def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
     """P-11: chunk count, candidate-buffer windows, key width and thinning change memory use and
@@ -305,6 +306,30 @@ def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
         assert st["n_chunks"] == opts["FORCE_CHUNKS"]
     if "CAND_CAPACITY" in opts:
         assert st["n_flushes"] > 1
+        assert st["join_general"] >= 1  # the pairs exceed one window: the fast join kernel hands over
+    if "JOIN_GENERAL" in opts:
+        assert st["join_general"] == st["n_chunks"]
+    if not opts:
+        assert st["join_general"] == 0
+
+
+@pytest.mark.parametrize("copies,sort_bits,general,expect_general", [
+    (10, 0, 0, 0),     # dense but inside one window and the list capacity: the fast kernel finishes
+    (10, 255, 0, 1),   # one bucket: the first tile lists every record, overflows, hands over
+    (40, 0, 0, 1),     # 3.7 M pairs: more than the default window
+    (40, 0, 1, 1),
+])
+def test_join_dense_runs(sd, oracle, copies, sort_bits, general, expect_general):
+    """Many sequences under one variant (m(m-1)/2 pairs per shared variant): exact copies of
+    each of 200 sequences, d = 1, so nearly every record has partners.  Whichever kernel finishes the
+    join, the result is the brute-force one."""
+    base = synth.tcr_set(200, 31)
+    rep = base.take(np.repeat(np.arange(base.n), copies))
+    c = sd.Context(0)
+    c.symdel_set_option(sd.OPT_JOIN_GENERAL, general)
+    c.symdel_set_option(sd.OPT_SORT_BITS, sort_bits)
+    assert_same(run_self(sd, c, rep, 1), oracle.bruteforce_self(rep.seqs, rep.offsets, 1))
+    assert c.symdel_get_stats()["join_general"] == expect_general
 
 
 def test_small_workspace_forces_chunking(torch, sd, ctx, oracle):
