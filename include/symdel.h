@@ -77,6 +77,7 @@ typedef struct {
     float ms_prepare, ms_generate, ms_sort, ms_emit, ms_dedup, ms_verify, ms_total; /* CUDA-event times; 0 unless SYMDEL_OPT_TIMING is set */
     float ms_sort_pass_avg; /* average duration of one onesweep pass over the variant records */
     int64_t sort_pass_records; /* records moved by one such pass */
+    int64_t join_redo_tiles;   /* join tiles that overflowed the small candidate list and were redone by the large-list kernel */
 } symdel_stats;
 
 /* Options (symdel_set_option); defaults in brackets. */

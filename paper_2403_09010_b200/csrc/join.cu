@@ -31,6 +31,8 @@
 // positions, so it is the same in every round); a round writes the records whose FIRST index lies in
 // [win_lo, win_hi), whole, at cand[index - win_lo] — the buffer keeps n_total + 64 slots of slack for
 // the overhang — and reports the end of what it wrote in info->win_end, where the next round starts.
+#include <type_traits>
+
 #include "kernels.h"
 
 
@@ -335,8 +337,8 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
 
 // =================================================================================================
 // Fast path: k_join_fast.  Same join, for the common case — every pair of the call fits the candidate
-// buffer (one window) and no tile lists more than JF_LMAX records.  It keeps NO copy of the tile in
-// shared memory: a tile streams its records twice through registers (the second time from L1/L2),
+// buffer (one window).  It keeps NO copy of the tile in shared memory: a tile streams its records
+// twice (the second time from registers / L1 / L2),
 //   1. "seen" / "seen twice" bitmaps as above (one shared-memory atomic per record),
 //   2. the records whose "seen twice" bit is set (a few per cent on sparse data) are appended to a
 //      shared-memory list,
@@ -347,47 +349,74 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
 // No bucket boundary is searched: tile t owns the buckets that start in [t*T, (t+1)*T), i.e. the
 // records of its range whose partitioned bits differ from those of record t*T - 1, plus the records
 // after the range that continue its last bucket (streamed until the partitioned bits change).
-// The order of the candidates is arbitrary (they are sorted next).  If the claim runs past the
-// buffer or a list overflows, the tile raises info->join_fallback and the host reruns the general
-// kernel above, which windows the output and chunks oversized buckets.
+// The order of the candidates is arbitrary (they are sorted next).
+//
+// Two instances: LMAX = 2048 listed records per tile (44 KB of shared memory: four tiles per SM) runs
+// first; a tile whose list overflows (dense data: most records have partners) puts its number on a
+// redo list, which the LMAX = 6144 instance then processes.  If a tile overflows even that, or the
+// claims run past the window, info->join_fallback is raised and the host reruns the general kernel
+// above, which windows the output and chunks oversized buckets.
+//
+// K32: the partitioned bits and the bitmap bits all sit in the high word of the record (the usual
+// layout); the filter phases then work on 32-bit words and keep only those in registers.
 constexpr int JF_THREADS = 512, JF_NW = JF_THREADS / 32, JF_IT = 8, JF_T = JF_THREADS * JF_IT;
-constexpr int JF_LMAX = 6144, JF_LIT = JF_LMAX / JF_THREADS;
-constexpr int JF_SLOT_BITS = 12, JF_SLOTS = 1 << JF_SLOT_BITS;
 constexpr int JF_BM_BITS = 16, JF_BM_WORDS = (1 << JF_BM_BITS) / 32;
 static_assert(JF_T == JN_T, "both kernels share sd_join_tiles");
-static_assert(JF_LMAX < 0xffff && JF_LIT <= 16, "node index width / nzmask width");
 
+template <int LMAX, int SLOT_BITS>
 struct JoinFastSmem {
-    u64 list[JF_LMAX];
+    u64 list[LMAX];
     u32 bit_a[JF_BM_WORDS];
     u32 bit_b[JF_BM_WORDS];
-    u32 head[JF_SLOTS];
-    unsigned short next[JF_LMAX];
+    u32 head[1 << SLOT_BITS];
+    unsigned short next[LMAX];
     u32 wsum[JF_NW];
     u32 nlist;
     u64 base;
 };
 
-__global__ void __launch_bounds__(JF_THREADS, 2) k_join_fast(const JoinParams P) {
+struct JoinFastParams {
+    JoinParams j;
+    const u32* tiles;  // nullptr: tile = block index; else the redo list
+    u32* redo;         // nullptr: a list overflow raises join_fallback; else tiles append themselves here
+};
+
+__device__ __forceinline__ u32 jf_atoms_add(u32* p, u32 v) {  // plain ATOMS.ADD (no compiler-inserted warp aggregation)
+    u32 old;
+    asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"((u32)__cvta_generic_to_shared(p)), "r"(v) : "memory");
+    return old;
+}
+
+template <bool K32, int LMAX, int SLOT_BITS, int MINB>
+__global__ void __launch_bounds__(JF_THREADS, MINB) k_join_fast(const JoinFastParams FP) {
+    typedef typename std::conditional<K32, u32, u64>::type K;  // the part of a record the filter looks at
+    typedef JoinFastSmem<LMAX, SLOT_BITS> Smem;
+    constexpr int SLOTS = 1 << SLOT_BITS, LIT = (LMAX + JF_THREADS - 1) / JF_THREADS;
+    static_assert(LMAX < 0xffff && LIT <= 32, "node index width / nzmask width");
     extern __shared__ __align__(16) unsigned char jn_smem[];
-    JoinFastSmem& S = *reinterpret_cast<JoinFastSmem*>(jn_smem);
+    Smem& S = *reinterpret_cast<Smem*>(jn_smem);
+    const JoinParams& P = FP.j;
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const u32 lane_lt = (1u << lane) - 1u;
     const u64 N = P.n;
-    const u64 g0 = (u64)blockIdx.x * JF_T;
+    const u32 tile = FP.tiles ? FP.tiles[blockIdx.x] : blockIdx.x;
+    const u64 g0 = (u64)tile * JF_T;
     const u64 E = min(g0 + (u64)JF_T, N);
-    const u64 v0 = g0 > 0 ? (P.rec[g0 - 1] & P.topmask) : 0ull;  // bucket of the record before the range
-    const u64 v1 = P.rec[E - 1] & P.topmask;                     // bucket that may continue after the range
-    if (g0 > 0 && v1 == v0) return;                              // no bucket starts here
+    auto key_of = [&](u64 y) -> K { return K32 ? (K)(y >> 32) : (K)y; };
+    const K topmask = key_of(P.topmask);
+    const int bm_shift = K32 ? P.bm_shift - 32 : P.bm_shift;
+    const K v0 = g0 > 0 ? (key_of(P.rec[g0 - 1]) & topmask) : (K)0;  // bucket of the record before the range
+    const K v1 = key_of(P.rec[E - 1]) & topmask;                      // bucket that may continue after the range
+    if (g0 > 0 && v1 == v0) return;                                   // no bucket starts here
 
     for (u32 i = tid; i < 2 * JF_BM_WORDS / 4; i += JF_THREADS)
         reinterpret_cast<uint4*>(S.bit_a)[i] = make_uint4(0u, 0u, 0u, 0u);  // bit_a and bit_b are adjacent
-    for (u32 i = tid; i < JF_SLOTS / 4; i += JF_THREADS)
+    for (u32 i = tid; i < SLOTS / 4; i += JF_THREADS)
         reinterpret_cast<uint4*>(S.head)[i] = make_uint4(JN_NIL, JN_NIL, JN_NIL, JN_NIL);
     if (tid == 0) S.nlist = 0;
 
-    // ---- the range, two records per 16-byte load: thread holds records 2*(tid + k*THREADS) + {0, 1} ----
-    u64 x[JF_IT];
+    // ---- the range, two records per 16-byte load: item 2k + e of the thread is record 2*(tid + k*THREADS) + e ----
+    K x[JF_IT];
     u32 mine = 0;
     const bool full = E - g0 == (u64)JF_T;
 #pragma unroll
@@ -395,10 +424,10 @@ __global__ void __launch_bounds__(JF_THREADS, 2) k_join_fast(const JoinParams P)
         const u32 r = 2 * (tid + k * JF_THREADS);
         if (full || g0 + r + 1 < E) {
             const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(P.rec + g0 + r);
-            x[2 * k] = t.x, x[2 * k + 1] = t.y;
+            x[2 * k] = key_of(t.x), x[2 * k + 1] = key_of(t.y);
             mine |= 3u << (2 * k);
         } else if (g0 + r < E) {
-            x[2 * k] = P.rec[g0 + r], x[2 * k + 1] = 0;
+            x[2 * k] = key_of(P.rec[g0 + r]), x[2 * k + 1] = 0;
             mine |= 1u << (2 * k);
         } else {
             x[2 * k] = x[2 * k + 1] = 0;
@@ -407,11 +436,11 @@ __global__ void __launch_bounds__(JF_THREADS, 2) k_join_fast(const JoinParams P)
     if (g0 > 0) {
 #pragma unroll
         for (int k = 0; k < JF_IT; ++k)
-            if ((x[k] & P.topmask) == v0) mine &= ~(1u << k);
+            if ((x[k] & topmask) == v0) mine &= ~(1u << k);
     }
     __syncthreads();
-    auto bm_of = [&](u64 y) -> u32 { return (u32)(y >> P.bm_shift) & ((1u << JF_BM_BITS) - 1u); };
-    auto mark = [&](u64 y) {
+    auto bm_of = [&](K y) -> u32 { return (u32)(y >> bm_shift) & ((1u << JF_BM_BITS) - 1u); };
+    auto mark = [&](K y) {
         const u32 b = bm_of(y), bit = 1u << (b & 31u);
         if (atomicOr(&S.bit_a[b >> 5], bit) & bit) atomicOr(&S.bit_b[b >> 5], bit);
     };
@@ -420,50 +449,69 @@ __global__ void __launch_bounds__(JF_THREADS, 2) k_join_fast(const JoinParams P)
     for (int k = 0; k < JF_IT; ++k)
         if ((mine >> k) & 1u) mark(x[k]);
     // the records after the range that continue its last bucket; every thread sees the same stride ends
+    u32 nstride = 0;
     for (u64 q0 = E; q0 < N; q0 += JF_THREADS) {
         const u64 q = q0 + tid;
         if (q < N) {
-            const u64 y = P.rec[q];
-            if ((y & P.topmask) == v1) mark(y);
+            const K y = key_of(P.rec[q]);
+            if ((y & topmask) == v1) mark(y);
         }
-        if ((P.rec[min(q0 + JF_THREADS, N) - 1] & P.topmask) != v1) break;
+        ++nstride;
+        if ((key_of(P.rec[min(q0 + JF_THREADS, N) - 1]) & topmask) != v1) break;
     }
     __syncthreads();
     // ---- 2. list the records whose "seen twice" bit is set ----
-    auto listed = [&](u64 y) -> bool {
+    auto listed = [&](K y) -> bool {
         const u32 b = bm_of(y);
         return (S.bit_b[b >> 5] >> (b & 31u)) & 1u;
     };
-    auto append = [&](bool c, u64 y) {
-        const u32 bal = __ballot_sync(SD_FULL, c);
-        if (bal == 0) return;
-        u32 at = 0;
-        if (lane == 0) at = atomicAdd(&S.nlist, (u32)__popc(bal));
-        at = __shfl_sync(SD_FULL, at, 0) + __popc(bal & lane_lt);
-        if (c && at < (u32)JF_LMAX) S.list[at] = y;
-    };
+    {
+        u32 bal[JF_IT], cnt = 0;
 #pragma unroll
-    for (int k = 0; k < JF_IT; ++k) append(((mine >> k) & 1u) && listed(x[k]), x[k]);
-    for (u64 q0 = E; q0 < N; q0 += JF_THREADS) {
-        const u64 q = q0 + tid;
+        for (int k = 0; k < JF_IT; ++k) {
+            bal[k] = __ballot_sync(SD_FULL, ((mine >> k) & 1u) && listed(x[k]));
+            cnt += __popc(bal[k]);
+        }
+        u32 at = 0;
+        if (lane == 0 && cnt) at = jf_atoms_add(&S.nlist, cnt);
+        at = __shfl_sync(SD_FULL, at, 0);
+#pragma unroll
+        for (int k = 0; k < JF_IT; ++k) {
+            if ((bal[k] >> lane) & 1u) {
+                const u32 slot = at + __popc(bal[k] & lane_lt);
+                if (slot < (u32)LMAX) S.list[slot] = K32 ? P.rec[g0 + 2 * (tid + (k >> 1) * JF_THREADS) + (k & 1)] : (u64)x[k];
+            }
+            at += __popc(bal[k]);
+        }
+    }
+    for (u32 sidx = 0; sidx < nstride; ++sidx) {
+        const u64 q = E + (u64)sidx * JF_THREADS + tid;
         u64 y = 0;
         bool c = false;
         if (q < N) {
             y = P.rec[q];
-            c = (y & P.topmask) == v1 && listed(y);
+            c = (key_of(y) & topmask) == v1 && listed(key_of(y));
         }
-        append(c, y);
-        if ((P.rec[min(q0 + JF_THREADS, N) - 1] & P.topmask) != v1) break;
+        const u32 bal = __ballot_sync(SD_FULL, c);
+        if (bal) {
+            u32 at = 0;
+            if (lane == 0) at = jf_atoms_add(&S.nlist, (u32)__popc(bal));
+            at = __shfl_sync(SD_FULL, at, 0) + __popc(bal & lane_lt);
+            if (c && at < (u32)LMAX) S.list[at] = y;
+        }
     }
     __syncthreads();
     const u32 nl = S.nlist;
     if (nl == 0) return;
-    if (nl > (u32)JF_LMAX) {
-        if (tid == 0) atomicOr(&P.info->join_fallback, 1u);
+    if (nl > (u32)LMAX) {
+        if (tid == 0) {
+            if (FP.redo) FP.redo[atomicAdd(&P.info->join_redo, 1u)] = tile;
+            else atomicOr(&P.info->join_fallback, 1u);
+        }
         return;
     }
     // ---- 3. chains ----
-    auto slot_of = [&](u64 y) -> u32 { return (u32)(y >> P.slot_shift) & (JF_SLOTS - 1); };
+    auto slot_of = [&](u64 y) -> u32 { return (u32)(y >> P.slot_shift) & (SLOTS - 1); };
     for (u32 i = tid; i < nl; i += JF_THREADS) S.next[i] = (unsigned short)atomicExch(&S.head[slot_of(S.list[i])], i);
     __syncthreads();
     // ---- 4. count, claim, write ----
@@ -471,9 +519,11 @@ __global__ void __launch_bounds__(JF_THREADS, 2) k_join_fast(const JoinParams P)
     {
         u32 k = 0;
         for (u32 i = tid; i < nl; i += JF_THREADS, ++k) {
+            u32 j = S.next[i];
+            if (j == JN_NIL) continue;
             const u64 y = S.list[i];
             u32 c = 0;
-            for (u32 j = S.next[i]; j != JN_NIL; j = S.next[j]) {
+            for (; j != JN_NIL; j = S.next[j]) {
                 const u64 z = S.list[j];
                 u64 packed;
                 if ((y ^ z) < P.hlim && jn_pair(y, z, P, packed)) ++c;
@@ -518,6 +568,9 @@ __global__ void __launch_bounds__(JF_THREADS, 2) k_join_fast(const JoinParams P)
         }
 }
 
+constexpr int JF_LMAX_S = 2048, JF_SLOTB_S = 11, JF_MINB_S = 3;
+constexpr int JF_LMAX_L = 6144, JF_SLOTB_L = 12, JF_MINB_L = 2;
+
 }  // namespace
 
 i64 sd_join_tiles(i64 n_records) { return (n_records + JN_T - 1) / JN_T; }
@@ -543,27 +596,58 @@ static JoinParams jn_params(const u64* records, i64 n_records, const Layout& lay
     return P;
 }
 
-// Fast path: all pairs in one window of `window` slots, arbitrary order; info->n_cand = total,
-// info->join_fallback != 0 if the general kernel has to redo the join (nothing usable was written).
-cudaError_t sd_join_fast(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, DevInfo* info,
-                         cudaStream_t st, i64* launches) {
-    const i64 tiles = sd_join_tiles(n_records);
-    if (tiles == 0) return cudaSuccess;
-    constexpr size_t smem = sizeof(JoinFastSmem);
+// Fast path: all pairs in one window of `window` slots, arbitrary order; info->n_cand = total.
+// Step 1 (sd_join_fast): the small-list instance over every tile; tiles whose list overflowed are in
+// redo[0 .. info->join_redo).  Step 2 (sd_join_fast_redo, only if join_redo != 0): the large-list
+// instance over those.  info->join_fallback != 0 after either: the general kernel has to redo the
+// join (nothing usable was written).
+template <bool K32>
+static cudaError_t jn_launch_fast(const JoinFastParams& FP, unsigned grid, bool large, cudaStream_t st) {
     static bool attr_set = false;
+    auto ks = k_join_fast<K32, JF_LMAX_S, JF_SLOTB_S, JF_MINB_S>;
+    auto kl = k_join_fast<K32, JF_LMAX_L, JF_SLOTB_L, JF_MINB_L>;
+    constexpr size_t ss = sizeof(JoinFastSmem<JF_LMAX_S, JF_SLOTB_S>), sl = sizeof(JoinFastSmem<JF_LMAX_L, JF_SLOTB_L>);
     cudaError_t e;
     if (!attr_set) {
-        if ((e = cudaFuncSetAttribute(k_join_fast, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(ks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ss)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(kl, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sl)) != cudaSuccess) return e;
         attr_set = true;
     }
-    if ((e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
-    if ((e = cudaMemsetAsync(&info->join_fallback, 0, sizeof(u32), st)) != cudaSuccess) return e;
-    JoinParams P = jn_params(records, n_records, lay, cand, window, info);
-    P.win_lo = 0;
-    P.win_hi = window;
-    k_join_fast<<<(unsigned)tiles, JF_THREADS, smem, st>>>(P);
-    if (launches) ++*launches;
+    if (large) kl<<<grid, JF_THREADS, sl, st>>>(FP);
+    else ks<<<grid, JF_THREADS, ss, st>>>(FP);
     return cudaGetLastError();
+}
+
+static bool jn_k32(const JoinParams& P) { return P.bm_shift >= 32 && (P.topmask & 0xffffffffull) == 0; }
+
+cudaError_t sd_join_fast(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, u32* redo,
+                         DevInfo* info, cudaStream_t st, i64* launches) {
+    const i64 tiles = sd_join_tiles(n_records);
+    if (tiles == 0) return cudaSuccess;
+    cudaError_t e;
+    if ((e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(&info->join_fallback, 0, 2 * sizeof(u32), st)) != cudaSuccess) return e;  // and join_redo
+    JoinFastParams FP{};
+    FP.j = jn_params(records, n_records, lay, cand, window, info);
+    FP.j.win_lo = 0;
+    FP.j.win_hi = window;
+    FP.tiles = nullptr;
+    FP.redo = redo;
+    if (launches) ++*launches;
+    return jn_k32(FP.j) ? jn_launch_fast<true>(FP, (unsigned)tiles, false, st) : jn_launch_fast<false>(FP, (unsigned)tiles, false, st);
+}
+
+cudaError_t sd_join_fast_redo(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, const u32* redo,
+                              u32 n_redo, DevInfo* info, cudaStream_t st, i64* launches) {
+    if (n_redo == 0) return cudaSuccess;
+    JoinFastParams FP{};
+    FP.j = jn_params(records, n_records, lay, cand, window, info);
+    FP.j.win_lo = 0;
+    FP.j.win_hi = window;
+    FP.tiles = redo;
+    FP.redo = nullptr;
+    if (launches) ++*launches;
+    return jn_k32(FP.j) ? jn_launch_fast<true>(FP, n_redo, true, st) : jn_launch_fast<false>(FP, n_redo, true, st);
 }
 
 cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 cand_cap, u64 win_lo, u64 win_hi,

@@ -69,10 +69,14 @@ i64 sd_join_tiles(i64 n_records);
 cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 cand_cap, u64 win_lo, u64 win_hi,
                     int first_round, u64* tile_prefix, DevInfo* info, cudaStream_t st, i64* launches);
 
-// Fast path of the join (one window, arbitrary candidate order).  info->n_cand = number of pairs;
-// info->join_fallback != 0: redo with sd_join (the pairs exceed `window` or a tile overflowed its list).
-cudaError_t sd_join_fast(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, DevInfo* info,
-                         cudaStream_t st, i64* launches);
+// Fast path of the join (one window of `window` slots, arbitrary candidate order).  sd_join_fast runs the
+// small-list kernel over all tiles; tiles whose list overflowed are left in redo[0 .. info->join_redo)
+// (redo: one u32 per tile) for sd_join_fast_redo.  info->n_cand = number of pairs; info->join_fallback != 0:
+// redo the whole join with sd_join (the pairs exceed `window`, or a tile overflowed the large list too).
+cudaError_t sd_join_fast(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, u32* redo,
+                         DevInfo* info, cudaStream_t st, i64* launches);
+cudaError_t sd_join_fast_redo(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, const u32* redo,
+                              u32 n_redo, DevInfo* info, cudaStream_t st, i64* launches);
 
 // ---- verify.cu ----------------------------------------------------------------------------------
 i64 sd_verify_tiles(i64 n);

@@ -302,10 +302,17 @@ restart:
         // ---- S3a: join (first window): the fast kernel when everything fits one window, else the general one ----
         bool general = ctx->opt_join_general != 0;
         if (!general) {
-            CK(sd_join_fast(sorted, N, lay, candA, (u64)ccap, info, st, &S.n_launches));
+            CK(sd_join_fast(sorted, N, lay, candA, (u64)ccap, (u32*)tile_prefix, info, st, &S.n_launches));
             rc = read_info(ctx, info, st);
             if (rc) return rc;
             if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+            if (ctx->h_info->join_redo && !ctx->h_info->join_fallback) {  // dense tiles: the large-list instance
+                S.join_redo_tiles += ctx->h_info->join_redo;
+                CK(sd_join_fast_redo(sorted, N, lay, candA, (u64)ccap, (const u32*)tile_prefix, ctx->h_info->join_redo, info, st,
+                                     &S.n_launches));
+                rc = read_info(ctx, info, st);
+                if (rc) return rc;
+            }
             general = ctx->h_info->join_fallback != 0;
             ctx->h_info->win_end = ctx->h_info->n_cand;
         }

@@ -36,7 +36,7 @@ class Stats(C.Structure):
         ("hash_bits", C.c_int32), ("id_bits", C.c_int32), ("sort_bits", C.c_int32), ("join_general", C.c_int32),
         ("ms_prepare", C.c_float), ("ms_generate", C.c_float), ("ms_sort", C.c_float), ("ms_emit", C.c_float),
         ("ms_dedup", C.c_float), ("ms_verify", C.c_float), ("ms_total", C.c_float), ("ms_sort_pass_avg", C.c_float),
-        ("sort_pass_records", C.c_int64),
+        ("sort_pass_records", C.c_int64), ("join_redo_tiles", C.c_int64),
     ]
 
     def as_dict(self):
