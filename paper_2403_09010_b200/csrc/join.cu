@@ -359,9 +359,8 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
 //
 // K32: the partitioned bits and the bitmap bits all sit in the high word of the record (the usual
 // layout); the filter phases then work on 32-bit words and keep only those in registers.
-constexpr int JF_THREADS = 512, JF_NW = JF_THREADS / 32, JF_IT = 8, JF_T = JF_THREADS * JF_IT;
+constexpr int JF_THREADS = 512, JF_NW = JF_THREADS / 32;
 constexpr int JF_BM_BITS = 16, JF_BM_WORDS = (1 << JF_BM_BITS) / 32;
-static_assert(JF_T == JN_T, "both kernels share sd_join_tiles");
 
 template <int LMAX, int SLOT_BITS>
 struct JoinFastSmem {
@@ -387,12 +386,12 @@ __device__ __forceinline__ u32 jf_atoms_add(u32* p, u32 v) {  // plain ATOMS.ADD
     return old;
 }
 
-template <bool K32, int LMAX, int SLOT_BITS, int MINB>
+template <bool K32, int IT, int LMAX, int SLOT_BITS, int MINB>
 __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_fast(const JoinFastParams FP) {
     typedef typename std::conditional<K32, u32, u64>::type K;  // the part of a record the filter looks at
     typedef JoinFastSmem<LMAX, SLOT_BITS> Smem;
-    constexpr int SLOTS = 1 << SLOT_BITS, LIT = (LMAX + JF_THREADS - 1) / JF_THREADS;
-    static_assert(LMAX < 0xffff && LIT <= 32, "node index width / nzmask width");
+    constexpr int SLOTS = 1 << SLOT_BITS, LIT = (LMAX + JF_THREADS - 1) / JF_THREADS, T = JF_THREADS * IT;
+    static_assert(LMAX < 0xffff && LIT <= 32 && IT % 2 == 0 && IT <= 32, "node index width / mask widths");
     extern __shared__ __align__(16) unsigned char jn_smem[];
     Smem& S = *reinterpret_cast<Smem*>(jn_smem);
     const JoinParams& P = FP.j;
@@ -400,8 +399,8 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_fast(const JoinFastPa
     const u32 lane_lt = (1u << lane) - 1u;
     const u64 N = P.n;
     const u32 tile = FP.tiles ? FP.tiles[blockIdx.x] : blockIdx.x;
-    const u64 g0 = (u64)tile * JF_T;
-    const u64 E = min(g0 + (u64)JF_T, N);
+    const u64 g0 = (u64)tile * T;
+    const u64 E = min(g0 + (u64)T, N);
     auto key_of = [&](u64 y) -> K { return K32 ? (K)(y >> 32) : (K)y; };
     const K topmask = key_of(P.topmask);
     const int bm_shift = K32 ? P.bm_shift - 32 : P.bm_shift;
@@ -416,18 +415,19 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_fast(const JoinFastPa
     if (tid == 0) S.nlist = 0;
 
     // ---- the range, two records per 16-byte load: item 2k + e of the thread is record 2*(tid + k*THREADS) + e ----
-    K x[JF_IT];
+    const u64* const rp = P.rec + g0 + 2 * tid;
+    K x[IT];
     u32 mine = 0;
-    const bool full = E - g0 == (u64)JF_T;
+    const bool full = E - g0 == (u64)T;
 #pragma unroll
-    for (int k = 0; k < JF_IT / 2; ++k) {
+    for (int k = 0; k < IT / 2; ++k) {
         const u32 r = 2 * (tid + k * JF_THREADS);
         if (full || g0 + r + 1 < E) {
-            const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(P.rec + g0 + r);
+            const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + 2 * k * JF_THREADS);
             x[2 * k] = key_of(t.x), x[2 * k + 1] = key_of(t.y);
             mine |= 3u << (2 * k);
         } else if (g0 + r < E) {
-            x[2 * k] = key_of(P.rec[g0 + r]), x[2 * k + 1] = 0;
+            x[2 * k] = key_of(rp[2 * k * JF_THREADS]), x[2 * k + 1] = 0;
             mine |= 1u << (2 * k);
         } else {
             x[2 * k] = x[2 * k + 1] = 0;
@@ -435,7 +435,7 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_fast(const JoinFastPa
     }
     if (g0 > 0) {
 #pragma unroll
-        for (int k = 0; k < JF_IT; ++k)
+        for (int k = 0; k < IT; ++k)
             if ((x[k] & topmask) == v0) mine &= ~(1u << k);
     }
     __syncthreads();
@@ -446,18 +446,18 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_fast(const JoinFastPa
     };
     // ---- 1. bitmaps ----
 #pragma unroll
-    for (int k = 0; k < JF_IT; ++k)
+    for (int k = 0; k < IT; ++k)
         if ((mine >> k) & 1u) mark(x[k]);
-    // the records after the range that continue its last bucket; every thread sees the same stride ends
-    u32 nstride = 0;
-    for (u64 q0 = E; q0 < N; q0 += JF_THREADS) {
-        const u64 q = q0 + tid;
+    // The records after the range that continue its last bucket: every warp walks its own strided
+    // positions until none of its lanes is in the bucket any more (the records are sorted on these bits).
+    for (u64 q = E + tid; __any_sync(SD_FULL, q < N); q += JF_THREADS) {
+        bool in = false;
         if (q < N) {
             const K y = key_of(P.rec[q]);
-            if ((y & topmask) == v1) mark(y);
+            in = (y & topmask) == v1;
+            if (in) mark(y);
         }
-        ++nstride;
-        if ((key_of(P.rec[min(q0 + JF_THREADS, N) - 1]) & topmask) != v1) break;
+        if (!__any_sync(SD_FULL, in)) break;
     }
     __syncthreads();
     // ---- 2. list the records whose "seen twice" bit is set ----
@@ -466,32 +466,37 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_fast(const JoinFastPa
         return (S.bit_b[b >> 5] >> (b & 31u)) & 1u;
     };
     {
-        u32 bal[JF_IT], cnt = 0;
+        u32 lm = 0;
 #pragma unroll
-        for (int k = 0; k < JF_IT; ++k) {
-            bal[k] = __ballot_sync(SD_FULL, ((mine >> k) & 1u) && listed(x[k]));
-            cnt += __popc(bal[k]);
+        for (int k = 0; k < IT; ++k)
+            if (((mine >> k) & 1u) && listed(x[k])) lm |= 1u << k;
+        // lane l's listed records go to slots [sum of popc(lm) over lanes < l, ...)
+        const u32 c = __popc(lm);
+        u32 inc = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const u32 t = __shfl_up_sync(SD_FULL, inc, o);
+            if (lane >= (u32)o) inc += t;
         }
         u32 at = 0;
-        if (lane == 0 && cnt) at = jf_atoms_add(&S.nlist, cnt);
-        at = __shfl_sync(SD_FULL, at, 0);
-#pragma unroll
-        for (int k = 0; k < JF_IT; ++k) {
-            if ((bal[k] >> lane) & 1u) {
-                const u32 slot = at + __popc(bal[k] & lane_lt);
-                if (slot < (u32)LMAX) S.list[slot] = K32 ? P.rec[g0 + 2 * (tid + (k >> 1) * JF_THREADS) + (k & 1)] : (u64)x[k];
-            }
-            at += __popc(bal[k]);
+        if (lane == 31 && inc) at = jf_atoms_add(&S.nlist, inc);
+        at = __shfl_sync(SD_FULL, at, 31) + inc - c;
+        while (lm) {
+            const int k = __ffs(lm) - 1;
+            lm &= lm - 1;
+            if (at < (u32)LMAX) S.list[at] = rp[(k >> 1) * (2 * JF_THREADS) + (k & 1)];
+            ++at;
         }
     }
-    for (u32 sidx = 0; sidx < nstride; ++sidx) {
-        const u64 q = E + (u64)sidx * JF_THREADS + tid;
+    for (u64 q = E + tid; __any_sync(SD_FULL, q < N); q += JF_THREADS) {
+        bool in = false, c = false;
         u64 y = 0;
-        bool c = false;
         if (q < N) {
             y = P.rec[q];
-            c = (key_of(y) & topmask) == v1 && listed(key_of(y));
+            in = (key_of(y) & topmask) == v1;
+            c = in && listed(key_of(y));
         }
+        if (!__any_sync(SD_FULL, in)) break;
         const u32 bal = __ballot_sync(SD_FULL, c);
         if (bal) {
             u32 at = 0;
@@ -532,6 +537,7 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_fast(const JoinFastPa
             cnt += c;
         }
     }
+    if (!__syncthreads_or(cnt != 0)) return;
     u32 inc = cnt;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -540,22 +546,25 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_fast(const JoinFastPa
     }
     if (lane == 31) S.wsum[warp] = inc;
     __syncthreads();
-    u32 carry = 0, total = 0;
+    if (warp == 0) {
+        const u32 w = lane < JF_NW ? S.wsum[lane] : 0u;
+        u32 winc = w;
 #pragma unroll
-    for (int w = 0; w < JF_NW; ++w) {
-        const u32 c = S.wsum[w];
-        if ((u32)w < warp) carry += c;
-        total += c;
-    }
-    if (total == 0) return;
-    if (tid == 0) {
-        const u64 base = (u64)atomicAdd((unsigned long long*)&P.info->n_cand, (unsigned long long)total);
-        if (base + total > P.win_hi) atomicOr(&P.info->join_fallback, 2u);  // does not fit the window: nothing is written
-        S.base = base;
+        for (int o = 1; o < JF_NW; o <<= 1) {
+            const u32 t = __shfl_up_sync(SD_FULL, winc, o);
+            if (lane >= (u32)o) winc += t;
+        }
+        if (lane < JF_NW) S.wsum[lane] = winc - w;
+        if (lane == JF_NW - 1) {
+            const u64 base = (u64)atomicAdd((unsigned long long*)&P.info->n_cand, (unsigned long long)winc);
+            // does not fit the window: nothing is written
+            if (base + winc > P.win_hi) atomicOr(&P.info->join_fallback, 2u), S.base = ~0ull;
+            else S.base = base;
+        }
     }
     __syncthreads();
-    u64 at = S.base + carry + inc - cnt;
-    if (S.base + total > P.win_hi) return;
+    if (S.base == ~0ull) return;
+    u64 at = S.base + S.wsum[warp] + inc - cnt;
     for (u32 m = nzmask, k = 0; m; m >>= 1, ++k)
         if (m & 1u) {
             const u32 i = tid + k * JF_THREADS;
@@ -568,8 +577,15 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_fast(const JoinFastPa
         }
 }
 
-constexpr int JF_LMAX_S = 2048, JF_SLOTB_S = 11, JF_MINB_S = 3;
-constexpr int JF_LMAX_L = 6144, JF_SLOTB_L = 12, JF_MINB_L = 2;
+#ifndef JF_IT
+#define JF_IT 8
+#endif
+#ifndef JF_MINB_S
+#define JF_MINB_S 4
+#endif
+constexpr int JF_T = JF_THREADS * JF_IT;
+constexpr int JF_LMAX_S = JF_IT > 8 ? 3072 : 2048, JF_SLOTB_S = 11;
+constexpr int JF_LMAX_L = JF_T + 4096, JF_SLOTB_L = 12, JF_MINB_L = JF_IT > 8 ? 1 : 2;
 
 }  // namespace
 
@@ -604,8 +620,8 @@ static JoinParams jn_params(const u64* records, i64 n_records, const Layout& lay
 template <bool K32>
 static cudaError_t jn_launch_fast(const JoinFastParams& FP, unsigned grid, bool large, cudaStream_t st) {
     static bool attr_set = false;
-    auto ks = k_join_fast<K32, JF_LMAX_S, JF_SLOTB_S, JF_MINB_S>;
-    auto kl = k_join_fast<K32, JF_LMAX_L, JF_SLOTB_L, JF_MINB_L>;
+    auto ks = k_join_fast<K32, JF_IT, JF_LMAX_S, JF_SLOTB_S, JF_MINB_S>;
+    auto kl = k_join_fast<K32, JF_IT, JF_LMAX_L, JF_SLOTB_L, JF_MINB_L>;
     constexpr size_t ss = sizeof(JoinFastSmem<JF_LMAX_S, JF_SLOTB_S>), sl = sizeof(JoinFastSmem<JF_LMAX_L, JF_SLOTB_L>);
     cudaError_t e;
     if (!attr_set) {
@@ -622,7 +638,7 @@ static bool jn_k32(const JoinParams& P) { return P.bm_shift >= 32 && (P.topmask 
 
 cudaError_t sd_join_fast(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, u32* redo,
                          DevInfo* info, cudaStream_t st, i64* launches) {
-    const i64 tiles = sd_join_tiles(n_records);
+    const i64 tiles = (n_records + JF_T - 1) / JF_T;
     if (tiles == 0) return cudaSuccess;
     cudaError_t e;
     if ((e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
