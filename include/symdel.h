@@ -77,6 +77,7 @@ typedef struct {
     float ms_prepare, ms_generate, ms_sort, ms_emit, ms_dedup, ms_verify, ms_total; /* CUDA-event times; 0 unless SYMDEL_OPT_TIMING is set */
     float ms_sort_pass_avg; /* average duration of one onesweep pass over the variant records */
     int64_t sort_pass_records; /* records moved by one such pass */
+    int64_t fused_chunks;      /* chunks that went through the fused pipeline (generation + partition in one kernel, bucket join) */
     int64_t join_redo_tiles;   /* join tiles that overflowed the small candidate list and were redone by the large-list kernel */
 } symdel_stats;
 
@@ -92,6 +93,7 @@ enum {
     SYMDEL_OPT_SORT_BITS = 8,     /* [0] 0 = automatic; 8..56 (multiple of 8): top hash bits that S2 radix-partitions; 255 = none (one bucket: the join chunks it) */
     SYMDEL_OPT_SORT_STABLE = 9,   /* [0] 1: every S2 pass takes the stable (ties keep input order) tile path (test hook; results are identical) */
     SYMDEL_OPT_JOIN_GENERAL = 11, /* [0] 1: always run the general join kernel (windowed output, chunked buckets) instead of trying the fast one first (test hook; results are identical) */
+    SYMDEL_OPT_EXACT_PIPELINE = 12, /* [0] 1: never use the fused pipeline (fixed-capacity bins); always count, scan, generate, onesweep-partition on exact histograms, windowed join (the path the fused one falls back to when a bin overflows; results are identical) */
     SYMDEL_OPT_SORT_GROUPING = 10 /* [0] 1: symdel_stage_sort_u64 sorts keys only: ties land in arbitrary order (the mode the pipeline uses) */
 };
 

@@ -26,6 +26,8 @@ struct DevInfo {
     u64 win_end;     // join: end (flat pair index) of what the last round wrote
     u32 join_fallback;  // k_join_fast: 1 = a tile's list overflowed, 2 = the pairs do not fit the window
     u32 join_redo;      // k_join_fast: tiles on the redo list (keep right after join_fallback: cleared together)
+    u32 part_overflow;  // fused pipeline: 1 = a level-1 bin was full, 2 = a level-2 bucket was full
+    u32 pad;
 };
 enum { SD_ERR_OFFSETS = 1, SD_ERR_TOO_LONG = 2, SD_ERR_RESIDUE = 4, SD_ERR_INTERNAL = 8, SD_ERR_OVERFLOW = 16 };
 enum { SD_TK_SORT = 0, SD_TK_EMIT = 1, SD_TK_VERIFY = 2, SD_TK_FINAL = 3, SD_TK_SCAN = 4 };

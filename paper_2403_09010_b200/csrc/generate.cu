@@ -619,6 +619,216 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Fused fast path: generation + level-1 partition (k_gen2_part).  Same enumeration and hash as k_gen2,
+// but a record is not written in id order: it is staged in shared memory under the top 8 bits of its
+// hash (GP_S slots per digit; one shared-memory atomic returns its slot) and the block flushes the
+// stage to 256 global BINS of fixed capacity `cap1` (one global atomic per digit and flush claims the
+// segment; each digit's records leave as one contiguous store).  No count pass, no offsets, no
+// histogram: the order of the records inside a bin is irrelevant to the join.  A record that finds its
+// digit's slots full goes straight to its bin (one global atomic).  A bin that would overflow raises
+// info->part_overflow: the host then redoes the chunk with the exact (histogram-based) pipeline.
+constexpr int GP_THREADS = 256, GP_NW = GP_THREADS / 32, GP_S = 32;
+#ifndef GP_FLUSH_AT
+#define GP_FLUSH_AT 2300
+#endif
+
+struct GenPartShared {
+    u64 stage[256 * GP_S];
+    u64 U[GP_NW][32];
+    u64 V[GP_NW][32];
+    u64 R[32];
+    u64 Bpow[33];
+    u32 cnt[256];   // records staged per digit since the last flush (may exceed GP_S: the excess went to the bins directly)
+    u32 gpos[256];  // flush: claimed start inside the bin; 0xffffffff = bin full
+    u32 total;      // records staged since the last flush
+    unsigned char map[GP_NW][32];
+};
+
+struct GenPartParams {
+    GenParams g;
+    u64* bins;    // 256 bins of cap1 records
+    u32* cur;     // 256 bin cursors (zeroed by the host)
+    u64 cap1;
+};
+
+__device__ __forceinline__ u32 gp_atoms_inc(u32* p) {  // plain ATOMS.ADD 1 with return (no compiler-inserted aggregation)
+    u32 old;
+    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(old) : "r"((u32)__cvta_generic_to_shared(p)) : "memory");
+    return old;
+}
+
+template <bool CHUNKED>
+__global__ void __launch_bounds__(GP_THREADS, 3) k_gen2_part(GenPartParams PP) {
+    extern __shared__ __align__(16) unsigned char gen_smem[];
+    GenPartShared& sh = *reinterpret_cast<GenPartShared*>(gen_smem);
+    const GenParams& P = PP.g;
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid < 32) sh.R[tid] = c_R[tid];
+    if (tid < 33) sh.Bpow[tid] = c_Bpow[tid];
+    sh.cnt[tid] = 0;
+    if (tid == 0) sh.total = 0;
+    __syncthreads();
+    const int d = P.d;
+    const bool thinning = P.thinning != 0;
+    const u64 binv1 = c_Binv[1], binv2 = c_Binv[2];
+    const int kshift = 64 - P.hash_bits, id_bits = P.id_bits;
+    const bool plain = kshift == id_bits;  // the record is the hash with its low id_bits replaced by the id
+    const u64 idmask = (1ull << id_bits) - 1ull;
+    u64* const Uw = sh.U[warp];
+    u64* const Vw = sh.V[warp];
+    u32 made = 0;  // records this lane staged since the warp last reported
+
+    auto push = [&](bool valid, u64 h, u64 gid) {
+        if (CHUNKED) valid = valid && gen_chunk_of(h, P.n_chunks) == P.chunk;
+        if (valid) {
+            const u32 dg = (u32)(h >> 56);
+            const u64 rec = plain ? ((h & ~idmask) | gid) : (((h >> kshift) << id_bits) | gid);
+            const u32 r = gp_atoms_inc(&sh.cnt[dg]);
+            if (r < (u32)GP_S) {
+                sh.stage[dg * GP_S + r] = rec;
+            } else {
+                const u32 at = atomicAdd(&PP.cur[dg], 1u);
+                if ((u64)at < PP.cap1) PP.bins[(u64)dg * PP.cap1 + at] = rec;
+                else atomicOr(&P.info->part_overflow, 1u);
+            }
+            ++made;
+        }
+    };
+
+    // warp task = 32 consecutive sequences of one set, cut into batches that fill the 32 lanes; the block
+    // advances one batch per warp and round, then decides about flushing
+    i64 wt = (i64)blockIdx.x * GP_NW + warp;
+    const i64 wstride = (i64)gridDim.x * GP_NW;
+    bool have = false;  // a task is loaded and has batches left
+    u32 s = 0, ns = 0, Li = 0, cum_incl = 0, cum_excl = 0;
+    u64 gid0 = 0;
+    i64 obase = 0;
+    const int8_t* seqs = nullptr;
+    while (true) {
+        if (!have && wt < P.groups_total) {
+            const bool in_b = wt >= P.groups_a;
+            const SeqSetDev& S = in_b ? P.b : P.a;
+            const i64 first = (in_b ? wt - P.groups_a : wt) * 32;
+            ns = (u32)min((i64)32, S.n - first);
+            gid0 = (u64)first + (in_b ? (u64)P.n_a : 0ull);
+            seqs = S.seqs;
+            i64 o0 = 0;
+            Li = 0;
+            if (lane < ns) {
+                o0 = S.off[first + lane];
+                Li = (u32)(S.off[first + lane + 1] - o0);
+            }
+            cum_incl = Li;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const u32 t = __shfl_up_sync(SD_FULL, cum_incl, o);
+                if (lane >= (u32)o) cum_incl += t;
+            }
+            cum_excl = cum_incl - Li;
+            obase = __shfl_sync(SD_FULL, o0, 0);
+            s = 0;
+            have = true;
+            wt += wstride;
+        }
+        if (have) {
+            // ---- one batch: sequences [s, e) of the task ----
+            const u32 base = __shfl_sync(SD_FULL, cum_excl, s);
+            const u32 fit = __ballot_sync(SD_FULL, lane >= s && lane < ns && (cum_incl - base) <= 32u);
+            const u32 e = s + __popc(fit);
+            const u32 total = __shfl_sync(SD_FULL, cum_incl, e - 1) - base;
+            const bool mine = lane >= s && lane < e;  // lane as SEQUENCE index of this batch
+            if (mine && Li == 0) push(true, K_LEN, gid0 + lane);  // the empty variant of an empty sequence
+            if (total > 0) {
+                // ---- lane as POSITION: which sequence, which offset inside it ----
+                const u32 hbit = (mine && Li > 0) ? (1u << (cum_excl - base)) : 0u;
+                const u32 heads = __reduce_or_sync(SD_FULL, hbit);
+                if (mine && Li > 0) sh.map[warp][cum_excl - base] = (unsigned char)lane;
+                __syncwarp();
+                const bool active = lane < total;
+                const u32 seg_start = active ? (31u - __clz(heads & (0xffffffffu >> (31u - lane)))) : 0u;
+                const u32 si = active ? sh.map[warp][seg_start] : 0u;
+                const u32 Lsrc = __shfl_sync(SD_FULL, Li, si);
+                const u32 L = active ? Lsrc : 0u;  // idle lanes: L = 0 switches every later predicate off
+                const u32 a = lane - seg_start;
+                const u64 gid = gid0 + si;
+                const u32 c = active ? ((u32)(unsigned char)seqs[obase + base + lane] & 31u) : 0u;
+                const u32 cn = __shfl_down_sync(SD_FULL, c, 1), cnn = __shfl_down_sync(SD_FULL, c, 2);
+                const bool has1 = a + 1 < L, has2 = a + 2 < L;
+                const bool canon1 = active && (!thinning || !has1 || c != cn);
+                const bool adjok = active && has1 && (!thinning || !has2 || (c != cnn && cn != cnn));
+                const u32 m1 = __ballot_sync(SD_FULL, canon1), madj = __ballot_sync(SD_FULL, adjok);
+                // ---- prefix hashes of the source sequences (segmented scan over lanes) ----
+                const u64 term = active ? sh.R[c] * sh.Bpow[a] : 0ull;
+                u64 aincl = term;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const u64 t = __shfl_up_sync(SD_FULL, aincl, o);
+                    if (a >= (u32)o) aincl += t;
+                }
+                const u64 aexcl = aincl - term;
+                const u64 AL = __shfl_sync(SD_FULL, aincl, active ? seg_start + L - 1 : 0);
+                const u64 Uv = aexcl - binv1 * aincl;
+                Uw[lane] = Uv;
+                Vw[lane] = binv1 * Uv;
+                __syncwarp();
+                push(active && a == 0, AL + (u64)(L + 1) * K_LEN, gid);
+                if (d >= 1) push(canon1, Uv + binv1 * AL + (u64)L * K_LEN, gid);
+                if (d >= 2) {
+                    const u64 C2 = binv2 * AL + (u64)(L - 1) * K_LEN;
+                    const u32 half = __reduce_max_sync(SD_FULL, L >> 1);
+                    const u32 m1s = m1 >> seg_start, madjs = madj >> seg_start;  // segment-relative masks
+                    const u64* const Us = Uw + seg_start;
+                    const u64* const Vs = Vw + seg_start;
+                    for (u32 dl = 1; dl <= half; ++dl) {
+                        u32 b = a + dl;
+                        b = (b >= L) ? b - L : b;
+                        const u32 p1 = min(a, b) & 31u, p2 = max(a, b) & 31u;
+                        const bool on = (2 * dl < L) || (2 * dl == L && a < dl);  // false on idle lanes (L = 0)
+                        const u32 both = (m1s >> p1) & (m1s >> p2);
+                        const u32 t = (p2 - p1 == 1u) ? (madjs >> p1) : both;
+                        push(on && (t & 1u), Us[p1] + Vs[p2] + C2, gid);
+                    }
+                }
+                __syncwarp();  // U/V/map are reused by the next batch
+            }
+            s = e;
+            have = s < ns;
+            const u32 wmade = __reduce_add_sync(SD_FULL, made);
+            made = 0;
+            if (lane == 0 && wmade) atomicAdd(&sh.total, wmade);
+        }
+        // ---- round end: anyone left?  flush when the stage is about full (always at the end) ----
+        const bool more = have || wt < P.groups_total;
+        const int any_more = __syncthreads_or(more);
+        const u32 staged = sh.total;
+        if (staged > (u32)GP_FLUSH_AT || (!any_more && staged > 0)) {
+            const u32 cn_ = min(sh.cnt[tid], (u32)GP_S);
+            u32 g = 0;
+            if (cn_) {
+                g = atomicAdd(&PP.cur[tid], cn_);
+                if ((u64)g + cn_ > PP.cap1) {
+                    atomicOr(&P.info->part_overflow, 1u);
+                    g = 0xffffffffu;
+                }
+            }
+            sh.gpos[tid] = g;
+            __syncthreads();
+#pragma unroll 4
+            for (int dd = 0; dd < 32; ++dd) {
+                const u32 dg = warp * 32 + dd;
+                const u32 c2 = min(sh.cnt[dg], (u32)GP_S), g2 = sh.gpos[dg];
+                if (lane < c2 && g2 != 0xffffffffu) PP.bins[(u64)dg * PP.cap1 + g2 + lane] = sh.stage[dg * GP_S + lane];
+            }
+            __syncthreads();
+            sh.cnt[tid] = 0;
+            if (tid == 0) sh.total = 0;
+            __syncthreads();
+        }
+        if (!any_more) break;
+    }
+}
+
 typedef void (*Gen2Kernel)(GenParams);
 template <bool COUNT_ONLY>
 Gen2Kernel gen2_pick(bool chunked, int npass) {
@@ -766,6 +976,34 @@ cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
         k_generate<false, true><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared) + (size_t)npass * 256 * 4, st>>>(P);
     else
         k_generate<false, false><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared) + (size_t)npass * 256 * 4, st>>>(P);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+// Fused generation + level-1 partition (fast generator only: see sd_gen_part_applies).  bins: 256 x cap1
+// records; cur: 256 cursors, zeroed here.  info->part_overflow != 0 afterwards: a bin was full.
+bool sd_gen_part_applies(const Layout& lay, int width) { return use_fast(lay, width) && lay.hash_bits >= 8; }
+
+cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1, DevInfo* info,
+                        cudaStream_t st, i64* launches) {
+    GenPartParams PP{};
+    PP.g = make_params2(a, b, lay, width);
+    if (PP.g.groups_total == 0) return cudaSuccess;
+    PP.g.info = info;
+    PP.bins = bins;
+    PP.cur = cur;
+    PP.cap1 = cap1;
+    static bool attr_set = false;
+    cudaError_t e;
+    if (!attr_set) {
+        if ((e = cudaFuncSetAttribute(k_gen2_part<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GenPartShared))) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(k_gen2_part<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GenPartShared))) != cudaSuccess) return e;
+        attr_set = true;
+    }
+    if ((e = cudaMemsetAsync(cur, 0, 256 * sizeof(u32), st)) != cudaSuccess) return e;
+    const int grid = (int)std::min<i64>((PP.g.groups_total + GP_NW - 1) / GP_NW, 148 * 3);
+    if (lay.n_chunks > 1) k_gen2_part<true><<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
+    else k_gen2_part<false><<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
     if (launches) ++*launches;
     return cudaGetLastError();
 }

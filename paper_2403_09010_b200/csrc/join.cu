@@ -587,6 +587,171 @@ constexpr int JF_T = JF_THREADS * JF_IT;
 constexpr int JF_LMAX_S = JF_IT > 8 ? 3072 : 2048, JF_SLOTB_S = 11;
 constexpr int JF_LMAX_L = JF_T + 4096, JF_SLOTB_L = 12, JF_MINB_L = JF_IT > 8 ? 1 : 2;
 
+
+// =================================================================================================
+// Bucket join of the fused pipeline: k_join_bkt.  The level-2 partition leaves every bucket in its own
+// fixed-capacity region with its record count, so nothing has to be found: a block takes `group`
+// consecutive buckets (about 4096 records) and runs the filter / list / chain / claim / write steps of
+// k_join_fast over them, with no boundary tests and no tails.  Buckets of one block share the bitmaps
+// and chains; records of different buckets never pair because the chain walk compares whole hashes.
+// Same two instances (small list first, redo list, large list), same fallback flag.
+struct JoinBktParams {
+    JoinParams j;       // rec = bucket regions; topmask unused
+    const u32* cnt;     // records per bucket
+    u32 cap;            // region stride (records; a multiple of 32)
+    u32 nbuckets, group;
+    const u32* tiles;   // nullptr: block b takes buckets [b*group, (b+1)*group); else the redo list
+    u32* redo;
+};
+
+template <bool K32, int LMAX, int SLOT_BITS, int MINB>
+__global__ void __launch_bounds__(JF_THREADS, MINB) k_join_bkt(const JoinBktParams BP) {
+    typedef typename std::conditional<K32, u32, u64>::type K;
+    typedef JoinFastSmem<LMAX, SLOT_BITS> Smem;
+    constexpr int SLOTS = 1 << SLOT_BITS, LIT = (LMAX + JF_THREADS - 1) / JF_THREADS;
+    static_assert(LMAX < 0xffff && LIT <= 32, "node index width / nzmask width");
+    extern __shared__ __align__(16) unsigned char jn_smem[];
+    Smem& S = *reinterpret_cast<Smem*>(jn_smem);
+    const JoinParams& P = BP.j;
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 lane_lt = (1u << lane) - 1u;
+    const u32 tile = BP.tiles ? BP.tiles[blockIdx.x] : blockIdx.x;
+    const u32 b0 = tile * BP.group, b1 = min(b0 + BP.group, BP.nbuckets);
+    auto key_of = [&](u64 y) -> K { return K32 ? (K)(y >> 32) : (K)y; };
+    const int bm_shift = K32 ? P.bm_shift - 32 : P.bm_shift;
+
+    for (u32 i = tid; i < 2 * JF_BM_WORDS / 4; i += JF_THREADS)
+        reinterpret_cast<uint4*>(S.bit_a)[i] = make_uint4(0u, 0u, 0u, 0u);  // bit_a and bit_b are adjacent
+    for (u32 i = tid; i < SLOTS / 4; i += JF_THREADS)
+        reinterpret_cast<uint4*>(S.head)[i] = make_uint4(JN_NIL, JN_NIL, JN_NIL, JN_NIL);
+    if (tid == 0) S.nlist = 0;
+    __syncthreads();
+    auto bm_of = [&](K y) -> u32 { return (u32)(y >> bm_shift) & ((1u << JF_BM_BITS) - 1u); };
+    auto mark = [&](K y) {
+        const u32 b = bm_of(y), bit = 1u << (b & 31u);
+        if (atomicOr(&S.bit_a[b >> 5], bit) & bit) atomicOr(&S.bit_b[b >> 5], bit);
+    };
+    // ---- 1. bitmaps (two records per 16-byte load; regions are 256-byte aligned) ----
+    for (u32 b = b0; b < b1; ++b) {
+        const u32 n = min(BP.cnt[b], BP.cap);
+        const u64* const rp = P.rec + (u64)b * BP.cap;
+        for (u32 i = 2 * tid; i < n; i += 2 * JF_THREADS) {
+            if (i + 1 < n) {
+                const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + i);
+                mark(key_of(t.x));
+                mark(key_of(t.y));
+            } else {
+                mark(key_of(rp[i]));
+            }
+        }
+    }
+    __syncthreads();
+    // ---- 2. list the records whose "seen twice" bit is set ----
+    auto listed = [&](K y) -> bool {
+        const u32 b = bm_of(y);
+        return (S.bit_b[b >> 5] >> (b & 31u)) & 1u;
+    };
+    for (u32 b = b0; b < b1; ++b) {
+        const u32 n = min(BP.cnt[b], BP.cap);
+        const u64* const rp = P.rec + (u64)b * BP.cap;
+        for (u32 i0 = 0; i0 < n; i0 += 2 * JF_THREADS) {  // block-uniform trip count: the ballots below are full-warp
+            const u32 i = i0 + 2 * tid;
+            u64 y0 = 0, y1 = 0;
+            bool c0 = false, c1 = false;
+            if (i + 1 < n) {
+                const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + i);
+                y0 = t.x, y1 = t.y;
+                c0 = listed(key_of(y0)), c1 = listed(key_of(y1));
+            } else if (i < n) {
+                y0 = rp[i];
+                c0 = listed(key_of(y0));
+            }
+            const u32 bal0 = __ballot_sync(SD_FULL, c0), bal1 = __ballot_sync(SD_FULL, c1);
+            if (bal0 | bal1) {
+                const u32 n0 = __popc(bal0);
+                u32 at = 0;
+                if (lane == 0) at = jf_atoms_add(&S.nlist, n0 + (u32)__popc(bal1));
+                at = __shfl_sync(SD_FULL, at, 0);
+                const u32 a0 = at + __popc(bal0 & lane_lt), a1 = at + n0 + __popc(bal1 & lane_lt);
+                if (c0 && a0 < (u32)LMAX) S.list[a0] = y0;
+                if (c1 && a1 < (u32)LMAX) S.list[a1] = y1;
+            }
+        }
+    }
+    __syncthreads();
+    const u32 nl = S.nlist;
+    if (nl == 0) return;
+    if (nl > (u32)LMAX) {
+        if (tid == 0) {
+            if (BP.redo) BP.redo[atomicAdd(&P.info->join_redo, 1u)] = tile;
+            else atomicOr(&P.info->join_fallback, 1u);
+        }
+        return;
+    }
+    // ---- 3. chains ----
+    auto slot_of = [&](u64 y) -> u32 { return (u32)(y >> P.slot_shift) & (SLOTS - 1); };
+    for (u32 i = tid; i < nl; i += JF_THREADS) S.next[i] = (unsigned short)atomicExch(&S.head[slot_of(S.list[i])], i);
+    __syncthreads();
+    // ---- 4. count, claim, write ----
+    u32 cnt = 0, nzmask = 0;
+    {
+        u32 k = 0;
+        for (u32 i = tid; i < nl; i += JF_THREADS, ++k) {
+            u32 j = S.next[i];
+            if (j == JN_NIL) continue;
+            const u64 y = S.list[i];
+            u32 c = 0;
+            for (; j != JN_NIL; j = S.next[j]) {
+                const u64 z = S.list[j];
+                u64 packed;
+                if ((y ^ z) < P.hlim && jn_pair(y, z, P, packed)) ++c;
+            }
+            if (c) nzmask |= 1u << k;
+            cnt += c;
+        }
+    }
+    if (!__syncthreads_or(cnt != 0)) return;
+    u32 inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const u32 t = __shfl_up_sync(SD_FULL, inc, o);
+        if (lane >= (u32)o) inc += t;
+    }
+    if (lane == 31) S.wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        const u32 w = lane < JF_NW ? S.wsum[lane] : 0u;
+        u32 winc = w;
+#pragma unroll
+        for (int o = 1; o < JF_NW; o <<= 1) {
+            const u32 t = __shfl_up_sync(SD_FULL, winc, o);
+            if (lane >= (u32)o) winc += t;
+        }
+        if (lane < JF_NW) S.wsum[lane] = winc - w;
+        if (lane == JF_NW - 1) {
+            const u64 base = (u64)atomicAdd((unsigned long long*)&P.info->n_cand, (unsigned long long)winc);
+            // does not fit the window: nothing is written
+            if (base + winc > P.win_hi) atomicOr(&P.info->join_fallback, 2u), S.base = ~0ull;
+            else S.base = base;
+        }
+    }
+    __syncthreads();
+    if (S.base == ~0ull) return;
+    u64 at = S.base + S.wsum[warp] + inc - cnt;
+    for (u32 m = nzmask, k = 0; m; m >>= 1, ++k)
+        if (m & 1u) {
+            const u32 i = tid + k * JF_THREADS;
+            const u64 y = S.list[i];
+            for (u32 j = S.next[i]; j != JN_NIL; j = S.next[j]) {
+                const u64 z = S.list[j];
+                u64 packed;
+                if ((y ^ z) < P.hlim && jn_pair(y, z, P, packed)) P.cand[at++] = packed;
+            }
+        }
+}
+
+constexpr int JB_LMAX_L = 8192;
+
 }  // namespace
 
 i64 sd_join_tiles(i64 n_records) { return (n_records + JN_T - 1) / JN_T; }
@@ -687,4 +852,54 @@ cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* c
     k_join<<<(unsigned)tiles, JN_THREADS, smem, st>>>(P);
     if (launches) ++*launches;
     return cudaGetLastError();
+}
+
+// ---- bucket join of the fused pipeline ------------------------------------------------------------
+// buckets: nbuckets regions of `cap` records with counts cnt.  lay.sort_bits = the partitioned bits.
+// Step 1 (tiles == nullptr): small-list instance over all bucket groups, overflowing groups land in
+// redo[0 .. info->join_redo).  Step 2 (tiles = redo, n_tiles = join_redo): large-list instance.
+template <bool K32>
+static cudaError_t jn_launch_bkt(const JoinBktParams& BP, unsigned grid, bool large, cudaStream_t st) {
+    static bool attr_set = false;
+    auto ks = k_join_bkt<K32, JF_LMAX_S, JF_SLOTB_S, JF_MINB_S>;
+    auto kl = k_join_bkt<K32, JB_LMAX_L, JF_SLOTB_L, 2>;
+    constexpr size_t ss = sizeof(JoinFastSmem<JF_LMAX_S, JF_SLOTB_S>), sl = sizeof(JoinFastSmem<JB_LMAX_L, JF_SLOTB_L>);
+    cudaError_t e;
+    if (!attr_set) {
+        if ((e = cudaFuncSetAttribute(ks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ss)) != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(kl, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sl)) != cudaSuccess) return e;
+        attr_set = true;
+    }
+    if (large) kl<<<grid, JF_THREADS, sl, st>>>(BP);
+    else ks<<<grid, JF_THREADS, ss, st>>>(BP);
+    return cudaGetLastError();
+}
+
+u32 sd_join_bkt_group(i64 n_records, u32 nbuckets) {  // buckets per block: about 4096 records
+    const i64 avg = std::max<i64>(1, n_records / nbuckets);
+    return (u32)std::min<i64>(std::max<i64>(1, 4096 / avg), 256);
+}
+
+cudaError_t sd_join_bkt(const u64* buckets, const u32* cnt, u32 cap, u32 nbuckets, u32 group, const Layout& lay, u64* cand,
+                        u64 window, const u32* tiles, u32 n_tiles, u32* redo, DevInfo* info, cudaStream_t st, i64* launches) {
+    cudaError_t e;
+    if (!tiles) {
+        if ((e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
+        if ((e = cudaMemsetAsync(&info->join_fallback, 0, 2 * sizeof(u32), st)) != cudaSuccess) return e;  // and join_redo
+        n_tiles = (nbuckets + group - 1) / group;
+    }
+    if (n_tiles == 0) return cudaSuccess;
+    JoinBktParams BP{};
+    BP.j = jn_params(buckets, 0, lay, cand, window, info);
+    BP.j.win_lo = 0;
+    BP.j.win_hi = window;
+    BP.cnt = cnt;
+    BP.cap = cap;
+    BP.nbuckets = nbuckets;
+    BP.group = group;
+    BP.tiles = tiles;
+    BP.redo = tiles ? nullptr : redo;
+    if (launches) ++*launches;
+    const bool k32 = BP.j.bm_shift >= 32;
+    return k32 ? jn_launch_bkt<true>(BP, n_tiles, tiles != nullptr, st) : jn_launch_bkt<false>(BP, n_tiles, tiles != nullptr, st);
 }

@@ -44,6 +44,10 @@ cudaError_t sd_sort_hist_scan(void* scratch, int npass, cudaStream_t st, i64* la
 cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, int stable, void* scratch, cudaStream_t st,
                            u64** result, i64* launches);
 
+// level-2 partition of the fused pipeline: bins (256 x cap1) -> buckets ((256 << b2) x cap2)
+cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u32* cnt2, i64 cap2, int b2, int shift,
+                     DevInfo* info, cudaStream_t st, i64* launches);
+
 // ---- generate.cu --------------------------------------------------------------------------------
 cudaError_t sd_init_tables();  // fills the __constant__ tables once per process
 cudaError_t sd_prepare(SeqSetDev s, int d, int is_b, DevInfo* info, cudaStream_t st, i64* launches);
@@ -58,6 +62,12 @@ cudaError_t sd_scan_counts(const u32* cnt, i64 n, u64* rec_off, u64* lb_status, 
 // digits starting at bit hist_bit of the record into ghist
 cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, const u64* rec_off, u64* records,
                         u32* ghist, int hist_bit, int npass, DevInfo* info, cudaStream_t st, i64* launches);
+
+// Fused fast path: generation + level-1 partition into 256 bins of cap1 records (cur: 256 cursors =
+// the bin counts afterwards).  info->part_overflow != 0: a bin was full, redo with the exact pipeline.
+bool sd_gen_part_applies(const Layout& lay, int width);
+cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1, DevInfo* info,
+                        cudaStream_t st, i64* launches);
 
 // ---- join.cu ------------------------------------------------------------------------------------
 i64 sd_join_tiles(i64 n_records);
@@ -77,6 +87,12 @@ cudaError_t sd_join_fast(const u64* records, i64 n_records, const Layout& lay, u
                          DevInfo* info, cudaStream_t st, i64* launches);
 cudaError_t sd_join_fast_redo(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, const u32* redo,
                               u32 n_redo, DevInfo* info, cudaStream_t st, i64* launches);
+
+// Bucket join of the fused pipeline (see join.cu).  tiles == nullptr: first step over all bucket groups
+// (clears n_cand / join_fallback / join_redo, fills redo); else the redo step over n_tiles listed groups.
+u32 sd_join_bkt_group(i64 n_records, u32 nbuckets);
+cudaError_t sd_join_bkt(const u64* buckets, const u32* cnt, u32 cap, u32 nbuckets, u32 group, const Layout& lay, u64* cand,
+                        u64 window, const u32* tiles, u32 n_tiles, u32* redo, DevInfo* info, cudaStream_t st, i64* launches);
 
 // ---- verify.cu ----------------------------------------------------------------------------------
 i64 sd_verify_tiles(i64 n);

@@ -316,6 +316,97 @@ __global__ void __launch_bounds__(THREADS, MINB) k_onesweep(const u64* __restric
         os_tile<THREADS, IPT, false>(key, out, tile_n, tile, shift, gbase, status, skeys, whist, wmask, s_gofs, s_warp);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Level-2 partition of the fused pipeline (k_part2).  Input: 256 level-1 bins of capacity cap1 with
+// their record counts cnt1 (written by k_gen2_part).  A tile of a bin is split on the next b2 hash bits
+// into that bin's 2^b2 BUCKETS, each a fixed-capacity region of cap2 records: bucket (bin, digit) lives
+// at ((bin << b2) + digit) * cap2 and cnt2 counts what it holds.  This is the grouping tile of
+// k_onesweep in claim mode — one shared-memory atomic per key returns its rank inside (tile, digit), one
+// global atomic per digit claims the tile's slice of the bucket, the tile leaves staged in digit order
+// — without histograms, tickets or look-back, because nothing downstream needs the records of a bucket
+// contiguous with the next bucket or in any order.  A bucket that would overflow raises
+// info->part_overflow (the host falls back to the exact pipeline).
+constexpr int P2_THREADS = 256, P2_IPT = 16, P2_TILE = P2_THREADS * P2_IPT;
+
+struct Part2Params {
+    const u64* bins;
+    const u32* cnt1;
+    u64 cap1;
+    u64* buckets;
+    u32* cnt2;
+    u32 cap2;
+    int b2, shift;  // digit = (record >> shift) & (2^b2 - 1)
+    u32 tiles_per_bin;
+    DevInfo* info;
+};
+
+__global__ void __launch_bounds__(P2_THREADS, 4) k_part2(const Part2Params P) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    u64* skeys = reinterpret_cast<u64*>(smem_raw);
+    __shared__ u32 bhist[256];
+    __shared__ u32 s_gofs[256];
+    __shared__ u32 s_warp[P2_THREADS / 32 + 1];
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 bin = blockIdx.x / P.tiles_per_bin, k0 = blockIdx.x % P.tiles_per_bin;
+    const u32 n_bin = (u32)min((u64)P.cnt1[bin], P.cap1);
+    const u32 base = k0 * P2_TILE;
+    if (base >= n_bin) return;
+    const u32 tile_n = min((u32)P2_TILE, n_bin - base);
+    const bool full = tile_n == (u32)P2_TILE;
+    const u64* in = P.bins + (u64)bin * P.cap1 + base;
+    const u32 dmask = (1u << P.b2) - 1u;
+    bhist[tid] = 0;
+    const u32 wbase = warp * (32 * P2_IPT);
+    u64 key[P2_IPT];
+#pragma unroll
+    for (int k = 0; k < P2_IPT; ++k) {
+        const u32 pos = wbase + 32 * k + lane;
+        key[k] = (full || pos < tile_n) ? in[pos] : 0ull;
+    }
+    __syncthreads();
+    u32 rank[P2_IPT / 2];  // two 16-bit ranks per word
+#pragma unroll
+    for (int k = 0; k < P2_IPT; ++k) {
+        u32 r = 0;
+        if (full || (wbase + 32 * k + lane) < tile_n) r = atomicAdd(&bhist[(u32)(key[k] >> P.shift) & dmask], 1u);
+        if (k & 1) rank[k >> 1] |= r << 16;
+        else rank[k >> 1] = r;
+    }
+    __syncthreads();
+    const u32 total = bhist[tid];
+    u32 claimed = 0;
+    bool dead = false;
+    if (total) {
+        claimed = atomicAdd(&P.cnt2[(bin << P.b2) + tid], total);
+        if (claimed + total > P.cap2) {
+            atomicOr(&P.info->part_overflow, 2u);
+            dead = true;
+        }
+    }
+    u32 tile_sum;
+    const u32 tstart = sd_block_excl_sum<P2_THREADS>(total, &tile_sum, s_warp);
+    bhist[tid] = tstart;
+    s_gofs[tid] = dead ? 0xffffffffu : ((bin << P.b2) + tid) * P.cap2 + claimed - tstart;
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < P2_IPT; ++k) {
+        if (full || (wbase + 32 * k + lane) < tile_n) {
+            const u32 r = (k & 1) ? (rank[k >> 1] >> 16) : (rank[k >> 1] & 0xffffu);
+            skeys[bhist[(u32)(key[k] >> P.shift) & dmask] + r] = key[k];
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < P2_IPT; ++k) {
+        const u32 pos = tid + k * P2_THREADS;
+        if (full || pos < tile_n) {
+            const u64 kk = skeys[pos];
+            const u32 g = s_gofs[(u32)(kk >> P.shift) & dmask];
+            if (g != 0xffffffffu) P.buckets[g + pos] = kk;
+        }
+    }
+}
+
 struct OsVariant {
     int threads, ipt;
     size_t smem;
@@ -410,5 +501,34 @@ cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass,
         std::swap(src, dst);
     }
     *result = src;
+    return cudaGetLastError();
+}
+
+// Level-2 partition of the fused pipeline: bins (256 x cap1, counts cnt1) -> buckets (2^(8+b2) x cap2,
+// counts cnt2, zeroed here).  shift = bit of the record where the b2-bit digit starts.  b2 == 0: no-op
+// for the caller (the bins are the buckets).
+cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u32* cnt2, i64 cap2, int b2, int shift,
+                     DevInfo* info, cudaStream_t st, i64* launches) {
+    static bool attr_set = false;
+    cudaError_t e;
+    constexpr size_t smem = (size_t)P2_TILE * 8;
+    if (!attr_set) {
+        if ((e = cudaFuncSetAttribute(k_part2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        attr_set = true;
+    }
+    if ((e = cudaMemsetAsync(cnt2, 0, ((size_t)256 << b2) * sizeof(u32), st)) != cudaSuccess) return e;
+    Part2Params P{};
+    P.bins = bins;
+    P.cnt1 = cnt1;
+    P.cap1 = (u64)cap1;
+    P.buckets = buckets;
+    P.cnt2 = cnt2;
+    P.cap2 = (u32)cap2;
+    P.b2 = b2;
+    P.shift = shift;
+    P.tiles_per_bin = (u32)((cap1 + P2_TILE - 1) / P2_TILE);
+    P.info = info;
+    k_part2<<<256 * P.tiles_per_bin, P2_THREADS, smem, st>>>(P);
+    if (launches) ++*launches;
     return cudaGetLastError();
 }

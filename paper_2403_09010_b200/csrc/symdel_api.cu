@@ -31,8 +31,8 @@ struct symdel_ctx {
     symdel_stats stats{};
     int opt_timing = 0;
     i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0, opt_general_gen = 0;
-    i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0, opt_join_general = 0;
-    DevInfo* h_info = nullptr;  // pinned
+    i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0, opt_join_general = 0, opt_exact = 0;
+    DevInfo* h_info = nullptr;  // pinned; followed by 256 u32 (the level-1 bin counts of the fused pipeline)
     void* arena = nullptr;      // device arena of the *_host entry points
     size_t arena_bytes = 0;
     cudaStream_t stream = nullptr;  // stream of the *_host entry points
@@ -87,15 +87,40 @@ u64 vcount_host(int L, int d) {
     return acc;
 }
 
+// Fused pipeline (generation + level-1 partition, level-2 partition, bucket join): fixed-capacity bins
+// and buckets sized for `nexp` expected records with hash-uniform keys, + 8 standard deviations.
+struct FusedPlan {
+    int b, b2;        // partitioned hash bits in all (8..16) and at level 2
+    i64 cap1, cap2;   // records per level-1 bin / level-2 bucket (multiples of 32)
+    i64 bins_rec, bkt_rec, nbuckets;
+};
+constexpr i64 FUSED_MAX_BUCKETS = 65536;
+FusedPlan plan_fused(i64 nexp) {
+    FusedPlan f{};
+    nexp = std::max<i64>(nexp, 1);
+    f.b = 8;
+    while (f.b < 16 && (double)nexp / std::pow(2.0, f.b) > 1800.0) ++f.b;
+    f.b2 = f.b - 8;
+    auto cap_of = [](double avg) { return (i64)((avg + 8.0 * std::sqrt(avg) + 64.0 + 31.0) / 32.0) * 32; };
+    f.cap1 = cap_of((double)nexp / 256.0);
+    f.nbuckets = (i64)256 << f.b2;
+    f.cap2 = f.b2 ? cap_of((double)nexp / (double)f.nbuckets) : 0;
+    f.bins_rec = 256 * f.cap1;
+    f.bkt_rec = f.b2 ? f.nbuckets * f.cap2 : 0;
+    return f;
+}
+
 i64 rec_bytes(i64 ncap, int npass) {
-    return 2 * align_up(ncap * 8) + align_up(sd_sort_scratch_bytes(ncap, npass)) + align_up((2 * sd_join_tiles(ncap) + 2) * 8);
+    const FusedPlan f = plan_fused(ncap);
+    return align_up(std::max(ncap, f.bins_rec) * 8) + align_up(std::max(ncap, f.bkt_rec) * 8) +
+           align_up(sd_sort_scratch_bytes(ncap, npass)) + align_up((2 * sd_join_tiles(ncap) + 2) * 8);
 }
 i64 cand_bytes(i64 ccap, int ppass) {
     return 2 * align_up(ccap * 8) + align_up(sd_sort_scratch_bytes(ccap, ppass)) + align_up((ccap / 256 + 2) * 8);
 }
 i64 fixed_bytes(i64 n_total) {
     return align_up((i64)sizeof(DevInfo)) + align_up(n_total * 4) + align_up((n_total + 1) * 8) +
-           align_up((sd_scan_tiles(n_total) + 1) * 8) + align_up(n_total * 48) + 4096;
+           align_up((sd_scan_tiles(n_total) + 1) * 8) + align_up(n_total * 48) + align_up((256 + 2 * FUSED_MAX_BUCKETS) * 4) + 4096;
 }
 
 struct Timer {
@@ -213,6 +238,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
 
     // ---- packed bit-plane table for the verifier ----
     void* slots = ws.take<char>(sd_pack_bytes(n_total, maxlen));
+    u32* fcnt = ws.take<u32>(256 + 2 * FUSED_MAX_BUCKETS);  // fused pipeline: level-1 cursors | level-2 counts | redo list
     if (!ws.ok) return SYMDEL_E_WORKSPACE;
     CK(sd_pack(A, B, maxlen, slots, st, &S.n_launches));
 
@@ -240,8 +266,10 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
         if (ncap < 4096) return SYMDEL_E_WORKSPACE;
         if (ctx->opt_force_chunks <= 0) P = (u32)std::max<i64>(1, (nmax + nmax / 8 + ncap - 1) / ncap);
     }
-    u64* recA = ws.take<u64>(ncap);
-    u64* recB = ws.take<u64>(ncap);
+    const FusedPlan fp = plan_fused(ncap);
+    u64* recA = ws.take<u64>(std::max(ncap, fp.bins_rec));
+    u64* recB = ws.take<u64>(std::max(ncap, fp.bkt_rec));
+    u32 *cur1 = fcnt, *cnt2 = fcnt + 256, *redo = fcnt + 256 + FUSED_MAX_BUCKETS;
     void* rec_scratch = ws.take<char>(sd_sort_scratch_bytes(ncap, npass_max));
     u64* tile_prefix = ws.take<u64>(2 * sd_join_tiles(ncap) + 2);
     const i64 cphys = ccap + cslack;
@@ -271,13 +299,64 @@ restart:
     CK(cudaMemsetAsync(&info->n_surv, 0, sizeof(u64) * 3, st));  // n_surv, n_out, n_unique
     for (u32 c = 0; c < P; ++c) {
         lay.chunk = c;
+        // ---- fused pipeline: generation + level-1 partition, level-2 partition, bucket join ----
+        bool fused_ok = false;
+        i64 C = 0, wend = 0, N = 0;
+        if (!ctx->opt_exact && ctx->opt_sort_bits < 0 && !ctx->opt_join_general && lay.hash_bits >= fp.b &&
+            sd_gen_part_applies(lay, width)) {
+            const size_t x0 = tm.mark();
+            lay.sort_bits = fp.b;
+            CK(cudaMemsetAsync(&info->part_overflow, 0, sizeof(u32), st));
+            CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, info, st, &S.n_launches));
+            const size_t x1 = tm.mark();
+            if (fp.b2)
+                CK(sd_part2(recA, cur1, fp.cap1, recB, cnt2, fp.cap2, fp.b2, lay.id_bits + lay.hash_bits - fp.b, info, st,
+                            &S.n_launches));
+            const size_t x2 = tm.mark();
+            const u64* bkt = fp.b2 ? recB : recA;
+            const u32* bcnt = fp.b2 ? cnt2 : cur1;
+            const u32 bcap = (u32)(fp.b2 ? fp.cap2 : fp.cap1), nb = (u32)fp.nbuckets;
+            const u32 group = sd_join_bkt_group(ncap, nb);
+            CK(sd_join_bkt(bkt, bcnt, bcap, nb, group, lay, candA, (u64)ccap, nullptr, 0, redo, info, st, &S.n_launches));
+            u32* h_cur = reinterpret_cast<u32*>(ctx->h_info + 1);
+            CK(cudaMemcpyAsync(h_cur, cur1, 256 * sizeof(u32), cudaMemcpyDeviceToHost, st));
+            rc = read_info(ctx, info, st);
+            if (rc) return rc;
+            if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+            fused_ok = !ctx->h_info->part_overflow && !ctx->h_info->join_fallback;
+            if (fused_ok && ctx->h_info->join_redo) {  // dense bucket groups: the large-list instance
+                S.join_redo_tiles += ctx->h_info->join_redo;
+                CK(sd_join_bkt(bkt, bcnt, bcap, nb, group, lay, candA, (u64)ccap, redo, ctx->h_info->join_redo, nullptr, info, st,
+                               &S.n_launches));
+                rc = read_info(ctx, info, st);
+                if (rc) return rc;
+                fused_ok = !ctx->h_info->join_fallback;
+            }
+            if (fused_ok) {
+                for (int i = 0; i < 256; ++i) N += h_cur[i];
+                C = (i64)ctx->h_info->n_cand;
+                wend = C;
+                const size_t x3 = tm.mark();
+                tm.span(ST_GEN, x0, x1);
+                tm.span(ST_SORT, x1, x2);
+                tm.span(ST_EMIT, x2, x3);
+                pass_count += fp.b2 ? 1 : 0;
+                S.sort_pass_records = N;
+                S.sort_bits = fp.b;
+                S.n_records += N;
+                S.n_candidates += C;
+                ++S.fused_chunks;
+            }
+        }
+        u64* sorted = nullptr;
+        if (!fused_ok) {
         const size_t e0 = tm.mark();
         // ---- S1: count, scan, generate ----
         CK(sd_count(A, B, lay, width, cnt, info, st, &S.n_launches));
         CK(sd_scan_counts(cnt, n_total, rec_off, scan_lb, info, st, &S.n_launches));
         rc = read_info(ctx, info, st);
         if (rc) return rc;
-        const i64 N = (i64)ctx->h_info->n_records;
+        N = (i64)ctx->h_info->n_records;
         if (N > ncap || N >= ((i64)1 << 30)) {
             if (ctx->opt_force_chunks > 0 && N <= ncap) return SYMDEL_E_TOO_MANY;
             P *= 2;
@@ -295,7 +374,6 @@ restart:
         CK(sd_sort_hist_scan(rec_scratch, npass, st, &S.n_launches));
         const size_t e1 = tm.mark();
         // ---- S2: radix partition on the top sort_bits (exactly npass onesweep launches between e1 and e2) ----
-        u64* sorted = nullptr;
         CK(sd_sort_passes(recA, recB, N, sort_begin, npass, ctx->opt_sort_stable ? 1 : 0, rec_scratch, st, &sorted,
                           &S.n_launches));
         const size_t e2 = tm.mark();
@@ -323,8 +401,8 @@ restart:
             if (rc) return rc;
             if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
         }
-        const i64 C = (i64)ctx->h_info->n_cand;
-        i64 wend = (i64)ctx->h_info->win_end;
+        C = (i64)ctx->h_info->n_cand;
+        wend = (i64)ctx->h_info->win_end;
         S.n_candidates += C;
         const size_t e3 = tm.mark();
         tm.span(ST_GEN, e0, e1);
@@ -332,6 +410,7 @@ restart:
         tm.span(ST_EMIT, e2, e3);
         pass_count += npass;
         S.sort_pass_records = N;
+        }  // exact pipeline
         for (i64 w0 = 0; w0 < C;) {
             const size_t f0 = tm.mark();
             if (w0 > 0) {
@@ -498,7 +577,7 @@ int symdel_create(symdel_ctx** out, int device) {
     symdel_ctx* ctx = new symdel_ctx();
     ctx->device = device;
     cudaError_t e = cudaSetDevice(device);
-    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_info, sizeof(DevInfo));
+    if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_info, sizeof(DevInfo) + 256 * sizeof(u32));
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = sd_init_tables();
     if (e != cudaSuccess) {
@@ -536,6 +615,7 @@ int symdel_set_option(symdel_ctx* ctx, int option, int64_t value) {
         case SYMDEL_OPT_SORT_STABLE: ctx->opt_sort_stable = value != 0; break;
         case SYMDEL_OPT_SORT_GROUPING: ctx->opt_sort_grouping = value != 0; break;
         case SYMDEL_OPT_JOIN_GENERAL: ctx->opt_join_general = value != 0; break;
+        case SYMDEL_OPT_EXACT_PIPELINE: ctx->opt_exact = value != 0; break;
         case SYMDEL_OPT_NO_THINNING: ctx->opt_no_thinning = value != 0; break;
         case SYMDEL_OPT_GENERAL_GENERATE: ctx->opt_general_gen = value != 0; break;
         case SYMDEL_OPT_SORT_VARIANT:

@@ -18,7 +18,7 @@ _lib = None
 OK = 0
 E_ARG, E_OFFSETS, E_TOO_LONG, E_RESIDUE, E_TOO_MANY, E_WORKSPACE, E_CAPACITY, E_CUDA, E_INTERNAL = range(-1, -10, -1)
 OPT_TIMING, OPT_FORCE_CHUNKS, OPT_CAND_CAPACITY, OPT_HASH_BITS, OPT_NO_THINNING, OPT_SORT_VARIANT, OPT_GENERAL_GENERATE = 1, 2, 3, 4, 5, 6, 7
-OPT_SORT_BITS, OPT_SORT_STABLE, OPT_SORT_GROUPING, OPT_JOIN_GENERAL = 8, 9, 10, 11
+OPT_SORT_BITS, OPT_SORT_STABLE, OPT_SORT_GROUPING, OPT_JOIN_GENERAL, OPT_EXACT_PIPELINE = 8, 9, 10, 11, 12
 D_MAX, L_MAX = 4, 64
 
 EXPORTS = [
@@ -36,7 +36,7 @@ class Stats(C.Structure):
         ("hash_bits", C.c_int32), ("id_bits", C.c_int32), ("sort_bits", C.c_int32), ("join_general", C.c_int32),
         ("ms_prepare", C.c_float), ("ms_generate", C.c_float), ("ms_sort", C.c_float), ("ms_emit", C.c_float),
         ("ms_dedup", C.c_float), ("ms_verify", C.c_float), ("ms_total", C.c_float), ("ms_sort_pass_avg", C.c_float),
-        ("sort_pass_records", C.c_int64), ("join_redo_tiles", C.c_int64),
+        ("sort_pass_records", C.c_int64), ("fused_chunks", C.c_int64), ("join_redo_tiles", C.c_int64),
     ]
 
     def as_dict(self):

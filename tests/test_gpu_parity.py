@@ -288,6 +288,7 @@ def test_validation_protocol_5000(sd, ctx, oracle, family, d):
     {"SORT_BITS": 255, "CAND_CAPACITY": 1500}, {"HASH_BITS": 13, "SORT_BITS": 8},
     {"SORT_BITS": 8, "HASH_BITS": 12, "CAND_CAPACITY": 100000, "FORCE_CHUNKS": 2},
     {"JOIN_GENERAL": 1}, {"JOIN_GENERAL": 1, "FORCE_CHUNKS": 3}, {"JOIN_GENERAL": 1, "SORT_BITS": 255},
+    {"EXACT_PIPELINE": 1}, {"EXACT_PIPELINE": 1, "FORCE_CHUNKS": 2},
 ])
 def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
     """P-11: chunk count, candidate-buffer windows, key width and thinning change memory use and
@@ -309,8 +310,11 @@ def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
         assert st["join_general"] >= 1  # the pairs exceed one window: the fast join kernel hands over
     if "JOIN_GENERAL" in opts:
         assert st["join_general"] == st["n_chunks"]
-    if not opts:
-        assert st["join_general"] == 0
+    if (not opts or set(opts) <= {"FORCE_CHUNKS", "HASH_BITS", "NO_THINNING"}) and opts.get("HASH_BITS", 64) >= 16:
+        assert st["join_general"] == 0  # (a hash of 8 bits piles thousands of records on each key: the lists overflow)
+        assert st["fused_chunks"] == st["n_chunks"]
+    if "EXACT_PIPELINE" in opts or "GENERAL_GENERATE" in opts or "SORT_BITS" in opts:
+        assert st["fused_chunks"] == 0
 
 
 @pytest.mark.parametrize("copies,sort_bits,general,expect_general", [
@@ -333,6 +337,19 @@ def test_join_dense_runs(sd, oracle, copies, sort_bits, general, expect_general)
     assert st["join_general"] == expect_general
     if copies == 10 and sort_bits == 0:
         assert st["join_redo_tiles"] > 0  # dense tiles overflow the small list and are redone with the large one
+
+
+def test_fused_bin_overflow_falls_back(sd, oracle):
+    """The fused pipeline sizes its bins for hash-uniform keys.  100 exact copies of each of 600 sequences
+    at d = 0 (one record per sequence) pile whole groups of 100 onto single hash values: some bin runs
+    full, the chunk is redone by the exact pipeline, the result is the same (reading A-7)."""
+    base = synth.tcr_set(600, 33)
+    rep = base.take(np.repeat(np.arange(base.n), 100))
+    c = sd.Context(0)
+    exp = oracle.symdel_self(rep.seqs, rep.offsets, 0)
+    assert_same(run_self(sd, c, rep, 0, capacity=4_000_000), exp)
+    assert c.symdel_get_stats()["fused_chunks"] == 0
+    assert len(exp[0]) == base.n * 100 * 99 // 2
 
 
 def test_small_workspace_forces_chunking(torch, sd, ctx, oracle):
