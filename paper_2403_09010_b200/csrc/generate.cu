@@ -20,6 +20,8 @@
 // Order: records are written in ascending id, at rec_off[id] + rank, where rec_off is the exclusive
 // scan of the per-sequence counts produced by the count pass — no atomics, deterministic layout,
 // and (with the stable sort) ids ascend inside every run of equal keys.
+#include <cstddef>
+
 #include "kernels.h"
 
 namespace {
@@ -628,53 +630,56 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
 // histogram: the order of the records inside a bin is irrelevant to the join.  A record that finds its
 // digit's slots full goes straight to its bin (one global atomic).  A bin that would overflow raises
 // info->part_overflow: the host then redoes the chunk with the exact (histogram-based) pipeline.
-constexpr int GP_THREADS = 256, GP_NW = GP_THREADS / 32, GP_S = 32;
-#ifndef GP_FLUSH_AT
-#define GP_FLUSH_AT 2300
+#ifndef GP_THREADS
+#define GP_THREADS 256
 #endif
+#ifndef GP_FLUSH_AT
+#define GP_FLUSH_AT 2800
+#endif
+#ifndef GP_MINB
+#define GP_MINB 3
+#endif
+constexpr int GP_NW = GP_THREADS / 32, GP_S = 32;
+static_assert(GP_THREADS >= 256 && GP_THREADS % 32 == 0, "one thread per digit in the flush");
 
 struct GenPartShared {
-    u64 stage[256 * GP_S];
+    u64 stage[256 * GP_S];  // digit dg, rank r -> stage[dg * GP_S + ((r + dg) & (GP_S - 1))] (skewed: ranks are alike across digits)
     u64 U[GP_NW][32];
     u64 V[GP_NW][32];
     u64 R[32];
     u64 Bpow[33];
-    u32 cnt[256];   // records staged per digit since the last flush (may exceed GP_S: the excess went to the bins directly)
-    u32 gpos[256];  // flush: claimed start inside the bin; 0xffffffff = bin full
-    u32 total;      // records staged since the last flush
+    u32 cnt[256];     // records staged per digit since the last flush (may exceed GP_S: the excess went to the bins directly)
+    uint2 fl[256];    // flush: {index of the claimed segment in bins (0xffffffff = bin full), records to copy}
+    u32 total;        // records staged since the last flush
     unsigned char map[GP_NW][32];
 };
 
+static_assert(offsetof(GenPartShared, V) - offsetof(GenPartShared, U) == GP_NW * 256, "k_gen2_part addresses V[warp] through U[warp]");
+
 struct GenPartParams {
     GenParams g;
-    u64* bins;    // 256 bins of cap1 records
+    u64* bins;    // 256 bins of cap1 records (256 * cap1 < 2^32)
     u32* cur;     // 256 bin cursors (zeroed by the host)
-    u64 cap1;
+    u32 cap1;
 };
 
-__device__ __forceinline__ u32 gp_atoms_inc(u32* p) {  // plain ATOMS.ADD 1 with return (no compiler-inserted aggregation)
-    u32 old;
-    asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(old) : "r"((u32)__cvta_generic_to_shared(p)) : "memory");
-    return old;
-}
-
-template <bool CHUNKED>
-__global__ void __launch_bounds__(GP_THREADS, 3) k_gen2_part(GenPartParams PP) {
+template <bool CHUNKED, bool PLAIN>
+__global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams PP) {
     extern __shared__ __align__(16) unsigned char gen_smem[];
     GenPartShared& sh = *reinterpret_cast<GenPartShared*>(gen_smem);
     const GenParams& P = PP.g;
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid < 32) sh.R[tid] = c_R[tid];
     if (tid < 33) sh.Bpow[tid] = c_Bpow[tid];
-    sh.cnt[tid] = 0;
+    if (tid < 256) sh.cnt[tid] = 0;
     if (tid == 0) sh.total = 0;
     __syncthreads();
     const int d = P.d;
     const bool thinning = P.thinning != 0;
     const u64 binv1 = c_Binv[1], binv2 = c_Binv[2];
-    const int kshift = 64 - P.hash_bits, id_bits = P.id_bits;
-    const bool plain = kshift == id_bits;  // the record is the hash with its low id_bits replaced by the id
-    const u64 idmask = (1ull << id_bits) - 1ull;
+    const int kshift = 64 - P.hash_bits, id_bits = P.id_bits;  // PLAIN: kshift == id_bits, the record is the hash with its low id_bits replaced by the id
+    const u32 idmask_lo = id_bits >= 32 ? 0xffffffffu : ((1u << id_bits) - 1u);
+    const u32 cnt_sa = (u32)__cvta_generic_to_shared(sh.cnt);
     u64* const Uw = sh.U[warp];
     u64* const Vw = sh.V[warp];
     u32 made = 0;  // records this lane staged since the warp last reported
@@ -683,13 +688,16 @@ __global__ void __launch_bounds__(GP_THREADS, 3) k_gen2_part(GenPartParams PP) {
         if (CHUNKED) valid = valid && gen_chunk_of(h, P.n_chunks) == P.chunk;
         if (valid) {
             const u32 dg = (u32)(h >> 56);
-            const u64 rec = plain ? ((h & ~idmask) | gid) : (((h >> kshift) << id_bits) | gid);
-            const u32 r = gp_atoms_inc(&sh.cnt[dg]);
+            u64 rec;
+            if (PLAIN) rec = ((u64)(u32)(h >> 32) << 32) | (((u32)h & ~idmask_lo) | (u32)gid);  // id_bits <= 31 here
+            else rec = ((h >> kshift) << id_bits) | gid;
+            u32 r;  // plain ATOMS.ADD with return (no compiler-inserted aggregation)
+            asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(r) : "r"(cnt_sa + dg * 4u) : "memory");
             if (r < (u32)GP_S) {
-                sh.stage[dg * GP_S + r] = rec;
+                sh.stage[dg * GP_S + ((r + dg) & (GP_S - 1))] = rec;
             } else {
                 const u32 at = atomicAdd(&PP.cur[dg], 1u);
-                if ((u64)at < PP.cap1) PP.bins[(u64)dg * PP.cap1 + at] = rec;
+                if (at < PP.cap1) PP.bins[(u64)dg * PP.cap1 + at] = rec;
                 else atomicOr(&P.info->part_overflow, 1u);
             }
             ++made;
@@ -775,19 +783,30 @@ __global__ void __launch_bounds__(GP_THREADS, 3) k_gen2_part(GenPartParams PP) {
                 push(active && a == 0, AL + (u64)(L + 1) * K_LEN, gid);
                 if (d >= 1) push(canon1, Uv + binv1 * AL + (u64)L * K_LEN, gid);
                 if (d >= 2) {
+                    // pairs {a, (a + dl) mod L}: lane a runs dl = 1 .. dlmax (every unordered pair once); the
+                    // partner b sits after a (no wrap: H = U[a] + V[b]) or before it (wrap: H = U[b] + V[a])
                     const u64 C2 = binv2 * AL + (u64)(L - 1) * K_LEN;
+                    const u64 UC = Uv + C2, VC = binv1 * Uv + C2;
                     const u32 half = __reduce_max_sync(SD_FULL, L >> 1);
-                    const u32 m1s = m1 >> seg_start, madjs = madj >> seg_start;  // segment-relative masks
-                    const u64* const Us = Uw + seg_start;
-                    const u64* const Vs = Vw + seg_start;
-                    for (u32 dl = 1; dl <= half; ++dl) {
+                    const u32 dlmax = active ? ((L - 1) >> 1) + (((L & 1u) == 0u && a < (L >> 1)) ? 1u : 0u) : 0u;
+                    const u32 m1s = m1 >> seg_start;  // segment-relative mask
+                    const bool c1a = canon1;
+                    const u32 uv_sa = (u32)__cvta_generic_to_shared(Uw + seg_start);  // V[warp] lies GP_NW * 256 bytes after U[warp]
+                    {   // dl = 1: the adjacent pair {a, a + 1} has its own rule; the wrapped pair {0, L - 1} is adjacent only if L == 2
+                        const bool wrap = a + 1 >= L;
+                        const u32 b = wrap ? 0u : a + 1;
+                        const bool ok = wrap ? (L == 2u ? ((madj >> seg_start) & 1u) != 0u : (c1a && (m1s & 1u))) : adjok;
+                        u64 o;
+                        asm volatile("ld.shared.u64 %0, [%1];" : "=l"(o) : "r"(uv_sa + b * 8u + (wrap ? 0u : (u32)(GP_NW * 256))));
+                        push(1u <= dlmax && ok, o + (wrap ? VC : UC), gid);
+                    }
+                    for (u32 dl = 2; dl <= half; ++dl) {
                         u32 b = a + dl;
-                        b = (b >= L) ? b - L : b;
-                        const u32 p1 = min(a, b) & 31u, p2 = max(a, b) & 31u;
-                        const bool on = (2 * dl < L) || (2 * dl == L && a < dl);  // false on idle lanes (L = 0)
-                        const u32 both = (m1s >> p1) & (m1s >> p2);
-                        const u32 t = (p2 - p1 == 1u) ? (madjs >> p1) : both;
-                        push(on && (t & 1u), Us[p1] + Vs[p2] + C2, gid);
+                        const bool wrap = b >= L;
+                        b = wrap ? b - L : b;
+                        u64 o;
+                        asm volatile("ld.shared.u64 %0, [%1];" : "=l"(o) : "r"(uv_sa + (b & 31u) * 8u + (wrap ? 0u : (u32)(GP_NW * 256))));
+                        push(dl <= dlmax && c1a && ((m1s >> (b & 31u)) & 1u), o + (wrap ? VC : UC), gid);
                     }
                 }
                 __syncwarp();  // U/V/map are reused by the next batch
@@ -803,25 +822,27 @@ __global__ void __launch_bounds__(GP_THREADS, 3) k_gen2_part(GenPartParams PP) {
         const int any_more = __syncthreads_or(more);
         const u32 staged = sh.total;
         if (staged > (u32)GP_FLUSH_AT || (!any_more && staged > 0)) {
-            const u32 cn_ = min(sh.cnt[tid], (u32)GP_S);
-            u32 g = 0;
-            if (cn_) {
-                g = atomicAdd(&PP.cur[tid], cn_);
-                if ((u64)g + cn_ > PP.cap1) {
-                    atomicOr(&P.info->part_overflow, 1u);
-                    g = 0xffffffffu;
+            if (tid < 256) {
+                const u32 cn_ = min(sh.cnt[tid], (u32)GP_S);
+                u32 g = 0;
+                if (cn_) {
+                    g = atomicAdd(&PP.cur[tid], cn_);
+                    if (g + cn_ > PP.cap1) {
+                        atomicOr(&P.info->part_overflow, 1u);
+                        g = 0xffffffffu;
+                    } else {
+                        g += tid * PP.cap1;
+                    }
                 }
-            }
-            sh.gpos[tid] = g;
-            __syncthreads();
-#pragma unroll 4
-            for (int dd = 0; dd < 32; ++dd) {
-                const u32 dg = warp * 32 + dd;
-                const u32 c2 = min(sh.cnt[dg], (u32)GP_S), g2 = sh.gpos[dg];
-                if (lane < c2 && g2 != 0xffffffffu) PP.bins[(u64)dg * PP.cap1 + g2 + lane] = sh.stage[dg * GP_S + lane];
+                sh.fl[tid] = make_uint2(g, g == 0xffffffffu ? 0u : cn_);
             }
             __syncthreads();
-            sh.cnt[tid] = 0;
+            for (u32 dg = warp; dg < 256; dg += GP_NW) {
+                const uint2 f = sh.fl[dg];
+                if (lane < f.y) PP.bins[f.x + lane] = sh.stage[dg * GP_S + ((lane + dg) & (GP_S - 1))];
+            }
+            __syncthreads();
+            if (tid < 256) sh.cnt[tid] = 0;
             if (tid == 0) sh.total = 0;
             __syncthreads();
         }
@@ -992,18 +1013,20 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     PP.g.info = info;
     PP.bins = bins;
     PP.cur = cur;
-    PP.cap1 = cap1;
+    PP.cap1 = (u32)cap1;
+    typedef void (*Kern)(GenPartParams);
+    static const Kern kerns[4] = {k_gen2_part<false, false>, k_gen2_part<false, true>, k_gen2_part<true, false>, k_gen2_part<true, true>};
     static bool attr_set = false;
     cudaError_t e;
     if (!attr_set) {
-        if ((e = cudaFuncSetAttribute(k_gen2_part<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GenPartShared))) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(k_gen2_part<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GenPartShared))) != cudaSuccess) return e;
+        for (Kern k : kerns)
+            if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GenPartShared))) != cudaSuccess) return e;
         attr_set = true;
     }
     if ((e = cudaMemsetAsync(cur, 0, 256 * sizeof(u32), st)) != cudaSuccess) return e;
-    const int grid = (int)std::min<i64>((PP.g.groups_total + GP_NW - 1) / GP_NW, 148 * 3);
-    if (lay.n_chunks > 1) k_gen2_part<true><<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
-    else k_gen2_part<false><<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
+    const int grid = (int)std::min<i64>((PP.g.groups_total + GP_NW - 1) / GP_NW, 148 * GP_MINB);
+    const bool plain = lay.hash_bits + lay.id_bits == 64 && lay.id_bits <= 31;
+    kerns[(lay.n_chunks > 1 ? 2 : 0) + (plain ? 1 : 0)]<<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
     if (launches) ++*launches;
     return cudaGetLastError();
 }
