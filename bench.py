@@ -43,12 +43,12 @@ def load_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def load_traffic():
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture."""
+def load_traffic(kernel: str):
+    """dram bytes per launch of `kernel` from the committed ncu --set full capture (profiles/traffic.json)."""
     p = ROOT / "profiles" / "traffic.json"
     if p.exists():
         try:
-            return json.loads(p.read_text()).get("k_onesweep_records_dram_bytes_per_launch")
+            return json.loads(p.read_text()).get("dram_bytes_per_launch", {}).get(kernel)
         except Exception:
             return None
     return None
@@ -250,36 +250,58 @@ def main():
 
     st = stats_acc[-1]
     n_rec = st["sort_pass_records"]
-    pass_ms = float(np.mean([x["ms_sort_pass_avg"] for x in stats_acc]))
+    n_cand = st["n_candidates"]
+    fused = st["fused_chunks"] == st["n_chunks"]
     peak, peak_src = load_peak()
-    achieved = 16.0 * n_rec / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
     stage = {k: float(np.mean([x[k] for x in stats_acc])) for k in
              ("ms_prepare", "ms_generate", "ms_sort", "ms_emit", "ms_dedup", "ms_verify", "ms_total")}
-    # algorithmic bytes of the whole step: 8 (gen write) + 16/pass + 8 (emit read) per record,
-    # 8 + 8 + 16/pass + 8 per candidate, 12 per output, + inputs
-    npass = st["hash_bits"] // 8
+    in_bytes = s.seqs.size + 8 * (s.n + 1)
     ppass = (2 * st["id_bits"] + 7) // 8
-    step_bytes = n_rec * (8 + 16 * npass + 8) + st["n_candidates"] * (8 + 8 + 16 * ppass + 8) + n_out * 12 + s.seqs.size + 8 * (s.n + 1)
+    # Algorithmic bytes.  Fused pipeline: generation writes 8 B/record into the level-1 bins,
+    # the level-2 partition reads and writes 8 B/record, the join reads 8 B/record and writes 8 B/candidate.
+    # Exact pipeline: 8 (write) + 16 per onesweep pass + 8 (join read) per record.
+    npass = 1 if fused else st["sort_bits"] // 8
+    pass_ms = float(np.mean([x["ms_sort_pass_avg"] for x in stats_acc]))
+    step_bytes = (n_rec * (8 + 16 * npass + 8) + n_cand * (8 + 8 + 16 * ppass + 8) + n_out * 12 + in_bytes)
+    kname = "k_part2" if fused else "k_onesweep"
+    achieved = 16.0 * n_rec / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
+
+    def hbm(name, ms_key, nbytes):
+        gbs = nbytes / (stage[ms_key] * 1e-3) / 1e9 if stage[ms_key] > 0 else 0.0
+        return {"stage": name, "ms": stage[ms_key], "share_of_step": stage[ms_key] / stage["ms_total"],
+                "algorithmic_bytes": int(nbytes), "achieved_gbs": gbs, "frac_of_peak": gbs / peak}
+
+    stages = [
+        hbm("generate + level-1 partition (k_gen2_part; instruction-issue bound, see DESIGN.md)" if fused else
+            "count + scan + generate", "ms_generate", 8 * n_rec + in_bytes),
+        hbm("level-2 partition (k_part2)" if fused else f"{npass} onesweep passes", "ms_sort", 16 * n_rec * npass),
+        hbm("join (k_join_bkt)" if fused else "join", "ms_emit", 8 * n_rec + 8 * n_cand),
+        hbm(f"candidate sort ({ppass} onesweep passes)", "ms_dedup", n_cand * (8 + 16 * ppass)),
+        hbm("unique + verify + unpack", "ms_verify", 8 * n_cand + 64 * st["n_unique"] + 12 * n_out),
+    ]
     line = {
         "metric": METRIC, "value": job_value(n_out, world, ms), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u64", "data": "synthetic",
         "config": {"workload": WORKLOAD if args.config == 3 else f"config {args.config}", "n": s.n, "d": d,
-                   "pairs_per_step": n_out, "records": n_rec, "candidates": st["n_candidates"],
+                   "pairs_per_step": n_out, "records": n_rec, "candidates": n_cand,
                    "unique_candidates": st["n_unique"], "hash_bits": st["hash_bits"], "id_bits": st["id_bits"],
+                   "partition_bits": st["sort_bits"], "pipeline": "fused" if fused else "exact",
                    "chunks": st["n_chunks"], "l2": "flushed between steps (512 MiB memset, untimed)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "wall_time_s": ms * 1e-3, "records_per_s": world * n_rec / (ms * 1e-3),
         "step_hbm_gbs": step_bytes / (ms * 1e-3) / 1e9, "step_hbm_frac": step_bytes / (ms * 1e-3) / 1e9 / peak,
-        "stage_ms": stage,
+        "stage_ms": stage, "stages": stages,
         "e2e": {"value": job_value(n_out, world, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": int(s.seqs.nbytes + s.offsets.nbytes), "d2h_bytes_per_step": int(12 * n_out),
                 "api": "symdel_self_host (pinned host buffers)"},
         "gpu_launches": int(sum(x["n_launches"] for x in stats_acc)),
-        "roofline": {"bound": "hbm", "kernel": "k_onesweep (one 8-bit LSD pass over the variant records)",
+        "roofline": {"bound": "hbm",
+                     "kernel": f"{kname} (one 8-bit radix-partition pass over the variant records: the sort stage)",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": load_traffic(), "peak_source": peak_src,
+                     "traffic": load_traffic(kname), "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": 16 * n_rec, "launch_ms": pass_ms,
+                     "share_of_step": stage["ms_sort"] / stage["ms_total"],
                      "frac_of_nominal_8000": achieved / 8000.0},
         "clocks": clocks,
     }
