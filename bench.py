@@ -157,6 +157,9 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); the metric is quoted on 3")
     ap.add_argument("--ref-sample", type=int, default=150000, help="sequences in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--prefix", type=int, default=0,
+                    help="prefix-truncated candidate generation (App. B; same output, fewer records); default off: the "
+                         "headline generates every deletion variant of every sequence")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -182,6 +185,8 @@ def main():
     s = sets[0]
     ctx = symdel.Context(local)
     ctx.symdel_set_option(symdel.OPT_TIMING, 1)
+    if args.prefix:
+        ctx.symdel_set_option(symdel.OPT_PREFIX_LEN, args.prefix)
     dev = torch.device("cuda", local)
     seqs_d = torch.from_numpy(s.seqs).to(dev)
     offs_d = torch.from_numpy(s.offsets).to(dev)
@@ -287,6 +292,7 @@ def main():
                    "pairs_per_step": n_out, "records": n_rec, "candidates": n_cand,
                    "unique_candidates": st["n_unique"], "hash_bits": st["hash_bits"], "id_bits": st["id_bits"],
                    "partition_bits": st["sort_bits"], "pipeline": "fused" if fused else "exact",
+                   "prefix_len": args.prefix or None,
                    "chunks": st["n_chunks"], "l2": "flushed between steps (512 MiB memset, untimed)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "wall_time_s": ms * 1e-3, "records_per_s": world * n_rec / (ms * 1e-3),

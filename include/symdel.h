@@ -94,6 +94,7 @@ enum {
     SYMDEL_OPT_SORT_STABLE = 9,   /* [0] 1: every S2 pass takes the stable (ties keep input order) tile path (test hook; results are identical) */
     SYMDEL_OPT_JOIN_GENERAL = 11, /* [0] 1: always run the general join kernel (windowed output, chunked buckets) instead of trying the fast one first (test hook; results are identical) */
     SYMDEL_OPT_EXACT_PIPELINE = 12, /* [0] 1: never use the fused pipeline (fixed-capacity bins); always count, scan, generate, onesweep-partition on exact histograms, windowed join (the path the fused one falls back to when a bin overflows; results are identical) */
+    SYMDEL_OPT_PREFIX_LEN = 13,   /* [0] P > 0: prefix-truncated candidate generation (App. B; XTNeighbor uses 18): deletion variants are generated from the first P residues of every sequence, verification stays on the whole sequences.  Exact for P > d (calls with P <= d return SYMDEL_E_ARG); fewer records, more candidates */
     SYMDEL_OPT_SORT_GROUPING = 10 /* [0] 1: symdel_stage_sort_u64 sorts keys only: ties land in arbitrary order (the mode the pipeline uses) */
 };
 

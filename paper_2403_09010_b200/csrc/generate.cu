@@ -39,7 +39,7 @@ constexpr u64 K_LEN = 0x9fb21c651e98df25ull;
 __device__ __forceinline__ u32 gen_chunk_of(u64 h, u32 n_chunks) { return __umulhi((u32)h * 0x9e3779b1u, n_chunks); }
 
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, DevInfo* info) {
+__global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, int prefix, DevInfo* info) {
     u64 nmax = 0;
     u32 maxlen = 0, err = 0;
     const i64 stride = (i64)gridDim.x * blockDim.x;
@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, D
         if (L < 0 || a < 0) err |= SD_ERR_OFFSETS;
         else if (L > SD_L_MAX) err |= SD_ERR_TOO_LONG;
         else {
-            nmax += c_vcum[L * (SD_D_MAX + 2) + d + 1];
+            nmax += c_vcum[min(L, (i64)prefix) * (SD_D_MAX + 2) + d + 1];
             maxlen = max(maxlen, (u32)L);
         }
     }
@@ -143,6 +143,7 @@ struct GenParams {
     i64 n_a;
     int d, width, thinning, hash_bits, id_bits, npass, hshift;  // hshift: bit of the KEY where the first counted digit starts
     u32 n_chunks, chunk;
+    u32 prefix;  // variants are generated from the first `prefix` residues only (App. B); >= SD_L_MAX: whole sequences
     const u64* rec_off;
     u64* records;
     u32* cnt;
@@ -150,13 +151,13 @@ struct GenParams {
     DevInfo* info;
 };
 
-__global__ void __launch_bounds__(128) k_count_dp(SeqSetDev A, SeqSetDev B, int d, int thinning, u32* __restrict__ cnt) {
+__global__ void __launch_bounds__(128) k_count_dp(SeqSetDev A, SeqSetDev B, int d, int thinning, int prefix, u32* __restrict__ cnt) {
     const i64 g = (i64)blockIdx.x * 128 + threadIdx.x;
     if (g >= A.n + B.n) return;
     const SeqSetDev& S = g < A.n ? A : B;
     const i64 i0 = g < A.n ? g : g - A.n;
     const i64 o = S.off[i0];
-    const int L = (int)(S.off[i0 + 1] - o);
+    const int L = min((int)(S.off[i0 + 1] - o), prefix);
     if (!thinning) {
         cnt[g] = c_vcum[L * (SD_D_MAX + 2) + d + 1];
         return;
@@ -316,7 +317,7 @@ __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
             u32 L = 0;
             if (tid < ng) {
                 const i64 a = S.off[first + tid];
-                L = (u32)(S.off[first + tid + 1] - a);
+                L = min((u32)(S.off[first + tid + 1] - a), P.prefix);
                 sh.off[tid] = a;
             }
             sh.len[tid] = L;
@@ -501,7 +502,7 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
         u32 Li = 0;
         if (lane < ns) {
             o0 = S.off[first + lane];
-            Li = (u32)(S.off[first + lane + 1] - o0);
+            Li = min((u32)(S.off[first + lane + 1] - o0), P.prefix);
         }
         u32 cum_incl = Li;
 #pragma unroll
@@ -510,7 +511,6 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
             if (lane >= (u32)o) cum_incl += t;
         }
         const u32 cum_excl = cum_incl - Li;
-        const i64 obase = __shfl_sync(SD_FULL, o0, 0);
         u64 rec_base_i = 0;
         if (!COUNT_ONLY && lane < ns) rec_base_i = P.rec_off[gid0 + lane];
 
@@ -548,7 +548,8 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
                 const u32 a = lane - seg_start;
                 const u64 gid = gid0 + si;
                 const u32 segmask = active ? (((L == 32u) ? 0xffffffffu : ((1u << L) - 1u)) << seg_start) : 0u;
-                const u32 c = active ? ((u32)(unsigned char)S.seqs[obase + base + lane] & 31u) : 0u;
+                const i64 osrc = __shfl_sync(SD_FULL, o0, si);  // (all lanes take part: never inside the ternary)
+                const u32 c = active ? ((u32)(unsigned char)S.seqs[osrc + a] & 31u) : 0u;
                 const u32 cn = __shfl_down_sync(SD_FULL, c, 1), cnn = __shfl_down_sync(SD_FULL, c, 2);
                 const bool has1 = a + 1 < L, has2 = a + 2 < L;
                 const bool canon1 = active && (!thinning || !has1 || c != cn);
@@ -711,7 +712,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     bool have = false;  // a task is loaded and has batches left
     u32 s = 0, ns = 0, Li = 0, cum_incl = 0, cum_excl = 0;
     u64 gid0 = 0;
-    i64 obase = 0;
+    i64 o0 = 0;  // lane as sequence index: offset of its residues
     const int8_t* seqs = nullptr;
     while (true) {
         if (!have && wt < P.groups_total) {
@@ -721,11 +722,11 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
             ns = (u32)min((i64)32, S.n - first);
             gid0 = (u64)first + (in_b ? (u64)P.n_a : 0ull);
             seqs = S.seqs;
-            i64 o0 = 0;
+            o0 = 0;
             Li = 0;
             if (lane < ns) {
                 o0 = S.off[first + lane];
-                Li = (u32)(S.off[first + lane + 1] - o0);
+                Li = min((u32)(S.off[first + lane + 1] - o0), P.prefix);
             }
             cum_incl = Li;
 #pragma unroll
@@ -734,7 +735,6 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                 if (lane >= (u32)o) cum_incl += t;
             }
             cum_excl = cum_incl - Li;
-            obase = __shfl_sync(SD_FULL, o0, 0);
             s = 0;
             have = true;
             wt += wstride;
@@ -760,7 +760,8 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                 const u32 L = active ? Lsrc : 0u;  // idle lanes: L = 0 switches every later predicate off
                 const u32 a = lane - seg_start;
                 const u64 gid = gid0 + si;
-                const u32 c = active ? ((u32)(unsigned char)seqs[obase + base + lane] & 31u) : 0u;
+                const i64 osrc = __shfl_sync(SD_FULL, o0, si);  // (all lanes take part: never inside the ternary)
+                const u32 c = active ? ((u32)(unsigned char)seqs[osrc + a] & 31u) : 0u;
                 const u32 cn = __shfl_down_sync(SD_FULL, c, 1), cnn = __shfl_down_sync(SD_FULL, c, 2);
                 const bool has1 = a + 1 < L, has2 = a + 2 < L;
                 const bool canon1 = active && (!thinning || !has1 || c != cn);
@@ -884,6 +885,7 @@ GenParams make_params(SeqSetDev a, SeqSetDev b, const Layout& lay, int width) {
     P.id_bits = lay.id_bits;
     P.n_chunks = lay.n_chunks;
     P.chunk = lay.chunk;
+    P.prefix = lay.prefix > 0 ? (u32)lay.prefix : (u32)SD_L_MAX;
     return P;
 }
 
@@ -945,10 +947,10 @@ cudaError_t sd_init_tables() {
     return cudaSuccess;
 }
 
-cudaError_t sd_prepare(SeqSetDev s, int d, int is_b, DevInfo* info, cudaStream_t st, i64* launches) {
+cudaError_t sd_prepare(SeqSetDev s, int d, int is_b, int prefix, DevInfo* info, cudaStream_t st, i64* launches) {
     if (s.n == 0) return cudaSuccess;
     int blocks = (int)std::min<i64>((s.n + 255) / 256, 148 * 8);
-    k_prepare<<<blocks, 256, 0, st>>>(s, d, is_b, info);
+    k_prepare<<<blocks, 256, 0, st>>>(s, d, is_b, prefix > 0 ? prefix : SD_L_MAX, info);
     if (launches) ++*launches;
     return cudaGetLastError();
 }
@@ -962,7 +964,7 @@ cudaError_t sd_count(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u32
     P.info = info;
     if (fast) gen2_pick<true>(lay.n_chunks > 1, 0)<<<gen2_grid(P.groups_total), G2_THREADS, sizeof(Gen2Shared), st>>>(P);
     else if (lay.n_chunks > 1) k_generate<true, true><<<gen_grid(P.groups_total), GEN_THREADS, sizeof(GenShared), st>>>(P);
-    else k_count_dp<<<(unsigned)((a.n + b.n + 127) / 128), 128, 0, st>>>(a, b, lay.d, lay.thinning, cnt);
+    else k_count_dp<<<(unsigned)((a.n + b.n + 127) / 128), 128, 0, st>>>(a, b, lay.d, lay.thinning, (int)P.prefix, cnt);
     if (launches) ++*launches;
     return cudaGetLastError();
 }

@@ -28,6 +28,7 @@ struct Layout {
     int b_bits;        // bits of the second pair component (self: id_bits; cross: bits of n_b)
     int pair_bits;     // a_bits + b_bits
     int thinning;
+    int prefix;         // > 0: variants come from the first `prefix` residues of every sequence (App. B)
     int force_general;  // test hook: never take the d <= 2 fast generation path
     u32 n_chunks, chunk;
 };
@@ -50,7 +51,7 @@ cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u
 
 // ---- generate.cu --------------------------------------------------------------------------------
 cudaError_t sd_init_tables();  // fills the __constant__ tables once per process
-cudaError_t sd_prepare(SeqSetDev s, int d, int is_b, DevInfo* info, cudaStream_t st, i64* launches);
+cudaError_t sd_prepare(SeqSetDev s, int d, int is_b, int prefix, DevInfo* info, cudaStream_t st, i64* launches);
 // count pass: cnt[gid] = number of records sequence gid contributes (u32 per sequence)
 cudaError_t sd_count(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u32* cnt, DevInfo* info, cudaStream_t st,
                      i64* launches);

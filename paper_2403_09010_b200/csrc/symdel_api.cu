@@ -31,7 +31,7 @@ struct symdel_ctx {
     symdel_stats stats{};
     int opt_timing = 0;
     i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0, opt_general_gen = 0;
-    i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0, opt_join_general = 0, opt_exact = 0;
+    i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0, opt_join_general = 0, opt_exact = 0, opt_prefix = 0;
     DevInfo* h_info = nullptr;  // pinned; followed by 256 u32 (the level-1 bin counts of the fused pipeline)
     void* arena = nullptr;      // device arena of the *_host entry points
     size_t arena_bytes = 0;
@@ -196,8 +196,10 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
 
     // ---- S0 ----
     CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
-    CK(sd_prepare(A, d, 0, info, st, &S.n_launches));
-    if (cross) CK(sd_prepare(B, d, 1, info, st, &S.n_launches));
+    const int prefix = (int)ctx->opt_prefix;  // App. B: exact only if the prefix is longer than the threshold
+    if (prefix > 0 && prefix <= d) return SYMDEL_E_ARG;
+    CK(sd_prepare(A, d, 0, prefix, info, st, &S.n_launches));
+    if (cross) CK(sd_prepare(B, d, 1, prefix, info, st, &S.n_launches));
     int rc = read_info(ctx, info, st);
     if (rc) return rc;
     if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
@@ -215,6 +217,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     lay.pair_bits = (cross ? bits_for(A.n) : lay.id_bits) + lay.b_bits;
     lay.thinning = ctx->opt_no_thinning ? 0 : 1;
     lay.force_general = ctx->opt_general_gen ? 1 : 0;
+    lay.prefix = prefix;
     {
         // Hash field: every bit the id leaves free (SYMDEL_OPT_HASH_BITS narrows it: more colliding
         // variants, same result).  S2 radix-partitions only its top sort_bits: enough 8-bit digits for the
@@ -283,7 +286,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     u64* final_lb = ws.take<u64>(scap / 256 + 2);
     if (!ws.ok) return SYMDEL_E_WORKSPACE;
 
-    const int width = maxlen + 1;
+    const int width = (prefix > 0 ? std::min(maxlen, prefix) : maxlen) + 1;  // generation works on the (truncated) sequences
     i64 n_surv = 0, flushes = 0;
     enum { ST_GEN, ST_SORT, ST_EMIT, ST_DEDUP, ST_VERIFY };
     i64 pass_count = 0;
@@ -616,6 +619,10 @@ int symdel_set_option(symdel_ctx* ctx, int option, int64_t value) {
         case SYMDEL_OPT_SORT_GROUPING: ctx->opt_sort_grouping = value != 0; break;
         case SYMDEL_OPT_JOIN_GENERAL: ctx->opt_join_general = value != 0; break;
         case SYMDEL_OPT_EXACT_PIPELINE: ctx->opt_exact = value != 0; break;
+        case SYMDEL_OPT_PREFIX_LEN:
+            if (value > SD_L_MAX) return SYMDEL_E_ARG;
+            ctx->opt_prefix = value;
+            break;
         case SYMDEL_OPT_NO_THINNING: ctx->opt_no_thinning = value != 0; break;
         case SYMDEL_OPT_GENERAL_GENERATE: ctx->opt_general_gen = value != 0; break;
         case SYMDEL_OPT_SORT_VARIANT:
@@ -740,7 +747,7 @@ int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const int64_t* of
     SeqSetDev A{seqs, offsets, n}, B{nullptr, nullptr, 0};
     CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
     CK(cudaMemsetAsync(hist, 0, 8 * 256 * 4, st));
-    CK(sd_prepare(A, d, 0, info, st, nullptr));
+    CK(sd_prepare(A, d, 0, 0, info, st, nullptr));
     int rc = read_info(ctx, info, st);
     if (rc) return rc;
     if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
@@ -781,8 +788,8 @@ int symdel_stage_lev(symdel_ctx* ctx, const int8_t* a_seqs, const int64_t* a_off
     void* slots = ws.take<char>(sd_pack_bytes(n_a + n_b, SD_L_MAX));
     if (!ws.ok) return SYMDEL_E_WORKSPACE;
     CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
-    CK(sd_prepare(A, 0, 0, info, st, nullptr));
-    CK(sd_prepare(B, 0, 1, info, st, nullptr));
+    CK(sd_prepare(A, 0, 0, 0, info, st, nullptr));
+    CK(sd_prepare(B, 0, 1, 0, info, st, nullptr));
     int rc = read_info(ctx, info, st);
     if (rc) return rc;
     if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);

@@ -352,6 +352,42 @@ def test_fused_bin_overflow_falls_back(sd, oracle):
     assert len(exp[0]) == base.n * 100 * 99 // 2
 
 
+@pytest.mark.parametrize("family,d,P,opts", [
+    ("tcr", 1, 2, {}), ("tcr", 2, 3, {}), ("tcr", 2, 8, {}), ("tcr", 2, 12, {"FORCE_CHUNKS": 3}), ("tcr", 2, 18, {"EXACT_PIPELINE": 1}),
+    ("tcr", 2, 10, {"EXACT_PIPELINE": 1}), ("bcr", 3, 12, {}), ("bcr", 3, 4, {}), ("bcr", 2, 18, {}), ("bcr", 1, 40, {}),
+])
+def test_prefix_truncation_is_exact(sd, oracle, family, d, P, opts):
+    """NEXT-1 / App. B: generating the variants of the first P > d residues only, and
+    verifying on the whole sequences, returns exactly the same pairs — with fewer records."""
+    s = synth.tcr_set(6000, 41) if family == "tcr" else synth.bcr_set(4000, 42, n_lineages=400)
+    exp = oracle.symdel_self(s.seqs, s.offsets, d)
+    c = sd.Context(0)
+    assert_same(run_self(sd, c, s, d), exp)
+    full = c.symdel_get_stats()["n_records"]
+    c.symdel_set_option(sd.OPT_PREFIX_LEN, P)
+    for k, v in opts.items():
+        c.symdel_set_option(getattr(sd, "OPT_" + k), v)
+    assert_same(run_self(sd, c, s, d), exp)
+    if P < int(s.lengths.min()):
+        assert c.symdel_get_stats()["n_records"] < full
+
+
+def test_prefix_not_longer_than_threshold_is_rejected(sd, ctx):
+    s = synth.tcr_set(100, 43)
+    ctx.symdel_set_option(sd.OPT_PREFIX_LEN, 2)
+    with pytest.raises(sd.SymdelError) as e:
+        run_self(sd, ctx, s, 2)
+    assert e.value.code == sd.E_ARG
+
+
+def test_prefix_truncation_cross(sd, oracle):
+    q, r = synth.cross_sets(400, 6000, 44)
+    exp = oracle.symdel_cross(q.seqs, q.offsets, r.seqs, r.offsets, 2)
+    c = sd.Context(0)
+    c.symdel_set_option(sd.OPT_PREFIX_LEN, 9)
+    assert_same(run_cross(sd, c, q, r, 2), exp)
+
+
 def test_small_workspace_forces_chunking(torch, sd, ctx, oracle):
     s = synth.tcr_set(20000, 22)
     exp = oracle.symdel_self(s.seqs, s.offsets, 2)

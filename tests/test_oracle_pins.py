@@ -173,6 +173,32 @@ def test_p4_cat_coat(oracle):
     assert ca in oracle.deletion_variants(enc("CAT"), 1) and ca in oracle.deletion_variants(enc("COA"), 1)
 
 
+@pytest.mark.parametrize("d,P", [(1, 2), (1, 5), (2, 3), (2, 8), (3, 4), (3, 12)])
+def test_p4_prefix_lemma_random_pairs(oracle, d, P):
+    """App. B: if lev(u, v) <= d and P > d, the prefixes u[:P], v[:P] share a deletion variant
+    within depth d.  Random pairs built by <= d edits; the variants come from the oracle's plain enumeration."""
+    rng = np.random.default_rng(1000 * d + P)
+    n_checked = 0
+    for _ in range(300):
+        L = int(rng.integers(1, 16))
+        u = rng.integers(1, 5, L).astype(np.int8)  # small alphabet: many repeats
+        v = list(u)
+        for _e in range(int(rng.integers(0, d + 1))):
+            op = int(rng.integers(0, 3))
+            if op == 0 and v:
+                v[int(rng.integers(0, len(v)))] = int(rng.integers(1, 5))
+            elif op == 1:
+                v.insert(int(rng.integers(0, len(v) + 1)), int(rng.integers(1, 5)))
+            elif v:
+                del v[int(rng.integers(0, len(v)))]
+        v = np.asarray(v, dtype=np.int8)
+        if oracle.lev(u, v) > d:
+            continue
+        n_checked += 1
+        assert set(oracle.deletion_variants(u[:P], d)) & set(oracle.deletion_variants(v[:P], d)), (u, v)
+    assert n_checked > 200
+
+
 # ---- P-3 m(m-1)/2 candidates per group (PAPER.md:96) -------------------------------------------
 @pytest.mark.parametrize("m", [2, 3, 7, 12])
 def test_p3_pairs_per_group(oracle, m):
