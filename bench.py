@@ -157,6 +157,9 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); the metric is quoted on 3")
     ap.add_argument("--ref-sample", type=int, default=150000, help="sequences in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dense", action="store_true",
+                    help="NEXT-2 workload instead of config 3: synth.dense_set(1,000,000, seed 11, fanout 64), d=2 "
+                         "(real-repertoire-like density: candidates ~ records; not the BASELINE.json headline)")
     ap.add_argument("--prefix", type=int, default=0,
                     help="prefix-truncated candidate generation (App. B; same output, fewer records); default off: the "
                          "headline generates every deletion variant of every sequence")
@@ -180,7 +183,10 @@ def main():
 
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    kind, d, sets = synth.config(args.config)
+    if args.dense:
+        kind, d, sets = "self", 2, (synth.dense_set(1_000_000, 11, fanout=64),)
+    else:
+        kind, d, sets = synth.config(args.config)
     assert kind == "self"
     s = sets[0]
     ctx = symdel.Context(local)
@@ -190,7 +196,7 @@ def main():
     dev = torch.device("cuda", local)
     seqs_d = torch.from_numpy(s.seqs).to(dev)
     offs_d = torch.from_numpy(s.offsets).to(dev)
-    cap = 4 << 20
+    cap = (32 << 20) if args.dense else (4 << 20)
     ws_bytes = symdel.symdel_workspace_bytes(s.n, s.seqs.size, 0, 0, int(s.lengths.max()), d, cap)
     ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
     out = tuple(torch.empty(cap, dtype=torch.int32, device=dev) for _ in range(3))
@@ -288,7 +294,8 @@ def main():
         "metric": METRIC, "value": job_value(n_out, world, ms), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u64", "data": "synthetic",
-        "config": {"workload": WORKLOAD if args.config == 3 else f"config {args.config}", "n": s.n, "d": d,
+        "config": {"workload": ("NEXT-2 dense: synth.dense_set(1e6, seed 11, fanout 64), d=2" if args.dense else
+                                WORKLOAD if args.config == 3 else f"config {args.config}"), "n": s.n, "d": d,
                    "pairs_per_step": n_out, "records": n_rec, "candidates": n_cand,
                    "unique_candidates": st["n_unique"], "hash_bits": st["hash_bits"], "id_bits": st["id_bits"],
                    "partition_bits": st["sort_bits"], "pipeline": "fused" if fused else "exact",
@@ -311,7 +318,7 @@ def main():
                      "frac_of_nominal_8000": achieved / 8000.0},
         "clocks": clocks,
     }
-    if not args.no_cpu_baseline and world == 1:
+    if not args.no_cpu_baseline and world == 1 and not args.dense:
         n_sample = min(s.n, args.ref_sample)
         pairs, dt = cpu_baseline_run(n_sample, d, s)
         line["cpu_baseline"] = {"value": pairs / dt, "unit": UNIT, "cores": 1, "kind": "oracle",

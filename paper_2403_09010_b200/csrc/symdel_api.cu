@@ -249,7 +249,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     const i64 R = ws.left() - 8192;
     // a window of the candidate buffer ends with a whole record's pairs: at most one per other sequence
     const i64 cslack = n_total + 64;
-    i64 ccap = ctx->opt_cand_cap > 0 ? ctx->opt_cand_cap : std::max<i64>(1 << 20, nmax / 2);
+    i64 ccap = ctx->opt_cand_cap > 0 ? ctx->opt_cand_cap : std::max<i64>(1 << 20, 2 * nmax);
     i64 scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity + (ctx->opt_cand_cap > 0 ? ccap : 0));
     i64 ncap = std::max<i64>(nmax, 1);
     u32 P = ctx->opt_force_chunks > 0 ? (u32)ctx->opt_force_chunks : 1;
@@ -530,7 +530,7 @@ int run_host(symdel_ctx* ctx, const int8_t* a_seqs, const i64* a_off, i64 n_a, c
     }
     const i64 n_total = n_a + n_b;
     const int npass_max = 7, ppass_max = 8;
-    const i64 ccap = std::max<i64>(1 << 20, nmax / 2), scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity);
+    const i64 ccap = std::max<i64>(1 << 20, 2 * nmax), scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity);
     const i64 ws_bytes = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nmax, 1), npass_max) + cand_bytes(ccap + n_total + 64, ppass_max) +
                          cand_bytes(scap, ppass_max) + 65536;
     const i64 in_bytes = align_up(res_a + 16) + align_up((n_a + 1) * 8) + align_up(res_b + 16) + align_up((n_b + 1) * 8);
@@ -666,7 +666,7 @@ int symdel_workspace_bytes(int64_t n_a, int64_t residues_a, int64_t n_b, int64_t
     const i64 n_total = n_a + n_b;
     const u64 vm = vcount_host(max_len, d);
     const i64 nbound = n_total + (max_len ? (i64)(((u64)(residues_a + residues_b) * (vm - 1) + max_len - 1) / max_len) : 0);
-    const i64 ccap = std::max<i64>(1 << 20, nbound / 2), scap = std::max<i64>(std::max<i64>(1 << 20, nbound / 4), capacity);
+    const i64 ccap = std::max<i64>(1 << 20, 2 * nbound), scap = std::max<i64>(std::max<i64>(1 << 20, nbound / 4), capacity);
     *bytes_host = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nbound, 1), 7) + cand_bytes(ccap + n_total + 64, 8) + cand_bytes(scap, 8) +
                   65536;
     return SYMDEL_OK;

@@ -222,6 +222,15 @@ def bcr_set(n_total: int, seed, n_lineages: int | None = None, lo=8, hi=30, mean
     return from_padded(rows, lens)
 
 
+def dense_set(n_total: int, seed, fanout: int = 64, kmax: int = 2) -> SeqSet:
+    """NEXT-2: a dense-neighbourhood repertoire, the regime the paper reports for real
+    data (137 M matched pairs from 120 M variants at 1 M sequences).  n_total / fanout TCR-shaped
+    seeds, each with a Geometric(1 / fanout) number of descendants = the seed + k ~ U{1..kmax} edits, emitted
+    contiguously, cut to n_total, deduplicated: whole clusters lie within distance 2 * kmax of one another."""
+    return bcr_set(n_total, seed, n_lineages=max(1, n_total // fanout), lo=8, hi=24, mean=15.0, sd=2.0, kmax=kmax,
+                   p_geom=1.0 / fanout)
+
+
 def cross_sets(n_query: int, n_ref: int, seed: int, p_derived=0.2, lo=8, hi=24, mean=15.0, sd=2.0, kmax=3):
     """G-6 (config 4): reference = TCR set (seed); queries: with prob. 0.2 a uniformly chosen
     reference sequence + k ~ U{1,2,3} edits, else an independent seed; query RNG =

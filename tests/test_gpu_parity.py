@@ -388,6 +388,21 @@ def test_prefix_truncation_cross(sd, oracle):
     assert_same(run_cross(sd, c, q, r, 2), exp)
 
 
+@pytest.mark.parametrize("d,fanout,opts", [(1, 64, {}), (2, 64, {}), (2, 16, {"EXACT_PIPELINE": 1}), (2, 200, {}),
+                                           (2, 64, {"CAND_CAPACITY": 200000})])
+def test_dense_neighbourhoods(sd, oracle, d, fanout, opts):
+    """NEXT-2: clusters of near-identical sequences (candidates ~ records, long runs of one variant, most records
+    with partners: PAPER.md:96, 287-294).  Same bit-exact bar against the oracle's hash-map SymDel."""
+    s = synth.dense_set(12000, 51, fanout=fanout)
+    exp = oracle.symdel_self(s.seqs, s.offsets, d)
+    c = sd.Context(0)
+    for k, v in opts.items():
+        c.symdel_set_option(getattr(sd, "OPT_" + k), v)
+    assert_same(run_self(sd, c, s, d, capacity=len(exp[0]) + 16), exp)
+    st = c.symdel_get_stats()
+    assert st["n_candidates"] > st["n_records"] // 20
+
+
 def test_small_workspace_forces_chunking(torch, sd, ctx, oracle):
     s = synth.tcr_set(20000, 22)
     exp = oracle.symdel_self(s.seqs, s.offsets, 2)

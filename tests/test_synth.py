@@ -47,3 +47,11 @@ def test_take_roundtrip():
     t = s.take(p)
     for k in (0, 17, s.n - 1):
         assert np.array_equal(t.seq(k), s.seq(p[k]))
+
+
+def test_dense_set_shape():
+    s = synth.dense_set(5000, 3, fanout=50)
+    assert 4000 < s.n <= 5000 and s.lengths.min() >= 8 and s.lengths.max() <= 24
+    assert s.seqs.min() >= 1 and s.seqs.max() <= 20
+    s2 = synth.dense_set(5000, 3, fanout=50)
+    assert np.array_equal(s.seqs, s2.seqs) and np.array_equal(s.offsets, s2.offsets)
