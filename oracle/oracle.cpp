@@ -182,6 +182,43 @@ void* oracle_bruteforce_cross(const int8_t* qs, const int64_t* qo, int64_t nq, c
     return res;
 }
 
+// ---- Hamming mode (NEXT-3, Fig. S3 A/C) ---------------------------------
+// The paper benchmarks "Hamming distance, d = 1, 2" without restating the definition; reading A-17:
+// the Hamming distance is defined for sequences of EQUAL length as the number of positions at which
+// they differ; pairs of unequal length are never neighbours.  Plain double loop, same output order.
+static int hamming_plain(const int8_t* a, const int8_t* b, int L) {
+    int h = 0;
+    for (int t = 0; t < L; ++t) h += a[t] != b[t] ? 1 : 0;
+    return h;
+}
+
+void* oracle_bruteforce_hamming_self(const int8_t* seqs, const int64_t* off, int64_t n, int d) {
+    auto* res = new Result();
+    for (int64_t i = 0; i < n; ++i) {
+        int li = seq_len(off, i);
+        for (int64_t j = i + 1; j < n; ++j) {
+            if (seq_len(off, j) != li) continue;
+            int dist = hamming_plain(seqs + off[i], seqs + off[j], li);
+            if (dist <= d) res->out.push_back({(int32_t)i, (int32_t)j, dist});
+        }
+    }
+    return res;
+}
+
+void* oracle_bruteforce_hamming_cross(const int8_t* qs, const int64_t* qo, int64_t nq, const int8_t* rs, const int64_t* ro,
+                                      int64_t nr, int d) {
+    auto* res = new Result();
+    for (int64_t q = 0; q < nq; ++q) {
+        int lq = seq_len(qo, q);
+        for (int64_t r = 0; r < nr; ++r) {
+            if (seq_len(ro, r) != lq) continue;
+            int dist = hamming_plain(qs + qo[q], rs + ro[r], lq);
+            if (dist <= d) res->out.push_back({(int32_t)q, (int32_t)r, dist});
+        }
+    }
+    return res;
+}
+
 // Neighbours of ONE probe sequence among a set (used to sample rows at full config sizes).
 void* oracle_bruteforce_row(const int8_t* p, int lp, const int8_t* rs, const int64_t* ro, int64_t nr, int d) {
     auto* res = new Result();

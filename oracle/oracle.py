@@ -40,6 +40,10 @@ def lib():
         L.oracle_bruteforce_self.argtypes = [p8, p64, C.c_int64, C.c_int, C.c_int]
         L.oracle_bruteforce_cross.restype = vp
         L.oracle_bruteforce_cross.argtypes = [p8, p64, C.c_int64, p8, p64, C.c_int64, C.c_int, C.c_int]
+        L.oracle_bruteforce_hamming_self.restype = vp
+        L.oracle_bruteforce_hamming_self.argtypes = [p8, p64, C.c_int64, C.c_int]
+        L.oracle_bruteforce_hamming_cross.restype = vp
+        L.oracle_bruteforce_hamming_cross.argtypes = [p8, p64, C.c_int64, p8, p64, C.c_int64, C.c_int]
         L.oracle_bruteforce_row.restype = vp
         L.oracle_bruteforce_row.argtypes = [p8, C.c_int, p8, p64, C.c_int64, C.c_int]
         L.oracle_symdel_self.restype = vp
@@ -122,6 +126,18 @@ def bruteforce_cross(qs, qo, rs, ro, d: int, threads: int = 0):
     rs, ro = _csr(rs, ro)
     return _take(lib().oracle_bruteforce_cross(_p8(qs), _p64(qo), qo.size - 1, _p8(rs), _p64(ro), ro.size - 1, int(d),
                                                int(threads)))
+
+
+def hamming_self(seqs, offsets, d: int):
+    """NEXT-3: every (i, j, hamming) with i < j, equal lengths and <= d mismatches (plain double loop)."""
+    seqs, offsets = _csr(seqs, offsets)
+    return _take(lib().oracle_bruteforce_hamming_self(_p8(seqs), _p64(offsets), offsets.size - 1, int(d)))
+
+
+def hamming_cross(qs, qo, rs, ro, d: int):
+    qs, qo = _csr(qs, qo)
+    rs, ro = _csr(rs, ro)
+    return _take(lib().oracle_bruteforce_hamming_cross(_p8(qs), _p64(qo), qo.size - 1, _p8(rs), _p64(ro), ro.size - 1, int(d)))
 
 
 def bruteforce_row(probe, rs, ro, d: int):

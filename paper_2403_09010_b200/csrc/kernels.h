@@ -29,6 +29,7 @@ struct Layout {
     int pair_bits;     // a_bits + b_bits
     int thinning;
     int prefix;         // > 0: variants come from the first `prefix` residues of every sequence (App. B)
+    int metric;         // 0: Levenshtein; 1: Hamming (equal lengths only, mismatch count)
     int force_general;  // test hook: never take the d <= 2 fast generation path
     u32 n_chunks, chunk;
 };

@@ -31,7 +31,7 @@ struct symdel_ctx {
     symdel_stats stats{};
     int opt_timing = 0;
     i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0, opt_general_gen = 0;
-    i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0, opt_join_general = 0, opt_exact = 0, opt_prefix = 0;
+    i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0, opt_join_general = 0, opt_exact = 0, opt_prefix = 0, opt_metric = 0;
     DevInfo* h_info = nullptr;  // pinned; followed by 256 u32 (the level-1 bin counts of the fused pipeline)
     void* arena = nullptr;      // device arena of the *_host entry points
     size_t arena_bytes = 0;
@@ -218,6 +218,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     lay.thinning = ctx->opt_no_thinning ? 0 : 1;
     lay.force_general = ctx->opt_general_gen ? 1 : 0;
     lay.prefix = prefix;
+    lay.metric = (int)ctx->opt_metric;
     {
         // Hash field: every bit the id leaves free (SYMDEL_OPT_HASH_BITS narrows it: more colliding
         // variants, same result).  S2 radix-partitions only its top sort_bits: enough 8-bit digits for the
@@ -619,6 +620,10 @@ int symdel_set_option(symdel_ctx* ctx, int option, int64_t value) {
         case SYMDEL_OPT_SORT_GROUPING: ctx->opt_sort_grouping = value != 0; break;
         case SYMDEL_OPT_JOIN_GENERAL: ctx->opt_join_general = value != 0; break;
         case SYMDEL_OPT_EXACT_PIPELINE: ctx->opt_exact = value != 0; break;
+        case SYMDEL_OPT_METRIC:
+            if (value > 1) return SYMDEL_E_ARG;
+            ctx->opt_metric = value;
+            break;
         case SYMDEL_OPT_PREFIX_LEN:
             if (value > SD_L_MAX) return SYMDEL_E_ARG;
             ctx->opt_prefix = value;

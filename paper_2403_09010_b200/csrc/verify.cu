@@ -108,6 +108,17 @@ __device__ __forceinline__ int myers_lev(const Planes<W>& P, const Planes<W>& T)
     return score;
 }
 
+// Hamming mode (NEXT-3, Fig. S3): defined for equal lengths only; a position differs iff any of
+// the five code bit-planes differs.  Returns > any threshold for unequal lengths.
+template <typename W>
+__device__ __forceinline__ int hamming_planes(const Planes<W>& P, const Planes<W>& T) {
+    if (P.len != T.len) return 1 << 20;
+    W x = 0;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) x |= P.b[k] ^ T.b[k];
+    return sizeof(W) == 8 ? __popcll((unsigned long long)x) : __popc((unsigned)x);
+}
+
 constexpr int VF_THREADS = 256, VF_IPT = 4, VF_TILE = VF_THREADS * VF_IPT;
 
 // Tile of 1024 sorted candidates: (1) flag the unique ones and compact their positions into shared
@@ -163,7 +174,7 @@ __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ c
         const Planes<W> pb = load_planes<W>(slots, lay.cross ? (u64)lay.n_a + b : b);
         const int dl = pa.len > pb.len ? pa.len - pb.len : pb.len - pa.len;
         if (dl <= lay.d) {
-            const int dist = myers_lev<W>(pa, pb);
+            const int dist = lay.metric ? hamming_planes<W>(pa, pb) : myers_lev<W>(pa, pb);
             if (dist <= lay.d) s_res[pos] = (unsigned char)dist;
         }
     }

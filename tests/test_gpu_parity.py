@@ -403,6 +403,31 @@ def test_dense_neighbourhoods(sd, oracle, d, fanout, opts):
     assert st["n_candidates"] > st["n_records"] // 20
 
 
+@pytest.mark.parametrize("family,d,opts", [("tcr", 1, {}), ("tcr", 2, {}), ("tcr", 2, {"EXACT_PIPELINE": 1, "FORCE_CHUNKS": 2}),
+                                           ("bcr", 3, {}), ("dense", 2, {}), ("tcr", 2, {"PREFIX_LEN": 9})])
+def test_hamming_mode(sd, oracle, family, d, opts):
+    """NEXT-3 (Fig. S3 A/C): equal-length pairs with <= d mismatches, against the oracle's plain
+    double loop."""
+    s = {"tcr": lambda: synth.tcr_set(5000, 71), "bcr": lambda: synth.bcr_set(4000, 72, n_lineages=400),
+         "dense": lambda: synth.dense_set(5000, 73)}[family]()
+    c = sd.Context(0)
+    c.symdel_set_option(sd.OPT_METRIC, sd.METRIC_HAMMING)
+    for k, v in opts.items():
+        c.symdel_set_option(getattr(sd, "OPT_" + k), v)
+    exp = oracle.hamming_self(s.seqs, s.offsets, d)
+    assert len(exp[0]) > 100
+    assert_same(run_self(sd, c, s, d), exp)
+
+
+def test_hamming_mode_cross_and_long(sd, oracle):
+    q, r = synth.cross_sets(500, 5000, 74)
+    c = sd.Context(0)
+    c.symdel_set_option(sd.OPT_METRIC, sd.METRIC_HAMMING)
+    assert_same(run_cross(sd, c, q, r, 2), oracle.hamming_cross(q.seqs, q.offsets, r.seqs, r.offsets, 2))
+    s = synth.bcr_set(1500, 75, n_lineages=100, lo=30, hi=60, mean=45.0, sd=6.0)  # 64-bit plane words
+    assert_same(run_self(sd, c, s, 2), oracle.hamming_self(s.seqs, s.offsets, 2))
+
+
 def test_small_workspace_forces_chunking(torch, sd, ctx, oracle):
     s = synth.tcr_set(20000, 22)
     exp = oracle.symdel_self(s.seqs, s.offsets, 2)

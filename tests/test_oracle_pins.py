@@ -373,3 +373,46 @@ def test_p10_equal_length_substitutions_hamming(oracle):
     ham = (rows[:, None, :] != rows[None, :, :]).sum(-1)
     exp = {(a, b, int(ham[a, b])) for a in range(n) for b in range(a + 1, n) if ham[a, b] <= 2}
     assert as_set((i, j, d)) == exp
+
+
+# ---- NEXT-3 Hamming mode (Fig. S3 A/C; reading A-17) -----------------------------------
+def test_hamming_hand_cases(oracle):
+    s = S("CASSL", "CASSL", "CATSL", "CTTSL", "CASS", "ACASS", "LSSAC")
+    i, j, d = oracle.hamming_self(s.seqs, s.offsets, 2)
+    got = {(int(a), int(b)): int(c) for a, b, c in zip(i, j, d)}
+    # equal lengths only: CASS (4) pairs with nothing; ACASS vs CASSL: a shift, 4 mismatches (lev 2) -> not a pair
+    assert got == {(0, 1): 0, (0, 2): 1, (1, 2): 1, (0, 3): 2, (1, 3): 2, (2, 3): 1}
+    i1, j1, d1 = oracle.hamming_self(s.seqs, s.offsets, 1)
+    assert {(int(a), int(b)) for a, b in zip(i1, j1)} == {(0, 1), (0, 2), (1, 2), (2, 3)}
+
+
+def test_hamming_equals_numpy_all_pairs(oracle):
+    """Re-derivation with numpy on padded rows: mismatch counts of equal-length rows."""
+    s = synth.tcr_set(1200, 61)
+    rows, lens = synth.to_padded(s)
+    exp = []
+    for a in range(s.n):
+        same = np.nonzero(lens[a + 1:] == lens[a])[0] + a + 1
+        h = (rows[same] != rows[a]).sum(axis=1)
+        exp += [(a, int(b), int(x)) for b, x in zip(same, h) if x <= 2]
+    i, j, d = oracle.hamming_self(s.seqs, s.offsets, 2)
+    assert list(zip(i.tolist(), j.tolist(), d.tolist())) == exp
+    assert len(exp) > 50
+
+
+def test_hamming_vs_levenshtein_relations(oracle):
+    """On equal lengths lev <= hamming; so the Hamming neighbours are a subset of the Levenshtein ones, every
+    Levenshtein pair of equal length at distance <= 1 is a Hamming pair at the same distance, and cross agrees
+    with self."""
+    s = synth.tcr_set(1500, 62)
+    hi, hj, hd = oracle.hamming_self(s.seqs, s.offsets, 2)
+    li, lj, ld = oracle.bruteforce_self(s.seqs, s.offsets, 2)
+    lev = {(int(a), int(b)): int(c) for a, b, c in zip(li, lj, ld)}
+    ham = {(int(a), int(b)): int(c) for a, b, c in zip(hi, hj, hd)}
+    assert set(ham) <= set(lev) and all(lev[k] <= v for k, v in ham.items())
+    L = s.lengths
+    for (a, b), v in lev.items():
+        if v <= 1 and L[a] == L[b]:
+            assert ham[(a, b)] == v
+    ci, cj, cd = oracle.hamming_cross(s.seqs, s.offsets, s.seqs, s.offsets, 2)
+    assert {(int(a), int(b)): int(c) for a, b, c in zip(ci, cj, cd) if a < b} == ham
