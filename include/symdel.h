@@ -138,6 +138,18 @@ SYMDEL_API int symdel_cross_host(symdel_ctx* ctx, const int8_t* q_seqs_host, con
                       int32_t* out_i_host, int32_t* out_j_host, int32_t* out_dist_host, int64_t capacity,
                       int64_t* n_pairs_host);
 
+/* NEXT-4: "aggregates an M x M overlap matrix from identified neighbor pairs, where each entry
+ * contains the number of neighbors between two repertoires".  out_i/out_j: the n_pairs result pairs of a
+ * symdel_self / symdel_cross call (device); labels_i[x] / labels_j[y] in [0, n_repertoires): the repertoire of
+ * the sequence behind first / second pair component (device; the same array for a self-search);
+ * matrix: device int64[M * M], row-major, OVERWRITTEN: matrix[p][q] = #pairs with labels (p, q).  symmetric = 1
+ * (self-search, reading A-18): a pair with labels p != q also counts in [q][p]; within-repertoire pairs count once
+ * on the diagonal.  workspace: >= 256 device bytes.  Synchronises the stream.  SYMDEL_E_ARG if a label is out of
+ * range (the matrix is then unspecified) or n_repertoires is outside 1..4096. */
+SYMDEL_API int symdel_overlap_matrix(symdel_ctx* ctx, const int32_t* out_i, const int32_t* out_j, int64_t n_pairs,
+                          const int32_t* labels_i, const int32_t* labels_j, int n_repertoires, int symmetric,
+                          int64_t* matrix, void* workspace, int64_t workspace_bytes, void* cuda_stream);
+
 /* ---- stage-level entry points (kernel parity tests and micro-benchmarks) ---------------------
  * S2/K2: stable LSD radix sort of n 64-bit keys on bits [begin_bit, end_bit) (end - begin a
  *   multiple of 8).  keys and tmp: device arrays of n; the sorted result is left in `keys`.

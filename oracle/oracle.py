@@ -161,5 +161,18 @@ def symdel_cross(qs, qo, rs, ro, d: int, with_counters=False):
                  with_counters)
 
 
+def overlap_matrix(i, j, labels_i, labels_j, n_repertoires: int, symmetric: bool):
+    """NEXT-4: M x M matrix, entry (p, q) = number of neighbour pairs between repertoires p and q.
+    Plain loop over the pairs.  symmetric (self-search, reading A-18): a pair with labels p != q counts in
+    [p][q] and [q][p]; a within-repertoire pair counts once on the diagonal."""
+    m = np.zeros((n_repertoires, n_repertoires), dtype=np.int64)
+    for a, b in zip(np.asarray(i).tolist(), np.asarray(j).tolist()):
+        p, q = int(labels_i[a]), int(labels_j[b])
+        m[p, q] += 1
+        if symmetric and p != q:
+            m[q, p] += 1
+    return m
+
+
 def max_threads() -> int:
     return int(lib().oracle_max_threads())

@@ -112,3 +112,6 @@ cudaError_t sd_finalize(const u64* surv, i64 n_surv, const Layout& lay, int dedu
 // plain distances for index pairs (stage test); slots = sd_pack of (A, B)
 cudaError_t sd_lev_pairs(const void* slots, i64 n_a, int maxlen, const i32* ia, const i32* ib, i64 n_pairs, i32* dist,
                          cudaStream_t st);
+// NEXT-4: M x M overlap matrix of the output pairs under per-sequence repertoire labels
+cudaError_t sd_overlap(const i32* pi, const i32* pj, i64 n, const i32* lab_i, const i32* lab_j, int M, int symmetric,
+                       u64* matrix, u32* err, cudaStream_t st);

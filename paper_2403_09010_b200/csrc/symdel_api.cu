@@ -707,6 +707,22 @@ int symdel_cross_host(symdel_ctx* ctx, const int8_t* q_seqs_host, const int64_t*
                     out_dist_host, capacity, n_pairs_host);
 }
 
+int symdel_overlap_matrix(symdel_ctx* ctx, const int32_t* out_i, const int32_t* out_j, int64_t n_pairs, const int32_t* labels_i,
+                          const int32_t* labels_j, int n_repertoires, int symmetric, int64_t* matrix, void* workspace,
+                          int64_t workspace_bytes, void* cuda_stream) {
+    if (!ctx || n_pairs < 0 || n_repertoires < 1 || n_repertoires > 4096 || !matrix || !labels_i || !labels_j || !workspace ||
+        workspace_bytes < 256 || (n_pairs > 0 && (!out_i || !out_j)))
+        return SYMDEL_E_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CK(cudaSetDevice(ctx->device));
+    u32* err = (u32*)workspace;
+    CK(cudaMemsetAsync(err, 0, sizeof(u32), st));
+    CK(sd_overlap(out_i, out_j, n_pairs, labels_i, labels_j, n_repertoires, symmetric ? 1 : 0, (u64*)matrix, err, st));
+    CK(cudaMemcpyAsync(&ctx->h_info->err, err, sizeof(u32), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return ctx->h_info->err ? SYMDEL_E_ARG : SYMDEL_OK;
+}
+
 // ---- stage-level entry points ------------------------------------------------------------------
 int64_t symdel_stage_sort_workspace_bytes(int64_t n) { return align_up(sd_sort_scratch_bytes(std::max<i64>(n, 1), 8)) + 256; }
 

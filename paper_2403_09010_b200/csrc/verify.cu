@@ -262,7 +262,56 @@ __global__ void __launch_bounds__(256) k_lev_pairs(const void* __restrict__ slot
     dist[t] = myers_lev<W>(load_planes<W>(slots, (u64)ia[t]), load_planes<W>(slots, (u64)(n_a + ib[t])));
 }
 
+// ---- NEXT-4: M x M repertoire-overlap matrix --------------------------------------------
+// "a wrapper that aggregates an M x M overlap matrix from identified neighbor pairs, where each entry
+// contains the number of neighbors between two repertoires".  One pass over the output pairs: block-private
+// shared-memory histogram (M <= 64), flushed with one 64-bit global atomic per non-zero cell.
+constexpr int OV_THREADS = 256, OV_MMAX_SMEM = 64;
+
+__global__ void __launch_bounds__(OV_THREADS) k_overlap(const i32* __restrict__ pi, const i32* __restrict__ pj, u64 n,
+                                                       const i32* __restrict__ lab_i, const i32* __restrict__ lab_j, int M,
+                                                       int symmetric, unsigned long long* __restrict__ matrix, u32* err) {
+    extern __shared__ u32 s_cell[];
+    const bool use_smem = M <= OV_MMAX_SMEM;
+    if (use_smem) {
+        for (int c = threadIdx.x; c < M * M; c += OV_THREADS) s_cell[c] = 0;
+        __syncthreads();
+    }
+    const u64 stride = (u64)gridDim.x * OV_THREADS;
+    for (u64 t = (u64)blockIdx.x * OV_THREADS + threadIdx.x; t < n; t += stride) {
+        const i32 a = lab_i[pi[t]], b = lab_j[pj[t]];
+        if (a < 0 || a >= M || b < 0 || b >= M) {
+            atomicOr(err, (u32)SD_ERR_INTERNAL);
+            continue;
+        }
+        if (use_smem) {
+            atomicAdd(&s_cell[a * M + b], 1u);
+            if (symmetric && a != b) atomicAdd(&s_cell[b * M + a], 1u);
+        } else {
+            atomicAdd(&matrix[(u64)a * M + b], 1ull);
+            if (symmetric && a != b) atomicAdd(&matrix[(u64)b * M + a], 1ull);
+        }
+    }
+    if (use_smem) {
+        __syncthreads();
+        for (int c = threadIdx.x; c < M * M; c += OV_THREADS)
+            if (s_cell[c]) atomicAdd(&matrix[c], (unsigned long long)s_cell[c]);
+    }
+}
+
 }  // namespace
+
+// matrix (M x M, row-major, zeroed here) += the label pairs of the n output pairs; *err gets SD_ERR_INTERNAL if
+// a label lies outside [0, M)
+cudaError_t sd_overlap(const i32* pi, const i32* pj, i64 n, const i32* lab_i, const i32* lab_j, int M, int symmetric,
+                       u64* matrix, u32* err, cudaStream_t st) {
+    cudaError_t e = cudaMemsetAsync(matrix, 0, (size_t)M * M * 8, st);
+    if (e != cudaSuccess || n == 0) return e;
+    const unsigned blocks = (unsigned)std::min<i64>((n + OV_THREADS * 8 - 1) / (OV_THREADS * 8), 148 * 8);
+    const size_t smem = M <= OV_MMAX_SMEM ? (size_t)M * M * 4 : 0;
+    k_overlap<<<blocks, OV_THREADS, smem, st>>>(pi, pj, (u64)n, lab_i, lab_j, M, symmetric, (unsigned long long*)matrix, err);
+    return cudaGetLastError();
+}
 
 i64 sd_verify_tiles(i64 n) { return (n + VF_TILE - 1) / VF_TILE; }
 

@@ -26,7 +26,7 @@ EXPORTS = [
     "symdel_create", "symdel_destroy", "symdel_set_option", "symdel_get_stats", "symdel_last_cuda_error",
     "symdel_strerror", "symdel_workspace_bytes", "symdel_self", "symdel_cross", "symdel_self_host",
     "symdel_cross_host", "symdel_stage_sort_workspace_bytes", "symdel_stage_sort_u64", "symdel_stage_generate",
-    "symdel_stage_lev",
+    "symdel_stage_lev", "symdel_overlap_matrix",
 ]
 
 
@@ -78,6 +78,7 @@ def lib():
         L.symdel_stage_sort_u64.argtypes = [vp, vp, vp, i64, i32, i32, vp, i64, vp]
         L.symdel_stage_generate.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, i64, C.POINTER(i64), vp, i64, vp]
         L.symdel_stage_lev.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp]
+        L.symdel_overlap_matrix.argtypes = [vp, vp, vp, i64, vp, vp, i32, i32, vp, vp, i64, vp]
         _lib = L
     return _lib
 
@@ -237,6 +238,18 @@ class Context:
         if rc:
             self._raise(rc, "symdel_stage_lev")
         return dist
+
+    def symdel_overlap_matrix(self, out_i, out_j, labels_i, labels_j, n_repertoires: int, symmetric: bool):
+        """M x M overlap matrix (int64 CUDA tensor) of result pairs under per-sequence repertoire labels (int32)."""
+        torch = _torch()
+        m = torch.empty((n_repertoires, n_repertoires), dtype=torch.int64, device=labels_i.device)
+        ws = torch.empty(256, dtype=torch.uint8, device=labels_i.device)
+        q = lambda t: C.c_void_p(t.data_ptr())
+        rc = lib().symdel_overlap_matrix(self._h, q(out_i), q(out_j), out_i.numel(), q(labels_i), q(labels_j), n_repertoires,
+                                         1 if symmetric else 0, q(m), q(ws), 256, _stream_ptr(torch))
+        if rc:
+            self._raise(rc, "symdel_overlap_matrix")
+        return m
 
 
 def _hp(a):

@@ -428,6 +428,28 @@ def test_hamming_mode_cross_and_long(sd, oracle):
     assert_same(run_self(sd, c, s, 2), oracle.hamming_self(s.seqs, s.offsets, 2))
 
 
+@pytest.mark.parametrize("M", [1, 2, 7, 64, 100])
+def test_overlap_matrix(torch, sd, ctx, oracle, M):
+    """NEXT-4: M x M repertoire-overlap matrix of the neighbour pairs, self and cross form."""
+    s = synth.tcr_set(6000, 91)
+    ds, do = sd.to_device(s)
+    i, j, _ = ctx.symdel_self(ds, do, 2)
+    labs = np.random.default_rng(M).integers(0, M, s.n).astype(np.int32)
+    lt = torch.from_numpy(labs).cuda()
+    got = ctx.symdel_overlap_matrix(i, j, lt, lt, M, True).cpu().numpy()
+    assert (got == oracle.overlap_matrix(i.cpu().numpy(), j.cpu().numpy(), labs, labs, M, True)).all()
+    q, r = synth.cross_sets(500, 5000, 92)
+    qi, rj, _ = ctx.symdel_cross(*sd.to_device(q), *sd.to_device(r), 2)
+    lq = np.random.default_rng(M + 1).integers(0, M, q.n).astype(np.int32)
+    lr = np.random.default_rng(M + 2).integers(0, M, r.n).astype(np.int32)
+    got = ctx.symdel_overlap_matrix(qi, rj, torch.from_numpy(lq).cuda(), torch.from_numpy(lr).cuda(), M, False).cpu().numpy()
+    assert (got == oracle.overlap_matrix(qi.cpu().numpy(), rj.cpu().numpy(), lq, lr, M, False)).all()
+    if M > 1:
+        with pytest.raises(sd.SymdelError) as e:
+            ctx.symdel_overlap_matrix(i, j, lt, lt, M - 1, True)  # some label == M - 1 is out of range
+        assert e.value.code == sd.E_ARG
+
+
 def test_small_workspace_forces_chunking(torch, sd, ctx, oracle):
     s = synth.tcr_set(20000, 22)
     exp = oracle.symdel_self(s.seqs, s.offsets, 2)

@@ -416,3 +416,24 @@ def test_hamming_vs_levenshtein_relations(oracle):
             assert ham[(a, b)] == v
     ci, cj, cd = oracle.hamming_cross(s.seqs, s.offsets, s.seqs, s.offsets, 2)
     assert {(int(a), int(b)): int(c) for a, b, c in zip(ci, cj, cd) if a < b} == ham
+
+
+# ---- NEXT-4 M x M overlap matrix (reading A-18) ----------------------------------------
+def test_overlap_matrix_hand_case_and_invariants(oracle):
+    # sequences 0..5 in repertoires [0, 0, 1, 1, 2, 2]; pairs (0,1) within rep 0; (0,2), (1,3) between 0 and 1; (2,4) 1-2
+    lab = np.array([0, 0, 1, 1, 2, 2], dtype=np.int32)
+    i, j = np.array([0, 0, 1, 2]), np.array([1, 2, 3, 4])
+    m = oracle.overlap_matrix(i, j, lab, lab, 3, True)
+    assert m.tolist() == [[1, 2, 0], [2, 0, 1], [0, 1, 0]]
+    assert (m == m.T).all() and np.triu(m).sum() == len(i)
+    # cross form: rows = query repertoires, columns = reference repertoires, no mirroring
+    mq = oracle.overlap_matrix(np.array([0, 1, 1]), np.array([5, 5, 0]), np.array([1, 0], np.int32), lab, 3, False)
+    assert mq.tolist() == [[1, 0, 1], [0, 0, 1], [0, 0, 0]] and mq.sum() == 3
+    # against numpy's scatter-add on a real result
+    s = synth.tcr_set(3000, 81)
+    ri, rj, _ = oracle.symdel_self(s.seqs, s.offsets, 2)
+    labs = (np.arange(s.n) % 5).astype(np.int32)
+    ref = np.zeros((5, 5), np.int64)
+    np.add.at(ref, (labs[ri], labs[rj]), 1)
+    ref = ref + ref.T - np.diag(np.diag(ref))
+    assert (oracle.overlap_matrix(ri, rj, labs, labs, 5, True) == ref).all()
