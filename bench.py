@@ -318,6 +318,21 @@ def main():
                      "frac_of_nominal_8000": achieved / 8000.0},
         "clocks": clocks,
     }
+    if fused:
+        # The LONGEST kernel is not the HBM-bound one: k_gen2_part is bound by instruction issue.
+        # Its executed warp instructions per launch come from the committed ncu capture (not an algorithmic count);
+        # peak = 148 SMs x 4 schedulers x 1 warp instruction per clock at the SM clock sampled during the run.
+        winst = load_traffic("k_gen2_part_warp_instructions")
+        sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+        issue_peak = 148 * 4 * sm_mhz * 1e6 / 1e9
+        if winst and args.config == 3 and not args.dense and not args.prefix:
+            ach = winst / (stage["ms_generate"] * 1e-3) / 1e9
+            line["roofline_longest_kernel"] = {
+                "bound": "alu", "kernel": "k_gen2_part (generation + level-1 partition)", "achieved": ach,
+                "peak": issue_peak, "unit": "G warp-instructions/s (executed, from profiles/traffic.json)",
+                "frac": ach / issue_peak, "launch_ms": stage["ms_generate"],
+                "share_of_step": stage["ms_generate"] / stage["ms_total"],
+                "hbm_gbs": (8 * n_rec + in_bytes) / (stage["ms_generate"] * 1e-3) / 1e9}
     if not args.no_cpu_baseline and world == 1 and not args.dense:
         n_sample = min(s.n, args.ref_sample)
         pairs, dt = cpu_baseline_run(n_sample, d, s)
