@@ -359,7 +359,10 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
 //
 // K32: the partitioned bits and the bitmap bits all sit in the high word of the record (the usual
 // layout); the filter phases then work on 32-bit words and keep only those in registers.
-constexpr int JF_THREADS = 512, JF_NW = JF_THREADS / 32;
+#ifndef JF_THREADS_
+#define JF_THREADS_ 512
+#endif
+constexpr int JF_THREADS = JF_THREADS_, JF_NW = JF_THREADS / 32;
 constexpr int JF_BM_BITS = 16, JF_BM_WORDS = (1 << JF_BM_BITS) / 32;
 
 template <int LMAX, int SLOT_BITS>
@@ -614,7 +617,6 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_bkt(const JoinBktPara
     Smem& S = *reinterpret_cast<Smem*>(jn_smem);
     const JoinParams& P = BP.j;
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const u32 lane_lt = (1u << lane) - 1u;
     const u32 tile = BP.tiles ? BP.tiles[blockIdx.x] : blockIdx.x;
     const u32 b0 = tile * BP.group, b1 = min(b0 + BP.group, BP.nbuckets);
     auto key_of = [&](u64 y) -> K { return K32 ? (K)(y >> 32) : (K)y; };
@@ -654,27 +656,24 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_bkt(const JoinBktPara
     for (u32 b = b0; b < b1; ++b) {
         const u32 n = min(BP.cnt[b], BP.cap);
         const u64* const rp = P.rec + (u64)b * BP.cap;
-        for (u32 i0 = 0; i0 < n; i0 += 2 * JF_THREADS) {  // block-uniform trip count: the ballots below are full-warp
-            const u32 i = i0 + 2 * tid;
-            u64 y0 = 0, y1 = 0;
-            bool c0 = false, c1 = false;
+        // one shared-memory atomic per LISTED record (about one in ten): cheaper in issue slots than warp aggregation
+        for (u32 i = 2 * tid; i < n; i += 2 * JF_THREADS) {
+            u64 y0, y1 = 0;
+            bool c1 = false;
             if (i + 1 < n) {
                 const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + i);
                 y0 = t.x, y1 = t.y;
-                c0 = listed(key_of(y0)), c1 = listed(key_of(y1));
-            } else if (i < n) {
+                c1 = listed(key_of(y1));
+            } else {
                 y0 = rp[i];
-                c0 = listed(key_of(y0));
             }
-            const u32 bal0 = __ballot_sync(SD_FULL, c0), bal1 = __ballot_sync(SD_FULL, c1);
-            if (bal0 | bal1) {
-                const u32 n0 = __popc(bal0);
-                u32 at = 0;
-                if (lane == 0) at = jf_atoms_add(&S.nlist, n0 + (u32)__popc(bal1));
-                at = __shfl_sync(SD_FULL, at, 0);
-                const u32 a0 = at + __popc(bal0 & lane_lt), a1 = at + n0 + __popc(bal1 & lane_lt);
-                if (c0 && a0 < (u32)LMAX) S.list[a0] = y0;
-                if (c1 && a1 < (u32)LMAX) S.list[a1] = y1;
+            if (listed(key_of(y0))) {
+                const u32 at = jf_atoms_add(&S.nlist, 1u);
+                if (at < (u32)LMAX) S.list[at] = y0;
+            }
+            if (c1) {
+                const u32 at = jf_atoms_add(&S.nlist, 1u);
+                if (at < (u32)LMAX) S.list[at] = y1;
             }
         }
     }
