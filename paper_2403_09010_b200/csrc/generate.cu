@@ -651,7 +651,7 @@ struct GenPartShared {
     u64 Bpow[33];
     u32 cnt[256];     // records staged per digit since the last flush (may exceed GP_S: the excess went to the bins directly)
     uint2 fl[256];    // flush: {index of the claimed segment in bins (0xffffffff = bin full), records to copy}
-    u32 total;        // records staged since the last flush
+    u32 total[3];     // records staged in round r go to total[r % 3] (three words: a fast warp of round r + 1 never touches the word the slow warps of round r still read)
     unsigned char map[GP_NW][32];
 };
 
@@ -673,7 +673,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     if (tid < 32) sh.R[tid] = c_R[tid];
     if (tid < 33) sh.Bpow[tid] = c_Bpow[tid];
     if (tid < 256) sh.cnt[tid] = 0;
-    if (tid == 0) sh.total = 0;
+    if (tid < 3) sh.total[tid] = 0;
     __syncthreads();
     const int d = P.d;
     const bool thinning = P.thinning != 0;
@@ -710,6 +710,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     i64 wt = (i64)blockIdx.x * GP_NW + warp;
     const i64 wstride = (i64)gridDim.x * GP_NW;
     bool have = false;  // a task is loaded and has batches left
+    u32 rnd = 0, staged = 0;  // round index mod 3; records staged since the last flush (block-uniform)
     u32 s = 0, ns = 0, Li = 0, cum_incl = 0, cum_excl = 0;
     u64 gid0 = 0;
     i64 o0 = 0;  // lane as sequence index: offset of its residues
@@ -816,12 +817,14 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
             have = s < ns;
             const u32 wmade = __reduce_add_sync(SD_FULL, made);
             made = 0;
-            if (lane == 0 && wmade) atomicAdd(&sh.total, wmade);
+            if (lane == 0 && wmade) atomicAdd(&sh.total[rnd], wmade);
         }
         // ---- round end: anyone left?  flush when the stage is about full (always at the end) ----
         const bool more = have || wt < P.groups_total;
         const int any_more = __syncthreads_or(more);
-        const u32 staged = sh.total;
+        staged += sh.total[rnd];
+        rnd = rnd == 2 ? 0 : rnd + 1;
+        if (tid == 0) sh.total[rnd == 2 ? 0 : rnd + 1] = 0;  // the word of the round after next: nobody reads or adds to it now
         if (staged > (u32)GP_FLUSH_AT || (!any_more && staged > 0)) {
             if (tid < 256) {
                 const u32 cn_ = min(sh.cnt[tid], (u32)GP_S);
@@ -844,11 +847,157 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
             }
             __syncthreads();
             if (tid < 256) sh.cnt[tid] = 0;
-            if (tid == 0) sh.total = 0;
+            staged = 0;
             __syncthreads();
         }
         if (!any_more) break;
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused general path (k_generate_part): the enumeration of k_generate (any d <= 4, any length <= 64)
+// with the staging / flushing of k_gen2_part.  One sweep per round instead of two: no counts, no scan,
+// no offsets — a canonical deletion set is hashed and pushed under its top 8 hash bits.
+constexpr int GQ_S = 16;           // stage slots per digit (a round makes at most GEN_THREADS * GEN_R = 2048 records)
+#ifndef GQ_FLUSH_AT
+#define GQ_FLUSH_AT 900
+#endif
+
+struct GenPartStage {
+    u64 stage[256 * GQ_S];  // digit dg, rank r -> stage[dg * GQ_S + ((r + dg) & (GQ_S - 1))]
+    u32 cnt[256];
+    uint2 fl[256];
+    u32 total[3];  // as in GenPartShared
+};
+
+template <bool CHUNKED>
+__global__ void __launch_bounds__(GEN_THREADS, 3) k_generate_part(GenPartParams PP) {
+    extern __shared__ __align__(16) unsigned char gen_smem[];
+    GenShared& sh = *reinterpret_cast<GenShared*>(gen_smem);
+    GenPartStage& ps = *reinterpret_cast<GenPartStage*>(gen_smem + ((sizeof(GenShared) + 15) & ~(size_t)15));
+    const GenParams& P = PP.g;
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int i = tid; i < (SD_L_MAX + 1) * (SD_D_MAX + 1); i += GEN_THREADS) sh.binom[i] = c_binom[i];
+    for (int i = tid; i < (SD_L_MAX + 1) * (SD_D_MAX + 2); i += GEN_THREADS) sh.vcum[i] = c_vcum[i];
+    if (tid < 32) sh.R[tid] = c_R[tid];
+    if (tid <= SD_L_MAX) sh.Bpow[tid] = c_Bpow[tid];
+    ps.cnt[tid] = 0;
+    if (tid < 3) ps.total[tid] = 0;
+    u32 rnd = 0, staged = 0;
+    const int d = P.d;
+    const bool thinning = P.thinning != 0;
+    const int kshift = 64 - P.hash_bits, id_bits = P.id_bits;
+    const u32 cnt_sa = (u32)__cvta_generic_to_shared(ps.cnt);
+
+    auto flush = [&]() {  // all threads; the caller has synchronised
+        {
+            const u32 cn_ = min(ps.cnt[tid], (u32)GQ_S);
+            u32 g = 0;
+            if (cn_) {
+                g = atomicAdd(&PP.cur[tid], cn_);
+                if (g + cn_ > PP.cap1) {
+                    atomicOr(&P.info->part_overflow, 1u);
+                    g = 0xffffffffu;
+                } else {
+                    g += tid * PP.cap1;
+                }
+            }
+            ps.fl[tid] = make_uint2(g, g == 0xffffffffu ? 0u : cn_);
+        }
+        __syncthreads();
+        // two digits per warp instruction: lanes 0-15 and 16-31
+        for (u32 dg = 2 * warp + (lane >> 4); dg < 256; dg += 2 * GEN_NW) {
+            const uint2 f = ps.fl[dg];
+            const u32 o = lane & 15u;
+            if (o < f.y) PP.bins[f.x + o] = ps.stage[dg * GQ_S + ((o + dg) & (GQ_S - 1))];
+        }
+        __syncthreads();
+        ps.cnt[tid] = 0;
+        staged = 0;
+        __syncthreads();
+    };
+
+    for (i64 gi = blockIdx.x; gi < P.groups_total; gi += gridDim.x) {
+        const bool in_b = gi >= P.groups_a;
+        const SeqSetDev& S = in_b ? P.b : P.a;
+        const i64 first = (in_b ? gi - P.groups_a : gi) * GEN_G;
+        const u32 ng = (u32)min((i64)GEN_G, S.n - first);
+        const u64 gid0 = (u64)first + (in_b ? (u64)P.n_a : 0ull);
+        __syncthreads();  // previous group fully consumed (also orders the table fill above)
+        if (tid < GEN_G) {
+            u32 L = 0;
+            if (tid < ng) {
+                const i64 a = S.off[first + tid];
+                L = min((u32)(S.off[first + tid + 1] - a), P.prefix);
+                sh.off[tid] = a;
+            }
+            sh.len[tid] = L;
+            u32 v = tid < ng ? sh.vcum[L * (SD_D_MAX + 2) + d + 1] : 0, inc = v;  // V(L, d), scanned over the group
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const u32 t = __shfl_up_sync(SD_FULL, inc, o);
+                if (lane >= (u32)o) inc += t;
+            }
+            sh.vbase[tid + 1] = inc;
+            if (tid == 0) sh.vbase[0] = 0;
+        }
+        __syncthreads();
+        for (u32 idx = tid; idx < ng * (u32)P.width; idx += GEN_THREADS) {
+            const u32 g = idx / (u32)P.width, q = idx - g * (u32)P.width;
+            sh.seq[g][q] = q < sh.len[g] ? (unsigned char)S.seqs[sh.off[g] + q] : (unsigned char)0;
+        }
+        __syncthreads();
+        if (tid < ng) {  // per-sequence tables (as in k_generate)
+            const u32 L = sh.len[tid];
+            const unsigned char* sq = sh.seq[tid];
+            u64 acc = 0;
+            for (u32 q = 0; q < L; ++q) {
+                const u64 nxt = acc + sh.R[sq[q] & 31] * sh.Bpow[q];
+                sh.U[tid][q] = acc - c_Binv[1] * nxt;
+                acc = nxt;
+            }
+            for (int k = 0; k <= SD_D_MAX; ++k) sh.C[tid][k] = c_Binv[k] * acc + (u64)(L - k + 1) * K_LEN;
+            for (int j = 1; j <= SD_D_MAX; ++j) {
+                u64 m = 0;
+                for (u32 q = 0; q < L; ++q)
+                    if (!thinning || q + j >= L || sq[q] != sq[q + j]) m |= 1ull << q;
+                sh.NE[tid][j - 1] = m;
+            }
+        }
+        __syncthreads();
+
+        const u32 T = sh.vbase[ng];
+        for (u32 rb = 0; rb < T; rb += GEN_THREADS * GEN_R) {
+            const u32 f0 = min(T, rb + tid * GEN_R), f1 = min(T, f0 + GEN_R);
+            u32 made = 0;
+            gen_walk(sh, f0, f1, ng, d, [&](u32 g, u32, int k, const int* p) {
+                if (!gen_canonical(sh, g, k, p)) return;
+                const u64 h = gen_hash(sh, g, k, p);
+                if (CHUNKED && gen_chunk_of(h, P.n_chunks) != P.chunk) return;
+                const u32 dg = (u32)(h >> 56);
+                const u64 rec = ((h >> kshift) << id_bits) | (gid0 + g);
+                u32 r;
+                asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(r) : "r"(cnt_sa + dg * 4u) : "memory");
+                if (r < (u32)GQ_S) {
+                    ps.stage[dg * GQ_S + ((r + dg) & (GQ_S - 1))] = rec;
+                } else {
+                    const u32 at = atomicAdd(&PP.cur[dg], 1u);
+                    if (at < PP.cap1) PP.bins[(u64)dg * PP.cap1 + at] = rec;
+                    else atomicOr(&P.info->part_overflow, 1u);
+                }
+                ++made;
+            });
+            const u32 wmade = __reduce_add_sync(SD_FULL, made);
+            if (lane == 0 && wmade) atomicAdd(&ps.total[rnd], wmade);
+            __syncthreads();
+            staged += ps.total[rnd];
+            rnd = rnd == 2 ? 0 : rnd + 1;
+            if (tid == 0) ps.total[rnd == 2 ? 0 : rnd + 1] = 0;  // the word of the round after next
+            if (staged > (u32)GQ_FLUSH_AT) flush();  // block-uniform
+        }
+    }
+    __syncthreads();
+    if (staged > 0) flush();
 }
 
 typedef void (*Gen2Kernel)(GenParams);
@@ -1005,12 +1154,16 @@ cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
 
 // Fused generation + level-1 partition (fast generator only: see sd_gen_part_applies).  bins: 256 x cap1
 // records; cur: 256 cursors, zeroed here.  info->part_overflow != 0 afterwards: a bin was full.
-bool sd_gen_part_applies(const Layout& lay, int width) { return use_fast(lay, width) && lay.hash_bits >= 8; }
+bool sd_gen_part_applies(const Layout& lay, int width) {
+    (void)width;
+    return lay.hash_bits >= 8;
+}
 
 cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1, DevInfo* info,
                         cudaStream_t st, i64* launches) {
+    const bool fast = use_fast(lay, width);
     GenPartParams PP{};
-    PP.g = make_params2(a, b, lay, width);
+    PP.g = fast ? make_params2(a, b, lay, width) : make_params(a, b, lay, width);
     if (PP.g.groups_total == 0) return cudaSuccess;
     PP.g.info = info;
     PP.bins = bins;
@@ -1018,17 +1171,26 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     PP.cap1 = (u32)cap1;
     typedef void (*Kern)(GenPartParams);
     static const Kern kerns[4] = {k_gen2_part<false, false>, k_gen2_part<false, true>, k_gen2_part<true, false>, k_gen2_part<true, true>};
+    static const Kern gkerns[2] = {k_generate_part<false>, k_generate_part<true>};
+    constexpr size_t gsm = ((sizeof(GenShared) + 15) & ~(size_t)15) + sizeof(GenPartStage);
     static bool attr_set = false;
     cudaError_t e;
     if (!attr_set) {
         for (Kern k : kerns)
             if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GenPartShared))) != cudaSuccess) return e;
+        for (Kern k : gkerns)
+            if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm)) != cudaSuccess) return e;
         attr_set = true;
     }
     if ((e = cudaMemsetAsync(cur, 0, 256 * sizeof(u32), st)) != cudaSuccess) return e;
-    const int grid = (int)std::min<i64>((PP.g.groups_total + GP_NW - 1) / GP_NW, 148 * GP_MINB);
-    const bool plain = lay.hash_bits + lay.id_bits == 64 && lay.id_bits <= 31;
-    kerns[(lay.n_chunks > 1 ? 2 : 0) + (plain ? 1 : 0)]<<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
+    if (fast) {
+        const int grid = (int)std::min<i64>((PP.g.groups_total + GP_NW - 1) / GP_NW, 148 * GP_MINB);
+        const bool plain = lay.hash_bits + lay.id_bits == 64 && lay.id_bits <= 31;
+        kerns[(lay.n_chunks > 1 ? 2 : 0) + (plain ? 1 : 0)]<<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
+    } else {
+        const int grid = (int)std::min<i64>(PP.g.groups_total, 148 * 3);
+        gkerns[lay.n_chunks > 1 ? 1 : 0]<<<grid, GEN_THREADS, gsm, st>>>(PP);
+    }
     if (launches) ++*launches;
     return cudaGetLastError();
 }

@@ -313,8 +313,10 @@ def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
     if (not opts or set(opts) <= {"FORCE_CHUNKS", "HASH_BITS", "NO_THINNING"}) and opts.get("HASH_BITS", 64) >= 16:
         assert st["join_general"] == 0  # (a hash of 8 bits piles thousands of records on each key: the lists overflow)
         assert st["fused_chunks"] == st["n_chunks"]
-    if "EXACT_PIPELINE" in opts or "GENERAL_GENERATE" in opts or "SORT_BITS" in opts:
+    if "EXACT_PIPELINE" in opts or "SORT_BITS" in opts:
         assert st["fused_chunks"] == 0
+    if set(opts) <= {"GENERAL_GENERATE", "FORCE_CHUNKS"} and "GENERAL_GENERATE" in opts:
+        assert st["fused_chunks"] == st["n_chunks"]  # k_generate_part: the general generator, fused
 
 
 @pytest.mark.parametrize("copies,sort_bits,general,expect_general", [
