@@ -640,6 +640,9 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
 #ifndef GP_MINB
 #define GP_MINB 3
 #endif
+#ifndef GP_BATCHES
+#define GP_BATCHES 2  // batches per warp between two block-wide flush decisions
+#endif
 constexpr int GP_NW = GP_THREADS / 32, GP_S = 32;
 static_assert(GP_THREADS >= 256 && GP_THREADS % 32 == 0, "one thread per digit in the flush");
 
@@ -716,6 +719,8 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     i64 o0 = 0;  // lane as sequence index: offset of its residues
     const int8_t* seqs = nullptr;
     while (true) {
+#pragma unroll 1
+        for (int rep = 0; rep < GP_BATCHES; ++rep) {
         if (!have && wt < P.groups_total) {
             const bool in_b = wt >= P.groups_a;
             const SeqSetDev& S = in_b ? P.b : P.a;
@@ -818,6 +823,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
             const u32 wmade = __reduce_add_sync(SD_FULL, made);
             made = 0;
             if (lane == 0 && wmade) atomicAdd(&sh.total[rnd], wmade);
+        }
         }
         // ---- round end: anyone left?  flush when the stage is about full (always at the end) ----
         const bool more = have || wt < P.groups_total;

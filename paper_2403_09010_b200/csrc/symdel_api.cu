@@ -33,8 +33,10 @@ struct symdel_ctx {
     i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0, opt_general_gen = 0;
     i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0, opt_join_general = 0, opt_exact = 0, opt_prefix = 0, opt_metric = 0;
     DevInfo* h_info = nullptr;  // pinned; followed by 256 u32 (the level-1 bin counts of the fused pipeline)
-    void* arena = nullptr;      // device arena of the *_host entry points
+    void* arena = nullptr;      // device arena of the *_host entry points: outputs + workspace
     size_t arena_bytes = 0;
+    void* in_arena = nullptr;   // ... and their inputs (separate: the copies start before the workspace size is known)
+    size_t in_arena_bytes = 0;
     cudaStream_t stream = nullptr;  // stream of the *_host entry points
     std::vector<cudaEvent_t> events;
 };
@@ -490,13 +492,13 @@ restart:
     return n_out > capacity ? SYMDEL_E_CAPACITY : SYMDEL_OK;
 }
 
-int ensure_arena(symdel_ctx* ctx, size_t bytes) {
-    if (ctx->arena_bytes >= bytes) return SYMDEL_OK;
-    if (ctx->arena) cudaFree(ctx->arena);
-    ctx->arena = nullptr;
-    ctx->arena_bytes = 0;
-    CK(cudaMalloc(&ctx->arena, bytes));
-    ctx->arena_bytes = bytes;
+int ensure_arena(symdel_ctx* ctx, void** arena, size_t* have, size_t bytes) {
+    if (*have >= bytes) return SYMDEL_OK;
+    if (*arena) cudaFree(*arena);
+    *arena = nullptr;
+    *have = 0;
+    CK(cudaMalloc(arena, bytes));
+    *have = bytes;
     return SYMDEL_OK;
 }
 
@@ -513,9 +515,28 @@ int run_host(symdel_ctx* ctx, const int8_t* a_seqs, const i64* a_off, i64 n_a, c
     CK(cudaSetDevice(ctx->device));
     const i64 res_a = a_off[n_a], res_b = cross ? b_off[n_b] : 0;
     if (res_a < 0 || res_b < 0) return SYMDEL_E_OFFSETS;
-    // exact record bound from the host offsets
+    // ---- inputs first: the copies run while the host sizes the workspace ----
+    const i64 in_bytes = align_up(res_a + 16) + align_up((n_a + 1) * 8) + align_up(res_b + 16) + align_up((n_b + 1) * 8);
+    int rc = ensure_arena(ctx, &ctx->in_arena, &ctx->in_arena_bytes, (size_t)(in_bytes + 4096));
+    if (rc) return rc;
+    cudaStream_t st = ctx->stream;
+    Bump in(ctx->in_arena, (i64)ctx->in_arena_bytes);
+    int8_t* d_as = in.take<int8_t>(res_a + 16);
+    i64* d_ao = in.take<i64>(n_a + 1);
+    int8_t* d_bs = in.take<int8_t>(res_b + 16);
+    i64* d_bo = in.take<i64>(n_b + 1);
+    if (!in.ok) return SYMDEL_E_INTERNAL;
+    CK(cudaMemcpyAsync(d_ao, a_off, (size_t)(n_a + 1) * 8, cudaMemcpyHostToDevice, st));
+    if (res_a) CK(cudaMemcpyAsync(d_as, a_seqs, (size_t)res_a, cudaMemcpyHostToDevice, st));
+    if (cross) {
+        CK(cudaMemcpyAsync(d_bo, b_off, (size_t)(n_b + 1) * 8, cudaMemcpyHostToDevice, st));
+        if (res_b) CK(cudaMemcpyAsync(d_bs, b_seqs, (size_t)res_b, cudaMemcpyHostToDevice, st));
+    }
+    // exact record bound from the host offsets (a malformed input leaves through an error below; the copies
+    // already queued only touch the context's own arena)
     i64 nmax = 0;
     int maxlen = 0;
+    bool bad_off = false, too_long = false;
     for (int s = 0; s < (cross ? 2 : 1); ++s) {
         const i64* off = s ? b_off : a_off;
         const i64 n = s ? n_b : n_a;
@@ -523,38 +544,32 @@ int run_host(symdel_ctx* ctx, const int8_t* a_seqs, const i64* a_off, i64 n_a, c
         for (int L = 0; L <= SD_L_MAX; ++L) vtab[L] = vcount_host(L, d);
         for (i64 i = 0; i < n; ++i) {
             const i64 L = off[i + 1] - off[i];
-            if (L < 0) return SYMDEL_E_OFFSETS;
-            if (L > SD_L_MAX) return SYMDEL_E_TOO_LONG;
-            nmax += (i64)vtab[L];
-            maxlen = std::max(maxlen, (int)L);
+            if (L < 0) bad_off = true;
+            else if (L > SD_L_MAX) too_long = true;
+            else {
+                nmax += (i64)vtab[L];
+                maxlen = std::max(maxlen, (int)L);
+            }
         }
+    }
+    if (bad_off || too_long) {
+        cudaStreamSynchronize(st);
+        return bad_off ? SYMDEL_E_OFFSETS : SYMDEL_E_TOO_LONG;
     }
     const i64 n_total = n_a + n_b;
     const int npass_max = 7, ppass_max = 8;
     const i64 ccap = std::max<i64>(1 << 20, 2 * nmax), scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity);
     const i64 ws_bytes = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nmax, 1), npass_max) + cand_bytes(ccap + n_total + 64, ppass_max) +
                          cand_bytes(scap, ppass_max) + 65536;
-    const i64 in_bytes = align_up(res_a + 16) + align_up((n_a + 1) * 8) + align_up(res_b + 16) + align_up((n_b + 1) * 8);
     const i64 out_bytes = 3 * align_up(capacity * 4 + 16);
-    int rc = ensure_arena(ctx, (size_t)(in_bytes + out_bytes + ws_bytes + 4096));
+    rc = ensure_arena(ctx, &ctx->arena, &ctx->arena_bytes, (size_t)(out_bytes + ws_bytes + 4096));
     if (rc) return rc;
-    cudaStream_t st = ctx->stream;
     Bump ar(ctx->arena, (i64)ctx->arena_bytes);
-    int8_t* d_as = ar.take<int8_t>(res_a + 16);
-    i64* d_ao = ar.take<i64>(n_a + 1);
-    int8_t* d_bs = ar.take<int8_t>(res_b + 16);
-    i64* d_bo = ar.take<i64>(n_b + 1);
     i32* d_i = ar.take<i32>(capacity + 4);
     i32* d_j = ar.take<i32>(capacity + 4);
     i32* d_d = ar.take<i32>(capacity + 4);
     void* d_ws = ar.take<char>(ws_bytes);
     if (!ar.ok) return SYMDEL_E_INTERNAL;
-    if (res_a) CK(cudaMemcpyAsync(d_as, a_seqs, (size_t)res_a, cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(d_ao, a_off, (size_t)(n_a + 1) * 8, cudaMemcpyHostToDevice, st));
-    if (cross) {
-        if (res_b) CK(cudaMemcpyAsync(d_bs, b_seqs, (size_t)res_b, cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(d_bo, b_off, (size_t)(n_b + 1) * 8, cudaMemcpyHostToDevice, st));
-    }
     SeqSetDev A{d_as, d_ao, n_a}, B{d_bs, d_bo, cross ? n_b : 0};
     rc = run_pipeline(ctx, A, B, cross, d, d_ws, ws_bytes, d_i, d_j, d_d, capacity, n_pairs_host, st);
     if (rc != SYMDEL_OK && rc != SYMDEL_E_CAPACITY) return rc;
@@ -596,6 +611,7 @@ void symdel_destroy(symdel_ctx* ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     if (ctx->arena) cudaFree(ctx->arena);
+    if (ctx->in_arena) cudaFree(ctx->in_arena);
     if (ctx->h_info) cudaFreeHost(ctx->h_info);
     if (ctx->stream) cudaStreamDestroy(ctx->stream);
     for (auto e : ctx->events) cudaEventDestroy(e);
