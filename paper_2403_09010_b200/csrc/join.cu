@@ -598,6 +598,14 @@ constexpr int JF_LMAX_L = JF_T + 4096, JF_SLOTB_L = 12, JF_MINB_L = JF_IT > 8 ? 
 // k_join_fast over them, with no boundary tests and no tails.  Buckets of one block share the bitmaps
 // and chains; records of different buckets never pair because the chain walk compares whole hashes.
 // Same two instances (small list first, redo list, large list), same fallback flag.
+#ifndef JB_TARGET
+#define JB_TARGET 4096  // records per block of k_join_bkt
+#endif
+#ifndef JB_PF_
+#define JB_PF_ 4
+#endif
+constexpr int JB_PF = JB_PF_;  // k_join_bkt: 16-byte loads per thread kept in flight (prefetch path)
+
 struct JoinBktParams {
     JoinParams j;       // rec = bucket regions; topmask unused
     const u32* cnt;     // records per bucket
@@ -622,6 +630,33 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_bkt(const JoinBktPara
     auto key_of = [&](u64 y) -> K { return K32 ? (K)(y >> 32) : (K)y; };
     const int bm_shift = K32 ? P.bm_shift - 32 : P.bm_shift;
 
+    // Prefetch path (the usual case: the block's buckets need at most JB_PF 16-byte loads per thread): every load
+    // is issued before anything else and the filter words stay in registers for both sweeps.
+    u32 itb = 0;  // 16-byte loads per thread and bucket
+    for (u32 b = b0; b < b1; ++b) itb = max(itb, (min(BP.cnt[b], BP.cap) + 2 * JF_THREADS - 1) / (2 * JF_THREADS));
+    const u32 ns = (b1 - b0) * itb;
+    const bool pf = ns <= (u32)JB_PF;
+    K kx[2 * JB_PF];
+    u32 vm = 0;  // bit e: kx[e] holds a record
+    if (pf) {
+#pragma unroll
+        for (int sl = 0; sl < JB_PF; ++sl) {
+            kx[2 * sl] = kx[2 * sl + 1] = 0;
+            if ((u32)sl < ns) {
+                const u32 g = (u32)sl / itb, b = b0 + g;
+                const u32 n = min(BP.cnt[b], BP.cap), i = 2 * tid + ((u32)sl - g * itb) * (2 * JF_THREADS);
+                const u64* const rp = P.rec + (u64)b * BP.cap;
+                if (i + 1 < n) {
+                    const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + i);
+                    kx[2 * sl] = key_of(t.x), kx[2 * sl + 1] = key_of(t.y);
+                    vm |= 3u << (2 * sl);
+                } else if (i < n) {
+                    kx[2 * sl] = key_of(rp[i]);
+                    vm |= 1u << (2 * sl);
+                }
+            }
+        }
+    }
     for (u32 i = tid; i < 2 * JF_BM_WORDS / 4; i += JF_THREADS)
         reinterpret_cast<uint4*>(S.bit_a)[i] = make_uint4(0u, 0u, 0u, 0u);  // bit_a and bit_b are adjacent
     for (u32 i = tid; i < SLOTS / 4; i += JF_THREADS)
@@ -633,47 +668,56 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_bkt(const JoinBktPara
         const u32 b = bm_of(y), bit = 1u << (b & 31u);
         if (atomicOr(&S.bit_a[b >> 5], bit) & bit) atomicOr(&S.bit_b[b >> 5], bit);
     };
-    // ---- 1. bitmaps (two records per 16-byte load; regions are 256-byte aligned) ----
-    for (u32 b = b0; b < b1; ++b) {
-        const u32 n = min(BP.cnt[b], BP.cap);
-        const u64* const rp = P.rec + (u64)b * BP.cap;
-        for (u32 i = 2 * tid; i < n; i += 2 * JF_THREADS) {
-            if (i + 1 < n) {
-                const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + i);
-                mark(key_of(t.x));
-                mark(key_of(t.y));
-            } else {
-                mark(key_of(rp[i]));
-            }
-        }
-    }
-    __syncthreads();
-    // ---- 2. list the records whose "seen twice" bit is set ----
     auto listed = [&](K y) -> bool {
         const u32 b = bm_of(y);
         return (S.bit_b[b >> 5] >> (b & 31u)) & 1u;
     };
-    for (u32 b = b0; b < b1; ++b) {
-        const u32 n = min(BP.cnt[b], BP.cap);
-        const u64* const rp = P.rec + (u64)b * BP.cap;
-        // one shared-memory atomic per LISTED record (about one in ten): cheaper in issue slots than warp aggregation
-        for (u32 i = 2 * tid; i < n; i += 2 * JF_THREADS) {
-            u64 y0, y1 = 0;
-            bool c1 = false;
-            if (i + 1 < n) {
-                const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + i);
-                y0 = t.x, y1 = t.y;
-                c1 = listed(key_of(y1));
-            } else {
-                y0 = rp[i];
+    auto append = [&](u64 y) {  // one shared-memory atomic per LISTED record (about one in ten on sparse data)
+        const u32 at = jf_atoms_add(&S.nlist, 1u);
+        if (at < (u32)LMAX) S.list[at] = y;
+    };
+    if (pf) {
+        // ---- 1. bitmaps ----
+#pragma unroll
+        for (int e = 0; e < 2 * JB_PF; ++e)
+            if ((vm >> e) & 1u) mark(kx[e]);
+        __syncthreads();
+        // ---- 2. list the records whose "seen twice" bit is set (whole record re-read: L1/L2) ----
+#pragma unroll
+        for (int e = 0; e < 2 * JB_PF; ++e)
+            if (((vm >> e) & 1u) && listed(kx[e])) {
+                const u32 sl = (u32)e >> 1, g = sl / itb;
+                append(P.rec[(u64)(b0 + g) * BP.cap + 2 * tid + (sl - g * itb) * (2 * JF_THREADS) + ((u32)e & 1u)]);
             }
-            if (listed(key_of(y0))) {
-                const u32 at = jf_atoms_add(&S.nlist, 1u);
-                if (at < (u32)LMAX) S.list[at] = y0;
+    } else {
+        // ---- 1. bitmaps (two records per 16-byte load; regions are 256-byte aligned) ----
+        for (u32 b = b0; b < b1; ++b) {
+            const u32 n = min(BP.cnt[b], BP.cap);
+            const u64* const rp = P.rec + (u64)b * BP.cap;
+            for (u32 i = 2 * tid; i < n; i += 2 * JF_THREADS) {
+                if (i + 1 < n) {
+                    const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + i);
+                    mark(key_of(t.x));
+                    mark(key_of(t.y));
+                } else {
+                    mark(key_of(rp[i]));
+                }
             }
-            if (c1) {
-                const u32 at = jf_atoms_add(&S.nlist, 1u);
-                if (at < (u32)LMAX) S.list[at] = y1;
+        }
+        __syncthreads();
+        // ---- 2. list the records whose "seen twice" bit is set ----
+        for (u32 b = b0; b < b1; ++b) {
+            const u32 n = min(BP.cnt[b], BP.cap);
+            const u64* const rp = P.rec + (u64)b * BP.cap;
+            for (u32 i = 2 * tid; i < n; i += 2 * JF_THREADS) {
+                if (i + 1 < n) {
+                    const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + i);
+                    if (listed(key_of(t.x))) append(t.x);
+                    if (listed(key_of(t.y))) append(t.y);
+                } else {
+                    const u64 y = rp[i];
+                    if (listed(key_of(y))) append(y);
+                }
             }
         }
     }
@@ -876,7 +920,7 @@ static cudaError_t jn_launch_bkt(const JoinBktParams& BP, unsigned grid, bool la
 
 u32 sd_join_bkt_group(i64 n_records, u32 nbuckets) {  // buckets per block: about 4096 records
     const i64 avg = std::max<i64>(1, n_records / nbuckets);
-    return (u32)std::min<i64>(std::max<i64>(1, 4096 / avg), 256);
+    return (u32)std::min<i64>(std::max<i64>(1, JB_TARGET / avg), 256);
 }
 
 cudaError_t sd_join_bkt(const u64* buckets, const u32* cnt, u32 cap, u32 nbuckets, u32 group, const Layout& lay, u64* cand,
