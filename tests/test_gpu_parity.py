@@ -452,6 +452,21 @@ def test_overlap_matrix(torch, sd, ctx, oracle, M):
         assert e.value.code == sd.E_ARG
 
 
+@pytest.mark.parametrize("d,opts", [(2, {}), (3, {}), (4, {}), (4, {"EXACT_PIPELINE": 1}), (3, {"FORCE_CHUNKS": 3}),
+                                    (4, {"PREFIX_LEN": 20})])
+def test_long_sequences_up_to_the_limits(sd, oracle, d, opts):
+    """Edge of the limits: lengths 33..64 = SYMDEL_L_MAX (general generator, 64-bit verifier words) up to
+    d = 4 = SYMDEL_D_MAX (V(64, 4) = 679,121 deletion sets per sequence), against brute force."""
+    s = synth.bcr_set(60, 95, n_lineages=6, lo=33, hi=64, mean=50.0, sd=10.0, kmax=4)
+    assert s.lengths.max() > 56
+    c = sd.Context(0)
+    for k, v in opts.items():
+        c.symdel_set_option(getattr(sd, "OPT_" + k), v)
+    exp = oracle.bruteforce_self(s.seqs, s.offsets, d)
+    assert len(exp[0]) > 20
+    assert_same(run_self(sd, c, s, d), exp)
+
+
 def test_small_workspace_forces_chunking(torch, sd, ctx, oracle):
     s = synth.tcr_set(20000, 22)
     exp = oracle.symdel_self(s.seqs, s.offsets, 2)
