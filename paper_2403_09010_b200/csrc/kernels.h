@@ -105,6 +105,9 @@ cudaError_t sd_pack(SeqSetDev a, SeqSetDev b, int maxlen, void* slots, cudaStrea
 // (pair << 3 | dist) in order to surv[surv_base + ...]; info->n_surv = total; info->n_unique += unique.
 cudaError_t sd_verify(const u64* cand, i64 n_cand, const void* slots, const Layout& lay, int maxlen, u64* surv,
                       u64 surv_base, u64 surv_capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
+// the same when this is known to be the ONLY flush of the search: survivors go straight to the SoA outputs
+cudaError_t sd_verify_direct(const u64* cand, i64 n_cand, const void* slots, const Layout& lay, int maxlen, i32* out_i, i32* out_j,
+                             i32* out_dist, i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
 // surv sorted ascending (and unique unless dedup = 1).  Unpacks to SoA outputs, first `capacity`
 // only; info->n_out = total.
 cudaError_t sd_finalize(const u64* surv, i64 n_surv, const Layout& lay, int dedup, i32* out_i, i32* out_j, i32* out_dist,

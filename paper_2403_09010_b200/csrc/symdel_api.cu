@@ -291,6 +291,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
 
     const int width = (prefix > 0 ? std::min(maxlen, prefix) : maxlen) + 1;  // generation works on the (truncated) sequences
     i64 n_surv = 0, flushes = 0;
+    bool direct = false;  // the single flush wrote the outputs itself
     enum { ST_GEN, ST_SORT, ST_EMIT, ST_DEDUP, ST_VERIFY };
     i64 pass_count = 0;
 
@@ -300,6 +301,7 @@ restart:
     pass_count = 0;
     n_surv = 0;
     flushes = 0;
+    direct = false;
     S.n_records = S.n_candidates = 0;
     lay.n_chunks = P;
     CK(cudaMemsetAsync(&info->n_surv, 0, sizeof(u64) * 3, st));  // n_surv, n_out, n_unique
@@ -437,9 +439,15 @@ restart:
             u64* csorted = nullptr;
             CK(sd_sort_passes(candA, candB, nc, 0, ppass, 0, cand_scratch, st, &csorted, &S.n_launches));
             const size_t f2 = tm.mark();
-            // ---- S4: unique + verify; survivors appended at n_surv ----
-            CK(sd_verify(csorted, nc, slots, lay, maxlen, survA, (u64)n_surv, (u64)scap, verify_lb, info, st,
-                         &S.n_launches));
+            // ---- S4: unique + verify; survivors appended at n_surv — or, when this window holds every candidate of
+            //      the only chunk, unpacked straight into the outputs (no survivor list, no finalize) ----
+            direct = P == 1 && w0 == 0 && wend == C;
+            if (direct)
+                CK(sd_verify_direct(csorted, nc, slots, lay, maxlen, out_i, out_j, out_dist, capacity, verify_lb, info, st,
+                                    &S.n_launches));
+            else
+                CK(sd_verify(csorted, nc, slots, lay, maxlen, survA, (u64)n_surv, (u64)scap, verify_lb, info, st,
+                             &S.n_launches));
             rc = read_info(ctx, info, st);
             if (rc) return rc;
             if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
@@ -456,7 +464,9 @@ restart:
     // ---- final: (sort + unique) and unpack ----
     const size_t g0 = tm.mark();
     i64 n_out = 0;
-    if (n_surv > 0) {
+    if (direct) {
+        n_out = (i64)ctx->h_info->n_out;
+    } else if (n_surv > 0) {
         const u64* fin = survA;
         if (flushes > 1) {
             CK(sd_sort_prepare(surv_scratch, n_surv, spass, st));

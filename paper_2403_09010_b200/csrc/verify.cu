@@ -125,10 +125,14 @@ constexpr int VF_THREADS = 256, VF_IPT = 4, VF_TILE = VF_THREADS * VF_IPT;
 // memory, (2) spread the COMPACTED list over the threads for the distance computation (after dedup
 // only a fraction of the candidates is left: this keeps every lane busy), (3) ordered compaction of
 // the survivors (block scan + 32-wide decoupled look-back) so the output stays sorted.
-template <typename W>
+// DIRECT: this call is known to be the only flush of the whole search, so the survivors are final: they are
+// unpacked straight into (out_i, out_j, out_dist) (first surv_capacity of them) and info->n_out = their number.
+template <typename W, bool DIRECT>
 __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ cand, u64 n, const void* __restrict__ slots,
                                                       Layout lay, u64* __restrict__ surv, u64 surv_base,
-                                                      u64 surv_capacity, u64* lb_status, DevInfo* info) {
+                                                      u64 surv_capacity, u64* lb_status, DevInfo* info,
+                                                      i32* __restrict__ out_i, i32* __restrict__ out_j,
+                                                      i32* __restrict__ out_dist) {
     __shared__ unsigned short s_list[VF_TILE];
     __shared__ unsigned char s_res[VF_TILE];
     __shared__ u32 s_warp[VF_THREADS / 32 + 1];
@@ -194,7 +198,10 @@ __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ c
         if (tid == 0) {
             s_excl = excl;
             if (nuniq) atomicAdd((unsigned long long*)&info->n_unique, (unsigned long long)nuniq);
-            if (tile == gridDim.x - 1) info->n_surv = surv_base + excl + total;
+            if (tile == gridDim.x - 1) {
+                info->n_surv = surv_base + excl + total;
+                if (DIRECT) info->n_out = excl + total;
+            }
         }
     }
     __syncthreads();
@@ -203,8 +210,18 @@ __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ c
     for (int k = 0; k < VF_IPT; ++k) {
         if (keepmask & (1u << k)) {
             const u32 pos = tid * VF_IPT + k;
-            if (out < surv_capacity) surv[out] = (cand[base + pos] << 3) | (u64)s_res[pos];
-            else atomicOr(&info->err, (u32)SD_ERR_OVERFLOW);
+            if (DIRECT) {
+                if (out < surv_capacity) {  // beyond the caller's capacity: counted, not written (SYMDEL_E_CAPACITY)
+                    const u64 c = cand[base + pos];
+                    out_i[out] = (i32)(c >> lay.b_bits);
+                    out_j[out] = (i32)(c & bmask);
+                    out_dist[out] = (i32)s_res[pos];
+                }
+            } else if (out < surv_capacity) {
+                surv[out] = (cand[base + pos] << 3) | (u64)s_res[pos];
+            } else {
+                atomicOr(&info->err, (u32)SD_ERR_OVERFLOW);
+            }
             ++out;
         }
     }
@@ -334,11 +351,29 @@ cudaError_t sd_verify(const u64* cand, i64 n_cand, const void* slots, const Layo
     cudaError_t e = cudaMemsetAsync(lb_status, 0, (size_t)tiles * 8, st);
     if (e != cudaSuccess) return e;
     if (maxlen <= 32)
-        k_verify<u32><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, surv, surv_base, surv_capacity,
-                                                              lb_status, info);
+        k_verify<u32, false><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, surv, surv_base, surv_capacity,
+                                                                     lb_status, info, nullptr, nullptr, nullptr);
     else
-        k_verify<u64><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, surv, surv_base, surv_capacity,
-                                                              lb_status, info);
+        k_verify<u64, false><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, surv, surv_base, surv_capacity,
+                                                                     lb_status, info, nullptr, nullptr, nullptr);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+// The only flush of a search: unique + verify + unpack in one kernel.  info->n_out = number of result pairs
+// (the first `capacity` are written).
+cudaError_t sd_verify_direct(const u64* cand, i64 n_cand, const void* slots, const Layout& lay, int maxlen, i32* out_i, i32* out_j,
+                             i32* out_dist, i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches) {
+    const i64 tiles = sd_verify_tiles(n_cand);
+    if (tiles == 0) return cudaSuccess;
+    cudaError_t e = cudaMemsetAsync(lb_status, 0, (size_t)tiles * 8, st);
+    if (e != cudaSuccess) return e;
+    if (maxlen <= 32)
+        k_verify<u32, true><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, nullptr, 0, (u64)capacity, lb_status,
+                                                                    info, out_i, out_j, out_dist);
+    else
+        k_verify<u64, true><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, nullptr, 0, (u64)capacity, lb_status,
+                                                                    info, out_i, out_j, out_dist);
     if (launches) ++*launches;
     return cudaGetLastError();
 }
