@@ -28,6 +28,7 @@ struct DevInfo {
     u32 join_redo;      // k_join_fast: tiles on the redo list (keep right after join_fallback: cleared together)
     u32 part_overflow;  // fused pipeline: 1 = a level-1 bin was full, 2 = a level-2 bucket was full
     u32 pad;
+    u64 residues;       // sum of the (prefix-truncated) sequence lengths
 };
 enum { SD_ERR_OFFSETS = 1, SD_ERR_TOO_LONG = 2, SD_ERR_RESIDUE = 4, SD_ERR_INTERNAL = 8, SD_ERR_OVERFLOW = 16 };
 enum { SD_TK_SORT = 0, SD_TK_EMIT = 1, SD_TK_VERIFY = 2, SD_TK_FINAL = 3, SD_TK_SCAN = 4 };

@@ -40,7 +40,7 @@ __device__ __forceinline__ u32 gen_chunk_of(u64 h, u32 n_chunks) { return __umul
 
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, int prefix, DevInfo* info) {
-    u64 nmax = 0;
+    u64 nmax = 0, res = 0;
     u32 maxlen = 0, err = 0;
     const i64 stride = (i64)gridDim.x * blockDim.x;
     const i64 t0 = (i64)blockIdx.x * blockDim.x + threadIdx.x;
@@ -52,6 +52,7 @@ __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, i
         else if (L > SD_L_MAX) err |= SD_ERR_TOO_LONG;
         else {
             nmax += c_vcum[min(L, (i64)prefix) * (SD_D_MAX + 2) + d + 1];
+            res += (u64)min(L, (i64)prefix);
             maxlen = max(maxlen, (u32)L);
         }
     }
@@ -63,11 +64,13 @@ __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, i
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         nmax += __shfl_xor_sync(SD_FULL, nmax, o);
+        res += __shfl_xor_sync(SD_FULL, res, o);
         maxlen = max(maxlen, __shfl_xor_sync(SD_FULL, maxlen, o));
         err |= __shfl_xor_sync(SD_FULL, err, o);
     }
     if ((threadIdx.x & 31) == 0) {
         if (nmax) atomicAdd((unsigned long long*)&info->nmax, (unsigned long long)nmax);
+        if (res) atomicAdd((unsigned long long*)&info->residues, (unsigned long long)res);
         if (nmax && is_b) atomicAdd((unsigned long long*)&info->nmax_b, (unsigned long long)nmax);
         if (maxlen) atomicMax(&info->maxlen, maxlen);
         if (err) atomicOr(&info->err, err);
@@ -635,13 +638,13 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
 #define GP_THREADS 256
 #endif
 #ifndef GP_FLUSH_AT
-#define GP_FLUSH_AT 2800
+#define GP_FLUSH_AT 2800  // flush when more than this is staged after a round (i.e. after nearly every full round)
 #endif
 #ifndef GP_MINB
 #define GP_MINB 3
 #endif
-#ifndef GP_BATCHES
-#define GP_BATCHES 2  // batches per warp between two block-wide flush decisions
+#ifndef GP_ROUND
+#define GP_ROUND 5400  // records a block stages per round (21 per digit of the 32 slots); the host turns it into batches per warp
 #endif
 constexpr int GP_NW = GP_THREADS / 32, GP_S = 32;
 static_assert(GP_THREADS >= 256 && GP_THREADS % 32 == 0, "one thread per digit in the flush");
@@ -665,6 +668,7 @@ struct GenPartParams {
     u64* bins;    // 256 bins of cap1 records (256 * cap1 < 2^32)
     u32* cur;     // 256 bin cursors (zeroed by the host)
     u32 cap1;
+    u32 batches;  // k_gen2_part: batches per warp and round
 };
 
 template <bool CHUNKED, bool PLAIN>
@@ -720,7 +724,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     const int8_t* seqs = nullptr;
     while (true) {
 #pragma unroll 1
-        for (int rep = 0; rep < GP_BATCHES; ++rep) {
+        for (u32 rep = 0; rep < PP.batches; ++rep) {  // the same trip count in every warp: rounds stay balanced
         if (!have && wt < P.groups_total) {
             const bool in_b = wt >= P.groups_a;
             const SeqSetDev& S = in_b ? P.b : P.a;
@@ -1165,8 +1169,8 @@ bool sd_gen_part_applies(const Layout& lay, int width) {
     return lay.hash_bits >= 8;
 }
 
-cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1, DevInfo* info,
-                        cudaStream_t st, i64* launches) {
+cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1,
+                        double records_per_residue, DevInfo* info, cudaStream_t st, i64* launches) {
     const bool fast = use_fast(lay, width);
     GenPartParams PP{};
     PP.g = fast ? make_params2(a, b, lay, width) : make_params(a, b, lay, width);
@@ -1175,6 +1179,10 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     PP.bins = bins;
     PP.cur = cur;
     PP.cap1 = (u32)cap1;
+    {   // a batch fills the 32 lanes with residues: about 32 * records_per_residue records (thinning and padding: ~0.85)
+        const double per_round = GP_NW * 32.0 * std::max(records_per_residue, 0.03) * 0.85;
+        PP.batches = (u32)std::min(8.0, std::max(1.0, std::floor(GP_ROUND / per_round + 0.5)));
+    }
     typedef void (*Kern)(GenPartParams);
     static const Kern kerns[4] = {k_gen2_part<false, false>, k_gen2_part<false, true>, k_gen2_part<true, false>, k_gen2_part<true, true>};
     static const Kern gkerns[2] = {k_generate_part<false>, k_generate_part<true>};

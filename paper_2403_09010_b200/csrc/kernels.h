@@ -68,8 +68,9 @@ cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
 // Fused fast path: generation + level-1 partition into 256 bins of cap1 records (cur: 256 cursors =
 // the bin counts afterwards).  info->part_overflow != 0: a bin was full, redo with the exact pipeline.
 bool sd_gen_part_applies(const Layout& lay, int width);
-cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1, DevInfo* info,
-                        cudaStream_t st, i64* launches);
+// records_per_residue = (deletion sets of this chunk) / (residues): sizes the generation rounds
+cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1,
+                        double records_per_residue, DevInfo* info, cudaStream_t st, i64* launches);
 
 // ---- join.cu ------------------------------------------------------------------------------------
 i64 sd_join_tiles(i64 n_records);

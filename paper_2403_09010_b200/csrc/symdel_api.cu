@@ -206,6 +206,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     if (rc) return rc;
     if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
     const i64 nmax = (i64)ctx->h_info->nmax;
+    const i64 residues = (i64)ctx->h_info->residues;
     const int maxlen = (int)ctx->h_info->maxlen;
     const size_t ev_prepared = tm.mark();
 
@@ -252,7 +253,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     const i64 R = ws.left() - 8192;
     // a window of the candidate buffer ends with a whole record's pairs: at most one per other sequence
     const i64 cslack = n_total + 64;
-    i64 ccap = ctx->opt_cand_cap > 0 ? ctx->opt_cand_cap : std::max<i64>(1 << 20, 2 * nmax);
+    i64 ccap = ctx->opt_cand_cap > 0 ? ctx->opt_cand_cap : std::max<i64>(1 << 20, std::min<i64>(2 * nmax, nmax / 2 + ((i64)128 << 20)));
     i64 scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity + (ctx->opt_cand_cap > 0 ? ccap : 0));
     i64 ncap = std::max<i64>(nmax, 1);
     u32 P = ctx->opt_force_chunks > 0 ? (u32)ctx->opt_force_chunks : 1;
@@ -315,7 +316,8 @@ restart:
             const size_t x0 = tm.mark();
             lay.sort_bits = fp.b;
             CK(cudaMemsetAsync(&info->part_overflow, 0, sizeof(u32), st));
-            CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, info, st, &S.n_launches));
+            CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, (double)nmax / (double)std::max<i64>(residues, 1) / (double)P, info,
+                           st, &S.n_launches));
             const size_t x1 = tm.mark();
             if (fp.b2)
                 CK(sd_part2(recA, cur1, fp.cap1, recB, cnt2, fp.cap2, fp.b2, lay.id_bits + lay.hash_bits - fp.b, info, st,
@@ -568,7 +570,7 @@ int run_host(symdel_ctx* ctx, const int8_t* a_seqs, const i64* a_off, i64 n_a, c
     }
     const i64 n_total = n_a + n_b;
     const int npass_max = 7, ppass_max = 8;
-    const i64 ccap = std::max<i64>(1 << 20, 2 * nmax), scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity);
+    const i64 ccap = std::max<i64>(1 << 20, std::min<i64>(2 * nmax, nmax / 2 + ((i64)128 << 20))), scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity);
     const i64 ws_bytes = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nmax, 1), npass_max) + cand_bytes(ccap + n_total + 64, ppass_max) +
                          cand_bytes(scap, ppass_max) + 65536;
     const i64 out_bytes = 3 * align_up(capacity * 4 + 16);
@@ -697,7 +699,7 @@ int symdel_workspace_bytes(int64_t n_a, int64_t residues_a, int64_t n_b, int64_t
     const i64 n_total = n_a + n_b;
     const u64 vm = vcount_host(max_len, d);
     const i64 nbound = n_total + (max_len ? (i64)(((u64)(residues_a + residues_b) * (vm - 1) + max_len - 1) / max_len) : 0);
-    const i64 ccap = std::max<i64>(1 << 20, 2 * nbound), scap = std::max<i64>(std::max<i64>(1 << 20, nbound / 4), capacity);
+    const i64 ccap = std::max<i64>(1 << 20, std::min<i64>(2 * nbound, nbound / 2 + ((i64)128 << 20))), scap = std::max<i64>(std::max<i64>(1 << 20, nbound / 4), capacity);
     *bytes_host = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nbound, 1), 7) + cand_bytes(ccap + n_total + 64, 8) + cand_bytes(scap, 8) +
                   65536;
     return SYMDEL_OK;
