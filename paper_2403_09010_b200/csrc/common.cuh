@@ -60,27 +60,7 @@ __device__ __forceinline__ void sd_st_relaxed32(u32* p, u32 v) {
     asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// Called by ONE thread of the tile.  Returns the exclusive prefix of `aggregate` over tiles < tile.
-__device__ __forceinline__ u64 sd_lookback(u64* status, u32 tile, u64 aggregate) {
-    if (tile == 0) {
-        sd_st_relaxed(status, SD_LB_PRE | aggregate);
-        return 0;
-    }
-    sd_st_relaxed(status + tile, SD_LB_AGG | aggregate);
-    u64 excl = 0;
-    i64 p = (i64)tile - 1;
-    while (true) {
-        u64 s;
-        do { s = sd_ld_relaxed(status + p); } while ((s >> 62) == 0);
-        excl += s & SD_LB_MASK;
-        if ((s >> 62) == 2) break;
-        --p;
-    }
-    sd_st_relaxed(status + tile, SD_LB_PRE | (excl + aggregate));
-    return excl;
-}
-
-// Warp-parallel variant: called by all 32 lanes of ONE converged warp; inspects 32 predecessors per
+// Called by all 32 lanes of ONE converged warp; inspects 32 predecessors per
 // round trip (lane 0 = nearest), so the walk back to the closest inclusive prefix costs
 // ceil(depth / 32) L2 latencies instead of depth.  Returns the exclusive prefix to every lane.
 __device__ __forceinline__ u64 sd_lookback_warp(u64* status, u32 tile, u64 aggregate) {
@@ -139,33 +119,4 @@ __device__ __forceinline__ u32 sd_block_excl_sum(u32 v, u32* total, u32* s_warp 
     *total = s_warp[THREADS / 32];
     __syncthreads();  // s_warp may be reused by the caller
     return r;
-}
-
-// exclusive max-scan of signed positions (identity = -1)
-template <int THREADS>
-__device__ __forceinline__ i32 sd_block_excl_max(i32 v, i32* s_warp /* [THREADS/32] */) {
-    const u32 lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    i32 inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        i32 t = __shfl_up_sync(SD_FULL, inc, o);
-        if (lane >= o) inc = max(inc, t);
-    }
-    if (lane == 31) s_warp[warp] = inc;
-    __syncthreads();
-    i32 carry = -1;
-    for (u32 w = 0; w < warp; ++w) carry = max(carry, s_warp[w]);
-    i32 prev = __shfl_up_sync(SD_FULL, inc, 1);
-    if (lane == 0) prev = -1;
-    __syncthreads();
-    return max(carry, prev);
-}
-
-__device__ __forceinline__ u64 sd_mix64(u64 x) {  // bijective finaliser
-    x ^= x >> 32;
-    x *= 0xd6e8feb86659fd93ull;
-    x ^= x >> 32;
-    x *= 0xd6e8feb86659fd93ull;
-    x ^= x >> 32;
-    return x;
 }

@@ -53,6 +53,7 @@ __global__ void __launch_bounds__(256) k_hist_scan(u32* __restrict__ ghist) {
 #define OS_MATCH_OR 1
 #endif
 
+#if !OS_MATCH_OR
 // Peer mask of the lanes holding the same 8-bit digit, built from 8 ballots (the MATCH.ANY
 // instruction measured ~170 cycles per warp on sm_100a; 8 x (VOTE + LOP3) is ~10x cheaper).
 __device__ __forceinline__ u32 os_match8(u32 dg, u32 init) {
@@ -80,6 +81,7 @@ __device__ __forceinline__ u32 os_match8(u32 dg, u32 init) {
 #undef OS_MATCH_BIT
     return peers;
 }
+#endif
 
 // Shared tail of both tile paths: per-digit decoupled look-back, then the coalesced write-out of the
 // tile staged in digit order.  `total` / `tstart` (threads < 256): this tile's count and tile-local
