@@ -264,23 +264,17 @@ __device__ __forceinline__ void gen_walk(const GenShared& sh, u32 f, u32 fend, u
     }
 }
 
+// Leftmost-embedding rule on bit masks: D = the deleted positions; a deleted position p whose deleted run
+// p, p+1, .. has length exactly j meets its next KEPT position at p + j, and must satisfy NE[j-1] bit p
+// (s[p] != s[p + j], or p + j beyond the end).  k <= 4, so runs are at most 4 long.  Branch-free.
 __device__ __forceinline__ bool gen_canonical(const GenShared& sh, u32 g, int k, const int* p) {
-    bool ok = true;
+    u64 D = 0;
 #pragma unroll
-    for (int m = 0; m < 4; ++m) {
-        if (m < k) {
-            int j = 1;  // distance to the next KEPT position after p[m]
-            if (m + 1 < k && p[(m + 1) & 3] == p[m] + 1) {
-                j = 2;
-                if (m + 2 < k && p[(m + 2) & 3] == p[m] + 2) {
-                    j = 3;
-                    if (m + 3 < k && p[(m + 3) & 3] == p[m] + 3) j = 4;
-                }
-            }
-            ok = ok && ((sh.NE[g][j - 1] >> p[m]) & 1ull);
-        }
-    }
-    return ok;
+    for (int m = 0; m < 4; ++m)
+        if (m < k) D |= 1ull << p[m];
+    const u64 r2 = D & (D >> 1), r3 = r2 & (D >> 2), r4 = r3 & (D >> 3);
+    const u64 bad = ((D & ~r2) & ~sh.NE[g][0]) | ((r2 & ~r3) & ~sh.NE[g][1]) | ((r3 & ~r4) & ~sh.NE[g][2]) | (r4 & ~sh.NE[g][3]);
+    return bad == 0;
 }
 
 __device__ __forceinline__ u64 gen_hash(const GenShared& sh, u32 g, int k, const int* p) {
