@@ -862,7 +862,16 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
 // Fused general path (k_generate_part): the enumeration of k_generate (any d <= 4, any length <= 64)
 // with the staging / flushing of k_gen2_part.  One sweep per round instead of two: no counts, no scan,
 // no offsets — a canonical deletion set is hashed and pushed under its top 8 hash bits.
-constexpr int GQ_S = 16;           // stage slots per digit (a round makes at most GEN_THREADS * GEN_R = 2048 records)
+#ifndef GQ_S
+#define GQ_S 16  // stage slots per digit (16 or 32)
+#endif
+#ifndef GQ_R
+#define GQ_R 8   // consecutive deletion sets per thread and round: a round makes at most GEN_THREADS * GQ_R records
+#endif
+#ifndef GQ_MINB
+#define GQ_MINB 3
+#endif
+static_assert(GQ_S == 16 || GQ_S == 32, "flush copies 32 / GQ_S digits per warp instruction");
 #ifndef GQ_FLUSH_AT
 #define GQ_FLUSH_AT 900
 #endif
@@ -875,7 +884,7 @@ struct GenPartStage {
 };
 
 template <bool CHUNKED>
-__global__ void __launch_bounds__(GEN_THREADS, 3) k_generate_part(GenPartParams PP) {
+__global__ void __launch_bounds__(GEN_THREADS, GQ_MINB) k_generate_part(GenPartParams PP) {
     extern __shared__ __align__(16) unsigned char gen_smem[];
     GenShared& sh = *reinterpret_cast<GenShared*>(gen_smem);
     GenPartStage& ps = *reinterpret_cast<GenPartStage*>(gen_smem + ((sizeof(GenShared) + 15) & ~(size_t)15));
@@ -909,10 +918,11 @@ __global__ void __launch_bounds__(GEN_THREADS, 3) k_generate_part(GenPartParams 
             ps.fl[tid] = make_uint2(g, g == 0xffffffffu ? 0u : cn_);
         }
         __syncthreads();
-        // two digits per warp instruction: lanes 0-15 and 16-31
-        for (u32 dg = 2 * warp + (lane >> 4); dg < 256; dg += 2 * GEN_NW) {
+        // 32 / GQ_S digits per warp instruction (GQ_S = 16: lanes 0-15 and 16-31)
+        constexpr u32 DPW = 32 / GQ_S;
+        for (u32 dg = DPW * warp + lane / GQ_S; dg < 256; dg += DPW * GEN_NW) {
             const uint2 f = ps.fl[dg];
-            const u32 o = lane & 15u;
+            const u32 o = lane & (GQ_S - 1);
             if (o < f.y) PP.bins[f.x + o] = ps.stage[dg * GQ_S + ((o + dg) & (GQ_S - 1))];
         }
         __syncthreads();
@@ -971,8 +981,8 @@ __global__ void __launch_bounds__(GEN_THREADS, 3) k_generate_part(GenPartParams 
         __syncthreads();
 
         const u32 T = sh.vbase[ng];
-        for (u32 rb = 0; rb < T; rb += GEN_THREADS * GEN_R) {
-            const u32 f0 = min(T, rb + tid * GEN_R), f1 = min(T, f0 + GEN_R);
+        for (u32 rb = 0; rb < T; rb += GEN_THREADS * GQ_R) {
+            const u32 f0 = min(T, rb + tid * GQ_R), f1 = min(T, f0 + GQ_R);
             u32 made = 0;
             gen_walk(sh, f0, f1, ng, d, [&](u32 g, u32, int k, const int* p) {
                 if (!gen_canonical(sh, g, k, p)) return;
@@ -1196,7 +1206,7 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
         const bool plain = lay.hash_bits + lay.id_bits == 64 && lay.id_bits <= 31;
         kerns[(lay.n_chunks > 1 ? 2 : 0) + (plain ? 1 : 0)]<<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
     } else {
-        const int grid = (int)std::min<i64>(PP.g.groups_total, 148 * 3);
+        const int grid = (int)std::min<i64>(PP.g.groups_total, 148 * GQ_MINB);
         gkerns[lay.n_chunks > 1 ? 1 : 0]<<<grid, GEN_THREADS, gsm, st>>>(PP);
     }
     if (launches) ++*launches;
