@@ -311,8 +311,9 @@ restart:
         // ---- fused pipeline: generation + level-1 partition, level-2 partition, bucket join ----
         bool fused_ok = false;
         i64 C = 0, wend = 0, N = 0;
+        // (a chunk expected to hold 2^30 records or more goes to the exact pipeline, which splits it further)
         if (!ctx->opt_exact && ctx->opt_sort_bits < 0 && !ctx->opt_join_general && lay.hash_bits >= fp.b &&
-            sd_gen_part_applies(lay, width)) {
+            nmax / (i64)P < ((i64)1 << 30) && sd_gen_part_applies(lay, width)) {
             const size_t x0 = tm.mark();
             lay.sort_bits = fp.b;
             CK(cudaMemsetAsync(&info->part_overflow, 0, sizeof(u32), st));
