@@ -130,7 +130,13 @@ def run_reference(args):
     from paper_2403_09010_b200 import synth
 
     kind, d, (s,) = synth.config(3)
-    n_sample = min(s.n, args.ref_sample)
+    # bounded sample: unless --ref-sample fixes the size, a 10,000-sequence calibration run gives the oracle's cost per
+    # sequence on this box and the whole run (warm-up + steps) is sized to about two minutes
+    n_sample = args.ref_sample
+    if not n_sample:
+        _, t_cal = cpu_baseline_run(10000, d, s)
+        n_sample = int(min(150000, max(5000, 120.0 / max(1, args.warmup + args.steps) / (t_cal / 10000.0))))
+    n_sample = min(s.n, n_sample)
     times, pairs = [], 0
     for it in range(args.warmup + args.steps):
         pairs, dt = cpu_baseline_run(n_sample, d, s)
@@ -155,7 +161,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="symdel", choices=["symdel", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); the metric is quoted on 3")
-    ap.add_argument("--ref-sample", type=int, default=150000, help="sequences in the oracle's bounded sample")
+    ap.add_argument("--ref-sample", type=int, default=0,
+                    help="sequences in the oracle's bounded sample (0: 150,000 for cpu_baseline; for --impl reference sized "
+                         "so that warm-up + steps take about two minutes)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--dense", action="store_true",
                     help="NEXT-2 workload instead of config 3: synth.dense_set(1,000,000, seed 11, fanout 64), d=2 "
@@ -334,7 +342,7 @@ def main():
                 "share_of_step": stage["ms_generate"] / stage["ms_total"],
                 "hbm_gbs": (8 * n_rec + in_bytes) / (stage["ms_generate"] * 1e-3) / 1e9}
     if not args.no_cpu_baseline and world == 1 and not args.dense:
-        n_sample = min(s.n, args.ref_sample)
+        n_sample = min(s.n, args.ref_sample or 150000)
         pairs, dt = cpu_baseline_run(n_sample, d, s)
         line["cpu_baseline"] = {"value": pairs / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": f"same generator and seed at n={n_sample}, d={d}: {pairs} pairs in {dt:.1f} s "
