@@ -1,21 +1,24 @@
 // symdel_api.cu — the C ABI of include/symdel.h and the host-side pipeline (S0-S5).
 //
-// Pipeline of one call (App. F.3 "XTNeighbor base algorithm", re-designed):
-//   S0  prepare : validate CSR input, longest sequence, upper bound of the record count
-//   for each key-range chunk c of P (S5; P = 1 when the workspace allows):
-//     S1  count + scan + generate : (hash, id) records of the variants whose hash falls in chunk c
-//     S2  sort                    : onesweep LSD radix sort on the hash bits (stable: ids stay ascending)
-//     S3a emit                    : runs of equal hash -> candidate pairs, in windows of the candidate buffer
-//     for each window:
-//       S3b sort candidates; S4 unique + verify -> survivors (pair << 3 | dist), appended in order
-//   if more than one flush happened: sort survivors, unique
-//   unpack survivors -> (out_i, out_j, out_dist), ascending (i, j)
+// One call (App. F.3 "XTNeighbor base algorithm", re-designed):
+//   S0  prepare : validate CSR input, longest sequence, upper bound of the record count, pack for the verifier
+//   for each key-range chunk c of P (S5; P = 1 when the workspace allows), one of two pipelines:
+//     FUSED (default)                                        EXACT (options, or after an overflow)
+//     S1+S2 k_gen*_part : variants hashed and staged under   S1 count + scan + generate : records in id order
+//           their top 8 hash bits -> 256 fixed-capacity bins S2 onesweep passes on exact histograms (8 bits each)
+//     S2    k_part2     : next b2 bits -> fixed-capacity     S3a k_join_fast (one window) else k_join (windowed,
+//           buckets with counts                                  chunks oversized buckets)
+//     S3a   k_join_bkt  : shared-memory hash join per bucket
+//     then, per window of the candidate buffer:
+//       S3b sort the packed pair ids; S4 unique + verify -> survivors (pair << 3 | dist) appended in order,
+//           or straight into the outputs when the window is the only flush of the search
+//   if more than one flush happened: sort survivors, unique, unpack -> (out_i, out_j, out_dist), ascending (i, j)
 // Equal keys always land in the same chunk and a verified pair carries the same distance wherever it
 // was found, so chunking and windowing change memory use only.  This replaces the paper's 2-D-buffer
 // streaming (App. C; App. F.4) whose purpose — bounded memory — it serves.
 //
-// Host <-> device crossings per call: one pinned-memory read-back after S0, one per chunk after the
-// count scan (grid sizes), one after the first emit (candidate count), two at the end.
+// Host <-> device crossings per call (fused, one chunk, one window): one pinned-memory read-back after S0,
+// one after the join (candidate count, overflow flags), one at the end.
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
