@@ -194,8 +194,10 @@ __global__ void __launch_bounds__(128) k_count_dp(SeqSetDev A, SeqSetDev B, int 
     cnt[g] = total;
 }
 
-struct GenShared {
-    u64 U[GEN_G][SD_L_MAX];          // U[p] = A[p] - Binv * A[p + 1]
+// LW = residues per row of U: SD_L_MAX in general, 32 when the longest (truncated) sequence fits (half the shared memory)
+template <int LW>
+struct GenSharedT {
+    u64 U[GEN_G][LW];                // U[p] = A[p] - Binv * A[p + 1]
     u64 C[GEN_G][SD_D_MAX + 1];      // C[k] = Binv^k * A[L] + (L - k + 1) * K_LEN
     u64 NE[GEN_G][SD_D_MAX];         // NE[j-1] bit t: t + j >= L or s[t] != s[t + j]
     u64 R[32];
@@ -210,10 +212,11 @@ struct GenShared {
     u32 running;
     unsigned char seq[GEN_G][SEQ_STRIDE];
 };
+typedef GenSharedT<SD_L_MAX> GenShared;
 
 // Walks the deletion sets numbered [f, fend) of the group and calls fn(g, L, k, p) for each.
-template <typename Fn>
-__device__ __forceinline__ void gen_walk(const GenShared& sh, u32 f, u32 fend, u32 ng, int d, Fn&& fn) {
+template <typename SH, typename Fn>
+__device__ __forceinline__ void gen_walk(const SH& sh, u32 f, u32 fend, u32 ng, int d, Fn&& fn) {
     int p[4] = {0, 0, 0, 0};
     u32 g = 0, L = 0, left = 0;  // left = sets remaining in the current (sequence, k) class
     int k = 0;
@@ -267,7 +270,8 @@ __device__ __forceinline__ void gen_walk(const GenShared& sh, u32 f, u32 fend, u
 // Leftmost-embedding rule on bit masks: D = the deleted positions; a deleted position p whose deleted run
 // p, p+1, .. has length exactly j meets its next KEPT position at p + j, and must satisfy NE[j-1] bit p
 // (s[p] != s[p + j], or p + j beyond the end).  k <= 4, so runs are at most 4 long.  Branch-free.
-__device__ __forceinline__ bool gen_canonical(const GenShared& sh, u32 g, int k, const int* p) {
+template <typename SH>
+__device__ __forceinline__ bool gen_canonical(const SH& sh, u32 g, int k, const int* p) {
     u64 D = 0;
 #pragma unroll
     for (int m = 0; m < 4; ++m)
@@ -277,7 +281,8 @@ __device__ __forceinline__ bool gen_canonical(const GenShared& sh, u32 g, int k,
     return bad == 0;
 }
 
-__device__ __forceinline__ u64 gen_hash(const GenShared& sh, u32 g, int k, const int* p) {
+template <typename SH>
+__device__ __forceinline__ u64 gen_hash(const SH& sh, u32 g, int k, const int* p) {
     u64 h = sh.C[g][k];
     if (k > 0) h += sh.U[g][p[0]];
     if (k > 1) h += c_Binv[1] * sh.U[g][p[1]];
@@ -883,11 +888,12 @@ struct GenPartStage {
     u32 total[3];  // as in GenPartShared
 };
 
-template <bool CHUNKED>
-__global__ void __launch_bounds__(GEN_THREADS, GQ_MINB) k_generate_part(GenPartParams PP) {
+template <bool CHUNKED, int LW>
+__global__ void __launch_bounds__(GEN_THREADS, LW <= 32 ? GQ_MINB + 1 : GQ_MINB) k_generate_part(GenPartParams PP) {
+    typedef GenSharedT<LW> SH;
     extern __shared__ __align__(16) unsigned char gen_smem[];
-    GenShared& sh = *reinterpret_cast<GenShared*>(gen_smem);
-    GenPartStage& ps = *reinterpret_cast<GenPartStage*>(gen_smem + ((sizeof(GenShared) + 15) & ~(size_t)15));
+    SH& sh = *reinterpret_cast<SH*>(gen_smem);
+    GenPartStage& ps = *reinterpret_cast<GenPartStage*>(gen_smem + ((sizeof(SH) + 15) & ~(size_t)15));
     const GenParams& P = PP.g;
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     for (int i = tid; i < (SD_L_MAX + 1) * (SD_D_MAX + 1); i += GEN_THREADS) sh.binom[i] = c_binom[i];
@@ -1189,15 +1195,16 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     }
     typedef void (*Kern)(GenPartParams);
     static const Kern kerns[4] = {k_gen2_part<false, false>, k_gen2_part<false, true>, k_gen2_part<true, false>, k_gen2_part<true, true>};
-    static const Kern gkerns[2] = {k_generate_part<false>, k_generate_part<true>};
-    constexpr size_t gsm = ((sizeof(GenShared) + 15) & ~(size_t)15) + sizeof(GenPartStage);
+    static const Kern gkerns[4] = {k_generate_part<false, SD_L_MAX>, k_generate_part<true, SD_L_MAX>, k_generate_part<false, 32>, k_generate_part<true, 32>};
+    constexpr size_t gsm64 = ((sizeof(GenSharedT<SD_L_MAX>) + 15) & ~(size_t)15) + sizeof(GenPartStage);
+    constexpr size_t gsm32 = ((sizeof(GenSharedT<32>) + 15) & ~(size_t)15) + sizeof(GenPartStage);
     static bool attr_set = false;
     cudaError_t e;
     if (!attr_set) {
         for (Kern k : kerns)
             if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GenPartShared))) != cudaSuccess) return e;
-        for (Kern k : gkerns)
-            if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsm)) != cudaSuccess) return e;
+        for (int i = 0; i < 4; ++i)
+            if ((e = cudaFuncSetAttribute(gkerns[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(i < 2 ? gsm64 : gsm32))) != cudaSuccess) return e;
         attr_set = true;
     }
     if ((e = cudaMemsetAsync(cur, 0, 256 * sizeof(u32), st)) != cudaSuccess) return e;
@@ -1206,8 +1213,9 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
         const bool plain = lay.hash_bits + lay.id_bits == 64 && lay.id_bits <= 31;
         kerns[(lay.n_chunks > 1 ? 2 : 0) + (plain ? 1 : 0)]<<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
     } else {
-        const int grid = (int)std::min<i64>(PP.g.groups_total, 148 * GQ_MINB);
-        gkerns[lay.n_chunks > 1 ? 1 : 0]<<<grid, GEN_THREADS, gsm, st>>>(PP);
+        const bool narrow = width - 1 <= 32;  // rows of 32 residues: a fourth block fits on the SM
+        const int grid = (int)std::min<i64>(PP.g.groups_total, 148 * (narrow ? GQ_MINB + 1 : GQ_MINB));
+        gkerns[(narrow ? 2 : 0) + (lay.n_chunks > 1 ? 1 : 0)]<<<grid, GEN_THREADS, narrow ? gsm32 : gsm64, st>>>(PP);
     }
     if (launches) ++*launches;
     return cudaGetLastError();
