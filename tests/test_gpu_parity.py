@@ -467,6 +467,25 @@ def test_long_sequences_up_to_the_limits(sd, oracle, d, opts):
     assert_same(run_self(sd, c, s, d), exp)
 
 
+@pytest.mark.parametrize("family,d", [("tcr", 2), ("bcr", 3), ("dense", 1)])
+def test_pipelines_agree_on_stage_counters(sd, family, d):
+    """The fused and the exact pipeline use the same hash and the same thinning rule: beyond the identical output,
+    the number of records, of candidate pairs and of unique candidates must coincide (they are unpinned against
+    the paper, but pinned against each other)."""
+    s = {"tcr": lambda: synth.tcr_set(8000, 97), "bcr": lambda: synth.bcr_set(3000, 98, n_lineages=300),
+         "dense": lambda: synth.dense_set(8000, 99)}[family]()
+    stats, outs = [], []
+    for exact in (0, 1):
+        c = sd.Context(0)
+        c.symdel_set_option(sd.OPT_EXACT_PIPELINE, exact)
+        outs.append(run_self(sd, c, s, d))
+        stats.append(c.symdel_get_stats())
+    assert_same(outs[0], outs[1])
+    assert stats[0]["fused_chunks"] == 1 and stats[1]["fused_chunks"] == 0
+    for k in ("n_records", "n_candidates", "n_unique", "n_outputs"):
+        assert stats[0][k] == stats[1][k], k
+
+
 def test_small_workspace_forces_chunking(torch, sd, ctx, oracle):
     s = synth.tcr_set(20000, 22)
     exp = oracle.symdel_self(s.seqs, s.offsets, 2)
