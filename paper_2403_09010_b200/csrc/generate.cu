@@ -642,6 +642,12 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
 #ifndef GP_MINB
 #define GP_MINB 3
 #endif
+#ifndef GP_OVF
+#define GP_OVF 128
+#endif
+#ifndef GP_TRIP
+#define GP_TRIP 16  // d = 3: (g1, g2) iterations per step of a batch
+#endif
 #ifndef GP_ROUND
 #define GP_ROUND 5400  // records a block stages per round (21 per digit of the 32 slots); the host turns it into batches per warp
 #endif
@@ -657,6 +663,8 @@ struct GenPartShared {
     u32 cnt[256];     // records staged per digit since the last flush (may exceed GP_S: the excess went to the bins directly)
     uint2 fl[256];    // flush: {index of the claimed segment in bins (0xffffffff = bin full), records to copy}
     u32 total[3];     // records staged in round r go to total[r % 3] (three words: a fast warp of round r + 1 never touches the word the slow warps of round r still read)
+    u32 novf;         // records in ovf[] (may count past GP_OVF: those went to the bins directly)
+    u64 ovf[GP_OVF];  // records whose digit had no free slot: placed at the next flush (near-identical neighbouring sequences — clonal lineages — push the same digits in bursts)
     unsigned char map[GP_NW][32];
 };
 
@@ -670,7 +678,14 @@ struct GenPartParams {
     u32 batches;  // k_gen2_part: batches per warp and round
 };
 
-template <bool CHUNKED, bool PLAIN>
+// D3 (d == 3): the triples {p1 < p2 < p3} follow the pairs.  A triple is the three points a, a + g1, a + g1 + g2
+// on the circle of L positions with gaps (g1, g2, g3 = L - g1 - g2); of its three starting points exactly one is
+// kept: the one whose LAST gap is the largest (g3 > g1 and g3 >= g2; all gaps equal: a < g1) — so every lane of a
+// sequence enumerates the same (g1, g2) and the work is balanced.  H = U[p1] + V[p2] + Binv * V[p3] + C3.  The
+// leftmost-embedding rule is the bit-mask test of gen_canonical on segment-relative masks.  A batch then makes
+// thousands of records, so it is RESUMABLE: step 0 = everything up to the pairs, step g1 = the triples of that
+// first gap; the block's flush decision falls between steps.
+template <bool CHUNKED, bool PLAIN, bool D3>
 __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams PP) {
     extern __shared__ __align__(16) unsigned char gen_smem[];
     GenPartShared& sh = *reinterpret_cast<GenPartShared*>(gen_smem);
@@ -680,6 +695,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     if (tid < 33) sh.Bpow[tid] = c_Bpow[tid];
     if (tid < 256) sh.cnt[tid] = 0;
     if (tid < 3) sh.total[tid] = 0;
+    if (tid == 0) sh.novf = 0;
     __syncthreads();
     const int d = P.d;
     const bool thinning = P.thinning != 0;
@@ -703,9 +719,14 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
             if (r < (u32)GP_S) {
                 sh.stage[dg * GP_S + ((r + dg) & (GP_S - 1))] = rec;
             } else {
-                const u32 at = atomicAdd(&PP.cur[dg], 1u);
-                if (at < PP.cap1) PP.bins[(u64)dg * PP.cap1 + at] = rec;
-                else atomicOr(&P.info->part_overflow, 1u);
+                const u32 o = atomicAdd(&sh.novf, 1u);
+                if (o < (u32)GP_OVF) {
+                    sh.ovf[o] = rec;
+                } else {
+                    const u32 at = atomicAdd(&PP.cur[dg], 1u);
+                    if (at < PP.cap1) PP.bins[(u64)dg * PP.cap1 + at] = rec;
+                    else atomicOr(&P.info->part_overflow, 1u);
+                }
             }
             ++made;
         }
@@ -713,7 +734,9 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
 
     // warp task = 32 consecutive sequences of one set, cut into batches that fill the 32 lanes; the block
     // advances one batch per warp and round, then decides about flushing
-    i64 wt = (i64)blockIdx.x * GP_NW + warp;
+    // (the warps of a block take tasks far apart in the input: neighbouring sequences are often near-identical —
+    // clonal lineages — and would all push the same digits at the same time)
+    i64 wt = (i64)warp * gridDim.x + blockIdx.x;
     const i64 wstride = (i64)gridDim.x * GP_NW;
     bool have = false;  // a task is loaded and has batches left
     u32 rnd = 0, staged = 0;  // round index mod 3; records staged since the last flush (block-uniform)
@@ -721,6 +744,9 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     u64 gid0 = 0;
     i64 o0 = 0;  // lane as sequence index: offset of its residues
     const int8_t* seqs = nullptr;
+    // D3: the state of a batch between its steps
+    u32 step = 0, t_g2 = 1, t_a = 0, t_L = 0, t_seg = 0, t_e = 0, t_g1max = 0, t_ne1 = 0, t_ne2 = 0, t_ne3 = 0, t_Lmax = 0;
+    u64 t_gid = 0, t_C3 = 0;
     while (true) {
 #pragma unroll 1
         for (u32 rep = 0; rep < PP.batches; ++rep) {  // the same trip count in every warp: rounds stay balanced
@@ -748,7 +774,47 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
             have = true;
             wt += wstride;
         }
-        if (have) {
+        if (D3 && have && step > 0) {
+            // ---- one step of a batch's triples: GP_TRIP (g1, g2) iterations from where the last step stopped, so
+            //      that a step costs every warp the same whatever its sequence lengths ----
+            const u32 a = t_a, L = t_L;
+            const u32 uv_sa = (u32)__cvta_generic_to_shared(Uw + t_seg);
+            for (u32 it = 0; it < (u32)GP_TRIP && step <= t_g1max; ++it) {
+                const u32 g1 = step, g2 = t_g2;
+                const u32 g2hi = min((t_Lmax - g1) >> 1, t_Lmax - 2 * g1);  // g3 >= g2 and g3 > g1 (or all equal) at the longest length
+                const u32 g3 = L - g1 - g2;  // meaningless (huge) where g1 + g2 >= L: `ok` is false there
+                const bool ok = g1 + g2 < L && ((g3 > g1 && g3 >= g2) || (g1 == g2 && g2 == g3 && a < g1));
+                u32 y = a + g1, z = y + g2;
+                const bool wy = y >= L, wz = z >= L;
+                y = (wy ? y - L : y) & 31u;
+                z = (wz ? z - L : z) & 31u;
+                // sorted positions: no wrap (a, y, z); z wrapped (z, a, y); both wrapped (y, z, a)
+                const u32 p1 = wy ? y : (wz ? z : a), p2 = wy ? z : (wz ? a : y), p3 = wy ? a : (wz ? y : z);
+                const u32 D = (1u << a) | (1u << y) | (1u << z);
+                const u32 r2 = D & (D >> 1), r3 = r2 & (D >> 2);
+                const u32 bad = ((D & ~r2) & ~t_ne1) | ((r2 & ~r3) & ~t_ne2) | (r3 & ~t_ne3);
+                u64 u1, v2, v3;
+                asm volatile("ld.shared.u64 %0, [%1];" : "=l"(u1) : "r"(uv_sa + p1 * 8u));
+                asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v2) : "r"(uv_sa + p2 * 8u + (u32)(GP_NW * 256)));
+                asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v3) : "r"(uv_sa + p3 * 8u + (u32)(GP_NW * 256)));
+                push(g2 <= g2hi && ok && bad == 0, u1 + v2 + binv1 * v3 + t_C3, t_gid);
+                if (g2 >= g2hi) {
+                    ++step;
+                    t_g2 = 1;
+                } else {
+                    ++t_g2;
+                }
+            }
+            if (step > t_g1max) {
+                step = 0;
+                __syncwarp();  // U/V/map are reused by the next batch
+                s = t_e;
+                have = s < ns;
+            }
+            const u32 wmade = __reduce_add_sync(SD_FULL, made);
+            made = 0;
+            if (lane == 0 && wmade) atomicAdd(&sh.total[rnd], wmade);
+        } else if (have) {
             // ---- one batch: sequences [s, e) of the task ----
             const u32 base = __shfl_sync(SD_FULL, cum_excl, s);
             const u32 fit = __ballot_sync(SD_FULL, lane >= s && lane < ns && (cum_incl - base) <= 32u);
@@ -819,10 +885,24 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                         push(dl <= dlmax && c1a && ((m1s >> (b & 31u)) & 1u), o + (wrap ? VC : UC), gid);
                     }
                 }
-                __syncwarp();  // U/V/map are reused by the next batch
+                if (D3) {  // the triples follow, one first gap per step
+                    const u32 cnnn = __shfl_down_sync(SD_FULL, c, 3);
+                    const bool ne2 = active && (!thinning || !has2 || c != cnn);
+                    const bool ne3 = active && (!thinning || !(a + 3 < L) || c != cnnn);
+                    const u32 b2 = __ballot_sync(SD_FULL, ne2), b3 = __ballot_sync(SD_FULL, ne3);
+                    t_Lmax = __reduce_max_sync(SD_FULL, L);
+                    t_g1max = t_Lmax >= 3 ? (t_Lmax - 1) >> 1 : 0;
+                    t_a = a, t_L = L, t_seg = seg_start, t_e = e, t_gid = gid;
+                    t_ne1 = m1 >> seg_start, t_ne2 = b2 >> seg_start, t_ne3 = b3 >> seg_start;
+                    t_C3 = binv1 * binv2 * AL + (u64)(L - 2) * K_LEN;
+                    if (t_g1max > 0) step = 1, t_g2 = 1;
+                }
+                if (!D3 || step == 0) __syncwarp();  // U/V/map are reused by the next batch
             }
-            s = e;
-            have = s < ns;
+            if (!D3 || step == 0) {
+                s = e;
+                have = s < ns;
+            }
             const u32 wmade = __reduce_add_sync(SD_FULL, made);
             made = 0;
             if (lane == 0 && wmade) atomicAdd(&sh.total[rnd], wmade);
@@ -854,8 +934,16 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                 const uint2 f = sh.fl[dg];
                 if (lane < f.y) PP.bins[f.x + lane] = sh.stage[dg * GP_S + ((lane + dg) & (GP_S - 1))];
             }
+            for (u32 i = tid; i < min(sh.novf, (u32)GP_OVF); i += GP_THREADS) {  // the overflow records, one global atomic each
+                const u64 rec = sh.ovf[i];
+                const u32 dg = (u32)(rec >> (P.id_bits + P.hash_bits - 8)) & 255u;
+                const u32 at = atomicAdd(&PP.cur[dg], 1u);
+                if (at < PP.cap1) PP.bins[(u64)dg * PP.cap1 + at] = rec;
+                else atomicOr(&P.info->part_overflow, 1u);
+            }
             __syncthreads();
             if (tid < 256) sh.cnt[tid] = 0;
+            if (tid == 0) sh.novf = 0;
             staged = 0;
             __syncthreads();
         }
@@ -1061,6 +1149,8 @@ GenParams make_params(SeqSetDev a, SeqSetDev b, const Layout& lay, int width) {
 int gen_grid(i64 groups) { return (int)std::min<i64>(groups, 148 * 6); }
 
 bool use_fast(const Layout& lay, int width) { return lay.d <= 2 && width - 1 <= 32 && !lay.force_general; }
+// the fused lane-per-position generator also does d = 3
+bool use_fast_part(const Layout& lay, int width) { return lay.d <= 3 && width - 1 <= 32 && !lay.force_general; }
 
 GenParams make_params2(SeqSetDev a, SeqSetDev b, const Layout& lay, int width) {
     GenParams P = make_params(a, b, lay, width);
@@ -1180,8 +1270,8 @@ bool sd_gen_part_applies(const Layout& lay, int width) {
 }
 
 cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1,
-                        double records_per_residue, DevInfo* info, cudaStream_t st, i64* launches) {
-    const bool fast = use_fast(lay, width);
+                        double records_per_residue, double avg_len, DevInfo* info, cudaStream_t st, i64* launches) {
+    const bool fast = use_fast_part(lay, width);
     GenPartParams PP{};
     PP.g = fast ? make_params2(a, b, lay, width) : make_params(a, b, lay, width);
     if (PP.g.groups_total == 0) return cudaSuccess;
@@ -1190,11 +1280,15 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     PP.cur = cur;
     PP.cap1 = (u32)cap1;
     {   // a batch fills the 32 lanes with residues: about 32 * records_per_residue records (thinning and padding: ~0.85)
-        const double per_round = GP_NW * 32.0 * std::max(records_per_residue, 0.03) * 0.85;
+        // d = 3: the unit of a round is a step of GP_TRIP triple iterations (about 0.55 of the lane slots make a record)
+        (void)avg_len;
+        const double per_round = lay.d == 3 ? GP_NW * 32.0 * GP_TRIP * 0.55 : GP_NW * 32.0 * std::max(records_per_residue, 0.03) * 0.85;
         PP.batches = (u32)std::min(8.0, std::max(1.0, std::floor(GP_ROUND / per_round + 0.5)));
     }
     typedef void (*Kern)(GenPartParams);
-    static const Kern kerns[4] = {k_gen2_part<false, false>, k_gen2_part<false, true>, k_gen2_part<true, false>, k_gen2_part<true, true>};
+    static const Kern kerns[8] = {k_gen2_part<false, false, false>, k_gen2_part<false, true, false>, k_gen2_part<true, false, false>,
+                                  k_gen2_part<true, true, false>,  k_gen2_part<false, false, true>, k_gen2_part<false, true, true>,
+                                  k_gen2_part<true, false, true>,  k_gen2_part<true, true, true>};
     static const Kern gkerns[4] = {k_generate_part<false, SD_L_MAX>, k_generate_part<true, SD_L_MAX>, k_generate_part<false, 32>, k_generate_part<true, 32>};
     constexpr size_t gsm64 = ((sizeof(GenSharedT<SD_L_MAX>) + 15) & ~(size_t)15) + sizeof(GenPartStage);
     constexpr size_t gsm32 = ((sizeof(GenSharedT<32>) + 15) & ~(size_t)15) + sizeof(GenPartStage);
@@ -1211,7 +1305,7 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     if (fast) {
         const int grid = (int)std::min<i64>((PP.g.groups_total + GP_NW - 1) / GP_NW, 148 * GP_MINB);
         const bool plain = lay.hash_bits + lay.id_bits == 64 && lay.id_bits <= 31;
-        kerns[(lay.n_chunks > 1 ? 2 : 0) + (plain ? 1 : 0)]<<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
+        kerns[(lay.d == 3 ? 4 : 0) + (lay.n_chunks > 1 ? 2 : 0) + (plain ? 1 : 0)]<<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
     } else {
         const bool narrow = width - 1 <= 32;  // rows of 32 residues: a fourth block fits on the SM
         const int grid = (int)std::min<i64>(PP.g.groups_total, 148 * (narrow ? GQ_MINB + 1 : GQ_MINB));

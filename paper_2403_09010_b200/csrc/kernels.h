@@ -70,7 +70,7 @@ cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
 bool sd_gen_part_applies(const Layout& lay, int width);
 // records_per_residue = (deletion sets of this chunk) / (residues): sizes the generation rounds
 cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1,
-                        double records_per_residue, DevInfo* info, cudaStream_t st, i64* launches);
+                        double records_per_residue, double avg_len, DevInfo* info, cudaStream_t st, i64* launches);
 
 // ---- join.cu ------------------------------------------------------------------------------------
 i64 sd_join_tiles(i64 n_records);

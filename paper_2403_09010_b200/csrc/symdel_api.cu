@@ -320,8 +320,8 @@ restart:
             const size_t x0 = tm.mark();
             lay.sort_bits = fp.b;
             CK(cudaMemsetAsync(&info->part_overflow, 0, sizeof(u32), st));
-            CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, (double)nmax / (double)std::max<i64>(residues, 1) / (double)P, info,
-                           st, &S.n_launches));
+            CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, (double)nmax / (double)std::max<i64>(residues, 1) / (double)P,
+                           (double)residues / (double)n_total, info, st, &S.n_launches));
             const size_t x1 = tm.mark();
             if (fp.b2)
                 CK(sd_part2(recA, cur1, fp.cap1, recB, cnt2, fp.cap2, fp.b2, lay.id_bits + lay.hash_bits - fp.b, info, st,
