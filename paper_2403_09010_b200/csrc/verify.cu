@@ -119,7 +119,10 @@ __device__ __forceinline__ int hamming_planes(const Planes<W>& P, const Planes<W
     return sizeof(W) == 8 ? __popcll((unsigned long long)x) : __popc((unsigned)x);
 }
 
-constexpr int VF_THREADS = 256, VF_IPT = 4, VF_TILE = VF_THREADS * VF_IPT;
+#ifndef VF_IPT_
+#define VF_IPT_ 8
+#endif
+constexpr int VF_THREADS = 256, VF_IPT = VF_IPT_, VF_TILE = VF_THREADS * VF_IPT;
 
 // Tile of 1024 sorted candidates: (1) flag the unique ones and compact their positions into shared
 // memory, (2) spread the COMPACTED list over the threads for the distance computation (after dedup
