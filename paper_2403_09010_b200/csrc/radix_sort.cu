@@ -328,7 +328,13 @@ __global__ void __launch_bounds__(THREADS, MINB) k_onesweep(const u64* __restric
 // — without histograms, tickets or look-back, because nothing downstream needs the records of a bucket
 // contiguous with the next bucket or in any order.  A bucket that would overflow raises
 // info->part_overflow (the host falls back to the exact pipeline).
-constexpr int P2_THREADS = 256, P2_IPT = 16, P2_TILE = P2_THREADS * P2_IPT;
+#ifndef P2_IPT_
+#define P2_IPT_ 16
+#endif
+#ifndef P2_MINB
+#define P2_MINB 4
+#endif
+constexpr int P2_THREADS = 256, P2_IPT = P2_IPT_, P2_TILE = P2_THREADS * P2_IPT;
 
 struct Part2Params {
     const u64* bins;
@@ -342,7 +348,7 @@ struct Part2Params {
     DevInfo* info;
 };
 
-__global__ void __launch_bounds__(P2_THREADS, 4) k_part2(const Part2Params P) {
+__global__ void __launch_bounds__(P2_THREADS, P2_MINB) k_part2(const Part2Params P) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     u64* skeys = reinterpret_cast<u64*>(smem_raw);
     __shared__ u32 bhist[256];
