@@ -41,7 +41,10 @@ namespace {
 constexpr int JN_THREADS = 512, JN_NW = JN_THREADS / 32, JN_T = 4096, JN_CAP = 6144;
 constexpr int JN_IT = JN_CAP / JN_THREADS;                     // strided iterations that cover a full window
 constexpr int JN_SLOT_BITS = 12, JN_SLOTS = 1 << JN_SLOT_BITS;  // chain heads
-constexpr int JN_BM_BITS = 16, JN_BM_WORDS = (1 << JN_BM_BITS) / 32;
+#ifndef JBM_BITS
+#define JBM_BITS 16  // filter bitmap: 2^JBM_BITS bits each ("seen", "seen twice")
+#endif
+constexpr int JN_BM_BITS = JBM_BITS, JN_BM_WORDS = (1 << JN_BM_BITS) / 32;
 constexpr u32 JN_NIL = 0xffffu, JN_NONE = 0xffffffffu;
 static_assert(JN_CAP < 0xffff && JN_CAP % JN_THREADS == 0 && JN_IT <= 32, "node index / nzmask width");
 
@@ -363,7 +366,7 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
 #define JF_THREADS_ 512
 #endif
 constexpr int JF_THREADS = JF_THREADS_, JF_NW = JF_THREADS / 32;
-constexpr int JF_BM_BITS = 16, JF_BM_WORDS = (1 << JF_BM_BITS) / 32;
+constexpr int JF_BM_BITS = JBM_BITS, JF_BM_WORDS = (1 << JF_BM_BITS) / 32;
 
 template <int LMAX, int SLOT_BITS>
 struct JoinFastSmem {
