@@ -26,6 +26,15 @@
  * across the ABI.  On error the outputs are unspecified unless stated.  All calls are synchronous
  * with respect to the result: when they return, outputs and *n_pairs_host are final.
  * There is no CPU fallback: without a CUDA device every compute entry point fails with SYMDEL_E_CUDA.
+ *
+ * Devices and threads.  A context belongs to the device given to symdel_create: every call through it selects
+ * that device (cudaSetDevice) and expects device pointers and the stream of that device.  All per-device state
+ * of the library (constant hash tables, kernel attributes) is set up by symdel_create for the context's own
+ * device, so contexts on several GPUs can coexist in one process.  A context is NOT re-entrant: at most one host
+ * thread may be inside a call on a given context at any time (it owns one pinned status block, one stats
+ * record and, for the *_host calls, one arena).  Different contexts — on the same or on different devices — may
+ * be used from different host threads concurrently; symdel_create / symdel_destroy may be called concurrently.
+ * symdel_strerror and symdel_workspace_bytes are pure functions.
  */
 #ifndef SYMDEL_H
 #define SYMDEL_H
@@ -53,7 +62,9 @@ enum {
     SYMDEL_E_RESIDUE = -4,   /* residue code outside 1..31 */
     SYMDEL_E_TOO_MANY = -5,  /* n_a + n_b >= 2^30 */
     SYMDEL_E_WORKSPACE = -6, /* workspace too small even at maximum chunking */
-    SYMDEL_E_CAPACITY = -7,  /* more result pairs than `capacity`: *n_pairs_host = required count, the first `capacity` pairs are valid */
+    SYMDEL_E_CAPACITY = -7,  /* more result pairs than `capacity`: the first `capacity` pairs (ascending) are valid; *n_pairs_host = the required
+                                count — exact, except when a chunked / windowed search had to cut its survivor list (stats.surv_merges > 0
+                                and the list exceeded `capacity`): then a lower bound of it, still > capacity */
     SYMDEL_E_CUDA = -8,      /* CUDA error (sticky); code via symdel_last_cuda_error */
     SYMDEL_E_INTERNAL = -9   /* internal consistency check failed (never expected) */
 };
@@ -79,6 +90,7 @@ typedef struct {
     int64_t sort_pass_records; /* records moved by one such pass */
     int64_t fused_chunks;      /* chunks that went through the fused pipeline (generation + partition in one kernel, bucket join) */
     int64_t join_redo_tiles;   /* join tiles that overflowed the small candidate list and were redone by the large-list kernel */
+    int64_t surv_merges;       /* multi-flush searches: times the survivor list was sorted and deduplicated to make room */
 } symdel_stats;
 
 /* Options (symdel_set_option); defaults in brackets. */
@@ -89,13 +101,14 @@ enum {
     SYMDEL_OPT_HASH_BITS = 4,     /* [0] 0 = every bit the id leaves free; else 1..63: hash bits kept per record (test hook: a narrow hash makes colliding variants, the result is unchanged) */
     SYMDEL_OPT_NO_THINNING = 5,   /* [0] 1: emit one record per deletion SET instead of per distinct variant (test hook) */
     SYMDEL_OPT_GENERAL_GENERATE = 7, /* [0] 1: use the general (any d, any length) generation kernel even where the d <= 2 fast path applies (test hook) */
-    SYMDEL_OPT_SORT_VARIANT = 6,  /* [0] tile shape of the onesweep kernel (process-wide tuning hook; results are identical) */
+    SYMDEL_OPT_SORT_VARIANT = 6,  /* [0] 0..3: tile shape of the onesweep kernel used by this context (test hook: other tile geometries; results are identical) */
     SYMDEL_OPT_SORT_BITS = 8,     /* [0] 0 = automatic; 8..56 (multiple of 8): top hash bits that S2 radix-partitions; 255 = none (one bucket: the join chunks it) */
     SYMDEL_OPT_SORT_STABLE = 9,   /* [0] 1: every S2 pass takes the stable (ties keep input order) tile path (test hook; results are identical) */
     SYMDEL_OPT_JOIN_GENERAL = 11, /* [0] 1: always run the general join kernel (windowed output, chunked buckets) instead of trying the fast one first (test hook; results are identical) */
     SYMDEL_OPT_EXACT_PIPELINE = 12, /* [0] 1: never use the fused pipeline (fixed-capacity bins); always count, scan, generate, onesweep-partition on exact histograms, windowed join (the path the fused one falls back to when a bin overflows; results are identical) */
     SYMDEL_OPT_PREFIX_LEN = 13,   /* [0] P > 0: prefix-truncated candidate generation (App. B; XTNeighbor uses 18): deletion variants are generated from the first P residues of every sequence, verification stays on the whole sequences.  Exact for P > d (calls with P <= d return SYMDEL_E_ARG); fewer records, more candidates */
     SYMDEL_OPT_METRIC = 14,       /* [0] 0: Levenshtein distance (the paper's metric).  1: Hamming distance (Fig. S3 A/C): only pairs of EQUAL length with <= d mismatching positions are returned, dist = the mismatch count; candidates come from the same deletion-variant join (hamming <= d implies lev <= d) */
+    SYMDEL_OPT_SURV_CAPACITY = 15, /* [0] >0: size of the survivor list of multi-flush searches in pairs (test hook; never below capacity + one candidate window) */
     SYMDEL_OPT_SORT_GROUPING = 10 /* [0] 1: symdel_stage_sort_u64 sorts keys only: ties land in arbitrary order (the mode the pipeline uses) */
 };
 
@@ -144,11 +157,14 @@ SYMDEL_API int symdel_cross_host(symdel_ctx* ctx, const int8_t* q_seqs_host, con
  * the sequence behind first / second pair component (device; the same array for a self-search);
  * matrix: device int64[M * M], row-major, OVERWRITTEN: matrix[p][q] = #pairs with labels (p, q).  symmetric = 1
  * (self-search, reading A-18): a pair with labels p != q also counts in [q][p]; within-repertoire pairs count once
- * on the diagonal.  workspace: >= 256 device bytes.  Synchronises the stream.  SYMDEL_E_ARG if a label is out of
- * range (the matrix is then unspecified) or n_repertoires is outside 1..4096. */
+ * on the diagonal.  n_labels_i / n_labels_j: lengths of the label arrays (= the sizes of the searched sets).
+ * workspace: >= 256 device bytes.  Synchronises the stream.  SYMDEL_E_ARG if a pair index lies outside its label
+ * array or a label outside [0, n_repertoires) (the matrix is then unspecified; nothing is read out of bounds), or
+ * if n_repertoires is outside 1..4096. */
 SYMDEL_API int symdel_overlap_matrix(symdel_ctx* ctx, const int32_t* out_i, const int32_t* out_j, int64_t n_pairs,
-                          const int32_t* labels_i, const int32_t* labels_j, int n_repertoires, int symmetric,
-                          int64_t* matrix, void* workspace, int64_t workspace_bytes, void* cuda_stream);
+                          const int32_t* labels_i, int64_t n_labels_i, const int32_t* labels_j, int64_t n_labels_j,
+                          int n_repertoires, int symmetric, int64_t* matrix, void* workspace, int64_t workspace_bytes,
+                          void* cuda_stream);
 
 /* ---- stage-level entry points (kernel parity tests and micro-benchmarks) ---------------------
  * S2/K2: stable LSD radix sort of n 64-bit keys on bits [begin_bit, end_bit) (end - begin a
@@ -166,7 +182,8 @@ SYMDEL_API int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const 
                           int64_t* n_records_host, void* workspace, int64_t workspace_bytes, void* cuda_stream);
 
 /* S4/K6: dist[t] = lev(a_{ia[t]}, b_{ib[t]}) by the bit-parallel verifier, for n_pairs index pairs.
- *   workspace: device scratch of at least 512 + 48 * (n_a + n_b) bytes (the packed bit-plane table). */
+ *   workspace: device scratch of at least 512 + 48 * (n_a + n_b) bytes (the packed bit-plane table).
+ *   An index outside [0, n_a) / [0, n_b) gives dist[t] = -1 and the call returns SYMDEL_E_ARG. */
 SYMDEL_API int symdel_stage_lev(symdel_ctx* ctx, const int8_t* a_seqs, const int64_t* a_offsets, int64_t n_a,
                      const int8_t* b_seqs, const int64_t* b_offsets, int64_t n_b, const int32_t* ia,
                      const int32_t* ib, int64_t n_pairs, int32_t* dist, void* workspace, int64_t workspace_bytes,

@@ -1,7 +1,6 @@
 """Builds libsymdel.so in-tree with nvcc for sm_100a (no JIT cache, no torch extension)."""
 from __future__ import annotations
 
-import os
 import shutil
 import subprocess
 from pathlib import Path
@@ -26,8 +25,7 @@ def build_native(force: bool = False, verbose: bool = False) -> Path:
     if not force and not needs_build():
         return SO
     nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
-    extra = os.environ.get("SYMDEL_NVCC_EXTRA", "").split()  # tuning hook: e.g. -DJF_IT=8
-    cmd = [nvcc, *NVCC_FLAGS, *extra, "-shared", *[str(CSRC / s) for s in SOURCES], "-o", str(SO)]
+    cmd = [nvcc, *NVCC_FLAGS, "-shared", *[str(CSRC / s) for s in SOURCES], "-o", str(SO)]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.run(cmd, check=True)

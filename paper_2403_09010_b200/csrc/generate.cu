@@ -6,8 +6,9 @@
 // (reading A-1: the 0-deletion original is included).  As in SymScan, the tuple holds
 // a hash of the variant and the index of the sequence, (h_ij, i) (footnote 1):
 //     record = (top hash_bits of H(variant)) << id_bits | id
-// H is a polynomial hash over 5-bit residue codes, H(v) = mix64(sum_k R[v_k] * B^k + len * K) mod
-// 2^64 (B odd).  With the prefix sums A[j] = sum_{t<j} R[s_t] * B^t of the SOURCE sequence, the hash of
+// H is a polynomial hash over 5-bit residue codes, H(v) = sum_k R[v_k] * B^k + (len + 1) * K mod 2^64
+// (R[c], B, K: fixed odd 64-bit constants; no finaliser — the partition digits are the TOP bits of the
+// polynomial itself, which the odd multipliers already mix).  With the prefix sums A[j] = sum_{t<j} R[s_t] * B^t of the SOURCE sequence, the hash of
 // the variant that deletes positions p_1 < ... < p_k is
 //     sum_{m=0..k} B^{-m} * (A[p_{m+1}] - A[p_m + 1]),   p_0 = -1, p_{k+1} = L,
 // so a variant costs k+1 multiply-adds instead of a pass over its residues.
@@ -17,9 +18,10 @@
 // s[p] == s[q] with q the next kept position after p.  Exactly one set per distinct (variant, id)
 // survives, so repeated residues produce no duplicate records.
 //
-// Order: records are written in ascending id, at rec_off[id] + rank, where rec_off is the exclusive
-// scan of the per-sequence counts produced by the count pass — no atomics, deterministic layout,
-// and (with the stable sort) ids ascend inside every run of equal keys.
+// Order: the exact pipeline (k_gen2 / k_generate) writes records in ascending id, at rec_off[id] + rank,
+// where rec_off is the exclusive scan of the per-sequence counts produced by the count pass — no atomics,
+// deterministic layout.  The fused pipeline (k_gen2_part / k_generate_part, the default) skips counting:
+// records are staged under their top 8 hash bits and flushed to fixed-capacity bins in arbitrary order.
 #include <cstddef>
 
 #include "kernels.h"
@@ -56,11 +58,8 @@ __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, i
             maxlen = max(maxlen, (u32)L);
         }
     }
-    const i64 total = s.n > 0 ? s.off[s.n] : 0;
-    for (i64 t = t0; t < total; t += stride) {
-        int c = s.seqs[t];
-        if (c < 1 || c > 31) err |= SD_ERR_RESIDUE;
-    }
+    // (the residue codes are range-checked by k_pack / k_check_residues, which run only after the offsets
+    //  have been found valid: a malformed offsets array must never steer a read of `seqs`)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         nmax += __shfl_xor_sync(SD_FULL, nmax, o);
@@ -75,6 +74,19 @@ __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, i
         if (maxlen) atomicMax(&info->maxlen, maxlen);
         if (err) atomicOr(&info->err, err);
     }
+}
+
+// Residue range check on its own (the stage entry point that does not pack).  Launched after k_prepare: does
+// nothing unless the offsets were valid, and then offsets[n] <= 64 n bounds the scan.
+__global__ void __launch_bounds__(256) k_check_residues(SeqSetDev s, DevInfo* info) {
+    if (info->err) return;
+    const i64 total = s.n > 0 ? s.off[s.n] : 0;
+    u32 bad = 0;
+    for (i64 t = (i64)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (i64)gridDim.x * blockDim.x) {
+        const int c = s.seqs[t];
+        if (c < 1 || c > 31) bad = 1;
+    }
+    if (__any_sync(SD_FULL, bad) && (threadIdx.x & 31) == 0) atomicOr(&info->err, (u32)SD_ERR_RESIDUE);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -633,24 +645,14 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
 // histogram: the order of the records inside a bin is irrelevant to the join.  A record that finds its
 // digit's slots full goes straight to its bin (one global atomic).  A bin that would overflow raises
 // info->part_overflow: the host then redoes the chunk with the exact (histogram-based) pipeline.
-#ifndef GP_THREADS
-#define GP_THREADS 256
-#endif
-#ifndef GP_FLUSH_AT
-#define GP_FLUSH_AT 2800  // flush when more than this is staged after a round (i.e. after nearly every full round)
-#endif
-#ifndef GP_MINB
-#define GP_MINB 3
-#endif
-#ifndef GP_OVF
-#define GP_OVF 128
-#endif
-#ifndef GP_TRIP
-#define GP_TRIP 16  // d = 3: (g1, g2) iterations per step of a batch
-#endif
-#ifndef GP_ROUND
-#define GP_ROUND 5400  // records a block stages per round (21 per digit of the 32 slots); the host turns it into batches per warp
-#endif
+// (values swept on config 3 / config 5 in round 1: 512 threads, 2 or 4 resident blocks, rounds of 3600 / 7200 records
+//  and flush thresholds from 2000 to 4500 all landed within 3 % of these)
+constexpr int GP_THREADS = 256;    // threads per block
+constexpr int GP_MINB = 3;         // resident blocks per SM (64 KB stage each)
+constexpr int GP_FLUSH_AT = 2800;  // flush when more than this is staged after a round (i.e. after nearly every full round)
+constexpr int GP_OVF = 128;        // overflow list entries
+constexpr int GP_TRIP = 16;        // d = 3: (g1, g2) iterations per step of a batch
+constexpr int GP_ROUND = 5400;     // records a block stages per round (21 per digit of the 32 slots); the host turns it into batches per warp
 constexpr int GP_NW = GP_THREADS / 32, GP_S = 32;
 static_assert(GP_THREADS >= 256 && GP_THREADS % 32 == 0, "one thread per digit in the flush");
 
@@ -955,19 +957,11 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
 // Fused general path (k_generate_part): the enumeration of k_generate (any d <= 4, any length <= 64)
 // with the staging / flushing of k_gen2_part.  One sweep per round instead of two: no counts, no scan,
 // no offsets — a canonical deletion set is hashed and pushed under its top 8 hash bits.
-#ifndef GQ_S
-#define GQ_S 16  // stage slots per digit (16 or 32)
-#endif
-#ifndef GQ_R
-#define GQ_R 8   // consecutive deletion sets per thread and round: a round makes at most GEN_THREADS * GQ_R records
-#endif
-#ifndef GQ_MINB
-#define GQ_MINB 3
-#endif
+constexpr int GQ_S = 16;          // stage slots per digit (16 or 32; 32 halves the resident blocks: slower on config 5 shapes)
+constexpr int GQ_R = 8;           // consecutive deletion sets per thread and round: a round makes at most GEN_THREADS * GQ_R records
+constexpr int GQ_MINB = 3;        // resident blocks per SM (one more with 32-residue table rows)
+constexpr int GQ_FLUSH_AT = 900;  // flush when more than this is staged after a round
 static_assert(GQ_S == 16 || GQ_S == 32, "flush copies 32 / GQ_S digits per warp instruction");
-#ifndef GQ_FLUSH_AT
-#define GQ_FLUSH_AT 900
-#endif
 
 struct GenPartStage {
     u64 stage[256 * GQ_S];  // digit dg, rank r -> stage[dg * GQ_S + ((r + dg) & (GQ_S - 1))]
@@ -1160,12 +1154,23 @@ GenParams make_params2(SeqSetDev a, SeqSetDev b, const Layout& lay, int width) {
 }
 int gen2_grid(i64 wtasks) { return (int)std::min<i64>((wtasks + G2_NW - 1) / G2_NW, 148 * 8); }
 
+// the fused generators: [d == 3][chunked][plain] and [narrow rows][chunked]
+typedef void (*GenPartKernel)(GenPartParams);
+const GenPartKernel GEN2_PART_KERNELS[8] = {k_gen2_part<false, false, false>, k_gen2_part<false, true, false>, k_gen2_part<true, false, false>,
+                                            k_gen2_part<true, true, false>,  k_gen2_part<false, false, true>, k_gen2_part<false, true, true>,
+                                            k_gen2_part<true, false, true>,  k_gen2_part<true, true, true>};
+const GenPartKernel GENERATE_PART_KERNELS[4] = {k_generate_part<false, SD_L_MAX>, k_generate_part<true, SD_L_MAX>,
+                                                k_generate_part<false, 32>, k_generate_part<true, 32>};
+constexpr size_t GENERATE_PART_SMEM64 = ((sizeof(GenSharedT<SD_L_MAX>) + 15) & ~(size_t)15) + sizeof(GenPartStage);
+constexpr size_t GENERATE_PART_SMEM32 = ((sizeof(GenSharedT<32>) + 15) & ~(size_t)15) + sizeof(GenPartStage);
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------
-cudaError_t sd_init_tables() {
-    static bool done = false;
-    if (done) return cudaSuccess;
+// Per-device state of this translation unit: the __constant__ hash / binomial tables and the dynamic shared-memory
+// limits of the generator kernels.  Constants and function attributes belong to the CURRENT device, so this runs for
+// every context (symdel_create, under its lock) — never behind a process-wide flag.
+cudaError_t sd_generate_setup() {
     u64 R[32], Bpow[SD_L_MAX + 1], Binv[SD_D_MAX + 1];
     u64 st = 0x243f6a8885a308d3ull;
     for (int c = 0; c < 32; ++c) R[c] = splitmix64(st) | 1ull;
@@ -1176,7 +1181,7 @@ cudaError_t sd_init_tables() {
     for (int it = 0; it < 6; ++it) inv *= 2 - B * inv;
     Binv[0] = 1;
     for (int m = 1; m <= SD_D_MAX; ++m) Binv[m] = Binv[m - 1] * inv;
-    static u32 binom[(SD_L_MAX + 1) * (SD_D_MAX + 1)], vcum[(SD_L_MAX + 1) * (SD_D_MAX + 2)];
+    u32 binom[(SD_L_MAX + 1) * (SD_D_MAX + 1)], vcum[(SD_L_MAX + 1) * (SD_D_MAX + 2)];
     for (int n = 0; n <= SD_L_MAX; ++n) {
         for (int k = 0; k <= SD_D_MAX; ++k) {
             u64 c = 1;
@@ -1201,8 +1206,11 @@ cudaError_t sd_init_tables() {
     if ((e = cudaFuncSetAttribute(k_generate<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, gsm)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k_generate<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, gsm)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k_generate<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, gsm)) != cudaSuccess) return e;
-
-    done = true;
+    for (GenPartKernel k : GEN2_PART_KERNELS)
+        if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GenPartShared))) != cudaSuccess) return e;
+    for (int i = 0; i < 4; ++i)
+        if ((e = cudaFuncSetAttribute(GENERATE_PART_KERNELS[i], cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)(i < 2 ? GENERATE_PART_SMEM64 : GENERATE_PART_SMEM32))) != cudaSuccess) return e;
     return cudaSuccess;
 }
 
@@ -1211,6 +1219,12 @@ cudaError_t sd_prepare(SeqSetDev s, int d, int is_b, int prefix, DevInfo* info, 
     int blocks = (int)std::min<i64>((s.n + 255) / 256, 148 * 8);
     k_prepare<<<blocks, 256, 0, st>>>(s, d, is_b, prefix > 0 ? prefix : SD_L_MAX, info);
     if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
+cudaError_t sd_check_residues(SeqSetDev s, DevInfo* info, cudaStream_t st) {
+    if (s.n == 0) return cudaSuccess;
+    k_check_residues<<<(int)std::min<i64>((s.n + 15) / 16, 148 * 8), 256, 0, st>>>(s, info);
     return cudaGetLastError();
 }
 
@@ -1285,31 +1299,16 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
         const double per_round = lay.d == 3 ? GP_NW * 32.0 * GP_TRIP * 0.55 : GP_NW * 32.0 * std::max(records_per_residue, 0.03) * 0.85;
         PP.batches = (u32)std::min(8.0, std::max(1.0, std::floor(GP_ROUND / per_round + 0.5)));
     }
-    typedef void (*Kern)(GenPartParams);
-    static const Kern kerns[8] = {k_gen2_part<false, false, false>, k_gen2_part<false, true, false>, k_gen2_part<true, false, false>,
-                                  k_gen2_part<true, true, false>,  k_gen2_part<false, false, true>, k_gen2_part<false, true, true>,
-                                  k_gen2_part<true, false, true>,  k_gen2_part<true, true, true>};
-    static const Kern gkerns[4] = {k_generate_part<false, SD_L_MAX>, k_generate_part<true, SD_L_MAX>, k_generate_part<false, 32>, k_generate_part<true, 32>};
-    constexpr size_t gsm64 = ((sizeof(GenSharedT<SD_L_MAX>) + 15) & ~(size_t)15) + sizeof(GenPartStage);
-    constexpr size_t gsm32 = ((sizeof(GenSharedT<32>) + 15) & ~(size_t)15) + sizeof(GenPartStage);
-    static bool attr_set = false;
     cudaError_t e;
-    if (!attr_set) {
-        for (Kern k : kerns)
-            if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GenPartShared))) != cudaSuccess) return e;
-        for (int i = 0; i < 4; ++i)
-            if ((e = cudaFuncSetAttribute(gkerns[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(i < 2 ? gsm64 : gsm32))) != cudaSuccess) return e;
-        attr_set = true;
-    }
     if ((e = cudaMemsetAsync(cur, 0, 256 * sizeof(u32), st)) != cudaSuccess) return e;
     if (fast) {
         const int grid = (int)std::min<i64>((PP.g.groups_total + GP_NW - 1) / GP_NW, 148 * GP_MINB);
         const bool plain = lay.hash_bits + lay.id_bits == 64 && lay.id_bits <= 31;
-        kerns[(lay.d == 3 ? 4 : 0) + (lay.n_chunks > 1 ? 2 : 0) + (plain ? 1 : 0)]<<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
+        GEN2_PART_KERNELS[(lay.d == 3 ? 4 : 0) + (lay.n_chunks > 1 ? 2 : 0) + (plain ? 1 : 0)]<<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
     } else {
         const bool narrow = width - 1 <= 32;  // rows of 32 residues: a fourth block fits on the SM
         const int grid = (int)std::min<i64>(PP.g.groups_total, 148 * (narrow ? GQ_MINB + 1 : GQ_MINB));
-        gkerns[(narrow ? 2 : 0) + (lay.n_chunks > 1 ? 1 : 0)]<<<grid, GEN_THREADS, narrow ? gsm32 : gsm64, st>>>(PP);
+        GENERATE_PART_KERNELS[(narrow ? 2 : 0) + (lay.n_chunks > 1 ? 1 : 0)]<<<grid, GEN_THREADS, narrow ? GENERATE_PART_SMEM32 : GENERATE_PART_SMEM64, st>>>(PP);
     }
     if (launches) ++*launches;
     return cudaGetLastError();

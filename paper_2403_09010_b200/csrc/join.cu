@@ -41,9 +41,7 @@ namespace {
 constexpr int JN_THREADS = 512, JN_NW = JN_THREADS / 32, JN_T = 4096, JN_CAP = 6144;
 constexpr int JN_IT = JN_CAP / JN_THREADS;                     // strided iterations that cover a full window
 constexpr int JN_SLOT_BITS = 12, JN_SLOTS = 1 << JN_SLOT_BITS;  // chain heads
-#ifndef JBM_BITS
-#define JBM_BITS 16  // filter bitmap: 2^JBM_BITS bits each ("seen", "seen twice")
-#endif
+constexpr int JBM_BITS = 16;  // filter bitmap: 2^JBM_BITS bits each ("seen", "seen twice"); 15 bits: +6 %, 14 bits: +16 % on config 3
 constexpr int JN_BM_BITS = JBM_BITS, JN_BM_WORDS = (1 << JN_BM_BITS) / 32;
 constexpr u32 JN_NIL = 0xffffu, JN_NONE = 0xffffffffu;
 static_assert(JN_CAP < 0xffff && JN_CAP % JN_THREADS == 0 && JN_IT <= 32, "node index / nzmask width");
@@ -362,10 +360,7 @@ __global__ void __launch_bounds__(JN_THREADS, 2) k_join(const JoinParams P) {
 //
 // K32: the partitioned bits and the bitmap bits all sit in the high word of the record (the usual
 // layout); the filter phases then work on 32-bit words and keep only those in registers.
-#ifndef JF_THREADS_
-#define JF_THREADS_ 512
-#endif
-constexpr int JF_THREADS = JF_THREADS_, JF_NW = JF_THREADS / 32;
+constexpr int JF_THREADS = 512, JF_NW = JF_THREADS / 32;
 constexpr int JF_BM_BITS = JBM_BITS, JF_BM_WORDS = (1 << JF_BM_BITS) / 32;
 
 template <int LMAX, int SLOT_BITS>
@@ -583,12 +578,8 @@ __global__ void __launch_bounds__(JF_THREADS, MINB) k_join_fast(const JoinFastPa
         }
 }
 
-#ifndef JF_IT
-#define JF_IT 8
-#endif
-#ifndef JF_MINB_S
-#define JF_MINB_S 4
-#endif
+constexpr int JF_IT = 8;      // records per thread of a k_join_fast tile
+constexpr int JF_MINB_S = 4;  // resident blocks of the small-list instances
 constexpr int JF_T = JF_THREADS * JF_IT;
 constexpr int JF_LMAX_S = JF_IT > 8 ? 3072 : 2048, JF_SLOTB_S = 11;
 constexpr int JF_LMAX_L = JF_T + 4096, JF_SLOTB_L = 12, JF_MINB_L = JF_IT > 8 ? 1 : 2;
@@ -596,211 +587,191 @@ constexpr int JF_LMAX_L = JF_T + 4096, JF_SLOTB_L = 12, JF_MINB_L = JF_IT > 8 ? 
 
 // =================================================================================================
 // Bucket join of the fused pipeline: k_join_bkt.  The level-2 partition leaves every bucket in its own
-// fixed-capacity region with its record count, so nothing has to be found: a block takes `group`
-// consecutive buckets (about 4096 records) and runs the filter / list / chain / claim / write steps of
-// k_join_fast over them, with no boundary tests and no tails.  Buckets of one block share the bitmaps
-// and chains; records of different buckets never pair because the chain walk compares whole hashes.
-// Same two instances (small list first, redo list, large list), same fallback flag.
-#ifndef JB_TARGET
-#define JB_TARGET 4096  // records per block of k_join_bkt
-#endif
-#ifndef JB_PF_
-#define JB_PF_ 4
-#endif
-constexpr int JB_PF = JB_PF_;  // k_join_bkt: 16-byte loads per thread kept in flight (prefetch path)
-
+// fixed-capacity region with its record count, so nothing has to be found: ONE BLOCK PER BUCKET, and the
+// bucket is joined in a single sweep by a chained hash table in shared memory:
+//   0. the bucket comes into shared memory by one 1-D bulk asynchronous copy (cp.async.bulk, the TMA engine;
+//      completion counted in bytes on an mbarrier) while the threads clear the chain heads — no per-thread
+//      address arithmetic, no registers held across the phases;
+//   1. sweep: every record swaps its position into the head of its slot (the hash bits right below the
+//      partitioned ones; one shared-memory atomic exchange) and keeps the previous head as its `next` — IN the
+//      staged record: its top NB bits are the same for the whole bucket (partitioned hash bits, or zeros above a
+//      narrowed hash), so they carry the link and a chain step is ONE 8-byte shared load.  A record that found its
+//      slot empty (about four in five on sparse data) is finished: whoever pairs with it comes LATER and will find it;
+//   2. the others walk their chain — the records inserted BEFORE them — comparing the rest of the hash, so every
+//      unordered pair is met exactly once, by its later member: count, ONE shared atomic per thread with pairs +
+//      ONE global atomic per block claim the output range ("preallocating the outputs"), second
+//      walk writes.
+// No bitmaps, no candidate list, no list overflow: dense buckets (every record with partners) take the same
+// path, their chains are just longer.  The kernel is latency-bound (dependent shared-memory accesses): what
+// counts is resident warps, hence 34 KB of shared memory per block (six blocks of 256 threads per SM; with
+// five, +12 %; with four, +35 %).  Two instances: regions of up to 2560 records (NB = 12) and up to 18432
+// (1024 threads, one block per SM, NB = 15: chunks of more than ~10^8 records).  If the claims run past the
+// candidate window info->join_fallback is raised (the host then uses the exact pipeline).
 struct JoinBktParams {
     JoinParams j;       // rec = bucket regions; topmask unused
     const u32* cnt;     // records per bucket
     u32 cap;            // region stride (records; a multiple of 32)
-    u32 nbuckets, group;
-    const u32* tiles;   // nullptr: block b takes buckets [b*group, (b+1)*group); else the redo list
-    u32* redo;
+    u32 nbuckets;
 };
 
-template <bool K32, int LMAX, int SLOT_BITS, int MINB>
-__global__ void __launch_bounds__(JF_THREADS, MINB) k_join_bkt(const JoinBktParams BP) {
-    typedef typename std::conditional<K32, u32, u64>::type K;
-    typedef JoinFastSmem<LMAX, SLOT_BITS> Smem;
-    constexpr int SLOTS = 1 << SLOT_BITS, LIT = (LMAX + JF_THREADS - 1) / JF_THREADS;
-    static_assert(LMAX < 0xffff && LIT <= 32, "node index width / nzmask width");
+// ---- bulk asynchronous copy + mbarrier (PTX; SASS: UBLKCP / SYNCS) ----
+__device__ __forceinline__ u32 jb_smem(const void* p) { return (u32)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void jb_mbar_init(u64* bar, u32 count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(jb_smem(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void jb_fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void jb_mbar_expect_tx(u64* bar, u32 bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(jb_smem(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void jb_bulk_g2s(void* dst, const void* src, u32 bytes, u64* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(jb_smem(dst)),
+                 "l"(src), "r"(bytes), "r"(jb_smem(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void jb_mbar_wait(u64* bar, u32 parity) {
+    u32 done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(jb_smem(bar)), "r"(parity)
+            : "memory");
+    }
+}
+__device__ __forceinline__ u32 jb_atoms_exch(u32* p, u32 v) {
+    u32 old;
+    asm volatile("atom.shared.exch.b32 %0, [%1], %2;" : "=r"(old) : "r"(jb_smem(p)), "r"(v) : "memory");
+    return old;
+}
+
+template <int STAGE, int SLOT_BITS>
+struct JoinBktSmem {
+    u64 stage[STAGE];          // the bucket; after the sweep the top NB bits of a record = the record inserted into its slot before it
+    u32 head[1 << SLOT_BITS];  // last record inserted into the slot (all ones in NB bits: none)
+    u64 mbar;
+    u64 base;
+    u32 total;
+};
+
+template <int THREADS, int STAGE, int SLOT_BITS, int NB, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams BP) {
+    typedef JoinBktSmem<STAGE, SLOT_BITS> Smem;
+    constexpr int SLOTS = 1 << SLOT_BITS, IT = (STAGE / 2 + THREADS - 1) / THREADS;  // 16-byte loads per thread that cover the stage
+    constexpr u32 NIL = (1u << NB) - 1u;
+    constexpr u64 KEEP = ~0ull >> NB;  // the bits of a staged record that are still the record
+    static_assert(STAGE <= (int)NIL && STAGE % 2 == 0 && 2 * IT <= 32 && SLOTS % (4 * THREADS) == 0 && NB <= 16, "link / flag mask widths");
     extern __shared__ __align__(16) unsigned char jn_smem[];
     Smem& S = *reinterpret_cast<Smem*>(jn_smem);
     const JoinParams& P = BP.j;
-    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const u32 tile = BP.tiles ? BP.tiles[blockIdx.x] : blockIdx.x;
-    const u32 b0 = tile * BP.group, b1 = min(b0 + BP.group, BP.nbuckets);
-    auto key_of = [&](u64 y) -> K { return K32 ? (K)(y >> 32) : (K)y; };
-    const int bm_shift = K32 ? P.bm_shift - 32 : P.bm_shift;
-
-    // Prefetch path (the usual case: the block's buckets need at most JB_PF 16-byte loads per thread): every load
-    // is issued before anything else and the filter words stay in registers for both sweeps.
-    u32 itb = 0;  // 16-byte loads per thread and bucket
-    for (u32 b = b0; b < b1; ++b) itb = max(itb, (min(BP.cnt[b], BP.cap) + 2 * JF_THREADS - 1) / (2 * JF_THREADS));
-    const u32 ns = (b1 - b0) * itb;
-    const bool pf = ns <= (u32)JB_PF;
-    K kx[2 * JB_PF];
-    u32 vm = 0;  // bit e: kx[e] holds a record
-    if (pf) {
-#pragma unroll
-        for (int sl = 0; sl < JB_PF; ++sl) {
-            kx[2 * sl] = kx[2 * sl + 1] = 0;
-            if ((u32)sl < ns) {
-                const u32 g = (u32)sl / itb, b = b0 + g;
-                const u32 n = min(BP.cnt[b], BP.cap), i = 2 * tid + ((u32)sl - g * itb) * (2 * JF_THREADS);
-                const u64* const rp = P.rec + (u64)b * BP.cap;
-                if (i + 1 < n) {
-                    const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + i);
-                    kx[2 * sl] = key_of(t.x), kx[2 * sl + 1] = key_of(t.y);
-                    vm |= 3u << (2 * sl);
-                } else if (i < n) {
-                    kx[2 * sl] = key_of(rp[i]);
-                    vm |= 1u << (2 * sl);
-                }
-            }
-        }
+    const u32 tid = threadIdx.x;
+    const u32 bucket = blockIdx.x;
+    const u32 n = min(BP.cnt[bucket], BP.cap);
+    if (n < 2) return;  // nothing to pair (block-uniform)
+    if (tid == 0) {
+        S.total = 0;
+        jb_mbar_init(&S.mbar, 1);
+        jb_fence_proxy_async();
+        const u32 bytes = ((n + 1u) & ~1u) * 8u;  // whole 16-byte units (the region is a multiple of 256 bytes)
+        jb_mbar_expect_tx(&S.mbar, bytes);
+        jb_bulk_g2s(S.stage, P.rec + (u64)bucket * BP.cap, bytes, &S.mbar);
     }
-    for (u32 i = tid; i < 2 * JF_BM_WORDS / 4; i += JF_THREADS)
-        reinterpret_cast<uint4*>(S.bit_a)[i] = make_uint4(0u, 0u, 0u, 0u);  // bit_a and bit_b are adjacent
-    for (u32 i = tid; i < SLOTS / 4; i += JF_THREADS)
-        reinterpret_cast<uint4*>(S.head)[i] = make_uint4(JN_NIL, JN_NIL, JN_NIL, JN_NIL);
-    if (tid == 0) S.nlist = 0;
-    __syncthreads();
-    auto bm_of = [&](K y) -> u32 { return (u32)(y >> bm_shift) & ((1u << JF_BM_BITS) - 1u); };
-    auto mark = [&](K y) {
-        const u32 b = bm_of(y), bit = 1u << (b & 31u);
-        if (atomicOr(&S.bit_a[b >> 5], bit) & bit) atomicOr(&S.bit_b[b >> 5], bit);
-    };
-    auto listed = [&](K y) -> bool {
-        const u32 b = bm_of(y);
-        return (S.bit_b[b >> 5] >> (b & 31u)) & 1u;
-    };
-    auto append = [&](u64 y) {  // one shared-memory atomic per LISTED record (about one in ten on sparse data)
-        const u32 at = jf_atoms_add(&S.nlist, 1u);
-        if (at < (u32)LMAX) S.list[at] = y;
-    };
-    if (pf) {
-        // ---- 1. bitmaps ----
 #pragma unroll
-        for (int e = 0; e < 2 * JB_PF; ++e)
-            if ((vm >> e) & 1u) mark(kx[e]);
-        __syncthreads();
-        // ---- 2. list the records whose "seen twice" bit is set (whole record re-read: L1/L2) ----
+    for (int k = 0; k < SLOTS / (4 * THREADS); ++k)
+        reinterpret_cast<uint4*>(S.head)[tid + k * THREADS] = make_uint4(NIL, NIL, NIL, NIL);
+    __syncthreads();  // heads cleared, barrier initialised
+    jb_mbar_wait(&S.mbar, 0);
+    // ---- 1. sweep ----
+    const int slot_shift = P.slot_shift;
+    unsigned short* const link16 = reinterpret_cast<unsigned short*>(S.stage) + 3;  // bits 48..63 of record i: link16[4 * i]
+    u32 flag = 0;  // bit 2k + e: my record 2 * (tid + k * THREADS) + e found an earlier record in its slot
 #pragma unroll
-        for (int e = 0; e < 2 * JB_PF; ++e)
-            if (((vm >> e) & 1u) && listed(kx[e])) {
-                const u32 sl = (u32)e >> 1, g = sl / itb;
-                append(P.rec[(u64)(b0 + g) * BP.cap + 2 * tid + (sl - g * itb) * (2 * JF_THREADS) + ((u32)e & 1u)]);
-            }
-    } else {
-        // ---- 1. bitmaps (two records per 16-byte load; regions are 256-byte aligned) ----
-        for (u32 b = b0; b < b1; ++b) {
-            const u32 n = min(BP.cnt[b], BP.cap);
-            const u64* const rp = P.rec + (u64)b * BP.cap;
-            for (u32 i = 2 * tid; i < n; i += 2 * JF_THREADS) {
-                if (i + 1 < n) {
-                    const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + i);
-                    mark(key_of(t.x));
-                    mark(key_of(t.y));
-                } else {
-                    mark(key_of(rp[i]));
-                }
-            }
-        }
-        __syncthreads();
-        // ---- 2. list the records whose "seen twice" bit is set ----
-        for (u32 b = b0; b < b1; ++b) {
-            const u32 n = min(BP.cnt[b], BP.cap);
-            const u64* const rp = P.rec + (u64)b * BP.cap;
-            for (u32 i = 2 * tid; i < n; i += 2 * JF_THREADS) {
-                if (i + 1 < n) {
-                    const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(rp + i);
-                    if (listed(key_of(t.x))) append(t.x);
-                    if (listed(key_of(t.y))) append(t.y);
-                } else {
-                    const u64 y = rp[i];
-                    if (listed(key_of(y))) append(y);
-                }
+    for (int k = 0; k < IT; ++k) {
+        const u32 i = 2 * (tid + k * THREADS);
+        if (i < n) {
+            const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(S.stage + i);
+            const u32 o0 = jb_atoms_exch(&S.head[(u32)(t.x >> slot_shift) & (SLOTS - 1)], i);
+            link16[4 * i] = (unsigned short)((o0 << (16 - NB)) | ((u32)(t.x >> 48) & ((1u << (16 - NB)) - 1u)));
+            flag |= (o0 != NIL ? 1u : 0u) << (2 * k);
+            if (i + 1 < n) {
+                const u32 o1 = jb_atoms_exch(&S.head[(u32)(t.y >> slot_shift) & (SLOTS - 1)], i + 1);
+                link16[4 * i + 4] = (unsigned short)((o1 << (16 - NB)) | ((u32)(t.y >> 48) & ((1u << (16 - NB)) - 1u)));
+                flag |= (o1 != NIL ? 2u : 0u) << (2 * k);
             }
         }
     }
     __syncthreads();
-    const u32 nl = S.nlist;
-    if (nl == 0) return;
-    if (nl > (u32)LMAX) {
-        if (tid == 0) {
-            if (BP.redo) BP.redo[atomicAdd(&P.info->join_redo, 1u)] = tile;
-            else atomicOr(&P.info->join_fallback, 1u);
+    // ---- 2. count, claim, write ----
+    auto pos_of = [&](u32 e) -> u32 { return 2 * (tid + (e >> 1) * THREADS) + (e & 1u); };
+    u32 cnt = 0, nz = 0;
+    for (u32 m = flag; m; m &= m - 1) {
+        const u32 e = __ffs(m) - 1;
+        const u64 y = S.stage[pos_of(e)];
+        u32 c = 0;
+        for (u32 j = (u32)(y >> (64 - NB)); j != NIL;) {
+            const u64 z = S.stage[j];
+            u64 packed;
+            if (((y ^ z) & KEEP) < P.hlim && jn_pair(y, z, P, packed)) ++c;
+            j = (u32)(z >> (64 - NB));
         }
-        return;
+        if (c) nz |= 1u << e;
+        cnt += c;
     }
-    // ---- 3. chains ----
-    auto slot_of = [&](u64 y) -> u32 { return (u32)(y >> P.slot_shift) & (SLOTS - 1); };
-    for (u32 i = tid; i < nl; i += JF_THREADS) S.next[i] = (unsigned short)atomicExch(&S.head[slot_of(S.list[i])], i);
+    u32 mine = 0;  // this thread's offset inside the block's output range (any order: the candidates are sorted next)
+    if (cnt) mine = jf_atoms_add(&S.total, cnt);
     __syncthreads();
-    // ---- 4. count, claim, write ----
-    u32 cnt = 0, nzmask = 0;
-    {
-        u32 k = 0;
-        for (u32 i = tid; i < nl; i += JF_THREADS, ++k) {
-            u32 j = S.next[i];
-            if (j == JN_NIL) continue;
-            const u64 y = S.list[i];
-            u32 c = 0;
-            for (; j != JN_NIL; j = S.next[j]) {
-                const u64 z = S.list[j];
-                u64 packed;
-                if ((y ^ z) < P.hlim && jn_pair(y, z, P, packed)) ++c;
-            }
-            if (c) nzmask |= 1u << k;
-            cnt += c;
-        }
-    }
-    if (!__syncthreads_or(cnt != 0)) return;
-    u32 inc = cnt;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const u32 t = __shfl_up_sync(SD_FULL, inc, o);
-        if (lane >= (u32)o) inc += t;
-    }
-    if (lane == 31) S.wsum[warp] = inc;
-    __syncthreads();
-    if (warp == 0) {
-        const u32 w = lane < JF_NW ? S.wsum[lane] : 0u;
-        u32 winc = w;
-#pragma unroll
-        for (int o = 1; o < JF_NW; o <<= 1) {
-            const u32 t = __shfl_up_sync(SD_FULL, winc, o);
-            if (lane >= (u32)o) winc += t;
-        }
-        if (lane < JF_NW) S.wsum[lane] = winc - w;
-        if (lane == JF_NW - 1) {
-            const u64 base = (u64)atomicAdd((unsigned long long*)&P.info->n_cand, (unsigned long long)winc);
-            // does not fit the window: nothing is written
-            if (base + winc > P.win_hi) atomicOr(&P.info->join_fallback, 2u), S.base = ~0ull;
-            else S.base = base;
-        }
+    const u32 total = S.total;
+    if (total == 0) return;
+    if (tid == 0) {
+        const u64 base = (u64)atomicAdd((unsigned long long*)&P.info->n_cand, (unsigned long long)total);
+        // does not fit the window: nothing is written
+        if (base + total > P.win_hi) atomicOr(&P.info->join_fallback, 2u), S.base = ~0ull;
+        else S.base = base;
     }
     __syncthreads();
     if (S.base == ~0ull) return;
-    u64 at = S.base + S.wsum[warp] + inc - cnt;
-    for (u32 m = nzmask, k = 0; m; m >>= 1, ++k)
-        if (m & 1u) {
-            const u32 i = tid + k * JF_THREADS;
-            const u64 y = S.list[i];
-            for (u32 j = S.next[i]; j != JN_NIL; j = S.next[j]) {
-                const u64 z = S.list[j];
-                u64 packed;
-                if ((y ^ z) < P.hlim && jn_pair(y, z, P, packed)) P.cand[at++] = packed;
-            }
+    u64 at = S.base + mine;
+    for (u32 m = nz; m; m &= m - 1) {
+        const u64 y = S.stage[pos_of(__ffs(m) - 1)];
+        for (u32 j = (u32)(y >> (64 - NB)); j != NIL;) {
+            const u64 z = S.stage[j];
+            u64 packed;
+            if (((y ^ z) & KEEP) < P.hlim && jn_pair(y, z, P, packed)) P.cand[at++] = packed;
+            j = (u32)(z >> (64 - NB));
         }
+    }
 }
 
-constexpr int JB_LMAX_L = 8192;
+// the two instances: (threads, stage, chain-head bits, link bits, resident blocks)
+constexpr int JB_THREADS_S = 256, JB_STAGE_S = 2560, JB_SLOTB_S = 12, JB_NB_S = 12, JB_MINB_S = 6;
+constexpr int JB_THREADS_L = 1024, JB_STAGE_L = 18432, JB_SLOTB_L = 14, JB_NB_L = 15, JB_MINB_L = 1;
+static_assert(6 * (sizeof(JoinBktSmem<JB_STAGE_S, JB_SLOTB_S>) + 1024) <= 233472, "six blocks of the small instance per SM");
 
 }  // namespace
 
 i64 sd_join_tiles(i64 n_records) { return (n_records + JN_T - 1) / JN_T; }
+
+// Per-device state of this translation unit (dynamic shared-memory limits of the join kernels): set for the current
+// device by every symdel_create — function attributes belong to a device, not to the process.
+template <bool K32>
+static cudaError_t jn_setup_k() {
+    cudaError_t e;
+    const int ss = (int)sizeof(JoinFastSmem<JF_LMAX_S, JF_SLOTB_S>), sl = (int)sizeof(JoinFastSmem<JF_LMAX_L, JF_SLOTB_L>);
+    if ((e = cudaFuncSetAttribute(k_join_fast<K32, JF_IT, JF_LMAX_S, JF_SLOTB_S, JF_MINB_S>, cudaFuncAttributeMaxDynamicSharedMemorySize, ss)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_join_fast<K32, JF_IT, JF_LMAX_L, JF_SLOTB_L, JF_MINB_L>, cudaFuncAttributeMaxDynamicSharedMemorySize, sl)) != cudaSuccess) return e;
+    return cudaSuccess;
+}
+cudaError_t sd_join_setup() {
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(k_join, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(JoinSmem))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)sizeof(JoinBktSmem<JB_STAGE_S, JB_SLOTB_S>))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)sizeof(JoinBktSmem<JB_STAGE_L, JB_SLOTB_L>))) != cudaSuccess) return e;
+    if ((e = jn_setup_k<true>()) != cudaSuccess) return e;
+    return jn_setup_k<false>();
+}
 
 static JoinParams jn_params(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 cand_cap, DevInfo* info) {
     JoinParams P{};
@@ -830,22 +801,15 @@ static JoinParams jn_params(const u64* records, i64 n_records, const Layout& lay
 // join (nothing usable was written).
 template <bool K32>
 static cudaError_t jn_launch_fast(const JoinFastParams& FP, unsigned grid, bool large, cudaStream_t st) {
-    static bool attr_set = false;
     auto ks = k_join_fast<K32, JF_IT, JF_LMAX_S, JF_SLOTB_S, JF_MINB_S>;
     auto kl = k_join_fast<K32, JF_IT, JF_LMAX_L, JF_SLOTB_L, JF_MINB_L>;
     constexpr size_t ss = sizeof(JoinFastSmem<JF_LMAX_S, JF_SLOTB_S>), sl = sizeof(JoinFastSmem<JF_LMAX_L, JF_SLOTB_L>);
-    cudaError_t e;
-    if (!attr_set) {
-        if ((e = cudaFuncSetAttribute(ks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ss)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(kl, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sl)) != cudaSuccess) return e;
-        attr_set = true;
-    }
     if (large) kl<<<grid, JF_THREADS, sl, st>>>(FP);
     else ks<<<grid, JF_THREADS, ss, st>>>(FP);
     return cudaGetLastError();
 }
 
-static bool jn_k32(const JoinParams& P) { return P.bm_shift >= 32 && (P.topmask & 0xffffffffull) == 0; }
+static inline int jn_k32(const JoinParams& P) { return P.bm_shift >= 32 && (P.topmask & 0xffffffffull) == 0; }
 
 cudaError_t sd_join_fast(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, u32* redo,
                          DevInfo* info, cudaStream_t st, i64* launches) {
@@ -882,12 +846,7 @@ cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* c
     const i64 tiles = sd_join_tiles(n_records);
     if (tiles == 0) return cudaSuccess;
     constexpr size_t smem = sizeof(JoinSmem);
-    static bool attr_set = false;
     cudaError_t e;
-    if (!attr_set) {
-        if ((e = cudaFuncSetAttribute(k_join, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        attr_set = true;
-    }
     if (first_round && (e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(&info->win_end, 0, sizeof(u64), st)) != cudaSuccess) return e;
     JoinParams P = jn_params(records, n_records, lay, cand, cand_cap, info);
@@ -902,39 +861,18 @@ cudaError_t sd_join(const u64* records, i64 n_records, const Layout& lay, u64* c
 
 // ---- bucket join of the fused pipeline ------------------------------------------------------------
 // buckets: nbuckets regions of `cap` records with counts cnt.  lay.sort_bits = the partitioned bits.
-// Step 1 (tiles == nullptr): small-list instance over all bucket groups, overflowing groups land in
-// redo[0 .. info->join_redo).  Step 2 (tiles = redo, n_tiles = join_redo): large-list instance.
-template <bool K32>
-static cudaError_t jn_launch_bkt(const JoinBktParams& BP, unsigned grid, bool large, cudaStream_t st) {
-    static bool attr_set = false;
-    auto ks = k_join_bkt<K32, JF_LMAX_S, JF_SLOTB_S, JF_MINB_S>;
-    auto kl = k_join_bkt<K32, JB_LMAX_L, JF_SLOTB_L, 2>;
-    constexpr size_t ss = sizeof(JoinFastSmem<JF_LMAX_S, JF_SLOTB_S>), sl = sizeof(JoinFastSmem<JB_LMAX_L, JF_SLOTB_L>);
-    cudaError_t e;
-    if (!attr_set) {
-        if ((e = cudaFuncSetAttribute(ks, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ss)) != cudaSuccess) return e;
-        if ((e = cudaFuncSetAttribute(kl, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sl)) != cudaSuccess) return e;
-        attr_set = true;
-    }
-    if (large) kl<<<grid, JF_THREADS, sl, st>>>(BP);
-    else ks<<<grid, JF_THREADS, ss, st>>>(BP);
-    return cudaGetLastError();
-}
+// info->n_cand = number of pairs written to cand[0 .. ); info->join_fallback != 0: they did not fit `window`.
+int sd_join_bkt_max_cap() { return JB_STAGE_L; }
+// the fused pipeline needs this many bits on top of every record of a bucket that are the same for the whole bucket
+// (partitioned hash bits, or zeros above a narrowed hash): they carry the chain link
+int sd_join_bkt_link_bits(u32 cap) { return cap <= (u32)JB_STAGE_S ? JB_NB_S : JB_NB_L; }
 
-u32 sd_join_bkt_group(i64 n_records, u32 nbuckets) {  // buckets per block: about 4096 records
-    const i64 avg = std::max<i64>(1, n_records / nbuckets);
-    return (u32)std::min<i64>(std::max<i64>(1, JB_TARGET / avg), 256);
-}
-
-cudaError_t sd_join_bkt(const u64* buckets, const u32* cnt, u32 cap, u32 nbuckets, u32 group, const Layout& lay, u64* cand,
-                        u64 window, const u32* tiles, u32 n_tiles, u32* redo, DevInfo* info, cudaStream_t st, i64* launches) {
+cudaError_t sd_join_bkt(const u64* buckets, const u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
+                        DevInfo* info, cudaStream_t st, i64* launches) {
     cudaError_t e;
-    if (!tiles) {
-        if ((e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
-        if ((e = cudaMemsetAsync(&info->join_fallback, 0, 2 * sizeof(u32), st)) != cudaSuccess) return e;  // and join_redo
-        n_tiles = (nbuckets + group - 1) / group;
-    }
-    if (n_tiles == 0) return cudaSuccess;
+    if ((e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(&info->join_fallback, 0, 2 * sizeof(u32), st)) != cudaSuccess) return e;  // and join_redo
+    if (nbuckets == 0) return cudaSuccess;
     JoinBktParams BP{};
     BP.j = jn_params(buckets, 0, lay, cand, window, info);
     BP.j.win_lo = 0;
@@ -942,10 +880,14 @@ cudaError_t sd_join_bkt(const u64* buckets, const u32* cnt, u32 cap, u32 nbucket
     BP.cnt = cnt;
     BP.cap = cap;
     BP.nbuckets = nbuckets;
-    BP.group = group;
-    BP.tiles = tiles;
-    BP.redo = tiles ? nullptr : redo;
+    // chain slot = the hash bits right below the partitioned ones (clamped to the hash field)
+    const int top = lay.id_bits + lay.hash_bits;
+    const bool small = cap <= (u32)JB_STAGE_S;
+    BP.j.slot_shift = std::max(lay.id_bits, top - lay.sort_bits - (small ? JB_SLOTB_S : JB_SLOTB_L));
     if (launches) ++*launches;
-    const bool k32 = BP.j.bm_shift >= 32;
-    return k32 ? jn_launch_bkt<true>(BP, n_tiles, tiles != nullptr, st) : jn_launch_bkt<false>(BP, n_tiles, tiles != nullptr, st);
+    if (small)
+        k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S><<<nbuckets, JB_THREADS_S, sizeof(JoinBktSmem<JB_STAGE_S, JB_SLOTB_S>), st>>>(BP);
+    else
+        k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L><<<nbuckets, JB_THREADS_L, sizeof(JoinBktSmem<JB_STAGE_L, JB_SLOTB_L>), st>>>(BP);
+    return cudaGetLastError();
 }

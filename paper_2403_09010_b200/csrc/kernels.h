@@ -36,23 +36,27 @@ struct Layout {
 
 // ---- radix_sort.cu ------------------------------------------------------------------------------
 i64 sd_sort_tiles(i64 n);
-int sd_sort_set_variant(int v);  // tuning hook: tile shape of k_onesweep
+int sd_sort_variants();           // number of selectable tile shapes of k_onesweep
+cudaError_t sd_sort_setup();      // per-device setup (function attributes); symdel_create
 i64 sd_sort_scratch_bytes(i64 n, int npass);
 cudaError_t sd_sort_prepare(void* scratch, i64 n, int npass, cudaStream_t st);
 u32* sd_sort_hist_ptr(void* scratch);
 cudaError_t sd_sort_histogram(const u64* keys, i64 n, int begin_bit, int npass, void* scratch, cudaStream_t st,
                               i64* launches);
 cudaError_t sd_sort_hist_scan(void* scratch, int npass, cudaStream_t st, i64* launches);
-cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, int stable, void* scratch, cudaStream_t st,
-                           u64** result, i64* launches);
+cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, int stable, int variant, void* scratch,
+                           cudaStream_t st, u64** result, i64* launches);
 
 // level-2 partition of the fused pipeline: bins (256 x cap1) -> buckets ((256 << b2) x cap2)
 cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u32* cnt2, i64 cap2, int b2, int shift,
                      DevInfo* info, cudaStream_t st, i64* launches);
 
 // ---- generate.cu --------------------------------------------------------------------------------
-cudaError_t sd_init_tables();  // fills the __constant__ tables once per process
+cudaError_t sd_generate_setup();  // per-device setup: the __constant__ tables and function attributes; symdel_create
+// validates the offsets and lengths (info->err), accumulates nmax / residues / maxlen; never reads `seqs`
 cudaError_t sd_prepare(SeqSetDev s, int d, int is_b, int prefix, DevInfo* info, cudaStream_t st, i64* launches);
+// residue codes in 1..31 (info->err |= SD_ERR_RESIDUE); a no-op unless sd_prepare left info->err == 0
+cudaError_t sd_check_residues(SeqSetDev s, DevInfo* info, cudaStream_t st);
 // count pass: cnt[gid] = number of records sequence gid contributes (u32 per sequence)
 cudaError_t sd_count(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u32* cnt, DevInfo* info, cudaStream_t st,
                      i64* launches);
@@ -74,6 +78,7 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
 
 // ---- join.cu ------------------------------------------------------------------------------------
 i64 sd_join_tiles(i64 n_records);
+cudaError_t sd_join_setup();  // per-device setup (function attributes); symdel_create
 // records: partitioned on the top lay.sort_bits bits of the hash field.  Emits the candidate pairs of
 // the records whose first flat pair index lies in [win_lo, win_hi) to cand[index - win_lo] (cand_cap
 // physical slots: the window plus slack for the last record's overhang); info->win_end = end of what
@@ -91,17 +96,19 @@ cudaError_t sd_join_fast(const u64* records, i64 n_records, const Layout& lay, u
 cudaError_t sd_join_fast_redo(const u64* records, i64 n_records, const Layout& lay, u64* cand, u64 window, const u32* redo,
                               u32 n_redo, DevInfo* info, cudaStream_t st, i64* launches);
 
-// Bucket join of the fused pipeline (see join.cu).  tiles == nullptr: first step over all bucket groups
-// (clears n_cand / join_fallback / join_redo, fills redo); else the redo step over n_tiles listed groups.
-u32 sd_join_bkt_group(i64 n_records, u32 nbuckets);
-cudaError_t sd_join_bkt(const u64* buckets, const u32* cnt, u32 cap, u32 nbuckets, u32 group, const Layout& lay, u64* cand,
-                        u64 window, const u32* tiles, u32 n_tiles, u32* redo, DevInfo* info, cudaStream_t st, i64* launches);
+// Bucket join of the fused pipeline (see join.cu): one block per bucket (regions of `cap` <= sd_join_bkt_max_cap()
+// records).  Clears and fills info->n_cand; info->join_fallback != 0: the pairs did not fit `window`.
+int sd_join_bkt_max_cap();
+int sd_join_bkt_link_bits(u32 cap);  // bits on top of a record that must be constant within a bucket
+cudaError_t sd_join_bkt(const u64* buckets, const u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
+                        DevInfo* info, cudaStream_t st, i64* launches);
 
 // ---- verify.cu ----------------------------------------------------------------------------------
 i64 sd_verify_tiles(i64 n);
 // packed bit-plane table of all sequences (A then B): 32 B (maxlen <= 32) or 48 B per sequence
 i64 sd_pack_bytes(i64 n_total, int maxlen);
-cudaError_t sd_pack(SeqSetDev a, SeqSetDev b, int maxlen, void* slots, cudaStream_t st, i64* launches);
+// (also range-checks every residue code: info->err |= SD_ERR_RESIDUE; call only after the offsets were found valid)
+cudaError_t sd_pack(SeqSetDev a, SeqSetDev b, int maxlen, void* slots, DevInfo* info, cudaStream_t st, i64* launches);
 // cand sorted ascending.  Drops repeats and a == b (self), computes lev, keeps <= d, appends
 // (pair << 3 | dist) in order to surv[surv_base + ...]; info->n_surv = total; info->n_unique += unique.
 cudaError_t sd_verify(const u64* cand, i64 n_cand, const void* slots, const Layout& lay, int maxlen, u64* surv,
@@ -110,12 +117,14 @@ cudaError_t sd_verify(const u64* cand, i64 n_cand, const void* slots, const Layo
 cudaError_t sd_verify_direct(const u64* cand, i64 n_cand, const void* slots, const Layout& lay, int maxlen, i32* out_i, i32* out_j,
                              i32* out_dist, i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
 // surv sorted ascending (and unique unless dedup = 1).  Unpacks to SoA outputs, first `capacity`
-// only; info->n_out = total.
+// only; info->n_out = total.  packed_out != nullptr: writes the kept words to packed_out instead (the merge of
+// the survivor list between flushes).
 cudaError_t sd_finalize(const u64* surv, i64 n_surv, const Layout& lay, int dedup, i32* out_i, i32* out_j, i32* out_dist,
-                        i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
+                        u64* packed_out, i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
 // plain distances for index pairs (stage test); slots = sd_pack of (A, B)
-cudaError_t sd_lev_pairs(const void* slots, i64 n_a, int maxlen, const i32* ia, const i32* ib, i64 n_pairs, i32* dist,
-                         cudaStream_t st);
+// (an index outside [0, n_a) / [0, n_b): dist = -1 and SD_ERR_INTERNAL in *err)
+cudaError_t sd_lev_pairs(const void* slots, i64 n_a, i64 n_b, int maxlen, const i32* ia, const i32* ib, i64 n_pairs, i32* dist,
+                         u32* err, cudaStream_t st);
 // NEXT-4: M x M overlap matrix of the output pairs under per-sequence repertoire labels
-cudaError_t sd_overlap(const i32* pi, const i32* pj, i64 n, const i32* lab_i, const i32* lab_j, int M, int symmetric,
-                       u64* matrix, u32* err, cudaStream_t st);
+cudaError_t sd_overlap(const i32* pi, const i32* pj, i64 n, const i32* lab_i, i64 n_i, const i32* lab_j, i64 n_j, int M,
+                       int symmetric, u64* matrix, u32* err, cudaStream_t st);

@@ -1,17 +1,22 @@
-// radix_sort.cu — S2/K2: stable LSD radix sort of 64-bit records, onesweep style.
+// radix_sort.cu — S2/K2: radix partition / LSD radix sort of 64-bit words, onesweep style.
 //
 // "Second, sort those tuples by the deletion variant.  This guarantees that all strings with
 // matching deletion variants will be stored contiguously." (§I.B step 2; App. F.2
 // step 2; App. F.3 step 2).  The paper's tools use a parallel CPU sort
-// and a GPU merge sort; this is a hand-written least-significant-digit radix sort instead:
-//   * one up-front pass builds the 256-bin histogram of every digit place (k_histogram) — the
-//     variant-generation kernel fuses this into its own pass and skips the extra read;
-//   * one kernel per 8-bit digit (k_onesweep): each tile ranks its keys with warp-level match
-//     groups and per-warp shared-memory counters, obtains its cross-tile exclusive prefix per digit
-//     by decoupled look-back over a status array (tile order = atomic ticket, so predecessors have
-//     always started), stages the tile in shared memory in digit order and writes each digit's keys
-//     to one contiguous global segment.
-// Every pass reads n*8 and writes n*8 bytes: the algorithmic traffic of the sort is 16 B/record/pass.
+// and a GPU merge sort.  Here equal variants only have to MEET, so the variant records are not
+// sorted in full:
+//   * fused pipeline (default): k_part2 splits each level-1 bin written by the generator on the next
+//     hash bits into fixed-capacity buckets (one pass, no histogram, no look-back); the join compares
+//     the remaining hash bits;
+//   * exact pipeline (fallback): k_onesweep passes over the top `sort_bits` of the hash only, on exact
+//     histograms that the generation kernel accumulates in its own pass;
+//   * the packed candidate pair ids (S3b) and the merged survivors ARE sorted in full: k_histogram
+//     (one read builds every digit place) + one k_onesweep per 8-bit digit.
+// k_onesweep: each tile ranks its keys with per-warp shared-memory counters and peer masks, obtains
+// its cross-tile exclusive prefix per digit by decoupled look-back over a status array (tile order =
+// atomic ticket, so predecessors have always started), stages the tile in shared memory in digit
+// order and writes each digit's keys to one contiguous global segment.
+// Every pass reads n*8 and writes n*8 bytes: 16 B/word/pass of algorithmic traffic.
 #include "kernels.h"
 
 namespace {
@@ -46,42 +51,7 @@ __global__ void __launch_bounds__(256) k_hist_scan(u32* __restrict__ ghist) {
 #define OS_FLAG_AGG (1u << 30)
 #define OS_FLAG_PRE (2u << 30)
 #define OS_MASK ((1u << 30) - 1)
-#ifndef OS_LB
-#define OS_LB 4
-#endif
-#ifndef OS_MATCH_OR
-#define OS_MATCH_OR 1
-#endif
-
-#if !OS_MATCH_OR
-// Peer mask of the lanes holding the same 8-bit digit, built from 8 ballots (the MATCH.ANY
-// instruction measured ~170 cycles per warp on sm_100a; 8 x (VOTE + LOP3) is ~10x cheaper).
-__device__ __forceinline__ u32 os_match8(u32 dg, u32 init) {
-    u32 peers = init;
-    // per bit: LOP3 (test -> predicate), VOTE, one of two predicated LOP3s (peers &= v / peers &= ~v)
-#define OS_MATCH_BIT(B)                                                                          \
-    asm volatile(                                                                                \
-        "{\n\t.reg .pred p;\n\t.reg .b32 t, v;\n\t"                                              \
-        "and.b32 t, %1, " #B ";\n\t"                                                             \
-        "setp.ne.u32 p, t, 0;\n\t"                                                               \
-        "vote.sync.ballot.b32 v, p, 0xffffffff;\n\t"                                             \
-        "@p and.b32 %0, %0, v;\n\t"                                                              \
-        "@!p lop3.b32 %0, %0, v, 0, 0x30;\n\t"                                                   \
-        "}"                                                                                      \
-        : "+r"(peers)                                                                            \
-        : "r"(dg))
-    OS_MATCH_BIT(1);
-    OS_MATCH_BIT(2);
-    OS_MATCH_BIT(4);
-    OS_MATCH_BIT(8);
-    OS_MATCH_BIT(16);
-    OS_MATCH_BIT(32);
-    OS_MATCH_BIT(64);
-    OS_MATCH_BIT(128);
-#undef OS_MATCH_BIT
-    return peers;
-}
-#endif
+constexpr int OS_LB = 4;  // look-back: predecessors inspected per round trip
 
 // Shared tail of both tile paths: per-digit decoupled look-back, then the coalesced write-out of the
 // tile staged in digit order.  `total` / `tstart` (threads < 256): this tile's count and tile-local
@@ -133,11 +103,7 @@ __device__ __forceinline__ void os_lookback_and_write(u64* __restrict__ out, con
         const u32 pos = tid + k * THREADS;
         if (FULLT || pos < tile_n) {
             const u64 kk = skeys[pos];
-#ifdef OS_DBG_LINEAR
-            out[(u64)tile * (THREADS * IPT) + pos] = kk + s_gofs[(u32)(kk >> shift) & 255u];
-#else
             out[s_gofs[(u32)(kk >> shift) & 255u] + pos] = kk;
-#endif
         }
     }
 }
@@ -182,7 +148,6 @@ __device__ __forceinline__ void os_tile(const u64 (&key)[IPT], u64* __restrict__
     __syncthreads();
 
     // ---- rank inside the warp's chunk (stable: position order = (k, lane)) and stage in digit order ----
-#if OS_MATCH_OR
     // peer mask by one shared-memory atomic OR per key (measured 2.5x cheaper than 8 ballots on sm_100a)
     u32* mymask = wmask + warp * 256;
 #pragma unroll
@@ -202,21 +167,6 @@ __device__ __forceinline__ void os_tile(const u64 (&key)[IPT], u64* __restrict__
         __syncwarp();
         if (valid) skeys[pre + below] = key[k];
     }
-#else
-    (void)wmask;
-#pragma unroll
-    for (int k = 0; k < IPT; ++k) {
-        const bool valid = FULLT || (wbase + 32 * k + lane) < tile_n;
-        const u32 dg = (u32)(key[k] >> shift) & 255u;
-        const u32 peers = os_match8(dg, FULLT ? SD_FULL : __ballot_sync(SD_FULL, valid));
-        const u32 pre = myhist[dg];
-        __syncwarp();
-        const u32 below = __popc(peers & lane_lt);
-        if (valid && below == 0) myhist[dg] = pre + __popc(peers);
-        __syncwarp();
-        if (valid) skeys[pre + below] = key[k];
-    }
-#endif
     os_lookback_and_write<THREADS, IPT, FULLT>(out, tile_n, tile, shift, gbase, st, total, tstart, skeys, s_gofs, false, 0u);
 }
 
@@ -328,13 +278,7 @@ __global__ void __launch_bounds__(THREADS, MINB) k_onesweep(const u64* __restric
 // — without histograms, tickets or look-back, because nothing downstream needs the records of a bucket
 // contiguous with the next bucket or in any order.  A bucket that would overflow raises
 // info->part_overflow (the host falls back to the exact pipeline).
-#ifndef P2_IPT_
-#define P2_IPT_ 16
-#endif
-#ifndef P2_MINB
-#define P2_MINB 4
-#endif
-constexpr int P2_THREADS = 256, P2_IPT = P2_IPT_, P2_TILE = P2_THREADS * P2_IPT;
+constexpr int P2_THREADS = 256, P2_IPT = 16, P2_MINB = 4, P2_TILE = P2_THREADS * P2_IPT;  // (tiles of 12 / 20 / 24 keys per thread: within 2 %)
 
 struct Part2Params {
     const u64* bins;
@@ -424,27 +368,29 @@ template <int THREADS, int IPT, int MINB>
 constexpr OsVariant os_variant() {
     return {THREADS, IPT, (size_t)THREADS * IPT * 8 + 2 * (THREADS / 32) * 256 * 4 + 256 * 4, k_onesweep<THREADS, IPT, MINB>};
 }
+// Tile shapes.  [0] is the one the pipeline uses (round 1 swept 17 shapes on config 3: 256 x 16 with four
+// resident blocks was the fastest pass, 3.6 TB/s; 512 x 16 and 384 x 18 within 3 %); the others stay
+// selectable per context (SYMDEL_OPT_SORT_VARIANT) so that the parity tests cover other tile geometries.
 const OsVariant OS_VARIANTS[] = {os_variant<256, 16, 4>(), os_variant<512, 16, 2>(), os_variant<384, 18, 2>(),
-                                 os_variant<256, 20, 3>(), os_variant<512, 12, 2>(), os_variant<256, 12, 4>(),
-#ifdef OS_SWEEP
-                                 os_variant<256, 24, 2>(), os_variant<384, 20, 2>(), os_variant<384, 16, 2>(), os_variant<320, 20, 2>(),
-                                 os_variant<256, 18, 3>(), os_variant<384, 14, 3>(), os_variant<256, 28, 2>(), os_variant<384, 22, 2>(),
-                                 os_variant<512, 14, 2>(), os_variant<320, 24, 2>(), os_variant<288, 24, 2>(),
-#endif
-};
+                                 os_variant<256, 12, 4>()};
 constexpr int OS_NVARIANTS = sizeof(OS_VARIANTS) / sizeof(OS_VARIANTS[0]);
 constexpr int OS_MIN_TILE = 256 * 12;  // scratch is sized for the smallest tile of any variant
-int g_os_variant = 0;
 
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------
 i64 sd_sort_tiles(i64 n) { return (n + OS_MIN_TILE - 1) / OS_MIN_TILE; }
 
-int sd_sort_set_variant(int v) {
-    if (v < 0 || v >= OS_NVARIANTS) return -1;
-    g_os_variant = v;
-    return 0;
+int sd_sort_variants() { return OS_NVARIANTS; }
+
+// Per-device state of this translation unit (dynamic shared-memory limits): set for the current device by every
+// symdel_create.
+cudaError_t sd_sort_setup() {
+    cudaError_t e;
+    for (int v = 0; v < OS_NVARIANTS; ++v)
+        if ((e = cudaFuncSetAttribute(OS_VARIANTS[v].kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OS_VARIANTS[v].smem)) != cudaSuccess)
+            return e;
+    return cudaFuncSetAttribute(k_part2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)P2_TILE * 8));
 }
 
 // scratch layout: [npass][256] u32 histograms | [npass] tickets (padded to 256 B) | [npass][tiles][256] u32 status
@@ -480,20 +426,11 @@ cudaError_t sd_sort_hist_scan(void* scratch, int npass, cudaStream_t st, i64* la
 // Returns in *result the buffer (keys or tmp) that holds the sorted records.
 // stable = 1: ties keep their input order.  stable = 0: keys-only sort, ties in arbitrary order (lets
 // uniform tiles take the cheaper grouping path).
-cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, int stable, void* scratch,
+cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, int stable, int variant, void* scratch,
                            cudaStream_t st, u64** result, i64* launches) {
     *result = keys;
     if (n == 0 || npass == 0) return cudaSuccess;
-    static bool attr_set = false;
-    if (!attr_set) {
-        for (int v = 0; v < OS_NVARIANTS; ++v) {
-            cudaError_t e = cudaFuncSetAttribute(OS_VARIANTS[v].kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                 (int)OS_VARIANTS[v].smem);
-            if (e != cudaSuccess) return e;
-        }
-        attr_set = true;
-    }
-    const OsVariant& V = OS_VARIANTS[g_os_variant];
+    const OsVariant& V = OS_VARIANTS[variant >= 0 && variant < OS_NVARIANTS ? variant : 0];
     u32* hist = sd_sort_hist_ptr(scratch);
     u32* tickets = hist + npass * 256;
     u32* status = tickets + 64;
@@ -517,13 +454,8 @@ cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass,
 // for the caller (the bins are the buckets).
 cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u32* cnt2, i64 cap2, int b2, int shift,
                      DevInfo* info, cudaStream_t st, i64* launches) {
-    static bool attr_set = false;
     cudaError_t e;
     constexpr size_t smem = (size_t)P2_TILE * 8;
-    if (!attr_set) {
-        if ((e = cudaFuncSetAttribute(k_part2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        attr_set = true;
-    }
     if ((e = cudaMemsetAsync(cnt2, 0, ((size_t)256 << b2) * sizeof(u32), st)) != cudaSuccess) return e;
     Part2Params P{};
     P.bins = bins;

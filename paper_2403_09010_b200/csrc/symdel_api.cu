@@ -23,6 +23,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "../../include/symdel.h"
@@ -34,6 +35,7 @@ struct symdel_ctx {
     symdel_stats stats{};
     int opt_timing = 0;
     i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0, opt_general_gen = 0;
+    i64 opt_sort_variant = 0, opt_surv_cap = 0;
     i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0, opt_join_general = 0, opt_exact = 0, opt_prefix = 0, opt_metric = 0;
     DevInfo* h_info = nullptr;  // pinned; followed by 256 u32 (the level-1 bin counts of the fused pipeline)
     void* arena = nullptr;      // device arena of the *_host entry points: outputs + workspace
@@ -95,7 +97,7 @@ u64 vcount_host(int L, int d) {
 // Fused pipeline (generation + level-1 partition, level-2 partition, bucket join): fixed-capacity bins
 // and buckets sized for `nexp` expected records with hash-uniform keys, + 8 standard deviations.
 struct FusedPlan {
-    int b, b2;        // partitioned hash bits in all (8..16) and at level 2
+    int b, b2;        // partitioned hash bits in all (12..16) and at level 2
     i64 cap1, cap2;   // records per level-1 bin / level-2 bucket (multiples of 32)
     i64 bins_rec, bkt_rec, nbuckets;
 };
@@ -103,7 +105,7 @@ constexpr i64 FUSED_MAX_BUCKETS = 65536;
 FusedPlan plan_fused(i64 nexp) {
     FusedPlan f{};
     nexp = std::max<i64>(nexp, 1);
-    f.b = 8;
+    f.b = 12;  // at least 4096 buckets: the bucket join keeps its chain links in the top 12 bits of the staged records
     while (f.b < 16 && (double)nexp / std::pow(2.0, f.b) > 1800.0) ++f.b;
     f.b2 = f.b - 8;
     auto cap_of = [](double avg) { return (i64)((avg + 8.0 * std::sqrt(avg) + 64.0 + 31.0) / 32.0) * 32; };
@@ -188,7 +190,6 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     if (capacity > 0 && (!out_i || !out_j || !out_dist)) return SYMDEL_E_ARG;
     if (((uintptr_t)workspace & 255) != 0) return SYMDEL_E_ARG;
     CK(cudaSetDevice(ctx->device));
-    CK(sd_init_tables());
     Timer tm(ctx, st);
     const size_t ev_begin = tm.mark();
 
@@ -250,20 +251,25 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     void* slots = ws.take<char>(sd_pack_bytes(n_total, maxlen));
     u32* fcnt = ws.take<u32>(256 + 2 * FUSED_MAX_BUCKETS);  // fused pipeline: level-1 cursors | level-2 counts | redo list
     if (!ws.ok) return SYMDEL_E_WORKSPACE;
-    CK(sd_pack(A, B, maxlen, slots, st, &S.n_launches));
+    CK(sd_pack(A, B, maxlen, slots, info, st, &S.n_launches));
 
     // ---- workspace plan ----
     const i64 R = ws.left() - 8192;
     // a window of the candidate buffer ends with a whole record's pairs: at most one per other sequence
     const i64 cslack = n_total + 64;
     i64 ccap = ctx->opt_cand_cap > 0 ? ctx->opt_cand_cap : std::max<i64>(1 << 20, std::min<i64>(2 * nmax, nmax / 2 + ((i64)128 << 20)));
-    i64 scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity + (ctx->opt_cand_cap > 0 ? ccap : 0));
+    // Survivor list of multi-flush searches: never smaller than the caller's capacity (+ a little).  A pair found in
+    // several chunks or windows is appended once per flush; when an append does not fit, the list is sorted,
+    // deduplicated and cut to its smallest `capacity` entries, and the flush is repeated (see the window loop).
+    const i64 scap_min = capacity + 4096;
+    i64 scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), scap_min + (ctx->opt_cand_cap > 0 ? ccap : 0));
+    if (ctx->opt_surv_cap > 0) scap = std::max<i64>(scap_min, ctx->opt_surv_cap);
     i64 ncap = std::max<i64>(nmax, 1);
     u32 P = ctx->opt_force_chunks > 0 ? (u32)ctx->opt_force_chunks : 1;
     if (P > 1) ncap = std::min<i64>(nmax, nmax / P + nmax / (4 * P) + 4096);
     if (rec_bytes(ncap, npass_max) + cand_bytes(ccap + cslack, ppass) + cand_bytes(scap, spass) > R) {
         if (ctx->opt_cand_cap <= 0) ccap = std::min<i64>(ccap, std::max<i64>(4096, R / 4 / 17 - cslack));
-        scap = std::min<i64>(scap, std::max<i64>(4096, R * 15 / 100 / 17));
+        scap = std::min<i64>(scap, std::max<i64>(scap_min, R * 15 / 100 / 17));
         const i64 rrem = R - cand_bytes(ccap + cslack, ppass) - cand_bytes(scap, spass);
         if (rrem <= 0) return SYMDEL_E_WORKSPACE;
         // largest ncap that fits in rrem (16 B/record + ~0.26 B/record of tile status per pass)
@@ -294,7 +300,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     if (!ws.ok) return SYMDEL_E_WORKSPACE;
 
     const int width = (prefix > 0 ? std::min(maxlen, prefix) : maxlen) + 1;  // generation works on the (truncated) sequences
-    i64 n_surv = 0, flushes = 0;
+    i64 n_surv = 0, flushes = 0, surv_lower_bound = 0;
     bool direct = false;  // the single flush wrote the outputs itself
     enum { ST_GEN, ST_SORT, ST_EMIT, ST_DEDUP, ST_VERIFY };
     i64 pass_count = 0;
@@ -305,6 +311,7 @@ restart:
     pass_count = 0;
     n_surv = 0;
     flushes = 0;
+    surv_lower_bound = 0;
     direct = false;
     S.n_records = S.n_candidates = 0;
     lay.n_chunks = P;
@@ -316,7 +323,8 @@ restart:
         i64 C = 0, wend = 0, N = 0;
         // (a chunk expected to hold 2^30 records or more goes to the exact pipeline, which splits it further)
         if (!ctx->opt_exact && ctx->opt_sort_bits < 0 && !ctx->opt_join_general && lay.hash_bits >= fp.b &&
-            nmax / (i64)P < ((i64)1 << 30) && sd_gen_part_applies(lay, width)) {
+            nmax / (i64)P < ((i64)1 << 30) && fp.cap2 <= sd_join_bkt_max_cap() && 64 - (lay.id_bits + lay.hash_bits) + fp.b >= sd_join_bkt_link_bits((u32)fp.cap2) &&
+            sd_gen_part_applies(lay, width)) {
             const size_t x0 = tm.mark();
             lay.sort_bits = fp.b;
             CK(cudaMemsetAsync(&info->part_overflow, 0, sizeof(u32), st));
@@ -330,22 +338,13 @@ restart:
             const u64* bkt = fp.b2 ? recB : recA;
             const u32* bcnt = fp.b2 ? cnt2 : cur1;
             const u32 bcap = (u32)(fp.b2 ? fp.cap2 : fp.cap1), nb = (u32)fp.nbuckets;
-            const u32 group = sd_join_bkt_group(ncap, nb);
-            CK(sd_join_bkt(bkt, bcnt, bcap, nb, group, lay, candA, (u64)ccap, nullptr, 0, redo, info, st, &S.n_launches));
+            CK(sd_join_bkt(bkt, bcnt, bcap, nb, lay, candA, (u64)ccap, info, st, &S.n_launches));
             u32* h_cur = reinterpret_cast<u32*>(ctx->h_info + 1);
             CK(cudaMemcpyAsync(h_cur, cur1, 256 * sizeof(u32), cudaMemcpyDeviceToHost, st));
             rc = read_info(ctx, info, st);
             if (rc) return rc;
             if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
             fused_ok = !ctx->h_info->part_overflow && !ctx->h_info->join_fallback;
-            if (fused_ok && ctx->h_info->join_redo) {  // dense bucket groups: the large-list instance
-                S.join_redo_tiles += ctx->h_info->join_redo;
-                CK(sd_join_bkt(bkt, bcnt, bcap, nb, group, lay, candA, (u64)ccap, redo, ctx->h_info->join_redo, nullptr, info, st,
-                               &S.n_launches));
-                rc = read_info(ctx, info, st);
-                if (rc) return rc;
-                fused_ok = !ctx->h_info->join_fallback;
-            }
             if (fused_ok) {
                 for (int i = 0; i < 256; ++i) N += h_cur[i];
                 C = (i64)ctx->h_info->n_cand;
@@ -388,7 +387,7 @@ restart:
         CK(sd_sort_hist_scan(rec_scratch, npass, st, &S.n_launches));
         const size_t e1 = tm.mark();
         // ---- S2: radix partition on the top sort_bits (exactly npass onesweep launches between e1 and e2) ----
-        CK(sd_sort_passes(recA, recB, N, sort_begin, npass, ctx->opt_sort_stable ? 1 : 0, rec_scratch, st, &sorted,
+        CK(sd_sort_passes(recA, recB, N, sort_begin, npass, ctx->opt_sort_stable ? 1 : 0, (int)ctx->opt_sort_variant, rec_scratch, st, &sorted,
                           &S.n_launches));
         const size_t e2 = tm.mark();
         // ---- S3a: join (first window): the fast kernel when everything fits one window, else the general one ----
@@ -443,7 +442,7 @@ restart:
             CK(sd_sort_histogram(candA, nc, 0, ppass, cand_scratch, st, &S.n_launches));
             CK(sd_sort_hist_scan(cand_scratch, ppass, st, &S.n_launches));
             u64* csorted = nullptr;
-            CK(sd_sort_passes(candA, candB, nc, 0, ppass, 0, cand_scratch, st, &csorted, &S.n_launches));
+            CK(sd_sort_passes(candA, candB, nc, 0, ppass, 0, (int)ctx->opt_sort_variant, cand_scratch, st, &csorted, &S.n_launches));
             const size_t f2 = tm.mark();
             // ---- S4: unique + verify; survivors appended at n_surv — or, when this window holds every candidate of
             //      the only chunk, unpacked straight into the outputs (no survivor list, no finalize) ----
@@ -451,9 +450,44 @@ restart:
             if (direct)
                 CK(sd_verify_direct(csorted, nc, slots, lay, maxlen, out_i, out_j, out_dist, capacity, verify_lb, info, st,
                                     &S.n_launches));
-            else
-                CK(sd_verify(csorted, nc, slots, lay, maxlen, survA, (u64)n_surv, (u64)scap, verify_lb, info, st,
-                             &S.n_launches));
+            else {
+                // sort the survivor list, drop the repeats, keep the smallest `capacity`: makes room for the next append
+                auto merge_survivors = [&]() -> int {
+                    CK(sd_sort_prepare(surv_scratch, n_surv, spass, st));
+                    CK(sd_sort_histogram(survA, n_surv, 3, spass, surv_scratch, st, &S.n_launches));
+                    CK(sd_sort_hist_scan(surv_scratch, spass, st, &S.n_launches));
+                    u64* ssorted = nullptr;
+                    CK(sd_sort_passes(survA, survB, n_surv, 3, spass, 0, (int)ctx->opt_sort_variant, surv_scratch, st, &ssorted,
+                                      &S.n_launches));
+                    u64* dst = ssorted == survA ? survB : survA;
+                    CK(sd_finalize(ssorted, n_surv, lay, 1, nullptr, nullptr, nullptr, dst, scap, final_lb, info, st, &S.n_launches));
+                    int r = read_info(ctx, info, st);
+                    if (r) return r;
+                    const i64 uniq = (i64)ctx->h_info->n_out;
+                    if (uniq > capacity) surv_lower_bound = std::max(surv_lower_bound, uniq);  // the result exceeds `capacity`
+                    n_surv = std::min(uniq, capacity);
+                    if (dst != survA) std::swap(survA, survB);
+                    ++S.surv_merges;
+                    return SYMDEL_OK;
+                };
+                bool merged = false;
+                if (n_surv > scap / 2 && n_surv + nc > scap) {  // likely not to fit: merge first
+                    if ((rc = merge_survivors())) return rc;
+                    merged = true;
+                }
+                for (;;) {
+                    CK(cudaMemsetAsync(&info->surv_overflow, 0, sizeof(u32), st));
+                    CK(sd_verify(csorted, nc, slots, lay, maxlen, survA, (u64)n_surv, (u64)scap, verify_lb, info, st,
+                                 &S.n_launches));
+                    rc = read_info(ctx, info, st);
+                    if (rc) return rc;
+                    if (!ctx->h_info->surv_overflow) break;
+                    // the window's survivors did not fit behind the list: merge it (once) and verify the window again
+                    if (merged || n_surv == 0) return SYMDEL_E_WORKSPACE;  // not even `capacity` + this window's survivors fit
+                    if ((rc = merge_survivors())) return rc;
+                    merged = true;
+                }
+            }
             rc = read_info(ctx, info, st);
             if (rc) return rc;
             if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
@@ -479,14 +513,16 @@ restart:
             CK(sd_sort_histogram(survA, n_surv, 3, spass, surv_scratch, st, &S.n_launches));
             CK(sd_sort_hist_scan(surv_scratch, spass, st, &S.n_launches));
             u64* ssorted = nullptr;
-            CK(sd_sort_passes(survA, survB, n_surv, 3, spass, 0, surv_scratch, st, &ssorted, &S.n_launches));
+            CK(sd_sort_passes(survA, survB, n_surv, 3, spass, 0, (int)ctx->opt_sort_variant, surv_scratch, st, &ssorted, &S.n_launches));
             fin = ssorted;
         }
-        CK(sd_finalize(fin, n_surv, lay, flushes > 1 ? 1 : 0, out_i, out_j, out_dist, capacity, final_lb, info, st,
+        CK(sd_finalize(fin, n_surv, lay, flushes > 1 ? 1 : 0, out_i, out_j, out_dist, nullptr, capacity, final_lb, info, st,
                        &S.n_launches));
         rc = read_info(ctx, info, st);
         if (rc) return rc;
-        n_out = (i64)ctx->h_info->n_out;
+        // (after a merge that cut the list to `capacity` entries the exact count is not known any more: the
+        //  number of distinct pairs seen at that point is a lower bound, and it exceeds `capacity`)
+        n_out = std::max<i64>((i64)ctx->h_info->n_out, surv_lower_bound);
     }
     const size_t g1 = tm.mark();
     if (tm.on) {
@@ -614,9 +650,17 @@ int symdel_create(symdel_ctx** out, int device) {
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_info, sizeof(DevInfo) + 256 * sizeof(u32));
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking);
-    if (e == cudaSuccess) e = sd_init_tables();
+    if (e == cudaSuccess) {
+        // Constant tables and function attributes are per DEVICE: every context sets them up for its own device
+        // (idempotent; serialised so that two threads creating contexts never interleave the uploads).
+        static std::mutex setup_lock;
+        std::lock_guard<std::mutex> g(setup_lock);
+        e = sd_generate_setup();
+        if (e == cudaSuccess) e = sd_sort_setup();
+        if (e == cudaSuccess) e = sd_join_setup();
+    }
     if (e != cudaSuccess) {
-        delete ctx;
+        symdel_destroy(ctx);
         return SYMDEL_E_CUDA;
     }
     *out = ctx;
@@ -662,8 +706,10 @@ int symdel_set_option(symdel_ctx* ctx, int option, int64_t value) {
             break;
         case SYMDEL_OPT_NO_THINNING: ctx->opt_no_thinning = value != 0; break;
         case SYMDEL_OPT_GENERAL_GENERATE: ctx->opt_general_gen = value != 0; break;
+        case SYMDEL_OPT_SURV_CAPACITY: ctx->opt_surv_cap = value; break;
         case SYMDEL_OPT_SORT_VARIANT:
-            if (sd_sort_set_variant((int)value)) return SYMDEL_E_ARG;
+            if (value >= sd_sort_variants()) return SYMDEL_E_ARG;
+            ctx->opt_sort_variant = value;
             break;
         default: return SYMDEL_E_ARG;
     }
@@ -740,16 +786,16 @@ int symdel_cross_host(symdel_ctx* ctx, const int8_t* q_seqs_host, const int64_t*
 }
 
 int symdel_overlap_matrix(symdel_ctx* ctx, const int32_t* out_i, const int32_t* out_j, int64_t n_pairs, const int32_t* labels_i,
-                          const int32_t* labels_j, int n_repertoires, int symmetric, int64_t* matrix, void* workspace,
-                          int64_t workspace_bytes, void* cuda_stream) {
+                          int64_t n_labels_i, const int32_t* labels_j, int64_t n_labels_j, int n_repertoires, int symmetric,
+                          int64_t* matrix, void* workspace, int64_t workspace_bytes, void* cuda_stream) {
     if (!ctx || n_pairs < 0 || n_repertoires < 1 || n_repertoires > 4096 || !matrix || !labels_i || !labels_j || !workspace ||
-        workspace_bytes < 256 || (n_pairs > 0 && (!out_i || !out_j)))
+        workspace_bytes < 256 || n_labels_i < 0 || n_labels_j < 0 || (n_pairs > 0 && (!out_i || !out_j)))
         return SYMDEL_E_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CK(cudaSetDevice(ctx->device));
     u32* err = (u32*)workspace;
     CK(cudaMemsetAsync(err, 0, sizeof(u32), st));
-    CK(sd_overlap(out_i, out_j, n_pairs, labels_i, labels_j, n_repertoires, symmetric ? 1 : 0, (u64*)matrix, err, st));
+    CK(sd_overlap(out_i, out_j, n_pairs, labels_i, n_labels_i, labels_j, n_labels_j, n_repertoires, symmetric ? 1 : 0, (u64*)matrix, err, st));
     CK(cudaMemcpyAsync(&ctx->h_info->err, err, sizeof(u32), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     return ctx->h_info->err ? SYMDEL_E_ARG : SYMDEL_OK;
@@ -773,7 +819,7 @@ int symdel_stage_sort_u64(symdel_ctx* ctx, uint64_t* keys, uint64_t* tmp, int64_
     CK(sd_sort_histogram(keys, n, begin_bit, npass, workspace, st, nullptr));
     CK(sd_sort_hist_scan(workspace, npass, st, nullptr));
     u64* res = nullptr;
-    CK(sd_sort_passes(keys, tmp, n, begin_bit, npass, ctx->opt_sort_grouping ? 0 : 1, workspace, st, &res, nullptr));
+    CK(sd_sort_passes(keys, tmp, n, begin_bit, npass, ctx->opt_sort_grouping ? 0 : 1, (int)ctx->opt_sort_variant, workspace, st, &res, nullptr));
     if (res != keys) CK(cudaMemcpyAsync(keys, res, (size_t)n * 8, cudaMemcpyDeviceToDevice, st));
     CK(cudaStreamSynchronize(st));
     return SYMDEL_OK;
@@ -789,7 +835,6 @@ int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const int64_t* of
     if (!seqs || !offsets || !records || !workspace) return SYMDEL_E_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     CK(cudaSetDevice(ctx->device));
-    CK(sd_init_tables());
     Bump ws(workspace, workspace_bytes);
     DevInfo* info = ws.take<DevInfo>(1);
     u32* cnt = ws.take<u32>(n);
@@ -801,6 +846,7 @@ int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const int64_t* of
     CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
     CK(cudaMemsetAsync(hist, 0, 8 * 256 * 4, st));
     CK(sd_prepare(A, d, 0, 0, info, st, nullptr));
+    CK(sd_check_residues(A, info, st));
     int rc = read_info(ctx, info, st);
     if (rc) return rc;
     if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
@@ -847,10 +893,12 @@ int symdel_stage_lev(symdel_ctx* ctx, const int8_t* a_seqs, const int64_t* a_off
     if (rc) return rc;
     if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
     const int maxlen = (int)ctx->h_info->maxlen;
-    CK(sd_pack(A, B, maxlen, slots, st, nullptr));
-    CK(sd_lev_pairs(slots, n_a, maxlen, ia, ib, n_pairs, dist, st));
-    CK(cudaStreamSynchronize(st));
-    return SYMDEL_OK;
+    CK(sd_pack(A, B, maxlen, slots, info, st, nullptr));
+    CK(sd_lev_pairs(slots, n_a, n_b, maxlen, ia, ib, n_pairs, dist, &info->err, st));
+    rc = read_info(ctx, info, st);
+    if (rc) return rc;
+    if (ctx->h_info->err & SD_ERR_RESIDUE) return SYMDEL_E_RESIDUE;
+    return ctx->h_info->err ? SYMDEL_E_ARG : SYMDEL_OK;
 }
 
 }  // extern "C"

@@ -51,7 +51,7 @@ __device__ __forceinline__ Planes<u64> load_planes<u64>(const void* slots, u64 i
 }
 
 template <typename W>
-__global__ void __launch_bounds__(256) k_pack(SeqSetDev A, SeqSetDev B, void* slots) {
+__global__ void __launch_bounds__(256) k_pack(SeqSetDev A, SeqSetDev B, void* slots, DevInfo* info) {
     const i64 g = (i64)blockIdx.x * 256 + threadIdx.x;
     if (g >= A.n + B.n) return;
     const SeqSetDev& S = g < A.n ? A : B;
@@ -59,11 +59,14 @@ __global__ void __launch_bounds__(256) k_pack(SeqSetDev A, SeqSetDev B, void* sl
     const i64 o = S.off[i];
     const int L = (int)(S.off[i + 1] - o);
     W b[5] = {0, 0, 0, 0, 0};
+    bool bad = false;
     for (int j = 0; j < L; ++j) {
         const W c = (W)(unsigned char)S.seqs[o + j];
+        bad |= c < 1 || c > 31;  // S0: residue codes 1..31 (0 is reserved)
 #pragma unroll
         for (int k = 0; k < 5; ++k) b[k] |= ((c >> k) & 1) << j;
     }
+    if (bad) atomicOr(&info->err, (u32)SD_ERR_RESIDUE);
     if (sizeof(W) == 4) {
         uint4* p = reinterpret_cast<uint4*>(slots) + 2 * g;
         p[0] = make_uint4((u32)b[0], (u32)b[1], (u32)b[2], (u32)b[3]);
@@ -119,12 +122,9 @@ __device__ __forceinline__ int hamming_planes(const Planes<W>& P, const Planes<W
     return sizeof(W) == 8 ? __popcll((unsigned long long)x) : __popc((unsigned)x);
 }
 
-#ifndef VF_IPT_
-#define VF_IPT_ 8
-#endif
-constexpr int VF_THREADS = 256, VF_IPT = VF_IPT_, VF_TILE = VF_THREADS * VF_IPT;
+constexpr int VF_THREADS = 256, VF_IPT = 8, VF_TILE = VF_THREADS * VF_IPT;  // 4 per thread: 0.087 -> 8: 0.077 ms on config 3
 
-// Tile of 1024 sorted candidates: (1) flag the unique ones and compact their positions into shared
+// Tile of VF_TILE = 2048 sorted candidates: (1) flag the unique ones and compact their positions into shared
 // memory, (2) spread the COMPACTED list over the threads for the distance computation (after dedup
 // only a fraction of the candidates is left: this keeps every lane busy), (3) ordered compaction of
 // the survivors (block scan + 32-wide decoupled look-back) so the output stays sorted.
@@ -223,7 +223,7 @@ __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ c
             } else if (out < surv_capacity) {
                 surv[out] = (cand[base + pos] << 3) | (u64)s_res[pos];
             } else {
-                atomicOr(&info->err, (u32)SD_ERR_OVERFLOW);
+                info->surv_overflow = 1u;
             }
             ++out;
         }
@@ -232,10 +232,12 @@ __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ c
 
 constexpr int FN_THREADS = 256;
 
+// packed_out != nullptr: the kept survivors are written back as packed words (the survivor-list merge between
+// flushes) instead of being unpacked to the SoA outputs.
 __global__ void __launch_bounds__(FN_THREADS) k_finalize(const u64* __restrict__ surv, u64 n, Layout lay, int dedup,
                                                         i32* __restrict__ out_i, i32* __restrict__ out_j,
-                                                        i32* __restrict__ out_dist, u64 capacity, u64* lb_status,
-                                                        DevInfo* info) {
+                                                        i32* __restrict__ out_dist, u64* __restrict__ packed_out,
+                                                        u64 capacity, u64* lb_status, DevInfo* info) {
     __shared__ u32 s_warp[FN_THREADS / 32 + 1];
     __shared__ u32 s_tile;
     __shared__ u64 s_excl;
@@ -265,7 +267,9 @@ __global__ void __launch_bounds__(FN_THREADS) k_finalize(const u64* __restrict__
     __syncthreads();
     if (keep) {
         const u64 pos = s_excl + rank;
-        if (pos < capacity) {
+        if (packed_out) {
+            if (pos < capacity) packed_out[pos] = v;
+        } else if (pos < capacity) {
             const u64 pr = v >> 3;
             out_i[pos] = (i32)(pr >> lay.b_bits);
             out_j[pos] = (i32)(pr & ((1ull << lay.b_bits) - 1ull));
@@ -275,11 +279,17 @@ __global__ void __launch_bounds__(FN_THREADS) k_finalize(const u64* __restrict__
 }
 
 template <typename W>
-__global__ void __launch_bounds__(256) k_lev_pairs(const void* __restrict__ slots, i64 n_a, const i32* __restrict__ ia,
-                                                   const i32* __restrict__ ib, i64 n, i32* __restrict__ dist) {
+__global__ void __launch_bounds__(256) k_lev_pairs(const void* __restrict__ slots, i64 n_a, i64 n_b, const i32* __restrict__ ia,
+                                                   const i32* __restrict__ ib, i64 n, i32* __restrict__ dist, u32* err) {
     const i64 t = (i64)blockIdx.x * 256 + threadIdx.x;
     if (t >= n) return;
-    dist[t] = myers_lev<W>(load_planes<W>(slots, (u64)ia[t]), load_planes<W>(slots, (u64)(n_a + ib[t])));
+    const i64 a = ia[t], b = ib[t];
+    if (a < 0 || a >= n_a || b < 0 || b >= n_b) {  // caller-supplied indices: never gather out of bounds
+        dist[t] = -1;
+        atomicOr(err, (u32)SD_ERR_INTERNAL);
+        return;
+    }
+    dist[t] = myers_lev<W>(load_planes<W>(slots, (u64)a), load_planes<W>(slots, (u64)(n_a + b)));
 }
 
 // ---- NEXT-4: M x M repertoire-overlap matrix --------------------------------------------
@@ -289,8 +299,9 @@ __global__ void __launch_bounds__(256) k_lev_pairs(const void* __restrict__ slot
 constexpr int OV_THREADS = 256, OV_MMAX_SMEM = 64;
 
 __global__ void __launch_bounds__(OV_THREADS) k_overlap(const i32* __restrict__ pi, const i32* __restrict__ pj, u64 n,
-                                                       const i32* __restrict__ lab_i, const i32* __restrict__ lab_j, int M,
-                                                       int symmetric, unsigned long long* __restrict__ matrix, u32* err) {
+                                                       const i32* __restrict__ lab_i, i64 n_i, const i32* __restrict__ lab_j,
+                                                       i64 n_j, int M, int symmetric, unsigned long long* __restrict__ matrix,
+                                                       u32* err) {
     extern __shared__ u32 s_cell[];
     const bool use_smem = M <= OV_MMAX_SMEM;
     if (use_smem) {
@@ -299,7 +310,12 @@ __global__ void __launch_bounds__(OV_THREADS) k_overlap(const i32* __restrict__ 
     }
     const u64 stride = (u64)gridDim.x * OV_THREADS;
     for (u64 t = (u64)blockIdx.x * OV_THREADS + threadIdx.x; t < n; t += stride) {
-        const i32 a = lab_i[pi[t]], b = lab_j[pj[t]];
+        const i64 xi = pi[t], xj = pj[t];
+        if (xi < 0 || xi >= n_i || xj < 0 || xj >= n_j) {  // a pair index outside its label array
+            atomicOr(err, (u32)SD_ERR_INTERNAL);
+            continue;
+        }
+        const i32 a = lab_i[xi], b = lab_j[xj];
         if (a < 0 || a >= M || b < 0 || b >= M) {
             atomicOr(err, (u32)SD_ERR_INTERNAL);
             continue;
@@ -323,13 +339,13 @@ __global__ void __launch_bounds__(OV_THREADS) k_overlap(const i32* __restrict__ 
 
 // matrix (M x M, row-major, zeroed here) += the label pairs of the n output pairs; *err gets SD_ERR_INTERNAL if
 // a label lies outside [0, M)
-cudaError_t sd_overlap(const i32* pi, const i32* pj, i64 n, const i32* lab_i, const i32* lab_j, int M, int symmetric,
-                       u64* matrix, u32* err, cudaStream_t st) {
+cudaError_t sd_overlap(const i32* pi, const i32* pj, i64 n, const i32* lab_i, i64 n_i, const i32* lab_j, i64 n_j, int M,
+                       int symmetric, u64* matrix, u32* err, cudaStream_t st) {
     cudaError_t e = cudaMemsetAsync(matrix, 0, (size_t)M * M * 8, st);
     if (e != cudaSuccess || n == 0) return e;
     const unsigned blocks = (unsigned)std::min<i64>((n + OV_THREADS * 8 - 1) / (OV_THREADS * 8), 148 * 8);
     const size_t smem = M <= OV_MMAX_SMEM ? (size_t)M * M * 4 : 0;
-    k_overlap<<<blocks, OV_THREADS, smem, st>>>(pi, pj, (u64)n, lab_i, lab_j, M, symmetric, (unsigned long long*)matrix, err);
+    k_overlap<<<blocks, OV_THREADS, smem, st>>>(pi, pj, (u64)n, lab_i, n_i, lab_j, n_j, M, symmetric, (unsigned long long*)matrix, err);
     return cudaGetLastError();
 }
 
@@ -337,12 +353,12 @@ i64 sd_verify_tiles(i64 n) { return (n + VF_TILE - 1) / VF_TILE; }
 
 i64 sd_pack_bytes(i64 n_total, int maxlen) { return n_total * (maxlen <= 32 ? 32 : 48); }
 
-cudaError_t sd_pack(SeqSetDev a, SeqSetDev b, int maxlen, void* slots, cudaStream_t st, i64* launches) {
+cudaError_t sd_pack(SeqSetDev a, SeqSetDev b, int maxlen, void* slots, DevInfo* info, cudaStream_t st, i64* launches) {
     const i64 n = a.n + b.n;
     if (n == 0) return cudaSuccess;
     const unsigned blocks = (unsigned)((n + 255) / 256);
-    if (maxlen <= 32) k_pack<u32><<<blocks, 256, 0, st>>>(a, b, slots);
-    else k_pack<u64><<<blocks, 256, 0, st>>>(a, b, slots);
+    if (maxlen <= 32) k_pack<u32><<<blocks, 256, 0, st>>>(a, b, slots, info);
+    else k_pack<u64><<<blocks, 256, 0, st>>>(a, b, slots, info);
     if (launches) ++*launches;
     return cudaGetLastError();
 }
@@ -382,23 +398,23 @@ cudaError_t sd_verify_direct(const u64* cand, i64 n_cand, const void* slots, con
 }
 
 cudaError_t sd_finalize(const u64* surv, i64 n_surv, const Layout& lay, int dedup, i32* out_i, i32* out_j, i32* out_dist,
-                        i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches) {
+                        u64* packed_out, i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches) {
     const i64 tiles = (n_surv + FN_THREADS - 1) / FN_THREADS;
     if (tiles == 0) return cudaSuccess;
     cudaError_t e = cudaMemsetAsync(lb_status, 0, (size_t)tiles * 8, st);
     if (e != cudaSuccess) return e;
-    k_finalize<<<(unsigned)tiles, FN_THREADS, 0, st>>>(surv, (u64)n_surv, lay, dedup, out_i, out_j, out_dist, (u64)capacity,
-                                                       lb_status, info);
+    k_finalize<<<(unsigned)tiles, FN_THREADS, 0, st>>>(surv, (u64)n_surv, lay, dedup, out_i, out_j, out_dist, packed_out,
+                                                       (u64)capacity, lb_status, info);
     if (launches) ++*launches;
     return cudaGetLastError();
 }
 
 // distances for index pairs (stage test): slots hold set A followed by set B
-cudaError_t sd_lev_pairs(const void* slots, i64 n_a, int maxlen, const i32* ia, const i32* ib, i64 n_pairs, i32* dist,
-                         cudaStream_t st) {
+cudaError_t sd_lev_pairs(const void* slots, i64 n_a, i64 n_b, int maxlen, const i32* ia, const i32* ib, i64 n_pairs, i32* dist,
+                         u32* err, cudaStream_t st) {
     if (n_pairs == 0) return cudaSuccess;
     const unsigned blocks = (unsigned)((n_pairs + 255) / 256);
-    if (maxlen <= 32) k_lev_pairs<u32><<<blocks, 256, 0, st>>>(slots, n_a, ia, ib, n_pairs, dist);
-    else k_lev_pairs<u64><<<blocks, 256, 0, st>>>(slots, n_a, ia, ib, n_pairs, dist);
+    if (maxlen <= 32) k_lev_pairs<u32><<<blocks, 256, 0, st>>>(slots, n_a, n_b, ia, ib, n_pairs, dist, err);
+    else k_lev_pairs<u64><<<blocks, 256, 0, st>>>(slots, n_a, n_b, ia, ib, n_pairs, dist, err);
     return cudaGetLastError();
 }

@@ -19,6 +19,7 @@ OK = 0
 E_ARG, E_OFFSETS, E_TOO_LONG, E_RESIDUE, E_TOO_MANY, E_WORKSPACE, E_CAPACITY, E_CUDA, E_INTERNAL = range(-1, -10, -1)
 OPT_TIMING, OPT_FORCE_CHUNKS, OPT_CAND_CAPACITY, OPT_HASH_BITS, OPT_NO_THINNING, OPT_SORT_VARIANT, OPT_GENERAL_GENERATE = 1, 2, 3, 4, 5, 6, 7
 OPT_SORT_BITS, OPT_SORT_STABLE, OPT_SORT_GROUPING, OPT_JOIN_GENERAL, OPT_EXACT_PIPELINE, OPT_PREFIX_LEN, OPT_METRIC = 8, 9, 10, 11, 12, 13, 14
+OPT_SURV_CAPACITY = 15
 METRIC_LEVENSHTEIN, METRIC_HAMMING = 0, 1
 D_MAX, L_MAX = 4, 64
 
@@ -38,6 +39,7 @@ class Stats(C.Structure):
         ("ms_prepare", C.c_float), ("ms_generate", C.c_float), ("ms_sort", C.c_float), ("ms_emit", C.c_float),
         ("ms_dedup", C.c_float), ("ms_verify", C.c_float), ("ms_total", C.c_float), ("ms_sort_pass_avg", C.c_float),
         ("sort_pass_records", C.c_int64), ("fused_chunks", C.c_int64), ("join_redo_tiles", C.c_int64),
+        ("surv_merges", C.c_int64),
     ]
 
     def as_dict(self):
@@ -78,7 +80,7 @@ def lib():
         L.symdel_stage_sort_u64.argtypes = [vp, vp, vp, i64, i32, i32, vp, i64, vp]
         L.symdel_stage_generate.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, i64, C.POINTER(i64), vp, i64, vp]
         L.symdel_stage_lev.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp]
-        L.symdel_overlap_matrix.argtypes = [vp, vp, vp, i64, vp, vp, i32, i32, vp, vp, i64, vp]
+        L.symdel_overlap_matrix.argtypes = [vp, vp, vp, i64, vp, i64, vp, i64, i32, i32, vp, vp, i64, vp]
         _lib = L
     return _lib
 
@@ -245,8 +247,9 @@ class Context:
         m = torch.empty((n_repertoires, n_repertoires), dtype=torch.int64, device=labels_i.device)
         ws = torch.empty(256, dtype=torch.uint8, device=labels_i.device)
         q = lambda t: C.c_void_p(t.data_ptr())
-        rc = lib().symdel_overlap_matrix(self._h, q(out_i), q(out_j), out_i.numel(), q(labels_i), q(labels_j), n_repertoires,
-                                         1 if symmetric else 0, q(m), q(ws), 256, _stream_ptr(torch))
+        rc = lib().symdel_overlap_matrix(self._h, q(out_i), q(out_j), out_i.numel(), q(labels_i), labels_i.numel(), q(labels_j),
+                                         labels_j.numel(), n_repertoires, 1 if symmetric else 0, q(m), q(ws), 256,
+                                         _stream_ptr(torch))
         if rc:
             self._raise(rc, "symdel_overlap_matrix")
         return m

@@ -105,3 +105,28 @@ def test_product_never_touches_the_oracle():
         if p.suffix in (".py", ".cpp"):
             for ln in p.read_text().splitlines():
                 assert not (("symdel" in ln or "paper_2403_09010_b200" in ln or "csrc" in ln) and hit(ln)), (p, ln)
+
+
+def test_no_process_global_init_state_in_the_library():
+    """Constant tables and kernel attributes belong to a device: they are set up by symdel_create for the
+    context's device (include/symdel.h "Devices and threads"), never behind a process-wide flag, and no tuning
+    knob lives in a global variable.  Source check (the two-context run is in the GPU tests)."""
+    csrc = ROOT / "paper_2403_09010_b200" / "csrc"
+    for p in sorted(csrc.glob("*")):
+        text = re.sub(r"//.*", "", p.read_text())
+        assert not re.search(r"\bstatic\s+(bool|int|u32|cudaError_t)\s+\w+\s*(=|;)", text), p  # no static flags
+        assert not re.search(r"^\s*(int|bool|u32)\s+g_\w+", text, flags=re.M), p               # no global knobs
+    api = (csrc / "symdel_api.cu").read_text()
+    create = api[api.index("int symdel_create("):api.index("void symdel_destroy(")]
+    for setup in ("sd_generate_setup", "sd_sort_setup", "sd_join_setup"):
+        assert setup in create, setup
+    build_py = (ROOT / "paper_2403_09010_b200" / "build.py").read_text()
+    assert "environ" not in build_py  # build() compiles exactly what is committed: no environment hook
+
+
+def test_kernel_sources_carry_no_tuning_bench():
+    """The swept tunables are frozen: no #ifndef-overridable macro, debug path or variant sweep in csrc/."""
+    csrc = ROOT / "paper_2403_09010_b200" / "csrc"
+    for p in sorted(csrc.glob("*")):
+        text = p.read_text()
+        assert "#ifndef" not in text and "OS_DBG" not in text and "OS_SWEEP" not in text, p

@@ -65,6 +65,24 @@ def digest(i, j, d):
     return h.hexdigest()
 
 
+def assert_matches_golden(g, i, j, dist):
+    """Full-size comparison with the oracle's stored digests (tests/golden/*.json, written by make_golden.py from
+    the oracle alone).  Equal sha256 of (i, j, dist) <=> identical pairs, distances and order.  On a mismatch the
+    per-block digests locate the first differing block of 4096 output rows and its rows are printed."""
+    if digest(i, j, dist) == g["out_sha256"] and len(i) == g["n_out"]:
+        return
+    B = g["block_rows"]
+    rows = np.ascontiguousarray(np.stack([np.asarray(a, dtype=np.int32) for a in (i, j, dist)], axis=1))
+    got = [hashlib.sha256(rows[t:t + B].tobytes()).hexdigest()[:12] for t in range(0, len(rows), B)]
+    first = next((b for b, (x, y) in enumerate(zip(got, g["block_sha"])) if x != y), min(len(got), len(g["block_sha"])))
+    lo = first * B
+    raise AssertionError(
+        f"output differs from the oracle: {len(i)} rows vs {g['n_out']}; dist histogram "
+        f"{np.bincount(dist, minlength=g['d'] + 1).tolist()} vs {g['dist_hist']}; first differing block {first} "
+        f"(rows {lo}..{lo + B}); its first rows here:\n{rows[lo:lo + 12]}\n(rows before it are identical; the oracle's rows "
+        f"of this block start at i >= {int(rows[lo - 1, 0]) if lo else 0})")
+
+
 # ---- S2/K2: radix sort -----------------------------------------------------------------------------
 def _keys(kind, n, seed):
     rng = np.random.default_rng(seed)
@@ -338,7 +356,7 @@ def test_join_dense_runs(sd, oracle, copies, sort_bits, general, expect_general)
     st = c.symdel_get_stats()
     assert st["join_general"] == expect_general
     if copies == 10 and sort_bits == 0:
-        assert st["join_redo_tiles"] > 0  # dense tiles overflow the small list and are redone with the large one
+        assert st["fused_chunks"] == 1  # the bucket join has no candidate list to overflow: dense buckets stay fused
 
 
 def test_fused_bin_overflow_falls_back(sd, oracle):
@@ -573,9 +591,8 @@ def test_config_full_size(sd, ctx, oracle, num):
     kind, d, (s,) = synth.config(num)
     assert s.sha256() == g["input_sha256"] and s.n == g["n"]
     i, j, dist = run_self(sd, ctx, s, d)
-    assert len(i) == g["n_out"]
+    assert_matches_golden(g, i, j, dist)  # identical pairs, distances and order as the oracle
     assert np.bincount(dist, minlength=d + 1).tolist() == g["dist_hist"]
-    assert digest(i, j, dist) == g["out_sha256"]  # identical pairs, distances and order as the oracle
     assert (i < j).all() and (np.diff(i.astype(np.int64) * (1 << 31) + j) > 0).all()
     _check_sampled_rows(oracle, s, d, i, j, dist, 24 if num >= 3 else 60, num)
     # every reported distance re-derived by the oracle's full-table recurrence (sample at full size)
@@ -589,7 +606,7 @@ def test_config4_scaled(sd, ctx, oracle):
     kind, d, (q, r) = synth.config(4, 0.1)
     assert q.sha256() + r.sha256() == g["input_sha256"]
     i, j, dist = run_cross(sd, ctx, q, r, d)
-    assert len(i) == g["n_out"] and digest(i, j, dist) == g["out_sha256"]
+    assert_matches_golden(g, i, j, dist)
 
 
 def test_config4_full_size(sd, ctx, oracle):
@@ -597,10 +614,175 @@ def test_config4_full_size(sd, ctx, oracle):
     kind, d, (q, r) = synth.config(4)
     assert q.sha256() + r.sha256() == g["input_sha256"]
     i, j, dist = run_cross(sd, ctx, q, r, d)
-    assert len(i) == g["n_out"] and np.bincount(dist, minlength=d + 1).tolist() == g["dist_hist"]
-    assert digest(i, j, dist) == g["out_sha256"]
+    assert_matches_golden(g, i, j, dist)
+    assert np.bincount(dist, minlength=d + 1).tolist() == g["dist_hist"]
     rng = np.random.default_rng(4)
     for t in np.unique(np.concatenate([i[:: max(1, len(i) // 10)][:10], rng.integers(0, q.n, 6)])):
         rr, dd = oracle.bruteforce_row(q.seq(int(t)), r.seqs, r.offsets, d)
         m = i == t
         assert np.array_equal(j[m], rr) and np.array_equal(dist[m], dd)
+
+
+# ---- S5 at full size: key-range chunking under a memory budget (BASELINE.json config 5) ------
+@pytest.mark.parametrize("num,opts,ws_frac", [
+    (5, {"FORCE_CHUNKS": 4}, None), (5, {"FORCE_CHUNKS": 16}, None), (5, {}, 0.1), (5, {"EXACT_PIPELINE": 1}, 0.07),
+    (3, {"FORCE_CHUNKS": 4}, None), (3, {"FORCE_CHUNKS": 16}, None), (3, {}, 0.1),
+])
+def test_config_full_size_chunked(torch, sd, oracle, num, opts, ws_frac):
+    """Config 5 "exercises chunked key-range streaming" (BASELINE.json) — on a 180 GB device only under a budget:
+    a forced chunk count, or a workspace that is a fraction of the un-chunked need (the planner then picks P).
+    Same golden digest as the un-chunked run: chunking changes memory use only (P-11)."""
+    g = _golden(f"config_{num}.json")
+    kind, d, (s,) = synth.config(num)
+    c = sd.Context(0)
+    for k, v in opts.items():
+        c.symdel_set_option(getattr(sd, "OPT_" + k), v)
+    ds, do = sd.to_device(s)
+    cap = 1 << 20
+    ws = None
+    if ws_frac is not None:
+        full = sd.symdel_workspace_bytes(s.n, s.seqs.size, 0, 0, int(s.lengths.max()), d, cap)
+        ws = torch.empty(int(full * ws_frac) // 256 * 256, dtype=torch.uint8, device="cuda")
+    i, j, dist = [t.cpu().numpy() for t in c.symdel_self(ds, do, d, workspace=ws, capacity=cap)]
+    st = c.symdel_get_stats()
+    assert_matches_golden(g, i, j, dist)
+    if "FORCE_CHUNKS" in opts:
+        assert st["n_chunks"] == opts["FORCE_CHUNKS"]
+    else:
+        assert st["n_chunks"] >= 4, st["n_chunks"]
+    if "EXACT_PIPELINE" not in opts:
+        assert st["fused_chunks"] == st["n_chunks"]  # every chunk stays on the fused pipeline
+    assert st["n_flushes"] >= st["n_chunks"]
+
+
+def test_dense_full_size(sd, ctx):
+    """NEXT-2 at the size bench.py --dense times: synth.dense_set(1,000,000, seed 11, fanout 64), d = 2 — 14.4 M
+    output pairs, candidates ~ records.  Golden written by the oracle alone."""
+    g = _golden("dense_1m.json")
+    s = synth.dense_set(1_000_000, 11, fanout=64)
+    assert s.sha256() == g["input_sha256"]
+    i, j, dist = run_self(sd, ctx, s, 2, capacity=g["n_out"] + 1024)
+    assert_matches_golden(g, i, j, dist)
+    st = ctx.symdel_get_stats()
+    assert st["n_candidates"] > st["n_records"] // 2
+
+
+# ---- run-to-run stability: every protocol built on atomics must give the same bits every time ---------------------
+@pytest.mark.parametrize("opts,reps", [({}, 200), ({"EXACT_PIPELINE": 1, "FORCE_CHUNKS": 3}, 50),
+                                       ({"FORCE_CHUNKS": 2, "CAND_CAPACITY": 100000}, 30)])
+def test_repeat_runs_are_bit_identical(torch, sd, opts, reps):
+    """Config 2, repeated in one process on one context and one workspace: claim-mode atomics, tickets, look-back and
+    shared overflow lists make the ORDER of intermediate data vary from run to run; the output may not."""
+    g = _golden("config_2.json")
+    kind, d, (s,) = synth.config(2)
+    c = sd.Context(0)
+    for k, v in opts.items():
+        c.symdel_set_option(getattr(sd, "OPT_" + k), v)
+    ds, do = sd.to_device(s)
+    cap = 1 << 18
+    ws = torch.empty(sd.symdel_workspace_bytes(s.n, s.seqs.size, 0, 0, int(s.lengths.max()), d, cap), dtype=torch.uint8, device="cuda")
+    out = tuple(torch.empty(cap, dtype=torch.int32, device="cuda") for _ in range(3))
+    for rep in range(reps):
+        i, j, dist = [t.cpu().numpy() for t in c.symdel_self(ds, do, d, workspace=ws, out=out)]
+        assert digest(i, j, dist) == g["out_sha256"], rep
+        if rep % 16 == 0:
+            ws.random_(0, 255)  # stale workspace contents must not matter
+            for o in out:
+                o.fill_(-7)
+
+
+# ---- boundary: devices, threads, capacity ---------------------------------------------------------------------------
+def test_two_contexts_in_one_process(torch, sd, oracle):
+    """Per-device state is set up by symdel_create for the context's device (include/symdel.h "Devices and threads"):
+    two live contexts, used alternately and from two host threads, and one per visible device."""
+    import threading
+
+    s = synth.tcr_set(5000, 61)
+    exp = oracle.symdel_self(s.seqs, s.offsets, 2)
+    a, b = sd.Context(0), sd.Context(0)
+    for c in (a, b, a, b):
+        assert_same(run_self(sd, c, s, 2), exp)
+    res = {}
+
+    def work(name, c):
+        with torch.cuda.stream(torch.cuda.Stream()):
+            res[name] = [run_self(sd, c, s, 2) for _ in range(5)]
+
+    ts = [threading.Thread(target=work, args=(n, c)) for n, c in (("a", a), ("b", b))]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    for name in ("a", "b"):
+        for got in res[name]:
+            assert_same(got, exp)
+    for dev in range(1, torch.cuda.device_count()):  # a context on every other visible GPU (one GPU on the test box)
+        with torch.cuda.device(dev):
+            c = sd.Context(dev)
+            ds, do = sd.to_device(s, f"cuda:{dev}")
+            assert_same([t.cpu().numpy() for t in c.symdel_self(ds, do, 2)], exp)
+
+
+@pytest.mark.parametrize("opts", [{"FORCE_CHUNKS": 4}, {"CAND_CAPACITY": 3000}, {"FORCE_CHUNKS": 3, "CAND_CAPACITY": 2000},
+                                  {"EXACT_PIPELINE": 1, "FORCE_CHUNKS": 2}])
+def test_capacity_error_in_multi_flush_searches(sd, oracle, opts):
+    """SYMDEL_E_CAPACITY on the chunked / windowed path (symdel.h): the first `capacity` pairs are valid and the
+    required count is reported; a pair found in several chunks is appended once per flush, and the survivor list is
+    merged (sorted, deduplicated) instead of running out of room."""
+    s = synth.tcr_set(6000, 21)
+    exp = oracle.symdel_self(s.seqs, s.offsets, 2)
+    n_exp = len(exp[0])
+    assert n_exp > 1500
+    for surv_cap, capacity in ((0, 1000), (1, 1000), (1, n_exp), (1, n_exp + 5)):
+        c = sd.Context(0)
+        for k, v in opts.items():
+            c.symdel_set_option(getattr(sd, "OPT_" + k), v)
+        c.symdel_set_option(sd.OPT_SURV_CAPACITY, surv_cap)  # 1 = the smallest legal survivor list
+        ds, do = sd.to_device(s)
+        out = tuple(__import__("torch").full((capacity,), -1, dtype=__import__("torch").int32, device="cuda") for _ in range(3))
+        if capacity >= n_exp:
+            got = [t.cpu().numpy() for t in c.symdel_self(ds, do, 2, out=out)]
+            assert_same(got, exp)
+            continue
+        with pytest.raises(sd.SymdelError) as e:
+            c.symdel_self(ds, do, 2, out=out)
+        assert e.value.code == sd.E_CAPACITY
+        st = c.symdel_get_stats()
+        if st["surv_merges"] == 0:
+            assert c.last_required == n_exp  # exact count
+        else:
+            assert capacity < c.last_required <= n_exp  # a lower bound that still exceeds the capacity
+        for o, x in zip(out, exp):
+            assert np.array_equal(o.cpu().numpy(), x[:capacity])  # the first `capacity` pairs, ascending
+
+
+def test_out_of_range_indices_are_rejected(torch, sd, ctx):
+    """Caller-supplied indices never steer a read out of bounds: symdel_stage_lev and symdel_overlap_matrix."""
+    s = synth.tcr_set(300, 5)
+    ds, do = sd.to_device(s)
+    ia = torch.tensor([0, 5, s.n - 1], dtype=torch.int32, device="cuda")
+    assert (ctx.symdel_stage_lev(ds, do, ds, do, ia, ia).cpu().numpy() == 0).all()
+    for bad in (s.n, -1, 2**31 - 1):
+        ib = torch.tensor([0, bad, 7], dtype=torch.int32, device="cuda")
+        with pytest.raises(sd.SymdelError) as e:
+            ctx.symdel_stage_lev(ds, do, ds, do, ia, ib)
+        assert e.value.code == sd.E_ARG
+    labs = torch.zeros(s.n, dtype=torch.int32, device="cuda")
+    pi = torch.tensor([1, 2, s.n - 1], dtype=torch.int32, device="cuda")
+    assert int(ctx.symdel_overlap_matrix(pi, pi, labs, labs, 2, True).sum()) == 3
+    for bad in (s.n, -5):
+        pj = torch.tensor([1, bad, 3], dtype=torch.int32, device="cuda")
+        with pytest.raises(sd.SymdelError) as e:
+            ctx.symdel_overlap_matrix(pi, pj, labs, labs, 2, True)
+        assert e.value.code == sd.E_ARG
+
+
+def test_malformed_offsets_never_steer_a_read(torch, sd, ctx):
+    """A garbage offsets array is reported as SYMDEL_E_OFFSETS / _TOO_LONG before any residue is read through it."""
+    s = synth.tcr_set(500, 8)
+    ds, do = sd.to_device(s)
+    for pos, val in ((500, 1 << 40), (250, -3), (0, 1), (499, 1 << 50)):
+        bad = do.clone()
+        bad[pos] = val
+        with pytest.raises(sd.SymdelError) as e:
+            ctx.symdel_self(ds, bad, 2)
+        assert e.value.code in (sd.E_OFFSETS, sd.E_TOO_LONG), (pos, e.value.code)
+    assert len(ctx.symdel_self(ds, do, 1)[0]) >= 0  # the context still works (no sticky CUDA error)

@@ -273,6 +273,26 @@ def test_order_and_orientation(oracle):  # readings A-3, A-10
         assert as_set((i, j, d)) == {(0, 1, 1), (0, 2, 0), (0, 3, 1), (1, 2, 1), (1, 3, 2), (2, 3, 1)}
 
 
+def test_cross_orientation_hand_worked(oracle):
+    """(q, r) orientation of the two-set form pinned on the oracle itself by an ASYMMETRIC hand-worked case
+    ("for both the query and reference sets"; Fig. 1): the first component indexes
+    the query set, the second the reference set, sorted by (q, r).  Q = [ACDF], R = [GGGG, ACDEF, ACDF]:
+    ACDF -> ACDEF is one insertion, ACDF = ACDF, and GGGG is four substitutions away."""
+    q, r = S("ACDF"), S("GGGG", "ACDEF", "ACDF")
+    for f in (oracle.symdel_cross, oracle.bruteforce_cross):
+        i, j, d = f(q.seqs, q.offsets, r.seqs, r.offsets, 1)[:3]
+        assert list(zip(i.tolist(), j.tolist(), d.tolist())) == [(0, 1, 1), (0, 2, 0)]
+        # swapped roles: three queries against one reference -> the indices swap sides
+        i, j, d = f(r.seqs, r.offsets, q.seqs, q.offsets, 1)[:3]
+        assert list(zip(i.tolist(), j.tolist(), d.tolist())) == [(1, 0, 1), (2, 0, 0)]
+    # two queries, asymmetric sizes and a query index > every reference index of its matches
+    q2, r2 = S("WWWW", "ACDEF", "CDEFA"), S("ACDF", "CDEF")
+    exp = [(1, 0, 1), (1, 1, 1), (2, 1, 1)]  # ACDEF-ACDF (del E), ACDEF-CDEF (del A), CDEFA-CDEF (del A); CDEFA-ACDF = 3
+    for f in (oracle.symdel_cross, oracle.bruteforce_cross):
+        i, j, d = f(q2.seqs, q2.offsets, r2.seqs, r2.offsets, 1)[:3]
+        assert list(zip(i.tolist(), j.tolist(), d.tolist())) == exp
+
+
 # ---- P-6 exactness: symdel == brute force on 5,000 sequences, d = 1, 2, 3 (PAPER.md:166) -------
 @pytest.mark.parametrize("family", ["tcr", "bcr"])
 @pytest.mark.parametrize("d", [1, 2, 3])
