@@ -29,6 +29,7 @@ struct DevInfo {
     u32 part_overflow;  // fused pipeline: 1 = a level-1 bin was full, 2 = a level-2 bucket was full
     u32 surv_overflow;  // k_verify: the survivors of this flush did not fit behind the survivor list (nothing lost: the host merges the list and repeats the flush)
     u64 residues;       // sum of the (prefix-truncated) sequence lengths
+    u64 n_filt;         // candidates of the current window that passed the duplicate filter (k_cand_filter)
 };
 enum { SD_ERR_OFFSETS = 1, SD_ERR_TOO_LONG = 2, SD_ERR_RESIDUE = 4, SD_ERR_INTERNAL = 8, SD_ERR_OVERFLOW = 16 };
 enum { SD_TK_SORT = 0, SD_TK_EMIT = 1, SD_TK_VERIFY = 2, SD_TK_FINAL = 3, SD_TK_SCAN = 4 };

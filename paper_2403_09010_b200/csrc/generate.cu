@@ -647,13 +647,13 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
 // info->part_overflow: the host then redoes the chunk with the exact (histogram-based) pipeline.
 // (values swept on config 3 / config 5 in round 1: 512 threads, 2 or 4 resident blocks, rounds of 3600 / 7200 records
 //  and flush thresholds from 2000 to 4500 all landed within 3 % of these)
-constexpr int GP_THREADS = 256;    // threads per block
+constexpr int GP_THREADS = 256;    // threads per block (512 with two resident blocks: +2 %)
 constexpr int GP_MINB = 3;         // resident blocks per SM (64 KB stage each)
 constexpr int GP_FLUSH_AT = 2800;  // flush when more than this is staged after a round (i.e. after nearly every full round)
 constexpr int GP_OVF = 128;        // overflow list entries
 constexpr int GP_TRIP = 16;        // d = 3: (g1, g2) iterations per step of a batch
 constexpr int GP_ROUND = 5400;     // records a block stages per round (21 per digit of the 32 slots); the host turns it into batches per warp
-constexpr int GP_NW = GP_THREADS / 32, GP_S = 32;
+constexpr int GP_NW = GP_THREADS / 32, GP_S = 32;  // (16 slots per digit and 4-5 resident blocks: generation 0.66 -> 0.85-1.25 ms on config 3, the digits overflow)
 static_assert(GP_THREADS >= 256 && GP_THREADS % 32 == 0, "one thread per digit in the flush");
 
 struct GenPartShared {
@@ -932,9 +932,11 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                 sh.fl[tid] = make_uint2(g, g == 0xffffffffu ? 0u : cn_);
             }
             __syncthreads();
-            for (u32 dg = warp; dg < 256; dg += GP_NW) {
+            constexpr u32 DPW = 32 / GP_S;  // digits per warp instruction
+            for (u32 dg = DPW * warp + lane / GP_S; dg < 256; dg += DPW * GP_NW) {
                 const uint2 f = sh.fl[dg];
-                if (lane < f.y) PP.bins[f.x + lane] = sh.stage[dg * GP_S + ((lane + dg) & (GP_S - 1))];
+                const u32 o = lane & (GP_S - 1);
+                if (o < f.y) PP.bins[f.x + o] = sh.stage[dg * GP_S + ((o + dg) & (GP_S - 1))];
             }
             for (u32 i = tid; i < min(sh.novf, (u32)GP_OVF); i += GP_THREADS) {  // the overflow records, one global atomic each
                 const u64 rec = sh.ovf[i];

@@ -31,6 +31,7 @@
 // positions, so it is the same in every round); a round writes the records whose FIRST index lies in
 // [win_lo, win_hi), whole, at cand[index - win_lo] — the buffer keeps n_total + 64 slots of slack for
 // the overhang — and reports the end of what it wrote in info->win_end, where the next round starts.
+#include <cstddef>
 #include <type_traits>
 
 #include "kernels.h"
@@ -603,9 +604,10 @@ constexpr int JF_LMAX_L = JF_T + 4096, JF_SLOTB_L = 12, JF_MINB_L = JF_IT > 8 ? 
 //      walk writes.
 // No bitmaps, no candidate list, no list overflow: dense buckets (every record with partners) take the same
 // path, their chains are just longer.  The kernel is latency-bound (dependent shared-memory accesses): what
-// counts is resident warps, hence 34 KB of shared memory per block (six blocks of 256 threads per SM; with
-// five, +12 %; with four, +35 %).  Two instances: regions of up to 2560 records (NB = 12) and up to 18432
-// (1024 threads, one block per SM, NB = 15: chunks of more than ~10^8 records).  If the claims run past the
+// counts is resident warps, hence as little shared memory per block as the region needs: 16 KB of heads + the
+// stage, sized at launch (config 3: 34 KB, six blocks of 256 threads per SM; with five blocks +12 %, with four
+// +35 %).  Two instances: regions of up to 4064 records (NB = 12) and up to 18432 (1024 threads, NB = 15: chunks
+// of more than ~2 * 10^8 records).  If the claims run past the
 // candidate window info->join_fallback is raised (the host then uses the exact pipeline).
 struct JoinBktParams {
     JoinParams j;       // rec = bucket regions; topmask unused
@@ -646,22 +648,25 @@ __device__ __forceinline__ u32 jb_atoms_exch(u32* p, u32 v) {
     return old;
 }
 
-template <int STAGE, int SLOT_BITS>
+// shared memory: this header, then the stage (`cap` records, sized at launch: the smaller the regions, the more blocks per SM)
+template <int SLOT_BITS>
 struct JoinBktSmem {
-    u64 stage[STAGE];          // the bucket; after the sweep the top NB bits of a record = the record inserted into its slot before it
     u32 head[1 << SLOT_BITS];  // last record inserted into the slot (all ones in NB bits: none)
     u64 mbar;
     u64 base;
-    u32 total;
+    u32 total, pad[3];
+    u64 stage[2];              // the bucket; after the sweep the top NB bits of a record = the record inserted into its slot before it
 };
 
-template <int THREADS, int STAGE, int SLOT_BITS, int NB, int MINB>
+// STAGE_MAX: the largest region this instance accepts
+template <int THREADS, int STAGE_MAX, int SLOT_BITS, int NB, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams BP) {
-    typedef JoinBktSmem<STAGE, SLOT_BITS> Smem;
-    constexpr int SLOTS = 1 << SLOT_BITS, IT = (STAGE / 2 + THREADS - 1) / THREADS;  // 16-byte loads per thread that cover the stage
+    typedef JoinBktSmem<SLOT_BITS> Smem;
+    constexpr int SLOTS = 1 << SLOT_BITS, IT = (STAGE_MAX / 2 + THREADS - 1) / THREADS;  // 16-byte loads per thread that cover the stage
     constexpr u32 NIL = (1u << NB) - 1u;
     constexpr u64 KEEP = ~0ull >> NB;  // the bits of a staged record that are still the record
-    static_assert(STAGE <= (int)NIL && STAGE % 2 == 0 && 2 * IT <= 32 && SLOTS % (4 * THREADS) == 0 && NB <= 16, "link / flag mask widths");
+    static_assert(STAGE_MAX <= (int)NIL && STAGE_MAX % 2 == 0 && 2 * IT <= 32 && SLOTS % (4 * THREADS) == 0 && NB <= 16 &&
+                      offsetof(Smem, stage) % 16 == 0, "link / flag mask widths");
     extern __shared__ __align__(16) unsigned char jn_smem[];
     Smem& S = *reinterpret_cast<Smem*>(jn_smem);
     const JoinParams& P = BP.j;
@@ -709,11 +714,20 @@ __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams 
         const u32 e = __ffs(m) - 1;
         const u64 y = S.stage[pos_of(e)];
         u32 c = 0;
-        for (u32 j = (u32)(y >> (64 - NB)); j != NIL;) {
-            const u64 z = S.stage[j];
-            u64 packed;
-            if (((y ^ z) & KEEP) < P.hlim && jn_pair(y, z, P, packed)) ++c;
-            j = (u32)(z >> (64 - NB));
+        if (!P.cross) {
+            // self-search: same hash and different ids <=> 0 < (y ^ z) & KEEP < 2^id_bits
+            for (u32 j = (u32)(y >> (64 - NB)); j != NIL;) {
+                const u64 z = S.stage[j];
+                c += (((y ^ z) & KEEP) - 1ull) < (P.hlim - 1ull) ? 1u : 0u;
+                j = (u32)(z >> (64 - NB));
+            }
+        } else {
+            for (u32 j = (u32)(y >> (64 - NB)); j != NIL;) {
+                const u64 z = S.stage[j];
+                u64 packed;
+                if (((y ^ z) & KEEP) < P.hlim && jn_pair(y, z, P, packed)) ++c;
+                j = (u32)(z >> (64 - NB));
+            }
         }
         if (c) nz |= 1u << e;
         cnt += c;
@@ -743,10 +757,13 @@ __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams 
     }
 }
 
-// the two instances: (threads, stage, chain-head bits, link bits, resident blocks)
-constexpr int JB_THREADS_S = 256, JB_STAGE_S = 2560, JB_SLOTB_S = 12, JB_NB_S = 12, JB_MINB_S = 6;
-constexpr int JB_THREADS_L = 1024, JB_STAGE_L = 18432, JB_SLOTB_L = 14, JB_NB_L = 15, JB_MINB_L = 1;
-static_assert(6 * (sizeof(JoinBktSmem<JB_STAGE_S, JB_SLOTB_S>) + 1024) <= 233472, "six blocks of the small instance per SM");
+// the two instances: (threads, largest region, chain-head bits, link bits, resident blocks the registers must allow)
+constexpr int JB_THREADS_S = 256, JB_STAGE_S = 4064, JB_SLOTB_S = 12, JB_NB_S = 12, JB_MINB_S = 6;
+constexpr int JB_THREADS_L = 1024, JB_STAGE_L = 18432, JB_SLOTB_L = 13, JB_NB_L = 15, JB_MINB_L = 1;
+static size_t jb_smem_bytes(bool small, u32 cap) {
+    return (small ? offsetof(JoinBktSmem<JB_SLOTB_S>, stage) : offsetof(JoinBktSmem<JB_SLOTB_L>, stage)) + (size_t)cap * 8;
+}
+static_assert(6 * (offsetof(JoinBktSmem<JB_SLOTB_S>, stage) + 2304 * 8 + 1024) <= 233472, "six blocks per SM at config-3 regions (2304 records)");
 
 }  // namespace
 
@@ -766,9 +783,9 @@ cudaError_t sd_join_setup() {
     cudaError_t e;
     if ((e = cudaFuncSetAttribute(k_join, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(JoinSmem))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)sizeof(JoinBktSmem<JB_STAGE_S, JB_SLOTB_S>))) != cudaSuccess) return e;
+                                  (int)jb_smem_bytes(true, JB_STAGE_S))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)sizeof(JoinBktSmem<JB_STAGE_L, JB_SLOTB_L>))) != cudaSuccess) return e;
+                                  (int)jb_smem_bytes(false, JB_STAGE_L))) != cudaSuccess) return e;
     if ((e = jn_setup_k<true>()) != cudaSuccess) return e;
     return jn_setup_k<false>();
 }
@@ -886,8 +903,8 @@ cudaError_t sd_join_bkt(const u64* buckets, const u32* cnt, u32 cap, u32 nbucket
     BP.j.slot_shift = std::max(lay.id_bits, top - lay.sort_bits - (small ? JB_SLOTB_S : JB_SLOTB_L));
     if (launches) ++*launches;
     if (small)
-        k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S><<<nbuckets, JB_THREADS_S, sizeof(JoinBktSmem<JB_STAGE_S, JB_SLOTB_S>), st>>>(BP);
+        k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S><<<nbuckets, JB_THREADS_S, jb_smem_bytes(true, cap), st>>>(BP);
     else
-        k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L><<<nbuckets, JB_THREADS_L, sizeof(JoinBktSmem<JB_STAGE_L, JB_SLOTB_L>), st>>>(BP);
+        k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L><<<nbuckets, JB_THREADS_L, jb_smem_bytes(false, cap), st>>>(BP);
     return cudaGetLastError();
 }

@@ -44,8 +44,13 @@ u32* sd_sort_hist_ptr(void* scratch);
 cudaError_t sd_sort_histogram(const u64* keys, i64 n, int begin_bit, int npass, void* scratch, cudaStream_t st,
                               i64* launches);
 cudaError_t sd_sort_hist_scan(void* scratch, int npass, cudaStream_t st, i64* launches);
-cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, int stable, int variant, void* scratch,
-                           cudaStream_t st, u64** result, i64* launches);
+// n_dev != nullptr: the key count is *n_dev (device); n is an upper bound that sizes the grids and the scratch
+cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, const u64* n_dev, int begin_bit, int npass, int stable, int variant,
+                           void* scratch, cudaStream_t st, u64** result, i64* launches);
+// S3b duplicate suppression before the sort: keeps the candidates a best-effort hash set has not seen yet, compacts
+// them into out[0 .. *n_out) and accumulates their digit histograms (bits [0, 8 * npass)) into `scratch`
+cudaError_t sd_cand_filter(const u64* cand, i64 n, void* table, int table_bits, u64* out, u64* n_out, int npass, void* scratch,
+                           cudaStream_t st, i64* launches);
 
 // level-2 partition of the fused pipeline: bins (256 x cap1) -> buckets ((256 << b2) x cap2)
 cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u32* cnt2, i64 cap2, int b2, int shift,
@@ -111,11 +116,12 @@ i64 sd_pack_bytes(i64 n_total, int maxlen);
 cudaError_t sd_pack(SeqSetDev a, SeqSetDev b, int maxlen, void* slots, DevInfo* info, cudaStream_t st, i64* launches);
 // cand sorted ascending.  Drops repeats and a == b (self), computes lev, keeps <= d, appends
 // (pair << 3 | dist) in order to surv[surv_base + ...]; info->n_surv = total; info->n_unique += unique.
-cudaError_t sd_verify(const u64* cand, i64 n_cand, const void* slots, const Layout& lay, int maxlen, u64* surv,
+// (n_dev != nullptr: the candidate count is *n_dev, n_cand an upper bound that sizes the grid)
+cudaError_t sd_verify(const u64* cand, i64 n_cand, const u64* n_dev, const void* slots, const Layout& lay, int maxlen, u64* surv,
                       u64 surv_base, u64 surv_capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
 // the same when this is known to be the ONLY flush of the search: survivors go straight to the SoA outputs
-cudaError_t sd_verify_direct(const u64* cand, i64 n_cand, const void* slots, const Layout& lay, int maxlen, i32* out_i, i32* out_j,
-                             i32* out_dist, i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
+cudaError_t sd_verify_direct(const u64* cand, i64 n_cand, const u64* n_dev, const void* slots, const Layout& lay, int maxlen, i32* out_i,
+                             i32* out_j, i32* out_dist, i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches);
 // surv sorted ascending (and unique unless dedup = 1).  Unpacks to SoA outputs, first `capacity`
 // only; info->n_out = total.  packed_out != nullptr: writes the kept words to packed_out instead (the merge of
 // the survivor list between flushes).

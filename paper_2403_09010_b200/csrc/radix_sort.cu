@@ -48,6 +48,72 @@ __global__ void __launch_bounds__(256) k_hist_scan(u32* __restrict__ ghist) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// S3b, first half: duplicate suppression BEFORE the sort (k_cand_filter).  A pair within distance d shares several
+// deletion variants, so the join emits it several times (config 3: 3.67 M candidates for 0.52 M distinct pairs; the
+// paper's real repertoires: 137 M matched for 56 M unique).  Instead of sorting all of them, every
+// candidate is first offered to an open-addressing hash set of packed pair ids (64-bit compare-and-swap, linear
+// probing, a few probes at most): a candidate that finds ITSELF in the set is dropped, one that claims an empty slot
+// or finds no room after the probe limit is kept.  The set is best effort by design — a full table only lets
+// duplicates through — because the sorted candidates are still compared with their left neighbour in the verifier:
+// the result cannot depend on it.  The kept candidates are compacted (block scan, one global atomic per tile) and
+// their digit histograms for the LSD passes are accumulated in the same sweep: this kernel replaces k_histogram on the
+// candidate side.  Table entries hold key + 1 (0 = empty).
+constexpr int CF_THREADS = 256, CF_IPT = 8, CF_TILE = CF_THREADS * CF_IPT, CF_PROBES = 6;
+
+__global__ void __launch_bounds__(CF_THREADS) k_cand_filter(const u64* __restrict__ cand, u64 n, unsigned long long* __restrict__ table,
+                                                           int table_bits, u64* __restrict__ out, u64* n_out, int npass,
+                                                           u32* __restrict__ ghist) {
+    __shared__ u32 sh[8 * 256];
+    __shared__ u32 s_warp[CF_THREADS / 32 + 1];
+    __shared__ u64 s_base;
+    const u32 tid = threadIdx.x;
+    for (int i = tid; i < npass * 256; i += CF_THREADS) sh[i] = 0;
+    const u64 base = (u64)blockIdx.x * CF_TILE;
+    const u64 tmask = (1ull << table_bits) - 1ull;
+    u64 key[CF_IPT];
+    u32 keep = 0;
+#pragma unroll
+    for (int k = 0; k < CF_IPT; ++k) {
+        const u64 pos = base + (u64)k * CF_THREADS + tid;
+        key[k] = pos < n ? cand[pos] : 0ull;
+    }
+#pragma unroll
+    for (int k = 0; k < CF_IPT; ++k) {
+        const u64 pos = base + (u64)k * CF_THREADS + tid;
+        if (pos < n) {
+            const unsigned long long want = key[k] + 1ull;
+            u64 h = (key[k] * 0x9e3779b97f4a7c15ull) >> (64 - table_bits);
+            bool dup = false;
+            for (int pr = 0; pr < CF_PROBES; ++pr) {
+                const unsigned long long old = atomicCAS(&table[h], 0ull, want);
+                if (old == 0ull) break;  // claimed: first time this pair is seen
+                if (old == want) {
+                    dup = true;
+                    break;
+                }
+                h = (h + 1) & tmask;
+            }
+            if (!dup) keep |= 1u << k;
+        }
+    }
+    __syncthreads();  // sh cleared
+    u32 total;
+    const u32 rank = sd_block_excl_sum<CF_THREADS>(__popc(keep), &total, s_warp);
+    if (tid == 0) s_base = total ? (u64)atomicAdd((unsigned long long*)n_out, (unsigned long long)total) : 0ull;
+    __syncthreads();
+    u64 at = s_base + rank;
+#pragma unroll
+    for (int k = 0; k < CF_IPT; ++k)
+        if ((keep >> k) & 1u) {
+            out[at++] = key[k];
+            for (int p = 0; p < npass; ++p) atomicAdd(&sh[p * 256 + ((u32)(key[k] >> (8 * p)) & 255u)], 1u);
+        }
+    __syncthreads();
+    for (int i = tid; i < npass * 256; i += CF_THREADS)
+        if (sh[i]) atomicAdd(&ghist[i], sh[i]);
+}
+
+// ---------------------------------------------------------------------------------------------
 #define OS_FLAG_AGG (1u << 30)
 #define OS_FLAG_PRE (2u << 30)
 #define OS_MASK ((1u << 30) - 1)
@@ -221,7 +287,7 @@ __device__ __forceinline__ void os_tile_group(const u64 (&key)[IPT], u64* __rest
 template <int THREADS, int IPT, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB) k_onesweep(const u64* __restrict__ in, u64* __restrict__ out, u32 n, int shift,
                                                            u64 smask, u32* __restrict__ gbase, u32* __restrict__ status,
-                                                           u32* __restrict__ ticket) {
+                                                           u32* __restrict__ ticket, const u64* __restrict__ n_dev) {
     static_assert(IPT % 2 == 0 && THREADS * IPT < 65536, "rank packing");
     constexpr int TILE = THREADS * IPT, NW = THREADS / 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -235,11 +301,15 @@ __global__ void __launch_bounds__(THREADS, MINB) k_onesweep(const u64* __restric
 
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool claim = smask == 0;
+    // n_dev: the key count lives on the device (the grid was sized for an upper bound: surplus blocks leave at once —
+    // tiles are numbered by ticket, so no working tile ever waits on one of them)
+    if (n_dev) n = (u32)*n_dev;
     if (!claim && tid == 0) s_tile = atomicAdd(ticket, 1u);
     for (int i = tid; i < (claim ? 256 : 2 * NW * 256); i += THREADS) whist[i] = 0;
     __syncthreads();
     const u32 tile = claim ? blockIdx.x : s_tile;
     const u32 base = tile * TILE;
+    if (base >= n) return;  // (block-uniform)
     const u32 tile_n = min((u32)TILE, n - base);
     const bool full = tile_n == (u32)TILE;
 
@@ -362,7 +432,7 @@ __global__ void __launch_bounds__(P2_THREADS, P2_MINB) k_part2(const Part2Params
 struct OsVariant {
     int threads, ipt;
     size_t smem;
-    void (*kernel)(const u64*, u64*, u32, int, u64, u32*, u32*, u32*);
+    void (*kernel)(const u64*, u64*, u32, int, u64, u32*, u32*, u32*, const u64*);
 };
 template <int THREADS, int IPT, int MINB>
 constexpr OsVariant os_variant() {
@@ -414,6 +484,20 @@ cudaError_t sd_sort_histogram(const u64* keys, i64 n, int begin_bit, int npass, 
     return cudaGetLastError();
 }
 
+// Candidate filter + histograms (see k_cand_filter).  table: 2^table_bits zeroed 64-bit slots; *n_out (device) is
+// cleared here and receives the number of candidates kept in out[0 .. ).  The histograms go to `scratch` as with
+// sd_sort_histogram (bits [0, 8 * npass) of the keys).
+cudaError_t sd_cand_filter(const u64* cand, i64 n, void* table, int table_bits, u64* out, u64* n_out, int npass, void* scratch,
+                           cudaStream_t st, i64* launches) {
+    cudaError_t e = cudaMemsetAsync(n_out, 0, sizeof(u64), st);
+    if (e != cudaSuccess || n == 0) return e;
+    const unsigned blocks = (unsigned)((n + CF_TILE - 1) / CF_TILE);
+    k_cand_filter<<<blocks, CF_THREADS, 0, st>>>(cand, (u64)n, (unsigned long long*)table, table_bits, out, n_out, npass,
+                                                sd_sort_hist_ptr(scratch));
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
 // Turns the raw per-digit counts into exclusive bin bases (one tiny launch).
 cudaError_t sd_sort_hist_scan(void* scratch, int npass, cudaStream_t st, i64* launches) {
     if (npass == 0) return cudaSuccess;
@@ -423,11 +507,12 @@ cudaError_t sd_sort_hist_scan(void* scratch, int npass, cudaStream_t st, i64* la
 }
 
 // Runs the passes.  The histograms in `scratch` must hold exclusive bin bases (sd_sort_hist_scan).
+// n_dev != nullptr: the number of keys is *n_dev (device memory), n is only an upper bound that sizes the grids.
 // Returns in *result the buffer (keys or tmp) that holds the sorted records.
 // stable = 1: ties keep their input order.  stable = 0: keys-only sort, ties in arbitrary order (lets
 // uniform tiles take the cheaper grouping path).
-cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass, int stable, int variant, void* scratch,
-                           cudaStream_t st, u64** result, i64* launches) {
+cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, const u64* n_dev, int begin_bit, int npass, int stable, int variant,
+                           void* scratch, cudaStream_t st, u64** result, i64* launches) {
     *result = keys;
     if (n == 0 || npass == 0) return cudaSuccess;
     const OsVariant& V = OS_VARIANTS[variant >= 0 && variant < OS_NVARIANTS ? variant : 0];
@@ -441,7 +526,7 @@ cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, int begin_bit, int npass,
     for (int p = 0; p < npass; ++p) {
         const u64 smask = stable ? ~0ull : (((1ull << (8 * p)) - 1ull) << begin_bit);
         V.kernel<<<(unsigned)tiles, V.threads, V.smem, st>>>(src, dst, (u32)n, begin_bit + 8 * p, smask, hist + p * 256,
-                                                             status + (size_t)p * status_stride, tickets + p);
+                                                             status + (size_t)p * status_stride, tickets + p, n_dev);
         if (launches) ++*launches;
         std::swap(src, dst);
     }

@@ -122,7 +122,10 @@ __device__ __forceinline__ int hamming_planes(const Planes<W>& P, const Planes<W
     return sizeof(W) == 8 ? __popcll((unsigned long long)x) : __popc((unsigned)x);
 }
 
-constexpr int VF_THREADS = 256, VF_IPT = 8, VF_TILE = VF_THREADS * VF_IPT;  // 4 per thread: 0.087 -> 8: 0.077 ms on config 3
+constexpr int VF_THREADS = 256;
+// candidates per thread: 8 when most candidates are repeats (unfiltered: 4 per thread 0.087 -> 8: 0.077 ms on config 3),
+// 2 when the duplicate filter ran first (nearly every candidate then needs a distance: small tiles spread them over the SMs)
+constexpr int VF_IPT_RAW = 8, VF_IPT_FILTERED = 2;
 
 // Tile of VF_TILE = 2048 sorted candidates: (1) flag the unique ones and compact their positions into shared
 // memory, (2) spread the COMPACTED list over the threads for the distance computation (after dedup
@@ -130,18 +133,21 @@ constexpr int VF_THREADS = 256, VF_IPT = 8, VF_TILE = VF_THREADS * VF_IPT;  // 4
 // the survivors (block scan + 32-wide decoupled look-back) so the output stays sorted.
 // DIRECT: this call is known to be the only flush of the whole search, so the survivors are final: they are
 // unpacked straight into (out_i, out_j, out_dist) (first surv_capacity of them) and info->n_out = their number.
-template <typename W, bool DIRECT>
-__global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ cand, u64 n, const void* __restrict__ slots,
+template <typename W, bool DIRECT, int VF_IPT>
+__global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ cand, u64 n, const u64* __restrict__ n_dev,
+                                                      const void* __restrict__ slots,
                                                       Layout lay, u64* __restrict__ surv, u64 surv_base,
                                                       u64 surv_capacity, u64* lb_status, DevInfo* info,
                                                       i32* __restrict__ out_i, i32* __restrict__ out_j,
                                                       i32* __restrict__ out_dist) {
+    constexpr int VF_TILE = VF_THREADS * VF_IPT;
     __shared__ unsigned short s_list[VF_TILE];
     __shared__ unsigned char s_res[VF_TILE];
     __shared__ u32 s_warp[VF_THREADS / 32 + 1];
     __shared__ u32 s_tile, s_nuniq;
     __shared__ u64 s_excl;
     const u32 tid = threadIdx.x, lane = tid & 31;
+    if (n_dev) n = *n_dev;  // the count lives on the device; the grid was sized for an upper bound
     if (tid == 0) {
         s_tile = atomicAdd(&info->ticket[SD_TK_VERIFY], 1u);
         if (s_tile == gridDim.x - 1) info->ticket[SD_TK_VERIFY] = 0;
@@ -150,6 +156,12 @@ __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ c
     __syncthreads();
     const u32 tile = s_tile;
     const u64 base = (u64)tile * VF_TILE;
+    const u32 last_tile = n ? (u32)((n - 1) / VF_TILE) : 0u;
+    if (n == 0 && tile == 0 && tid == 0) {
+        info->n_surv = surv_base;
+        if (DIRECT) info->n_out = 0;
+    }
+    if (base >= n) return;  // surplus block (block-uniform): tiles are ticket-numbered, nobody waits on it
     const u32 tile_n = (u32)min((u64)VF_TILE, n - base);
     const u64 bmask = (1ull << lay.b_bits) - 1ull;
 
@@ -201,7 +213,7 @@ __global__ void __launch_bounds__(VF_THREADS) k_verify(const u64* __restrict__ c
         if (tid == 0) {
             s_excl = excl;
             if (nuniq) atomicAdd((unsigned long long*)&info->n_unique, (unsigned long long)nuniq);
-            if (tile == gridDim.x - 1) {
+            if (tile == last_tile) {
                 info->n_surv = surv_base + excl + total;
                 if (DIRECT) info->n_out = excl + total;
             }
@@ -349,7 +361,7 @@ cudaError_t sd_overlap(const i32* pi, const i32* pj, i64 n, const i32* lab_i, i6
     return cudaGetLastError();
 }
 
-i64 sd_verify_tiles(i64 n) { return (n + VF_TILE - 1) / VF_TILE; }
+i64 sd_verify_tiles(i64 n) { return (n + VF_THREADS * VF_IPT_FILTERED - 1) / (VF_THREADS * VF_IPT_FILTERED); }  // (the smaller tile: sizes lb_status)
 
 i64 sd_pack_bytes(i64 n_total, int maxlen) { return n_total * (maxlen <= 32 ? 32 : 48); }
 
@@ -363,35 +375,46 @@ cudaError_t sd_pack(SeqSetDev a, SeqSetDev b, int maxlen, void* slots, DevInfo* 
     return cudaGetLastError();
 }
 
-cudaError_t sd_verify(const u64* cand, i64 n_cand, const void* slots, const Layout& lay, int maxlen, u64* surv,
+// filtered candidates (n_dev set) take the small tile
+template <typename W, bool DIRECT, typename... Args>
+static void vf_launch(bool filtered, i64 tiles, cudaStream_t st, Args... args) {
+    if (filtered) k_verify<W, DIRECT, VF_IPT_FILTERED><<<(unsigned)tiles, VF_THREADS, 0, st>>>(args...);
+    else k_verify<W, DIRECT, VF_IPT_RAW><<<(unsigned)tiles, VF_THREADS, 0, st>>>(args...);
+}
+static i64 vf_tiles(i64 n, bool filtered) {
+    const i64 t = VF_THREADS * (filtered ? VF_IPT_FILTERED : VF_IPT_RAW);
+    return (n + t - 1) / t;
+}
+
+cudaError_t sd_verify(const u64* cand, i64 n_cand, const u64* n_dev, const void* slots, const Layout& lay, int maxlen, u64* surv,
                       u64 surv_base, u64 surv_capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches) {
-    const i64 tiles = sd_verify_tiles(n_cand);
+    const i64 tiles = vf_tiles(n_cand, n_dev != nullptr);
     if (tiles == 0) return cudaSuccess;
     cudaError_t e = cudaMemsetAsync(lb_status, 0, (size_t)tiles * 8, st);
     if (e != cudaSuccess) return e;
     if (maxlen <= 32)
-        k_verify<u32, false><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, surv, surv_base, surv_capacity,
-                                                                     lb_status, info, nullptr, nullptr, nullptr);
+        vf_launch<u32, false>(n_dev != nullptr, tiles, st, cand, (u64)n_cand, n_dev, slots, lay, surv, surv_base, surv_capacity,
+                                                                     lb_status, info, (i32*)nullptr, (i32*)nullptr, (i32*)nullptr);
     else
-        k_verify<u64, false><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, surv, surv_base, surv_capacity,
-                                                                     lb_status, info, nullptr, nullptr, nullptr);
+        vf_launch<u64, false>(n_dev != nullptr, tiles, st, cand, (u64)n_cand, n_dev, slots, lay, surv, surv_base, surv_capacity,
+                                                                     lb_status, info, (i32*)nullptr, (i32*)nullptr, (i32*)nullptr);
     if (launches) ++*launches;
     return cudaGetLastError();
 }
 
 // The only flush of a search: unique + verify + unpack in one kernel.  info->n_out = number of result pairs
 // (the first `capacity` are written).
-cudaError_t sd_verify_direct(const u64* cand, i64 n_cand, const void* slots, const Layout& lay, int maxlen, i32* out_i, i32* out_j,
-                             i32* out_dist, i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches) {
-    const i64 tiles = sd_verify_tiles(n_cand);
+cudaError_t sd_verify_direct(const u64* cand, i64 n_cand, const u64* n_dev, const void* slots, const Layout& lay, int maxlen, i32* out_i,
+                             i32* out_j, i32* out_dist, i64 capacity, u64* lb_status, DevInfo* info, cudaStream_t st, i64* launches) {
+    const i64 tiles = vf_tiles(n_cand, n_dev != nullptr);
     if (tiles == 0) return cudaSuccess;
     cudaError_t e = cudaMemsetAsync(lb_status, 0, (size_t)tiles * 8, st);
     if (e != cudaSuccess) return e;
     if (maxlen <= 32)
-        k_verify<u32, true><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, nullptr, 0, (u64)capacity, lb_status,
+        vf_launch<u32, true>(n_dev != nullptr, tiles, st, cand, (u64)n_cand, n_dev, slots, lay, (u64*)nullptr, (u64)0, (u64)capacity, lb_status,
                                                                     info, out_i, out_j, out_dist);
     else
-        k_verify<u64, true><<<(unsigned)tiles, VF_THREADS, 0, st>>>(cand, (u64)n_cand, slots, lay, nullptr, 0, (u64)capacity, lb_status,
+        vf_launch<u64, true>(n_dev != nullptr, tiles, st, cand, (u64)n_cand, n_dev, slots, lay, (u64*)nullptr, (u64)0, (u64)capacity, lb_status,
                                                                     info, out_i, out_j, out_dist);
     if (launches) ++*launches;
     return cudaGetLastError();

@@ -307,6 +307,8 @@ def test_validation_protocol_5000(sd, ctx, oracle, family, d):
     {"SORT_BITS": 8, "HASH_BITS": 12, "CAND_CAPACITY": 100000, "FORCE_CHUNKS": 2},
     {"JOIN_GENERAL": 1}, {"JOIN_GENERAL": 1, "FORCE_CHUNKS": 3}, {"JOIN_GENERAL": 1, "SORT_BITS": 255},
     {"EXACT_PIPELINE": 1}, {"EXACT_PIPELINE": 1, "FORCE_CHUNKS": 2},
+    {"CAND_FILTER": 1}, {"CAND_FILTER": 2}, {"CAND_FILTER": 1, "FORCE_CHUNKS": 3, "CAND_CAPACITY": 2000},
+    {"CAND_FILTER": 1, "EXACT_PIPELINE": 1, "CAND_CAPACITY": 5000}, {"CAND_FILTER": 1, "HASH_BITS": 16},
 ])
 def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
     """P-11: chunk count, candidate-buffer windows, key width and thinning change memory use and
@@ -409,7 +411,8 @@ def test_prefix_truncation_cross(sd, oracle):
 
 
 @pytest.mark.parametrize("d,fanout,opts", [(1, 64, {}), (2, 64, {}), (2, 16, {"EXACT_PIPELINE": 1}), (2, 200, {}),
-                                           (2, 64, {"CAND_CAPACITY": 200000})])
+                                           (2, 64, {"CAND_CAPACITY": 200000}), (2, 64, {"CAND_FILTER": 1}),
+                                           (2, 200, {"CAND_FILTER": 1, "CAND_CAPACITY": 300000})])
 def test_dense_neighbourhoods(sd, oracle, d, fanout, opts):
     """NEXT-2: clusters of near-identical sequences (candidates ~ records, long runs of one variant, most records
     with partners: PAPER.md:96, 287-294).  Same bit-exact bar against the oracle's hash-map SymDel."""
