@@ -122,6 +122,88 @@ def cpu_baseline_run(n_sample: int, d: int, s):
     return len(i), dt
 
 
+def digest(i, j, d):
+    """sha256 of the int32 arrays (i, j, dist): the format of tests/golden/*.json (written by the oracle alone)."""
+    import hashlib
+
+    h = hashlib.sha256()
+    for a in (i, j, d):
+        h.update(np.ascontiguousarray(a, dtype=np.int32).tobytes())
+    return h.hexdigest()
+
+
+def golden(name):
+    p = ROOT / "tests" / "golden" / name
+    return json.loads(p.read_text()) if p.exists() else None
+
+
+def run_workload(torch, symdel, dev, name, kind, d, sets, gold, opts=None, ws_frac=None, steps=5, cap=1 << 21):
+    """One of the other workloads (configs 1, 2, 4, 5, dense, forced pipelines): `steps` device-resident steps after one
+    warm-up, CUDA events, result checked against the oracle's golden digest.  Not part of the headline's timed region."""
+    ctx = symdel.Context(dev.index)
+    for k, v in (opts or {}).items():
+        ctx.symdel_set_option(getattr(symdel, "OPT_" + k), v)
+    devs = [symdel.to_device(s, dev) for s in sets]
+    args = [t for pair in devs for t in pair]
+    n_a, n_b = sets[0].n, (sets[1].n if kind == "cross" else 0)
+    res_a, res_b = int(sets[0].seqs.size), (int(sets[1].seqs.size) if kind == "cross" else 0)
+    maxlen = max(int(s.lengths.max()) for s in sets)
+    full = symdel.symdel_workspace_bytes(n_a, res_a, n_b, res_b, maxlen, d, cap)
+    ws = torch.empty(int(full * (ws_frac or 1.0)) // 256 * 256, dtype=torch.uint8, device=dev)
+    out = tuple(torch.empty(cap, dtype=torch.int32, device=dev) for _ in range(3))
+    call = ctx.symdel_self if kind == "self" else ctx.symdel_cross
+    stream = torch.cuda.current_stream()
+    ms, r = [], None
+    for it in range(steps + 1):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        r = call(*args, d, workspace=ws, out=out)
+        e1.record(stream)
+        e1.synchronize()
+        if it:
+            ms.append(e0.elapsed_time(e1))
+    st = ctx.symdel_get_stats()
+    i, j, dist = [t.cpu().numpy() for t in r]
+    row = {"workload": name, "ms": float(np.mean(ms)), "pairs": int(len(i)), "records": st["n_records"],
+           "candidates": st["n_candidates"], "chunks": st["n_chunks"], "flushes": st["n_flushes"],
+           "pipeline": "fused" if st["fused_chunks"] == st["n_chunks"] else "exact" if st["fused_chunks"] == 0 else "mixed",
+           "workspace_bytes": int(ws.numel()), "steps": steps,
+           "verified": bool(gold and digest(i, j, dist) == gold["out_sha256"]) if gold else None}
+    ctx.close()
+    del ws, out, devs, args
+    torch.cuda.empty_cache()
+    return row
+
+
+def other_workloads(torch, symdel, synth, dev):
+    """the workloads README/DESIGN quote, measured in the driver's own run."""
+    rows = []
+
+    def add(name, kind, d, sets, gold, **kw):
+        try:
+            rows.append(run_workload(torch, symdel, dev, name, kind, d, sets, gold, **kw))
+        except Exception as e:  # a failed side workload must not lose the headline
+            rows.append({"workload": name, "error": repr(e)[:200]})
+
+    for num in (1, 2, 5):
+        kind, d, sets = synth.config(num)
+        add(f"config {num}", kind, d, sets, golden(f"config_{num}.json"))
+    kind, d, sets = synth.config(5)
+    add("config 5, workspace = 10 % of the un-chunked need (key-range chunking, S5)", kind, d, sets, golden("config_5.json"),
+        ws_frac=0.1)
+    add("config 5, FORCE_CHUNKS = 4", kind, d, sets, golden("config_5.json"), opts={"FORCE_CHUNKS": 4})
+    kind, d, sets = synth.config(3)
+    add("config 3, exact pipeline (SYMDEL_OPT_EXACT_PIPELINE)", kind, d, sets, golden("config_3.json"),
+        opts={"EXACT_PIPELINE": 1})
+    add("config 3, workspace = 10 % (chunked)", kind, d, sets, golden("config_3.json"), ws_frac=0.1)
+    add("config 3, prefix P = 12 (NEXT-1)", kind, d, sets, golden("config_3.json"), opts={"PREFIX_LEN": 12})
+    sets = (synth.dense_set(1_000_000, 11, fanout=64),)
+    add("NEXT-2 dense: synth.dense_set(1e6, seed 11, fanout 64), d=2", "self", 2, sets, golden("dense_1m.json"), cap=32 << 20)
+    kind, d, sets = synth.config(4)
+    add("config 4 (cross 100k x 5M)", kind, d, sets, golden("config_4.json"), cap=1 << 22)
+    return rows
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle (oracle_symdel_self, App. F.1 hash map, 1 thread)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -165,6 +247,7 @@ def main():
                     help="sequences in the oracle's bounded sample (0: 150,000 for cpu_baseline; for --impl reference sized "
                          "so that warm-up + steps take about two minutes)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-workloads", action="store_true", help="skip the `workloads` rows (the other configs, 5 steps each)")
     ap.add_argument("--dense", action="store_true",
                     help="NEXT-2 workload instead of config 3: synth.dense_set(1,000,000, seed 11, fanout 64), d=2 "
                          "(real-repertoire-like density: candidates ~ records; not the BASELINE.json headline)")
@@ -261,6 +344,16 @@ def main():
     e2e_ms = float(np.mean([x[0] for x in e2e]))
     assert e2e[0][1] == n_out
 
+    # the timed result against the oracle's golden digest (tests/golden, written by the oracle alone)
+    gold_name = "dense_1m.json" if args.dense else f"config_{args.config}.json"
+    gold = golden(gold_name)
+    i_d, j_d, d_d = ctx.symdel_self(seqs_d, offs_d, d, workspace=ws, out=out)
+    dig_dev = digest(i_d.cpu().numpy(), j_d.cpu().numpy(), d_d.cpu().numpy())
+    dig_host = digest(*[o[:n_out].numpy() for o in out_h])
+    verified = bool(gold) and dig_dev == gold["out_sha256"] and dig_host == gold["out_sha256"]
+    if gold and not verified:
+        raise SystemExit(f"bench: output digest differs from tests/golden/{gold_name} (device {dig_dev[:12]}, host {dig_host[:12]})")
+
     ms, e2e_ms = max_over_ranks([float(np.mean(ms_steps)), e2e_ms], dist, dev)
     if rank != 0:
         if dist is not None:
@@ -282,22 +375,26 @@ def main():
     npass = 1 if fused else st["sort_bits"] // 8
     pass_ms = float(np.mean([x["ms_sort_pass_avg"] for x in stats_acc]))
     step_bytes = (n_rec * (8 + 16 * npass + 8) + n_cand * (8 + 8 + 16 * ppass + 8) + n_out * 12 + in_bytes)
-    kname = "k_part2" if fused else "k_onesweep"
-    achieved = 16.0 * n_rec / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
-
-    def hbm(name, ms_key, nbytes):
+    def hbm(name, kernel, ms_key, nbytes):
         gbs = nbytes / (stage[ms_key] * 1e-3) / 1e9 if stage[ms_key] > 0 else 0.0
-        return {"stage": name, "ms": stage[ms_key], "share_of_step": stage[ms_key] / stage["ms_total"],
-                "algorithmic_bytes": int(nbytes), "achieved_gbs": gbs, "frac_of_peak": gbs / peak}
+        return {"stage": name, "kernel": kernel, "ms": stage[ms_key], "share_of_step": stage[ms_key] / stage["ms_total"],
+                "algorithmic_bytes": int(nbytes), "achieved_gbs": gbs, "frac_of_peak": gbs / peak,
+                "traffic": load_traffic(kernel)}
 
+    # K1 writes 8 B/record (+ the input once); a partition pass moves 16 B/record; the join reads
+    # 8 B/record and writes 8 B/candidate.  Each of the first three stages is ONE kernel launch on the fused pipeline.
     stages = [
-        hbm("generate + level-1 partition (k_gen2_part; instruction-issue bound, see DESIGN.md)" if fused else
-            "count + scan + generate", "ms_generate", 8 * n_rec + in_bytes),
-        hbm("level-2 partition (k_part2)" if fused else f"{npass} onesweep passes", "ms_sort", 16 * n_rec * npass),
-        hbm("join (k_join_bkt)" if fused else "join", "ms_emit", 8 * n_rec + 8 * n_cand),
-        hbm(f"candidate sort ({ppass} onesweep passes)", "ms_dedup", n_cand * (8 + 16 * ppass)),
-        hbm("unique + verify + unpack", "ms_verify", 8 * n_cand + 64 * st["n_unique"] + 12 * n_out),
+        hbm("S1 generate + level-1 partition" if fused else "S1 count + scan + generate", "k_gen2_part" if fused else "k_gen2",
+            "ms_generate", 8 * n_rec + in_bytes),
+        hbm("S2 level-2 partition" if fused else f"S2 {npass} onesweep passes", "k_part2" if fused else "k_onesweep",
+            "ms_sort", 16 * n_rec * npass),
+        hbm("S3a join / emission", "k_join_bkt" if fused else "k_join_fast", "ms_emit", 8 * n_rec + 8 * n_cand),
+        hbm(f"S3b candidate filter + sort ({ppass} onesweep passes)", "k_cand_filter + k_onesweep", "ms_dedup",
+            n_cand * 16 + st["n_unique"] * 16 * ppass),
+        hbm("S4 unique + verify + unpack", "k_verify", "ms_verify", 8 * n_cand + 64 * st["n_unique"] + 12 * n_out),
     ]
+    # `roofline` describes the DOMINANT kernel of the step: the single-kernel stage with the largest share
+    top = max(stages[:3], key=lambda r: r["ms"])
     line = {
         "metric": METRIC, "value": job_value(n_out, world, ms), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -310,6 +407,7 @@ def main():
                    "prefix_len": args.prefix or None,
                    "chunks": st["n_chunks"], "l2": "flushed between steps (512 MiB memset, untimed)",
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "verified": verified,
         "wall_time_s": ms * 1e-3, "records_per_s": world * n_rec / (ms * 1e-3),
         "step_hbm_gbs": step_bytes / (ms * 1e-3) / 1e9, "step_hbm_frac": step_bytes / (ms * 1e-3) / 1e9 / peak,
         "stage_ms": stage, "stages": stages,
@@ -317,36 +415,28 @@ def main():
                 "h2d_bytes_per_step": int(s.seqs.nbytes + s.offsets.nbytes), "d2h_bytes_per_step": int(12 * n_out),
                 "api": "symdel_self_host (pinned host buffers)"},
         "gpu_launches": int(sum(x["n_launches"] for x in stats_acc)),
-        "roofline": {"bound": "hbm",
-                     "kernel": f"{kname} (one 8-bit radix-partition pass over the variant records: the sort stage)",
-                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": load_traffic(kname), "peak_source": peak_src,
-                     "algorithmic_bytes_per_launch": 16 * n_rec, "launch_ms": pass_ms,
-                     "share_of_step": stage["ms_sort"] / stage["ms_total"],
-                     "frac_of_nominal_8000": achieved / 8000.0},
+        "roofline": {"bound": "hbm", "kernel": f"{top['kernel']} ({top['stage']}; the longest kernel of the step)",
+                     "achieved": top["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": top["frac_of_peak"],
+                     "traffic": top["traffic"], "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": top["algorithmic_bytes"], "launch_ms": top["ms"],
+                     "share_of_step": top["share_of_step"], "frac_of_nominal_8000": top["achieved_gbs"] / 8000.0},
         "clocks": clocks,
     }
-    if fused:
-        # The LONGEST kernel is not the HBM-bound one: k_gen2_part is bound by instruction issue.
-        # Its executed warp instructions per launch come from the committed ncu capture (not an algorithmic count);
-        # peak = 148 SMs x 4 schedulers x 1 warp instruction per clock at the SM clock sampled during the run.
-        winst = load_traffic("k_gen2_part_warp_instructions")
-        sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
-        issue_peak = 148 * 4 * sm_mhz * 1e6 / 1e9
-        if winst and args.config == 3 and not args.dense and not args.prefix:
-            ach = winst / (stage["ms_generate"] * 1e-3) / 1e9
-            line["roofline_longest_kernel"] = {
-                "bound": "alu", "kernel": "k_gen2_part (generation + level-1 partition)", "achieved": ach,
-                "peak": issue_peak, "unit": "G warp-instructions/s (executed, from profiles/traffic.json)",
-                "frac": ach / issue_peak, "launch_ms": stage["ms_generate"],
-                "share_of_step": stage["ms_generate"] / stage["ms_total"],
-                "hbm_gbs": (8 * n_rec + in_bytes) / (stage["ms_generate"] * 1e-3) / 1e9}
     if not args.no_cpu_baseline and world == 1 and not args.dense:
         n_sample = min(s.n, args.ref_sample or 150000)
         pairs, dt = cpu_baseline_run(n_sample, d, s)
         line["cpu_baseline"] = {"value": pairs / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": f"same generator and seed at n={n_sample}, d={d}: {pairs} pairs in {dt:.1f} s "
                                           "(oracle_symdel_self, App. F.1 hash map)"}
+        if gold and gold.get("oracle_wall_s"):
+            line["cpu_baseline_full"] = {
+                "value": gold["n_out"] / gold["oracle_wall_s"], "unit": UNIT, "cores": 1, "kind": "oracle",
+                "sample": f"the whole workload, recorded when tests/golden/{gold_name} was written (another host): "
+                          f"{gold['n_out']} pairs in {gold['oracle_wall_s']} s"}
+    if world == 1 and not args.no_workloads and args.config == 3 and not args.dense and not args.prefix:
+        del ws, out, flush
+        torch.cuda.empty_cache()
+        line["workloads"] = other_workloads(torch, symdel, synth, dev)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -650,27 +650,28 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
 constexpr int GP_THREADS = 256;    // threads per block (512 with two resident blocks: +2 %)
 constexpr int GP_MINB = 3;         // resident blocks per SM (64 KB stage each)
 constexpr int GP_FLUSH_AT = 2800;  // flush when more than this is staged after a round (i.e. after nearly every full round)
-constexpr int GP_OVF = 128;        // overflow list entries
+constexpr int GP_OVF = 64;         // overflow list entries
 constexpr int GP_TRIP = 16;        // d = 3: (g1, g2) iterations per step of a batch
 constexpr int GP_ROUND = 5400;     // records a block stages per round (21 per digit of the 32 slots); the host turns it into batches per warp
 constexpr int GP_NW = GP_THREADS / 32, GP_S = 32;  // (16 slots per digit and 4-5 resident blocks: generation 0.66 -> 0.85-1.25 ms on config 3, the digits overflow)
 static_assert(GP_THREADS >= 256 && GP_THREADS % 32 == 0, "one thread per digit in the flush");
 
+constexpr int GP_ROW = GP_S + 1;  // stage row stride in records: rank r of digit dg sits in 8-byte word dg * 33 + r, i.e. bank pair (dg + r) mod 16 — ranks are alike across digits, the odd stride spreads them
 struct GenPartShared {
-    u64 stage[256 * GP_S];  // digit dg, rank r -> stage[dg * GP_S + ((r + dg) & (GP_S - 1))] (skewed: ranks are alike across digits)
-    u64 U[GP_NW][32];
-    u64 V[GP_NW][32];
+    u64 stage[256 * GP_ROW];
+    // per warp, for the sequence whose first lane is s0 and whose length is L: W[2 * s0 + j] = V[j] for j < L and U[j - L]
+    // for L <= j < 2L — the partner (a + dl) mod L of position a is ONE load at index a + dl, no wrap arithmetic
+    u64 W[GP_NW][64];
     u64 R[32];
     u64 Bpow[33];
-    u32 cnt[256];     // records staged per digit since the last flush (may exceed GP_S: the excess went to the bins directly)
-    uint2 fl[256];    // flush: {index of the claimed segment in bins (0xffffffff = bin full), records to copy}
-    u32 total[3];     // records staged in round r go to total[r % 3] (three words: a fast warp of round r + 1 never touches the word the slow warps of round r still read)
+    u32 cnt[256];     // BYTES staged per digit since the last flush (8 per record; may exceed 8 * GP_S: the excess went to the overflow list)
+    u32 gofs[256];    // flush: index of the claimed segment in bins (0xffffffff = bin full)
+    u32 total[3];     // D3: records staged in round r go to total[r % 3] (three words: a fast warp of round r + 1 never touches the word the slow warps of round r still read)
     u32 novf;         // records in ovf[] (may count past GP_OVF: those went to the bins directly)
     u64 ovf[GP_OVF];  // records whose digit had no free slot: placed at the next flush (near-identical neighbouring sequences — clonal lineages — push the same digits in bursts)
     unsigned char map[GP_NW][32];
 };
-
-static_assert(offsetof(GenPartShared, V) - offsetof(GenPartShared, U) == GP_NW * 256, "k_gen2_part addresses V[warp] through U[warp]");
+static_assert(sizeof(GenPartShared) <= (233472 - GP_MINB * 1024) / GP_MINB, "GP_MINB blocks per SM");
 
 struct GenPartParams {
     GenParams g;
@@ -704,44 +705,49 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     const u64 binv1 = c_Binv[1], binv2 = c_Binv[2];
     const int kshift = 64 - P.hash_bits, id_bits = P.id_bits;  // PLAIN: kshift == id_bits, the record is the hash with its low id_bits replaced by the id
     const u32 idmask_lo = id_bits >= 32 ? 0xffffffffu : ((1u << id_bits) - 1u);
-    const u32 cnt_sa = (u32)__cvta_generic_to_shared(sh.cnt);
-    u64* const Uw = sh.U[warp];
-    u64* const Vw = sh.V[warp];
-    u32 made = 0;  // records this lane staged since the warp last reported
+    // shared-window addresses of the counters and the stage, computed once and kept in registers (left to itself the
+    // compiler re-derives them from SR_CgaCtaId at every use: three instructions per record)
+    u32 cnt_sa = (u32)__cvta_generic_to_shared(sh.cnt), stage_sa = (u32)__cvta_generic_to_shared(sh.stage);
+    asm volatile("" : "+r"(cnt_sa), "+r"(stage_sa));
+    u64* const Ww = sh.W[warp];
+    u32 made = 0;  // D3: records this lane staged since the warp last reported
 
-    auto push = [&](bool valid, u64 h, u64 gid) {
-        if (CHUNKED) valid = valid && gen_chunk_of(h, P.n_chunks) == P.chunk;
-        if (valid) {
-            const u32 dg = (u32)(h >> 56);
-            u64 rec;
-            if (PLAIN) rec = ((u64)(u32)(h >> 32) << 32) | (((u32)h & ~idmask_lo) | (u32)gid);  // id_bits <= 31 here
-            else rec = ((h >> kshift) << id_bits) | gid;
-            u32 r;  // plain ATOMS.ADD with return (no compiler-inserted aggregation)
-            asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(r) : "r"(cnt_sa + dg * 4u) : "memory");
-            if (r < (u32)GP_S) {
-                sh.stage[dg * GP_S + ((r + dg) & (GP_S - 1))] = rec;
+    // one record: its digit's counter (in bytes) hands out the slot; rank r of digit dg -> byte dg * 264 + 8 r of the stage
+    auto push1 = [&](u64 h, u64 gid) {
+        if (CHUNKED && gen_chunk_of(h, P.n_chunks) != P.chunk) return;
+        const u32 dg = (u32)(h >> 56);
+        u64 rec;
+        if (PLAIN) rec = ((u64)(u32)(h >> 32) << 32) | (((u32)h & ~idmask_lo) | (u32)gid);  // id_bits <= 31 here
+        else rec = ((h >> kshift) << id_bits) | gid;
+        u32 r8;  // plain ATOMS.ADD with return (no compiler-inserted aggregation)
+        asm volatile("atom.shared.add.u32 %0, [%1], 8;" : "=r"(r8) : "r"(cnt_sa + dg * 4u) : "memory");
+        const u32 row = stage_sa + dg * (u32)(GP_ROW * 8);
+        if (r8 < (u32)(GP_S * 8)) {
+            asm volatile("st.shared.u64 [%0], %1;" ::"r"(row + r8), "l"(rec) : "memory");
+        } else {
+            const u32 o = atomicAdd(&sh.novf, 1u);
+            if (o < (u32)GP_OVF) {
+                sh.ovf[o] = rec;
             } else {
-                const u32 o = atomicAdd(&sh.novf, 1u);
-                if (o < (u32)GP_OVF) {
-                    sh.ovf[o] = rec;
-                } else {
-                    const u32 at = atomicAdd(&PP.cur[dg], 1u);
-                    if (at < PP.cap1) PP.bins[(u64)dg * PP.cap1 + at] = rec;
-                    else atomicOr(&P.info->part_overflow, 1u);
-                }
+                const u32 at = atomicAdd(&PP.cur[dg], 1u);
+                if (at < PP.cap1) PP.bins[(u64)dg * PP.cap1 + at] = rec;
+                else atomicOr(&P.info->part_overflow, 1u);
             }
-            ++made;
         }
+        if (D3) ++made;
+    };
+    auto push = [&](bool valid, u64 h, u64 gid) {
+        if (valid) push1(h, gid);
     };
 
     // warp task = 32 consecutive sequences of one set, cut into batches that fill the 32 lanes; the block
-    // advances one batch per warp and round, then decides about flushing
+    // advances `batches` batches per warp and round, then flushes
     // (the warps of a block take tasks far apart in the input: neighbouring sequences are often near-identical —
     // clonal lineages — and would all push the same digits at the same time)
     i64 wt = (i64)warp * gridDim.x + blockIdx.x;
     const i64 wstride = (i64)gridDim.x * GP_NW;
     bool have = false;  // a task is loaded and has batches left
-    u32 rnd = 0, staged = 0;  // round index mod 3; records staged since the last flush (block-uniform)
+    u32 rnd = 0, staged = 0;  // D3: round index mod 3; records staged since the last flush (block-uniform)
     u32 s = 0, ns = 0, Li = 0, cum_incl = 0, cum_excl = 0;
     u64 gid0 = 0;
     i64 o0 = 0;  // lane as sequence index: offset of its residues
@@ -780,7 +786,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
             // ---- one step of a batch's triples: GP_TRIP (g1, g2) iterations from where the last step stopped, so
             //      that a step costs every warp the same whatever its sequence lengths ----
             const u32 a = t_a, L = t_L;
-            const u32 uv_sa = (u32)__cvta_generic_to_shared(Uw + t_seg);
+            const u32 v_sa = (u32)__cvta_generic_to_shared(Ww + 2 * t_seg), u_sa = v_sa + 8u * L;
             for (u32 it = 0; it < (u32)GP_TRIP && step <= t_g1max; ++it) {
                 const u32 g1 = step, g2 = t_g2;
                 const u32 g2hi = min((t_Lmax - g1) >> 1, t_Lmax - 2 * g1);  // g3 >= g2 and g3 > g1 (or all equal) at the longest length
@@ -796,9 +802,9 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                 const u32 r2 = D & (D >> 1), r3 = r2 & (D >> 2);
                 const u32 bad = ((D & ~r2) & ~t_ne1) | ((r2 & ~r3) & ~t_ne2) | (r3 & ~t_ne3);
                 u64 u1, v2, v3;
-                asm volatile("ld.shared.u64 %0, [%1];" : "=l"(u1) : "r"(uv_sa + p1 * 8u));
-                asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v2) : "r"(uv_sa + p2 * 8u + (u32)(GP_NW * 256)));
-                asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v3) : "r"(uv_sa + p3 * 8u + (u32)(GP_NW * 256)));
+                asm volatile("ld.shared.u64 %0, [%1];" : "=l"(u1) : "r"(u_sa + p1 * 8u));
+                asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v2) : "r"(v_sa + p2 * 8u));
+                asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v3) : "r"(v_sa + p3 * 8u));
                 push(g2 <= g2hi && ok && bad == 0, u1 + v2 + binv1 * v3 + t_C3, t_gid);
                 if (g2 >= g2hi) {
                     ++step;
@@ -809,7 +815,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
             }
             if (step > t_g1max) {
                 step = 0;
-                __syncwarp();  // U/V/map are reused by the next batch
+                __syncwarp();  // W/map are reused by the next batch
                 s = t_e;
                 have = s < ns;
             }
@@ -855,8 +861,10 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                 const u64 aexcl = aincl - term;
                 const u64 AL = __shfl_sync(SD_FULL, aincl, active ? seg_start + L - 1 : 0);
                 const u64 Uv = aexcl - binv1 * aincl;
-                Uw[lane] = Uv;
-                Vw[lane] = binv1 * Uv;
+                if (active) {  // (2 * seg_start + 2L <= 64: the batch holds at most 32 residues)
+                    Ww[2 * seg_start + a] = binv1 * Uv;
+                    Ww[2 * seg_start + L + a] = Uv;
+                }
                 __syncwarp();
                 push(active && a == 0, AL + (u64)(L + 1) * K_LEN, gid);
                 if (d >= 1) push(canon1, Uv + binv1 * AL + (u64)L * K_LEN, gid);
@@ -868,23 +876,27 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                     const u32 half = __reduce_max_sync(SD_FULL, L >> 1);
                     const u32 dlmax = active ? ((L - 1) >> 1) + (((L & 1u) == 0u && a < (L >> 1)) ? 1u : 0u) : 0u;
                     const u32 m1s = m1 >> seg_start;  // segment-relative mask
-                    const bool c1a = canon1;
-                    const u32 uv_sa = (u32)__cvta_generic_to_shared(Uw + seg_start);  // V[warp] lies GP_NW * 256 bytes after U[warp]
-                    {   // dl = 1: the adjacent pair {a, a + 1} has its own rule; the wrapped pair {0, L - 1} is adjacent only if L == 2
-                        const bool wrap = a + 1 >= L;
-                        const u32 b = wrap ? 0u : a + 1;
-                        const bool ok = wrap ? (L == 2u ? ((madj >> seg_start) & 1u) != 0u : (c1a && (m1s & 1u))) : adjok;
-                        u64 o;
-                        asm volatile("ld.shared.u64 %0, [%1];" : "=l"(o) : "r"(uv_sa + b * 8u + (wrap ? 0u : (u32)(GP_NW * 256))));
-                        push(1u <= dlmax && ok, o + (wrap ? VC : UC), gid);
-                    }
-                    for (u32 dl = 2; dl <= half; ++dl) {
-                        u32 b = a + dl;
-                        const bool wrap = b >= L;
-                        b = wrap ? b - L : b;
-                        u64 o;
-                        asm volatile("ld.shared.u64 %0, [%1];" : "=l"(o) : "r"(uv_sa + (b & 31u) * 8u + (wrap ? 0u : (u32)(GP_NW * 256))));
-                        push(dl <= dlmax && c1a && ((m1s >> (b & 31u)) & 1u), o + (wrap ? VC : UC), gid);
+                    // vmask bit dl: the pair {a, (a + dl) mod L} makes a record.  dl >= 2: both members are canonical
+                    // single deletions; dl = 1: the adjacent pair {a, a + 1} has its own rule, the wrapped pair
+                    // {0, L - 1} is adjacent only if L == 2
+                    const u32 m1L = L >= 32u ? m1s : (m1s & ((1u << L) - 1u));
+                    const u32 rot = (u32)((((u64)m1L << L) | (u64)m1L) >> a);  // bit dl = m1s bit (a + dl) mod L
+                    const bool wrap1 = a + 1 >= L;
+                    const bool ok1 = wrap1 ? (L == 2u ? ((madj >> seg_start) & 1u) != 0u : (canon1 && (m1s & 1u))) : adjok;
+                    u32 vmask = (canon1 ? rot : 0u) & ((2u << dlmax) - 1u) & ~3u;
+                    if (ok1 && dlmax >= 1u) vmask |= 2u;
+                    const u32 wth = L - a;  // dl >= wth: the partner wrapped
+                    const u32 w_sa = (u32)__cvta_generic_to_shared(Ww + 2 * seg_start + a);
+                    u64 UCr = UC, VCr = VC;
+                    asm volatile("" : "+l"(UCr), "+l"(VCr));  // both in registers (else the wrap select is re-derived as a 64-bit multiply per record)
+                    u32 vm = __brev(vmask) << 1;  // bit 31 = dl 1: the sign tells whether this lane has a record
+#pragma unroll 4
+                    for (u32 dl = 1; dl <= half; ++dl, vm <<= 1) {
+                        if ((int)vm < 0) {
+                            u64 o;
+                            asm volatile("ld.shared.u64 %0, [%1];" : "=l"(o) : "r"(w_sa + dl * 8u));
+                            push1(o + (dl >= wth ? VCr : UCr), gid);
+                        }
                     }
                 }
                 if (D3) {  // the triples follow, one first gap per step
@@ -899,26 +911,33 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                     t_C3 = binv1 * binv2 * AL + (u64)(L - 2) * K_LEN;
                     if (t_g1max > 0) step = 1, t_g2 = 1;
                 }
-                if (!D3 || step == 0) __syncwarp();  // U/V/map are reused by the next batch
+                if (!D3 || step == 0) __syncwarp();  // W/map are reused by the next batch
             }
             if (!D3 || step == 0) {
                 s = e;
                 have = s < ns;
             }
-            const u32 wmade = __reduce_add_sync(SD_FULL, made);
-            made = 0;
-            if (lane == 0 && wmade) atomicAdd(&sh.total[rnd], wmade);
+            if (D3) {
+                const u32 wmade = __reduce_add_sync(SD_FULL, made);
+                made = 0;
+                if (lane == 0 && wmade) atomicAdd(&sh.total[rnd], wmade);
+            }
         }
         }
-        // ---- round end: anyone left?  flush when the stage is about full (always at the end) ----
+        // ---- round end: anyone left?  d <= 2: the host sized the round to fill the stage, flush.  D3: flush when the
+        //      stage is about full (always at the end) ----
         const bool more = have || wt < P.groups_total;
         const int any_more = __syncthreads_or(more);
-        staged += sh.total[rnd];
-        rnd = rnd == 2 ? 0 : rnd + 1;
-        if (tid == 0) sh.total[rnd == 2 ? 0 : rnd + 1] = 0;  // the word of the round after next: nobody reads or adds to it now
-        if (staged > (u32)GP_FLUSH_AT || (!any_more && staged > 0)) {
+        bool flush = true;
+        if (D3) {
+            staged += sh.total[rnd];
+            rnd = rnd == 2 ? 0 : rnd + 1;
+            if (tid == 0) sh.total[rnd == 2 ? 0 : rnd + 1] = 0;  // the word of the round after next: nobody reads or adds to it now
+            flush = staged > (u32)GP_FLUSH_AT || (!any_more && staged > 0);
+        }
+        if (flush) {
             if (tid < 256) {
-                const u32 cn_ = min(sh.cnt[tid], (u32)GP_S);
+                const u32 cn_ = min(sh.cnt[tid] >> 3, (u32)GP_S);
                 u32 g = 0;
                 if (cn_) {
                     g = atomicAdd(&PP.cur[tid], cn_);
@@ -929,14 +948,15 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                         g += tid * PP.cap1;
                     }
                 }
-                sh.fl[tid] = make_uint2(g, g == 0xffffffffu ? 0u : cn_);
+                sh.gofs[tid] = g;
             }
             __syncthreads();
-            constexpr u32 DPW = 32 / GP_S;  // digits per warp instruction
-            for (u32 dg = DPW * warp + lane / GP_S; dg < 256; dg += DPW * GP_NW) {
-                const uint2 f = sh.fl[dg];
-                const u32 o = lane & (GP_S - 1);
-                if (o < f.y) PP.bins[f.x + o] = sh.stage[dg * GP_S + ((o + dg) & (GP_S - 1))];
+            u64* const bins = PP.bins;
+#pragma unroll 4
+            for (u32 k = 0; k < 256 / GP_NW; ++k) {
+                const u32 dg = warp * (256 / GP_NW) + k;
+                const u32 g = sh.gofs[dg], cn_ = sh.cnt[dg] >> 3;  // (cn_ may exceed GP_S: lanes stop at 32)
+                if (lane < cn_ && g != 0xffffffffu) bins[g + lane] = sh.stage[dg * GP_ROW + lane];
             }
             for (u32 i = tid; i < min(sh.novf, (u32)GP_OVF); i += GP_THREADS) {  // the overflow records, one global atomic each
                 const u64 rec = sh.ovf[i];
