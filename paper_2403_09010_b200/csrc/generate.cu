@@ -653,8 +653,9 @@ constexpr int GP_FLUSH_AT = 2800;  // flush when more than this is staged after 
 constexpr int GP_OVF = 64;         // overflow list entries
 constexpr int GP_TRIP = 16;        // d = 3: (g1, g2) iterations per step of a batch
 constexpr int GP_ROUND = 5400;     // records a block stages per round (21 per digit of the 32 slots); the host turns it into batches per warp
+                                   // (round 2: rounds of 3,300 records cost +10 %, i.e. ~2.3 us per flush stay exposed; 22 slots with four resident blocks: +7 %)
 constexpr int GP_NW = GP_THREADS / 32, GP_S = 32;  // (16 slots per digit and 4-5 resident blocks: generation 0.66 -> 0.85-1.25 ms on config 3, the digits overflow)
-static_assert(GP_THREADS >= 256 && GP_THREADS % 32 == 0, "one thread per digit in the flush");
+static_assert(GP_THREADS >= 256 && GP_THREADS % 32 == 0 && GP_S <= 32, "one thread per digit in the flush, one lane per slot of a row");
 
 constexpr int GP_ROW = GP_S + 1;  // stage row stride in records: rank r of digit dg sits in 8-byte word dg * 33 + r, i.e. bank pair (dg + r) mod 16 — ranks are alike across digits, the odd stride spreads them
 struct GenPartShared {
@@ -955,7 +956,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
 #pragma unroll 4
             for (u32 k = 0; k < 256 / GP_NW; ++k) {
                 const u32 dg = warp * (256 / GP_NW) + k;
-                const u32 g = sh.gofs[dg], cn_ = sh.cnt[dg] >> 3;  // (cn_ may exceed GP_S: lanes stop at 32)
+                const u32 g = sh.gofs[dg], cn_ = min(sh.cnt[dg] >> 3, (u32)GP_S);
                 if (lane < cn_ && g != 0xffffffffu) bins[g + lane] = sh.stage[dg * GP_ROW + lane];
             }
             for (u32 i = tid; i < min(sh.novf, (u32)GP_OVF); i += GP_THREADS) {  // the overflow records, one global atomic each

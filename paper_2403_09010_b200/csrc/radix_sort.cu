@@ -398,17 +398,10 @@ __global__ void __launch_bounds__(P2_THREADS, P2_MINB) k_part2(const Part2Params
     const u32 total = bhist[tid];
     u32 claimed = 0;
     bool dead = false;
-    if (total) {
-        claimed = atomicAdd(&P.cnt2[(bin << P.b2) + tid], total);
-        if (claimed + total > P.cap2) {
-            atomicOr(&P.info->part_overflow, 2u);
-            dead = true;
-        }
-    }
+    if (total) claimed = atomicAdd(&P.cnt2[(bin << P.b2) + tid], total);
     u32 tile_sum;
     const u32 tstart = sd_block_excl_sum<P2_THREADS>(total, &tile_sum, s_warp);
     bhist[tid] = tstart;
-    s_gofs[tid] = dead ? 0xffffffffu : ((bin << P.b2) + tid) * P.cap2 + claimed - tstart;
     __syncthreads();
 #pragma unroll
     for (int k = 0; k < P2_IPT; ++k) {
@@ -417,6 +410,12 @@ __global__ void __launch_bounds__(P2_THREADS, P2_MINB) k_part2(const Part2Params
             skeys[bhist[(u32)(key[k] >> P.shift) & dmask] + r] = key[k];
         }
     }
+    // the claim is looked at only now: its round trip to L2 ran under the scan and the staging stores
+    if (total && claimed + total > P.cap2) {
+        atomicOr(&P.info->part_overflow, 2u);
+        dead = true;
+    }
+    s_gofs[tid] = dead ? 0xffffffffu : ((bin << P.b2) + tid) * P.cap2 + claimed - tstart;
     __syncthreads();
 #pragma unroll
     for (int k = 0; k < P2_IPT; ++k) {
