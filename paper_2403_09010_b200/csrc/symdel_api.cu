@@ -43,6 +43,9 @@ struct symdel_ctx {
     void* in_arena = nullptr;   // ... and their inputs (separate: the copies start before the workspace size is known)
     size_t in_arena_bytes = 0;
     cudaStream_t stream = nullptr;  // stream of the *_host entry points
+    cudaStream_t side = nullptr;    // the verifier's bit-plane table is packed here, beside generation (forked from / joined into the caller's stream by events)
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    bool side_pending = false;      // work was forked to `side` and the caller's stream has not been made to wait for it yet
     std::vector<cudaEvent_t> events;
 };
 
@@ -177,7 +180,7 @@ int err_from_flags(u32 f) {
 }
 
 // -------------------------------------------------------------------------------------------------
-int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, void* workspace, i64 workspace_bytes,
+int run_pipeline_body(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, void* workspace, i64 workspace_bytes,
                  i32* out_i, i32* out_j, i32* out_dist, i64 capacity, i64* n_pairs_host, cudaStream_t st) {
     if (!ctx || !n_pairs_host || d < 0 || d > SD_D_MAX || A.n < 0 || B.n < 0 || capacity < 0) return SYMDEL_E_ARG;
     *n_pairs_host = 0;
@@ -251,7 +254,18 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     void* slots = ws.take<char>(sd_pack_bytes(n_total, maxlen));
     u32* fcnt = ws.take<u32>(256 + 2 * FUSED_MAX_BUCKETS);  // fused pipeline: level-1 cursors | level-2 counts | redo list
     if (!ws.ok) return SYMDEL_E_WORKSPACE;
-    CK(sd_pack(A, B, maxlen, slots, info, st, &S.n_launches));
+    // (only the verifier reads the table, and k_pack's residue check is looked at after the join: the kernel runs on the
+    //  side stream while the caller's stream generates; join_side() makes the caller's stream wait for it)
+    CK(cudaEventRecord(ctx->ev_fork, st));
+    CK(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+    CK(sd_pack(A, B, maxlen, slots, info, ctx->side, &S.n_launches));
+    CK(cudaEventRecord(ctx->ev_join, ctx->side));
+    ctx->side_pending = true;
+    auto join_side = [&]() -> cudaError_t {
+        if (!ctx->side_pending) return cudaSuccess;
+        ctx->side_pending = false;
+        return cudaStreamWaitEvent(st, ctx->ev_join, 0);
+    };
 
     // ---- workspace plan ----
     const i64 R = ws.left() - 8192;
@@ -285,7 +299,7 @@ int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, vo
     const FusedPlan fp = plan_fused(ncap);
     u64* recA = ws.take<u64>(std::max(ncap, fp.bins_rec));
     u64* recB = ws.take<u64>(std::max(ncap, fp.bkt_rec));
-    u32 *cur1 = fcnt, *cnt2 = fcnt + 256, *redo = fcnt + 256 + FUSED_MAX_BUCKETS;
+    u32 *cur1 = fcnt, *cnt2 = fcnt + 256;
     void* rec_scratch = ws.take<char>(sd_sort_scratch_bytes(ncap, npass_max));
     u64* tile_prefix = ws.take<u64>(2 * sd_join_tiles(ncap) + 2);
     const i64 cphys = ccap + cslack;
@@ -340,6 +354,7 @@ restart:
             const u32 bcap = (u32)(fp.b2 ? fp.cap2 : fp.cap1), nb = (u32)fp.nbuckets;
             CK(sd_join_bkt(bkt, bcnt, bcap, nb, lay, candA, (u64)ccap, info, st, &S.n_launches));
             u32* h_cur = reinterpret_cast<u32*>(ctx->h_info + 1);
+            CK(join_side());
             CK(cudaMemcpyAsync(h_cur, cur1, 256 * sizeof(u32), cudaMemcpyDeviceToHost, st));
             rc = read_info(ctx, info, st);
             if (rc) return rc;
@@ -367,6 +382,7 @@ restart:
         // ---- S1: count, scan, generate ----
         CK(sd_count(A, B, lay, width, cnt, info, st, &S.n_launches));
         CK(sd_scan_counts(cnt, n_total, rec_off, scan_lb, info, st, &S.n_launches));
+        CK(join_side());
         rc = read_info(ctx, info, st);
         if (rc) return rc;
         N = (i64)ctx->h_info->n_records;
@@ -566,6 +582,18 @@ restart:
     return n_out > capacity ? SYMDEL_E_CAPACITY : SYMDEL_OK;
 }
 
+// Every way out of the pipeline leaves the caller's stream ordered after the side stream's work (which reads and
+// writes the caller's workspace): a caller may release the workspace in stream order right after the call.
+int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, void* workspace, i64 workspace_bytes, i32* out_i,
+                 i32* out_j, i32* out_dist, i64 capacity, i64* n_pairs_host, cudaStream_t st) {
+    const int rc = run_pipeline_body(ctx, A, B, cross, d, workspace, workspace_bytes, out_i, out_j, out_dist, capacity, n_pairs_host, st);
+    if (ctx && ctx->side_pending) {
+        ctx->side_pending = false;
+        if (cudaStreamWaitEvent(st, ctx->ev_join, 0) != cudaSuccess) cudaStreamSynchronize(ctx->side);
+    }
+    return rc;
+}
+
 int ensure_arena(symdel_ctx* ctx, void** arena, size_t* have, size_t bytes) {
     if (*have >= bytes) return SYMDEL_OK;
     if (*arena) cudaFree(*arena);
@@ -672,6 +700,9 @@ int symdel_create(symdel_ctx** out, int device) {
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaMallocHost((void**)&ctx->h_info, sizeof(DevInfo) + 256 * sizeof(u32));
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->side, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
     if (e == cudaSuccess) {
         // Constant tables and function attributes are per DEVICE: every context sets them up for its own device
         // (idempotent; serialised so that two threads creating contexts never interleave the uploads).
@@ -696,6 +727,9 @@ void symdel_destroy(symdel_ctx* ctx) {
     if (ctx->in_arena) cudaFree(ctx->in_arena);
     if (ctx->h_info) cudaFreeHost(ctx->h_info);
     if (ctx->stream) cudaStreamDestroy(ctx->stream);
+    if (ctx->side) cudaStreamDestroy(ctx->side);
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     for (auto e : ctx->events) cudaEventDestroy(e);
     delete ctx;
 }
