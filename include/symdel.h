@@ -91,6 +91,7 @@ typedef struct {
     int64_t fused_chunks;      /* chunks that went through the fused pipeline (generation + partition in one kernel, bucket join) */
     int64_t join_redo_tiles;   /* join tiles that overflowed the small candidate list and were redone by the large-list kernel */
     int64_t surv_merges;       /* multi-flush searches: times the survivor list was sorted and deduplicated to make room */
+    int64_t join_windows;      /* fused pipeline: extra passes of the bucket join (the pairs of a chunk exceeded one candidate window) */
 } symdel_stats;
 
 /* Options (symdel_set_option); defaults in brackets. */

@@ -26,6 +26,7 @@ struct DevInfo {
     u64 win_end;     // join: end (flat pair index) of what the last round wrote
     u32 join_fallback;  // k_join_fast: 1 = a tile's list overflowed, 2 = the pairs do not fit the window
     u32 join_redo;      // k_join_fast: tiles on the redo list (keep right after join_fallback: cleared together)
+    u64 nofit_inv;      // k_join_bkt: ~(smallest claim base that did not fit the window), 0 = every claim fit (keep right after join_redo: cleared together)
     u32 part_overflow;  // fused pipeline: 1 = a level-1 bin was full, 2 = a level-2 bucket was full
     u32 surv_overflow;  // k_verify: the survivors of this flush did not fit behind the survivor list (nothing lost: the host merges the list and repeats the flush)
     u64 residues;       // sum of the (prefix-truncated) sequence lengths

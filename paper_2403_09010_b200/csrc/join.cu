@@ -609,9 +609,10 @@ constexpr int JF_LMAX_L = JF_T + 4096, JF_SLOTB_L = 12, JF_MINB_L = JF_IT > 8 ? 
 // +35 %).  Two instances: regions of up to 4064 records (NB = 12) and up to 18432 (1024 threads, NB = 15: chunks
 // of more than ~2 * 10^8 records).  If the claims run past the
 // candidate window info->join_fallback is raised (the host then uses the exact pipeline).
+constexpr u32 JB_OPEN = 0x80000000u;
 struct JoinBktParams {
     JoinParams j;       // rec = bucket regions; topmask unused
-    const u32* cnt;     // records per bucket
+    u32* cnt;           // records per bucket; bit 31 = its pairs did not fit the window of an earlier pass (windowed searches: later passes join exactly these)
     u32 cap;            // region stride (records; a multiple of 32)
     u32 nbuckets;
 };
@@ -672,8 +673,16 @@ __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams 
     const JoinParams& P = BP.j;
     const u32 tid = threadIdx.x;
     const u32 bucket = blockIdx.x;
-    const u32 n = min(BP.cnt[bucket], BP.cap);
-    if (n < 2) return;  // nothing to pair (block-uniform)
+    const u32 cword = BP.cnt[bucket];
+    if (!P.first_round && !(cword & JB_OPEN)) return;  // later pass of a windowed search: only the buckets left open (block-uniform)
+    const u32 n = min(cword & ~JB_OPEN, BP.cap);
+    if (n < 2) return;  // nothing to pair
+    // later pass of a windowed search and the window is already full: this bucket waits for the next pass (nothing loaded,
+    // nothing counted).  One thread looks, the barrier makes the decision the block's.
+    if (!P.first_round && __syncthreads_or(tid == 0 && sd_ld_relaxed(&P.info->n_cand) >= P.win_hi)) {
+        if (tid == 0) atomicOr(&P.info->join_fallback, 2u);
+        return;
+    }
     if (tid == 0) {
         S.total = 0;
         jb_mbar_init(&S.mbar, 1);
@@ -736,12 +745,24 @@ __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams 
     if (cnt) mine = jf_atoms_add(&S.total, cnt);
     __syncthreads();
     const u32 total = S.total;
-    if (total == 0) return;
+    if (total == 0) {
+        if (tid == 0 && (cword & JB_OPEN)) BP.cnt[bucket] = cword & ~JB_OPEN;
+        return;
+    }
     if (tid == 0) {
         const u64 base = (u64)atomicAdd((unsigned long long*)&P.info->n_cand, (unsigned long long)total);
-        // does not fit the window: nothing is written
-        if (base + total > P.win_hi) atomicOr(&P.info->join_fallback, 2u), S.base = ~0ull;
-        else S.base = base;
+        // Does not fit the window: nothing is written, the bucket stays open for the next pass.  Claims are totally
+        // ordered by the atomic: every claim after the first that does not fit starts beyond the window too, so the
+        // pairs written are exactly [0, win_end) with win_end = the smallest base that did not fit.
+        if (base + total > P.win_hi) {
+            atomicOr(&P.info->join_fallback, 2u);
+            atomicMax((unsigned long long*)&P.info->nofit_inv, (unsigned long long)~base);
+            if (!(cword & JB_OPEN)) BP.cnt[bucket] = cword | JB_OPEN;
+            S.base = ~0ull;
+        } else {
+            S.base = base;
+            if (cword & JB_OPEN) BP.cnt[bucket] = cword & ~JB_OPEN;
+        }
     }
     __syncthreads();
     if (S.base == ~0ull) return;
@@ -884,16 +905,18 @@ int sd_join_bkt_max_cap() { return JB_STAGE_L; }
 // (partitioned hash bits, or zeros above a narrowed hash): they carry the chain link
 int sd_join_bkt_link_bits(u32 cap) { return cap <= (u32)JB_STAGE_S ? JB_NB_S : JB_NB_L; }
 
-cudaError_t sd_join_bkt(const u64* buckets, const u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
-                        DevInfo* info, cudaStream_t st, i64* launches) {
+cudaError_t sd_join_bkt(const u64* buckets, u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
+                        int first_pass, DevInfo* info, cudaStream_t st, i64* launches) {
     cudaError_t e;
     if ((e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
-    if ((e = cudaMemsetAsync(&info->join_fallback, 0, 2 * sizeof(u32), st)) != cudaSuccess) return e;  // and join_redo
+    static_assert(offsetof(DevInfo, nofit_inv) == offsetof(DevInfo, join_fallback) + 8, "cleared together");
+    if ((e = cudaMemsetAsync(&info->join_fallback, 0, 2 * sizeof(u32) + sizeof(u64), st)) != cudaSuccess) return e;  // and join_redo, nofit_inv
     if (nbuckets == 0) return cudaSuccess;
     JoinBktParams BP{};
     BP.j = jn_params(buckets, 0, lay, cand, window, info);
     BP.j.win_lo = 0;
     BP.j.win_hi = window;
+    BP.j.first_round = first_pass;
     BP.cnt = cnt;
     BP.cap = cap;
     BP.nbuckets = nbuckets;

@@ -102,11 +102,13 @@ cudaError_t sd_join_fast_redo(const u64* records, i64 n_records, const Layout& l
                               u32 n_redo, DevInfo* info, cudaStream_t st, i64* launches);
 
 // Bucket join of the fused pipeline (see join.cu): one block per bucket (regions of `cap` <= sd_join_bkt_max_cap()
-// records).  Clears and fills info->n_cand; info->join_fallback != 0: the pairs did not fit `window`.
+// records).  Clears and fills info->n_cand; info->join_fallback != 0: the pairs did not fit `window`:
+// cand[0 .. min(n_cand, ~info->nofit_inv)) holds the pairs of the buckets that fit; the others are marked open (bit 31 of their
+// count) and a further call with first_pass = 0 joins exactly those.
 int sd_join_bkt_max_cap();
 int sd_join_bkt_link_bits(u32 cap);  // bits on top of a record that must be constant within a bucket
-cudaError_t sd_join_bkt(const u64* buckets, const u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
-                        DevInfo* info, cudaStream_t st, i64* launches);
+cudaError_t sd_join_bkt(const u64* buckets, u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
+                        int first_pass, DevInfo* info, cudaStream_t st, i64* launches);
 
 // ---- verify.cu ----------------------------------------------------------------------------------
 i64 sd_verify_tiles(i64 n);

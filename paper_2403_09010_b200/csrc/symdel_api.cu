@@ -51,9 +51,15 @@ struct symdel_ctx {
 
 namespace {
 
+#ifdef SD_DEBUG_SYNC
+#define CK_DBG_SYNC(call) if (e__ == cudaSuccess) { e__ = cudaDeviceSynchronize(); if (e__ != cudaSuccess) fprintf(stderr, "[sd] %s -> %s\n", #call, cudaGetErrorString(e__)); }
+#else
+#define CK_DBG_SYNC(call)
+#endif
 #define CK(call)                                  \
     do {                                          \
         cudaError_t e__ = (call);                 \
+        CK_DBG_SYNC(call)                         \
         if (e__ != cudaSuccess) {                 \
             ctx->last_cuda = e__;                 \
             return SYMDEL_E_CUDA;                 \
@@ -332,11 +338,16 @@ restart:
     CK(cudaMemsetAsync(&info->n_surv, 0, sizeof(u64) * 3, st));  // n_surv, n_out, n_unique
     for (u32 c = 0; c < P; ++c) {
         lay.chunk = c;
+        bool chunk_exact = false;  // a windowed fused search met a bucket whose pairs exceed a whole window: the chunk is redone by the exact pipeline
+    redo_chunk:
         // ---- fused pipeline: generation + level-1 partition, level-2 partition, bucket join ----
-        bool fused_ok = false;
+        bool fused_ok = false, fused_more = false;  // fused_more: buckets whose pairs did not fit the window wait for the next pass
         i64 C = 0, wend = 0, N = 0;
+        const u64* f_bkt = nullptr;
+        u32* f_bcnt = nullptr;
+        u32 f_bcap = 0, f_nb = 0;
         // (a chunk expected to hold 2^30 records or more goes to the exact pipeline, which splits it further)
-        if (!ctx->opt_exact && ctx->opt_sort_bits < 0 && !ctx->opt_join_general && lay.hash_bits >= fp.b &&
+        if (!chunk_exact && !ctx->opt_exact && ctx->opt_sort_bits < 0 && !ctx->opt_join_general && lay.hash_bits >= fp.b &&
             nmax / (i64)P < ((i64)1 << 30) && fp.cap2 <= sd_join_bkt_max_cap() && 64 - (lay.id_bits + lay.hash_bits) + fp.b >= sd_join_bkt_link_bits((u32)fp.cap2) &&
             sd_gen_part_applies(lay, width)) {
             const size_t x0 = tm.mark();
@@ -349,20 +360,23 @@ restart:
                 CK(sd_part2(recA, cur1, fp.cap1, recB, cnt2, fp.cap2, fp.b2, lay.id_bits + lay.hash_bits - fp.b, info, st,
                             &S.n_launches));
             const size_t x2 = tm.mark();
-            const u64* bkt = fp.b2 ? recB : recA;
-            const u32* bcnt = fp.b2 ? cnt2 : cur1;
-            const u32 bcap = (u32)(fp.b2 ? fp.cap2 : fp.cap1), nb = (u32)fp.nbuckets;
-            CK(sd_join_bkt(bkt, bcnt, bcap, nb, lay, candA, (u64)ccap, info, st, &S.n_launches));
+            f_bkt = fp.b2 ? recB : recA;
+            f_bcnt = fp.b2 ? cnt2 : cur1;
+            f_bcap = (u32)(fp.b2 ? fp.cap2 : fp.cap1), f_nb = (u32)fp.nbuckets;
             u32* h_cur = reinterpret_cast<u32*>(ctx->h_info + 1);
+            CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 1, info, st, &S.n_launches));
             CK(join_side());
-            CK(cudaMemcpyAsync(h_cur, cur1, 256 * sizeof(u32), cudaMemcpyDeviceToHost, st));
+            CK(cudaMemcpyAsync(h_cur, cur1, 256 * sizeof(u32), cudaMemcpyDeviceToHost, st));  // (bit 31 of a count is the join's "open" mark)
             rc = read_info(ctx, info, st);
             if (rc) return rc;
             if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
-            fused_ok = !ctx->h_info->part_overflow && !ctx->h_info->join_fallback;
+            // pairs beyond one window: the buckets that fit are done, the others are joined by later passes (window loop below)
+            fused_more = ctx->h_info->join_fallback != 0;
+            C = (i64)std::min<u64>(ctx->h_info->n_cand, ~ctx->h_info->nofit_inv);
+            fused_ok = !ctx->h_info->part_overflow && !(fused_more && C == 0);
+            if (!fused_ok) fused_more = false, C = 0;
             if (fused_ok) {
-                for (int i = 0; i < 256; ++i) N += h_cur[i];
-                C = (i64)ctx->h_info->n_cand;
+                for (int i = 0; i < 256; ++i) N += h_cur[i] & 0x7fffffffu;
                 wend = C;
                 const size_t x3 = tm.mark();
                 tm.span(ST_GEN, x0, x1);
@@ -440,9 +454,29 @@ restart:
         pass_count += npass;
         S.sort_pass_records = N;
         }  // exact pipeline
-        for (i64 w0 = 0; w0 < C;) {
+        for (i64 w0 = 0; w0 < C || fused_more;) {
             const size_t f0 = tm.mark();
-            if (w0 > 0) {
+            if (fused_ok && w0 > 0) {
+                // ---- next pass of the bucket join: the buckets not marked done, into a fresh window ----
+                CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 0, info, st, &S.n_launches));
+                rc = read_info(ctx, info, st);
+                if (rc) return rc;
+                if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+                fused_more = ctx->h_info->join_fallback != 0;
+                const i64 X = (i64)std::min<u64>(ctx->h_info->n_cand, ~ctx->h_info->nofit_inv);
+                if (fused_more && X == 0) {  // one bucket's pairs exceed a whole window (what was appended so far stays: the final pass removes repeats)
+                    chunk_exact = true;
+                    S.n_records -= N;
+                    --S.fused_chunks;
+                    ++flushes;  // (forces the final sort + unique even if nothing else is flushed twice)
+                    goto redo_chunk;
+                }
+                C += X;
+                wend = w0 + X;
+                S.n_candidates += X;
+                ++S.join_windows;
+                if (X == 0) break;  // the remaining buckets had no pairs
+            } else if (w0 > 0) {
                 CK(sd_join(sorted, N, lay, candA, (u64)cphys, (u64)w0, (u64)(w0 + ccap), 0, tile_prefix, info, st,
                            &S.n_launches));
                 rc = read_info(ctx, info, st);
@@ -464,8 +498,9 @@ restart:
             if (use_filter) {
                 // duplicate suppression before the sort: a best-effort hash set in a record buffer that is free now
                 // (fused: the level-1 bins; exact: the ping-pong buffer that does not hold the partitioned records)
-                u64* table = sorted == recA ? recB : recA;
-                const i64 table_room = sorted == recA ? std::max(ncap, fp.bkt_rec) : std::max(ncap, fp.bins_rec);
+                const bool in_b = fused_ok ? fp.b2 == 0 : sorted == recA;  // fused: the buckets (recB, or recA without a level 2) may be joined again
+                u64* table = in_b ? recB : recA;
+                const i64 table_room = in_b ? std::max(ncap, fp.bkt_rec) : std::max(ncap, fp.bins_rec);
                 int tb = 16;
                 while (tb < 27 && ((i64)1 << tb) < nc) ++tb;
                 while (tb > 10 && ((i64)1 << tb) > table_room) --tb;
@@ -484,7 +519,7 @@ restart:
             const size_t f2 = tm.mark();
             // ---- S4: unique + verify; survivors appended at n_surv — or, when this window holds every candidate of
             //      the only chunk, unpacked straight into the outputs (no survivor list, no finalize) ----
-            direct = P == 1 && w0 == 0 && wend == C;
+            direct = P == 1 && w0 == 0 && wend == C && !fused_more && flushes == 0;
             if (direct)
                 CK(sd_verify_direct(csorted, nc, nc_dev, slots, lay, maxlen, out_i, out_j, out_dist, capacity, verify_lb, info, st,
                                     &S.n_launches));

@@ -39,7 +39,7 @@ class Stats(C.Structure):
         ("ms_prepare", C.c_float), ("ms_generate", C.c_float), ("ms_sort", C.c_float), ("ms_emit", C.c_float),
         ("ms_dedup", C.c_float), ("ms_verify", C.c_float), ("ms_total", C.c_float), ("ms_sort_pass_avg", C.c_float),
         ("sort_pass_records", C.c_int64), ("fused_chunks", C.c_int64), ("join_redo_tiles", C.c_int64),
-        ("surv_merges", C.c_int64),
+        ("surv_merges", C.c_int64), ("join_windows", C.c_int64),
     ]
 
     def as_dict(self):

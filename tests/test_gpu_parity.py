@@ -327,7 +327,11 @@ def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
         assert st["n_chunks"] == opts["FORCE_CHUNKS"]
     if "CAND_CAPACITY" in opts:
         assert st["n_flushes"] > 1
-        assert st["join_general"] >= 1  # the pairs exceed one window: the fast join kernel hands over
+        if set(opts) <= {"CAND_CAPACITY", "FORCE_CHUNKS", "CAND_FILTER", "HASH_BITS"}:
+            # the pairs exceed one window: the bucket join runs again over the buckets that did not fit (fused all the way)
+            assert st["join_windows"] >= 1 and st["join_general"] == 0 and st["fused_chunks"] == st["n_chunks"]
+        else:
+            assert st["join_general"] >= 1  # exact pipeline: the fast join kernel hands over to the windowed one
     if "JOIN_GENERAL" in opts:
         assert st["join_general"] == st["n_chunks"]
     if (not opts or set(opts) <= {"FORCE_CHUNKS", "HASH_BITS", "NO_THINNING"}) and opts.get("HASH_BITS", 64) >= 16:
@@ -342,7 +346,7 @@ def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
 @pytest.mark.parametrize("copies,sort_bits,general,expect_general", [
     (10, 0, 0, 0),     # dense but inside one window and the list capacity: the fast kernel finishes
     (10, 255, 0, 1),   # one bucket: the first tile lists every record, overflows, hands over
-    (40, 0, 0, 1),     # 3.7 M pairs: more than the default window
+    (40, 0, 0, 1),     # 40 copies overflow the fixed-capacity buckets (exact pipeline); 3.7 M pairs: more than its default window
     (40, 0, 1, 1),
 ])
 def test_join_dense_runs(sd, oracle, copies, sort_bits, general, expect_general):
@@ -656,6 +660,36 @@ def test_config_full_size_chunked(torch, sd, oracle, num, opts, ws_frac):
     if "EXACT_PIPELINE" not in opts:
         assert st["fused_chunks"] == st["n_chunks"]  # every chunk stays on the fused pipeline
     assert st["n_flushes"] >= st["n_chunks"]
+
+
+@pytest.mark.parametrize("num,window", [(3, 1_000_000), (5, 3_000_000)])
+def test_config_full_size_windowed_bucket_join(torch, sd, num, window):
+    """The paper's large regime has more matched pairs than one candidate buffer holds (Table S1: 11.3 B
+    pairs from 1.2 B variants).  With the candidate window capped, the fused pipeline joins the buckets that fit, flushes,
+    and joins the rest in further passes: same golden digest, no hand-over to the exact pipeline."""
+    g = _golden(f"config_{num}.json")
+    kind, d, (s,) = synth.config(num)
+    c = sd.Context(0)
+    c.symdel_set_option(sd.OPT_CAND_CAPACITY, window)
+    ds, do = sd.to_device(s)
+    i, j, dist = [t.cpu().numpy() for t in c.symdel_self(ds, do, d, capacity=1 << 20)]
+    st = c.symdel_get_stats()
+    assert_matches_golden(g, i, j, dist)
+    assert st["fused_chunks"] == st["n_chunks"] == 1 and st["join_general"] == 0
+    assert st["join_windows"] >= st["n_candidates"] // window - 1 >= 2 and st["n_flushes"] == st["join_windows"] + 1
+
+
+def test_windowed_bucket_join_single_bucket_exceeds_window(sd, oracle):
+    """A bucket whose own pairs exceed a whole window cannot be windowed bucket by bucket: the chunk is handed to the exact
+    pipeline (windowed join inside a bucket), whatever was flushed before; the final pass removes the repeats."""
+    rows, lens = synth.to_padded(synth.tcr_set(1500, 5))
+    s = synth.from_padded(np.concatenate([rows] * 30), np.concatenate([lens] * 30))
+    exp = oracle.symdel_self(s.seqs, s.offsets, 1)
+    c = sd.Context(0)
+    c.symdel_set_option(sd.OPT_CAND_CAPACITY, 300)  # 30 copies: 435 pairs on every variant key
+    assert_same(run_self(sd, c, s, 1, capacity=len(exp[0]) + 16), exp)
+    st = c.symdel_get_stats()
+    assert st["join_general"] >= 1
 
 
 def test_dense_full_size(sd, ctx):
