@@ -42,21 +42,31 @@ __device__ __forceinline__ u32 gen_chunk_of(u64 h, u32 n_chunks) { return __umul
 
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, int prefix, DevInfo* info) {
+    // V(L, d) for every length, in shared memory: the lanes of a warp ask for different lengths, which the constant
+    // cache would serve one address at a time
+    __shared__ u32 s_v[SD_L_MAX + 1];
+    __shared__ u64 s_nmax[8], s_res[8];
+    __shared__ u32 s_maxlen[8], s_err[8];
+    if (threadIdx.x <= SD_L_MAX) s_v[threadIdx.x] = c_vcum[threadIdx.x * (SD_D_MAX + 2) + d + 1];
+    __syncthreads();
     u64 nmax = 0, res = 0;
     u32 maxlen = 0, err = 0;
     const i64 stride = (i64)gridDim.x * blockDim.x;
     const i64 t0 = (i64)blockIdx.x * blockDim.x + threadIdx.x;
+    i64 a = t0 < s.n ? s.off[t0] : 0;
     for (i64 i = t0; i < s.n; i += stride) {
-        i64 a = s.off[i], b = s.off[i + 1];
+        const i64 b = s.off[i + 1];
+        const i64 an = i + stride < s.n ? s.off[i + stride] : 0;  // (next iteration's first offset, in flight with this one's second)
         if (i == 0 && a != 0) err |= SD_ERR_OFFSETS;
         i64 L = b - a;
         if (L < 0 || a < 0) err |= SD_ERR_OFFSETS;
         else if (L > SD_L_MAX) err |= SD_ERR_TOO_LONG;
         else {
-            nmax += c_vcum[min(L, (i64)prefix) * (SD_D_MAX + 2) + d + 1];
+            nmax += s_v[min(L, (i64)prefix)];
             res += (u64)min(L, (i64)prefix);
             maxlen = max(maxlen, (u32)L);
         }
+        a = an;
     }
     // (the residue codes are range-checked by k_pack / k_check_residues, which run only after the offsets
     //  have been found valid: a malformed offsets array must never steer a read of `seqs`)
@@ -67,7 +77,12 @@ __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, i
         maxlen = max(maxlen, __shfl_xor_sync(SD_FULL, maxlen, o));
         err |= __shfl_xor_sync(SD_FULL, err, o);
     }
-    if ((threadIdx.x & 31) == 0) {
+    // one set of global atomics per BLOCK (they all hit the same few words of info)
+    const u32 warp = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0) s_nmax[warp] = nmax, s_res[warp] = res, s_maxlen[warp] = maxlen, s_err[warp] = err;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 8; ++w) nmax += s_nmax[w], res += s_res[w], maxlen = max(maxlen, s_maxlen[w]), err |= s_err[w];
         if (nmax) atomicAdd((unsigned long long*)&info->nmax, (unsigned long long)nmax);
         if (res) atomicAdd((unsigned long long*)&info->residues, (unsigned long long)res);
         if (nmax && is_b) atomicAdd((unsigned long long*)&info->nmax_b, (unsigned long long)nmax);
