@@ -10,6 +10,8 @@ typedef int64_t i64;
 typedef int32_t i32;
 
 #define SD_FULL 0xffffffffu
+#define SD_L_MAX 64  // longest sequence (one Myers word) = SYMDEL_L_MAX of include/symdel.h
+#define SD_D_MAX 4   // = SYMDEL_D_MAX
 
 // ---- device status block (one per call, in the workspace; copied to pinned host memory) --------
 struct DevInfo {
@@ -31,6 +33,7 @@ struct DevInfo {
     u32 surv_overflow;  // k_verify: the survivors of this flush did not fit behind the survivor list (nothing lost: the host merges the list and repeats the flush)
     u64 residues;       // sum of the (prefix-truncated) sequence lengths
     u64 n_filt;         // candidates of the current window that passed the duplicate filter (k_cand_filter)
+    u32 len_hist[SD_L_MAX + 1];  // sequences per (prefix-truncated) length: the host lays the key-range chunks out over the variant lengths
 };
 enum { SD_ERR_OFFSETS = 1, SD_ERR_TOO_LONG = 2, SD_ERR_RESIDUE = 4, SD_ERR_INTERNAL = 8, SD_ERR_OVERFLOW = 16 };
 enum { SD_TK_SORT = 0, SD_TK_EMIT = 1, SD_TK_VERIFY = 2, SD_TK_FINAL = 3, SD_TK_SCAN = 4 };

@@ -36,9 +36,17 @@ __constant__ u32 c_vcum[(SD_L_MAX + 1) * (SD_D_MAX + 2)];   // sum_{j<k} C(n, j)
 
 constexpr u64 K_LEN = 0x9fb21c651e98df25ull;
 
-// Key-range chunk of a variant hash (S5): a function of the LOW word only, so the sorted key (the top
-// hash_bits) stays uniformly distributed inside every chunk.
-__device__ __forceinline__ u32 gen_chunk_of(u64 h, u32 n_chunks) { return __umulhi((u32)h * 0x9e3779b1u, n_chunks); }
+// Key-range chunks (S5).  Variants of different LENGTHS never meet, so the chunks are laid out along the axis
+// (variant length, hash fraction): position = vlen << 32 | f(low word of the hash), chunk = [chunk_lo, chunk_hi).  A
+// sequence of length L only has to enumerate the deletion depths k whose variant length L - k reaches into the chunk —
+// over all chunks every deletion set is enumerated once, except at the lengths a chunk boundary cuts (those are split
+// by the hash fraction: a function of the LOW word only, so the partitioned top bits stay uniform inside every chunk).
+__device__ __forceinline__ bool gen_in_chunk(u64 h, u32 vlen, u64 lo, u64 hi) {
+    const u64 pos = ((u64)vlen << 32) | (u64)((u32)h * 0x9e3779b1u);
+    return pos >= lo && pos < hi;
+}
+// does any record of variant length vlen belong to the chunk?
+__device__ __forceinline__ bool gen_len_in_chunk(u32 vlen, u64 lo, u64 hi) { return (((u64)vlen + 1) << 32) > lo && ((u64)vlen << 32) < hi; }
 
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, int prefix, DevInfo* info) {
@@ -47,7 +55,8 @@ __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, i
     __shared__ u32 s_v[SD_L_MAX + 1];
     __shared__ u64 s_nmax[8], s_res[8];
     __shared__ u32 s_maxlen[8], s_err[8];
-    if (threadIdx.x <= SD_L_MAX) s_v[threadIdx.x] = c_vcum[threadIdx.x * (SD_D_MAX + 2) + d + 1];
+    __shared__ u32 s_lh[SD_L_MAX + 1];  // sequences of this block per (truncated) length
+    if (threadIdx.x <= SD_L_MAX) s_v[threadIdx.x] = c_vcum[threadIdx.x * (SD_D_MAX + 2) + d + 1], s_lh[threadIdx.x] = 0;
     __syncthreads();
     u64 nmax = 0, res = 0;
     u32 maxlen = 0, err = 0;
@@ -65,6 +74,7 @@ __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, i
             nmax += s_v[min(L, (i64)prefix)];
             res += (u64)min(L, (i64)prefix);
             maxlen = max(maxlen, (u32)L);
+            atomicAdd(&s_lh[min(L, (i64)prefix)], 1u);
         }
         a = an;
     }
@@ -89,6 +99,7 @@ __global__ void __launch_bounds__(256) k_prepare(SeqSetDev s, int d, int is_b, i
         if (maxlen) atomicMax(&info->maxlen, maxlen);
         if (err) atomicOr(&info->err, err);
     }
+    if (threadIdx.x <= SD_L_MAX && s_lh[threadIdx.x]) atomicAdd(&info->len_hist[threadIdx.x], s_lh[threadIdx.x]);
 }
 
 // Residue range check on its own (the stage entry point that does not pack).  Launched after k_prepare: does
@@ -173,6 +184,7 @@ struct GenParams {
     i64 n_a;
     int d, width, thinning, hash_bits, id_bits, npass, hshift;  // hshift: bit of the KEY where the first counted digit starts
     u32 n_chunks, chunk;
+    u64 chunk_lo, chunk_hi;
     u32 prefix;  // variants are generated from the first `prefix` residues only (App. B); >= SD_L_MAX: whole sequences
     const u64* rec_off;
     u64* records;
@@ -396,7 +408,7 @@ __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
             u32 mine = 0, gcur = 0xffffffffu, gacc = 0;
             gen_walk(sh, f0, f1, ng, d, [&](u32 g, u32, int k, const int* p) {
                 bool ok = gen_canonical(sh, g, k, p);
-                if (CHUNKED && ok) ok = gen_chunk_of(gen_hash(sh, g, k, p), P.n_chunks) == P.chunk;
+                if (CHUNKED && ok) ok = gen_in_chunk(gen_hash(sh, g, k, p), sh.len[g] - (u32)k, P.chunk_lo, P.chunk_hi);
                 if (COUNT_ONLY) {
                     if (g != gcur) {
                         if (gacc) atomicAdd(&sh.cnt[gcur], gacc);
@@ -433,7 +445,7 @@ __global__ void __launch_bounds__(GEN_THREADS) k_generate(GenParams P) {
             gen_walk(sh, f0, f1, ng, d, [&](u32 g, u32, int k, const int* p) {
                 if (!gen_canonical(sh, g, k, p)) return;
                 const u64 h = gen_hash(sh, g, k, p);
-                if (CHUNKED && gen_chunk_of(h, P.n_chunks) != P.chunk) return;
+                if (CHUNKED && !gen_in_chunk(h, sh.len[g] - (u32)k, P.chunk_lo, P.chunk_hi)) return;
                 const u64 key = h >> kshift;
                 *out++ = (key << P.id_bits) | (gid0 + g);
                 for (int ps = 0; ps < P.npass; ++ps) atomicAdd(&s_hist[ps * 256 + ((u32)(key >> (P.hshift + 8 * ps)) & 255u)], 1u);
@@ -481,9 +493,9 @@ struct Gen2Shared {
 // One emission round of the fast path: lanes with `valid` append (hash, id) to their sequence's
 // record range (rank by ballot inside the sequence's lane segment) and count the key's digits.
 template <bool COUNT_ONLY, bool CHUNKED, int NPASS>
-__device__ __forceinline__ void g2_emit(bool valid, u64 h, const GenParams& P, u32 segmask, u32 lane_lt, u64 gid,
+__device__ __forceinline__ void g2_emit(bool valid, u64 h, u32 vlen, const GenParams& P, u32 segmask, u32 lane_lt, u64 gid,
                                         int kshift, u64*& out, u32& run, u32* s_hist) {
-    if (CHUNKED) valid = valid && gen_chunk_of(h, P.n_chunks) == P.chunk;
+    if (CHUNKED) valid = valid && gen_in_chunk(h, vlen, P.chunk_lo, P.chunk_hi);
     const u32 bal = __ballot_sync(SD_FULL, valid) & segmask;
     if (!COUNT_ONLY) {
         if (valid) {
@@ -553,7 +565,7 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
             // ---- empty sequences: one record (the empty variant) each ----
             if (mine && Li == 0) {
                 const u64 h = K_LEN;  // A[L] = 0, (L + 1) * K
-                const bool ok = !CHUNKED || gen_chunk_of(h, P.n_chunks) == P.chunk;
+                const bool ok = !CHUNKED || gen_in_chunk(h, 0, P.chunk_lo, P.chunk_hi);
                 if (COUNT_ONLY) {
                     P.cnt[gid0 + lane] = ok ? 1u : 0u;
                 } else if (ok) {
@@ -614,9 +626,9 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
                     const u64 C2 = binv2 * AL + (u64)(L - 1) * K_LEN;
                     u64* out = P.records + rec_base;
 
-                    g2_emit<COUNT_ONLY, CHUNKED, NPASS>(active && a == 0, C0, P, segmask, lane_lt, gid, kshift, out, run, s_hist);
+                    g2_emit<COUNT_ONLY, CHUNKED, NPASS>(active && a == 0, C0, L, P, segmask, lane_lt, gid, kshift, out, run, s_hist);
                     if (d >= 1)
-                        g2_emit<COUNT_ONLY, CHUNKED, NPASS>(canon1, Uv + C1, P, segmask, lane_lt, gid, kshift, out, run, s_hist);
+                        g2_emit<COUNT_ONLY, CHUNKED, NPASS>(canon1, Uv + C1, L - 1, P, segmask, lane_lt, gid, kshift, out, run, s_hist);
                     if (d >= 2) {
                         const u32 half = __reduce_max_sync(SD_FULL, L >> 1);
                         const u32 m1s = m1 >> seg_start, madjs = madj >> seg_start;  // segment-relative masks
@@ -630,7 +642,7 @@ __global__ void __launch_bounds__(G2_THREADS) k_gen2(GenParams P) {
                             const u32 both = (m1s >> p1) & (m1s >> p2);
                             const u32 t = (p2 - p1 == 1u) ? (madjs >> p1) : both;
                             const u64 h = Us[p1] + Vs[p2] + C2;
-                            g2_emit<COUNT_ONLY, CHUNKED, NPASS>(on && (t & 1u), h, P, segmask, lane_lt, gid, kshift, out, run,
+                            g2_emit<COUNT_ONLY, CHUNKED, NPASS>(on && (t & 1u), h, L - 2, P, segmask, lane_lt, gid, kshift, out, run,
                                                                 s_hist);
                         }
                     }
@@ -729,8 +741,9 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     u32 made = 0;  // D3: records this lane staged since the warp last reported
 
     // one record: its digit's counter (in bytes) hands out the slot; rank r of digit dg -> byte dg * 264 + 8 r of the stage
-    auto push1 = [&](u64 h, u64 gid) {
-        if (CHUNKED && gen_chunk_of(h, P.n_chunks) != P.chunk) return;
+    const u64 ch_lo = P.chunk_lo, ch_hi = P.chunk_hi;
+    auto push1 = [&](u64 h, u64 gid, u32 vlen) {
+        if (CHUNKED && !gen_in_chunk(h, vlen, ch_lo, ch_hi)) return;
         const u32 dg = (u32)(h >> 56);
         u64 rec;
         if (PLAIN) rec = ((u64)(u32)(h >> 32) << 32) | (((u32)h & ~idmask_lo) | (u32)gid);  // id_bits <= 31 here
@@ -752,8 +765,8 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
         }
         if (D3) ++made;
     };
-    auto push = [&](bool valid, u64 h, u64 gid) {
-        if (valid) push1(h, gid);
+    auto push = [&](bool valid, u64 h, u64 gid, u32 vlen) {
+        if (valid) push1(h, gid, vlen);
     };
 
     // warp task = 32 consecutive sequences of one set, cut into batches that fill the 32 lanes; the block
@@ -763,6 +776,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     i64 wt = (i64)warp * gridDim.x + blockIdx.x;
     const i64 wstride = (i64)gridDim.x * GP_NW;
     bool have = false;  // a task is loaded and has batches left
+    bool is_empty = false;  // lane as sequence index: a sequence of length 0 (its one record is the empty variant)
     u32 rnd = 0, staged = 0;  // D3: round index mod 3; records staged since the last flush (block-uniform)
     u32 s = 0, ns = 0, Li = 0, cum_incl = 0, cum_excl = 0;
     u64 gid0 = 0;
@@ -786,6 +800,13 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
             if (lane < ns) {
                 o0 = S.off[first + lane];
                 Li = min((u32)(S.off[first + lane + 1] - o0), P.prefix);
+            }
+            is_empty = lane < ns && Li == 0;
+            if (CHUNKED) {
+                // a sequence none of whose deletion depths reaches into this chunk takes no lanes at all
+                bool rel = false;
+                for (int k = 0; k <= d; ++k) rel = rel || (Li >= (u32)k && gen_len_in_chunk(Li - (u32)k, ch_lo, ch_hi));
+                if (!rel) Li = 0, is_empty = false;
             }
             cum_incl = Li;
 #pragma unroll
@@ -821,7 +842,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                 asm volatile("ld.shared.u64 %0, [%1];" : "=l"(u1) : "r"(u_sa + p1 * 8u));
                 asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v2) : "r"(v_sa + p2 * 8u));
                 asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v3) : "r"(v_sa + p3 * 8u));
-                push(g2 <= g2hi && ok && bad == 0, u1 + v2 + binv1 * v3 + t_C3, t_gid);
+                push(g2 <= g2hi && ok && bad == 0, u1 + v2 + binv1 * v3 + t_C3, t_gid, L - 3u);
                 if (g2 >= g2hi) {
                     ++step;
                     t_g2 = 1;
@@ -845,7 +866,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
             const u32 e = s + __popc(fit);
             const u32 total = __shfl_sync(SD_FULL, cum_incl, e - 1) - base;
             const bool mine = lane >= s && lane < e;  // lane as SEQUENCE index of this batch
-            if (mine && Li == 0) push(true, K_LEN, gid0 + lane);  // the empty variant of an empty sequence
+            if (mine && is_empty) push(true, K_LEN, gid0 + lane, 0u);  // the empty variant of an empty sequence
             if (total > 0) {
                 // ---- lane as POSITION: which sequence, which offset inside it ----
                 const u32 hbit = (mine && Li > 0) ? (1u << (cum_excl - base)) : 0u;
@@ -882,14 +903,17 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                     Ww[2 * seg_start + L + a] = Uv;
                 }
                 __syncwarp();
-                push(active && a == 0, AL + (u64)(L + 1) * K_LEN, gid);
-                if (d >= 1) push(canon1, Uv + binv1 * AL + (u64)L * K_LEN, gid);
+                // chunked: only the deletion depths whose variant length reaches into this chunk are enumerated
+                const bool in0 = !CHUNKED || gen_len_in_chunk(L, ch_lo, ch_hi), in1 = !CHUNKED || gen_len_in_chunk(L - 1u, ch_lo, ch_hi);
+                const bool in2 = !CHUNKED || (L >= 2u && gen_len_in_chunk(L - 2u, ch_lo, ch_hi));
+                push(active && a == 0 && in0, AL + (u64)(L + 1) * K_LEN, gid, L);
+                if (d >= 1) push(canon1 && in1, Uv + binv1 * AL + (u64)L * K_LEN, gid, L - 1u);
                 if (d >= 2) {
                     // pairs {a, (a + dl) mod L}: lane a runs dl = 1 .. dlmax (every unordered pair once); the
                     // partner b sits after a (no wrap: H = U[a] + V[b]) or before it (wrap: H = U[b] + V[a])
                     const u64 C2 = binv2 * AL + (u64)(L - 1) * K_LEN;
                     const u64 UC = Uv + C2, VC = binv1 * Uv + C2;
-                    const u32 half = __reduce_max_sync(SD_FULL, L >> 1);
+                    const u32 half = __reduce_max_sync(SD_FULL, in2 ? L >> 1 : 0u);
                     const u32 dlmax = active ? ((L - 1) >> 1) + (((L & 1u) == 0u && a < (L >> 1)) ? 1u : 0u) : 0u;
                     const u32 m1s = m1 >> seg_start;  // segment-relative mask
                     // vmask bit dl: the pair {a, (a + dl) mod L} makes a record.  dl >= 2: both members are canonical
@@ -901,6 +925,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                     const bool ok1 = wrap1 ? (L == 2u ? ((madj >> seg_start) & 1u) != 0u : (canon1 && (m1s & 1u))) : adjok;
                     u32 vmask = (canon1 ? rot : 0u) & ((2u << dlmax) - 1u) & ~3u;
                     if (ok1 && dlmax >= 1u) vmask |= 2u;
+                    if (!in2) vmask = 0u;
                     const u32 wth = L - a;  // dl >= wth: the partner wrapped
                     const u32 w_sa = (u32)__cvta_generic_to_shared(Ww + 2 * seg_start + a);
                     u64 UCr = UC, VCr = VC;
@@ -911,7 +936,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                         if ((int)vm < 0) {
                             u64 o;
                             asm volatile("ld.shared.u64 %0, [%1];" : "=l"(o) : "r"(w_sa + dl * 8u));
-                            push1(o + (dl >= wth ? VCr : UCr), gid);
+                            push1(o + (dl >= wth ? VCr : UCr), gid, L - 2u);
                         }
                     }
                 }
@@ -920,9 +945,10 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                     const bool ne2 = active && (!thinning || !has2 || c != cnn);
                     const bool ne3 = active && (!thinning || !(a + 3 < L) || c != cnnn);
                     const u32 b2 = __ballot_sync(SD_FULL, ne2), b3 = __ballot_sync(SD_FULL, ne3);
-                    t_Lmax = __reduce_max_sync(SD_FULL, L);
+                    const bool in3 = !CHUNKED || (L >= 3u && gen_len_in_chunk(L - 3u, ch_lo, ch_hi));
+                    t_Lmax = __reduce_max_sync(SD_FULL, in3 ? L : 0u);
                     t_g1max = t_Lmax >= 3 ? (t_Lmax - 1) >> 1 : 0;
-                    t_a = a, t_L = L, t_seg = seg_start, t_e = e, t_gid = gid;
+                    t_a = a, t_L = in3 ? L : 0u, t_seg = seg_start, t_e = e, t_gid = gid;
                     t_ne1 = m1 >> seg_start, t_ne2 = b2 >> seg_start, t_ne3 = b3 >> seg_start;
                     t_C3 = binv1 * binv2 * AL + (u64)(L - 2) * K_LEN;
                     if (t_g1max > 0) step = 1, t_g2 = 1;
@@ -1113,7 +1139,7 @@ __global__ void __launch_bounds__(GEN_THREADS, LW <= 32 ? GQ_MINB + 1 : GQ_MINB)
             gen_walk(sh, f0, f1, ng, d, [&](u32 g, u32, int k, const int* p) {
                 if (!gen_canonical(sh, g, k, p)) return;
                 const u64 h = gen_hash(sh, g, k, p);
-                if (CHUNKED && gen_chunk_of(h, P.n_chunks) != P.chunk) return;
+                if (CHUNKED && !gen_in_chunk(h, sh.len[g] - (u32)k, P.chunk_lo, P.chunk_hi)) return;
                 const u32 dg = (u32)(h >> 56);
                 const u64 rec = ((h >> kshift) << id_bits) | (gid0 + g);
                 u32 r;
@@ -1174,6 +1200,8 @@ GenParams make_params(SeqSetDev a, SeqSetDev b, const Layout& lay, int width) {
     P.id_bits = lay.id_bits;
     P.n_chunks = lay.n_chunks;
     P.chunk = lay.chunk;
+    P.chunk_lo = lay.chunk_lo;
+    P.chunk_hi = lay.chunk_hi;
     P.prefix = lay.prefix > 0 ? (u32)lay.prefix : (u32)SD_L_MAX;
     return P;
 }

@@ -7,8 +7,6 @@
 
 #include "common.cuh"
 
-#define SD_L_MAX 64
-#define SD_D_MAX 4
 
 // One CSR sequence set on the device.
 struct SeqSetDev {
@@ -32,6 +30,7 @@ struct Layout {
     int metric;         // 0: Levenshtein; 1: Hamming (equal lengths only, mismatch count)
     int force_general;  // test hook: never take the d <= 2 fast generation path
     u32 n_chunks, chunk;
+    u64 chunk_lo, chunk_hi;  // S5: this chunk holds the records with chunk_lo <= (variant length << 32 | hash fraction) < chunk_hi
 };
 
 // ---- radix_sort.cu ------------------------------------------------------------------------------

@@ -51,15 +51,9 @@ struct symdel_ctx {
 
 namespace {
 
-#ifdef SD_DEBUG_SYNC
-#define CK_DBG_SYNC(call) if (e__ == cudaSuccess) { e__ = cudaDeviceSynchronize(); if (e__ != cudaSuccess) fprintf(stderr, "[sd] %s -> %s\n", #call, cudaGetErrorString(e__)); }
-#else
-#define CK_DBG_SYNC(call)
-#endif
 #define CK(call)                                  \
     do {                                          \
         cudaError_t e__ = (call);                 \
-        CK_DBG_SYNC(call)                         \
         if (e__ != cudaSuccess) {                 \
             ctx->last_cuda = e__;                 \
             return SYMDEL_E_CUDA;                 \
@@ -222,6 +216,30 @@ int run_pipeline_body(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int 
     const i64 residues = (i64)ctx->h_info->residues;
     const int maxlen = (int)ctx->h_info->maxlen;
     const size_t ev_prepared = tm.mark();
+    // S5 layout: deletion sets per VARIANT length (upper bound: before thinning), cumulated.  Chunk c of P is the slice
+    // [c / P, (c + 1) / P) of that axis; inside a length the slice is cut by the hash fraction (generate.cu, gen_in_chunk).
+    double vl_cum[SD_L_MAX + 2];
+    vl_cum[0] = 0;
+    for (int vl = 0; vl <= SD_L_MAX; ++vl) {
+        double w = 0;
+        u64 binom = 1;  // C(vl + k, k)
+        for (int k = 0; k <= d && vl + k <= SD_L_MAX; ++k) {
+            if (k > 0) binom = binom * (u64)(vl + k) / (u64)k;
+            w += (double)ctx->h_info->len_hist[vl + k] * (double)binom;
+        }
+        vl_cum[vl + 1] = vl_cum[vl] + w;
+    }
+    auto chunk_pos = [&](u32 c, u32 of) -> u64 {  // where chunk c of `of` starts on the (variant length << 32 | hash fraction) axis
+        if (c == 0) return 0ull;
+        if (c >= of) return ~0ull;
+        const double target = vl_cum[SD_L_MAX + 1] * (double)c / (double)of;
+        int vl = 0;
+        while (vl < SD_L_MAX && vl_cum[vl + 1] <= target) ++vl;
+        const double w = vl_cum[vl + 1] - vl_cum[vl];
+        double frac = w > 0 ? (target - vl_cum[vl]) / w : 0;
+        frac = std::min<double>(std::max<double>(frac, 0), 0.99999999);
+        return ((u64)vl << 32) | (u64)(frac * 4294967296.0);
+    };
 
     Layout lay{};
     lay.n_a = A.n;
@@ -338,6 +356,8 @@ restart:
     CK(cudaMemsetAsync(&info->n_surv, 0, sizeof(u64) * 3, st));  // n_surv, n_out, n_unique
     for (u32 c = 0; c < P; ++c) {
         lay.chunk = c;
+        lay.chunk_lo = chunk_pos(c, P);
+        lay.chunk_hi = chunk_pos(c + 1, P);
         bool chunk_exact = false;  // a windowed fused search met a bucket whose pairs exceed a whole window: the chunk is redone by the exact pipeline
     redo_chunk:
         // ---- fused pipeline: generation + level-1 partition, level-2 partition, bucket join ----
