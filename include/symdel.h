@@ -143,7 +143,10 @@ SYMDEL_API int symdel_cross(symdel_ctx* ctx, const int8_t* q_seqs, const int64_t
                  void* cuda_stream);
 
 /* ---- the same calls with HOST buffers (inputs copied host->device and results device->host
- * inside the call; pinned host memory makes the copies asynchronous) ---------------------------- */
+ * inside the call; pinned host memory makes the copies asynchronous).  The offsets are sent first (input
+ * validation and sizing need nothing else), a large self-search sends the residues in slices and generates
+ * variants of a slice while the next is on its way.  The device arena is sized from an estimate of the record
+ * count; a low estimate only makes the search run in key-range chunks. ------------------------------------- */
 SYMDEL_API int symdel_self_host(symdel_ctx* ctx, const int8_t* seqs_host, const int64_t* offsets_host, int64_t n, int d,
                      int32_t* out_i_host, int32_t* out_j_host, int32_t* out_dist_host, int64_t capacity,
                      int64_t* n_pairs_host);

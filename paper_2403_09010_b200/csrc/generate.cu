@@ -707,6 +707,7 @@ struct GenPartParams {
     u32* cur;     // 256 bin cursors (zeroed by the host)
     u32 cap1;
     u32 batches;  // k_gen2_part: batches per warp and round
+    i64 task_begin, task_end;  // k_gen2_part: the warp tasks (groups of 32 sequences) of this launch — a slice when the input arrives in slices
 };
 
 // D3 (d == 3): the triples {p1 < p2 < p3} follow the pairs.  A triple is the three points a, a + g1, a + g1 + g2
@@ -773,7 +774,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     // advances `batches` batches per warp and round, then flushes
     // (the warps of a block take tasks far apart in the input: neighbouring sequences are often near-identical —
     // clonal lineages — and would all push the same digits at the same time)
-    i64 wt = (i64)warp * gridDim.x + blockIdx.x;
+    i64 wt = PP.task_begin + (i64)warp * gridDim.x + blockIdx.x;
     const i64 wstride = (i64)gridDim.x * GP_NW;
     bool have = false;  // a task is loaded and has batches left
     bool is_empty = false;  // lane as sequence index: a sequence of length 0 (its one record is the empty variant)
@@ -788,7 +789,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
     while (true) {
 #pragma unroll 1
         for (u32 rep = 0; rep < PP.batches; ++rep) {  // the same trip count in every warp: rounds stay balanced
-        if (!have && wt < P.groups_total) {
+        if (!have && wt < PP.task_end) {
             const bool in_b = wt >= P.groups_a;
             const SeqSetDev& S = in_b ? P.b : P.a;
             const i64 first = (in_b ? wt - P.groups_a : wt) * 32;
@@ -968,7 +969,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
         }
         // ---- round end: anyone left?  d <= 2: the host sized the round to fill the stage, flush.  D3: flush when the
         //      stage is about full (always at the end) ----
-        const bool more = have || wt < P.groups_total;
+        const bool more = have || wt < PP.task_end;
         const int any_more = __syncthreads_or(more);
         bool flush = true;
         if (D3) {
@@ -1349,8 +1350,11 @@ bool sd_gen_part_applies(const Layout& lay, int width) {
     return lay.hash_bits >= 8;
 }
 
+bool sd_gen_part_sliceable(const Layout& lay, int width) { return use_fast_part(lay, width); }
+
 cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1,
-                        double records_per_residue, double avg_len, DevInfo* info, cudaStream_t st, i64* launches) {
+                        double records_per_residue, double avg_len, i64 task_begin, i64 task_end, DevInfo* info, cudaStream_t st,
+                        i64* launches) {
     const bool fast = use_fast_part(lay, width);
     GenPartParams PP{};
     PP.g = fast ? make_params2(a, b, lay, width) : make_params(a, b, lay, width);
@@ -1365,10 +1369,16 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
         const double per_round = lay.d == 3 ? GP_NW * 32.0 * GP_TRIP * 0.55 : GP_NW * 32.0 * std::max(records_per_residue, 0.03) * 0.85;
         PP.batches = (u32)std::min(8.0, std::max(1.0, std::floor(GP_ROUND / per_round + 0.5)));
     }
+    // task range: [task_begin, task_end) of the warp tasks; (0, -1) = all.  Only the launch that starts at task 0 clears the cursors.
+    const bool sliced = task_end >= 0;
+    PP.task_begin = sliced ? task_begin : 0;
+    PP.task_end = sliced ? std::min(task_end, PP.g.groups_total) : PP.g.groups_total;
+    if (sliced && !fast) return cudaErrorInvalidValue;
+    if (PP.task_begin >= PP.task_end && PP.task_begin > 0) return cudaSuccess;
     cudaError_t e;
-    if ((e = cudaMemsetAsync(cur, 0, 256 * sizeof(u32), st)) != cudaSuccess) return e;
+    if (PP.task_begin == 0 && (e = cudaMemsetAsync(cur, 0, 256 * sizeof(u32), st)) != cudaSuccess) return e;
     if (fast) {
-        const int grid = (int)std::min<i64>((PP.g.groups_total + GP_NW - 1) / GP_NW, 148 * GP_MINB);
+        const int grid = (int)std::min<i64>((PP.task_end - PP.task_begin + GP_NW - 1) / GP_NW, 148 * GP_MINB);
         const bool plain = lay.hash_bits + lay.id_bits == 64 && lay.id_bits <= 31;
         GEN2_PART_KERNELS[(lay.d == 3 ? 4 : 0) + (lay.n_chunks > 1 ? 2 : 0) + (plain ? 1 : 0)]<<<grid, GP_THREADS, sizeof(GenPartShared), st>>>(PP);
     } else {

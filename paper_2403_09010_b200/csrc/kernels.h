@@ -77,8 +77,12 @@ cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
 // the bin counts afterwards).  info->part_overflow != 0: a bin was full, redo with the exact pipeline.
 bool sd_gen_part_applies(const Layout& lay, int width);
 // records_per_residue = (deletion sets of this chunk) / (residues): sizes the generation rounds
+// [task_begin, task_end): the warp tasks (groups of 32 consecutive sequences, A then B) of this launch; task_end < 0 = all.
+// Slices (sd_gen_part_sliceable only) append to the same bins: the launch starting at task 0 clears the cursors.
+bool sd_gen_part_sliceable(const Layout& lay, int width);
 cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1,
-                        double records_per_residue, double avg_len, DevInfo* info, cudaStream_t st, i64* launches);
+                        double records_per_residue, double avg_len, i64 task_begin, i64 task_end, DevInfo* info, cudaStream_t st,
+                        i64* launches);
 
 // ---- join.cu ------------------------------------------------------------------------------------
 i64 sd_join_tiles(i64 n_records);

@@ -47,6 +47,7 @@ struct symdel_ctx {
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     bool side_pending = false;      // work was forked to `side` and the caller's stream has not been made to wait for it yet
     std::vector<cudaEvent_t> events;
+    std::vector<cudaEvent_t> hp_events;  // host entry points: arrival of the input slices
 };
 
 namespace {
@@ -164,6 +165,16 @@ struct Timer {
     }
 };
 
+// The *_host entry points send the input in pieces on the side stream: all offsets first (S0 needs nothing else), then the
+// residues slice by slice, so that generation starts on the first slice while the others are being copied.
+constexpr int HP_MAX_SLICES = 8;
+struct HostPlan {
+    int n_slices = 0;                  // slices of set A's warp tasks (self-search; 1: no slicing)
+    i64 task_end[HP_MAX_SLICES] = {};  // slice i = tasks [task_end[i-1], task_end[i])
+    cudaEvent_t arrived[HP_MAX_SLICES] = {};
+    cudaEvent_t offsets_arrived = nullptr, all_arrived = nullptr;
+};
+
 int read_info(symdel_ctx* ctx, const DevInfo* d_info, cudaStream_t st) {
     CK(cudaMemcpyAsync(ctx->h_info, d_info, sizeof(DevInfo), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
@@ -181,7 +192,7 @@ int err_from_flags(u32 f) {
 
 // -------------------------------------------------------------------------------------------------
 int run_pipeline_body(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, void* workspace, i64 workspace_bytes,
-                 i32* out_i, i32* out_j, i32* out_dist, i64 capacity, i64* n_pairs_host, cudaStream_t st) {
+                 i32* out_i, i32* out_j, i32* out_dist, i64 capacity, i64* n_pairs_host, cudaStream_t st, const HostPlan* hp) {
     if (!ctx || !n_pairs_host || d < 0 || d > SD_D_MAX || A.n < 0 || B.n < 0 || capacity < 0) return SYMDEL_E_ARG;
     *n_pairs_host = 0;
     const i64 n_total = A.n + B.n;
@@ -207,6 +218,7 @@ int run_pipeline_body(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int 
     CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
     const int prefix = (int)ctx->opt_prefix;  // App. B: exact only if the prefix is longer than the threshold
     if (prefix > 0 && prefix <= d) return SYMDEL_E_ARG;
+    if (hp) CK(cudaStreamWaitEvent(st, hp->offsets_arrived, 0));  // (host entry points: S0 needs the offsets only)
     CK(sd_prepare(A, d, 0, prefix, info, st, &S.n_launches));
     if (cross) CK(sd_prepare(B, d, 1, prefix, info, st, &S.n_launches));
     int rc = read_info(ctx, info, st);
@@ -282,9 +294,16 @@ int run_pipeline_body(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int 
     //  side stream while the caller's stream generates; join_side() makes the caller's stream wait for it)
     CK(cudaEventRecord(ctx->ev_fork, st));
     CK(cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+    if (hp && hp->all_arrived) CK(cudaStreamWaitEvent(ctx->side, hp->all_arrived, 0));
     CK(sd_pack(A, B, maxlen, slots, info, ctx->side, &S.n_launches));
     CK(cudaEventRecord(ctx->ev_join, ctx->side));
     ctx->side_pending = true;
+    bool input_waited = !(hp && hp->all_arrived);
+    auto wait_input = [&]() -> cudaError_t {  // the caller's stream after the last input slice (host entry points)
+        if (input_waited) return cudaSuccess;
+        input_waited = true;
+        return cudaStreamWaitEvent(st, hp->all_arrived, 0);
+    };
     auto join_side = [&]() -> cudaError_t {
         if (!ctx->side_pending) return cudaSuccess;
         ctx->side_pending = false;
@@ -373,8 +392,20 @@ restart:
             const size_t x0 = tm.mark();
             lay.sort_bits = fp.b;
             CK(cudaMemsetAsync(&info->part_overflow, 0, sizeof(u32), st));
-            CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, (double)nmax / (double)std::max<i64>(residues, 1) / (double)P,
-                           (double)residues / (double)n_total, info, st, &S.n_launches));
+            const double rpr = (double)nmax / (double)std::max<i64>(residues, 1) / (double)P, avg_len = (double)residues / (double)n_total;
+            if (hp && hp->n_slices > 1 && !input_waited && sd_gen_part_sliceable(lay, width)) {
+                // generation follows the input slice by slice: slice i is generated while slice i + 1 is being copied
+                i64 t0 = 0;
+                for (int i = 0; i < hp->n_slices; ++i) {
+                    CK(cudaStreamWaitEvent(st, hp->arrived[i], 0));
+                    CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, rpr, avg_len, t0, hp->task_end[i], info, st, &S.n_launches));
+                    t0 = hp->task_end[i];
+                }
+                input_waited = true;
+            } else {
+                CK(wait_input());
+                CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, rpr, avg_len, 0, -1, info, st, &S.n_launches));
+            }
             const size_t x1 = tm.mark();
             if (fp.b2)
                 CK(sd_part2(recA, cur1, fp.cap1, recB, cnt2, fp.cap2, fp.b2, lay.id_bits + lay.hash_bits - fp.b, info, st,
@@ -413,6 +444,7 @@ restart:
         u64* sorted = nullptr;
         if (!fused_ok) {
         const size_t e0 = tm.mark();
+        CK(wait_input());
         // ---- S1: count, scan, generate ----
         CK(sd_count(A, B, lay, width, cnt, info, st, &S.n_launches));
         CK(sd_scan_counts(cnt, n_total, rec_off, scan_lb, info, st, &S.n_launches));
@@ -640,8 +672,8 @@ restart:
 // Every way out of the pipeline leaves the caller's stream ordered after the side stream's work (which reads and
 // writes the caller's workspace): a caller may release the workspace in stream order right after the call.
 int run_pipeline(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int d, void* workspace, i64 workspace_bytes, i32* out_i,
-                 i32* out_j, i32* out_dist, i64 capacity, i64* n_pairs_host, cudaStream_t st) {
-    const int rc = run_pipeline_body(ctx, A, B, cross, d, workspace, workspace_bytes, out_i, out_j, out_dist, capacity, n_pairs_host, st);
+                 i32* out_j, i32* out_dist, i64 capacity, i64* n_pairs_host, cudaStream_t st, const HostPlan* hp = nullptr) {
+    const int rc = run_pipeline_body(ctx, A, B, cross, d, workspace, workspace_bytes, out_i, out_j, out_dist, capacity, n_pairs_host, st, hp);
     if (ctx && ctx->side_pending) {
         ctx->side_pending = false;
         if (cudaStreamWaitEvent(st, ctx->ev_join, 0) != cudaSuccess) cudaStreamSynchronize(ctx->side);
@@ -672,47 +704,58 @@ int run_host(symdel_ctx* ctx, const int8_t* a_seqs, const i64* a_off, i64 n_a, c
     CK(cudaSetDevice(ctx->device));
     const i64 res_a = a_off[n_a], res_b = cross ? b_off[n_b] : 0;
     if (res_a < 0 || res_b < 0) return SYMDEL_E_OFFSETS;
-    // ---- inputs first: the copies run while the host sizes the workspace ----
+    // ---- inputs first: the copies run (on the side stream) while the host does S0 on its own copy of the offsets and sizes
+    //      the workspace; a large self-search is sent in slices so that generation can start when the first has arrived ----
     const i64 in_bytes = align_up(res_a + 16) + align_up((n_a + 1) * 8) + align_up(res_b + 16) + align_up((n_b + 1) * 8);
     int rc = ensure_arena(ctx, &ctx->in_arena, &ctx->in_arena_bytes, (size_t)(in_bytes + 4096));
     if (rc) return rc;
-    cudaStream_t st = ctx->stream;
+    cudaStream_t st = ctx->stream, cs = ctx->side;
     Bump in(ctx->in_arena, (i64)ctx->in_arena_bytes);
     int8_t* d_as = in.take<int8_t>(res_a + 16);
     i64* d_ao = in.take<i64>(n_a + 1);
     int8_t* d_bs = in.take<int8_t>(res_b + 16);
     i64* d_bo = in.take<i64>(n_b + 1);
     if (!in.ok) return SYMDEL_E_INTERNAL;
-    CK(cudaMemcpyAsync(d_ao, a_off, (size_t)(n_a + 1) * 8, cudaMemcpyHostToDevice, st));
-    if (res_a) CK(cudaMemcpyAsync(d_as, a_seqs, (size_t)res_a, cudaMemcpyHostToDevice, st));
-    if (cross) {
-        CK(cudaMemcpyAsync(d_bo, b_off, (size_t)(n_b + 1) * 8, cudaMemcpyHostToDevice, st));
-        if (res_b) CK(cudaMemcpyAsync(d_bs, b_seqs, (size_t)res_b, cudaMemcpyHostToDevice, st));
+    while (ctx->hp_events.size() < (size_t)HP_MAX_SLICES + 1) {
+        cudaEvent_t e;
+        CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        ctx->hp_events.push_back(e);
     }
-    // exact record bound from the host offsets (a malformed input leaves through an error below; the copies
-    // already queued only touch the context's own arena)
-    i64 nmax = 0;
-    int maxlen = 0;
-    bool bad_off = false, too_long = false;
-    for (int s = 0; s < (cross ? 2 : 1); ++s) {
-        const i64* off = s ? b_off : a_off;
-        const i64 n = s ? n_b : n_a;
-        u64 vtab[SD_L_MAX + 1];
-        for (int L = 0; L <= SD_L_MAX; ++L) vtab[L] = vcount_host(L, d);
-        for (i64 i = 0; i < n; ++i) {
-            const i64 L = off[i + 1] - off[i];
-            if (L < 0) bad_off = true;
-            else if (L > SD_L_MAX) too_long = true;
-            else {
-                nmax += (i64)vtab[L];
-                maxlen = std::max(maxlen, (int)L);
-            }
+    HostPlan hp;
+    // (the offsets are validated on the device, by k_prepare; here they only place the slice boundaries, clamped: the
+    //  copies never leave the context's own arena)
+    auto clampi = [](i64 x, i64 lo, i64 hi) { return x < lo ? lo : (x > hi ? hi : x); };
+    CK(cudaMemcpyAsync(d_ao, a_off, (size_t)(n_a + 1) * 8, cudaMemcpyHostToDevice, cs));
+    if (cross) CK(cudaMemcpyAsync(d_bo, b_off, (size_t)(n_b + 1) * 8, cudaMemcpyHostToDevice, cs));
+    hp.offsets_arrived = ctx->hp_events[HP_MAX_SLICES - 1];
+    CK(cudaEventRecord(hp.offsets_arrived, cs));
+    const i64 tasks_a = (n_a + 31) / 32;
+    hp.n_slices = (!cross && n_a >= 65536) ? 4 : 1;
+    {
+        i64 s0 = 0;
+        for (int i = 0; i < hp.n_slices; ++i) {
+            hp.task_end[i] = tasks_a * (i + 1) / hp.n_slices;
+            const i64 s1 = std::min<i64>(n_a, hp.task_end[i] * 32);
+            const i64 r0 = clampi(a_off[s0], 0, res_a), r1 = clampi(a_off[s1], r0, res_a);
+            if (r1 > r0) CK(cudaMemcpyAsync(d_as + r0, a_seqs + r0, (size_t)(r1 - r0), cudaMemcpyHostToDevice, cs));
+            hp.arrived[i] = ctx->hp_events[i];
+            CK(cudaEventRecord(hp.arrived[i], cs));
+            s0 = s1;
         }
     }
-    if (bad_off || too_long) {
-        cudaStreamSynchronize(st);
-        return bad_off ? SYMDEL_E_OFFSETS : SYMDEL_E_TOO_LONG;
-    }
+    if (cross && res_b) CK(cudaMemcpyAsync(d_bs, b_seqs, (size_t)res_b, cudaMemcpyHostToDevice, cs));
+    hp.all_arrived = ctx->hp_events[HP_MAX_SLICES];
+    CK(cudaEventRecord(hp.all_arrived, cs));
+    // Workspace: sized from an ESTIMATE of the record count (every sequence as long as the mean, rounded up, plus one) — no
+    // pass over a million host offsets on the critical path.  If the estimate is low the planner cuts the search into key-range
+    // chunks: slower, never wrong.  The exact count is S0's, on the device.
+    const i64 pfx = ctx->opt_prefix > 0 ? ctx->opt_prefix : SD_L_MAX;
+    auto est = [&](i64 n, i64 res) -> i64 {
+        if (n <= 0) return 0;
+        const i64 Lm = std::min<i64>(std::min<i64>((res + n - 1) / n + 1, pfx), SD_L_MAX);
+        return n * (i64)vcount_host((int)Lm, d);
+    };
+    const i64 nmax = est(n_a, res_a) + est(n_b, res_b);
     const i64 n_total = n_a + n_b;
     const int npass_max = 7, ppass_max = 8;
     const i64 ccap = std::max<i64>(1 << 20, std::min<i64>(2 * nmax, nmax / 2 + ((i64)128 << 20))), scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity);
@@ -728,8 +771,11 @@ int run_host(symdel_ctx* ctx, const int8_t* a_seqs, const i64* a_off, i64 n_a, c
     void* d_ws = ar.take<char>(ws_bytes);
     if (!ar.ok) return SYMDEL_E_INTERNAL;
     SeqSetDev A{d_as, d_ao, n_a}, B{d_bs, d_bo, cross ? n_b : 0};
-    rc = run_pipeline(ctx, A, B, cross, d, d_ws, ws_bytes, d_i, d_j, d_d, capacity, n_pairs_host, st);
-    if (rc != SYMDEL_OK && rc != SYMDEL_E_CAPACITY) return rc;
+    rc = run_pipeline(ctx, A, B, cross, d, d_ws, ws_bytes, d_i, d_j, d_d, capacity, n_pairs_host, st, &hp);
+    if (rc != SYMDEL_OK && rc != SYMDEL_E_CAPACITY) {
+        cudaStreamSynchronize(cs);  // (an early way out may not have waited for the copies: the caller's buffers are free on return)
+        return rc;
+    }
     const i64 ncopy = std::min<i64>(*n_pairs_host, capacity);
     if (ncopy > 0) {
         CK(cudaMemcpyAsync(out_i, d_i, (size_t)ncopy * 4, cudaMemcpyDeviceToHost, st));
@@ -786,6 +832,7 @@ void symdel_destroy(symdel_ctx* ctx) {
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
     for (auto e : ctx->events) cudaEventDestroy(e);
+    for (auto e : ctx->hp_events) cudaEventDestroy(e);
     delete ctx;
 }
 
