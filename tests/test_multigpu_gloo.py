@@ -50,3 +50,26 @@ def test_single_process_passthrough():
     import bench
 
     assert bench.max_over_ranks([1.5, 2.5], None, torch.device("cpu")) == [1.5, 2.5]
+
+
+def test_bench_digest_is_the_golden_format():
+    """bench.py hashes what it times and compares with tests/golden/*.json: its digest must be the one
+    tests/golden/make_golden.py writes (sha256 of the int32 arrays i, j, dist, concatenated)."""
+    import hashlib
+    import importlib.util
+
+    import numpy as np
+
+    sys.path.insert(0, str(ROOT))
+    import bench
+
+    spec = importlib.util.spec_from_file_location("make_golden", ROOT / "tests" / "golden" / "make_golden.py")
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    rng = np.random.default_rng(0)
+    i, j, d = (rng.integers(0, 1000, 257).astype(np.int64) for _ in range(3))
+    want = hashlib.sha256(b"".join(np.asarray(a, dtype=np.int32).tobytes() for a in (i, j, d))).hexdigest()
+    assert bench.digest(i, j, d) == mg.digest(i, j, d) == want
+    for name in ("config_1.json", "config_2.json", "config_3.json", "config_4.json", "config_5.json", "dense_1m.json"):
+        g = bench.golden(name)
+        assert g and len(g["out_sha256"]) == 64 and g["n_out"] > 0, name
