@@ -755,23 +755,49 @@ int run_host(symdel_ctx* ctx, const int8_t* a_seqs, const i64* a_off, i64 n_a, c
         const i64 Lm = std::min<i64>(std::min<i64>((res + n - 1) / n + 1, pfx), SD_L_MAX);
         return n * (i64)vcount_host((int)Lm, d);
     };
-    const i64 nmax = est(n_a, res_a) + est(n_b, res_b);
+    i64 nmax = est(n_a, res_a) + est(n_b, res_b);
     const i64 n_total = n_a + n_b;
     const int npass_max = 7, ppass_max = 8;
-    const i64 ccap = std::max<i64>(1 << 20, std::min<i64>(2 * nmax, nmax / 2 + ((i64)128 << 20))), scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity);
-    const i64 ws_bytes = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nmax, 1), npass_max) + cand_bytes(ccap + n_total + 64, ppass_max) +
-                         cand_bytes(scap, ppass_max) + 65536;
     const i64 out_bytes = 3 * align_up(capacity * 4 + 16);
-    rc = ensure_arena(ctx, &ctx->arena, &ctx->arena_bytes, (size_t)(out_bytes + ws_bytes + 4096));
-    if (rc) return rc;
-    Bump ar(ctx->arena, (i64)ctx->arena_bytes);
-    i32* d_i = ar.take<i32>(capacity + 4);
-    i32* d_j = ar.take<i32>(capacity + 4);
-    i32* d_d = ar.take<i32>(capacity + 4);
-    void* d_ws = ar.take<char>(ws_bytes);
-    if (!ar.ok) return SYMDEL_E_INTERNAL;
-    SeqSetDev A{d_as, d_ao, n_a}, B{d_bs, d_bo, cross ? n_b : 0};
-    rc = run_pipeline(ctx, A, B, cross, d, d_ws, ws_bytes, d_i, d_j, d_d, capacity, n_pairs_host, st, &hp);
+    i32 *d_i = nullptr, *d_j = nullptr, *d_d = nullptr;
+    for (int attempt = 0;; ++attempt) {
+        const i64 ccap = std::max<i64>(1 << 20, std::min<i64>(2 * nmax, nmax / 2 + ((i64)128 << 20))), scap = std::max<i64>(std::max<i64>(1 << 20, nmax / 4), capacity);
+        const i64 ws_bytes = fixed_bytes(n_total) + rec_bytes(std::max<i64>(nmax, 1), npass_max) + cand_bytes(ccap + n_total + 64, ppass_max) +
+                             cand_bytes(scap, ppass_max) + 65536;
+        rc = ensure_arena(ctx, &ctx->arena, &ctx->arena_bytes, (size_t)(out_bytes + ws_bytes + 4096));
+        if (rc) break;
+        Bump ar(ctx->arena, (i64)ctx->arena_bytes);
+        d_i = ar.take<i32>(capacity + 4);
+        d_j = ar.take<i32>(capacity + 4);
+        d_d = ar.take<i32>(capacity + 4);
+        // (an arena left larger by an earlier call is used whole: more room never hurts the plan)
+        const i64 ws_have = std::max<i64>(ws_bytes, (ar.left() - 4096) / 256 * 256);
+        void* d_ws = ar.take<char>(ws_have);
+        if (!ar.ok) {
+            rc = SYMDEL_E_INTERNAL;
+            break;
+        }
+        SeqSetDev A{d_as, d_ao, n_a}, B{d_bs, d_bo, cross ? n_b : 0};
+        rc = run_pipeline(ctx, A, B, cross, d, d_ws, ws_have, d_i, d_j, d_d, capacity, n_pairs_host, st, &hp);
+        if (rc != SYMDEL_E_WORKSPACE || attempt > 0) break;
+        // The estimate was too low even for a chunked search (lengths far from their mean, or an output capacity that
+        // leaves no room): size the arena from the exact count — one pass over the host offsets, this once — and repeat.
+        i64 exact = 0;
+        bool bad = false;
+        for (int sset = 0; sset < (cross ? 2 : 1); ++sset) {
+            const i64* off = sset ? b_off : a_off;
+            const i64 n = sset ? n_b : n_a;
+            u64 vtab[SD_L_MAX + 1];
+            for (int L = 0; L <= SD_L_MAX; ++L) vtab[L] = vcount_host((int)std::min<i64>(L, pfx), d);
+            for (i64 i = 0; i < n; ++i) {
+                const i64 L = off[i + 1] - off[i];
+                if (L < 0 || L > SD_L_MAX) bad = true;
+                else exact += (i64)vtab[L];
+            }
+        }
+        if (bad || exact <= nmax) break;  // (malformed offsets are reported by the device pass; nothing to gain otherwise)
+        nmax = exact;
+    }
     if (rc != SYMDEL_OK && rc != SYMDEL_E_CAPACITY) {
         cudaStreamSynchronize(cs);  // (an early way out may not have waited for the copies: the caller's buffers are free on return)
         return rc;

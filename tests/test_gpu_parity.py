@@ -571,6 +571,67 @@ def test_host_entry_points(torch, sd, ctx, oracle):
     assert_same([o[:k] for o in out2], oracle.symdel_cross(q.seqs, q.offsets, r.seqs, r.offsets, 2))
 
 
+@pytest.mark.parametrize("num,pinned", [(2, True), (2, False), (3, True), (5, True)])
+def test_host_entry_points_sliced_input(torch, sd, num, pinned):
+    """symdel_self_host on a large set: the offsets go first, the residues follow in slices and generation of a slice
+    overlaps the copy of the next (include/symdel.h, host entry points).  Same golden digest as the device entry point,
+    from pinned and from pageable host memory, three calls in a row on one context (the arena and the events are reused)."""
+    g = _golden(f"config_{num}.json")
+    kind, d, (s,) = synth.config(num)
+    assert s.n >= 65536  # the sliced path
+    c = sd.Context(0)
+    cap = 1 << 20
+    mk = (lambda a: torch.from_numpy(a).pin_memory()) if pinned else (lambda a: a)
+    hs, ho = mk(s.seqs), mk(s.offsets)
+    out = tuple((torch.empty(cap, dtype=torch.int32).pin_memory() if pinned else np.empty(cap, np.int32)) for _ in range(3))
+    for rep in range(3):
+        k = c.symdel_self_host(hs, ho, d, out)
+        i, j, dist = [(o[:k].numpy() if pinned else o[:k]) for o in out]
+        assert_matches_golden(g, i, j, dist)
+    st = c.symdel_get_stats()
+    assert st["n_chunks"] == 1 and st["fused_chunks"] == 1
+
+
+def test_host_entry_points_low_arena_estimate_only_chunks(torch, sd, oracle):
+    """The host entry points size their arena from the MEAN length; a set whose few long sequences carry most of the
+    deletion sets makes that estimate low — the search then runs in key-range chunks, the result is the same."""
+    rng = np.random.default_rng(5)
+    n = 70000
+    lens = np.where(rng.random(n) < 0.03, 60, 6).astype(np.int64)  # 3 % long sequences hold ~70 % of the records at d = 2
+    rows = rng.integers(1, 21, size=(n, 60)).astype(np.int8)
+    rows[n // 2:] = rows[: n - n // 2]  # second half = first half with one substitution: plenty of pairs
+    rows[n // 2:, 2] = rng.integers(1, 21, size=n - n // 2)
+    lens[n // 2:] = lens[: n - n // 2]
+    s = synth.from_padded(rows, lens)
+    exp = oracle.symdel_self(s.seqs, s.offsets, 2)
+    c = sd.Context(0)
+    out = tuple(np.empty(len(exp[0]) + 64, np.int32) for _ in range(3))
+    k = c.symdel_self_host(s.seqs, s.offsets, 2, out)
+    assert_same([o[:k] for o in out], exp)
+    assert c.symdel_get_stats()["n_chunks"] >= 2
+
+
+def test_host_entry_points_reject_malformed_offsets(torch, sd):
+    """Offsets are validated on the device (k_prepare) after the copy; the slice boundaries the host reads from them
+    are clamped to the arena, whatever they say."""
+    kind, d, (s,) = synth.config(2)
+    c = sd.Context(0)
+    out = tuple(np.empty(1 << 18, np.int32) for _ in range(3))
+    for where, val, code in ((s.n // 2, -5, sd.E_OFFSETS), (s.n // 3, int(s.offsets[-1]) + 10 ** 9, sd.E_OFFSETS), (100, None, sd.E_TOO_LONG)):
+        off = s.offsets.copy()
+        if val is None:
+            off[where + 1:] += 70  # one sequence of length > 64
+            seqs = np.concatenate([s.seqs, np.ones(70, np.int8)])
+        else:
+            off[where] = val
+            seqs = s.seqs
+        with pytest.raises(sd.SymdelError) as e:
+            c.symdel_self_host(seqs, off, d, out)
+        assert e.value.code == code, (where, val)
+    k = c.symdel_self_host(s.seqs, s.offsets, d, out)  # the context is still good
+    assert k == _golden("config_2.json")["n_out"]
+
+
 # ---- BASELINE.json configs at full size ---------------------------------------------------------------
 def _golden(name):
     p = GOLD / name
