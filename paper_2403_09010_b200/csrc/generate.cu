@@ -1353,8 +1353,8 @@ bool sd_gen_part_applies(const Layout& lay, int width) {
 bool sd_gen_part_sliceable(const Layout& lay, int width) { return use_fast_part(lay, width); }
 
 cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1,
-                        double records_per_residue, double avg_len, i64 task_begin, i64 task_end, DevInfo* info, cudaStream_t st,
-                        i64* launches) {
+                        double records_per_residue, double avg_len, i64 task_begin, i64 task_end, int cursors_cleared, DevInfo* info,
+                        cudaStream_t st, i64* launches) {
     const bool fast = use_fast_part(lay, width);
     GenPartParams PP{};
     PP.g = fast ? make_params2(a, b, lay, width) : make_params(a, b, lay, width);
@@ -1376,7 +1376,7 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     if (sliced && !fast) return cudaErrorInvalidValue;
     if (PP.task_begin >= PP.task_end && PP.task_begin > 0) return cudaSuccess;
     cudaError_t e;
-    if (PP.task_begin == 0 && (e = cudaMemsetAsync(cur, 0, 256 * sizeof(u32), st)) != cudaSuccess) return e;
+    if (PP.task_begin == 0 && !cursors_cleared && (e = cudaMemsetAsync(cur, 0, 256 * sizeof(u32), st)) != cudaSuccess) return e;
     if (fast) {
         const int grid = (int)std::min<i64>((PP.task_end - PP.task_begin + GP_NW - 1) / GP_NW, 148 * GP_MINB);
         const bool plain = lay.hash_bits + lay.id_bits == 64 && lay.id_bits <= 31;

@@ -906,11 +906,12 @@ int sd_join_bkt_max_cap() { return JB_STAGE_L; }
 int sd_join_bkt_link_bits(u32 cap) { return cap <= (u32)JB_STAGE_S ? JB_NB_S : JB_NB_L; }
 
 cudaError_t sd_join_bkt(const u64* buckets, u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
-                        int first_pass, DevInfo* info, cudaStream_t st, i64* launches) {
-    cudaError_t e;
-    if ((e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
+                        int first_pass, int info_fresh, DevInfo* info, cudaStream_t st, i64* launches) {
+    cudaError_t e = cudaSuccess;
+    // (info_fresh: the whole status block was cleared for this call and nothing has counted pairs or raised a join flag yet)
+    if (!info_fresh && (e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
     static_assert(offsetof(DevInfo, nofit_inv) == offsetof(DevInfo, join_fallback) + 8, "cleared together");
-    if ((e = cudaMemsetAsync(&info->join_fallback, 0, 2 * sizeof(u32) + sizeof(u64), st)) != cudaSuccess) return e;  // and join_redo, nofit_inv
+    if (!info_fresh && (e = cudaMemsetAsync(&info->join_fallback, 0, 2 * sizeof(u32) + sizeof(u64), st)) != cudaSuccess) return e;  // and join_redo, nofit_inv
     if (nbuckets == 0) return cudaSuccess;
     JoinBktParams BP{};
     BP.j = jn_params(buckets, 0, lay, cand, window, info);

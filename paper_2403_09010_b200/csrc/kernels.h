@@ -53,7 +53,7 @@ cudaError_t sd_cand_filter(const u64* cand, i64 n, void* table, int table_bits, 
 
 // level-2 partition of the fused pipeline: bins (256 x cap1) -> buckets ((256 << b2) x cap2)
 cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u32* cnt2, i64 cap2, int b2, int shift,
-                     DevInfo* info, cudaStream_t st, i64* launches);
+                     int counts_cleared, DevInfo* info, cudaStream_t st, i64* launches);
 
 // ---- generate.cu --------------------------------------------------------------------------------
 cudaError_t sd_generate_setup();  // per-device setup: the __constant__ tables and function attributes; symdel_create
@@ -78,11 +78,12 @@ cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
 bool sd_gen_part_applies(const Layout& lay, int width);
 // records_per_residue = (deletion sets of this chunk) / (residues): sizes the generation rounds
 // [task_begin, task_end): the warp tasks (groups of 32 consecutive sequences, A then B) of this launch; task_end < 0 = all.
-// Slices (sd_gen_part_sliceable only) append to the same bins: the launch starting at task 0 clears the cursors.
+// Slices (sd_gen_part_sliceable only) append to the same bins: the launch starting at task 0 clears the cursors (unless the
+// caller has: cursors_cleared).
 bool sd_gen_part_sliceable(const Layout& lay, int width);
 cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1,
-                        double records_per_residue, double avg_len, i64 task_begin, i64 task_end, DevInfo* info, cudaStream_t st,
-                        i64* launches);
+                        double records_per_residue, double avg_len, i64 task_begin, i64 task_end, int cursors_cleared, DevInfo* info,
+                        cudaStream_t st, i64* launches);
 
 // ---- join.cu ------------------------------------------------------------------------------------
 i64 sd_join_tiles(i64 n_records);
@@ -111,7 +112,7 @@ cudaError_t sd_join_fast_redo(const u64* records, i64 n_records, const Layout& l
 int sd_join_bkt_max_cap();
 int sd_join_bkt_link_bits(u32 cap);  // bits on top of a record that must be constant within a bucket
 cudaError_t sd_join_bkt(const u64* buckets, u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
-                        int first_pass, DevInfo* info, cudaStream_t st, i64* launches);
+                        int first_pass, int info_fresh, DevInfo* info, cudaStream_t st, i64* launches);
 
 // ---- verify.cu ----------------------------------------------------------------------------------
 i64 sd_verify_tiles(i64 n);

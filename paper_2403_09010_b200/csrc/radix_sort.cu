@@ -537,10 +537,10 @@ cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, const u64* n_dev, int beg
 // counts cnt2, zeroed here).  shift = bit of the record where the b2-bit digit starts.  b2 == 0: no-op
 // for the caller (the bins are the buckets).
 cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u32* cnt2, i64 cap2, int b2, int shift,
-                     DevInfo* info, cudaStream_t st, i64* launches) {
+                     int counts_cleared, DevInfo* info, cudaStream_t st, i64* launches) {
     cudaError_t e;
     constexpr size_t smem = (size_t)P2_TILE * 8;
-    if ((e = cudaMemsetAsync(cnt2, 0, ((size_t)256 << b2) * sizeof(u32), st)) != cudaSuccess) return e;
+    if (!counts_cleared && (e = cudaMemsetAsync(cnt2, 0, ((size_t)256 << b2) * sizeof(u32), st)) != cudaSuccess) return e;
     Part2Params P{};
     P.bins = bins;
     P.cnt1 = cnt1;

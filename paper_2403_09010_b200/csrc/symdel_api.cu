@@ -216,6 +216,7 @@ int run_pipeline_body(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int 
 
     // ---- S0 ----
     CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
+    bool info_fresh = true;  // until something other than S0 has written to the status block: the first fused attempt skips its clears
     const int prefix = (int)ctx->opt_prefix;  // App. B: exact only if the prefix is longer than the threshold
     if (prefix > 0 && prefix <= d) return SYMDEL_E_ARG;
     if (hp) CK(cudaStreamWaitEvent(st, hp->offsets_arrived, 0));  // (host entry points: S0 needs the offsets only)
@@ -372,7 +373,7 @@ restart:
     direct = false;
     S.n_records = S.n_candidates = 0;
     lay.n_chunks = P;
-    CK(cudaMemsetAsync(&info->n_surv, 0, sizeof(u64) * 3, st));  // n_surv, n_out, n_unique
+    if (!info_fresh) CK(cudaMemsetAsync(&info->n_surv, 0, sizeof(u64) * 3, st));  // n_surv, n_out, n_unique
     for (u32 c = 0; c < P; ++c) {
         lay.chunk = c;
         lay.chunk_lo = chunk_pos(c, P);
@@ -391,31 +392,35 @@ restart:
             sd_gen_part_applies(lay, width)) {
             const size_t x0 = tm.mark();
             lay.sort_bits = fp.b;
-            CK(cudaMemsetAsync(&info->part_overflow, 0, sizeof(u32), st));
+            if (!info_fresh) CK(cudaMemsetAsync(&info->part_overflow, 0, sizeof(u32), st));
+            const int fresh = info_fresh ? 1 : 0;
+            info_fresh = false;
+            // level-1 cursors and level-2 counts are neighbours: one clear for both, ahead of generation
+            CK(cudaMemsetAsync(fcnt, 0, (size_t)(256 + (fp.b2 ? fp.nbuckets : 0)) * sizeof(u32), st));
             const double rpr = (double)nmax / (double)std::max<i64>(residues, 1) / (double)P, avg_len = (double)residues / (double)n_total;
             if (hp && hp->n_slices > 1 && !input_waited && sd_gen_part_sliceable(lay, width)) {
                 // generation follows the input slice by slice: slice i is generated while slice i + 1 is being copied
                 i64 t0 = 0;
                 for (int i = 0; i < hp->n_slices; ++i) {
                     CK(cudaStreamWaitEvent(st, hp->arrived[i], 0));
-                    CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, rpr, avg_len, t0, hp->task_end[i], info, st, &S.n_launches));
+                    CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, rpr, avg_len, t0, hp->task_end[i], 1, info, st, &S.n_launches));
                     t0 = hp->task_end[i];
                 }
                 input_waited = true;
             } else {
                 CK(wait_input());
-                CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, rpr, avg_len, 0, -1, info, st, &S.n_launches));
+                CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, rpr, avg_len, 0, -1, 1, info, st, &S.n_launches));
             }
             const size_t x1 = tm.mark();
             if (fp.b2)
-                CK(sd_part2(recA, cur1, fp.cap1, recB, cnt2, fp.cap2, fp.b2, lay.id_bits + lay.hash_bits - fp.b, info, st,
+                CK(sd_part2(recA, cur1, fp.cap1, recB, cnt2, fp.cap2, fp.b2, lay.id_bits + lay.hash_bits - fp.b, 1, info, st,
                             &S.n_launches));
             const size_t x2 = tm.mark();
             f_bkt = fp.b2 ? recB : recA;
             f_bcnt = fp.b2 ? cnt2 : cur1;
             f_bcap = (u32)(fp.b2 ? fp.cap2 : fp.cap1), f_nb = (u32)fp.nbuckets;
             u32* h_cur = reinterpret_cast<u32*>(ctx->h_info + 1);
-            CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 1, info, st, &S.n_launches));
+            CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 1, fresh, info, st, &S.n_launches));
             CK(join_side());
             CK(cudaMemcpyAsync(h_cur, cur1, 256 * sizeof(u32), cudaMemcpyDeviceToHost, st));  // (bit 31 of a count is the join's "open" mark)
             rc = read_info(ctx, info, st);
@@ -444,6 +449,7 @@ restart:
         u64* sorted = nullptr;
         if (!fused_ok) {
         const size_t e0 = tm.mark();
+        info_fresh = false;
         CK(wait_input());
         // ---- S1: count, scan, generate ----
         CK(sd_count(A, B, lay, width, cnt, info, st, &S.n_launches));
@@ -510,7 +516,7 @@ restart:
             const size_t f0 = tm.mark();
             if (fused_ok && w0 > 0) {
                 // ---- next pass of the bucket join: the buckets not marked done, into a fresh window ----
-                CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 0, info, st, &S.n_launches));
+                CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 0, 0, info, st, &S.n_launches));
                 rc = read_info(ctx, info, st);
                 if (rc) return rc;
                 if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
