@@ -682,7 +682,7 @@ constexpr int GP_TRIP = 16;        // d = 3: (g1, g2) iterations per step of a b
 constexpr int GP_ROUND = 5400;     // records a block stages per round (21 per digit of the 32 slots); the host turns it into batches per warp
                                    // (round 2: rounds of 3,300 records cost +10 %, i.e. ~2.3 us per flush stay exposed; 22 slots with four resident blocks: +7 %)
 constexpr int GP_NW = GP_THREADS / 32, GP_S = 32;  // (16 slots per digit and 4-5 resident blocks: generation 0.66 -> 0.85-1.25 ms on config 3, the digits overflow)
-static_assert(GP_THREADS >= 256 && GP_THREADS % 32 == 0 && GP_S <= 32, "one thread per digit in the flush, one lane per slot of a row");
+static_assert(GP_THREADS == 256 && GP_S <= 32, "one thread per digit in the flush, one lane per slot of a row");
 
 constexpr int GP_ROW = GP_S + 1;  // stage row stride in records: rank r of digit dg sits in 8-byte word dg * 33 + r, i.e. bank pair (dg + r) mod 16 — ranks are alike across digits, the odd stride spreads them
 struct GenPartShared {
@@ -707,7 +707,8 @@ struct GenPartParams {
     u32* cur;     // 256 bin cursors (zeroed by the host)
     u32 cap1;
     u32 batches;  // k_gen2_part: batches per warp and round
-    i64 task_begin, task_end;  // k_gen2_part: the warp tasks (groups of 32 sequences) of this launch — a slice when the input arrives in slices
+    i64 task_begin, task_end;  // k_gen2_part: the warp tasks of this launch — a slice when the input arrives in slices
+    u32 task_seqs;             // k_gen2_part: consecutive sequences per warp task (a power of two <= 32; g.groups_* count tasks of this size)
 };
 
 // D3 (d == 3): the triples {p1 < p2 < p3} follow the pairs.  A triple is the three points a, a + g1, a + g1 + g2
@@ -792,8 +793,8 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
         if (!have && wt < PP.task_end) {
             const bool in_b = wt >= P.groups_a;
             const SeqSetDev& S = in_b ? P.b : P.a;
-            const i64 first = (in_b ? wt - P.groups_a : wt) * 32;
-            ns = (u32)min((i64)32, S.n - first);
+            const i64 first = (in_b ? wt - P.groups_a : wt) * (i64)PP.task_seqs;
+            ns = (u32)min((i64)PP.task_seqs, S.n - first);
             gid0 = (u64)first + (in_b ? (u64)P.n_a : 0ull);
             seqs = S.seqs;
             o0 = 0;
@@ -979,6 +980,7 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
             flush = staged > (u32)GP_FLUSH_AT || (!any_more && staged > 0);
         }
         if (flush) {
+            const u32 novf = min(sh.novf, (u32)GP_OVF);  // (final since the round barrier; everyone has it before the next barrier, after which thread 0 clears the word)
             if (tid < 256) {
                 const u32 cn_ = min(sh.cnt[tid] >> 3, (u32)GP_S);
                 u32 g = 0;
@@ -994,25 +996,26 @@ __global__ void __launch_bounds__(GP_THREADS, GP_MINB) k_gen2_part(GenPartParams
                 sh.gofs[tid] = g;
             }
             __syncthreads();
+            if (tid == 0) sh.novf = 0;
+            static_assert(256 / GP_NW == 32, "a warp copies, then clears, 32 rows: one counter per lane");
             u64* const bins = PP.bins;
 #pragma unroll 4
-            for (u32 k = 0; k < 256 / GP_NW; ++k) {
-                const u32 dg = warp * (256 / GP_NW) + k;
+            for (u32 k = 0; k < 32; ++k) {
+                const u32 dg = warp * 32 + k;
                 const u32 g = sh.gofs[dg], cn_ = min(sh.cnt[dg] >> 3, (u32)GP_S);
                 if (lane < cn_ && g != 0xffffffffu) bins[g + lane] = sh.stage[dg * GP_ROW + lane];
             }
-            for (u32 i = tid; i < min(sh.novf, (u32)GP_OVF); i += GP_THREADS) {  // the overflow records, one global atomic each
+            __syncwarp();
+            sh.cnt[warp * 32 + lane] = 0;  // (after the claims only this warp reads these counters)
+            for (u32 i = tid; i < novf; i += GP_THREADS) {  // the overflow records, one global atomic each
                 const u64 rec = sh.ovf[i];
                 const u32 dg = (u32)(rec >> (P.id_bits + P.hash_bits - 8)) & 255u;
                 const u32 at = atomicAdd(&PP.cur[dg], 1u);
                 if (at < PP.cap1) PP.bins[(u64)dg * PP.cap1 + at] = rec;
                 else atomicOr(&P.info->part_overflow, 1u);
             }
-            __syncthreads();
-            if (tid < 256) sh.cnt[tid] = 0;
-            if (tid == 0) sh.novf = 0;
             staged = 0;
-            __syncthreads();
+            __syncthreads();  // rows, counters and the overflow list are free again
         }
         if (!any_more) break;
     }
@@ -1369,11 +1372,26 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
         const double per_round = lay.d == 3 ? GP_NW * 32.0 * GP_TRIP * 0.55 : GP_NW * 32.0 * std::max(records_per_residue, 0.03) * 0.85;
         PP.batches = (u32)std::min(8.0, std::max(1.0, std::floor(GP_ROUND / per_round + 0.5)));
     }
-    // task range: [task_begin, task_end) of the warp tasks; (0, -1) = all.  Only the launch that starts at task 0 clears the cursors.
+    // Warp tasks of k_gen2_part: every warp should get many — the last task of the slowest warp of a block keeps the other
+    // seven waiting at the round barriers.  With 32-sequence tasks config 5 (d = 3, ~740 records per sequence) had 1.7 tasks per
+    // warp and spent 43 % of its warp time at the round barrier: tasks of 2 sequences 1.90 -> 1.41 ms.  At d <= 2 a smaller task
+    // costs more than it balances (every task end breaks the packing of sequences into lanes: config 3 with 16: +2 %), so
+    // tasks shrink only below 8 per warp.
+    PP.task_seqs = 32;
+    if (fast) {
+        const i64 warps = (i64)148 * GP_MINB * GP_NW;
+        const i64 want = lay.d == 3 ? 64 : 8, low = lay.d == 3 ? 2 : 4;
+        while (PP.task_seqs > low && (a.n + b.n) / PP.task_seqs < want * warps) PP.task_seqs >>= 1;
+        PP.g.groups_a = (a.n + PP.task_seqs - 1) / PP.task_seqs;
+        PP.g.groups_total = PP.g.groups_a + (b.n + PP.task_seqs - 1) / PP.task_seqs;
+    }
+    // task range of this launch, given in units of 32 sequences: [task_begin, task_end); (0, -1) = all.  Only the launch that
+    // starts at task 0 clears the cursors.
     const bool sliced = task_end >= 0;
-    PP.task_begin = sliced ? task_begin : 0;
-    PP.task_end = sliced ? std::min(task_end, PP.g.groups_total) : PP.g.groups_total;
-    if (sliced && !fast) return cudaErrorInvalidValue;
+    const i64 per32 = 32 / PP.task_seqs;
+    PP.task_begin = sliced ? task_begin * per32 : 0;
+    PP.task_end = sliced ? std::min(task_end * per32, PP.g.groups_total) : PP.g.groups_total;
+    if (sliced && (!fast || b.n != 0)) return cudaErrorInvalidValue;  // (slices are ranges of set A: self-search)
     if (PP.task_begin >= PP.task_end && PP.task_begin > 0) return cudaSuccess;
     cudaError_t e;
     if (PP.task_begin == 0 && !cursors_cleared && (e = cudaMemsetAsync(cur, 0, 256 * sizeof(u32), st)) != cudaSuccess) return e;
