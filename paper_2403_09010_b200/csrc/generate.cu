@@ -1381,7 +1381,8 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     if (fast) {
         const i64 warps = (i64)148 * GP_MINB * GP_NW;
         const i64 want = lay.d == 3 ? 64 : 8, low = lay.d == 3 ? 2 : 4;
-        while (PP.task_seqs > low && (a.n + b.n) / PP.task_seqs < want * warps) PP.task_seqs >>= 1;
+        const i64 n_launch = task_end >= 0 ? std::min<i64>(a.n + b.n, (task_end - task_begin) * 32) : a.n + b.n;  // (a slice: what THIS launch covers)
+        while (PP.task_seqs > low && n_launch / PP.task_seqs < want * warps) PP.task_seqs >>= 1;
         PP.g.groups_a = (a.n + PP.task_seqs - 1) / PP.task_seqs;
         PP.g.groups_total = PP.g.groups_a + (b.n + PP.task_seqs - 1) / PP.task_seqs;
     }
