@@ -678,7 +678,7 @@ constexpr int GP_THREADS = 256;    // threads per block (512 with two resident b
 constexpr int GP_MINB = 3;         // resident blocks per SM (64 KB stage each)
 constexpr int GP_FLUSH_AT = 2800;  // flush when more than this is staged after a round (i.e. after nearly every full round)
 constexpr int GP_OVF = 64;         // overflow list entries
-constexpr int GP_TRIP = 16;        // d = 3: (g1, g2) iterations per step of a batch
+constexpr int GP_TRIP = 8;         // d = 3: (g1, g2) iterations per step of a batch (more, smaller units per round even the warps out: config 5 with 4 / 8 / 16 / 32: 1.40 / 1.33 / 1.41 / 1.58 ms)
 constexpr int GP_ROUND = 5400;     // records a block stages per round (21 per digit of the 32 slots); the host turns it into batches per warp
                                    // (round 2: rounds of 3,300 records cost +10 %, i.e. ~2.3 us per flush stay exposed; 22 slots with four resident blocks: +7 %)
 constexpr int GP_NW = GP_THREADS / 32, GP_S = 32;  // (16 slots per digit and 4-5 resident blocks: generation 0.66 -> 0.85-1.25 ms on config 3, the digits overflow)
