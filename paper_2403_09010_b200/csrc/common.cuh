@@ -38,6 +38,29 @@ struct DevInfo {
 enum { SD_ERR_OFFSETS = 1, SD_ERR_TOO_LONG = 2, SD_ERR_RESIDUE = 4, SD_ERR_INTERNAL = 8, SD_ERR_OVERFLOW = 16 };
 enum { SD_TK_SORT = 0, SD_TK_EMIT = 1, SD_TK_VERIFY = 2, SD_TK_FINAL = 3, SD_TK_SCAN = 4 };
 
+// ---- programmatic dependent launch (PDL; SASS: ACQBULK / griddepcontrol) ----------------------------------------
+// The record kernels and the sort passes run back to back on one stream.  A kernel launched with sd_launch_dep may be
+// scheduled while its predecessor drains; it must call sd_dep_wait() before it touches anything the predecessor wrote
+// (here: as its first statement, so the semantics are those of plain stream order — what is gained is the launch latency
+// and the ramp of the next grid).  sd_dep_release() lets the successor in once every block of this grid has started.
+__device__ __forceinline__ void sd_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void sd_dep_release() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+template <typename... KArgs, typename... Args>
+static inline cudaError_t sd_launch_dep(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st,
+                                        Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // ---- decoupled look-back, one 64-bit value per tile ---------------------------------------------
 // status word: bits 63:62 = flag (0 invalid, 1 aggregate, 2 inclusive prefix), bits 61:0 = value.
 // A tile publishes its aggregate, then walks its predecessors summing aggregates until it meets an

@@ -672,6 +672,7 @@ __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams 
     Smem& S = *reinterpret_cast<Smem*>(jn_smem);
     const JoinParams& P = BP.j;
     const u32 tid = threadIdx.x;
+    sd_dep_wait();  // (launched as a dependent of the level-2 partition)
     const u32 bucket = blockIdx.x;
     const u32 cword = BP.cnt[bucket];
     if (!P.first_round && !(cword & JB_OPEN)) return;  // later pass of a windowed search: only the buckets left open (block-uniform)
@@ -927,8 +928,8 @@ cudaError_t sd_join_bkt(const u64* buckets, u32* cnt, u32 cap, u32 nbuckets, con
     BP.j.slot_shift = std::max(lay.id_bits, top - lay.sort_bits - (small ? JB_SLOTB_S : JB_SLOTB_L));
     if (launches) ++*launches;
     if (small)
-        k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S><<<nbuckets, JB_THREADS_S, jb_smem_bytes(true, cap), st>>>(BP);
+        e = sd_launch_dep(k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S>, nbuckets, (unsigned)JB_THREADS_S, jb_smem_bytes(true, cap), st, BP);
     else
         k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L><<<nbuckets, JB_THREADS_L, jb_smem_bytes(false, cap), st>>>(BP);
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
 }

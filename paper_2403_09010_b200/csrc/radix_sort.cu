@@ -40,6 +40,8 @@ __global__ void __launch_bounds__(THREADS) k_histogram(const u64* __restrict__ k
 
 // exclusive scan of each pass's 256 bins, in place; one block of 256 threads per pass
 __global__ void __launch_bounds__(256) k_hist_scan(u32* __restrict__ ghist) {
+    sd_dep_wait();
+    sd_dep_release();
     __shared__ u32 s_warp[9];
     u32* h = ghist + blockIdx.x * 256;
     u32 v = h[threadIdx.x], total;
@@ -299,6 +301,8 @@ __global__ void __launch_bounds__(THREADS, MINB) k_onesweep(const u64* __restric
     __shared__ u32 s_warp[NW + 1];
     __shared__ u64 s_ends[2];
 
+    sd_dep_wait();  // (the passes are launched as dependents of one another)
+    sd_dep_release();
     const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool claim = smask == 0;
     // n_dev: the key count lives on the device (the grid was sized for an upper bound: surplus blocks leave at once —
@@ -363,6 +367,8 @@ struct Part2Params {
 };
 
 __global__ void __launch_bounds__(P2_THREADS, P2_MINB) k_part2(const Part2Params P) {
+    sd_dep_wait();  // (launched as a dependent of the generator)
+    sd_dep_release();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     u64* skeys = reinterpret_cast<u64*>(smem_raw);
     __shared__ u32 bhist[256];
@@ -500,7 +506,7 @@ cudaError_t sd_cand_filter(const u64* cand, i64 n, void* table, int table_bits, 
 // Turns the raw per-digit counts into exclusive bin bases (one tiny launch).
 cudaError_t sd_sort_hist_scan(void* scratch, int npass, cudaStream_t st, i64* launches) {
     if (npass == 0) return cudaSuccess;
-    k_hist_scan<<<npass, 256, 0, st>>>(sd_sort_hist_ptr(scratch));
+    if (sd_launch_dep(k_hist_scan, (unsigned)npass, 256u, 0, st, sd_sort_hist_ptr(scratch)) != cudaSuccess) return cudaGetLastError();
     if (launches) ++*launches;
     return cudaGetLastError();
 }
@@ -524,8 +530,9 @@ cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, const u64* n_dev, int beg
     u64 *src = keys, *dst = tmp;
     for (int p = 0; p < npass; ++p) {
         const u64 smask = stable ? ~0ull : (((1ull << (8 * p)) - 1ull) << begin_bit);
-        V.kernel<<<(unsigned)tiles, V.threads, V.smem, st>>>(src, dst, (u32)n, begin_bit + 8 * p, smask, hist + p * 256,
-                                                             status + (size_t)p * status_stride, tickets + p, n_dev);
+        const cudaError_t e = sd_launch_dep(V.kernel, (unsigned)tiles, (unsigned)V.threads, V.smem, st, (const u64*)src, dst, (u32)n, begin_bit + 8 * p,
+                                            smask, hist + p * 256, status + (size_t)p * status_stride, tickets + p, n_dev);
+        if (e != cudaSuccess) return e;
         if (launches) ++*launches;
         std::swap(src, dst);
     }
@@ -552,7 +559,7 @@ cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u
     P.shift = shift;
     P.tiles_per_bin = (u32)((cap1 + P2_TILE - 1) / P2_TILE);
     P.info = info;
-    k_part2<<<256 * P.tiles_per_bin, P2_THREADS, smem, st>>>(P);
+    if ((e = sd_launch_dep(k_part2, 256 * P.tiles_per_bin, P2_THREADS, smem, st, P)) != cudaSuccess) return e;
     if (launches) ++*launches;
     return cudaGetLastError();
 }
