@@ -660,7 +660,7 @@ struct JoinBktSmem {
 };
 
 // STAGE_MAX: the largest region this instance accepts
-template <int THREADS, int STAGE_MAX, int SLOT_BITS, int NB, int MINB>
+template <int THREADS, int STAGE_MAX, int SLOT_BITS, int NB, int MINB, bool CROSS>
 __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams BP) {
     typedef JoinBktSmem<SLOT_BITS> Smem;
     constexpr int SLOTS = 1 << SLOT_BITS, IT = (STAGE_MAX / 2 + THREADS - 1) / THREADS;  // 16-byte loads per thread that cover the stage
@@ -701,18 +701,59 @@ __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams 
     const int slot_shift = P.slot_shift;
     unsigned short* const link16 = reinterpret_cast<unsigned short*>(S.stage) + 3;  // bits 48..63 of record i: link16[4 * i]
     u32 flag = 0;  // bit 2k + e: my record 2 * (tid + k * THREADS) + e found an earlier record in its slot
+    if (!CROSS) {
 #pragma unroll
-    for (int k = 0; k < IT; ++k) {
-        const u32 i = 2 * (tid + k * THREADS);
-        if (i < n) {
-            const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(S.stage + i);
-            const u32 o0 = jb_atoms_exch(&S.head[(u32)(t.x >> slot_shift) & (SLOTS - 1)], i);
-            link16[4 * i] = (unsigned short)((o0 << (16 - NB)) | ((u32)(t.x >> 48) & ((1u << (16 - NB)) - 1u)));
-            flag |= (o0 != NIL ? 1u : 0u) << (2 * k);
-            if (i + 1 < n) {
-                const u32 o1 = jb_atoms_exch(&S.head[(u32)(t.y >> slot_shift) & (SLOTS - 1)], i + 1);
-                link16[4 * i + 4] = (unsigned short)((o1 << (16 - NB)) | ((u32)(t.y >> 48) & ((1u << (16 - NB)) - 1u)));
-                flag |= (o1 != NIL ? 2u : 0u) << (2 * k);
+        for (int k = 0; k < IT; ++k) {
+            const u32 i = 2 * (tid + k * THREADS);
+            if (i < n) {
+                const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(S.stage + i);
+                const u32 o0 = jb_atoms_exch(&S.head[(u32)(t.x >> slot_shift) & (SLOTS - 1)], i);
+                link16[4 * i] = (unsigned short)((o0 << (16 - NB)) | ((u32)(t.x >> 48) & ((1u << (16 - NB)) - 1u)));
+                flag |= (o0 != NIL ? 1u : 0u) << (2 * k);
+                if (i + 1 < n) {
+                    const u32 o1 = jb_atoms_exch(&S.head[(u32)(t.y >> slot_shift) & (SLOTS - 1)], i + 1);
+                    link16[4 * i + 4] = (unsigned short)((o1 << (16 - NB)) | ((u32)(t.y >> 48) & ((1u << (16 - NB)) - 1u)));
+                    flag |= (o1 != NIL ? 2u : 0u) << (2 * k);
+                }
+            }
+        }
+    } else {
+        // Cross-search: only (query, reference) pairs count, and the queries are usually the small side (config 4: 2 % of
+        // the records).  Sweep 1a chains the QUERY records only; sweep 1b lets every reference record look at the head of
+        // its slot — a plain load, no atomic, and nearly always empty — and keeps it as its link: the walk below then
+        // runs from reference records through query records only.
+        const u64 idm = P.idmask, na = P.n_a;
+#pragma unroll
+        for (int k = 0; k < IT; ++k) {
+            const u32 i = 2 * (tid + k * THREADS);
+            if (i < n) {
+                const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(S.stage + i);
+                if ((t.x & idm) < na) {
+                    const u32 o0 = jb_atoms_exch(&S.head[(u32)(t.x >> slot_shift) & (SLOTS - 1)], i);
+                    link16[4 * i] = (unsigned short)((o0 << (16 - NB)) | ((u32)(t.x >> 48) & ((1u << (16 - NB)) - 1u)));
+                }
+                if (i + 1 < n && (t.y & idm) < na) {
+                    const u32 o1 = jb_atoms_exch(&S.head[(u32)(t.y >> slot_shift) & (SLOTS - 1)], i + 1);
+                    link16[4 * i + 4] = (unsigned short)((o1 << (16 - NB)) | ((u32)(t.y >> 48) & ((1u << (16 - NB)) - 1u)));
+                }
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < IT; ++k) {
+            const u32 i = 2 * (tid + k * THREADS);
+            if (i < n) {
+                const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(S.stage + i);  // (a query record's link bits are not looked at here)
+                if ((t.x & idm) >= na) {
+                    const u32 o0 = S.head[(u32)(t.x >> slot_shift) & (SLOTS - 1)];
+                    link16[4 * i] = (unsigned short)((o0 << (16 - NB)) | ((u32)(t.x >> 48) & ((1u << (16 - NB)) - 1u)));
+                    flag |= (o0 != NIL ? 1u : 0u) << (2 * k);
+                }
+                if (i + 1 < n && (t.y & idm) >= na) {
+                    const u32 o1 = S.head[(u32)(t.y >> slot_shift) & (SLOTS - 1)];
+                    link16[4 * i + 4] = (unsigned short)((o1 << (16 - NB)) | ((u32)(t.y >> 48) & ((1u << (16 - NB)) - 1u)));
+                    flag |= (o1 != NIL ? 2u : 0u) << (2 * k);
+                }
             }
         }
     }
@@ -724,7 +765,7 @@ __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams 
         const u32 e = __ffs(m) - 1;
         const u64 y = S.stage[pos_of(e)];
         u32 c = 0;
-        if (!P.cross) {
+        if (!CROSS) {
             // self-search: same hash and different ids <=> 0 < (y ^ z) & KEEP < 2^id_bits
             for (u32 j = (u32)(y >> (64 - NB)); j != NIL;) {
                 const u64 z = S.stage[j];
@@ -804,9 +845,13 @@ static cudaError_t jn_setup_k() {
 cudaError_t sd_join_setup() {
     cudaError_t e;
     if ((e = cudaFuncSetAttribute(k_join, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(JoinSmem))) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if ((e = cudaFuncSetAttribute(k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)jb_smem_bytes(true, JB_STAGE_S))) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if ((e = cudaFuncSetAttribute(k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)jb_smem_bytes(true, JB_STAGE_S))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)jb_smem_bytes(false, JB_STAGE_L))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)jb_smem_bytes(false, JB_STAGE_L))) != cudaSuccess) return e;
     if ((e = jn_setup_k<true>()) != cudaSuccess) return e;
     return jn_setup_k<false>();
@@ -927,9 +972,10 @@ cudaError_t sd_join_bkt(const u64* buckets, u32* cnt, u32 cap, u32 nbuckets, con
     const bool small = cap <= (u32)JB_STAGE_S;
     BP.j.slot_shift = std::max(lay.id_bits, top - lay.sort_bits - (small ? JB_SLOTB_S : JB_SLOTB_L));
     if (launches) ++*launches;
-    if (small)
-        e = sd_launch_dep(k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S>, nbuckets, (unsigned)JB_THREADS_S, jb_smem_bytes(true, cap), st, BP);
-    else
-        k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L><<<nbuckets, JB_THREADS_L, jb_smem_bytes(false, cap), st>>>(BP);
+    const size_t smem = jb_smem_bytes(small, cap);
+    if (small && !lay.cross) e = sd_launch_dep(k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S, false>, nbuckets, (unsigned)JB_THREADS_S, smem, st, BP);
+    else if (small) e = sd_launch_dep(k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S, true>, nbuckets, (unsigned)JB_THREADS_S, smem, st, BP);
+    else if (!lay.cross) e = sd_launch_dep(k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L, false>, nbuckets, (unsigned)JB_THREADS_L, smem, st, BP);
+    else e = sd_launch_dep(k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L, true>, nbuckets, (unsigned)JB_THREADS_L, smem, st, BP);
     return e != cudaSuccess ? e : cudaGetLastError();
 }
