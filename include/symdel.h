@@ -92,6 +92,7 @@ typedef struct {
     int64_t join_redo_tiles;   /* join tiles that overflowed the small candidate list and were redone by the large-list kernel */
     int64_t surv_merges;       /* multi-flush searches: times the survivor list was sorted and deduplicated to make room */
     int64_t join_windows;      /* fused pipeline: extra passes of the bucket join (the pairs of a chunk exceeded one candidate window) */
+    int64_t query_filter_bits; /* cross-search: 2^bits filter bits per level-1 bin when the query filter ran (0: it did not) */
 } symdel_stats;
 
 /* Options (symdel_set_option); defaults in brackets. */
@@ -111,6 +112,7 @@ enum {
     SYMDEL_OPT_METRIC = 14,       /* [0] 0: Levenshtein distance (the paper's metric).  1: Hamming distance (Fig. S3 A/C): only pairs of EQUAL length with <= d mismatching positions are returned, dist = the mismatch count; candidates come from the same deletion-variant join (hamming <= d implies lev <= d) */
     SYMDEL_OPT_SURV_CAPACITY = 15, /* [0] >0: size of the survivor list of multi-flush searches in pairs (test hook; never below capacity + one candidate window) */
     SYMDEL_OPT_CAND_FILTER = 16, /* [0] duplicate suppression before the candidate sort (a best-effort hash set of pair ids): 0 = automatic (on when the candidates are many but few per record), 1 = always, 2 = never (test hook; results are identical) */
+    SYMDEL_OPT_NO_QUERY_FILTER = 17, /* [0] 1: cross-search never drops reference records through the query filter (test hook: same result) */
     SYMDEL_OPT_SORT_GROUPING = 10 /* [0] 1: symdel_stage_sort_u64 sorts keys only: ties land in arbitrary order (the mode the pipeline uses) */
 };
 

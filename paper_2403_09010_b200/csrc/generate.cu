@@ -1358,6 +1358,9 @@ bool sd_gen_part_sliceable(const Layout& lay, int width) { return use_fast_part(
 cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, u64* bins, u32* cur, u64 cap1,
                         double records_per_residue, double avg_len, i64 task_begin, i64 task_end, int cursors_cleared, DevInfo* info,
                         cudaStream_t st, i64* launches) {
+    // task_end == -2 / -3: set A only / set B only (cross-search with the query filter: the queries are generated first)
+    const int which = task_end == -2 ? 1 : task_end == -3 ? 2 : 0;
+    if (which) task_end = -1;
     const bool fast = use_fast_part(lay, width);
     GenPartParams PP{};
     PP.g = fast ? make_params2(a, b, lay, width) : make_params(a, b, lay, width);
@@ -1381,7 +1384,7 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     if (fast) {
         const i64 warps = (i64)148 * GP_MINB * GP_NW;
         const i64 want = lay.d == 3 ? 64 : 8, low = lay.d == 3 ? 2 : 4;
-        const i64 n_launch = task_end >= 0 ? std::min<i64>(a.n + b.n, (task_end - task_begin) * 32) : a.n + b.n;  // (a slice: what THIS launch covers)
+        const i64 n_launch = which == 1 ? a.n : which == 2 ? b.n : task_end >= 0 ? std::min<i64>(a.n + b.n, (task_end - task_begin) * 32) : a.n + b.n;  // (what THIS launch covers)
         while (PP.task_seqs > low && n_launch / PP.task_seqs < want * warps) PP.task_seqs >>= 1;
         PP.g.groups_a = (a.n + PP.task_seqs - 1) / PP.task_seqs;
         PP.g.groups_total = PP.g.groups_a + (b.n + PP.task_seqs - 1) / PP.task_seqs;
@@ -1393,6 +1396,9 @@ cudaError_t sd_gen_part(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
     PP.task_begin = sliced ? task_begin * per32 : 0;
     PP.task_end = sliced ? std::min(task_end * per32, PP.g.groups_total) : PP.g.groups_total;
     if (sliced && (!fast || b.n != 0)) return cudaErrorInvalidValue;  // (slices are ranges of set A: self-search)
+    if (which && !fast) return cudaErrorInvalidValue;
+    if (which == 1) PP.task_end = PP.g.groups_a;
+    if (which == 2) PP.task_begin = PP.g.groups_a;
     if (PP.task_begin >= PP.task_end && PP.task_begin > 0) return cudaSuccess;
     cudaError_t e;
     if (PP.task_begin == 0 && !cursors_cleared && (e = cudaMemsetAsync(cur, 0, 256 * sizeof(u32), st)) != cudaSuccess) return e;

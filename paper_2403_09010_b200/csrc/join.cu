@@ -614,6 +614,7 @@ struct JoinBktParams {
     JoinParams j;       // rec = bucket regions; topmask unused
     u32* cnt;           // records per bucket; bit 31 = its pairs did not fit the window of an earlier pass (windowed searches: later passes join exactly these)
     u32 cap;            // region stride (records; a multiple of 32)
+    u32 stage_cap;      // records the launched instance stages (<= cap): a fuller bucket is left open for a pass of the large instance
     u32 nbuckets;
 };
 
@@ -678,6 +679,13 @@ __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams 
     if (!P.first_round && !(cword & JB_OPEN)) return;  // later pass of a windowed search: only the buckets left open (block-uniform)
     const u32 n = min(cword & ~JB_OPEN, BP.cap);
     if (n < 2) return;  // nothing to pair
+    if (n > BP.stage_cap) {  // (block-uniform) the small instance was launched on regions that may hold more than it stages
+        if (tid == 0) {
+            atomicOr(&P.info->join_fallback, 2u);
+            if (!(cword & JB_OPEN)) BP.cnt[bucket] = cword | JB_OPEN;
+        }
+        return;
+    }
     // later pass of a windowed search and the window is already full: this bucket waits for the next pass (nothing loaded,
     // nothing counted).  One thread looks, the barrier makes the decision the block's.
     if (!P.first_round && __syncthreads_or(tid == 0 && sd_ld_relaxed(&P.info->n_cand) >= P.win_hi)) {
@@ -952,7 +960,7 @@ int sd_join_bkt_max_cap() { return JB_STAGE_L; }
 int sd_join_bkt_link_bits(u32 cap) { return cap <= (u32)JB_STAGE_S ? JB_NB_S : JB_NB_L; }
 
 cudaError_t sd_join_bkt(const u64* buckets, u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
-                        int first_pass, int info_fresh, DevInfo* info, cudaStream_t st, i64* launches) {
+                        int first_pass, int info_fresh, int prefer_small, DevInfo* info, cudaStream_t st, i64* launches) {
     cudaError_t e = cudaSuccess;
     // (info_fresh: the whole status block was cleared for this call and nothing has counted pairs or raised a join flag yet)
     if (!info_fresh && (e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
@@ -969,10 +977,13 @@ cudaError_t sd_join_bkt(const u64* buckets, u32* cnt, u32 cap, u32 nbuckets, con
     BP.nbuckets = nbuckets;
     // chain slot = the hash bits right below the partitioned ones (clamped to the hash field)
     const int top = lay.id_bits + lay.hash_bits;
-    const bool small = cap <= (u32)JB_STAGE_S;
+    // prefer_small: the regions were sized for more records than they are expected to hold (the query filter of a cross-search
+    // dropped most of them): the small instance takes every bucket it can stage and leaves the others open for a later call
+    const bool small = cap <= (u32)JB_STAGE_S || prefer_small;
+    BP.stage_cap = small ? std::min<u32>(cap, (u32)JB_STAGE_S) : cap;
     BP.j.slot_shift = std::max(lay.id_bits, top - lay.sort_bits - (small ? JB_SLOTB_S : JB_SLOTB_L));
     if (launches) ++*launches;
-    const size_t smem = jb_smem_bytes(small, cap);
+    const size_t smem = jb_smem_bytes(small, BP.stage_cap);
     if (small && !lay.cross) e = sd_launch_dep(k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S, false>, nbuckets, (unsigned)JB_THREADS_S, smem, st, BP);
     else if (small) e = sd_launch_dep(k_join_bkt<JB_THREADS_S, JB_STAGE_S, JB_SLOTB_S, JB_NB_S, JB_MINB_S, true>, nbuckets, (unsigned)JB_THREADS_S, smem, st, BP);
     else if (!lay.cross) e = sd_launch_dep(k_join_bkt<JB_THREADS_L, JB_STAGE_L, JB_SLOTB_L, JB_NB_L, JB_MINB_L, false>, nbuckets, (unsigned)JB_THREADS_L, smem, st, BP);

@@ -52,8 +52,13 @@ cudaError_t sd_cand_filter(const u64* cand, i64 n, void* table, int table_bits, 
                            cudaStream_t st, i64* launches);
 
 // level-2 partition of the fused pipeline: bins (256 x cap1) -> buckets ((256 << b2) x cap2)
+#define SD_FBITS_MAX 18  // query filter: at most 2^18 bits (32 KB) per level-1 bin
+// bitmap != nullptr: the query filter of a cross-search (radix_sort.cu, k_bin_bitmap): 256 bitmaps of 2^fbits bits built by
+// sd_bin_bitmap from the first cnt_a[bin] records of every bin; fshift = position of the fbits hash bits below the bin digit
+cudaError_t sd_bin_bitmap(const u64* bins, const u32* cnt_a, i64 cap1, u32* bitmap, int fbits, int fshift, cudaStream_t st, i64* launches);
 cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u32* cnt2, i64 cap2, int b2, int shift,
-                     int counts_cleared, DevInfo* info, cudaStream_t st, i64* launches);
+                     int counts_cleared, const u32* bitmap, const u32* cnt_a, int fbits, int fshift, DevInfo* info, cudaStream_t st,
+                     i64* launches);
 
 // ---- generate.cu --------------------------------------------------------------------------------
 cudaError_t sd_generate_setup();  // per-device setup: the __constant__ tables and function attributes; symdel_create
@@ -77,6 +82,7 @@ cudaError_t sd_generate(SeqSetDev a, SeqSetDev b, const Layout& lay, int width, 
 // the bin counts afterwards).  info->part_overflow != 0: a bin was full, redo with the exact pipeline.
 bool sd_gen_part_applies(const Layout& lay, int width);
 // records_per_residue = (deletion sets of this chunk) / (residues): sizes the generation rounds
+// task_end == -2 / -3: set A only / set B only (the later launch appends: pass cursors_cleared).
 // [task_begin, task_end): the warp tasks (groups of 32 consecutive sequences, A then B) of this launch; task_end < 0 = all.
 // Slices (sd_gen_part_sliceable only) append to the same bins: the launch starting at task 0 clears the cursors (unless the
 // caller has: cursors_cleared).
@@ -112,7 +118,7 @@ cudaError_t sd_join_fast_redo(const u64* records, i64 n_records, const Layout& l
 int sd_join_bkt_max_cap();
 int sd_join_bkt_link_bits(u32 cap);  // bits on top of a record that must be constant within a bucket
 cudaError_t sd_join_bkt(const u64* buckets, u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
-                        int first_pass, int info_fresh, DevInfo* info, cudaStream_t st, i64* launches);
+                        int first_pass, int info_fresh, int prefer_small, DevInfo* info, cudaStream_t st, i64* launches);
 
 // ---- verify.cu ----------------------------------------------------------------------------------
 i64 sd_verify_tiles(i64 n);

@@ -364,7 +364,60 @@ struct Part2Params {
     int b2, shift;  // digit = (record >> shift) & (2^b2 - 1)
     u32 tiles_per_bin;
     DevInfo* info;
+    // query filter (cross-search, FILT instance): a record of set B is kept only if some record of set A of the same bin has
+    // the same fbits hash bits below the bin digit; the first cnt_a[bin] records of a bin are set A's (generated first)
+    const u32* bitmap;  // 256 bitmaps of 2^fbits bits
+    const u32* cnt_a;
+    int fbits, fshift;
 };
+
+// One tile of k_part2 from the ranking on: `key` / `valid` (bit k: key[k] takes part; FULL: all of them) in registers.
+template <bool FULL>
+__device__ __forceinline__ void p2_tile(const Part2Params& P, const u64 (&key)[P2_IPT], const u32 valid, const u32 n_valid, const u32 bin,
+                                        u64* skeys, u32* bhist, u32* s_gofs, u32* s_warp) {
+    const u32 tid = threadIdx.x;
+    const u32 dmask = (1u << P.b2) - 1u;
+    u32 rank[P2_IPT / 2];  // two 16-bit ranks per word
+#pragma unroll
+    for (int k = 0; k < P2_IPT; ++k) {
+        u32 r = 0;
+        if (FULL || ((valid >> k) & 1u)) r = atomicAdd(&bhist[(u32)(key[k] >> P.shift) & dmask], 1u);
+        if (k & 1) rank[k >> 1] |= r << 16;
+        else rank[k >> 1] = r;
+    }
+    __syncthreads();
+    const u32 total = bhist[tid];
+    u32 claimed = 0;
+    bool dead = false;
+    if (total) claimed = atomicAdd(&P.cnt2[(bin << P.b2) + tid], total);
+    u32 tile_sum;
+    const u32 tstart = sd_block_excl_sum<P2_THREADS>(total, &tile_sum, s_warp);
+    bhist[tid] = tstart;
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < P2_IPT; ++k) {
+        if (FULL || ((valid >> k) & 1u)) {
+            const u32 r = (k & 1) ? (rank[k >> 1] >> 16) : (rank[k >> 1] & 0xffffu);
+            skeys[bhist[(u32)(key[k] >> P.shift) & dmask] + r] = key[k];
+        }
+    }
+    // the claim is looked at only now: its round trip to L2 ran under the scan and the staging stores
+    if (total && claimed + total > P.cap2) {
+        atomicOr(&P.info->part_overflow, 2u);
+        dead = true;
+    }
+    s_gofs[tid] = dead ? 0xffffffffu : ((bin << P.b2) + tid) * P.cap2 + claimed - tstart;
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < P2_IPT; ++k) {
+        const u32 pos = tid + k * P2_THREADS;
+        if (FULL || pos < n_valid) {
+            const u64 kk = skeys[pos];
+            const u32 g = s_gofs[(u32)(kk >> P.shift) & dmask];
+            if (g != 0xffffffffu) P.buckets[g + pos] = kk;
+        }
+    }
+}
 
 __global__ void __launch_bounds__(P2_THREADS, P2_MINB) k_part2(const Part2Params P) {
     sd_dep_wait();  // (launched as a dependent of the generator)
@@ -380,58 +433,141 @@ __global__ void __launch_bounds__(P2_THREADS, P2_MINB) k_part2(const Part2Params
     const u32 base = k0 * P2_TILE;
     if (base >= n_bin) return;
     const u32 tile_n = min((u32)P2_TILE, n_bin - base);
-    const bool full = tile_n == (u32)P2_TILE;
     const u64* in = P.bins + (u64)bin * P.cap1 + base;
-    const u32 dmask = (1u << P.b2) - 1u;
     bhist[tid] = 0;
     const u32 wbase = warp * (32 * P2_IPT);
     u64 key[P2_IPT];
+    if (tile_n == (u32)P2_TILE) {  // (block-uniform)
 #pragma unroll
-    for (int k = 0; k < P2_IPT; ++k) {
-        const u32 pos = wbase + 32 * k + lane;
-        key[k] = (full || pos < tile_n) ? in[pos] : 0ull;
+        for (int k = 0; k < P2_IPT; ++k) key[k] = in[wbase + 32 * k + lane];
+        __syncthreads();
+        p2_tile<true>(P, key, 0xffffffffu, tile_n, bin, skeys, bhist, s_gofs, s_warp);
+    } else {
+        u32 valid = 0;
+#pragma unroll
+        for (int k = 0; k < P2_IPT; ++k) {
+            const u32 pos = wbase + 32 * k + lane;
+            const bool ok = pos < tile_n;
+            key[k] = ok ? in[pos] : 0ull;
+            valid |= (ok ? 1u : 0u) << k;
+        }
+        __syncthreads();
+        p2_tile<false>(P, key, valid, tile_n, bin, skeys, bhist, s_gofs, s_warp);
     }
-    __syncthreads();
-    u32 rank[P2_IPT / 2];  // two 16-bit ranks per word
-#pragma unroll
-    for (int k = 0; k < P2_IPT; ++k) {
-        u32 r = 0;
-        if (full || (wbase + 32 * k + lane) < tile_n) r = atomicAdd(&bhist[(u32)(key[k] >> P.shift) & dmask], 1u);
-        if (k & 1) rank[k >> 1] |= r << 16;
-        else rank[k >> 1] = r;
+}
+
+// The filtering form (cross-search, see k_bin_bitmap below): a block walks P2F_TILES consecutive tiles of one bin with the
+// bin's bitmap in shared memory, keeps what passes in a staging tile (one slice per warp), and partitions the staging tile
+// whenever the next input tile might not fit — most set-B records never reach the ranking, the scatter or HBM again.
+constexpr int P2F_TILES = 16, P2F_IPT = 8, P2F_IN = P2_THREADS * P2F_IPT;
+__global__ void __launch_bounds__(P2_THREADS, 3) k_part2f(const Part2Params P) {
+    sd_dep_wait();
+    sd_dep_release();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    u64* skeys = reinterpret_cast<u64*>(smem_raw);       // staging tile / digit-ordered tile
+    u32* sbm = reinterpret_cast<u32*>(skeys + P2_TILE);  // this bin's bitmap
+    __shared__ u32 bhist[256];
+    __shared__ u32 s_gofs[256];
+    __shared__ u32 s_warp[P2_THREADS / 32 + 1];
+    const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 groups = (P.tiles_per_bin + P2F_TILES - 1) / P2F_TILES;
+    const u32 bin = blockIdx.x / groups, t0 = (blockIdx.x % groups) * P2F_TILES;
+    const u32 n_bin = (u32)min((u64)P.cnt1[bin], P.cap1);
+    if (t0 * P2_TILE >= n_bin) return;
+    {
+        const u32 words = 1u << (P.fbits - 5);
+        const uint4* src = reinterpret_cast<const uint4*>(P.bitmap + (size_t)bin * words);
+        for (u32 i = tid; i < words / 4; i += P2_THREADS) reinterpret_cast<uint4*>(sbm)[i] = src[i];
     }
-    __syncthreads();
-    const u32 total = bhist[tid];
-    u32 claimed = 0;
-    bool dead = false;
-    if (total) claimed = atomicAdd(&P.cnt2[(bin << P.b2) + tid], total);
-    u32 tile_sum;
-    const u32 tstart = sd_block_excl_sum<P2_THREADS>(total, &tile_sum, s_warp);
-    bhist[tid] = tstart;
-    __syncthreads();
+    const u32 na = P.cnt_a[bin], fmask = (1u << P.fbits) - 1u;
+    // Staging: every warp keeps what passes in its own slice of the staging tile (ballot + popcount, no block-wide step);
+    // the block partitions the tile when some warp's slice could not take another input tile.
+    constexpr u32 SLICE = P2_TILE / (P2_THREADS / 32);  // 512 slots per warp
+    static_assert(SLICE >= 2 * 32 * P2F_IPT, "a slice takes at least two input tiles of its warp");
+    __shared__ u32 s_wcnt[P2_THREADS / 32];
+    if (tid < P2_THREADS / 32) s_wcnt[tid] = 0;
+    u32 wcnt = 0;  // records in this warp's slice (warp-uniform)
+    auto flush = [&]() {  // partitions the staging tile (called by all threads)
+        if (lane == 0) s_wcnt[warp] = wcnt;
+        __syncthreads();
+        u64 key[P2_IPT];
+        u32 valid = 0, n_stage = 0;
 #pragma unroll
-    for (int k = 0; k < P2_IPT; ++k) {
-        if (full || (wbase + 32 * k + lane) < tile_n) {
-            const u32 r = (k & 1) ? (rank[k >> 1] >> 16) : (rank[k >> 1] & 0xffffu);
-            skeys[bhist[(u32)(key[k] >> P.shift) & dmask] + r] = key[k];
+        for (int w = 0; w < P2_THREADS / 32; ++w) n_stage += s_wcnt[w];
+#pragma unroll
+        for (int k = 0; k < P2_IPT; ++k) {
+            const u32 pos = tid + k * P2_THREADS;
+            const bool ok = (pos % SLICE) < s_wcnt[pos / SLICE];
+            key[k] = ok ? skeys[pos] : 0ull;
+            valid |= (ok ? 1u : 0u) << k;
+        }
+        bhist[tid] = 0;
+        __syncthreads();  // staging tile read by everyone, histogram cleared
+        p2_tile<false>(P, key, valid, n_stage, bin, skeys, bhist, s_gofs, s_warp);
+        __syncthreads();  // skeys free again
+        wcnt = 0;
+    };
+    __syncthreads();  // bitmap loaded
+    // input in tiles of P2F_IPT keys per thread, the next tile's loads in flight while this one is tested and appended
+    const u32 r0 = t0 * P2_TILE, r1 = min(n_bin, (t0 + P2F_TILES) * (u32)P2_TILE);
+    const u64* in = P.bins + (u64)bin * P.cap1;
+    const u32 fw = warp * (32 * P2F_IPT);
+    const u32 lane_lt = (1u << lane) - 1u;
+    u64* const slice = skeys + warp * SLICE;
+    u64 nxt[P2F_IPT];
+#pragma unroll
+    for (int k = 0; k < P2F_IPT; ++k) {
+        const u32 pos = r0 + fw + 32 * k + lane;
+        nxt[k] = pos < r1 ? in[pos] : 0ull;
+    }
+    for (u32 base = r0; base < r1; base += P2F_IN) {
+        u64 key[P2F_IPT];
+#pragma unroll
+        for (int k = 0; k < P2F_IPT; ++k) key[k] = nxt[k];
+#pragma unroll
+        for (int k = 0; k < P2F_IPT; ++k) {
+            const u32 pos = base + P2F_IN + fw + 32 * k + lane;
+            nxt[k] = pos < r1 ? in[pos] : 0ull;
+        }
+        // could this tile overflow a slice?  (one barrier per input tile, and only this one)
+        if (__syncthreads_or(wcnt + 32 * P2F_IPT > SLICE)) flush();
+#pragma unroll
+        for (int k = 0; k < P2F_IPT; ++k) {
+            const u32 pos = base + fw + 32 * k + lane;
+            bool keep = false;
+            if (pos < r1) {
+                const u32 idx = (u32)(key[k] >> P.fshift) & fmask;
+                keep = pos < na || ((sbm[idx >> 5] >> (idx & 31u)) & 1u);
+            }
+            const u32 bal = __ballot_sync(SD_FULL, keep);
+            if (keep) slice[wcnt + __popc(bal & lane_lt)] = key[k];
+            wcnt += __popc(bal);
         }
     }
-    // the claim is looked at only now: its round trip to L2 ran under the scan and the staging stores
-    if (total && claimed + total > P.cap2) {
-        atomicOr(&P.info->part_overflow, 2u);
-        dead = true;
-    }
-    s_gofs[tid] = dead ? 0xffffffffu : ((bin << P.b2) + tid) * P.cap2 + claimed - tstart;
+    flush();
+}
+
+
+// Query filter of a cross-search (reading the paper's asymmetric use, "both the query and reference sets", with
+// a small query set): one block per level-1 bin marks, for the set-A records of the bin (its first cnt_a[bin] records: set A
+// is generated first), the fbits hash bits below the bin digit.  k_part2f then drops every set-B record whose bits are
+// not marked: no record of set A can have its hash, so it cannot make a pair — the result is unchanged.
+constexpr int BM_THREADS = 512;
+__global__ void __launch_bounds__(BM_THREADS) k_bin_bitmap(const u64* __restrict__ bins, const u32* __restrict__ cnt_a, u64 cap1,
+                                                          u32* __restrict__ bitmap, int fbits, int fshift) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    u32* sb = reinterpret_cast<u32*>(smem_raw);
+    const u32 bin = blockIdx.x, words = 1u << (fbits - 5), fmask = (1u << fbits) - 1u;
+    for (u32 i = threadIdx.x; i < words; i += BM_THREADS) sb[i] = 0;
     __syncthreads();
-#pragma unroll
-    for (int k = 0; k < P2_IPT; ++k) {
-        const u32 pos = tid + k * P2_THREADS;
-        if (full || pos < tile_n) {
-            const u64 kk = skeys[pos];
-            const u32 g = s_gofs[(u32)(kk >> P.shift) & dmask];
-            if (g != 0xffffffffu) P.buckets[g + pos] = kk;
-        }
+    const u32 n = (u32)min((u64)cnt_a[bin], cap1);
+    const u64* in = bins + (u64)bin * cap1;
+    for (u32 i = threadIdx.x; i < n; i += BM_THREADS) {
+        const u32 idx = (u32)(in[i] >> fshift) & fmask;
+        atomicOr(&sb[idx >> 5], 1u << (idx & 31u));
     }
+    __syncthreads();
+    for (u32 i = threadIdx.x; i < words; i += BM_THREADS) bitmap[(size_t)bin * words + i] = sb[i];
 }
 
 struct OsVariant {
@@ -465,6 +601,8 @@ cudaError_t sd_sort_setup() {
     for (int v = 0; v < OS_NVARIANTS; ++v)
         if ((e = cudaFuncSetAttribute(OS_VARIANTS[v].kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OS_VARIANTS[v].smem)) != cudaSuccess)
             return e;
+    if ((e = cudaFuncSetAttribute(k_part2f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)P2_TILE * 8 + (size_t)(1 << SD_FBITS_MAX) / 8))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_bin_bitmap, cudaFuncAttributeMaxDynamicSharedMemorySize, (1 << SD_FBITS_MAX) / 8)) != cudaSuccess) return e;
     return cudaFuncSetAttribute(k_part2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)P2_TILE * 8));
 }
 
@@ -543,10 +681,17 @@ cudaError_t sd_sort_passes(u64* keys, u64* tmp, i64 n, const u64* n_dev, int beg
 // Level-2 partition of the fused pipeline: bins (256 x cap1, counts cnt1) -> buckets (2^(8+b2) x cap2,
 // counts cnt2, zeroed here).  shift = bit of the record where the b2-bit digit starts.  b2 == 0: no-op
 // for the caller (the bins are the buckets).
+cudaError_t sd_bin_bitmap(const u64* bins, const u32* cnt_a, i64 cap1, u32* bitmap, int fbits, int fshift, cudaStream_t st, i64* launches) {
+    k_bin_bitmap<<<256, BM_THREADS, (size_t)(1 << fbits) / 8, st>>>(bins, cnt_a, (u64)cap1, bitmap, fbits, fshift);
+    if (launches) ++*launches;
+    return cudaGetLastError();
+}
+
 cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u32* cnt2, i64 cap2, int b2, int shift,
-                     int counts_cleared, DevInfo* info, cudaStream_t st, i64* launches) {
+                     int counts_cleared, const u32* bitmap, const u32* cnt_a, int fbits, int fshift, DevInfo* info, cudaStream_t st,
+                     i64* launches) {
     cudaError_t e;
-    constexpr size_t smem = (size_t)P2_TILE * 8;
+    const size_t smem = (size_t)P2_TILE * 8 + (bitmap ? (size_t)(1 << fbits) / 8 : 0);
     if (!counts_cleared && (e = cudaMemsetAsync(cnt2, 0, ((size_t)256 << b2) * sizeof(u32), st)) != cudaSuccess) return e;
     Part2Params P{};
     P.bins = bins;
@@ -559,7 +704,13 @@ cudaError_t sd_part2(const u64* bins, const u32* cnt1, i64 cap1, u64* buckets, u
     P.shift = shift;
     P.tiles_per_bin = (u32)((cap1 + P2_TILE - 1) / P2_TILE);
     P.info = info;
-    if ((e = sd_launch_dep(k_part2, 256 * P.tiles_per_bin, P2_THREADS, smem, st, P)) != cudaSuccess) return e;
+    P.bitmap = bitmap;
+    P.cnt_a = cnt_a;
+    P.fbits = fbits;
+    P.fshift = fshift;
+    if (bitmap) e = sd_launch_dep(k_part2f, 256 * ((P.tiles_per_bin + P2F_TILES - 1) / P2F_TILES), (unsigned)P2_THREADS, smem, st, P);
+    else e = sd_launch_dep(k_part2, 256 * P.tiles_per_bin, (unsigned)P2_THREADS, smem, st, P);
+    if (e != cudaSuccess) return e;
     if (launches) ++*launches;
     return cudaGetLastError();
 }

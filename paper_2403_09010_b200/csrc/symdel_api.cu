@@ -35,7 +35,7 @@ struct symdel_ctx {
     symdel_stats stats{};
     int opt_timing = 0;
     i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0, opt_general_gen = 0;
-    i64 opt_sort_variant = 0, opt_surv_cap = 0, opt_cand_filter = 0;
+    i64 opt_sort_variant = 0, opt_surv_cap = 0, opt_cand_filter = 0, opt_no_query_filter = 0;
     i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0, opt_join_general = 0, opt_exact = 0, opt_prefix = 0, opt_metric = 0;
     DevInfo* h_info = nullptr;  // pinned; followed by 256 u32 (the level-1 bin counts of the fused pipeline)
     void* arena = nullptr;      // device arena of the *_host entry points: outputs + workspace
@@ -398,6 +398,28 @@ restart:
             // level-1 cursors and level-2 counts are neighbours: one clear for both, ahead of generation
             CK(cudaMemsetAsync(fcnt, 0, (size_t)(256 + (fp.b2 ? fp.nbuckets : 0)) * sizeof(u32), st));
             const double rpr = (double)nmax / (double)std::max<i64>(residues, 1) / (double)P, avg_len = (double)residues / (double)n_total;
+            // Query filter (cross-search with the queries the small side): set A is generated first, its records mark a bitmap per
+            // level-1 bin, and the level-2 partition drops the set-B records that no set-A record can match (radix_sort.cu).
+            // The bitmaps live in the second candidate buffer, which nothing uses before the candidate sort.
+            int fbits = 0;
+            u32 *fbm = nullptr, *cnt_a = nullptr;
+            const int fshift_top = lay.id_bits + lay.hash_bits - 8;
+            if (cross && fp.b2 && !ctx->opt_no_query_filter && A.n * 4 <= B.n && sd_gen_part_sliceable(lay, width)) {
+                const double a_per_bin = (double)(nmax - (i64)ctx->h_info->nmax_b) / (double)P / 256.0;
+                fbits = 13;
+                while (fbits < SD_FBITS_MAX && (double)((i64)1 << fbits) < 6.0 * a_per_bin) ++fbits;
+                const i64 need = ((i64)256 << (fbits - 5)) * 4 + 256 * 4;
+                if (2.0 * a_per_bin > (double)((i64)1 << fbits) || lay.hash_bits < 8 + fbits || need > cphys * 8) fbits = 0;  // (too dense to pay, or no room)
+                if (fbits) fbm = reinterpret_cast<u32*>(candB), cnt_a = fbm + ((size_t)256 << (fbits - 5));
+            }
+            S.query_filter_bits = fbits;
+            if (fbits) {
+                CK(wait_input());
+                CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, rpr, avg_len, 0, -2, 1, info, st, &S.n_launches));
+                CK(cudaMemcpyAsync(cnt_a, cur1, 256 * sizeof(u32), cudaMemcpyDeviceToDevice, st));
+                CK(sd_bin_bitmap(recA, cnt_a, fp.cap1, fbm, fbits, fshift_top - fbits, st, &S.n_launches));
+                CK(sd_gen_part(A, B, lay, width, recA, cur1, (u64)fp.cap1, rpr, avg_len, 0, -3, 1, info, st, &S.n_launches));
+            } else
             if (hp && hp->n_slices > 1 && !input_waited && sd_gen_part_sliceable(lay, width)) {
                 // generation follows the input slice by slice: slice i is generated while slice i + 1 is being copied
                 i64 t0 = 0;
@@ -413,14 +435,14 @@ restart:
             }
             const size_t x1 = tm.mark();
             if (fp.b2)
-                CK(sd_part2(recA, cur1, fp.cap1, recB, cnt2, fp.cap2, fp.b2, lay.id_bits + lay.hash_bits - fp.b, 1, info, st,
+                CK(sd_part2(recA, cur1, fp.cap1, recB, cnt2, fp.cap2, fp.b2, lay.id_bits + lay.hash_bits - fp.b, 1, fbm, cnt_a, fbits, fshift_top - fbits, info, st,
                             &S.n_launches));
             const size_t x2 = tm.mark();
             f_bkt = fp.b2 ? recB : recA;
             f_bcnt = fp.b2 ? cnt2 : cur1;
             f_bcap = (u32)(fp.b2 ? fp.cap2 : fp.cap1), f_nb = (u32)fp.nbuckets;
             u32* h_cur = reinterpret_cast<u32*>(ctx->h_info + 1);
-            CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 1, fresh, info, st, &S.n_launches));
+            CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 1, fresh, fbits ? 1 : 0, info, st, &S.n_launches));
             CK(join_side());
             CK(cudaMemcpyAsync(h_cur, cur1, 256 * sizeof(u32), cudaMemcpyDeviceToHost, st));  // (bit 31 of a count is the join's "open" mark)
             rc = read_info(ctx, info, st);
@@ -429,7 +451,9 @@ restart:
             // pairs beyond one window: the buckets that fit are done, the others are joined by later passes (window loop below)
             fused_more = ctx->h_info->join_fallback != 0;
             C = (i64)std::min<u64>(ctx->h_info->n_cand, ~ctx->h_info->nofit_inv);
-            fused_ok = !ctx->h_info->part_overflow && !(fused_more && C == 0);
+            // (nothing written and buckets left open: one bucket's pairs exceed a whole window — unless the small join instance was
+            //  preferred and simply could not stage any bucket: then the next pass, with the large instance, decides)
+            fused_ok = !ctx->h_info->part_overflow && !(fused_more && C == 0 && !fbits);
             if (!fused_ok) fused_more = false, C = 0;
             if (fused_ok) {
                 for (int i = 0; i < 256; ++i) N += h_cur[i] & 0x7fffffffu;
@@ -514,9 +538,9 @@ restart:
         }  // exact pipeline
         for (i64 w0 = 0; w0 < C || fused_more;) {
             const size_t f0 = tm.mark();
-            if (fused_ok && w0 > 0) {
+            if (fused_ok && (w0 > 0 || C == 0)) {
                 // ---- next pass of the bucket join: the buckets not marked done, into a fresh window ----
-                CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 0, 0, info, st, &S.n_launches));
+                CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 0, 0, 0, info, st, &S.n_launches));
                 rc = read_info(ctx, info, st);
                 if (rc) return rc;
                 if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
@@ -901,6 +925,7 @@ int symdel_set_option(symdel_ctx* ctx, int option, int64_t value) {
             if (value > 2) return SYMDEL_E_ARG;
             ctx->opt_cand_filter = value;
             break;
+        case SYMDEL_OPT_NO_QUERY_FILTER: ctx->opt_no_query_filter = value != 0; break;
         case SYMDEL_OPT_SORT_VARIANT:
             if (value >= sd_sort_variants()) return SYMDEL_E_ARG;
             ctx->opt_sort_variant = value;

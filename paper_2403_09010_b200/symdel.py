@@ -19,7 +19,7 @@ OK = 0
 E_ARG, E_OFFSETS, E_TOO_LONG, E_RESIDUE, E_TOO_MANY, E_WORKSPACE, E_CAPACITY, E_CUDA, E_INTERNAL = range(-1, -10, -1)
 OPT_TIMING, OPT_FORCE_CHUNKS, OPT_CAND_CAPACITY, OPT_HASH_BITS, OPT_NO_THINNING, OPT_SORT_VARIANT, OPT_GENERAL_GENERATE = 1, 2, 3, 4, 5, 6, 7
 OPT_SORT_BITS, OPT_SORT_STABLE, OPT_SORT_GROUPING, OPT_JOIN_GENERAL, OPT_EXACT_PIPELINE, OPT_PREFIX_LEN, OPT_METRIC = 8, 9, 10, 11, 12, 13, 14
-OPT_SURV_CAPACITY, OPT_CAND_FILTER = 15, 16
+OPT_SURV_CAPACITY, OPT_CAND_FILTER, OPT_NO_QUERY_FILTER = 15, 16, 17
 METRIC_LEVENSHTEIN, METRIC_HAMMING = 0, 1
 D_MAX, L_MAX = 4, 64
 
@@ -39,7 +39,7 @@ class Stats(C.Structure):
         ("ms_prepare", C.c_float), ("ms_generate", C.c_float), ("ms_sort", C.c_float), ("ms_emit", C.c_float),
         ("ms_dedup", C.c_float), ("ms_verify", C.c_float), ("ms_total", C.c_float), ("ms_sort_pass_avg", C.c_float),
         ("sort_pass_records", C.c_int64), ("fused_chunks", C.c_int64), ("join_redo_tiles", C.c_int64),
-        ("surv_merges", C.c_int64), ("join_windows", C.c_int64),
+        ("surv_merges", C.c_int64), ("join_windows", C.c_int64), ("query_filter_bits", C.c_int64),
     ]
 
     def as_dict(self):

@@ -538,6 +538,30 @@ def test_cross_small(sd, ctx, oracle, d):
     assert_same(run_cross(sd, ctx, q, r, d), oracle.bruteforce_cross(q.seqs, q.offsets, r.seqs, r.offsets, d))
 
 
+@pytest.mark.parametrize("nq,nr,d,opts", [(300, 5000, 2, {}), (2000, 60000, 2, {}), (2000, 60000, 1, {"FORCE_CHUNKS": 3}),
+                                          (1500, 40000, 3, {}), (2000, 60000, 2, {"CAND_CAPACITY": 3000}), (5000, 20000, 2, {})])
+def test_cross_query_filter(sd, oracle, nq, nr, d, opts):
+    """Cross-search with the queries the small side: the level-2 partition drops the reference records whose hash bits no
+    query record of their bin has (k_bin_bitmap / k_part2<true>).  Same result with the filter and without it."""
+    q, r = synth.cross_sets(nq, nr, 17)
+    exp = oracle.symdel_cross(q.seqs, q.offsets, r.seqs, r.offsets, d)
+    for off in (0, 1):
+        c = sd.Context(0)
+        c.symdel_set_option(sd.OPT_NO_QUERY_FILTER, off)
+        for k, v in opts.items():
+            c.symdel_set_option(getattr(sd, "OPT_" + k), v)
+        assert_same(run_cross(sd, c, q, r, d), exp)
+        st = c.symdel_get_stats()
+        assert st["fused_chunks"] == st["n_chunks"]
+        assert (st["query_filter_bits"] > 0) == (off == 0 and q.n * 4 <= r.n), st["query_filter_bits"]
+    # the other orientation (references the small side): no filter, same pairs mirrored
+    c = sd.Context(0)
+    i, j, dist = run_cross(sd, c, r, q, d)
+    assert c.symdel_get_stats()["query_filter_bits"] == 0
+    order = np.lexsort((i, j))
+    assert_same([j[order], i[order], dist[order]], exp)
+
+
 def test_cross_symmetry_and_self_relation(sd, ctx):
     a, b = synth.tcr_set(3000, 12), synth.tcr_set(4000, 11)
     ab = run_cross(sd, ctx, a, b, 2)
