@@ -52,7 +52,7 @@ cudaError_t sd_cand_filter(const u64* cand, i64 n, void* table, int table_bits, 
                            cudaStream_t st, i64* launches);
 
 // level-2 partition of the fused pipeline: bins (256 x cap1) -> buckets ((256 << b2) x cap2)
-#define SD_FBITS_MAX 18  // query filter: at most 2^18 bits (32 KB) per level-1 bin
+#define SD_FBITS_MAX 19  // query filter: at most 2^19 bits (64 KB) per level-1 bin (config 4 with 17 / 18 / 19 bits: 6.4 / 5.8 / 5.5 ms: fewer survivors beat more resident blocks)
 // bitmap != nullptr: the query filter of a cross-search (radix_sort.cu, k_bin_bitmap): 256 bitmaps of 2^fbits bits built by
 // sd_bin_bitmap from the first cnt_a[bin] records of every bin; fshift = position of the fbits hash bits below the bin digit
 cudaError_t sd_bin_bitmap(const u64* bins, const u32* cnt_a, i64 cap1, u32* bitmap, int fbits, int fshift, cudaStream_t st, i64* launches);

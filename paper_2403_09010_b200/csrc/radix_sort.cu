@@ -460,7 +460,7 @@ __global__ void __launch_bounds__(P2_THREADS, P2_MINB) k_part2(const Part2Params
 // bin's bitmap in shared memory, keeps what passes in a staging tile (one slice per warp), and partitions the staging tile
 // whenever the next input tile might not fit — most set-B records never reach the ranking, the scatter or HBM again.
 constexpr int P2F_TILES = 16, P2F_IPT = 8, P2F_IN = P2_THREADS * P2F_IPT;
-__global__ void __launch_bounds__(P2_THREADS, 3) k_part2f(const Part2Params P) {
+__global__ void __launch_bounds__(P2_THREADS, 2) k_part2f(const Part2Params P) {
     sd_dep_wait();
     sd_dep_release();
     extern __shared__ __align__(16) unsigned char smem_raw[];
