@@ -66,7 +66,8 @@ enum {
                                 count — exact, except when a chunked / windowed search had to cut its survivor list (stats.surv_merges > 0
                                 and the list exceeded `capacity`): then a lower bound of it, still > capacity */
     SYMDEL_E_CUDA = -8,      /* CUDA error (sticky); code via symdel_last_cuda_error */
-    SYMDEL_E_INTERNAL = -9   /* internal consistency check failed (never expected) */
+    SYMDEL_E_INTERNAL = -9,  /* internal consistency check failed (never expected) */
+    SYMDEL_E_STATIC_LIMIT = -10 /* symdel_sort_u64_static: n > SYMDEL_STATIC_SORT_MAX_KEYS (its built-in scratch cannot grow) */
 };
 
 typedef struct symdel_ctx symdel_ctx; /* opaque; owns small pinned scratch, stats and (host entry points only) a device arena */
@@ -195,6 +196,29 @@ SYMDEL_API int symdel_stage_lev(symdel_ctx* ctx, const int8_t* a_seqs, const int
                      const int8_t* b_seqs, const int64_t* b_offsets, int64_t n_b, const int32_t* ia,
                      const int32_t* ib, int64_t n_pairs, int32_t* dist, void* workspace, int64_t workspace_bytes,
                      void* cuda_stream);
+
+/* ---- a sort that allocates nothing and needs no workspace --------------------------------------------------------
+ * symdel_sort_u64_static = symdel_stage_sort_u64 (stable LSD radix sort of n 64-bit keys on bits [begin_bit, end_bit),
+ * end - begin a multiple of 8, result left in `keys`; the sort of the sort-merge join) for callers
+ * that cannot give the library any device memory beyond the data itself: plug-ins inside an application whose pool
+ * already owns the whole GPU (cudaMalloc fails there), service loops where cudaMalloc / cudaFree are banned because they
+ * can synchronise the device, error paths that run after an out-of-memory.  The caller passes only `keys` (device,
+ * n x uint64, read and overwritten).  The ping-pong buffer and the status words sit in a __device__ array inside
+ * libsymdel.so: SYMDEL_STATIC_SORT_SCRATCH_BYTES (11 MiB) of every GPU that loads the library, held until the process
+ * exits — hence the limit n <= SYMDEL_STATIC_SORT_MAX_KEYS (2^20); a larger n returns SYMDEL_E_STATIC_LIMIT and
+ * touches nothing.  The call needs no symdel_ctx (creating one allocates) and performs no cudaMalloc / cudaFree or
+ * any other allocating call; it selects `device` (cudaSetDevice), issues its work on `cuda_stream` (a cudaStream_t of
+ * that device, NULL = default stream) and returns after synchronising that stream, like every call of this header.
+ *   - First call on a device: looks up the array's device address and sets the sort kernels' shared-memory limit.
+ *     Make that call before any stream capture begins; later calls on the device skip the set-up.
+ *   - One array per GPU, shared by all calls and never reset between them: each call clears the words that must start
+ *     at zero on `cuda_stream` before its kernels.  Calls on the same device whose GPU work may overlap (other streams,
+ *     other host threads) race on the array — the result is undefined; serialise them.
+ * Errors: SYMDEL_E_ARG (bad bit range, n < 0, null keys, device outside 0..63), SYMDEL_E_STATIC_LIMIT, SYMDEL_E_CUDA
+ * (no such device or a CUDA call failed; cudaGetLastError has the code — there is no context to keep it). */
+#define SYMDEL_STATIC_SORT_MAX_KEYS 1048576
+#define SYMDEL_STATIC_SORT_SCRATCH_BYTES 11534336 /* 8 MiB ping-pong keys + 3 MiB histograms / tickets / status words */
+SYMDEL_API int symdel_sort_u64_static(int device, uint64_t* keys, int64_t n, int begin_bit, int end_bit, void* cuda_stream);
 
 #ifdef __cplusplus
 }

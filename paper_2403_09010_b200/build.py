@@ -8,7 +8,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 SO = HERE / "libsymdel.so"
-SOURCES = ["symdel_api.cu", "generate.cu", "radix_sort.cu", "join.cu", "verify.cu"]
+SOURCES = ["symdel_api.cu", "generate.cu", "radix_sort.cu", "join.cu", "verify.cu", "static_sort.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
               "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
 

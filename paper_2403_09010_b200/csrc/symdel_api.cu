@@ -955,6 +955,7 @@ const char* symdel_strerror(int code) {
         case SYMDEL_E_CAPACITY: return "more result pairs than the output capacity";
         case SYMDEL_E_CUDA: return "CUDA error";
         case SYMDEL_E_INTERNAL: return "internal consistency check failed";
+        case SYMDEL_E_STATIC_LIMIT: return "more keys than the built-in scratch of symdel_sort_u64_static holds (SYMDEL_STATIC_SORT_MAX_KEYS)";
         default: return "unknown error";
     }
 }

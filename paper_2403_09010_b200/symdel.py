@@ -17,6 +17,8 @@ _lib = None
 
 OK = 0
 E_ARG, E_OFFSETS, E_TOO_LONG, E_RESIDUE, E_TOO_MANY, E_WORKSPACE, E_CAPACITY, E_CUDA, E_INTERNAL = range(-1, -10, -1)
+E_STATIC_LIMIT = -10
+STATIC_SORT_MAX_KEYS, STATIC_SORT_SCRATCH_BYTES = 1 << 20, 11 << 20
 OPT_TIMING, OPT_FORCE_CHUNKS, OPT_CAND_CAPACITY, OPT_HASH_BITS, OPT_NO_THINNING, OPT_SORT_VARIANT, OPT_GENERAL_GENERATE = 1, 2, 3, 4, 5, 6, 7
 OPT_SORT_BITS, OPT_SORT_STABLE, OPT_SORT_GROUPING, OPT_JOIN_GENERAL, OPT_EXACT_PIPELINE, OPT_PREFIX_LEN, OPT_METRIC = 8, 9, 10, 11, 12, 13, 14
 OPT_SURV_CAPACITY, OPT_CAND_FILTER, OPT_NO_QUERY_FILTER = 15, 16, 17
@@ -27,7 +29,7 @@ EXPORTS = [
     "symdel_create", "symdel_destroy", "symdel_set_option", "symdel_get_stats", "symdel_last_cuda_error",
     "symdel_strerror", "symdel_workspace_bytes", "symdel_self", "symdel_cross", "symdel_self_host",
     "symdel_cross_host", "symdel_stage_sort_workspace_bytes", "symdel_stage_sort_u64", "symdel_stage_generate",
-    "symdel_stage_lev", "symdel_overlap_matrix",
+    "symdel_stage_lev", "symdel_overlap_matrix", "symdel_sort_u64_static",
 ]
 
 
@@ -81,6 +83,7 @@ def lib():
         L.symdel_stage_generate.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, i64, C.POINTER(i64), vp, i64, vp]
         L.symdel_stage_lev.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp]
         L.symdel_overlap_matrix.argtypes = [vp, vp, vp, i64, vp, i64, vp, i64, i32, i32, vp, vp, i64, vp]
+        L.symdel_sort_u64_static.argtypes = [i32, vp, i64, i32, i32, vp]
         _lib = L
     return _lib
 
@@ -91,6 +94,22 @@ def symdel_workspace_bytes(n_a, residues_a, n_b=0, residues_b=0, max_len=L_MAX, 
     if rc:
         raise SymdelError(rc, "symdel_workspace_bytes")
     return int(out.value)
+
+
+def symdel_sort_u64_static(keys, begin_bit: int, end_bit: int):
+    """symdel_sort_u64_static: the stable radix sort of `Context.symdel_stage_sort_u64`, in place on a uint64-as-int64
+    CUDA tensor of at most STATIC_SORT_MAX_KEYS keys, for code that may not allocate device memory (a host application
+    that owns the whole GPU, a loop where cudaMalloc's device-wide synchronisation is not acceptable).  No Context, no
+    workspace and no temporary tensor: the scratch is an 11 MiB array built into libsymdel.so, one per GPU, shared by
+    every call — calls on one device must not overlap, and the first call on a device (it does a one-time address
+    look-up) belongs before any stream capture.  More keys than the limit raise SymdelError(E_STATIC_LIMIT)."""
+    torch = _torch()
+    dev = keys.device.index if keys.device.index is not None else torch.cuda.current_device()
+    with torch.cuda.device(dev):
+        rc = lib().symdel_sort_u64_static(dev, C.c_void_p(keys.data_ptr()), keys.numel(), begin_bit, end_bit, _stream_ptr(torch))
+    if rc:
+        raise SymdelError(rc, "symdel_sort_u64_static")
+    return keys
 
 
 def _torch():
