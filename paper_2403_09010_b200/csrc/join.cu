@@ -607,8 +607,19 @@ constexpr int JF_LMAX_L = JF_T + 4096, JF_SLOTB_L = 12, JF_MINB_L = JF_IT > 8 ? 
 // counts is resident warps, hence as little shared memory per block as the region needs: 16 KB of heads + the
 // stage, sized at launch (config 3: 34 KB, six blocks of 256 threads per SM; with five blocks +12 %, with four
 // +35 %).  Two instances: regions of up to 4064 records (NB = 12) and up to 18432 (1024 threads, NB = 15: chunks
-// of more than ~2 * 10^8 records).  If the claims run past the
-// candidate window info->join_fallback is raised (the host then uses the exact pipeline).
+// of more than ~2 * 10^8 records).
+// Cross-search instance (CROSS): only the QUERY records are chained by atomic exchange (sweep 1a); every reference
+// record then reads the head of its slot with a plain load and keeps it as its link (sweep 1b), so the walks run from
+// reference records through query records only.
+// Windowed searches (the pairs of a chunk exceed one candidate window).  A block claims its output range with ONE
+// atomicAdd on info->n_cand, so the claims are totally ordered.  A claim that ends beyond the window (win_hi) writes
+// nothing, marks its bucket open (JB_OPEN, bit 31 of the bucket's count), raises info->join_fallback and publishes its
+// base through info->nofit_inv = max(~base): every claim after the first that does not fit starts beyond the window
+// too, hence the pairs written are exactly [0, min base that did not fit) — the host takes that as the window's end
+// and launches further passes (first_round = 0) that join only the open buckets, each into a fresh window; a bucket
+// that fits clears its mark.  A bucket fuller than the launched instance stages (stage_cap) is left open the same way
+// for a pass of the large instance.  Only a single bucket whose pairs exceed a whole window (a pass that writes
+// nothing while buckets stay open) sends the chunk to the exact pipeline.
 constexpr u32 JB_OPEN = 0x80000000u;
 struct JoinBktParams {
     JoinParams j;       // rec = bucket regions; topmask unused
