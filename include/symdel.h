@@ -111,7 +111,7 @@ enum {
     SYMDEL_OPT_EXACT_PIPELINE = 12, /* [0] 1: never use the fused pipeline (fixed-capacity bins); always count, scan, generate, onesweep-partition on exact histograms, windowed join (the path the fused one falls back to when a bin overflows; results are identical) */
     SYMDEL_OPT_PREFIX_LEN = 13,   /* [0] P > 0: prefix-truncated candidate generation (App. B; XTNeighbor uses 18): deletion variants are generated from the first P residues of every sequence, verification stays on the whole sequences.  Exact for P > d (calls with P <= d return SYMDEL_E_ARG); fewer records, more candidates */
     SYMDEL_OPT_METRIC = 14,       /* [0] 0: Levenshtein distance (the paper's metric).  1: Hamming distance (Fig. S3 A/C): only pairs of EQUAL length with <= d mismatching positions are returned, dist = the mismatch count; candidates come from the same deletion-variant join (hamming <= d implies lev <= d) */
-    SYMDEL_OPT_SURV_CAPACITY = 15, /* [0] >0: size of the survivor list of multi-flush searches in pairs (test hook; never below capacity + one candidate window) */
+    SYMDEL_OPT_SURV_CAPACITY = 15, /* [0] >0: size of the survivor list of multi-flush searches in pairs (test hook; never below capacity + 4096: a candidate window whose survivors do not fit behind the list is verified in slices, the list being sorted, deduplicated and cut to its smallest `capacity` pairs in between) */
     SYMDEL_OPT_CAND_FILTER = 16, /* [0] duplicate suppression before the candidate sort (a best-effort hash set of pair ids): 0 = automatic (on when the candidates are many but few per record), 1 = always, 2 = never (test hook; results are identical) */
     SYMDEL_OPT_NO_QUERY_FILTER = 17, /* [0] 1: cross-search never drops reference records through the query filter (test hook: same result) */
     SYMDEL_OPT_SORT_GROUPING = 10 /* [0] 1: symdel_stage_sort_u64 sorts keys only: ties land in arbitrary order (the mode the pipeline uses) */

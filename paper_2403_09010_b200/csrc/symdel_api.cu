@@ -481,6 +481,7 @@ restart:
         CK(join_side());
         rc = read_info(ctx, info, st);
         if (rc) return rc;
+        if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);  // (k_pack's residue check is in by now: no generation, no re-chunking on bad input)
         N = (i64)ctx->h_info->n_records;
         if (N > ncap || N >= ((i64)1 << 30)) {
             if (ctx->opt_force_chunks > 0 && N <= ncap) return SYMDEL_E_TOO_MANY;
@@ -630,18 +631,42 @@ restart:
                     if ((rc = merge_survivors())) return rc;
                     merged = true;
                 }
+                // v0 / vn: the slice [v0, v0 + vn) of the sorted window that the next sd_verify takes (the whole window
+                // unless an overflow forces slices); vtotal: candidates in the window once it is known on the host
+                i64 v0 = 0, vn = nc, vtotal = nc;
+                const u64* vdev = nc_dev;
+                bool sliced = false;
                 for (;;) {
                     CK(cudaMemsetAsync(&info->surv_overflow, 0, sizeof(u32), st));
-                    CK(sd_verify(csorted, nc, nc_dev, slots, lay, maxlen, survA, (u64)n_surv, (u64)scap, verify_lb, info, st,
+                    CK(sd_verify(csorted + v0, vn, vdev, slots, lay, maxlen, survA, (u64)n_surv, (u64)scap, verify_lb, info, st,
                                  &S.n_launches));
                     rc = read_info(ctx, info, st);
                     if (rc) return rc;
-                    if (!ctx->h_info->surv_overflow) break;
-                    // the window's survivors did not fit behind the list: merge it (once) and verify the window again
-                    if (merged || n_surv == 0) return SYMDEL_E_WORKSPACE;  // not even `capacity` + this window's survivors fit
-                    if ((rc = merge_survivors())) return rc;
-                    merged = true;
+                    if (!ctx->h_info->surv_overflow) {
+                        v0 += vn;
+                        if (!sliced || v0 >= vtotal) break;
+                        // next slice: cut the list back to <= `capacity` entries first, so that the slice fits whatever it yields
+                        n_surv = (i64)ctx->h_info->n_surv;
+                        if (n_surv > 0 && (rc = merge_survivors())) return rc;
+                        vn = std::min<i64>(vtotal - v0, scap - n_surv);
+                        continue;
+                    }
+                    // the survivors did not fit behind the list (nothing was lost, n_surv stands): merge the list once ...
+                    if (!merged && n_surv > 0) {
+                        if ((rc = merge_survivors())) return rc;
+                        merged = true;
+                        continue;
+                    }
+                    // ... and if the list is as short as it gets (<= `capacity` entries of scap >= capacity + 4096) and the window
+                    // still yields more than the room behind it, verify the window in slices of at most that room: a candidate
+                    // gives at most one survivor, so a slice always fits.  The merges between slices keep the smallest `capacity`
+                    // pairs and the count of distinct pairs seen (surv_lower_bound), which is what SYMDEL_E_CAPACITY reports.
+                    if (vdev) vtotal = (i64)ctx->h_info->n_filt, vdev = nullptr;
+                    if (scap - n_surv <= 0) return SYMDEL_E_INTERNAL;
+                    vn = std::min<i64>(vtotal - v0, scap - n_surv);
+                    sliced = true;
                 }
+                if (sliced) ++flushes;  // (a repeated pair may straddle two slices: the final pass has to sort and deduplicate)
             }
             rc = read_info(ctx, info, st);
             if (rc) return rc;

@@ -876,6 +876,40 @@ def test_capacity_error_in_multi_flush_searches(sd, oracle, opts):
             assert np.array_equal(o.cpu().numpy(), x[:capacity])  # the first `capacity` pairs, ascending
 
 
+@pytest.mark.parametrize("opts", [{"FORCE_CHUNKS": 2}, {"CAND_CAPACITY": 150000}, {"FORCE_CHUNKS": 3, "CAND_FILTER": 1},
+                                  {"EXACT_PIPELINE": 1, "FORCE_CHUNKS": 2}])
+def test_survivor_list_smaller_than_one_flush(sd, oracle, opts):
+    """A flush that yields far more survivors than the room behind the survivor list (capacity + 4096 entries with
+    SYMDEL_OPT_SURV_CAPACITY = 1; the dense set gives tens of thousands per flush): the window is verified in slices
+    with merges in between — SYMDEL_E_CAPACITY with the first `capacity` pairs and a lower bound of the count when the
+    result is larger than `capacity`, the exact result when it fits; never SYMDEL_E_WORKSPACE."""
+    import torch
+
+    s = synth.dense_set(12000, 51, fanout=64)
+    exp = oracle.symdel_self(s.seqs, s.offsets, 2)
+    n_exp = len(exp[0])
+    assert n_exp > 100_000
+    ds, do = sd.to_device(s)
+    for capacity in (1000, n_exp // 3, n_exp):
+        c = sd.Context(0)
+        for k, v in opts.items():
+            c.symdel_set_option(getattr(sd, "OPT_" + k), v)
+        c.symdel_set_option(sd.OPT_SURV_CAPACITY, 1)
+        out = tuple(torch.full((capacity,), -1, dtype=torch.int32, device="cuda") for _ in range(3))
+        if capacity >= n_exp:
+            assert_same([t.cpu().numpy() for t in c.symdel_self(ds, do, 2, out=out)], exp)
+        else:
+            with pytest.raises(sd.SymdelError) as e:
+                c.symdel_self(ds, do, 2, out=out)
+            assert e.value.code == sd.E_CAPACITY
+            assert capacity < c.last_required <= n_exp
+            for o, x in zip(out, exp):
+                assert np.array_equal(o.cpu().numpy(), x[:capacity])
+        st = c.symdel_get_stats()
+        assert st["n_flushes"] >= 2 and st["surv_merges"] >= 1
+        c.close()
+
+
 def test_out_of_range_indices_are_rejected(torch, sd, ctx):
     """Caller-supplied indices never steer a read out of bounds: symdel_stage_lev and symdel_overlap_matrix."""
     s = synth.tcr_set(300, 5)
