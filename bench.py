@@ -109,6 +109,30 @@ def job_value(pairs_per_replica: int, world: int, ms: float) -> float:
     return world * pairs_per_replica / (ms * 1e-3)
 
 
+def host_info():
+    """CPU model, logical cores and the threads the oracle uses (it is single-threaded C++): SURVEY.md section 8(d)."""
+    model = None
+    try:
+        for ln in Path("/proc/cpuinfo").read_text().splitlines():
+            if ln.lower().startswith("model name"):
+                model = ln.split(":", 1)[1].strip()
+                break
+    except Exception:
+        pass
+    return {"cpu_model": model, "nproc": os.cpu_count(), "threads": 1}
+
+
+def oracle_record(gold, live=None):
+    """The oracle's time on one workload: `live` = (pairs, seconds) measured in this run, else the wall time recorded
+    when the golden file was written (another host, said so)."""
+    if live:
+        return {"value": live[0] / live[1], "unit": UNIT, "seconds": live[1], "where": "this run, this host", **host_info()}
+    if gold and gold.get("oracle_wall_s"):
+        return {"value": gold["n_out"] / gold["oracle_wall_s"], "unit": UNIT, "seconds": gold["oracle_wall_s"],
+                "where": "recorded by tests/golden/make_golden.py when the golden file was written (another host)", "threads": 1}
+    return None
+
+
 def cpu_baseline_run(n_sample: int, d: int, s):
     """The oracle as it stands on a bounded sample: the workload's generator and seed at n_sample
     sequences (a prefix of the 1M set would hold seeds only, i.e. no neighbours)."""
@@ -137,7 +161,7 @@ def golden(name):
     return json.loads(p.read_text()) if p.exists() else None
 
 
-def run_workload(torch, symdel, dev, name, kind, d, sets, gold, opts=None, ws_frac=None, steps=5, cap=1 << 21):
+def run_workload(torch, symdel, dev, name, kind, d, sets, gold, opts=None, ws_frac=None, steps=5, cap=1 << 21, oracle_live=False):
     """One of the other workloads (configs 1, 2, 4, 5, dense, forced pipelines): `steps` device-resident steps after one
     warm-up, CUDA events, result checked against the oracle's golden digest.  Not part of the headline's timed region."""
     ctx = symdel.Context(dev.index)
@@ -164,11 +188,34 @@ def run_workload(torch, symdel, dev, name, kind, d, sets, gold, opts=None, ws_fr
             ms.append(e0.elapsed_time(e1))
     st = ctx.symdel_get_stats()
     i, j, dist = [t.cpu().numpy() for t in r]
-    row = {"workload": name, "ms": float(np.mean(ms)), "pairs": int(len(i)), "records": st["n_records"],
+    # per-stage CUDA-event times: two more steps with the library's stage timers on (not part of `ms`)
+    ctx.symdel_set_option(symdel.OPT_TIMING, 1)
+    tst = []
+    for _ in range(2):
+        call(*args, d, workspace=ws, out=out)
+        tst.append(ctx.symdel_get_stats())
+    ctx.symdel_set_option(symdel.OPT_TIMING, 0)
+    stage_keys = ("ms_prepare", "ms_generate", "ms_sort", "ms_emit", "ms_dedup", "ms_verify", "ms_total")
+    stage_ms = {k: float(np.mean([x[k] for x in tst])) for k in stage_keys}
+    extra = {}
+    if st["fused_chunks"] == 0 and tst[-1]["ms_sort_pass_avg"] > 0:  # exact pipeline: the onesweep passes over the records
+        pass_ms = float(np.mean([x["ms_sort_pass_avg"] for x in tst]))
+        extra = {"onesweep_pass_ms": pass_ms, "onesweep_passes": st["sort_bits"] // 8, "onesweep_pass_records": st["sort_pass_records"],
+                 "onesweep_pass_gbs": 16 * st["sort_pass_records"] / (pass_ms * 1e-3) / 1e9}
+    row = {"workload": name, "ms": float(np.mean(ms)), "ms_min": float(np.min(ms)), "ms_median": float(np.median(ms)),
+           "stage_ms": stage_ms, **extra, "pairs": int(len(i)), "records": st["n_records"],
            "candidates": st["n_candidates"], "chunks": st["n_chunks"], "flushes": st["n_flushes"],
            "pipeline": "fused" if st["fused_chunks"] == st["n_chunks"] else "exact" if st["fused_chunks"] == 0 else "mixed",
            "workspace_bytes": int(ws.numel()), "steps": steps,
            "verified": bool(gold and digest(i, j, dist) == gold["out_sha256"]) if gold else None}
+    if oracle_live:  # the oracle on the same workload, timed here (only where it finishes in well under a minute)
+        from oracle import oracle
+
+        t0 = time.time()
+        oi = oracle.symdel_self(sets[0].seqs, sets[0].offsets, d)[0]
+        row["oracle"] = oracle_record(gold, (len(oi), time.time() - t0))
+    else:
+        row["oracle"] = oracle_record(gold)
     ctx.close()
     del ws, out, devs, args
     torch.cuda.empty_cache()
@@ -187,7 +234,7 @@ def other_workloads(torch, symdel, synth, dev):
 
     for num in (1, 2, 5):
         kind, d, sets = synth.config(num)
-        add(f"config {num}", kind, d, sets, golden(f"config_{num}.json"))
+        add(f"config {num}", kind, d, sets, golden(f"config_{num}.json"), oracle_live=num in (1, 2))
     kind, d, sets = synth.config(5)
     add("config 5, workspace = 10 % of the un-chunked need (key-range chunking, S5)", kind, d, sets, golden("config_5.json"),
         ws_frac=0.1)
@@ -231,7 +278,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "int64", "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, **host_info()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
@@ -362,7 +409,10 @@ def main():
     if gold and not verified:
         raise SystemExit(f"bench: output digest differs from tests/golden/{gold_name} (device {dig_dev[:12]}, host {dig_host[:12]})")
 
-    ms, e2e_ms = max_over_ranks([float(np.mean(ms_steps)), e2e_ms], dist, dev)
+    e2e_all = [x[0] for x in e2e]
+    ms, e2e_ms, ms_min, ms_med, e2e_min, e2e_med = max_over_ranks(
+        [float(np.mean(ms_steps)), e2e_ms, float(np.min(ms_steps)), float(np.median(ms_steps)), float(np.min(e2e_all)),
+         float(np.median(e2e_all))], dist, dev)
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -405,7 +455,8 @@ def main():
     top = max(stages[:3], key=lambda r: r["ms"])
     line = {
         "metric": METRIC, "value": job_value(n_out, world, ms), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "warmup": args.warmup, "ms_per_step": ms, "ms_per_step_min": ms_min, "ms_per_step_median": ms_med,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u64", "data": "synthetic",
         "config": {"workload": ("NEXT-2 dense: synth.dense_set(1e6, seed 11, fanout 64), d=2" if args.dense else
                                 WORKLOAD if args.config == 3 else f"config {args.config}"), "n": s.n, "d": d,
@@ -419,7 +470,8 @@ def main():
         "wall_time_s": ms * 1e-3, "records_per_s": world * n_rec / (ms * 1e-3),
         "step_hbm_gbs": step_bytes / (ms * 1e-3) / 1e9, "step_hbm_frac": step_bytes / (ms * 1e-3) / 1e9 / peak,
         "stage_ms": stage, "stages": stages,
-        "e2e": {"value": job_value(n_out, world, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms,
+        "e2e": {"value": job_value(n_out, world, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms, "ms_per_step_min": e2e_min,
+                "ms_per_step_median": e2e_med,
                 "h2d_bytes_per_step": int(s.seqs.nbytes + s.offsets.nbytes), "d2h_bytes_per_step": int(12 * n_out),
                 "api": "symdel_self_host (pinned host buffers)"},
         "gpu_launches": launches_timed,
@@ -433,10 +485,29 @@ def main():
                      "share_of_step": top["share_of_step"], "frac_of_nominal_8000": top["achieved_gbs"] / 8000.0},
         "clocks": clocks,
     }
+    # What limits the longest kernel: the HBM figure above is what the contract asks for; k_gen2_part itself is
+    # bound by instruction issue (DESIGN.md section 6 ablations), k_part2 is the HBM-bound kernel.  Issue roofline: warp
+    # instructions per launch (ncu --set full, profiles/traffic.json) / launch time against 148 SMs x 4 schedulers x SM clock.
+    winst = load_traffic(top["kernel"] + "_warp_instructions")
+    sm_mhz = (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0
+    if winst and top["ms"] > 0:
+        issue_peak = 148 * 4 * sm_mhz * 1e6 / 1e9  # G warp-instructions/s
+        issue = winst / (top["ms"] * 1e-3) / 1e9
+        line["roofline"]["limiter"] = ("hbm" if top["frac_of_peak"] >= 0.5 else "issue" if issue / issue_peak >= 0.45 else
+                                       "latency (shared-memory wavefronts / resident warps)")
+        line["roofline_issue"] = {"bound": "alu", "kernel": top["kernel"], "achieved": issue, "peak": issue_peak,
+                                  "unit": "G warp-instructions/s", "frac": issue / issue_peak,
+                                  "warp_instructions_per_launch": winst, "sm_mhz": sm_mhz,
+                                  "peak_source": "148 SMs x 4 warp schedulers x SM clock (one warp instruction per scheduler per cycle)",
+                                  "source": "instruction count from the committed ncu --set full capture (profiles/traffic.json)"}
+    hbm_stage = max(stages[:3], key=lambda r: r["frac_of_peak"])
+    line["roofline_hbm_bound_kernel"] = {"bound": "hbm", "kernel": hbm_stage["kernel"], "achieved": hbm_stage["achieved_gbs"], "peak": peak,
+                                         "unit": "GB/s", "frac": hbm_stage["frac_of_peak"], "traffic": hbm_stage["traffic"],
+                                         "launch_ms": hbm_stage["ms"], "share_of_step": hbm_stage["share_of_step"]}
     if not args.no_cpu_baseline and world == 1 and not args.dense:
         n_sample = min(s.n, args.ref_sample or 150000)
         pairs, dt = cpu_baseline_run(n_sample, d, s)
-        line["cpu_baseline"] = {"value": pairs / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+        line["cpu_baseline"] = {"value": pairs / dt, "unit": UNIT, "cores": 1, "kind": "oracle", **host_info(),
                                 "sample": f"same generator and seed at n={n_sample}, d={d}: {pairs} pairs in {dt:.1f} s "
                                           "(oracle_symdel_self, App. F.1 hash map)"}
         if gold and gold.get("oracle_wall_s"):

@@ -118,7 +118,7 @@ enum {
 };
 
 /* ---- context ------------------------------------------------------------------------------- */
-SYMDEL_API int symdel_create(symdel_ctx** ctx, int device);  /* selects `device`; SYMDEL_E_CUDA if none */
+SYMDEL_API int symdel_create(symdel_ctx** ctx, int device);  /* selects `device`; SYMDEL_E_CUDA if there is none or it is not a B200 (compute capability 10.0, 148 SMs, 227 KB shared memory per block: the kernels are built and sized for exactly that) */
 SYMDEL_API void symdel_destroy(symdel_ctx* ctx);
 SYMDEL_API int symdel_set_option(symdel_ctx* ctx, int option, int64_t value);
 SYMDEL_API int symdel_get_stats(const symdel_ctx* ctx, symdel_stats* stats_host);

@@ -877,6 +877,15 @@ int symdel_create(symdel_ctx** out, int device) {
     *out = nullptr;
     int count = 0;
     if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return SYMDEL_E_CUDA;
+    // The library is built for sm_100a only and its launch helpers size grids, warp tasks and shared-memory carve-outs for
+    // the B200 (148 SMs, 227 KB of shared memory per block): any other device is refused here rather than mis-tuned.
+    int cc_major = 0, cc_minor = 0, sms = 0, smem_optin = 0;
+    if (cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&cc_minor, cudaDevAttrComputeCapabilityMinor, device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device) != cudaSuccess)
+        return SYMDEL_E_CUDA;
+    if (cc_major != 10 || cc_minor != 0 || sms != 148 || smem_optin < 232448) return SYMDEL_E_CUDA;
     symdel_ctx* ctx = new symdel_ctx();
     ctx->device = device;
     cudaError_t e = cudaSetDevice(device);
