@@ -655,9 +655,10 @@ __device__ __forceinline__ void jb_mbar_wait(u64* bar, u32 parity) {
             : "memory");
     }
 }
-__device__ __forceinline__ u32 jb_atoms_exch(u32* p, u32 v) {
+// (the address is a shared-window offset computed once per block: a generic pointer would cost a cvta per exchange)
+__device__ __forceinline__ u32 jb_atoms_exch(u32 saddr, u32 v) {
     u32 old;
-    asm volatile("atom.shared.exch.b32 %0, [%1], %2;" : "=r"(old) : "r"(jb_smem(p)), "r"(v) : "memory");
+    asm volatile("atom.shared.exch.b32 %0, [%1], %2;" : "=r"(old) : "r"(saddr), "r"(v) : "memory");
     return old;
 }
 
@@ -718,22 +719,25 @@ __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams 
     jb_mbar_wait(&S.mbar, 0);
     // ---- 1. sweep ----
     const int slot_shift = P.slot_shift;
-    unsigned short* const link16 = reinterpret_cast<unsigned short*>(S.stage) + 3;  // bits 48..63 of record i: link16[4 * i]
+    // The link goes into the top NB bits of the record and the PAIR of records is written back by one 16-byte store
+    // (4 wavefronts per warp; two 2-byte stores at a 16-byte lane stride were 4-way bank conflicts: 8 wavefronts).
+    const u32 head_s = jb_smem(S.head);
     u32 flag = 0;  // bit 2k + e: my record 2 * (tid + k * THREADS) + e found an earlier record in its slot
     if (!CROSS) {
 #pragma unroll
         for (int k = 0; k < IT; ++k) {
             const u32 i = 2 * (tid + k * THREADS);
             if (i < n) {
-                const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(S.stage + i);
-                const u32 o0 = jb_atoms_exch(&S.head[(u32)(t.x >> slot_shift) & (SLOTS - 1)], i);
-                link16[4 * i] = (unsigned short)((o0 << (16 - NB)) | ((u32)(t.x >> 48) & ((1u << (16 - NB)) - 1u)));
+                ulonglong2 t = *reinterpret_cast<const ulonglong2*>(S.stage + i);
+                const u32 o0 = jb_atoms_exch(head_s + 4u * ((u32)(t.x >> slot_shift) & (SLOTS - 1)), i);
+                t.x = (t.x & KEEP) | ((u64)o0 << (64 - NB));
                 flag |= (o0 != NIL ? 1u : 0u) << (2 * k);
                 if (i + 1 < n) {
-                    const u32 o1 = jb_atoms_exch(&S.head[(u32)(t.y >> slot_shift) & (SLOTS - 1)], i + 1);
-                    link16[4 * i + 4] = (unsigned short)((o1 << (16 - NB)) | ((u32)(t.y >> 48) & ((1u << (16 - NB)) - 1u)));
+                    const u32 o1 = jb_atoms_exch(head_s + 4u * ((u32)(t.y >> slot_shift) & (SLOTS - 1)), i + 1);
+                    t.y = (t.y & KEEP) | ((u64)o1 << (64 - NB));
                     flag |= (o1 != NIL ? 2u : 0u) << (2 * k);
                 }
+                *reinterpret_cast<ulonglong2*>(S.stage + i) = t;
             }
         }
     } else {
@@ -746,15 +750,17 @@ __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams 
         for (int k = 0; k < IT; ++k) {
             const u32 i = 2 * (tid + k * THREADS);
             if (i < n) {
-                const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(S.stage + i);
-                if ((t.x & idm) < na) {
-                    const u32 o0 = jb_atoms_exch(&S.head[(u32)(t.x >> slot_shift) & (SLOTS - 1)], i);
-                    link16[4 * i] = (unsigned short)((o0 << (16 - NB)) | ((u32)(t.x >> 48) & ((1u << (16 - NB)) - 1u)));
+                ulonglong2 t = *reinterpret_cast<const ulonglong2*>(S.stage + i);
+                const bool q0 = (t.x & idm) < na, q1 = i + 1 < n && (t.y & idm) < na;
+                if (q0) {
+                    const u32 o0 = jb_atoms_exch(head_s + 4u * ((u32)(t.x >> slot_shift) & (SLOTS - 1)), i);
+                    t.x = (t.x & KEEP) | ((u64)o0 << (64 - NB));
                 }
-                if (i + 1 < n && (t.y & idm) < na) {
-                    const u32 o1 = jb_atoms_exch(&S.head[(u32)(t.y >> slot_shift) & (SLOTS - 1)], i + 1);
-                    link16[4 * i + 4] = (unsigned short)((o1 << (16 - NB)) | ((u32)(t.y >> 48) & ((1u << (16 - NB)) - 1u)));
+                if (q1) {
+                    const u32 o1 = jb_atoms_exch(head_s + 4u * ((u32)(t.y >> slot_shift) & (SLOTS - 1)), i + 1);
+                    t.y = (t.y & KEEP) | ((u64)o1 << (64 - NB));
                 }
+                if (q0 || q1) *reinterpret_cast<ulonglong2*>(S.stage + i) = t;  // (queries are the small side: most pairs hold none)
             }
         }
         __syncthreads();
@@ -762,17 +768,18 @@ __global__ void __launch_bounds__(THREADS, MINB) k_join_bkt(const JoinBktParams 
         for (int k = 0; k < IT; ++k) {
             const u32 i = 2 * (tid + k * THREADS);
             if (i < n) {
-                const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(S.stage + i);  // (a query record's link bits are not looked at here)
+                ulonglong2 t = *reinterpret_cast<const ulonglong2*>(S.stage + i);  // (a query record keeps the link sweep 1a gave it: only `idm` bits are looked at)
                 if ((t.x & idm) >= na) {
                     const u32 o0 = S.head[(u32)(t.x >> slot_shift) & (SLOTS - 1)];
-                    link16[4 * i] = (unsigned short)((o0 << (16 - NB)) | ((u32)(t.x >> 48) & ((1u << (16 - NB)) - 1u)));
+                    t.x = (t.x & KEEP) | ((u64)o0 << (64 - NB));
                     flag |= (o0 != NIL ? 1u : 0u) << (2 * k);
                 }
                 if (i + 1 < n && (t.y & idm) >= na) {
                     const u32 o1 = S.head[(u32)(t.y >> slot_shift) & (SLOTS - 1)];
-                    link16[4 * i + 4] = (unsigned short)((o1 << (16 - NB)) | ((u32)(t.y >> 48) & ((1u << (16 - NB)) - 1u)));
+                    t.y = (t.y & KEEP) | ((u64)o1 << (64 - NB));
                     flag |= (o1 != NIL ? 2u : 0u) << (2 * k);
                 }
+                *reinterpret_cast<ulonglong2*>(S.stage + i) = t;
             }
         }
     }
