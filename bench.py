@@ -161,7 +161,8 @@ def golden(name):
     return json.loads(p.read_text()) if p.exists() else None
 
 
-def run_workload(torch, symdel, dev, name, kind, d, sets, gold, opts=None, ws_frac=None, steps=5, cap=1 << 21, oracle_live=False):
+def run_workload(torch, symdel, dev, name, kind, d, sets, gold, opts=None, ws_frac=None, steps=5, cap=1 << 21, oracle_live=False,
+                 e2e_host=False):
     """One of the other workloads (configs 1, 2, 4, 5, dense, forced pipelines): `steps` device-resident steps after one
     warm-up, CUDA events, result checked against the oracle's golden digest.  Not part of the headline's timed region."""
     ctx = symdel.Context(dev.index)
@@ -208,6 +209,22 @@ def run_workload(torch, symdel, dev, name, kind, d, sets, gold, opts=None, ws_fr
            "pipeline": "fused" if st["fused_chunks"] == st["n_chunks"] else "exact" if st["fused_chunks"] == 0 else "mixed",
            "workspace_bytes": int(ws.numel()), "steps": steps,
            "verified": bool(gold and digest(i, j, dist) == gold["out_sha256"]) if gold else None}
+    if kind == "cross" and e2e_host:
+        # the same search through symdel_cross_host: pinned host buffers, H2D of both sets and D2H of the result inside the call
+        hb = [torch.from_numpy(a).pin_memory() for a in (sets[0].seqs, sets[0].offsets, sets[1].seqs, sets[1].offsets)]
+        ho = tuple(torch.empty(cap, dtype=torch.int32).pin_memory() for _ in range(3))
+        tms, k = [], 0
+        for it in range(steps + 1):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            k = ctx.symdel_cross_host(*hb, d, ho)
+            if it:
+                tms.append(1e3 * (time.perf_counter() - t0))
+        ok = bool(gold and digest(*[o[:k].numpy() for o in ho]) == gold["out_sha256"]) if gold else None
+        row["e2e"] = {"api": "symdel_cross_host (pinned host buffers)", "ms": float(np.mean(tms)), "ms_min": float(np.min(tms)),
+                      "ms_median": float(np.median(tms)), "h2d_bytes_per_step": int(sum(t.numel() * t.element_size() for t in hb)),
+                      "d2h_bytes_per_step": int(12 * k), "verified": ok}
+        del hb, ho
     if oracle_live:  # the oracle on the same workload, timed here (only where it finishes in well under a minute)
         from oracle import oracle
 
@@ -246,8 +263,13 @@ def other_workloads(torch, symdel, synth, dev):
     add("config 3, prefix P = 12 (NEXT-1)", kind, d, sets, golden("config_3.json"), opts={"PREFIX_LEN": 12})
     sets = (synth.dense_set(1_000_000, 11, fanout=64),)
     add("NEXT-2 dense: synth.dense_set(1e6, seed 11, fanout 64), d=2", "self", 2, sets, golden("dense_1m.json"), cap=32 << 20)
+    # beyond 2^30 records: the planner must split by itself; no oracle golden exists at this size
+    # (hours of hash map) — tests/test_gpu_parity.py::test_more_than_2_30_records pins the result another way
+    sets = (synth.bcr_set(400_000, 77, lo=26, hi=30, mean=28.0, sd=1.0),)
+    add("1.3 x 2^30 records: synth.bcr_set(400k, seed 77, L 26..30), d=3, no option (planner splits)", "self", 3, sets, None,
+        steps=3, cap=1 << 23)
     kind, d, sets = synth.config(4)
-    add("config 4 (cross 100k x 5M)", kind, d, sets, golden("config_4.json"), cap=1 << 22)
+    add("config 4 (cross 100k x 5M)", kind, d, sets, golden("config_4.json"), cap=1 << 22, e2e_host=True)
     return rows
 
 

@@ -715,6 +715,26 @@ def test_config4_full_size(sd, ctx, oracle):
         assert np.array_equal(j[m], rr) and np.array_equal(dist[m], dd)
 
 
+@pytest.mark.parametrize("pinned", [True, False])
+def test_config4_full_size_host_entry(torch, sd, pinned):
+    """symdel_cross_host at the size where the copies matter most (the two-set form of PAPER.md:43 through HOST buffers:
+    98 MB of residues and offsets in, the result out, inside the call): same golden digest as the device entry point,
+    from pinned and from pageable memory, two calls in a row on one context (arena reuse)."""
+    g = _golden("config_4.json")
+    kind, d, (q, r) = synth.config(4)
+    assert q.sha256() + r.sha256() == g["input_sha256"]
+    c = sd.Context(0)
+    cap = 1 << 20
+    mk = (lambda a: torch.from_numpy(a).pin_memory()) if pinned else (lambda a: a)
+    hq, hqo, hr, hro = mk(q.seqs), mk(q.offsets), mk(r.seqs), mk(r.offsets)
+    out = tuple((torch.empty(cap, dtype=torch.int32).pin_memory() if pinned else np.empty(cap, np.int32)) for _ in range(3))
+    for rep in range(2):
+        k = c.symdel_cross_host(hq, hqo, hr, hro, d, out)
+        i, j, dist = [(o[:k].numpy() if pinned else o[:k]) for o in out]
+        assert_matches_golden(g, i, j, dist)
+    c.close()
+
+
 # ---- S5 at full size: key-range chunking under a memory budget (BASELINE.json config 5; PAPER.md:270-274) ------
 @pytest.mark.parametrize("num,opts,ws_frac", [
     (5, {"FORCE_CHUNKS": 4}, None), (5, {"FORCE_CHUNKS": 16}, None), (5, {}, 0.1), (5, {"EXACT_PIPELINE": 1}, 0.07),
@@ -908,6 +928,43 @@ def test_survivor_list_smaller_than_one_flush(sd, oracle, opts):
         st = c.symdel_get_stats()
         assert st["n_flushes"] >= 2 and st["surv_merges"] >= 1
         c.close()
+
+
+def test_more_than_2_30_records(torch, sd, oracle):
+    """The regime the key-range chunking exists for (1.2 B deletion variants at 10 M sequences and
+    d = 2, 577 M at 1 M and d = 3): 400,000 BCR-like sequences of 26..30 residues at d = 3 hold about 1.4 x 2^30
+    deletion sets, more than one chunk may carry (record counts and bin cursors are 30-bit).  With NO option set the
+    planner has to split the search by itself (n_chunks >= 2).  The oracle's hash map would need hours here, so the
+    result is pinned in two other ways: it equals, element by element, the result of the same search forced into 8
+    chunks (a path the full-size goldens of configs 3 and 5 do pin), and 32 sampled rows are complete and correct
+    against the oracle's brute-force row (every neighbour of a sequence over the whole set)."""
+    from math import comb
+
+    d = 3
+    s = synth.bcr_set(400_000, 77, lo=26, hi=30, mean=28.0, sd=1.0)
+    nmax = sum(int(c) * sum(comb(L, k) for k in range(d + 1)) for L, c in enumerate(np.bincount(s.lengths)))
+    assert nmax > (1 << 30) + (1 << 28)
+    ds, do = sd.to_device(s)
+    cap = 1 << 23
+    nbytes = sd.symdel_workspace_bytes(s.n, s.seqs.size, 0, 0, int(s.lengths.max()), d, cap)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    out = tuple(torch.empty(cap, dtype=torch.int32, device="cuda") for _ in range(3))
+    c = sd.Context(0)
+    got = [t.cpu().numpy() for t in c.symdel_self(ds, do, d, workspace=ws, out=out)]
+    st = c.symdel_get_stats()
+    assert st["n_chunks"] >= 2 and st["n_records"] >= (1 << 30), st
+    c.close()
+    c = sd.Context(0)
+    c.symdel_set_option(sd.OPT_FORCE_CHUNKS, 8)
+    ref = [t.cpu().numpy() for t in c.symdel_self(ds, do, d, workspace=ws, out=out)]
+    st8 = c.symdel_get_stats()
+    assert st8["n_chunks"] == 8 and st8["n_records"] == st["n_records"]
+    c.close()
+    assert len(got[0]) > 100_000
+    assert_same(got, ref)
+    i, j, dist = got
+    assert np.all(i < j) and np.all(np.diff(i.astype(np.int64) * s.n + j) > 0)  # ascending (i, j), each pair once
+    _check_sampled_rows(oracle, s, d, i, j, dist, 32, 5)
 
 
 def test_out_of_range_indices_are_rejected(torch, sd, ctx):
