@@ -189,6 +189,19 @@ SYMDEL_API int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const 
                           int id_bits, int thinning, uint64_t* records, int64_t records_capacity,
                           int64_t* n_records_host, void* workspace, int64_t workspace_bytes, void* cuda_stream);
 
+/* S1+S2 fused (the generator of the default pipeline: k_gen2_part for d <= 3 and sequences of <= 32 residues, else
+ *   k_generate_part; SYMDEL_OPT_GENERAL_GENERATE forces the latter): the same records as symdel_stage_generate, but
+ *   pushed straight into 256 bins by the top 8 bits of their hash field — bins[b * bin_capacity + t], t < bin_counts[b]
+ *   (device u32[256], overwritten), in no particular order inside a bin.  bin_capacity: a multiple of 32, < 2^30.
+ *   n_chunks > 1 selects the key-range-chunk instance (S5): only records whose position (variant length << 32 | hash
+ *   fraction) lies in [chunk_lo, chunk_hi) are made; n_chunks == 1 ignores the two bounds.  *n_records_host = records
+ *   pushed.  SYMDEL_E_CAPACITY: some bin was full (records beyond bin_capacity were dropped; the pipeline then falls back to
+ *   its exact form).  workspace: >= 4096 device bytes.  n must be < 2^id_bits and hash_bits >= 8. */
+SYMDEL_API int symdel_stage_generate_fused(symdel_ctx* ctx, const int8_t* seqs, const int64_t* offsets, int64_t n, int d,
+                                int hash_bits, int id_bits, int thinning, int n_chunks, uint64_t chunk_lo, uint64_t chunk_hi,
+                                uint64_t* bins, int64_t bin_capacity, uint32_t* bin_counts, int64_t* n_records_host,
+                                void* workspace, int64_t workspace_bytes, void* cuda_stream);
+
 /* S4/K6: dist[t] = lev(a_{ia[t]}, b_{ib[t]}) by the bit-parallel verifier, for n_pairs index pairs.
  *   workspace: device scratch of at least 512 + 48 * (n_a + n_b) bytes (the packed bit-plane table).
  *   An index outside [0, n_a) / [0, n_b) gives dist[t] = -1 and the call returns SYMDEL_E_ARG. */

@@ -1127,6 +1127,61 @@ int symdel_stage_generate(symdel_ctx* ctx, const int8_t* seqs, const int64_t* of
     return SYMDEL_OK;
 }
 
+int symdel_stage_generate_fused(symdel_ctx* ctx, const int8_t* seqs, const int64_t* offsets, int64_t n, int d, int hash_bits, int id_bits,
+                                int thinning, int n_chunks, uint64_t chunk_lo, uint64_t chunk_hi, uint64_t* bins, int64_t bin_capacity,
+                                uint32_t* bin_counts, int64_t* n_records_host, void* workspace, int64_t workspace_bytes,
+                                void* cuda_stream) {
+    if (!ctx || !n_records_host || n < 0 || d < 0 || d > SD_D_MAX || hash_bits < 8 || hash_bits + id_bits > 64 || id_bits < 1 ||
+        n_chunks < 1 || bin_capacity < 32 || bin_capacity % 32 != 0 || bin_capacity >= ((i64)1 << 30) || n >= ((i64)1 << id_bits))
+        return SYMDEL_E_ARG;
+    *n_records_host = 0;
+    if (!bins || !bin_counts || !workspace) return SYMDEL_E_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CK(cudaSetDevice(ctx->device));
+    CK(cudaMemsetAsync(bin_counts, 0, 256 * sizeof(u32), st));
+    if (n == 0) {
+        CK(cudaStreamSynchronize(st));
+        return SYMDEL_OK;
+    }
+    if (!seqs || !offsets) return SYMDEL_E_ARG;
+    Bump ws(workspace, workspace_bytes);
+    DevInfo* info = ws.take<DevInfo>(1);
+    if (!ws.ok) return SYMDEL_E_WORKSPACE;
+    SeqSetDev A{seqs, offsets, n}, B{nullptr, nullptr, 0};
+    CK(cudaMemsetAsync(info, 0, sizeof(DevInfo), st));
+    CK(sd_prepare(A, d, 0, 0, info, st, nullptr));
+    CK(sd_check_residues(A, info, st));
+    int rc = read_info(ctx, info, st);
+    if (rc) return rc;
+    if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+    Layout lay{};
+    lay.n_a = n;
+    lay.d = d;
+    lay.id_bits = id_bits;
+    lay.b_bits = id_bits;
+    lay.pair_bits = 2 * id_bits;
+    lay.hash_bits = hash_bits;
+    lay.sort_bits = 8;
+    lay.thinning = thinning;
+    lay.force_general = ctx->opt_general_gen ? 1 : 0;
+    lay.n_chunks = (u32)n_chunks;
+    lay.chunk_lo = n_chunks > 1 ? chunk_lo : 0ull;
+    lay.chunk_hi = n_chunks > 1 ? chunk_hi : ~0ull;
+    const int width = (int)ctx->h_info->maxlen + 1;
+    if (!sd_gen_part_applies(lay, width)) return SYMDEL_E_ARG;
+    const double rpr = (double)ctx->h_info->nmax / (double)std::max<i64>((i64)ctx->h_info->residues, 1) / (double)n_chunks;
+    CK(sd_gen_part(A, B, lay, width, bins, bin_counts, (u64)bin_capacity, rpr, (double)ctx->h_info->residues / (double)n, 0, -1, 1, info, st, nullptr));
+    u32* h_cur = reinterpret_cast<u32*>(ctx->h_info + 1);
+    CK(cudaMemcpyAsync(h_cur, bin_counts, 256 * sizeof(u32), cudaMemcpyDeviceToHost, st));
+    rc = read_info(ctx, info, st);
+    if (rc) return rc;
+    if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
+    i64 total = 0;
+    for (int i = 0; i < 256; ++i) total += h_cur[i];
+    *n_records_host = total;
+    return ctx->h_info->part_overflow ? SYMDEL_E_CAPACITY : SYMDEL_OK;
+}
+
 int symdel_stage_lev(symdel_ctx* ctx, const int8_t* a_seqs, const int64_t* a_offsets, int64_t n_a, const int8_t* b_seqs,
                      const int64_t* b_offsets, int64_t n_b, const int32_t* ia, const int32_t* ib, int64_t n_pairs,
                      int32_t* dist, void* workspace, int64_t workspace_bytes, void* cuda_stream) {

@@ -30,6 +30,7 @@ EXPORTS = [
     "symdel_strerror", "symdel_workspace_bytes", "symdel_self", "symdel_cross", "symdel_self_host",
     "symdel_cross_host", "symdel_stage_sort_workspace_bytes", "symdel_stage_sort_u64", "symdel_stage_generate",
     "symdel_stage_lev", "symdel_overlap_matrix", "symdel_sort_u64_static",
+    "symdel_stage_generate_fused",
 ]
 
 
@@ -81,6 +82,8 @@ def lib():
         L.symdel_stage_sort_workspace_bytes.restype = i64
         L.symdel_stage_sort_u64.argtypes = [vp, vp, vp, i64, i32, i32, vp, i64, vp]
         L.symdel_stage_generate.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, i64, C.POINTER(i64), vp, i64, vp]
+        L.symdel_stage_generate_fused.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, i32, C.c_uint64, C.c_uint64, vp, i64, vp,
+                                                  C.POINTER(i64), vp, i64, vp]
         L.symdel_stage_lev.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, i64, vp]
         L.symdel_overlap_matrix.argtypes = [vp, vp, vp, i64, vp, i64, vp, i64, i32, i32, vp, vp, i64, vp]
         L.symdel_sort_u64_static.argtypes = [i32, vp, i64, i32, i32, vp]
@@ -246,6 +249,25 @@ class Context:
         if rc:
             self._raise(rc, "symdel_stage_generate")
         return rec[: int(cnt.value)]
+
+    def symdel_stage_generate_fused(self, seqs, offsets, d: int, hash_bits: int, id_bits: int, thinning: bool, bin_capacity: int,
+                                    n_chunks: int = 1, chunk_lo: int = 0, chunk_hi: int = 0):
+        """Returns (bins int64[256, bin_capacity], counts int32[256]) of the fused generator (CUDA tensors)."""
+        torch = _torch()
+        n = offsets.numel() - 1
+        bins = torch.zeros((256, bin_capacity), dtype=torch.int64, device=offsets.device)
+        counts = torch.zeros(256, dtype=torch.int32, device=offsets.device)
+        ws = torch.empty(1 << 16, dtype=torch.uint8, device=offsets.device)
+        cnt = C.c_int64(0)
+        rc = lib().symdel_stage_generate_fused(self._h, C.c_void_p(seqs.data_ptr()), C.c_void_p(offsets.data_ptr()), n, d, hash_bits,
+                                               id_bits, int(thinning), n_chunks, chunk_lo, chunk_hi, C.c_void_p(bins.data_ptr()),
+                                               bin_capacity, C.c_void_p(counts.data_ptr()), C.byref(cnt),
+                                               C.c_void_p(ws.data_ptr()), ws.numel(), _stream_ptr(torch))
+        if rc:
+            self.last_required = int(cnt.value)
+            self._raise(rc, "symdel_stage_generate_fused")
+        assert int(counts.sum()) == int(cnt.value)
+        return bins, counts
 
     def symdel_stage_lev(self, a_seqs, a_offsets, b_seqs, b_offsets, ia, ib):
         torch = _torch()

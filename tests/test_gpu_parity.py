@@ -224,6 +224,82 @@ def test_generate_groups_match_oracle_variants(torch, sd, ctx, oracle, d, thinni
     assert sorted(map(tuple, got_groups.values())) == sorted(map(tuple, (sorted(g) for g in exp_groups.values())))
 
 
+def _fused_records(ctx, ds, do, d, hash_bits, id_bits, thinning, cap, **kw):
+    """Records of the fused generator, bin by bin; checks that every record sits in the bin of its top 8 hash bits."""
+    bins, counts = ctx.symdel_stage_generate_fused(ds, do, d, hash_bits, id_bits, thinning, cap, **kw)
+    bins, counts = bins.cpu().numpy().view(np.uint64), counts.cpu().numpy()
+    assert counts.max(initial=0) <= cap
+    rec = np.concatenate([bins[b, :counts[b]] for b in range(256)])
+    where = np.repeat(np.arange(256, dtype=np.uint64), counts)
+    assert np.array_equal((rec >> np.uint64(id_bits + hash_bits - 8)) & np.uint64(255), where)
+    return rec
+
+
+@pytest.mark.parametrize("d", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("thinning", [True, False])
+@pytest.mark.parametrize("mode", ["plain", "narrow", "general"])
+def test_fused_generate_bins_match_oracle_variants(torch, sd, oracle, d, thinning, mode):
+    """Kernel-level pin of the generators of the DEFAULT pipeline (k_gen2_part for d <= 3, k_generate_part for d = 4 or
+    on request): the records they push into the level-1 bins, gathered, form the same multiset of id-groups per key as
+    the oracle's deletion-variant strings (App. F.1 step 1) — the comparison of
+    test_generate_groups_match_oracle_variants, on the fused kernels — and every record lies in the bin of its digit."""
+    s = synth.repeat_heavy_set(70, 3, alphabet=3, lo=0, hi=9 if d < 4 else 8)
+    ds, do = sd.to_device(s)
+    id_bits, hash_bits = (8, 56) if mode == "plain" else (8, 48)
+    c = sd.Context(0)
+    if mode == "general":
+        c.symdel_set_option(sd.OPT_GENERAL_GENERATE, 1)
+    rec = _fused_records(c, ds, do, d, hash_bits, id_bits, thinning, 4096)
+    c.close()
+    ids = (rec & np.uint64(255)).astype(np.int64)
+    keys = rec >> np.uint64(id_bits)
+    var = [oracle.deletion_variants(s.seq(i), d) for i in range(s.n)]
+    exp_cnt = np.array([len(set(v)) if thinning else len(v) for v in var])
+    assert np.array_equal(np.bincount(ids, minlength=s.n), exp_cnt)
+    got_groups = {}
+    for k, i in zip(keys.tolist(), ids.tolist()):
+        got_groups.setdefault(k, []).append(i)
+    exp_groups = {}
+    for i, v in enumerate(var):
+        for x in (set(v) if thinning else v):
+            exp_groups.setdefault(x, []).append(i)
+    assert sorted(tuple(sorted(g)) for g in got_groups.values()) == sorted(tuple(sorted(g)) for g in exp_groups.values())
+
+
+@pytest.mark.parametrize("family,d,general", [("tcr", 1, 0), ("tcr", 2, 0), ("tcr", 2, 1), ("bcr", 3, 0), ("bcr", 3, 1), ("bcr", 4, 0),
+                                              ("long", 2, 0)])
+def test_fused_generate_equals_exact_generate_and_chunks_partition_it(torch, sd, family, d, general):
+    """Many blocks, rounds and flushes: the fused generators make exactly the records of the exact generator (which the
+    oracle pins above), and the key-range-chunk instances (S5) split that set: the chunks are disjoint and their union
+    is the whole — for a cut inside a variant length (hash fraction) and for cuts at length boundaries."""
+    if family == "tcr":
+        s = synth.tcr_set(20000, 5)
+    elif family == "bcr":
+        s = synth.bcr_set(2500 if d == 3 else 600, 6, n_lineages=300)
+    else:  # longer than 32 residues: the 64-residue rows of the general kernel
+        rng = np.random.default_rng(8)
+        lens = rng.integers(20, 45, size=3000).astype(np.int32)
+        rows = rng.integers(1, 21, size=(3000, 44)).astype(np.int8)
+        rows[np.arange(44)[None, :] >= lens[:, None]] = 0
+        s = synth.from_padded(rows, lens)
+    ds, do = sd.to_device(s)
+    id_bits, hash_bits = 16, 48
+    c = sd.Context(0)
+    if general:
+        c.symdel_set_option(sd.OPT_GENERAL_GENERATE, 1)
+    exact = np.sort(c.symdel_stage_generate(ds, do, d, hash_bits, id_bits, True, 1 << 26).cpu().numpy().view(np.uint64))
+    cap = ((len(exact) // 256 * 3) // 2 + 4096) // 32 * 32
+    whole = np.sort(_fused_records(c, ds, do, d, hash_bits, id_bits, True, cap))
+    assert np.array_equal(whole, exact)
+    vl = int(np.median(s.lengths)) - 1
+    cuts = [0, (vl - 1) << 32, (vl << 32) | 0x5555_5555, (vl + 1) << 32, (1 << 64) - 1]
+    parts = [_fused_records(c, ds, do, d, hash_bits, id_bits, True, cap, n_chunks=4, chunk_lo=lo, chunk_hi=hi)
+             for lo, hi in zip(cuts[:-1], cuts[1:])]
+    c.close()
+    assert all(len(p) for p in parts)
+    assert np.array_equal(np.sort(np.concatenate(parts)), exact)  # disjoint (equal multisets) and complete
+
+
 # ---- full path: small / structured inputs -------------------------------------------------------------
 def test_hand_worked_cases(sd, ctx, oracle):
     s = synth.from_strings(["ACDEF", "ACDF", "ACGEF", "AB", "BA", "", "A", "ACCD", "ACD", "AAAA", "AAA", "CDEFA", "B"])
