@@ -114,6 +114,7 @@ enum {
     SYMDEL_OPT_SURV_CAPACITY = 15, /* [0] >0: size of the survivor list of multi-flush searches in pairs (test hook; never below capacity + 4096: a candidate window whose survivors do not fit behind the list is verified in slices, the list being sorted, deduplicated and cut to its smallest `capacity` pairs in between) */
     SYMDEL_OPT_CAND_FILTER = 16, /* [0] duplicate suppression before the candidate sort (a best-effort hash set of pair ids): 0 = automatic (on when the candidates are many but few per record), 1 = always, 2 = never (test hook; results are identical) */
     SYMDEL_OPT_NO_QUERY_FILTER = 17, /* [0] 1: cross-search never drops reference records through the query filter (test hook: same result) */
+    SYMDEL_OPT_FLUSH_PER_CHUNK = 18, /* [0] 1: a chunked search deduplicates and verifies its candidates after EVERY key-range chunk instead of letting the chunks append to one candidate window that is flushed when it fills or after the last chunk (test hook; results are identical) */
     SYMDEL_OPT_SORT_GROUPING = 10 /* [0] 1: symdel_stage_sort_u64 sorts keys only: ties land in arbitrary order (the mode the pipeline uses) */
 };
 

@@ -978,10 +978,12 @@ int sd_join_bkt_max_cap() { return JB_STAGE_L; }
 int sd_join_bkt_link_bits(u32 cap) { return cap <= (u32)JB_STAGE_S ? JB_NB_S : JB_NB_L; }
 
 cudaError_t sd_join_bkt(const u64* buckets, u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
-                        int first_pass, int info_fresh, int prefer_small, DevInfo* info, cudaStream_t st, i64* launches) {
+                        int first_pass, int info_fresh, int prefer_small, int append, DevInfo* info, cudaStream_t st, i64* launches) {
     cudaError_t e = cudaSuccess;
     // (info_fresh: the whole status block was cleared for this call and nothing has counted pairs or raised a join flag yet)
-    if (!info_fresh && (e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
+    // append: info->n_cand keeps its value — the window already holds that many pairs of earlier chunks (S5: one flush per
+    // full window, not per chunk) and the claims of this launch continue behind them
+    if (!info_fresh && !append && (e = cudaMemsetAsync(&info->n_cand, 0, sizeof(u64), st)) != cudaSuccess) return e;
     static_assert(offsetof(DevInfo, nofit_inv) == offsetof(DevInfo, join_fallback) + 8, "cleared together");
     if (!info_fresh && (e = cudaMemsetAsync(&info->join_fallback, 0, 2 * sizeof(u32) + sizeof(u64), st)) != cudaSuccess) return e;  // and join_redo, nofit_inv
     if (nbuckets == 0) return cudaSuccess;

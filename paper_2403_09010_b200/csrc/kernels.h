@@ -118,7 +118,8 @@ cudaError_t sd_join_fast_redo(const u64* records, i64 n_records, const Layout& l
 int sd_join_bkt_max_cap();
 int sd_join_bkt_link_bits(u32 cap);  // bits on top of a record that must be constant within a bucket
 cudaError_t sd_join_bkt(const u64* buckets, u32* cnt, u32 cap, u32 nbuckets, const Layout& lay, u64* cand, u64 window,
-                        int first_pass, int info_fresh, int prefer_small, DevInfo* info, cudaStream_t st, i64* launches);
+                        int first_pass, int info_fresh, int prefer_small, int append, DevInfo* info, cudaStream_t st, i64* launches);
+// (append = 1: info->n_cand is NOT cleared — the window already holds that many pairs and this launch claims behind them)
 
 // ---- verify.cu ----------------------------------------------------------------------------------
 i64 sd_verify_tiles(i64 n);

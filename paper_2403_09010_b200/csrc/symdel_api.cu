@@ -35,7 +35,7 @@ struct symdel_ctx {
     symdel_stats stats{};
     int opt_timing = 0;
     i64 opt_force_chunks = 0, opt_cand_cap = 0, opt_hash_bits = 0, opt_no_thinning = 0, opt_general_gen = 0;
-    i64 opt_sort_variant = 0, opt_surv_cap = 0, opt_cand_filter = 0, opt_no_query_filter = 0;
+    i64 opt_sort_variant = 0, opt_surv_cap = 0, opt_cand_filter = 0, opt_no_query_filter = 0, opt_flush_per_chunk = 0;
     i64 opt_sort_bits = -1, opt_sort_stable = 0, opt_sort_grouping = 0, opt_join_general = 0, opt_exact = 0, opt_prefix = 0, opt_metric = 0;
     DevInfo* h_info = nullptr;  // pinned; followed by 256 u32 (the level-1 bin counts of the fused pipeline)
     void* arena = nullptr;      // device arena of the *_host entry points: outputs + workspace
@@ -359,6 +359,11 @@ int run_pipeline_body(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int 
 
     const int width = (prefix > 0 ? std::min(maxlen, prefix) : maxlen) + 1;  // generation works on the (truncated) sequences
     i64 n_surv = 0, flushes = 0, surv_lower_bound = 0;
+    // S5 as SURVEY.md section 8(a) words it: the chunks of the fused pipeline APPEND their candidates to one window, and the
+    // window is deduplicated and verified "when the candidate buffer fills, or after the last chunk" — not once per chunk.
+    // acc = candidates of earlier chunks waiting in candA[0, acc); acc_rec = the records they came from.
+    bool accumulate = !ctx->opt_flush_per_chunk;
+    i64 acc = 0, acc_rec = 0;
     bool direct = false;  // the single flush wrote the outputs itself
     enum { ST_GEN, ST_SORT, ST_EMIT, ST_DEDUP, ST_VERIFY };
     i64 pass_count = 0;
@@ -371,6 +376,7 @@ restart:
     flushes = 0;
     surv_lower_bound = 0;
     direct = false;
+    acc = acc_rec = 0;
     S.n_records = S.n_candidates = 0;
     lay.n_chunks = P;
     if (!info_fresh) CK(cudaMemsetAsync(&info->n_surv, 0, sizeof(u64) * 3, st));  // n_surv, n_out, n_unique
@@ -442,7 +448,7 @@ restart:
             f_bcnt = fp.b2 ? cnt2 : cur1;
             f_bcap = (u32)(fp.b2 ? fp.cap2 : fp.cap1), f_nb = (u32)fp.nbuckets;
             u32* h_cur = reinterpret_cast<u32*>(ctx->h_info + 1);
-            CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 1, fresh, fbits ? 1 : 0, info, st, &S.n_launches));
+            CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 1, fresh, fbits ? 1 : 0, acc > 0 ? 1 : 0, info, st, &S.n_launches));
             CK(join_side());
             CK(cudaMemcpyAsync(h_cur, cur1, 256 * sizeof(u32), cudaMemcpyDeviceToHost, st));  // (bit 31 of a count is the join's "open" mark)
             rc = read_info(ctx, info, st);
@@ -454,6 +460,10 @@ restart:
             // (nothing written and buckets left open: one bucket's pairs exceed a whole window — unless the small join instance was
             //  preferred and simply could not stage any bucket: then the next pass, with the large instance, decides)
             fused_ok = !ctx->h_info->part_overflow && !(fused_more && C == 0 && !fbits);
+            if (!fused_ok && acc > 0) {  // (a full bin with candidates of earlier chunks still pending: start over, one flush per chunk)
+                accumulate = false;
+                goto restart;
+            }
             if (!fused_ok) fused_more = false, C = 0;
             if (fused_ok) {
                 for (int i = 0; i < 256; ++i) N += h_cur[i] & 0x7fffffffu;
@@ -466,8 +476,14 @@ restart:
                 S.sort_pass_records = N;
                 S.sort_bits = fp.b;
                 S.n_records += N;
-                S.n_candidates += C;
+                S.n_candidates += C - acc;  // (C counts the pending candidates of earlier chunks too)
                 ++S.fused_chunks;
+                // every pair of this chunk is in the window and there is room for about as many again: the flush waits
+                if (accumulate && !fused_more && c + 1 < P && C + 2 * (C - acc) <= ccap) {
+                    acc = C;
+                    acc_rec += N;
+                    continue;
+                }
             }
         }
         u64* sorted = nullptr;
@@ -541,7 +557,7 @@ restart:
             const size_t f0 = tm.mark();
             if (fused_ok && (w0 > 0 || C == 0)) {
                 // ---- next pass of the bucket join: the buckets not marked done, into a fresh window ----
-                CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 0, 0, 0, info, st, &S.n_launches));
+                CK(sd_join_bkt(f_bkt, f_bcnt, f_bcap, f_nb, lay, candA, (u64)ccap, 0, 0, 0, 0, info, st, &S.n_launches));
                 rc = read_info(ctx, info, st);
                 if (rc) return rc;
                 if (ctx->h_info->err) return err_from_flags(ctx->h_info->err);
@@ -577,7 +593,7 @@ restart:
             // The filter pays when the sort is throughput-bound and the distinct pairs (the table lines it touches) stay
             // cache-resident: config 5 (16.8 M candidates, 0.9 M distinct) 0.77 -> 0.42 ms; config 3 (3.7 M) 0.24 -> 0.21 ms;
             // dense 1 M (74 M candidates, 24 M distinct): the table misses L2, 3.8 -> 5.0 ms.
-            const bool use_filter = ctx->opt_cand_filter == 1 || (ctx->opt_cand_filter == 0 && nc >= ((i64)1 << 20) && nc < N / 4);
+            const bool use_filter = ctx->opt_cand_filter == 1 || (ctx->opt_cand_filter == 0 && nc >= ((i64)1 << 20) && nc < (N + acc_rec) / 4);
             if (use_filter) {
                 // duplicate suppression before the sort: a best-effort hash set in a record buffer that is free now
                 // (fused: the level-1 bins; exact: the ping-pong buffer that does not hold the partitioned records)
@@ -602,7 +618,7 @@ restart:
             const size_t f2 = tm.mark();
             // ---- S4: unique + verify; survivors appended at n_surv — or, when this window holds every candidate of
             //      the only chunk, unpacked straight into the outputs (no survivor list, no finalize) ----
-            direct = P == 1 && w0 == 0 && wend == C && !fused_more && flushes == 0;
+            direct = c + 1 == P && w0 == 0 && wend == C && !fused_more && flushes == 0;  // (earlier chunks, if any, are all in this window)
             if (direct)
                 CK(sd_verify_direct(csorted, nc, nc_dev, slots, lay, maxlen, out_i, out_j, out_dist, capacity, verify_lb, info, st,
                                     &S.n_launches));
@@ -677,9 +693,11 @@ restart:
             tm.span(ST_DEDUP, f1, f2);
             tm.span(ST_VERIFY, f2, f3);
             ++flushes;
+            acc = acc_rec = 0;
             w0 = wend;
         }
     }
+    if (acc > 0) return SYMDEL_E_INTERNAL;  // (the last chunk always flushes)
 
     // ---- final: (sort + unique) and unpack ----
     const size_t g0 = tm.mark();
@@ -960,6 +978,7 @@ int symdel_set_option(symdel_ctx* ctx, int option, int64_t value) {
             ctx->opt_cand_filter = value;
             break;
         case SYMDEL_OPT_NO_QUERY_FILTER: ctx->opt_no_query_filter = value != 0; break;
+        case SYMDEL_OPT_FLUSH_PER_CHUNK: ctx->opt_flush_per_chunk = value != 0; break;
         case SYMDEL_OPT_SORT_VARIANT:
             if (value >= sd_sort_variants()) return SYMDEL_E_ARG;
             ctx->opt_sort_variant = value;

@@ -21,7 +21,7 @@ E_STATIC_LIMIT = -10
 STATIC_SORT_MAX_KEYS, STATIC_SORT_SCRATCH_BYTES = 1 << 20, 11 << 20
 OPT_TIMING, OPT_FORCE_CHUNKS, OPT_CAND_CAPACITY, OPT_HASH_BITS, OPT_NO_THINNING, OPT_SORT_VARIANT, OPT_GENERAL_GENERATE = 1, 2, 3, 4, 5, 6, 7
 OPT_SORT_BITS, OPT_SORT_STABLE, OPT_SORT_GROUPING, OPT_JOIN_GENERAL, OPT_EXACT_PIPELINE, OPT_PREFIX_LEN, OPT_METRIC = 8, 9, 10, 11, 12, 13, 14
-OPT_SURV_CAPACITY, OPT_CAND_FILTER, OPT_NO_QUERY_FILTER = 15, 16, 17
+OPT_SURV_CAPACITY, OPT_CAND_FILTER, OPT_NO_QUERY_FILTER, OPT_FLUSH_PER_CHUNK = 15, 16, 17, 18
 METRIC_LEVENSHTEIN, METRIC_HAMMING = 0, 1
 D_MAX, L_MAX = 4, 64
 

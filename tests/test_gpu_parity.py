@@ -385,6 +385,8 @@ def test_validation_protocol_5000(sd, ctx, oracle, family, d):
     {"EXACT_PIPELINE": 1}, {"EXACT_PIPELINE": 1, "FORCE_CHUNKS": 2},
     {"CAND_FILTER": 1}, {"CAND_FILTER": 2}, {"CAND_FILTER": 1, "FORCE_CHUNKS": 3, "CAND_CAPACITY": 2000},
     {"CAND_FILTER": 1, "EXACT_PIPELINE": 1, "CAND_CAPACITY": 5000}, {"CAND_FILTER": 1, "HASH_BITS": 16},
+    {"FORCE_CHUNKS": 4, "FLUSH_PER_CHUNK": 1}, {"FORCE_CHUNKS": 16, "FLUSH_PER_CHUNK": 1},
+    {"FORCE_CHUNKS": 3, "CAND_CAPACITY": 777, "FLUSH_PER_CHUNK": 1},
 ])
 def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
     """P-11: chunk count, candidate-buffer windows, key width and thinning change memory use and
@@ -401,9 +403,13 @@ def test_output_invariant_under_chunks_windows_and_key_width(sd, oracle, opts):
     st = c.symdel_get_stats()
     if "FORCE_CHUNKS" in opts:
         assert st["n_chunks"] == opts["FORCE_CHUNKS"]
+    if set(opts) == {"FORCE_CHUNKS"}:
+        assert st["n_flushes"] == 1  # S5: the chunks append to one candidate window, flushed after the last chunk
+    if set(opts) == {"FORCE_CHUNKS", "FLUSH_PER_CHUNK"}:
+        assert st["n_flushes"] == st["n_chunks"]
     if "CAND_CAPACITY" in opts:
         assert st["n_flushes"] > 1
-        if set(opts) <= {"CAND_CAPACITY", "FORCE_CHUNKS", "CAND_FILTER", "HASH_BITS"}:
+        if set(opts) <= {"CAND_CAPACITY", "FORCE_CHUNKS", "CAND_FILTER", "HASH_BITS", "FLUSH_PER_CHUNK"}:
             # the pairs exceed one window: the bucket join runs again over the buckets that did not fit (fused all the way)
             assert st["join_windows"] >= 1 and st["join_general"] == 0 and st["fused_chunks"] == st["n_chunks"]
         else:
@@ -815,6 +821,7 @@ def test_config4_full_size_host_entry(torch, sd, pinned):
 @pytest.mark.parametrize("num,opts,ws_frac", [
     (5, {"FORCE_CHUNKS": 4}, None), (5, {"FORCE_CHUNKS": 16}, None), (5, {}, 0.1), (5, {"EXACT_PIPELINE": 1}, 0.07),
     (3, {"FORCE_CHUNKS": 4}, None), (3, {"FORCE_CHUNKS": 16}, None), (3, {}, 0.1),
+    (5, {"FORCE_CHUNKS": 4, "FLUSH_PER_CHUNK": 1}, None), (3, {"FLUSH_PER_CHUNK": 1}, 0.1),
 ])
 def test_config_full_size_chunked(torch, sd, oracle, num, opts, ws_frac):
     """Config 5 "exercises chunked key-range streaming" (BASELINE.json) — on a 180 GB device only under a budget:
@@ -840,7 +847,10 @@ def test_config_full_size_chunked(torch, sd, oracle, num, opts, ws_frac):
         assert st["n_chunks"] >= 4, st["n_chunks"]
     if "EXACT_PIPELINE" not in opts:
         assert st["fused_chunks"] == st["n_chunks"]  # every chunk stays on the fused pipeline
-    assert st["n_flushes"] >= st["n_chunks"]
+    if "EXACT_PIPELINE" in opts or "FLUSH_PER_CHUNK" in opts:
+        assert st["n_flushes"] >= st["n_chunks"]
+    else:  # S5: dedup + verify when the candidate window fills or after the last chunk, not per chunk
+        assert st["n_flushes"] < st["n_chunks"], (st["n_flushes"], st["n_chunks"])
 
 
 @pytest.mark.parametrize("num,window", [(3, 1_000_000), (5, 3_000_000)])
@@ -939,8 +949,8 @@ def test_two_contexts_in_one_process(torch, sd, oracle):
             assert_same([t.cpu().numpy() for t in c.symdel_self(ds, do, 2)], exp)
 
 
-@pytest.mark.parametrize("opts", [{"FORCE_CHUNKS": 4}, {"CAND_CAPACITY": 3000}, {"FORCE_CHUNKS": 3, "CAND_CAPACITY": 2000},
-                                  {"EXACT_PIPELINE": 1, "FORCE_CHUNKS": 2}])
+@pytest.mark.parametrize("opts", [{"FORCE_CHUNKS": 4}, {"FORCE_CHUNKS": 4, "FLUSH_PER_CHUNK": 1}, {"CAND_CAPACITY": 3000},
+                                  {"FORCE_CHUNKS": 3, "CAND_CAPACITY": 2000}, {"EXACT_PIPELINE": 1, "FORCE_CHUNKS": 2}])
 def test_capacity_error_in_multi_flush_searches(sd, oracle, opts):
     """SYMDEL_E_CAPACITY on the chunked / windowed path (symdel.h): the first `capacity` pairs are valid and the
     required count is reported; a pair found in several chunks is appended once per flush, and the survivor list is
@@ -972,8 +982,9 @@ def test_capacity_error_in_multi_flush_searches(sd, oracle, opts):
             assert np.array_equal(o.cpu().numpy(), x[:capacity])  # the first `capacity` pairs, ascending
 
 
-@pytest.mark.parametrize("opts", [{"FORCE_CHUNKS": 2}, {"CAND_CAPACITY": 150000}, {"FORCE_CHUNKS": 3, "CAND_FILTER": 1},
-                                  {"EXACT_PIPELINE": 1, "FORCE_CHUNKS": 2}])
+@pytest.mark.parametrize("opts", [{"FORCE_CHUNKS": 2, "FLUSH_PER_CHUNK": 1}, {"CAND_CAPACITY": 150000},
+                                  {"FORCE_CHUNKS": 3, "CAND_FILTER": 1, "FLUSH_PER_CHUNK": 1}, {"EXACT_PIPELINE": 1, "FORCE_CHUNKS": 2},
+                                  {"FORCE_CHUNKS": 3, "CAND_CAPACITY": 400000}])
 def test_survivor_list_smaller_than_one_flush(sd, oracle, opts):
     """A flush that yields far more survivors than the room behind the survivor list (capacity + 4096 entries with
     SYMDEL_OPT_SURV_CAPACITY = 1; the dense set gives tens of thousands per flush): the window is verified in slices
