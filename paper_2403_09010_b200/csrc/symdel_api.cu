@@ -324,6 +324,11 @@ int run_pipeline_body(symdel_ctx* ctx, SeqSetDev A, SeqSetDev B, int cross, int 
     if (ctx->opt_surv_cap > 0) scap = std::max<i64>(scap_min, ctx->opt_surv_cap);
     i64 ncap = std::max<i64>(nmax, 1);
     u32 P = ctx->opt_force_chunks > 0 ? (u32)ctx->opt_force_chunks : 1;
+    // A chunk carries fewer than 2^30 records (30-bit cursors and counts): a larger search is split up front, into chunks
+    // expected to hold <= 3/4 * 2^30, so that the record buffers and the fused plan (bins, buckets) are sized for a chunk
+    // and not for the whole (sized for the whole, the buckets would outgrow the join's stage and every chunk would take
+    // the exact pipeline).
+    if (ctx->opt_force_chunks <= 0 && nmax >= ((i64)3 << 28)) P = (u32)((nmax + ((i64)3 << 28) - 1) / ((i64)3 << 28));
     if (P > 1) ncap = std::min<i64>(nmax, nmax / P + nmax / (4 * P) + 4096);
     if (rec_bytes(ncap, npass_max) + cand_bytes(ccap + cslack, ppass) + cand_bytes(scap, spass) > R) {
         if (ctx->opt_cand_cap <= 0) ccap = std::min<i64>(ccap, std::max<i64>(4096, R / 4 / 17 - cslack));
