@@ -103,10 +103,11 @@ enum {
     SYMDEL_OPT_CAND_CAPACITY = 3, /* [0] >0: cap the candidate buffer at this many pairs (test hook for multi-flush) */
     SYMDEL_OPT_HASH_BITS = 4,     /* [0] 0 = every bit the id leaves free; else 1..63: hash bits kept per record (test hook: a narrow hash makes colliding variants, the result is unchanged) */
     SYMDEL_OPT_NO_THINNING = 5,   /* [0] 1: emit one record per deletion SET instead of per distinct variant (test hook) */
-    SYMDEL_OPT_GENERAL_GENERATE = 7, /* [0] 1: use the general (any d, any length) generation kernel even where the d <= 2 fast path applies (test hook) */
     SYMDEL_OPT_SORT_VARIANT = 6,  /* [0] 0..3: tile shape of the onesweep kernel used by this context (test hook: other tile geometries; results are identical) */
+    SYMDEL_OPT_GENERAL_GENERATE = 7, /* [0] 1: use the general (any d, any length) generation kernel even where the d <= 2 fast path applies (test hook) */
     SYMDEL_OPT_SORT_BITS = 8,     /* [0] 0 = automatic; 8..56 (multiple of 8): top hash bits that S2 radix-partitions; 255 = none (one bucket: the join chunks it) */
     SYMDEL_OPT_SORT_STABLE = 9,   /* [0] 1: every S2 pass takes the stable (ties keep input order) tile path (test hook; results are identical) */
+    SYMDEL_OPT_SORT_GROUPING = 10,/* [0] 1: symdel_stage_sort_u64 sorts keys only: ties land in arbitrary order (the mode the pipeline uses) */
     SYMDEL_OPT_JOIN_GENERAL = 11, /* [0] 1: always run the general join kernel (windowed output, chunked buckets) instead of trying the fast one first (test hook; results are identical) */
     SYMDEL_OPT_EXACT_PIPELINE = 12, /* [0] 1: never use the fused pipeline (fixed-capacity bins); always count, scan, generate, onesweep-partition on exact histograms, windowed join (the path the fused one falls back to when a bin overflows; results are identical) */
     SYMDEL_OPT_PREFIX_LEN = 13,   /* [0] P > 0: prefix-truncated candidate generation (App. B; XTNeighbor uses 18): deletion variants are generated from the first P residues of every sequence, verification stays on the whole sequences.  Exact for P > d (calls with P <= d return SYMDEL_E_ARG); fewer records, more candidates */
@@ -114,8 +115,7 @@ enum {
     SYMDEL_OPT_SURV_CAPACITY = 15, /* [0] >0: size of the survivor list of multi-flush searches in pairs (test hook; never below capacity + 4096: a candidate window whose survivors do not fit behind the list is verified in slices, the list being sorted, deduplicated and cut to its smallest `capacity` pairs in between) */
     SYMDEL_OPT_CAND_FILTER = 16, /* [0] duplicate suppression before the candidate sort (a best-effort hash set of pair ids): 0 = automatic (on when the candidates are many but few per record), 1 = always, 2 = never (test hook; results are identical) */
     SYMDEL_OPT_NO_QUERY_FILTER = 17, /* [0] 1: cross-search never drops reference records through the query filter (test hook: same result) */
-    SYMDEL_OPT_FLUSH_PER_CHUNK = 18, /* [0] 1: a chunked search deduplicates and verifies its candidates after EVERY key-range chunk instead of letting the chunks append to one candidate window that is flushed when it fills or after the last chunk (test hook; results are identical) */
-    SYMDEL_OPT_SORT_GROUPING = 10 /* [0] 1: symdel_stage_sort_u64 sorts keys only: ties land in arbitrary order (the mode the pipeline uses) */
+    SYMDEL_OPT_FLUSH_PER_CHUNK = 18 /* [0] 1: a chunked search deduplicates and verifies its candidates after EVERY key-range chunk instead of letting the chunks append to one candidate window that is flushed when it fills or after the last chunk (test hook; results are identical) */
 };
 
 /* ---- context ------------------------------------------------------------------------------- */
